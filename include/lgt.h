@@ -1,0 +1,147 @@
+/*
+ * lgt.h -- C ABI of the B200-native HMC molecular-dynamics force library (liblgt.so).
+ *
+ * The hot path of arXiv 2602.20516 ("Lattice Gauge Theory via LLVM-Level Automatic
+ * Differentiation"), hand-written as CUDA kernels for sm_100a:
+ *   Wilson plaquette action and staple force, Wilson-Dirac operator D / D^dag, CG on
+ *   D^dag D, two-flavour Wilson fermion force, su(3) projection, leapfrog kick / drift.
+ * Citations "PAPER.md:n" are lines of the paper text; "configs[0]" is BASELINE.json's
+ * statement of the two Wilson actions, which the paper names but does not write out.
+ *
+ * Conventions (DESIGN.md has the derivations and every reading of the paper):
+ *   dims = {Lx,Ly,Lz,Lt}; V = Lx*Ly*Lz*Lt; canonical site index s = x + Lx*(y + Ly*(z + Lz*t)).
+ *   CANONICAL LAYOUT, used by every pointer argument unless the call says "native":
+ *     links     U[s][mu][i][j]    complex (re,im), 3x3 row-major, mu = 0..3 = x,y,z,t
+ *     spinors   psi[s][alpha][a]  complex, alpha = 0..3 spin (chiral basis, gamma5 = diag(1,1,-1,-1)),
+ *                                 a = 0..2 colour
+ *     momenta and forces  P[s][mu][i][j]  traceless anti-Hermitian 3x3 (the paper's iP)
+ *   Element type is complex double for an LGT_F64 handle, complex float for LGT_F32.
+ *   All field pointers are DEVICE pointers to caller-owned buffers, unless the call's name ends
+ *   in _host.  Output scalars are written through HOST pointers.
+ *   The handle owns its copies of U, Pi, phi and all workspaces in the internal ("native")
+ *   structure-of-arrays layout; set/get calls convert.
+ *   Every call returns LGT_OK or a negative error code and never throws or aborts; after an
+ *   error lgt_last_error(ctx) gives a message.  Work is enqueued on the handle's stream; calls
+ *   that return host scalars synchronise that stream only.  A handle is not thread-safe.
+ *   There is no CPU fallback: without a CUDA device lgt_create fails with LGT_ECUDA.
+ *
+ * MD equations (Eqs. S2.1-S2.2, with Pi = iP anti-Hermitian):
+ *     U_mu(x) <- exp(dt Pi_mu(x)) U_mu(x),      Pi_mu(x) <- Pi_mu(x) - dt F_mu(x),
+ *   F = P_su(3)[...] (Eq. 7), normalised so that
+ *     d/dt S(exp(t tau^a) U_mu(x))|_0 = -2 tr(tau^a F_mu(x)),  tau^a = i lambda^a / 2,
+ *   and H = K + S_g + S_F with K = sum_{x,mu} ||Pi_mu(x)||_F^2.
+ */
+#ifndef LGT_H
+#define LGT_H
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct lgt_ctx lgt_ctx; /* opaque */
+
+enum { LGT_OK = 0, LGT_EINVAL = -1, LGT_ENOMEM = -2, LGT_ECUDA = -3, LGT_ENOCONV = -4, LGT_ESTATE = -5 };
+enum { LGT_F64 = 0, LGT_F32 = 1 };
+
+/* ---- lifetime -------------------------------------------------------------------------- */
+
+/* Creates a handle for one lattice on CUDA device `device`.
+ * dims[4] >= 1 each; beta = gauge coupling of S_g; kappa = hopping parameter of D (0 => gauge only);
+ * bc[4] = fermion boundary signs, each +1 or -1 (configs use {1,1,1,-1}); precision = LGT_F64 / LGT_F32;
+ * cuda_stream = a cudaStream_t to enqueue on, or NULL for the default stream.
+ * Links start as the unit field, momenta and pseudofermion as zero ("not set").
+ * Errors: LGT_EINVAL (bad argument), LGT_ECUDA (no device / CUDA failure), LGT_ENOMEM. */
+int lgt_create(lgt_ctx** out, const int dims[4], double beta, double kappa, const int bc[4],
+               int precision, int device, void* cuda_stream);
+int lgt_destroy(lgt_ctx* ctx);
+/* Message of the last error on this handle (or of the last failed lgt_create if ctx == NULL).
+ * Owned by the library; valid until the next call. */
+const char* lgt_last_error(const lgt_ctx* ctx);
+/* Library version string, static. */
+const char* lgt_version(void);
+
+/* ---- state upload / download (canonical layout, device pointers) ------------------------ */
+int lgt_set_links(lgt_ctx* ctx, const void* U);           /* [V][4][3][3] complex */
+int lgt_get_links(lgt_ctx* ctx, void* U);
+int lgt_set_momenta(lgt_ctx* ctx, const void* P);         /* [V][4][3][3]; only the traceless anti-Hermitian part is kept */
+int lgt_get_momenta(lgt_ctx* ctx, void* P);
+int lgt_set_pseudofermion(lgt_ctx* ctx, const void* phi); /* [V][4][3] complex */
+
+/* Same as the three setters / two getters above with HOST buffers (pageable or pinned): the
+ * host<->device copy is made by the library on the handle's stream and the call synchronises. */
+int lgt_set_links_host(lgt_ctx* ctx, const void* U);
+int lgt_get_links_host(lgt_ctx* ctx, void* U);
+int lgt_set_momenta_host(lgt_ctx* ctx, const void* P);
+int lgt_get_momenta_host(lgt_ctx* ctx, void* P);
+int lgt_set_pseudofermion_host(lgt_ctx* ctx, const void* phi);
+
+/* ---- A1: actions (configs[0]; PAPER.md:377 Eq. S3.1) ------------------------------------ */
+/* S_g = beta sum_x sum_{mu<nu} (1 - Re tr U_P/3);  S_F = Re phi^dag (D^dag D)^-1 phi (CG to `tol`,
+ * 0 if kappa == 0 or no pseudofermion is set);  K = sum ||Pi||_F^2.  Any output pointer may be NULL.
+ * cg_iters (may be NULL) receives the CG iteration count.  LGT_ENOCONV if CG hit max_iter. */
+int lgt_action(lgt_ctx* ctx, double tol, int max_iter, double* S_g, double* S_F, double* K, int* cg_iters);
+/* Mean plaquette (1/6V) sum Re tr U_P / 3. */
+int lgt_plaquette(lgt_ctx* ctx, double* plaq);
+
+/* ---- A2: Wilson-Dirac operator (configs[0]) --------------------------------------------- */
+/* (D psi)(x) = psi(x) - kappa sum_mu [ (1-gamma_mu) s_mu(x) U_mu(x) psi(x+mu)
+ *                                     + (1+gamma_mu) s_mu(x-mu) U_mu^dag(x-mu) psi(x-mu) ],
+ * s_mu(x) = bc[mu] on links that cross the mu boundary, else 1.  dagger != 0 applies D^dag
+ * (gamma_mu -> -gamma_mu).  in, out: canonical spinors [V][4][3], in != out. */
+int lgt_dslash(lgt_ctx* ctx, const void* in, void* out, int dagger);
+
+/* ---- A3: solver (PAPER.md:397-401 Eq. S3.6; :454) ---------------------------------------- */
+/* Solves (D^dag D) x = b by conjugate gradient from x0 = 0; stops when the recurrence residual
+ * satisfies |r|^2 <= tol^2 |b|^2 or after max_iter applications of D^dag D.
+ * iters, rel_resid (= |r|/|b|) may be NULL.  Returns LGT_ENOCONV if the cap was hit (x holds the
+ * last iterate). */
+int lgt_cg(lgt_ctx* ctx, const void* b, void* x, double tol, int max_iter, int* iters, double* rel_resid);
+
+/* ---- A4, A5: forces (PAPER.md:105-109 Eq. 7; :425 Eq. S3.12; :462-506 S4) ----------------- */
+/* F^g_mu(x) = (beta/6) P_su(3)[ U_mu(x) V_mu(x) ], V = sum of the six staples. F: [V][4][3][3]. */
+int lgt_gauge_force(lgt_ctx* ctx, void* F);
+/* F^f_mu(x) = -kappa P_su(3)[ s_mu(x) U_mu(x) C_mu(x) ],
+ * C_mu(x) = sum_spin (1-gamma_mu)X(x+mu) (x) Y(x)^dag + (1+gamma_mu)Y(x+mu) (x) X(x)^dag (colour outer products).
+ * X, Y: canonical spinors with X = (D^dag D)^-1 phi, Y = D X; if both are NULL they are obtained from the
+ * handle's pseudofermion by CG to (tol, max_iter).  cg_iters may be NULL. */
+int lgt_fermion_force(lgt_ctx* ctx, const void* X, const void* Y, void* F,
+                      double tol, int max_iter, int* cg_iters);
+
+/* ---- A6, A7: molecular dynamics (PAPER.md:95-99 Eq. 5; :261-263) -------------------------- */
+/* Pi <- Pi - eps (F^g + F^f); the fermion part (CG, Y = D X, fused force) runs if kappa != 0 and a
+ * pseudofermion is set.  cg_iters may be NULL. */
+int lgt_md_kick(lgt_ctx* ctx, double eps, double tol, int max_iter, int* cg_iters);
+/* U_mu(x) <- exp(eps Pi_mu(x)) U_mu(x), exponential by Cayley-Hamilton (ref. [6]). */
+int lgt_md_drift(lgt_ctx* ctx, double eps);
+/* One leapfrog step: kick(dt/2) drift(dt) kick(dt/2). cg_iters: sum over the two kicks. */
+int lgt_md_step(lgt_ctx* ctx, double dt, double tol, int max_iter, int* cg_iters);
+/* Leapfrog trajectory kick(dt/2) {drift(dt) kick(dt)}^(n-1) drift(dt) kick(dt/2), with H = K + S_g + S_F
+ * evaluated before and after (either pointer may be NULL to skip that evaluation). */
+int lgt_md_trajectory(lgt_ctx* ctx, int nsteps, double dt, double tol, int max_iter,
+                      double* H_initial, double* H_final, long* cg_iters);
+
+/* ---- native-layout spinor fields (for callers that keep fields resident between calls) ---- */
+/* Bytes of one spinor field in the handle's internal layout and precision. */
+long lgt_native_spinor_bytes(const lgt_ctx* ctx);
+/* canonical -> native and back; device pointers, src != dst. */
+int lgt_spinor_to_native(lgt_ctx* ctx, const void* canonical, void* native);
+int lgt_spinor_from_native(lgt_ctx* ctx, const void* native, void* canonical);
+/* out = D in / D^dag in on native-layout device buffers (one kernel launch, nothing else). */
+int lgt_dslash_native(lgt_ctx* ctx, const void* in, void* out, int dagger);
+/* Pi <- Pi - eps F^f from native-layout X, Y (one launch of the fused force kernel). */
+int lgt_fermion_force_native(lgt_ctx* ctx, const void* X, const void* Y, double eps);
+/* Pi <- Pi - eps F^g (one launch of the staple kernel). */
+int lgt_gauge_force_accumulate(lgt_ctx* ctx, double eps);
+/* CG on native buffers; b, x native spinors; also leaves Y = D x in `y` if y != NULL. */
+int lgt_cg_native(lgt_ctx* ctx, const void* b, void* x, void* y, double tol, int max_iter,
+                  int* iters, double* rel_resid);
+
+/* ---- introspection -------------------------------------------------------------------------- */
+/* Number of kernels this handle has launched since creation (bench.py's gpu_launches). */
+long lgt_launch_count(const lgt_ctx* ctx);
+/* The stream the handle enqueues on (cudaStream_t as void*). */
+void* lgt_stream(const lgt_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

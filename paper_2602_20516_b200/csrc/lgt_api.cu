@@ -1,0 +1,591 @@
+// lgt_api.cu -- the C ABI of include/lgt.h: handle, argument checks, kernel launches.
+// No torch, no host-side arithmetic on fields: every step of the path runs in the kernels of kernels.cuh.
+#include <cuda_runtime.h>
+
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+
+#include "../../include/lgt.h"
+#include "kernels.cuh"
+
+using namespace lgt;
+
+namespace {
+std::string g_create_error;
+}
+
+struct lgt_ctx {
+    Geom g;
+    double beta, kappa;
+    int prec;
+    int device;
+    cudaStream_t stream;
+    size_t esize;  // bytes of one complex number
+    void* U = nullptr;    // native links   [36][Vs] complex
+    void* P = nullptr;    // native momenta [16][Vs] pairs
+    void* phi = nullptr;  // native pseudofermion
+    bool has_phi = false;
+    void* ws[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};  // x, r, p, t, q, b
+    void* F = nullptr;      // compact force buffer for the canonical-output calls (lazy)
+    void* stage = nullptr;  // canonical staging buffer for *_host calls and conversions (lazy)
+    size_t stage_bytes = 0;
+    double* partials = nullptr;
+    unsigned* counter = nullptr;
+    CgState* st = nullptr;
+    double* scal = nullptr;  // device result slots
+    CgState* h_st = nullptr;  // pinned
+    double* h_scal = nullptr;  // pinned
+    int red_blocks = 0;
+    long launches = 0;
+    std::string err;
+};
+
+namespace {
+
+int fail(lgt_ctx* c, int code, const char* what, cudaError_t e = cudaSuccess) {
+    char buf[512];
+    if (e != cudaSuccess)
+        snprintf(buf, sizeof buf, "%s: %s", what, cudaGetErrorString(e));
+    else
+        snprintf(buf, sizeof buf, "%s", what);
+    if (c)
+        c->err = buf;
+    else
+        g_create_error = buf;
+    return code;
+}
+
+#define CU(call)                                                                  \
+    do {                                                                          \
+        cudaError_t e_ = (call);                                                  \
+        if (e_ != cudaSuccess) return fail(c, (e_ == cudaErrorMemoryAllocation) ? LGT_ENOMEM : LGT_ECUDA, #call, e_); \
+    } while (0)
+
+#define LAUNCH(c, kern, grid, block, ...)                           \
+    do {                                                            \
+        kern<<<(grid), (block), 0, (c)->stream>>>(__VA_ARGS__);     \
+        (c)->launches++;                                            \
+        cudaError_t e_ = cudaGetLastError();                        \
+        if (e_ != cudaSuccess) return fail((c), LGT_ECUDA, #kern, e_); \
+    } while (0)
+
+struct DeviceGuard {
+    int prev = -1;
+    explicit DeviceGuard(int dev) {
+        cudaGetDevice(&prev);
+        if (prev != dev) cudaSetDevice(dev);
+        else prev = -1;
+    }
+    ~DeviceGuard() {
+        if (prev >= 0) cudaSetDevice(prev);
+    }
+};
+
+inline size_t spinor_bytes(const lgt_ctx* c) { return (size_t)12 * c->g.Vs * c->esize; }
+inline size_t links_bytes(const lgt_ctx* c) { return (size_t)36 * c->g.Vs * c->esize; }
+inline size_t mom_bytes(const lgt_ctx* c) { return (size_t)16 * c->g.Vs * c->esize; }
+inline int site_blocks(const lgt_ctx* c, int bs) { return (c->g.V + bs - 1) / bs; }
+inline int stream_blocks(const lgt_ctx* c, size_t n) {
+    size_t b = (n + 255) / 256;
+    return (int)(b < (size_t)c->red_blocks ? (b ? b : 1) : c->red_blocks);
+}
+
+int ensure_stage(lgt_ctx* c, size_t bytes) {
+    if (c->stage_bytes >= bytes) return LGT_OK;
+    if (c->stage) cudaFree(c->stage);
+    c->stage = nullptr;
+    c->stage_bytes = 0;
+    CU(cudaMalloc(&c->stage, bytes));
+    c->stage_bytes = bytes;
+    return LGT_OK;
+}
+int ensure_force_buf(lgt_ctx* c) {
+    if (c->F) return LGT_OK;
+    CU(cudaMalloc(&c->F, mom_bytes(c)));
+    return LGT_OK;
+}
+
+template <class T> struct Ops {
+    typedef typename Vec2<T>::type T2;
+
+    static int to_native(lgt_ctx* c, const void* src, void* dst, int ncomp) {
+        size_t n = (size_t)c->g.V * ncomp;
+        LAUNCH(c, (reorder_kernel<T, 0>), stream_blocks(c, n), 256, c->g.V, c->g.Vs, ncomp, (const T2*)src, (T2*)dst);
+        return LGT_OK;
+    }
+    static int from_native(lgt_ctx* c, const void* src, void* dst, int ncomp) {
+        size_t n = (size_t)c->g.V * ncomp;
+        LAUNCH(c, (reorder_kernel<T, 1>), stream_blocks(c, n), 256, c->g.V, c->g.Vs, ncomp, (const T2*)src, (T2*)dst);
+        return LGT_OK;
+    }
+    static int momenta_to_native(lgt_ctx* c, const void* src, void* dst) {
+        LAUNCH(c, (momenta_reorder_kernel<T, 0>), stream_blocks(c, (size_t)4 * c->g.V), 256, c->g.V, c->g.Vs, (const T2*)src, (T2*)dst);
+        return LGT_OK;
+    }
+    static int momenta_from_native(lgt_ctx* c, const void* src, void* dst) {
+        LAUNCH(c, (momenta_reorder_kernel<T, 1>), stream_blocks(c, (size_t)4 * c->g.V), 256, c->g.V, c->g.Vs, (const T2*)src, (T2*)dst);
+        return LGT_OK;
+    }
+    static int unit_links(lgt_ctx* c) {
+        LAUNCH(c, (unit_links_kernel<T>), stream_blocks(c, (size_t)36 * c->g.V), 256, c->g.V, c->g.Vs, (T2*)c->U);
+        return LGT_OK;
+    }
+
+    // mode 0: plain; 1: CG "t = D p" (+ pAp, alpha); 2: CG "q = D^dag t"
+    static int dslash(lgt_ctx* c, const void* in, void* out, int dagger, int mode) {
+        const int grid = site_blocks(c, 128);
+        const T kappa = (T)c->kappa;
+        if (mode == 0) {
+            if (dagger)
+                LAUNCH(c, (dslash_kernel<T, 1, 0>), grid, 128, c->g, (const T2*)c->U, (const T2*)in, (T2*)out, kappa, c->st, c->partials, c->counter);
+            else
+                LAUNCH(c, (dslash_kernel<T, 0, 0>), grid, 128, c->g, (const T2*)c->U, (const T2*)in, (T2*)out, kappa, c->st, c->partials, c->counter);
+        } else if (mode == 1) {
+            LAUNCH(c, (dslash_kernel<T, 0, 1>), grid, 128, c->g, (const T2*)c->U, (const T2*)in, (T2*)out, kappa, c->st, c->partials, c->counter);
+        } else {
+            LAUNCH(c, (dslash_kernel<T, 1, 2>), grid, 128, c->g, (const T2*)c->U, (const T2*)in, (T2*)out, kappa, c->st, c->partials, c->counter);
+        }
+        return LGT_OK;
+    }
+
+    // CG on D^dag D (reading A-10): b, x native; y (optional) receives D x.
+    static int cg(lgt_ctx* c, const void* b, void* x, void* y, double tol, int max_iter, int* iters, double* rel) {
+        T2 *r = (T2*)c->ws[1], *p = (T2*)c->ws[2], *t = (T2*)c->ws[3], *q = (T2*)c->ws[4];
+        const size_t n = (size_t)12 * c->g.Vs;
+        const int nb = stream_blocks(c, n);
+        LAUNCH(c, (cg_init_kernel<T>), nb, 256, n, (const T2*)b, (T2*)x, r, p, c->st, tol * tol, max_iter, c->partials, c->counter);
+        int rc;
+        int launched = 0;
+        for (;;) {
+            CU(cudaMemcpyAsync(c->h_st, c->st, sizeof(CgState), cudaMemcpyDeviceToHost, c->stream));
+            CU(cudaStreamSynchronize(c->stream));
+            if (c->h_st->done) break;
+            // iterations are enqueued in chunks; kernels past convergence return at once
+            int chunk = max_iter - launched;
+            if (chunk > 8) chunk = 8;
+            if (chunk <= 0) chunk = 1;
+            for (int i = 0; i < chunk; i++) {
+                if ((rc = dslash(c, p, t, 0, 1)) != LGT_OK) return rc;
+                if ((rc = dslash(c, t, q, 1, 2)) != LGT_OK) return rc;
+                LAUNCH(c, (cg_update_xr_kernel<T>), nb, 256, n, (T2*)x, r, (const T2*)p, (const T2*)q, c->st, c->partials, c->counter);
+                LAUNCH(c, (cg_update_p_kernel<T>), nb, 256, n, p, (const T2*)r, c->st);
+            }
+            launched += chunk;
+        }
+        const CgState& h = *c->h_st;
+        if (iters) *iters = h.iter;
+        if (rel) *rel = (h.bb > 0.0) ? sqrt(h.rr / h.bb) : 0.0;
+        if (y && (rc = dslash(c, x, y, 0, 0)) != LGT_OK) return rc;
+        if (h.rr > h.tol2 * h.bb) return fail(c, LGT_ENOCONV, "CG did not reach the tolerance within max_iter");
+        return LGT_OK;
+    }
+
+    static int fermion_force(lgt_ctx* c, const void* X, const void* Y, void* P, int acc, double eps) {
+        dim3 grid(site_blocks(c, 128), 4);
+        if (acc)
+            LAUNCH(c, (fermion_force_kernel<T, 1>), grid, 128, c->g, (const T2*)c->U, (const T2*)X, (const T2*)Y, (T2*)P, (T)c->kappa, (T)eps);
+        else
+            LAUNCH(c, (fermion_force_kernel<T, 0>), grid, 128, c->g, (const T2*)c->U, (const T2*)X, (const T2*)Y, (T2*)P, (T)c->kappa, (T)eps);
+        return LGT_OK;
+    }
+    static int gauge_force(lgt_ctx* c, void* P, int acc, double eps) {
+        dim3 grid(site_blocks(c, 128), 4);
+        if (acc)
+            LAUNCH(c, (gauge_force_kernel<T, 1>), grid, 128, c->g, (const T2*)c->U, (T2*)P, (T)(c->beta / 6.0), (T)eps);
+        else
+            LAUNCH(c, (gauge_force_kernel<T, 0>), grid, 128, c->g, (const T2*)c->U, (T2*)P, (T)(c->beta / 6.0), (T)eps);
+        return LGT_OK;
+    }
+    static int link_update(lgt_ctx* c, double eps) {
+        dim3 grid(site_blocks(c, 128), 4);
+        LAUNCH(c, (link_update_kernel<T>), grid, 128, c->g, (T2*)c->U, (const T2*)c->P, (T)eps);
+        return LGT_OK;
+    }
+    static int plaquette_sum(lgt_ctx* c, double* dev_result) {
+        LAUNCH(c, (plaquette_kernel<T>), site_blocks(c, 128), 128, c->g, (const T2*)c->U, dev_result, c->partials, c->counter);
+        return LGT_OK;
+    }
+    static int kinetic(lgt_ctx* c, double* dev_result) {
+        LAUNCH(c, (kinetic_kernel<T>), stream_blocks(c, (size_t)4 * c->g.V), 256, c->g, (const T2*)c->P, dev_result, c->partials, c->counter);
+        return LGT_OK;
+    }
+    static int redot(lgt_ctx* c, const void* a, const void* b, double* dev_result) {
+        const size_t n = (size_t)12 * c->g.Vs;
+        LAUNCH(c, (redot_kernel<T>), stream_blocks(c, n), 256, n, (const T2*)a, (const T2*)b, dev_result, c->partials, c->counter);
+        return LGT_OK;
+    }
+};
+
+#define DISPATCH(c, fn, ...) ((c)->prec == LGT_F64 ? Ops<double>::fn(__VA_ARGS__) : Ops<float>::fn(__VA_ARGS__))
+
+int read_scalars(lgt_ctx* c, int n) {
+    CU(cudaMemcpyAsync(c->h_scal, c->scal, sizeof(double) * n, cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    return LGT_OK;
+}
+
+bool fermions_on(const lgt_ctx* c) { return c->kappa != 0.0 && c->has_phi; }
+
+// Pi -= eps (F^g + F^f)
+int kick(lgt_ctx* c, double eps, double tol, int max_iter, int* cg_iters) {
+    int rc, it = 0, conv = LGT_OK;
+    if ((rc = DISPATCH(c, gauge_force, c, c->P, 1, eps)) != LGT_OK) return rc;
+    if (fermions_on(c)) {
+        rc = DISPATCH(c, cg, c, c->phi, c->ws[0], c->ws[3], tol, max_iter, &it, nullptr);
+        if (rc == LGT_ENOCONV) conv = rc;
+        else if (rc != LGT_OK) return rc;
+        if ((rc = DISPATCH(c, fermion_force, c, c->ws[0], c->ws[3], c->P, 1, eps)) != LGT_OK) return rc;
+    }
+    if (cg_iters) *cg_iters = it;
+    return conv;
+}
+
+int hamiltonian(lgt_ctx* c, double tol, int max_iter, double* S_g, double* S_F, double* K, int* cg_iters) {
+    int rc, it = 0, conv = LGT_OK;
+    if ((rc = DISPATCH(c, plaquette_sum, c, c->scal + 0)) != LGT_OK) return rc;
+    if ((rc = DISPATCH(c, kinetic, c, c->scal + 1)) != LGT_OK) return rc;
+    bool ferm = fermions_on(c) && S_F != nullptr;
+    if (ferm) {
+        rc = DISPATCH(c, cg, c, c->phi, c->ws[0], nullptr, tol, max_iter, &it, nullptr);
+        if (rc == LGT_ENOCONV) conv = rc;
+        else if (rc != LGT_OK) return rc;
+        if ((rc = DISPATCH(c, redot, c, c->phi, c->ws[0], c->scal + 2)) != LGT_OK) return rc;
+    }
+    if ((rc = read_scalars(c, 3)) != LGT_OK) return rc;
+    if (S_g) *S_g = c->beta * (6.0 * (double)c->g.V - c->h_scal[0]);
+    if (K) *K = c->h_scal[1];
+    if (S_F) *S_F = ferm ? c->h_scal[2] : 0.0;
+    if (cg_iters) *cg_iters = it;
+    return conv;
+}
+
+}  // namespace
+
+#define CHECK_CTX(c) \
+    if (!(c)) return LGT_EINVAL; \
+    DeviceGuard guard_((c)->device)
+
+extern "C" {
+
+const char* lgt_version(void) { return "lgt-b200 0.1 (sm_100a)"; }
+
+const char* lgt_last_error(const lgt_ctx* c) { return c ? c->err.c_str() : g_create_error.c_str(); }
+
+int lgt_create(lgt_ctx** out, const int dims[4], double beta, double kappa, const int bc[4], int precision, int device,
+               void* cuda_stream) {
+    lgt_ctx* c = nullptr;
+    if (!out || !dims || !bc) return fail(nullptr, LGT_EINVAL, "lgt_create: null argument");
+    *out = nullptr;
+    long long V = 1;
+    for (int m = 0; m < 4; m++) {
+        if (dims[m] < 1) return fail(nullptr, LGT_EINVAL, "lgt_create: dims must be >= 1");
+        if (bc[m] != 1 && bc[m] != -1) return fail(nullptr, LGT_EINVAL, "lgt_create: bc entries must be +1 or -1");
+        V *= dims[m];
+        if (V > (1LL << 30)) return fail(nullptr, LGT_EINVAL, "lgt_create: lattice too large for 32-bit site indices");
+    }
+    if (precision != LGT_F64 && precision != LGT_F32) return fail(nullptr, LGT_EINVAL, "lgt_create: bad precision");
+    int ndev = 0;
+    cudaError_t e = cudaGetDeviceCount(&ndev);
+    if (e != cudaSuccess || ndev == 0)
+        return fail(nullptr, LGT_ECUDA, "lgt_create: no CUDA device (there is no CPU fallback)", e);
+    if (device < 0 || device >= ndev) return fail(nullptr, LGT_EINVAL, "lgt_create: bad device index");
+    try {
+        c = new lgt_ctx();
+    } catch (const std::bad_alloc&) {
+        return fail(nullptr, LGT_ENOMEM, "lgt_create: host allocation failed");
+    }
+    DeviceGuard guard(device);
+    c->device = device;
+    c->stream = (cudaStream_t)cuda_stream;
+    c->beta = beta;
+    c->kappa = kappa;
+    c->prec = precision;
+    c->esize = precision == LGT_F64 ? 16 : 8;
+    int stride = 1;
+    for (int m = 0; m < 4; m++) {
+        c->g.L[m] = dims[m];
+        c->g.bc[m] = bc[m];
+        c->g.stride[m] = stride;
+        stride *= dims[m];
+    }
+    c->g.V = (int)V;
+    c->g.Vs = (int)V;
+    int sms = 148;
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device);
+    c->red_blocks = sms * 8;
+    int rc = LGT_OK;
+    auto alloc = [&](void** p, size_t bytes) {
+        if (rc != LGT_OK) return;
+        cudaError_t ee = cudaMalloc(p, bytes);
+        if (ee != cudaSuccess) rc = fail(nullptr, ee == cudaErrorMemoryAllocation ? LGT_ENOMEM : LGT_ECUDA, "lgt_create: cudaMalloc", ee);
+    };
+    alloc(&c->U, links_bytes(c));
+    alloc(&c->P, mom_bytes(c));
+    alloc(&c->phi, spinor_bytes(c));
+    for (int i = 0; i < 6; i++) alloc(&c->ws[i], spinor_bytes(c));
+    size_t npart = (size_t)site_blocks(c, 128) + c->red_blocks + 64;
+    alloc((void**)&c->partials, npart * sizeof(double));
+    alloc((void**)&c->counter, sizeof(unsigned));
+    alloc((void**)&c->st, sizeof(CgState));
+    alloc((void**)&c->scal, 8 * sizeof(double));
+    if (rc == LGT_OK && (cudaMallocHost((void**)&c->h_st, sizeof(CgState)) != cudaSuccess ||
+                         cudaMallocHost((void**)&c->h_scal, 8 * sizeof(double)) != cudaSuccess))
+        rc = fail(nullptr, LGT_ENOMEM, "lgt_create: cudaMallocHost failed");
+    if (rc == LGT_OK) {
+        bool ok = cudaMemsetAsync(c->counter, 0, sizeof(unsigned), c->stream) == cudaSuccess &&
+                  cudaMemsetAsync(c->st, 0, sizeof(CgState), c->stream) == cudaSuccess &&
+                  cudaMemsetAsync(c->P, 0, mom_bytes(c), c->stream) == cudaSuccess &&
+                  cudaMemsetAsync(c->phi, 0, spinor_bytes(c), c->stream) == cudaSuccess;
+        if (!ok) rc = fail(nullptr, LGT_ECUDA, "lgt_create: cudaMemsetAsync failed");
+    }
+    if (rc == LGT_OK) {
+        rc = DISPATCH(c, unit_links, c);
+        if (rc != LGT_OK) g_create_error = c->err;
+    }
+    if (rc == LGT_OK && cudaStreamSynchronize(c->stream) != cudaSuccess) rc = fail(nullptr, LGT_ECUDA, "lgt_create: sync failed");
+    if (rc != LGT_OK) {
+        lgt_destroy(c);
+        return rc;
+    }
+    *out = c;
+    return LGT_OK;
+}
+
+int lgt_destroy(lgt_ctx* c) {
+    if (!c) return LGT_OK;
+    DeviceGuard guard(c->device);
+    cudaStreamSynchronize(c->stream);
+    cudaFree(c->U);
+    cudaFree(c->P);
+    cudaFree(c->phi);
+    for (int i = 0; i < 6; i++) cudaFree(c->ws[i]);
+    cudaFree(c->F);
+    cudaFree(c->stage);
+    cudaFree(c->partials);
+    cudaFree(c->counter);
+    cudaFree(c->st);
+    cudaFree(c->scal);
+    if (c->h_st) cudaFreeHost(c->h_st);
+    if (c->h_scal) cudaFreeHost(c->h_scal);
+    delete c;
+    return LGT_OK;
+}
+
+long lgt_launch_count(const lgt_ctx* c) { return c ? c->launches : 0; }
+void* lgt_stream(const lgt_ctx* c) { return c ? (void*)c->stream : nullptr; }
+long lgt_native_spinor_bytes(const lgt_ctx* c) { return c ? (long)spinor_bytes(c) : 0; }
+
+// ---- state
+int lgt_set_links(lgt_ctx* c, const void* U) {
+    CHECK_CTX(c);
+    if (!U) return fail(c, LGT_EINVAL, "lgt_set_links: null pointer");
+    return DISPATCH(c, to_native, c, U, c->U, 36);
+}
+int lgt_get_links(lgt_ctx* c, void* U) {
+    CHECK_CTX(c);
+    if (!U) return fail(c, LGT_EINVAL, "lgt_get_links: null pointer");
+    return DISPATCH(c, from_native, c, c->U, U, 36);
+}
+int lgt_set_momenta(lgt_ctx* c, const void* P) {
+    CHECK_CTX(c);
+    if (!P) return fail(c, LGT_EINVAL, "lgt_set_momenta: null pointer");
+    return DISPATCH(c, momenta_to_native, c, P, c->P);
+}
+int lgt_get_momenta(lgt_ctx* c, void* P) {
+    CHECK_CTX(c);
+    if (!P) return fail(c, LGT_EINVAL, "lgt_get_momenta: null pointer");
+    return DISPATCH(c, momenta_from_native, c, c->P, P);
+}
+int lgt_set_pseudofermion(lgt_ctx* c, const void* phi) {
+    CHECK_CTX(c);
+    if (!phi) return fail(c, LGT_EINVAL, "lgt_set_pseudofermion: null pointer");
+    int rc = DISPATCH(c, to_native, c, phi, c->phi, 12);
+    if (rc == LGT_OK) c->has_phi = true;
+    return rc;
+}
+
+#define HOST_SET(name, devcall, bytes_expr)                                                         \
+    int name(lgt_ctx* c, const void* h) {                                                           \
+        CHECK_CTX(c);                                                                               \
+        if (!h) return fail(c, LGT_EINVAL, #name ": null pointer");                                 \
+        size_t bytes = (bytes_expr);                                                                \
+        int rc = ensure_stage(c, bytes);                                                            \
+        if (rc != LGT_OK) return rc;                                                                \
+        CU(cudaMemcpyAsync(c->stage, h, bytes, cudaMemcpyHostToDevice, c->stream));                 \
+        rc = devcall(c, c->stage);                                                                  \
+        if (rc != LGT_OK) return rc;                                                                \
+        CU(cudaStreamSynchronize(c->stream));                                                       \
+        return LGT_OK;                                                                              \
+    }
+#define HOST_GET(name, devcall, bytes_expr)                                                         \
+    int name(lgt_ctx* c, void* h) {                                                                 \
+        CHECK_CTX(c);                                                                               \
+        if (!h) return fail(c, LGT_EINVAL, #name ": null pointer");                                 \
+        size_t bytes = (bytes_expr);                                                                \
+        int rc = ensure_stage(c, bytes);                                                            \
+        if (rc != LGT_OK) return rc;                                                                \
+        rc = devcall(c, c->stage);                                                                  \
+        if (rc != LGT_OK) return rc;                                                                \
+        CU(cudaMemcpyAsync(h, c->stage, bytes, cudaMemcpyDeviceToHost, c->stream));                 \
+        CU(cudaStreamSynchronize(c->stream));                                                       \
+        return LGT_OK;                                                                              \
+    }
+HOST_SET(lgt_set_links_host, lgt_set_links, (size_t)36 * c->g.V * c->esize)
+HOST_GET(lgt_get_links_host, lgt_get_links, (size_t)36 * c->g.V * c->esize)
+HOST_SET(lgt_set_momenta_host, lgt_set_momenta, (size_t)36 * c->g.V * c->esize)
+HOST_GET(lgt_get_momenta_host, lgt_get_momenta, (size_t)36 * c->g.V * c->esize)
+HOST_SET(lgt_set_pseudofermion_host, lgt_set_pseudofermion, (size_t)12 * c->g.V * c->esize)
+
+// ---- actions
+int lgt_action(lgt_ctx* c, double tol, int max_iter, double* S_g, double* S_F, double* K, int* cg_iters) {
+    CHECK_CTX(c);
+    return hamiltonian(c, tol, max_iter, S_g, S_F, K, cg_iters);
+}
+int lgt_plaquette(lgt_ctx* c, double* plaq) {
+    CHECK_CTX(c);
+    if (!plaq) return fail(c, LGT_EINVAL, "lgt_plaquette: null pointer");
+    int rc = DISPATCH(c, plaquette_sum, c, c->scal + 0);
+    if (rc != LGT_OK) return rc;
+    if ((rc = read_scalars(c, 1)) != LGT_OK) return rc;
+    *plaq = c->h_scal[0] / (6.0 * (double)c->g.V);
+    return LGT_OK;
+}
+
+// ---- Dirac operator
+int lgt_spinor_to_native(lgt_ctx* c, const void* canonical, void* native) {
+    CHECK_CTX(c);
+    if (!canonical || !native || canonical == native) return fail(c, LGT_EINVAL, "lgt_spinor_to_native: bad pointers");
+    return DISPATCH(c, to_native, c, canonical, native, 12);
+}
+int lgt_spinor_from_native(lgt_ctx* c, const void* native, void* canonical) {
+    CHECK_CTX(c);
+    if (!canonical || !native || canonical == native) return fail(c, LGT_EINVAL, "lgt_spinor_from_native: bad pointers");
+    return DISPATCH(c, from_native, c, native, canonical, 12);
+}
+int lgt_dslash_native(lgt_ctx* c, const void* in, void* out, int dagger) {
+    CHECK_CTX(c);
+    if (!in || !out || in == out) return fail(c, LGT_EINVAL, "lgt_dslash_native: in and out must be distinct non-null buffers");
+    return DISPATCH(c, dslash, c, in, out, dagger ? 1 : 0, 0);
+}
+int lgt_dslash(lgt_ctx* c, const void* in, void* out, int dagger) {
+    CHECK_CTX(c);
+    if (!in || !out || in == out) return fail(c, LGT_EINVAL, "lgt_dslash: in and out must be distinct non-null buffers");
+    int rc;
+    if ((rc = DISPATCH(c, to_native, c, in, c->ws[3], 12)) != LGT_OK) return rc;
+    if ((rc = DISPATCH(c, dslash, c, c->ws[3], c->ws[4], dagger ? 1 : 0, 0)) != LGT_OK) return rc;
+    return DISPATCH(c, from_native, c, c->ws[4], out, 12);
+}
+
+// ---- solver
+int lgt_cg_native(lgt_ctx* c, const void* b, void* x, void* y, double tol, int max_iter, int* iters, double* rel_resid) {
+    CHECK_CTX(c);
+    if (!b || !x || b == x) return fail(c, LGT_EINVAL, "lgt_cg_native: bad pointers");
+    if (!(tol >= 0.0) || max_iter < 0) return fail(c, LGT_EINVAL, "lgt_cg_native: bad tol / max_iter");
+    return DISPATCH(c, cg, c, b, x, y, tol, max_iter, iters, rel_resid);
+}
+int lgt_cg(lgt_ctx* c, const void* b, void* x, double tol, int max_iter, int* iters, double* rel_resid) {
+    CHECK_CTX(c);
+    if (!b || !x) return fail(c, LGT_EINVAL, "lgt_cg: null pointer");
+    if (!(tol >= 0.0) || max_iter < 0) return fail(c, LGT_EINVAL, "lgt_cg: bad tol / max_iter");
+    int rc;
+    if ((rc = DISPATCH(c, to_native, c, b, c->ws[5], 12)) != LGT_OK) return rc;
+    int conv = DISPATCH(c, cg, c, c->ws[5], c->ws[0], nullptr, tol, max_iter, iters, rel_resid);
+    if (conv != LGT_OK && conv != LGT_ENOCONV) return conv;
+    if ((rc = DISPATCH(c, from_native, c, c->ws[0], x, 12)) != LGT_OK) return rc;
+    return conv;
+}
+
+// ---- forces
+int lgt_gauge_force(lgt_ctx* c, void* F) {
+    CHECK_CTX(c);
+    if (!F) return fail(c, LGT_EINVAL, "lgt_gauge_force: null pointer");
+    int rc;
+    if ((rc = ensure_force_buf(c)) != LGT_OK) return rc;
+    if ((rc = DISPATCH(c, gauge_force, c, c->F, 0, 0.0)) != LGT_OK) return rc;
+    return DISPATCH(c, momenta_from_native, c, c->F, F);
+}
+int lgt_gauge_force_accumulate(lgt_ctx* c, double eps) {
+    CHECK_CTX(c);
+    return DISPATCH(c, gauge_force, c, c->P, 1, eps);
+}
+int lgt_fermion_force(lgt_ctx* c, const void* X, const void* Y, void* F, double tol, int max_iter, int* cg_iters) {
+    CHECK_CTX(c);
+    if (!F) return fail(c, LGT_EINVAL, "lgt_fermion_force: null pointer");
+    if ((X == nullptr) != (Y == nullptr)) return fail(c, LGT_EINVAL, "lgt_fermion_force: give both X and Y or neither");
+    int rc, conv = LGT_OK, it = 0;
+    if ((rc = ensure_force_buf(c)) != LGT_OK) return rc;
+    if (X) {
+        if ((rc = DISPATCH(c, to_native, c, X, c->ws[0], 12)) != LGT_OK) return rc;
+        if ((rc = DISPATCH(c, to_native, c, Y, c->ws[3], 12)) != LGT_OK) return rc;
+    } else {
+        if (!c->has_phi) return fail(c, LGT_ESTATE, "lgt_fermion_force: no pseudofermion set");
+        conv = DISPATCH(c, cg, c, c->phi, c->ws[0], c->ws[3], tol, max_iter, &it, nullptr);
+        if (conv != LGT_OK && conv != LGT_ENOCONV) return conv;
+    }
+    if (cg_iters) *cg_iters = it;
+    if ((rc = DISPATCH(c, fermion_force, c, c->ws[0], c->ws[3], c->F, 0, 0.0)) != LGT_OK) return rc;
+    if ((rc = DISPATCH(c, momenta_from_native, c, c->F, F)) != LGT_OK) return rc;
+    return conv;
+}
+int lgt_fermion_force_native(lgt_ctx* c, const void* X, const void* Y, double eps) {
+    CHECK_CTX(c);
+    if (!X || !Y) return fail(c, LGT_EINVAL, "lgt_fermion_force_native: null pointer");
+    return DISPATCH(c, fermion_force, c, X, Y, c->P, 1, eps);
+}
+
+// ---- molecular dynamics
+int lgt_md_kick(lgt_ctx* c, double eps, double tol, int max_iter, int* cg_iters) {
+    CHECK_CTX(c);
+    return kick(c, eps, tol, max_iter, cg_iters);
+}
+int lgt_md_drift(lgt_ctx* c, double eps) {
+    CHECK_CTX(c);
+    return DISPATCH(c, link_update, c, eps);
+}
+int lgt_md_step(lgt_ctx* c, double dt, double tol, int max_iter, int* cg_iters) {
+    CHECK_CTX(c);
+    int rc, it1 = 0, it2 = 0, conv = LGT_OK;
+    rc = kick(c, 0.5 * dt, tol, max_iter, &it1);
+    if (rc == LGT_ENOCONV) conv = rc; else if (rc != LGT_OK) return rc;
+    if ((rc = DISPATCH(c, link_update, c, dt)) != LGT_OK) return rc;
+    rc = kick(c, 0.5 * dt, tol, max_iter, &it2);
+    if (rc == LGT_ENOCONV) conv = rc; else if (rc != LGT_OK) return rc;
+    if (cg_iters) *cg_iters = it1 + it2;
+    return conv;
+}
+int lgt_md_trajectory(lgt_ctx* c, int nsteps, double dt, double tol, int max_iter, double* H_initial, double* H_final,
+                      long* cg_iters) {
+    CHECK_CTX(c);
+    if (nsteps < 0) return fail(c, LGT_EINVAL, "lgt_md_trajectory: nsteps < 0");
+    int rc, it = 0, conv = LGT_OK;
+    long total = 0;
+    double sg, sf, k;
+    if (H_initial) {
+        rc = hamiltonian(c, tol, max_iter, &sg, &sf, &k, &it);
+        if (rc == LGT_ENOCONV) conv = rc; else if (rc != LGT_OK) return rc;
+        *H_initial = k + sg + sf;
+    }
+    if (nsteps > 0) {
+        rc = kick(c, 0.5 * dt, tol, max_iter, &it);
+        if (rc == LGT_ENOCONV) conv = rc; else if (rc != LGT_OK) return rc;
+        total += it;
+        for (int n = 0; n < nsteps; n++) {
+            if ((rc = DISPATCH(c, link_update, c, dt)) != LGT_OK) return rc;
+            rc = kick(c, (n == nsteps - 1) ? 0.5 * dt : dt, tol, max_iter, &it);
+            if (rc == LGT_ENOCONV) conv = rc; else if (rc != LGT_OK) return rc;
+            total += it;
+        }
+    }
+    if (H_final) {
+        rc = hamiltonian(c, tol, max_iter, &sg, &sf, &k, &it);
+        if (rc == LGT_ENOCONV) conv = rc; else if (rc != LGT_OK) return rc;
+        *H_final = k + sg + sf;
+    }
+    if (cg_iters) *cg_iters = total;
+    CU(cudaStreamSynchronize(c->stream));
+    return conv;
+}
+
+}  // extern "C"

@@ -1,0 +1,333 @@
+"""Thin Python binding over the C-ABI CUDA library liblgt.so (include/lgt.h).
+
+Argument marshalling only: every step of the path runs in the CUDA kernels.  Functions carry
+the names of the C entry points; `Lattice` bundles a handle with torch-allocated buffers.
+PyTorch is used for device memory and streams, nothing else.  There is no CPU fallback: if the
+library is not built or no CUDA device is present, calls raise.
+"""
+import ctypes as C
+import os
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "liblgt.so")
+
+LGT_OK, LGT_EINVAL, LGT_ENOMEM, LGT_ECUDA, LGT_ENOCONV, LGT_ESTATE = 0, -1, -2, -3, -4, -5
+LGT_F64, LGT_F32 = 0, 1
+
+# every symbol include/lgt.h declares: (restype, argtypes)
+_vp, _i, _d, _l = C.c_void_p, C.c_int, C.c_double, C.c_long
+_ip, _dp, _lp = C.POINTER(C.c_int), C.POINTER(C.c_double), C.POINTER(C.c_long)
+SYMBOLS = {
+    "lgt_create": (_i, [C.POINTER(_vp), _ip, _d, _d, _ip, _i, _i, _vp]),
+    "lgt_destroy": (_i, [_vp]),
+    "lgt_last_error": (C.c_char_p, [_vp]),
+    "lgt_version": (C.c_char_p, []),
+    "lgt_set_links": (_i, [_vp, _vp]),
+    "lgt_get_links": (_i, [_vp, _vp]),
+    "lgt_set_momenta": (_i, [_vp, _vp]),
+    "lgt_get_momenta": (_i, [_vp, _vp]),
+    "lgt_set_pseudofermion": (_i, [_vp, _vp]),
+    "lgt_set_links_host": (_i, [_vp, _vp]),
+    "lgt_get_links_host": (_i, [_vp, _vp]),
+    "lgt_set_momenta_host": (_i, [_vp, _vp]),
+    "lgt_get_momenta_host": (_i, [_vp, _vp]),
+    "lgt_set_pseudofermion_host": (_i, [_vp, _vp]),
+    "lgt_action": (_i, [_vp, _d, _i, _dp, _dp, _dp, _ip]),
+    "lgt_plaquette": (_i, [_vp, _dp]),
+    "lgt_dslash": (_i, [_vp, _vp, _vp, _i]),
+    "lgt_cg": (_i, [_vp, _vp, _vp, _d, _i, _ip, _dp]),
+    "lgt_gauge_force": (_i, [_vp, _vp]),
+    "lgt_fermion_force": (_i, [_vp, _vp, _vp, _vp, _d, _i, _ip]),
+    "lgt_md_kick": (_i, [_vp, _d, _d, _i, _ip]),
+    "lgt_md_drift": (_i, [_vp, _d]),
+    "lgt_md_step": (_i, [_vp, _d, _d, _i, _ip]),
+    "lgt_md_trajectory": (_i, [_vp, _i, _d, _d, _i, _dp, _dp, _lp]),
+    "lgt_native_spinor_bytes": (_l, [_vp]),
+    "lgt_spinor_to_native": (_i, [_vp, _vp, _vp]),
+    "lgt_spinor_from_native": (_i, [_vp, _vp, _vp]),
+    "lgt_dslash_native": (_i, [_vp, _vp, _vp, _i]),
+    "lgt_fermion_force_native": (_i, [_vp, _vp, _vp, _d]),
+    "lgt_gauge_force_accumulate": (_i, [_vp, _d]),
+    "lgt_cg_native": (_i, [_vp, _vp, _vp, _vp, _d, _i, _ip, _dp]),
+    "lgt_launch_count": (_l, [_vp]),
+    "lgt_stream": (_vp, [_vp]),
+}
+
+_lib = None
+
+
+class LgtError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__("lgt error %d: %s" % (code, msg))
+        self.code = code
+
+
+def lib():
+    """Loads liblgt.so; raises if it has not been built (no fallback of any kind)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError("%s not found: build it with `python -m paper_2602_20516_b200.build` "
+                              "(there is no CPU fallback)" % LIB_PATH)
+        L = C.CDLL(LIB_PATH)
+        for name, (res, args) in SYMBOLS.items():
+            f = getattr(L, name)
+            f.restype, f.argtypes = res, args
+        _lib = L
+    return _lib
+
+
+def _ptr(t):
+    """Device (or host) address of a torch tensor / numpy array / int / None."""
+    if t is None:
+        return None
+    if isinstance(t, int):
+        return t
+    if hasattr(t, "data_ptr"):
+        assert t.is_contiguous()
+        return t.data_ptr()
+    assert t.flags["C_CONTIGUOUS"]
+    return t.ctypes.data
+
+
+def _check(ctx, rc, allow=()):
+    if rc != LGT_OK and rc not in allow:
+        msg = lib().lgt_last_error(ctx)
+        raise LgtError(rc, msg.decode() if msg else "")
+    return rc
+
+
+# ---- functions with the C names ---------------------------------------------------------------
+def lgt_version():
+    return lib().lgt_version().decode()
+
+
+def lgt_create(dims, beta, kappa, bc, precision=LGT_F64, device=0, stream=None):
+    h = _vp()
+    d = (C.c_int * 4)(*[int(x) for x in dims])
+    b = (C.c_int * 4)(*[int(x) for x in bc])
+    rc = lib().lgt_create(C.byref(h), d, float(beta), float(kappa), b, int(precision), int(device), stream)
+    if rc != LGT_OK:
+        raise LgtError(rc, lib().lgt_last_error(None).decode())
+    return h
+
+
+def lgt_destroy(ctx):
+    return lib().lgt_destroy(ctx)
+
+
+def lgt_set_links(ctx, U):
+    return _check(ctx, lib().lgt_set_links(ctx, _ptr(U)))
+
+
+def lgt_get_links(ctx, U):
+    return _check(ctx, lib().lgt_get_links(ctx, _ptr(U)))
+
+
+def lgt_set_momenta(ctx, P):
+    return _check(ctx, lib().lgt_set_momenta(ctx, _ptr(P)))
+
+
+def lgt_get_momenta(ctx, P):
+    return _check(ctx, lib().lgt_get_momenta(ctx, _ptr(P)))
+
+
+def lgt_set_pseudofermion(ctx, phi):
+    return _check(ctx, lib().lgt_set_pseudofermion(ctx, _ptr(phi)))
+
+
+def lgt_set_links_host(ctx, U):
+    return _check(ctx, lib().lgt_set_links_host(ctx, _ptr(U)))
+
+
+def lgt_get_links_host(ctx, U):
+    return _check(ctx, lib().lgt_get_links_host(ctx, _ptr(U)))
+
+
+def lgt_set_momenta_host(ctx, P):
+    return _check(ctx, lib().lgt_set_momenta_host(ctx, _ptr(P)))
+
+
+def lgt_get_momenta_host(ctx, P):
+    return _check(ctx, lib().lgt_get_momenta_host(ctx, _ptr(P)))
+
+
+def lgt_set_pseudofermion_host(ctx, phi):
+    return _check(ctx, lib().lgt_set_pseudofermion_host(ctx, _ptr(phi)))
+
+
+def lgt_action(ctx, tol=1e-12, max_iter=100000):
+    """Returns (S_g, S_F, K, cg_iters)."""
+    sg, sf, k, it = C.c_double(), C.c_double(), C.c_double(), C.c_int()
+    _check(ctx, lib().lgt_action(ctx, tol, max_iter, C.byref(sg), C.byref(sf), C.byref(k), C.byref(it)))
+    return sg.value, sf.value, k.value, it.value
+
+
+def lgt_plaquette(ctx):
+    p = C.c_double()
+    _check(ctx, lib().lgt_plaquette(ctx, C.byref(p)))
+    return p.value
+
+
+def lgt_dslash(ctx, inp, out, dagger=False):
+    return _check(ctx, lib().lgt_dslash(ctx, _ptr(inp), _ptr(out), int(bool(dagger))))
+
+
+def lgt_cg(ctx, b, x, tol, max_iter):
+    """Returns (iters, rel_resid, converged)."""
+    it, rel = C.c_int(), C.c_double()
+    rc = _check(ctx, lib().lgt_cg(ctx, _ptr(b), _ptr(x), tol, max_iter, C.byref(it), C.byref(rel)), allow=(LGT_ENOCONV,))
+    return it.value, rel.value, rc == LGT_OK
+
+
+def lgt_gauge_force(ctx, F):
+    return _check(ctx, lib().lgt_gauge_force(ctx, _ptr(F)))
+
+
+def lgt_fermion_force(ctx, X, Y, F, tol=1e-12, max_iter=100000):
+    """X, Y None: solved from the handle's pseudofermion.  Returns cg_iters."""
+    it = C.c_int()
+    _check(ctx, lib().lgt_fermion_force(ctx, _ptr(X), _ptr(Y), _ptr(F), tol, max_iter, C.byref(it)))
+    return it.value
+
+
+def lgt_md_kick(ctx, eps, tol=1e-12, max_iter=100000):
+    it = C.c_int()
+    _check(ctx, lib().lgt_md_kick(ctx, eps, tol, max_iter, C.byref(it)))
+    return it.value
+
+
+def lgt_md_drift(ctx, eps):
+    return _check(ctx, lib().lgt_md_drift(ctx, eps))
+
+
+def lgt_md_step(ctx, dt, tol=1e-12, max_iter=100000):
+    it = C.c_int()
+    _check(ctx, lib().lgt_md_step(ctx, dt, tol, max_iter, C.byref(it)))
+    return it.value
+
+
+def lgt_md_trajectory(ctx, nsteps, dt, tol=1e-12, max_iter=100000, measure=True):
+    """Returns (H_initial, H_final, cg_iters)."""
+    h0, h1, its = C.c_double(), C.c_double(), C.c_long()
+    _check(ctx, lib().lgt_md_trajectory(ctx, nsteps, dt, tol, max_iter,
+                                        C.byref(h0) if measure else None, C.byref(h1) if measure else None,
+                                        C.byref(its)))
+    return h0.value, h1.value, its.value
+
+
+def lgt_native_spinor_bytes(ctx):
+    return lib().lgt_native_spinor_bytes(ctx)
+
+
+def lgt_spinor_to_native(ctx, canonical, native):
+    return _check(ctx, lib().lgt_spinor_to_native(ctx, _ptr(canonical), _ptr(native)))
+
+
+def lgt_spinor_from_native(ctx, native, canonical):
+    return _check(ctx, lib().lgt_spinor_from_native(ctx, _ptr(native), _ptr(canonical)))
+
+
+def lgt_dslash_native(ctx, inp, out, dagger=False):
+    return _check(ctx, lib().lgt_dslash_native(ctx, _ptr(inp), _ptr(out), int(bool(dagger))))
+
+
+def lgt_fermion_force_native(ctx, X, Y, eps):
+    return _check(ctx, lib().lgt_fermion_force_native(ctx, _ptr(X), _ptr(Y), eps))
+
+
+def lgt_gauge_force_accumulate(ctx, eps):
+    return _check(ctx, lib().lgt_gauge_force_accumulate(ctx, eps))
+
+
+def lgt_cg_native(ctx, b, x, y, tol, max_iter):
+    it, rel = C.c_int(), C.c_double()
+    rc = _check(ctx, lib().lgt_cg_native(ctx, _ptr(b), _ptr(x), _ptr(y), tol, max_iter, C.byref(it), C.byref(rel)),
+                allow=(LGT_ENOCONV,))
+    return it.value, rel.value, rc == LGT_OK
+
+
+def lgt_launch_count(ctx):
+    return lib().lgt_launch_count(ctx)
+
+
+# ---- convenience wrapper -----------------------------------------------------------------------
+class Lattice:
+    """A handle plus torch buffers in the canonical layout.  numpy in / numpy out helpers for tests."""
+
+    def __init__(self, dims, beta, kappa, bc, precision=LGT_F64, device=0, stream=None):
+        import torch
+
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_2602_20516_b200 needs a CUDA device (there is no CPU fallback)")
+        self.torch = torch
+        self.dims = tuple(int(d) for d in dims)
+        self.V = 1
+        for d in self.dims:
+            self.V *= d
+        self.precision = precision
+        self.cdtype = torch.complex128 if precision == LGT_F64 else torch.complex64
+        self.device = torch.device("cuda", device)
+        self.ctx = lgt_create(dims, beta, kappa, bc, precision, device, stream)
+
+    def close(self):
+        if self.ctx is not None:
+            lgt_destroy(self.ctx)
+            self.ctx = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # device tensors
+    def empty(self, *shape):
+        return self.torch.empty(shape, dtype=self.cdtype, device=self.device)
+
+    def to_device(self, a):
+        return self.torch.from_numpy(a).to(self.cdtype).to(self.device).contiguous()
+
+    def native_spinor(self):
+        return self.torch.empty(lgt_native_spinor_bytes(self.ctx), dtype=self.torch.uint8, device=self.device)
+
+    # numpy helpers (upload, call, download)
+    def set_links(self, U):
+        lgt_set_links(self.ctx, self.to_device(U))
+
+    def get_links(self):
+        out = self.empty(self.V, 4, 3, 3)
+        lgt_get_links(self.ctx, out)
+        return out.cpu().numpy()
+
+    def set_momenta(self, P):
+        lgt_set_momenta(self.ctx, self.to_device(P))
+
+    def get_momenta(self):
+        out = self.empty(self.V, 4, 3, 3)
+        lgt_get_momenta(self.ctx, out)
+        return out.cpu().numpy()
+
+    def set_pseudofermion(self, phi):
+        lgt_set_pseudofermion(self.ctx, self.to_device(phi))
+
+    def dslash(self, psi, dagger=False):
+        out = self.empty(self.V, 4, 3)
+        lgt_dslash(self.ctx, self.to_device(psi), out, dagger)
+        return out.cpu().numpy()
+
+    def cg(self, b, tol, max_iter):
+        x = self.empty(self.V, 4, 3)
+        it, rel, ok = lgt_cg(self.ctx, self.to_device(b), x, tol, max_iter)
+        return x.cpu().numpy(), it, rel, ok
+
+    def gauge_force(self):
+        F = self.empty(self.V, 4, 3, 3)
+        lgt_gauge_force(self.ctx, F)
+        return F.cpu().numpy()
+
+    def fermion_force(self, X=None, Y=None, tol=1e-12, max_iter=100000):
+        F = self.empty(self.V, 4, 3, 3)
+        it = lgt_fermion_force(self.ctx, None if X is None else self.to_device(X),
+                               None if Y is None else self.to_device(Y), F, tol, max_iter)
+        return F.cpu().numpy(), it

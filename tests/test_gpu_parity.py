@@ -1,0 +1,288 @@
+"""GPU parity: the CUDA path through the C ABI vs the CPU oracle, element by element, on the same
+seeded inputs.  Tolerances (BASELINE.json north_star): per link / per site relative 1e-11 in fp64,
+2e-5 in fp32; CG iteration counts identical in fp64.
+"""
+import numpy as np
+import pytest
+
+import oracle
+from paper_2602_20516_b200 import synth
+from lattice_util import link_rel_err
+
+pytestmark = pytest.mark.gpu
+
+BC = (1, 1, 1, -1)
+TOL64 = 1e-11
+TOL32 = 2e-5
+
+
+@pytest.fixture(scope="module")
+def lgt():
+    import torch
+
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device; the product path has no CPU fallback")
+    from paper_2602_20516_b200 import lgt as m
+
+    m.lib()
+    return m
+
+
+def site_rel_err(a, ref):
+    """max over sites of |a - ref|_2 / |ref|_2 per site (12 complex numbers)."""
+    d = np.sqrt(np.sum(np.abs(a - ref) ** 2, axis=(-1, -2)))
+    n = np.sqrt(np.sum(np.abs(ref) ** 2, axis=(-1, -2)))
+    return float((d / n).max())
+
+
+def round32(a):
+    return a.astype(np.complex64).astype(np.complex128)
+
+
+# dims spanning several 128-thread blocks with ragged tails, odd extents, extents of 1 and 2
+DSLASH_DIMS = [(4, 4, 4, 4), (4, 3, 5, 6), (8, 8, 8, 8), (6, 2, 1, 10), (16, 16, 16, 16), (3, 3, 3, 3)]
+
+
+@pytest.mark.parametrize("dims", DSLASH_DIMS)
+@pytest.mark.parametrize("dag", [False, True])
+def test_dslash_fp64(lgt, dims, dag):
+    U = synth.warm_links(dims, 0.3, 7)
+    psi = synth.gaussian_spinor(dims, 8)
+    for bc in (BC, (1, 1, 1, 1), (-1, -1, 1, -1)):
+        lat = lgt.Lattice(dims, 5.6, 0.12, bc)
+        lat.set_links(U)
+        out = lat.dslash(psi, dagger=dag)
+        ref = oracle.dslash(dims, 0.12, bc, U, psi, dagger=dag)
+        assert site_rel_err(out, ref) < TOL64
+        lat.close()
+
+
+@pytest.mark.parametrize("dims", [(4, 3, 5, 6), (16, 16, 16, 16)])
+def test_dslash_fp32(lgt, dims):
+    U = round32(synth.warm_links(dims, 0.3, 7))
+    psi = round32(synth.gaussian_spinor(dims, 8))
+    lat = lgt.Lattice(dims, 5.6, 0.12, BC, precision=lgt.LGT_F32)
+    lat.set_links(U)
+    for dag in (False, True):
+        out = lat.dslash(psi, dagger=dag).astype(np.complex128)
+        ref = oracle.dslash(dims, 0.12, BC, U, psi, dagger=dag)
+        assert site_rel_err(out, ref) < TOL32
+    lat.close()
+
+
+def test_links_momenta_roundtrip(lgt):
+    dims = (4, 3, 5, 6)
+    U = synth.warm_links(dims, 0.3, 1)
+    P = synth.gaussian_momenta(dims, 2)
+    lat = lgt.Lattice(dims, 5.6, 0.12, BC)
+    assert np.array_equal(lat.get_links(), synth.unit_links(dims))  # initial state
+    assert not lat.get_momenta().any()
+    lat.set_links(U)
+    lat.set_momenta(P)
+    assert np.array_equal(lat.get_links(), U)
+    assert np.abs(lat.get_momenta() - P).max() < 1e-15
+    lat.close()
+
+
+@pytest.mark.parametrize("cfg", [0, 2])
+def test_cg_and_fermion_force_configs(lgt, cfg):
+    """configs[0] (4^4, tol 1e-14) and configs[2] (16^4, tol 1e-12): CG iteration count identical, X, Y = D X = eta,
+    S_F = |eta|^2 and the per-link force (Eq. 8 of the paper) against the oracle."""
+    c = synth.CONFIGS[cfg]
+    dims, kappa, bc, tol = c["dims"], c["kappa"], c["bc"], c["cg_tol"]
+    V = synth.volume(dims)
+    U = synth.config_links(cfg)
+    eta = synth.gaussian_spinor(dims, c["seed_eta"])
+    phi = oracle.dslash(dims, kappa, bc, U, eta, dagger=True)
+    X_ref, it_ref, rel_ref, ok_ref = oracle.cg(dims, kappa, bc, U, phi, tol, 10 * V)
+    Y_ref = oracle.dslash(dims, kappa, bc, U, X_ref)
+    F_ref = oracle.fermion_force(dims, kappa, bc, U, X_ref, Y_ref)
+    assert ok_ref
+
+    lat = lgt.Lattice(dims, 5.5, kappa, bc)
+    lat.set_links(U)
+    X, it, rel, ok = lat.cg(phi, tol, 10 * V)
+    assert ok and it == it_ref, (it, it_ref, rel, rel_ref)
+    assert rel <= tol
+    assert site_rel_err(X, X_ref) < 1e-9  # solution agrees to tol * sqrt(cond)
+    # force kernel alone, shared X and Y: rounding level
+    F_shared, _ = lat.fermion_force(X_ref, Y_ref)
+    e, plain = link_rel_err(F_shared, F_ref)
+    assert e < 1e-13, (e, plain)
+    # end to end from phi through the GPU's own CG
+    lat.set_pseudofermion(phi)
+    F, it2 = lat.fermion_force(None, None, tol=tol, max_iter=10 * V)
+    assert it2 == it_ref
+    e, plain = link_rel_err(F, F_ref)
+    assert e < TOL64, (e, plain)
+    # closed forms (pin P6): S_F = |eta|^2
+    S_g, S_F, K, _ = lgt.lgt_action(lat.ctx, tol, 10 * V)
+    n2 = np.sum(np.abs(eta) ** 2)
+    assert abs(S_F - n2) < 1e-11 * n2
+    S_g_ref, _ = oracle.gauge_action(dims, 5.5, U)
+    assert abs(S_g - S_g_ref) < 1e-12 * abs(S_g_ref)
+    lat.close()
+
+
+def test_fermion_force_fp32(lgt):
+    dims, kappa = (8, 8, 8, 8), 0.12
+    U = round32(synth.warm_links(dims, 0.3, 3))
+    X = round32(synth.gaussian_spinor(dims, 4))
+    Y = round32(synth.gaussian_spinor(dims, 5))
+    lat = lgt.Lattice(dims, 5.6, kappa, BC, precision=lgt.LGT_F32)
+    lat.set_links(U)
+    F, _ = lat.fermion_force(X, Y)
+    e, plain = link_rel_err(F.astype(np.complex128), oracle.fermion_force(dims, kappa, BC, U, X, Y))
+    assert e < TOL32, (e, plain)
+    lat.close()
+
+
+@pytest.mark.parametrize("dims", [(4, 3, 5, 6), (8, 8, 8, 8), (6, 2, 1, 10)])
+def test_gauge_force_and_action(lgt, dims):
+    beta = 6.0
+    U = synth.haar_links(dims, 1101)
+    lat = lgt.Lattice(dims, beta, 0.0, (1, 1, 1, 1))
+    lat.set_links(U)
+    F = lat.gauge_force()
+    e, plain = link_rel_err(F, oracle.gauge_force(dims, beta, U))
+    assert e < 1e-13, (e, plain)
+    S_ref, plaq_ref = oracle.gauge_action(dims, beta, U)
+    S_g, S_F, K, _ = lgt.lgt_action(lat.ctx)
+    assert abs(S_g - S_ref) < 1e-12 * abs(S_ref) and S_F == 0.0 and K == 0.0
+    assert abs(lgt.lgt_plaquette(lat.ctx) - plaq_ref) < 1e-14
+    lat.close()
+    # fp32
+    U32 = round32(U)
+    lat = lgt.Lattice(dims, beta, 0.0, (1, 1, 1, 1), precision=lgt.LGT_F32)
+    lat.set_links(U32)
+    e, plain = link_rel_err(lat.gauge_force().astype(np.complex128), oracle.gauge_force(dims, beta, U32))
+    assert e < TOL32, (e, plain)
+    lat.close()
+
+
+def test_unit_gauge(lgt):
+    dims = (4, 4, 4, 4)
+    lat = lgt.Lattice(dims, 5.5, 0.1, BC)
+    assert lgt.lgt_plaquette(lat.ctx) == 1.0
+    S_g, S_F, K, _ = lgt.lgt_action(lat.ctx)
+    assert S_g == 0.0
+    assert not lat.gauge_force().any()
+    lat.close()
+
+
+@pytest.mark.parametrize("scale", [1e-9, 1e-3, 0.02, 1.0, 4.0])
+def test_drift_matches_taylor_exponential(lgt, scale):
+    dims = (4, 3, 5, 6)
+    U = synth.warm_links(dims, 0.3, 1)
+    P = synth.gaussian_momenta(dims, 2)
+    # degenerate eigenvalue corners of the Cayley-Hamilton form: lambda_8 direction (both signs), zero momentum
+    l8 = 0.5j * synth.gell_mann()[7]
+    P[0, 0], P[1, 0], P[2, 0] = l8, -l8, 0.0
+    lat = lgt.Lattice(dims, 5.6, 0.12, BC)
+    lat.set_links(U)
+    lat.set_momenta(P)
+    lgt.lgt_md_drift(lat.ctx, scale)
+    ref = oracle.drift(dims, scale, P, U)
+    assert np.abs(lat.get_links() - ref).max() < 2e-14 * max(1.0, scale)
+    lat.close()
+
+
+def test_kick_and_momentum_kinetic(lgt):
+    c = synth.CONFIGS[0]
+    dims, beta, kappa, bc = c["dims"], c["beta"], c["kappa"], c["bc"]
+    U = synth.config_links(0)
+    P = synth.gaussian_momenta(dims, 5)
+    phi = oracle.dslash(dims, kappa, bc, U, synth.gaussian_spinor(dims, c["seed_eta"]), dagger=True)
+    lat = lgt.Lattice(dims, beta, kappa, bc)
+    lat.set_links(U)
+    lat.set_momenta(P)
+    lat.set_pseudofermion(phi)
+    S_g, S_F, K, _ = lgt.lgt_action(lat.ctx, 1e-13, 5000)
+    assert abs(K - oracle.kinetic(dims, P)) < 1e-12 * K
+    it = lgt.lgt_md_kick(lat.ctx, 0.05, 1e-13, 5000)
+    P_ref, it_ref, ok = oracle.kick(dims, beta, kappa, bc, U, phi, P, 0.05, 1e-13, 5000)
+    assert ok and it == it_ref
+    e, plain = link_rel_err(lat.get_momenta(), P_ref)
+    assert e < TOL64
+    lat.close()
+
+
+def test_config1_leapfrog_trajectory(lgt):
+    """configs[1]: 8^4 gauge-only, Haar links, 50 leapfrog steps at dt = 0.02: final state against the oracle's
+    trajectory, dH against the oracle's dH, dt^2 scaling and reversibility on the GPU itself."""
+    c = synth.CONFIGS[1]
+    dims, beta, bc = c["dims"], c["beta"], c["bc"]
+    U0 = synth.config_links(1)
+    P0 = synth.gaussian_momenta(dims, c["seed_mom"])
+    lat = lgt.Lattice(dims, beta, 0.0, bc)
+    lat.set_links(U0)
+    lat.set_momenta(P0)
+    H0, H1, _ = lgt.lgt_md_trajectory(lat.ctx, c["nsteps"], c["dt"])
+    U1, P1 = lat.get_links(), lat.get_momenta()
+    U_ref, P_ref, _, _ = oracle.trajectory(dims, beta, 0.0, bc, U0, None, P0, c["nsteps"], c["dt"])
+    H0_ref = oracle.hamiltonian(dims, beta, 0.0, bc, U0, None, P0)[0]
+    H1_ref = oracle.hamiltonian(dims, beta, 0.0, bc, U_ref, None, P_ref)[0]
+    assert abs(H0 - H0_ref) < 1e-12 * abs(H0_ref)
+    assert abs((H1 - H0) - (H1_ref - H0_ref)) < 1e-9 * abs(H0_ref) + 1e-6 * abs(H1_ref - H0_ref)
+    assert np.abs(U1 - U_ref).max() < 1e-11
+    assert link_rel_err(P1, P_ref)[0] < TOL64
+    # reversibility: flip the momenta, run again
+    lat.set_momenta(-P1)
+    lgt.lgt_md_trajectory(lat.ctx, c["nsteps"], c["dt"], measure=False)
+    assert np.abs(lat.get_links() - U0).max() < 1e-11
+    assert np.abs(lat.get_momenta() + P0).max() < 1e-10
+    # dt -> dt/2 at fixed length: |dH| drops by about 4
+    lat.set_links(U0)
+    lat.set_momenta(P0)
+    h0, h1, _ = lgt.lgt_md_trajectory(lat.ctx, 2 * c["nsteps"], c["dt"] / 2)
+    ratio = (H1 - H0) / (h1 - h0)
+    assert 3.5 < ratio < 4.5, ratio
+    lat.close()
+
+
+def test_md_step_with_fermions(lgt):
+    c = synth.CONFIGS[0]
+    dims, beta, kappa, bc = c["dims"], c["beta"], c["kappa"], c["bc"]
+    U0 = synth.config_links(0)
+    P0 = synth.gaussian_momenta(dims, 73)
+    phi = oracle.dslash(dims, kappa, bc, U0, synth.gaussian_spinor(dims, c["seed_eta"]), dagger=True)
+    lat = lgt.Lattice(dims, beta, kappa, bc)
+    lat.set_links(U0)
+    lat.set_momenta(P0)
+    lat.set_pseudofermion(phi)
+    its = lgt.lgt_md_step(lat.ctx, 0.05, 1e-13, 5000)
+    U_ref, P_ref, its_ref, ok = oracle.trajectory(dims, beta, kappa, bc, U0, phi, P0, 1, 0.05, tol=1e-13, max_iter=5000)
+    assert ok and its == its_ref
+    assert np.abs(lat.get_links() - U_ref).max() < 1e-12
+    assert link_rel_err(lat.get_momenta(), P_ref)[0] < TOL64
+    lat.close()
+
+
+def test_error_paths(lgt):
+    with pytest.raises(lgt.LgtError) as e:
+        lgt.lgt_create((4, 4, 4, 0), 5.5, 0.1, BC)
+    assert e.value.code == lgt.LGT_EINVAL
+    with pytest.raises(lgt.LgtError):
+        lgt.lgt_create((4, 4, 4, 4), 5.5, 0.1, (1, 1, 1, 0))
+    with pytest.raises(lgt.LgtError):
+        lgt.lgt_create((4, 4, 4, 4), 5.5, 0.1, BC, precision=7)
+    lat = lgt.Lattice((4, 4, 4, 4), 5.5, 0.1, BC)
+    with pytest.raises(lgt.LgtError) as e:
+        lgt.lgt_set_links(lat.ctx, None)
+    assert e.value.code == lgt.LGT_EINVAL
+    F = lat.empty(lat.V, 4, 3, 3)
+    with pytest.raises(lgt.LgtError) as e:  # no pseudofermion set
+        lgt.lgt_fermion_force(lat.ctx, None, None, F)
+    assert e.value.code == lgt.LGT_ESTATE
+    # CG cap: reports non-convergence, leaves the last iterate
+    U = synth.warm_links((4, 4, 4, 4), 0.3, 1)
+    lat.set_links(U)
+    b = synth.gaussian_spinor((4, 4, 4, 4), 2)
+    x, it, rel, ok = lat.cg(b, 1e-13, 3)
+    x_ref, it_ref, rel_ref, ok_ref = oracle.cg((4, 4, 4, 4), 0.1, BC, U, b, 1e-13, 3)
+    assert not ok and it == 3 and not ok_ref and abs(rel - rel_ref) < 1e-12
+    assert site_rel_err(x, x_ref) < 1e-12
+    # zero right-hand side: zero iterations, zero solution
+    x, it, rel, ok = lat.cg(np.zeros_like(b), 1e-13, 10)
+    assert ok and it == 0 and not x.any()
+    lat.close()
