@@ -1,0 +1,399 @@
+#!/usr/bin/env python
+"""bench.py -- one JSON line for the HMC MD-step hot path on B200.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 3]
+
+A "step" is one molecular-dynamics step of BASELINE.json configs[3] in the reading DESIGN.md A-13:
+kick(dt) = gauge force + CG on D^dag D to 1e-12 + Y = D X + fused fermion force, then drift(dt) = link update,
+on a 32^4 SU(3) lattice in fp64 (beta 5.6, kappa 0.12, antiperiodic time, dt 0.01, seeded warm-start links).
+`value` is the algorithmic HBM traffic of all kernels of the step divided by
+the device time of the step; `kernels` holds the metric's two named kernels (Dslash, fermion force) timed
+in isolation; `roofline` is the dominant kernel (Dslash inside CG) timed in place with CUDA events.
+N > 1: N independent replicas (one lattice per GPU, no data-path collective), weak scaling.
+--impl reference times the CPU oracle on a bounded sample of the same workload (rank 0 only).
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "fermion-force + Dslash HBM GB/s and GFLOP/s (fp64, 32^4) vs B200 roofline"
+
+# Algorithmic bytes and flops per site in units of one REAL number (x8 B in fp64, x4 B in fp32); DESIGN.md.
+REALS = dict(
+    dslash=2 * (36 + 12 + 12),               # U + in + out                      -> 960 B fp64
+    dslash_fused_r=2 * (36 + 12 + 2 * 12),   # U + t + r rw (q = D^dag t stays on chip) -> 1152 B
+    cg_update_xp=2 * (5 * 12),               # x rw, p rw, r r                   -> 960 B
+    cg_iter=2 * (60 + 72 + 60),              # the three launches above          -> 3072 B
+    cg_init=2 * (4 * 12),                    # b r; x, r, p w
+    fermion_force=2 * (36 + 12 + 12) + 2 * 32,  # U + X + Y + Pi (8 reals x 4 links) rw -> 1472 B
+    gauge_force=2 * 36 + 2 * 32,             # U + Pi rw                         -> 1088 B
+    link_update=32 + 2 * 2 * 36,             # Pi r + U rw                       -> 1408 B
+)
+FLOPS = dict(dslash=1368, dslash_fused_r=1368 + 96, cg_update_xp=96, cg_iter=2 * 1368 + 192, fermion_force=2300, gauge_force=10900, link_update=3500)
+
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel from the ncu --set full capture
+# summarised in profiles/ (None until captured for the current kernel).
+NCU_TRAFFIC_BYTES = {"dslash_f64_32^4": None}
+
+
+def step_reals(cg_iters):
+    return (REALS["gauge_force"] + REALS["cg_init"] + cg_iters * REALS["cg_iter"] + REALS["dslash"]
+            + REALS["fermion_force"] + REALS["link_update"])
+
+
+def step_flops(cg_iters):
+    return (FLOPS["gauge_force"] + cg_iters * FLOPS["cg_iter"] + FLOPS["dslash"] + FLOPS["fermion_force"]
+            + FLOPS["link_update"])
+
+
+def measured_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        try:
+            return float(json.load(open(path))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, copy bandwidth)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        self.thread.join(timeout=2)
+        sm = sorted(float(r[0]) for r in self.rows if len(r) >= 7 and r[0].replace(".", "").isdigit())
+        mx = [float(r[1]) for r in self.rows if len(r) >= 7 and r[1].replace(".", "").isdigit()]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [n for i, n in enumerate(names) if any(len(r) >= 7 and r[3 + i].lower() == "active" for r in self.rows)]
+        pw = [float(r[2]) for r in self.rows if len(r) >= 7 and r[2].replace(".", "").isdigit()]
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": reasons}
+
+
+def make_inputs(cfg):
+    """Seeded synthetic fields of the workload (numpy, canonical layout)."""
+    from paper_2602_20516_b200 import synth
+
+    dims = cfg["dims"]
+    U = synth.config_links(cfg)
+    P = synth.gaussian_momenta(dims, cfg.get("seed_mom", cfg["seed_links"] + 1))
+    eta = synth.gaussian_spinor(dims, cfg.get("seed_eta", cfg["seed_links"] + 2))
+    return U, P, eta
+
+
+# ------------------------------------------------------------------------------------------------ our arm
+def run_ours(args):
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+
+    from paper_2602_20516_b200 import lgt, synth
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    lgt.lib()
+
+    cfg = dict(synth.CONFIGS[args.config])
+    if args.lattice:
+        cfg["dims"] = tuple(args.lattice)
+    cfg["seed_links"] += 100 * rank  # replicas: one independent lattice per GPU
+    dims, beta, kappa, bc = cfg["dims"], cfg["beta"], cfg["kappa"], cfg["bc"]
+    tol, dt = cfg.get("cg_tol", 1e-12), cfg.get("dt", 0.01)
+    V = synth.volume(dims)
+    max_iter = 10 * V
+    U, P, eta = make_inputs(cfg)
+
+    stream = torch.cuda.current_stream().cuda_stream
+    lat = lgt.Lattice(dims, beta, kappa, bc, lgt.LGT_F64, local, stream)
+    ctx = lat.ctx
+    hU, hP = torch.from_numpy(U).pin_memory(), torch.from_numpy(P).pin_memory()
+    d_eta, d_phi = lat.to_device(eta), lat.empty(V, 4, 3)
+    lgt.lgt_set_links_host(ctx, hU)
+    lgt.lgt_dslash(ctx, d_eta, d_phi, True)  # phi = D^dag eta, made by the CUDA path itself
+    hphi = d_phi.cpu().pin_memory()
+    hU_out, hP_out = torch.empty_like(hU), torch.empty_like(hP)
+    del U, P, eta, d_eta
+
+    def reset_state():
+        lgt.lgt_set_links_host(ctx, hU)
+        lgt.lgt_set_momenta_host(ctx, hP)
+        lgt.lgt_set_pseudofermion_host(ctx, hphi)
+
+    def md_step():
+        it = lgt.lgt_md_kick(ctx, dt, tol, max_iter)
+        lgt.lgt_md_drift(ctx, dt)
+        return it
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    reset_state()
+    for _ in range(args.warmup):
+        md_step()
+
+    # ---- timed region: K steps, device time by CUDA events on the handle's stream, max over ranks
+    sampler = ClockSampler(local)
+    lgt.lgt_timing_reset(ctx)
+    lgt.lgt_timing_enable(ctx, True)
+    launches0 = lgt.lgt_launch_count(ctx)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    sampler.start()
+    barrier()
+    e0.record()
+    iters = [md_step() for _ in range(args.steps)]
+    e1.record()
+    barrier()
+    clocks = sampler.stop()
+    lgt.lgt_timing_enable(ctx, False)
+    elapsed_ms = e0.elapsed_time(e1)
+    launches = lgt.lgt_launch_count(ctx) - launches0
+    per_class = {name: lgt.lgt_timing_read(ctx, k) for k, name in enumerate(lgt.KERNEL_CLASSES)}
+    lgt.lgt_timing_reset(ctx)
+    total_reals = sum(step_reals(i) for i in iters) * V
+    total_flops = sum(step_flops(i) for i in iters) * V
+
+    # ---- end to end: host buffers in, host buffers out, through the C ABI, every step
+    k_e2e = max(1, min(args.steps, 3))
+    barrier()
+    t0 = time.perf_counter()
+    e2e_iters = []
+    for _ in range(k_e2e):
+        reset_state()
+        e2e_iters.append(md_step())
+        lgt.lgt_get_links_host(ctx, hU_out)
+        lgt.lgt_get_momenta_host(ctx, hP_out)
+    torch.cuda.synchronize()
+    e2e_s = time.perf_counter() - t0
+    e2e_reals = sum(step_reals(i) for i in e2e_iters) * V
+    h2d = hU.numel() * 16 + hP.numel() * 16 + hphi.numel() * 16
+    d2h = hU_out.numel() * 16 + hP_out.numel() * 16
+
+    # ---- max over ranks, aggregate
+    stats = torch.tensor([elapsed_ms, e2e_s], dtype=torch.float64, device="cuda")
+    sums = torch.tensor([total_reals, total_flops, e2e_reals, launches], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(stats, op=dist.ReduceOp.MAX)
+        dist.all_reduce(sums, op=dist.ReduceOp.SUM)
+    elapsed_ms, e2e_s = stats.tolist()
+    total_reals, total_flops, e2e_reals, launches_all = sums.tolist()
+
+    # ---- the metric's two kernels in isolation (inputs exceed L2: links 604 MB, spinors 201 MB each)
+    kernels = {}
+
+    def time_kernel(fn, n=20, warm=5):
+        for _ in range(warm):
+            fn()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        a.record()
+        for _ in range(n):
+            fn()
+        b.record()
+        torch.cuda.synchronize()
+        return a.elapsed_time(b) / n * 1e-3
+
+    def isolated(handle, real_bytes, tag):
+        hctx = handle.ctx
+        g = torch.Generator(device="cuda")
+        g.manual_seed(5)
+        bufs = []
+        for _ in range(3):
+            b = handle.native_spinor()
+            b.view(torch.float64 if real_bytes == 8 else torch.float32).normal_(generator=g)
+            bufs.append(b)
+        for name, fn, key in (
+                ("dslash", lambda: lgt.lgt_dslash_native(hctx, bufs[0], bufs[1], False), "dslash"),
+                ("dslash_dagger", lambda: lgt.lgt_dslash_native(hctx, bufs[0], bufs[1], True), "dslash"),
+                ("fermion_force", lambda: lgt.lgt_fermion_force_native(hctx, bufs[0], bufs[2], 1e-3), "fermion_force"),
+                ("gauge_force", lambda: lgt.lgt_gauge_force_accumulate(hctx, 1e-3), "gauge_force"),
+                ("link_update", lambda: lgt.lgt_md_drift(hctx, 1e-6), "link_update")):
+            t = time_kernel(fn)
+            kernels[name + tag] = {"us": round(t * 1e6, 2), "GB/s": round(REALS[key] * real_bytes * V / t / 1e9, 1),
+                                   "GFLOP/s": round(FLOPS[key] * V / t / 1e9, 1)}
+
+    if rank == 0:
+        isolated(lat, 8, "_f64")
+        lat32 = lgt.Lattice(dims, beta, kappa, bc, lgt.LGT_F32, local, stream)
+        lgt.lgt_get_links(ctx, d_U := lat.empty(V, 4, 3, 3))
+        lgt.lgt_set_links(lat32.ctx, d_U.to(torch.complex64))
+        del d_U
+        isolated(lat32, 4, "_f32")
+        lat32.close()
+
+    if rank != 0:
+        lat.close()
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    peak, peak_src = measured_peaks()
+    ds_ms, ds_n = per_class["dslash"]
+    ds_avg_s = ds_ms / max(ds_n, 1) * 1e-3
+    ds_bytes = REALS["dslash"] * 8 * V
+    achieved = ds_bytes / ds_avg_s / 1e9 if ds_n else None
+    shares = {name: round(ms / elapsed_ms, 4) for name, (ms, n) in per_class.items() if n}
+    in_place = {}
+    for name, key in (("dslash", "dslash"), ("dslash_dag_fused_r", "dslash_fused_r"), ("cg_blas1", "cg_update_xp"),
+                      ("fermion_force", "fermion_force"), ("gauge_force", "gauge_force"), ("link_update", "link_update")):
+        ms, n = per_class[name]
+        if n:
+            in_place[name] = {"launches": n, "avg_us": round(ms / n * 1e3, 2),
+                              "GB/s": round(REALS[key] * 8 * V / (ms / n * 1e-3) / 1e9, 1)}
+    value = total_reals * 8 / (elapsed_ms * 1e-3) / 1e9
+    out = {
+        "metric": METRIC,
+        "value": round(value, 1),
+        "unit": "GB/s",
+        "n_gpus": world,
+        "steps": args.steps,
+        "warmup": args.warmup,
+        "ms_per_step": round(elapsed_ms / args.steps, 3),
+        "higher_is_better": True,
+        "scaling": "weak",
+        "vs_baseline": None,
+        "dtype": "f64",
+        "data": "synthetic",
+        "config": {"workload": "configs[%d]: %s SU(3) one MD step = kick(dt) [gauge force, CG 1e-12 on D^dag D, Y = D X, "
+                               "fermion force] + drift(dt)" % (args.config, "x".join(map(str, dims))),
+                   "beta": beta, "kappa": kappa, "bc": list(bc), "dt": dt, "cg_tol": tol,
+                   "cg_iters_per_step": iters, "parallelism": "replicas x%d" % world,
+                   "l2": "inputs exceed L2 (links 604 MB, each spinor 201 MB at 32^4)"},
+        "gflops": round(total_flops / (elapsed_ms * 1e-3) / 1e9, 1),
+        "clocks": clocks,
+        "e2e": {"value": round(e2e_reals * 8 / e2e_s / 1e9, 1), "unit": "GB/s", "steps": k_e2e,
+                "ms_per_step": round(e2e_s / k_e2e * 1e3, 2), "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
+        "gpu_launches": int(launches_all),
+        "roofline": {"kernel": "dslash_kernel<double> (inside CG, %d launches)" % ds_n, "bound": "hbm",
+                     "achieved": round(achieved, 1) if achieved else None, "peak": peak, "unit": "GB/s",
+                     "frac": round(achieved / peak, 4) if achieved else None,
+                     "frac_of_nominal_8TBs": round(achieved / 8000.0, 4) if achieved else None,
+                     "peak_source": peak_src, "avg_launch_us": round(ds_avg_s * 1e6, 2),
+                     "algorithmic_bytes_per_launch": ds_bytes,
+                     "traffic": NCU_TRAFFIC_BYTES.get("dslash_f64_32^4") if tuple(dims) == (32, 32, 32, 32) else None,
+                     "share_of_step": shares, "kernels_in_place": in_place},
+        "kernels": kernels,
+    }
+    if world == 1 and not args.skip_cpu_baseline:
+        out["cpu_baseline"] = cpu_baseline(cfg, sample_iters=args.cpu_sample_iters)
+    lat.close()
+    if world > 1:
+        dist.destroy_process_group()
+    print(json.dumps(out), flush=True)
+
+
+# ------------------------------------------------------------------------------------------------ the oracle, timed
+def oracle_step(oracle, cfg, U, P, phi, sample_iters):
+    """One bounded sample of the MD step on the CPU oracle: same kick + drift, CG capped at sample_iters."""
+    dims, beta, kappa, bc = cfg["dims"], cfg["beta"], cfg["kappa"], cfg["bc"]
+    t0 = time.perf_counter()
+    P1, it, _ = oracle.kick(dims, beta, kappa, bc, U, phi, P, cfg.get("dt", 0.01), cfg.get("cg_tol", 1e-12), sample_iters)
+    oracle.drift(dims, cfg.get("dt", 0.01), P1, U)
+    return time.perf_counter() - t0, it
+
+
+def cpu_baseline(cfg, sample_iters, steps=1, warmup=0):
+    import oracle
+    from paper_2602_20516_b200 import synth
+
+    V = synth.volume(cfg["dims"])
+    U, P, eta = make_inputs(cfg)
+    phi = oracle.dslash(cfg["dims"], cfg["kappa"], cfg["bc"], U, eta, dagger=True)
+    for _ in range(warmup):
+        oracle_step(oracle, cfg, U, P, phi, sample_iters)
+    t, reals = 0.0, 0
+    for _ in range(steps):
+        dt_s, it = oracle_step(oracle, cfg, U, P, phi, sample_iters)
+        t += dt_s
+        reals += step_reals(it) * V
+    return {"value": round(reals * 8 / t / 1e9, 3), "unit": "GB/s", "cores": oracle.num_threads(), "kind": "oracle",
+            "seconds_per_sample": round(t / steps, 2),
+            "sample": "same %s lattice and fields; one MD step with CG capped at %d iterations "
+                      "(gauge force + %d x (2 Dslash + BLAS-1) + Y = D X + fermion force + drift), same byte accounting"
+                      % ("x".join(map(str, cfg["dims"])), sample_iters, sample_iters)}
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if rank != 0:
+        return
+    from paper_2602_20516_b200 import synth
+
+    cfg = dict(synth.CONFIGS[args.config])
+    if args.lattice:
+        cfg["dims"] = tuple(args.lattice)
+    t0 = time.perf_counter()
+    base = cpu_baseline(cfg, args.cpu_sample_iters, steps=args.steps, warmup=args.warmup)
+    out = {
+        "impl": "reference", "metric": METRIC, "value": base["value"], "unit": "GB/s", "n_gpus": world,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": round(base["seconds_per_sample"] * 1e3, 1),
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "configs[%d]: %s SU(3) MD step on the CPU oracle, bounded sample" %
+                               (args.config, "x".join(map(str, cfg["dims"])))},
+        "cpu_baseline": base,
+        "e2e": {"value": base["value"], "unit": "GB/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "wall_s": round(time.perf_counter() - t0, 1),
+    }
+    print(json.dumps(out), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=3, help="BASELINE.json configs index (3 = 32^4 MD step)")
+    ap.add_argument("--lattice", type=int, nargs=4, default=None, help="override dims (debugging only)")
+    ap.add_argument("--skip-cpu-baseline", action="store_true", help="profiling runs only: leave the oracle leg out")
+    ap.add_argument("--cpu-sample-iters", type=int, default=4, help="CG iterations in the oracle's bounded sample")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "ours":
+        args.warmup = 3  # timing rule: at least 3 warm-up steps
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -135,6 +135,21 @@ int lgt_gauge_force_accumulate(lgt_ctx* ctx, double eps);
 int lgt_cg_native(lgt_ctx* ctx, const void* b, void* x, void* y, double tol, int max_iter,
                   int* iters, double* rel_resid);
 
+/* ---- per-kernel timing (CUDA events on the handle's stream, used by bench.py's roofline line) ---- */
+enum { LGT_K_DSLASH = 0,        /* out = D in, D^dag in, and CG step "t = D p" (+ |t|^2) */
+       LGT_K_CG_BLAS = 1,       /* CG initialisation and the x, p update pass */
+       LGT_K_FERMION_FORCE = 2, LGT_K_GAUGE_FORCE = 3, LGT_K_LINK_UPDATE = 4,
+       LGT_K_OTHER = 5,         /* layout conversion, actions */
+       LGT_K_DSLASH_R = 6,      /* CG step "q = D^dag t, r -= alpha q" (+ |r|^2), q kept on chip */
+       LGT_K_COUNT = 7 };
+/* While enabled, every kernel launch is bracketed by a pair of CUDA events. */
+int lgt_timing_enable(lgt_ctx* ctx, int enable);
+/* Forgets the recorded launches (synchronises the stream). */
+int lgt_timing_reset(lgt_ctx* ctx);
+/* Synchronises, then returns the summed device time (ms) and the number of launches of one kernel class
+ * recorded since the last reset.  Either output may be NULL. */
+int lgt_timing_read(lgt_ctx* ctx, int kernel_class, double* ms_total, long* launches);
+
 /* ---- introspection -------------------------------------------------------------------------- */
 /* Number of kernels this handle has launched since creation (bench.py's gpu_launches). */
 long lgt_launch_count(const lgt_ctx* ctx);

@@ -1,23 +1,30 @@
 // kernels.cuh -- the CUDA kernels of the hot path (sm_100a, CUDA-core FMAs, no tensor cores:
 // 3x3 complex products are not a dense contraction).  Included once by lgt_api.cu.
 //
-// NATIVE LAYOUT (structure of arrays, site-major):
-//   spinor   psi[12][Vs]  complex, component k = 3*alpha + a   -> address (k*Vs + s)
-//   links    U[4][9][Vs]  complex, k = 9*mu + 3*i + j          -> address (k*Vs + s)
-//   momenta  P[4][4][Vs]  pairs of reals (8-real compact su(3)) k = 4*mu + q -> address (k*Vs + s)
-// so that a warp's 32 consecutive sites read 32 consecutive 16-byte words (fp64) per component.
-// s is the canonical lexicographic site index; Vs = V (field stride).
+// NATIVE LAYOUT: array of structures of arrays with 32 sites (one warp)
+// innermost.  With s the canonical lexicographic site index, blk = s / 32, lane = s % 32:
+//   spinor   psi[blk][12][32]   complex, component k = 3*alpha + a
+//   links    U[blk][4][9][32]   complex, component 9*mu + 3*i + j, WITH the fermion boundary sign folded in:
+//                               U_native = s_mu(x) U_mu(x)  (s = bc[mu] on links that cross the mu boundary)
+//   momenta  P[blk][4][4][32]   pairs of reals (8-real compact su(3) per link), component 4*mu + q
+// A warp reads 32 consecutive 16-byte words (fp64) per component, and every component of a site sits at a
+// compile-time offset from one per-site base address, so the hot loops carry almost no address arithmetic.
+// The sign folding is exact (+-1) and invisible to the gauge sector: every plaquette and every U V staple
+// product contains each boundary-crossing link an even number of times, and the link update is linear in U.
+// Fields are padded to a multiple of 32 sites (Vs); padding lanes of spinors and momenta hold zeros.
 #pragma once
 #include "su3.cuh"
 
 namespace lgt {
 
+constexpr int W = 32;  // sites per layout block
+
 struct Geom {
     int L[4];
     int stride[4];  // site-index stride of direction mu
-    int V;
-    int Vs;
-    int bc[4];
+    int V;          // sites
+    int Vs;         // sites padded to a multiple of 32
+    int bc[4];      // fermion boundary signs (used by the layout conversion only)
 };
 
 // CG recurrence scalars, resident on the device so that iterations need no host round trip.
@@ -54,13 +61,24 @@ __device__ __forceinline__ int nbr_bwd(const Geom& g, const Site& c, int s, int 
     return (c.x[mu] == 0) ? s + (g.L[mu] - 1) * g.stride[mu] : s - g.stride[mu];
 }
 
-template <class T> __device__ __forceinline__ void load_link(const typename Vec2<T>::type* U, const Geom& g, int mu, int s, cx<T> u[9]) {
-#pragma unroll
-    for (int k = 0; k < 9; k++) u[k] = ldc<T>(U + (size_t)(9 * mu + k) * g.Vs + s);
+// per-site base pointers; component k of the site is at base + k * W
+template <class P> __device__ __forceinline__ P* spinor_at(P* f, int s) { return f + ((size_t)(s >> 5) * (12 * W) + (s & 31)); }
+template <class P> __device__ __forceinline__ P* link_at(P* U, int s, int mu) {
+    return U + ((size_t)(s >> 5) * (36 * W) + mu * (9 * W) + (s & 31));
 }
-template <class T> __device__ __forceinline__ void load_spinor(const typename Vec2<T>::type* f, const Geom& g, int s, cx<T> p[12]) {
+template <class P> __device__ __forceinline__ P* mom_at(P* Pm, int s, int mu) {
+    return Pm + ((size_t)(s >> 5) * (16 * W) + mu * (4 * W) + (s & 31));
+}
+
+template <class T> __device__ __forceinline__ void load_link(const typename Vec2<T>::type* U, int mu, int s, cx<T> u[9]) {
+    const typename Vec2<T>::type* b = link_at(U, s, mu);
 #pragma unroll
-    for (int k = 0; k < 12; k++) p[k] = ldc<T>(f + (size_t)k * g.Vs + s);
+    for (int k = 0; k < 9; k++) u[k] = ldc<T>(b + k * W);
+}
+template <class T> __device__ __forceinline__ void load_spinor(const typename Vec2<T>::type* f, int s, cx<T> p[12]) {
+    const typename Vec2<T>::type* b = spinor_at(f, s);
+#pragma unroll
+    for (int k = 0; k < 12; k++) p[k] = ldc<T>(b + k * W);
 }
 
 // ---------------------------------------------------------------------------- deterministic reductions
@@ -89,8 +107,23 @@ __device__ __forceinline__ void block_reduce_finalize(double v, double* partials
     __syncthreads();
     if (is_last) {
         __threadfence();
-        double acc = 0.0;
-        for (unsigned i = threadIdx.x; i < gridDim.x; i += blockDim.x) acc += __ldcg(partials + i);
+        // 16 independent loads in flight per thread: this tail runs alone on the GPU, so a dependent
+        // load-add chain would cost one L2 round trip per partial
+        double a16[16];
+#pragma unroll
+        for (int j = 0; j < 16; j++) a16[j] = 0.0;
+        for (unsigned base = threadIdx.x; base < gridDim.x; base += 16 * blockDim.x) {
+#pragma unroll
+            for (int j = 0; j < 16; j++) {
+                const unsigned i = base + j * blockDim.x;
+                if (i < gridDim.x) a16[j] += __ldcg(partials + i);
+            }
+        }
+#pragma unroll
+        for (int w = 8; w > 0; w >>= 1)
+#pragma unroll
+            for (int j = 0; j < w; j++) a16[j] += a16[j + w];
+        double acc = a16[0];
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) acc += __shfl_down_sync(0xffffffffu, acc, o);
         __syncthreads();
@@ -108,57 +141,126 @@ __device__ __forceinline__ void block_reduce_finalize(double v, double* partials
     }
 }
 
+// Block sum only (fixed shuffle tree) to partials[blockIdx.x]; a separate one-block kernel finishes the sum.
+// Used by the two stencil kernels of the CG loop: nothing at the end of the hot kernel waits on an atomic.
+__device__ __forceinline__ void block_partial(double v, double* partials) {
+    __shared__ double warp_sums_p[32];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarp = (blockDim.x + 31) >> 5;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+    if (lane == 0) warp_sums_p[warp] = v;
+    __syncthreads();
+    if (warp == 0) {
+        double w = (lane < nwarp) ? warp_sums_p[lane] : 0.0;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) w += __shfl_down_sync(0xffffffffu, w, o);
+        if (lane == 0) partials[blockIdx.x] = w;
+    }
+}
+
+// One block of 1024 threads: sum of n block partials in a fixed order, then the CG scalar update.
+//   WHAT 1 (after t = D p):        pAp = sum, alpha = rr / pAp
+//   WHAT 2 (after r -= alpha q):   beta = sum / rr, rr = sum, iteration count, convergence flag
+template <int WHAT>
+__global__ void __launch_bounds__(1024) cg_scalars_kernel(int n, const double* __restrict__ partials, CgState* st) {
+    if (st->done) return;
+    __shared__ double warp_sums[32];
+    double a16[16];
+#pragma unroll
+    for (int j = 0; j < 16; j++) a16[j] = 0.0;
+    for (int base = threadIdx.x; base < n; base += 16 * 1024) {
+#pragma unroll
+        for (int j = 0; j < 16; j++) {
+            const int i = base + j * 1024;
+            if (i < n) a16[j] += __ldcg(partials + i);
+        }
+    }
+#pragma unroll
+    for (int w = 8; w > 0; w >>= 1)
+#pragma unroll
+        for (int j = 0; j < w; j++) a16[j] += a16[j + w];
+    double v = a16[0];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+    if (lane == 0) warp_sums[warp] = v;
+    __syncthreads();
+    if (warp == 0) {
+        double sum = warp_sums[lane];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) sum += __shfl_down_sync(0xffffffffu, sum, o);
+        if (lane == 0) {
+            if (WHAT == 1) {
+                st->pAp = sum;
+                st->alpha = st->rr / sum;
+            } else {
+                st->beta = sum / st->rr;
+                st->rr = sum;
+                st->iter += 1;
+                st->done = (!(sum > st->tol2 * st->bb) || st->iter >= st->max_iter) ? 1 : 0;
+            }
+        }
+    }
+}
+
 // ---------------------------------------------------------------------------- A2: Wilson-Dirac operator
-// Forward hop of direction MU: acc += (1 + SG gamma_MU) sign U_MU(s) psi(s+MU)
+// Forward hop of direction MU: acc += (1 + SG gamma_MU) U_MU(s) psi(s+MU)          (boundary sign is in U)
 template <int MU, int SG, class T>
 __device__ __forceinline__ void hop_fwd(const Geom& g, const typename Vec2<T>::type* U, const typename Vec2<T>::type* in,
                                         const Site& c, int s, cx<T> acc[12]) {
     const int sn = nbr_fwd(g, c, s, MU);
     cx<T> p[12], h[6], u[9], w[6];
-    load_spinor<T>(in, g, sn, p);
-    load_link<T>(U, g, MU, s, u);
+    load_spinor<T>(in, sn, p);
+    load_link<T>(U, MU, s, u);
     spin_project<MU, SG>(p, h);
-    if (g.bc[MU] < 0 && c.x[MU] == g.L[MU] - 1) {
-#pragma unroll
-        for (int k = 0; k < 6; k++) h[k] = mk<T>(-h[k].re, -h[k].im);
-    }
     su3_mul_half(u, h, w);
     spin_reconstruct_add<MU, SG>(w, acc);
 }
-// Backward hop: acc += (1 + SG gamma_MU) sign U_MU^dag(s-MU) psi(s-MU)
+// Backward hop: acc += (1 + SG gamma_MU) U_MU^dag(s-MU) psi(s-MU)
 template <int MU, int SG, class T>
 __device__ __forceinline__ void hop_bwd(const Geom& g, const typename Vec2<T>::type* U, const typename Vec2<T>::type* in,
                                         const Site& c, int s, cx<T> acc[12]) {
     const int sn = nbr_bwd(g, c, s, MU);
     cx<T> p[12], h[6], u[9], w[6];
-    load_spinor<T>(in, g, sn, p);
-    load_link<T>(U, g, MU, sn, u);
+    load_spinor<T>(in, sn, p);
+    load_link<T>(U, MU, sn, u);
     spin_project<MU, SG>(p, h);
-    if (g.bc[MU] < 0 && c.x[MU] == 0) {
-#pragma unroll
-        for (int k = 0; k < 6; k++) h[k] = mk<T>(-h[k].re, -h[k].im);
-    }
     su3_dag_mul_half(u, h, w);
     spin_reconstruct_add<MU, SG>(w, acc);
 }
 
-// out = D in (DAG = 0) or D^dag in (DAG = 1).  MODE 0: plain.  MODE 1: CG step "t = D p" with the fused
-// reduction pAp = |t|^2 and alpha = rr / pAp.  MODE 2: CG step "q = D^dag t" (only the done-flag check).
+// One thread per site, all eight hops, accumulators and operands in registers.  The register budget is left
+// to the compiler on purpose (2 blocks of 128 per SM at ~250 registers): on B200 this kernel is bound by memory
+// latency, and the deeper load batching the extra registers allow beats higher occupancy (profiles/).
+//   MODE 0: out = D in (DAG = 0) or D^dag in (DAG = 1).
+//   MODE 1: CG step 1, t = D p, with the fused block partials of |t|^2 (cg_scalars_kernel<1> finishes pAp, alpha).
+//   MODE 2: CG step 2, q = D^dag t kept in registers, r -= alpha q, fused block partials of |r|^2
+//           (cg_scalars_kernel<2> finishes beta, the iteration count and the stop test).  q never touches HBM.
+// In the CG modes the convergence flag is loaded first but tested only after the first hop's loads are in
+// flight, so that its latency is not paid at the head of every block.
 template <class T, int DAG, int MODE>
-__global__ void __launch_bounds__(128) dslash_kernel(Geom g, const typename Vec2<T>::type* __restrict__ U,
-                                                     const typename Vec2<T>::type* __restrict__ in,
-                                                     typename Vec2<T>::type* __restrict__ out, T kappa, CgState* st,
-                                                     double* partials, unsigned* counter) {
-    if (MODE != 0 && st->done) return;
+__global__ void __launch_bounds__(128, 1) dslash_kernel(Geom g, const typename Vec2<T>::type* __restrict__ U,
+                                                        const typename Vec2<T>::type* __restrict__ in,
+                                                        typename Vec2<T>::type* __restrict__ out, T kappa, CgState* st,
+                                                        double* partials, typename Vec2<T>::type* __restrict__ r) {
+    const int done = (MODE != 0) ? st->done : 0;
     const int s = blockIdx.x * blockDim.x + threadIdx.x;
     double nrm = 0.0;
     if (s < g.V) {
+        if (MODE == 2) {
+            // r is only needed by the epilogue: pull its lines into L2 now, without holding registers, so that the
+            // read-modify-write at the end does not expose a full DRAM latency
+            const typename Vec2<T>::type* br = spinor_at(r, s);
+#pragma unroll
+            for (int k = 0; k < 12; k++) asm volatile("prefetch.global.L2 [%0];" ::"l"(br + k * W));
+        }
         const Site c = site_coords(g, s);
         cx<T> acc[12];
 #pragma unroll
         for (int k = 0; k < 12; k++) acc[k] = mk<T>(0, 0);
         constexpr int F = DAG ? +1 : -1;  // D: (1 - gamma) forward, (1 + gamma) backward; D^dag: swapped
         hop_fwd<0, F, T>(g, U, in, c, s, acc);
+        if (MODE != 0 && done) return;  // uniform over the grid
         hop_bwd<0, -F, T>(g, U, in, c, s, acc);
         hop_fwd<1, F, T>(g, U, in, c, s, acc);
         hop_bwd<1, -F, T>(g, U, in, c, s, acc);
@@ -166,20 +268,39 @@ __global__ void __launch_bounds__(128) dslash_kernel(Geom g, const typename Vec2
         hop_bwd<2, -F, T>(g, U, in, c, s, acc);
         hop_fwd<3, F, T>(g, U, in, c, s, acc);
         hop_bwd<3, -F, T>(g, U, in, c, s, acc);
+        const typename Vec2<T>::type* bi = spinor_at(in, s);
+        if (MODE == 2) {
+            const T alpha = (T)st->alpha;
+            typename Vec2<T>::type* br = spinor_at(r, s);
 #pragma unroll
-        for (int k = 0; k < 12; k++) {
-            cx<T> p = ldc<T>(in + (size_t)k * g.Vs + s);
-            cx<T> o = mk<T>(fma(-kappa, acc[k].re, p.re), fma(-kappa, acc[k].im, p.im));
-            stc<T>(out + (size_t)k * g.Vs + s, o);
-            if (MODE == 1) nrm += (double)o.re * (double)o.re + (double)o.im * (double)o.im;
+            for (int k = 0; k < 12; k++) {
+                cx<T> tv = ldc<T>(bi + k * W);
+                cx<T> q = mk<T>(fma(-kappa, acc[k].re, tv.re), fma(-kappa, acc[k].im, tv.im));
+                cx<T> rv = ldc_rw<T>(br + k * W);
+                rv.re = fma(-alpha, q.re, rv.re);
+                rv.im = fma(-alpha, q.im, rv.im);
+                stc<T>(br + k * W, rv);
+                nrm += (double)rv.re * (double)rv.re + (double)rv.im * (double)rv.im;
+            }
+        } else {
+            typename Vec2<T>::type* bo = spinor_at(out, s);
+#pragma unroll
+            for (int k = 0; k < 12; k++) {
+                cx<T> pv = ldc<T>(bi + k * W);
+                cx<T> o = mk<T>(fma(-kappa, acc[k].re, pv.re), fma(-kappa, acc[k].im, pv.im));
+                stc<T>(bo + k * W, o);
+                if (MODE == 1) nrm += (double)o.re * (double)o.re + (double)o.im * (double)o.im;
+            }
+        }
+    } else {
+        if (MODE != 0 && done) return;
+        if (s < g.Vs && MODE != 2) {
+            typename Vec2<T>::type* bo = spinor_at(out, s);
+#pragma unroll
+            for (int k = 0; k < 12; k++) stc<T>(bo + k * W, mk<T>(0, 0));
         }
     }
-    if (MODE == 1) {
-        block_reduce_finalize(nrm, partials, counter, [st](double sum) {
-            st->pAp = sum;
-            st->alpha = st->rr / sum;
-        });
-    }
+    if (MODE != 0) block_partial(nrm, partials);
 }
 
 // ---------------------------------------------------------------------------- A3: CG BLAS-1 (fused)
@@ -213,45 +334,28 @@ __global__ void __launch_bounds__(256) cg_init_kernel(size_t n, const typename V
     });
 }
 
-// x += alpha p ; r -= alpha q ; rr_new = |r|^2 ; beta = rr_new / rr ; convergence test
+// CG step 3 of iteration `iteration`: x += alpha p, then (unless converged) p = r + beta p.  One pass over x, p, r.
+// Runs only if step 2 of the same iteration ran (st->iter == iteration), so launches enqueued past convergence
+// do nothing and the last x update is never lost.
 template <class T>
-__global__ void __launch_bounds__(256) cg_update_xr_kernel(size_t n, typename Vec2<T>::type* __restrict__ x,
-                                                           typename Vec2<T>::type* __restrict__ r,
-                                                           const typename Vec2<T>::type* __restrict__ p,
-                                                           const typename Vec2<T>::type* __restrict__ q, CgState* st,
-                                                           double* partials, unsigned* counter) {
-    if (st->done) return;
-    const T alpha = (T)st->alpha;
-    double acc = 0.0;
+__global__ void __launch_bounds__(256) cg_update_xp_kernel(size_t n, typename Vec2<T>::type* __restrict__ x,
+                                                           typename Vec2<T>::type* __restrict__ p,
+                                                           const typename Vec2<T>::type* __restrict__ r, const CgState* st,
+                                                           int iteration) {
+    if (st->iter != iteration) return;
+    const T alpha = (T)st->alpha, beta = (T)st->beta;
+    const bool done = st->done != 0;
     for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
-        typename Vec2<T>::type xv = x[i], rv = r[i], pv = __ldg(p + i), qv = __ldg(q + i);
+        typename Vec2<T>::type xv = x[i], pv = p[i];
         xv.x = fma(alpha, pv.x, xv.x);
         xv.y = fma(alpha, pv.y, xv.y);
-        rv.x = fma(-alpha, qv.x, rv.x);
-        rv.y = fma(-alpha, qv.y, rv.y);
         x[i] = xv;
-        r[i] = rv;
-        acc += (double)rv.x * (double)rv.x + (double)rv.y * (double)rv.y;
-    }
-    block_reduce_finalize(acc, partials, counter, [st](double sum) {
-        st->beta = sum / st->rr;
-        st->rr = sum;
-        st->iter += 1;
-        st->done = (!(sum > st->tol2 * st->bb) || st->iter >= st->max_iter) ? 1 : 0;
-    });
-}
-
-// p = r + beta p
-template <class T>
-__global__ void __launch_bounds__(256) cg_update_p_kernel(size_t n, typename Vec2<T>::type* __restrict__ p,
-                                                          const typename Vec2<T>::type* __restrict__ r, const CgState* st) {
-    if (st->done) return;
-    const T beta = (T)st->beta;
-    for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
-        typename Vec2<T>::type pv = p[i], rv = __ldg(r + i);
-        pv.x = fma(beta, pv.x, rv.x);
-        pv.y = fma(beta, pv.y, rv.y);
-        p[i] = pv;
+        if (!done) {
+            typename Vec2<T>::type rv = __ldg(r + i);
+            pv.x = fma(beta, pv.x, rv.x);
+            pv.y = fma(beta, pv.y, rv.y);
+            p[i] = pv;
+        }
     }
 }
 
@@ -268,9 +372,28 @@ __global__ void __launch_bounds__(256) redot_kernel(size_t n, const typename Vec
     block_reduce_finalize(acc, partials, counter, [result](double sum) { *result = sum; });
 }
 
+// Pi -= eps F (ACC) or F written, for one link in the compact 8-real form
+template <class T, int ACC>
+__device__ __forceinline__ void store_force(typename Vec2<T>::type* P, int s, int mu, const T f[8], T eps) {
+    typename Vec2<T>::type* b = mom_at(P, s, mu);
+#pragma unroll
+    for (int q = 0; q < 4; q++) {
+        typename Vec2<T>::type v;
+        if (ACC) {
+            v = b[q * W];
+            v.x = fma(-eps, f[2 * q], v.x);
+            v.y = fma(-eps, f[2 * q + 1], v.y);
+        } else {
+            v.x = f[2 * q];
+            v.y = f[2 * q + 1];
+        }
+        b[q * W] = v;
+    }
+}
+
 // ---------------------------------------------------------------------------- A5: fused fermion force
 // One thread per link (s, MU):  C = sum_t h^-[X(s+mu)]_t (x) conj(h^-[Y(s)]_t) + h^+[Y(s+mu)]_t (x) conj(h^+[X(s)]_t)
-// (the half-spinor form of the spin trace, tests pin P11), M = sign U C, F = -kappa P_su(3)[M];
+// (the half-spinor form of the spin trace, tests pin P11), M = U C, F = -kappa P_su(3)[M];
 // ACC: Pi -= eps F in place, else F written in compact form.  No spin-colour intermediate touches HBM.
 template <class T, int MU, int ACC>
 __device__ __forceinline__ void fermion_force_link(const Geom& g, const typename Vec2<T>::type* U,
@@ -282,9 +405,9 @@ __device__ __forceinline__ void fermion_force_link(const Geom& g, const typename
     mat_zero(C);
     {
         cx<T> p[12], a[6], b[6];
-        load_spinor<T>(X, g, sn, p);
+        load_spinor<T>(X, sn, p);
         spin_project<MU, -1>(p, a);
-        load_spinor<T>(Y, g, s, p);
+        load_spinor<T>(Y, s, p);
         spin_project<MU, -1>(p, b);
 #pragma unroll
         for (int t = 0; t < 2; t++)
@@ -292,9 +415,9 @@ __device__ __forceinline__ void fermion_force_link(const Geom& g, const typename
             for (int i = 0; i < 3; i++)
 #pragma unroll
                 for (int j = 0; j < 3; j++) cfma_jc(C[3 * i + j], a[3 * t + i], b[3 * t + j]);
-        load_spinor<T>(Y, g, sn, p);
+        load_spinor<T>(Y, sn, p);
         spin_project<MU, +1>(p, a);
-        load_spinor<T>(X, g, s, p);
+        load_spinor<T>(X, s, p);
         spin_project<MU, +1>(p, b);
 #pragma unroll
         for (int t = 0; t < 2; t++)
@@ -304,36 +427,23 @@ __device__ __forceinline__ void fermion_force_link(const Geom& g, const typename
                 for (int j = 0; j < 3; j++) cfma_jc(C[3 * i + j], a[3 * t + i], b[3 * t + j]);
     }
     cx<T> u[9], M[9];
-    load_link<T>(U, g, MU, s, u);
+    load_link<T>(U, MU, s, u);
     mul_nn(u, C, M);
-    T sc = -kappa;
-    if (g.bc[MU] < 0 && c.x[MU] == g.L[MU] - 1) sc = kappa;
     T f[8];
-    ta_compact(M, sc, f);
-#pragma unroll
-    for (int q = 0; q < 4; q++) {
-        typename Vec2<T>::type* addr = P + (size_t)(4 * MU + q) * g.Vs + s;
-        typename Vec2<T>::type v;
-        if (ACC) {
-            v = *addr;
-            v.x = fma(-eps, f[2 * q], v.x);
-            v.y = fma(-eps, f[2 * q + 1], v.y);
-        } else {
-            v.x = f[2 * q];
-            v.y = f[2 * q + 1];
-        }
-        *addr = v;
-    }
+    ta_compact(M, -kappa, f);
+    store_force<T, ACC>(P, s, MU, f, eps);
 }
 
+// Block = 128 threads = one 32-site layout block x 4 directions: warp w works on direction mu = w, so the four
+// warps share X(s), Y(s) through L1 and every field crosses HBM once.
 template <class T, int ACC>
 __global__ void __launch_bounds__(128) fermion_force_kernel(Geom g, const typename Vec2<T>::type* __restrict__ U,
                                                             const typename Vec2<T>::type* __restrict__ X,
                                                             const typename Vec2<T>::type* __restrict__ Y,
                                                             typename Vec2<T>::type* __restrict__ P, T kappa, T eps) {
-    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    const int s = blockIdx.x * W + (threadIdx.x & 31);
     if (s >= g.V) return;
-    switch (blockIdx.y) {
+    switch (threadIdx.x >> 5) {
         case 0: fermion_force_link<T, 0, ACC>(g, U, X, Y, P, kappa, eps, s); break;
         case 1: fermion_force_link<T, 1, ACC>(g, U, X, Y, P, kappa, eps, s); break;
         case 2: fermion_force_link<T, 2, ACC>(g, U, X, Y, P, kappa, eps, s); break;
@@ -342,15 +452,15 @@ __global__ void __launch_bounds__(128) fermion_force_kernel(Geom g, const typena
 }
 
 // ---------------------------------------------------------------------------- A4: staple gauge force
-// One thread per link (s, mu): V = sum_{nu != mu} [U_nu(s+mu) U_mu^dag(s+nu) U_nu^dag(s)
-//                                               + U_nu^dag(s+mu-nu) U_mu^dag(s-nu) U_nu(s-nu)],
-// F = (beta/6) P_su(3)[U_mu(s) V]; ACC: Pi -= eps F.
+// One thread per link (s, mu), warp w of the block = direction mu:
+//   V = sum_{nu != mu} [U_nu(s+mu) U_mu^dag(s+nu) U_nu^dag(s) + U_nu^dag(s+mu-nu) U_mu^dag(s-nu) U_nu(s-nu)],
+//   F = (beta/6) P_su(3)[U_mu(s) V]; ACC: Pi -= eps F.
 template <class T, int ACC>
 __global__ void __launch_bounds__(128) gauge_force_kernel(Geom g, const typename Vec2<T>::type* __restrict__ U,
                                                           typename Vec2<T>::type* __restrict__ P, T beta_over_6, T eps) {
-    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    const int s = blockIdx.x * W + (threadIdx.x & 31);
     if (s >= g.V) return;
-    const int mu = blockIdx.y;
+    const int mu = threadIdx.x >> 5;
     const Site c = site_coords(g, s);
     const int smu = nbr_fwd(g, c, s, mu);
     cx<T> V[9];
@@ -360,10 +470,10 @@ __global__ void __launch_bounds__(128) gauge_force_kernel(Geom g, const typename
         cx<T> a[9], b[9], t[9], r[9];
         const int snu = nbr_fwd(g, c, s, nu);
         // up: U_nu(s+mu) (U_nu(s) U_mu(s+nu))^dag
-        load_link<T>(U, g, nu, s, a);
-        load_link<T>(U, g, mu, snu, b);
+        load_link<T>(U, nu, s, a);
+        load_link<T>(U, mu, snu, b);
         mul_nn(a, b, t);
-        load_link<T>(U, g, nu, smu, a);
+        load_link<T>(U, nu, smu, a);
         mul_nd(a, t, r);
 #pragma unroll
         for (int k = 0; k < 9; k++) V[k] = V[k] + r[k];
@@ -372,33 +482,20 @@ __global__ void __launch_bounds__(128) gauge_force_kernel(Geom g, const typename
         Site cm = c;
         cm.x[mu] = (c.x[mu] == g.L[mu] - 1) ? 0 : c.x[mu] + 1;
         const int smudn = nbr_bwd(g, cm, smu, nu);
-        load_link<T>(U, g, mu, sdn, a);
-        load_link<T>(U, g, nu, smudn, b);
+        load_link<T>(U, mu, sdn, a);
+        load_link<T>(U, nu, smudn, b);
         mul_nn(a, b, t);
-        load_link<T>(U, g, nu, sdn, a);
+        load_link<T>(U, nu, sdn, a);
         mul_dn(t, a, r);
 #pragma unroll
         for (int k = 0; k < 9; k++) V[k] = V[k] + r[k];
     }
     cx<T> u[9], M[9];
-    load_link<T>(U, g, mu, s, u);
+    load_link<T>(U, mu, s, u);
     mul_nn(u, V, M);
     T f[8];
     ta_compact(M, beta_over_6, f);
-#pragma unroll
-    for (int q = 0; q < 4; q++) {
-        typename Vec2<T>::type* addr = P + (size_t)(4 * mu + q) * g.Vs + s;
-        typename Vec2<T>::type v;
-        if (ACC) {
-            v = *addr;
-            v.x = fma(-eps, f[2 * q], v.x);
-            v.y = fma(-eps, f[2 * q + 1], v.y);
-        } else {
-            v.x = f[2 * q];
-            v.y = f[2 * q + 1];
-        }
-        *addr = v;
-    }
+    store_force<T, ACC>(P, s, mu, f, eps);
 }
 
 // ---------------------------------------------------------------------------- A6: link update
@@ -465,13 +562,14 @@ template <class T> __device__ __forceinline__ void exp_iQ(const cx<T> Q[9], cx<T
 template <class T>
 __global__ void __launch_bounds__(128) link_update_kernel(Geom g, typename Vec2<T>::type* __restrict__ U,
                                                           const typename Vec2<T>::type* __restrict__ P, T eps) {
-    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    const int s = blockIdx.x * W + (threadIdx.x & 31);
     if (s >= g.V) return;
-    const int mu = blockIdx.y;
+    const int mu = threadIdx.x >> 5;
     T c[8];
+    const typename Vec2<T>::type* pb = mom_at(P, s, mu);
 #pragma unroll
     for (int q = 0; q < 4; q++) {
-        typename Vec2<T>::type v = __ldg(P + (size_t)(4 * mu + q) * g.Vs + s);
+        typename Vec2<T>::type v = __ldg(pb + q * W);
         c[2 * q] = v.x;
         c[2 * q + 1] = v.y;
     }
@@ -488,11 +586,12 @@ __global__ void __launch_bounds__(128) link_update_kernel(Geom g, typename Vec2<
     Q[7] = conj(Q[5]);
     cx<T> E[9], u[9], r[9];
     exp_iQ(Q, E);
+    typename Vec2<T>::type* ub = link_at(U, s, mu);
 #pragma unroll
-    for (int k = 0; k < 9; k++) u[k] = ldc_rw<T>(U + (size_t)(9 * mu + k) * g.Vs + s);
+    for (int k = 0; k < 9; k++) u[k] = ldc_rw<T>(ub + k * W);
     mul_nn(E, u, r);
 #pragma unroll
-    for (int k = 0; k < 9; k++) stc<T>(U + (size_t)(9 * mu + k) * g.Vs + s, r[k]);
+    for (int k = 0; k < 9; k++) stc<T>(ub + k * W, r[k]);
 }
 
 // ---------------------------------------------------------------------------- A1: actions
@@ -509,11 +608,11 @@ __global__ void __launch_bounds__(128) plaquette_kernel(Geom g, const typename V
             for (int nu = mu + 1; nu < 4; nu++) {
                 const int snu = nbr_fwd(g, c, s, nu);
                 cx<T> a[9], b[9], t1[9], t2[9];
-                load_link<T>(U, g, mu, s, a);
-                load_link<T>(U, g, nu, smu, b);
+                load_link<T>(U, mu, s, a);
+                load_link<T>(U, nu, smu, b);
                 mul_nn(a, b, t1);  // U_mu(s) U_nu(s+mu)
-                load_link<T>(U, g, nu, s, a);
-                load_link<T>(U, g, mu, snu, b);
+                load_link<T>(U, nu, s, a);
+                load_link<T>(U, mu, snu, b);
                 mul_nn(a, b, t2);  // U_nu(s) U_mu(s+nu)
                 // Re tr(t1 t2^dag)
                 T tr = 0;
@@ -532,15 +631,16 @@ template <class T>
 __global__ void __launch_bounds__(256) kinetic_kernel(Geom g, const typename Vec2<T>::type* __restrict__ P, double* result,
                                                       double* partials, unsigned* counter) {
     double acc = 0.0;
-    const size_t nlinks = (size_t)4 * g.V;
+    const size_t nlinks = (size_t)4 * g.Vs;
     for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < nlinks; i += (size_t)gridDim.x * blockDim.x) {
-        const int mu = (int)(i / g.V), s = (int)(i % g.V);
-        typename Vec2<T>::type d = __ldg(P + (size_t)(4 * mu) * g.Vs + s);
+        // i = (blk * 4 + mu) * 32 + lane
+        const typename Vec2<T>::type* b = P + (i >> 5) * (4 * W) + (i & 31);
+        typename Vec2<T>::type d = __ldg(b);
         double d0 = d.x, d1 = d.y, d2 = -(d0 + d1);
         double off = 0.0;
 #pragma unroll
         for (int q = 1; q < 4; q++) {
-            typename Vec2<T>::type v = __ldg(P + (size_t)(4 * mu + q) * g.Vs + s);
+            typename Vec2<T>::type v = __ldg(b + q * W);
             off += (double)v.x * v.x + (double)v.y * v.y;
         }
         acc += d0 * d0 + d1 * d1 + d2 * d2 + 2.0 * off;
@@ -549,47 +649,76 @@ __global__ void __launch_bounds__(256) kinetic_kernel(Geom g, const typename Vec
 }
 
 // ---------------------------------------------------------------------------- layout conversion
-// DIR 0: canonical [V][ncomp] complex -> native [ncomp][Vs];  DIR 1: back.
-template <class T, int DIR>
-__global__ void __launch_bounds__(256) reorder_kernel(int V, int Vs, int ncomp, const typename Vec2<T>::type* __restrict__ src,
+__device__ __forceinline__ int link_sign(const Geom& g, int s, int mu) {
+    if (g.bc[mu] > 0) return 1;
+    int x = (s / g.stride[mu]) % g.L[mu];
+    return (x == g.L[mu] - 1) ? -1 : 1;
+}
+
+// canonical [V][NCOMP] complex <-> native [blk][NCOMP][32].  DIR 0: to native (padding lanes zeroed), DIR 1: back.
+// LINKS: NCOMP = 36 and the fermion boundary sign is folded in (DIR 0) / taken out (DIR 1).
+template <class T, int DIR, int NCOMP, int LINKS>
+__global__ void __launch_bounds__(256) reorder_kernel(Geom g, const typename Vec2<T>::type* __restrict__ src,
                                                       typename Vec2<T>::type* __restrict__ dst) {
-    const size_t n = (size_t)V * ncomp;
+    const size_t n = (size_t)g.Vs * NCOMP;
     for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
-        // i enumerates the native order (k, s): coalesced on the native side
-        const int k = (int)(i / V), s = (int)(i % V);
-        if (DIR == 0)
-            dst[(size_t)k * Vs + s] = __ldg(src + (size_t)s * ncomp + k);
-        else
-            dst[(size_t)s * ncomp + k] = __ldg(src + (size_t)k * Vs + s);
+        // i enumerates the native order (blk, k, lane): coalesced on the native side
+        const int lane = (int)(i & 31);
+        const int k = (int)((i >> 5) % NCOMP);
+        const int s = (int)((i >> 5) / NCOMP) * W + lane;
+        T sg = 1;
+        if (LINKS && s < g.V) sg = (T)link_sign(g, s, k / 9);
+        if (DIR == 0) {
+            typename Vec2<T>::type v;
+            v.x = 0;
+            v.y = 0;
+            if (s < g.V) {
+                v = __ldg(src + (size_t)s * NCOMP + k);
+                v.x *= sg;
+                v.y *= sg;
+            }
+            dst[i] = v;
+        } else if (s < g.V) {
+            typename Vec2<T>::type v = __ldg(src + i);
+            v.x *= sg;
+            v.y *= sg;
+            dst[(size_t)s * NCOMP + k] = v;
+        }
     }
 }
 
-// canonical full 3x3 momenta [V][4][3][3] <-> compact native [4][4][Vs].  DIR 0 keeps the traceless
+// canonical full 3x3 momenta [V][4][3][3] <-> compact native [blk][4][4][32].  DIR 0 keeps the traceless
 // anti-Hermitian part of the input (P_su(3)).
 template <class T, int DIR>
-__global__ void __launch_bounds__(256) momenta_reorder_kernel(int V, int Vs, const typename Vec2<T>::type* src,
+__global__ void __launch_bounds__(256) momenta_reorder_kernel(Geom g, const typename Vec2<T>::type* src,
                                                               typename Vec2<T>::type* dst) {
-    const size_t n = (size_t)4 * V;
+    const size_t n = (size_t)4 * g.Vs;
     for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
-        const int mu = (int)(i / V), s = (int)(i % V);
+        const int lane = (int)(i & 31);
+        const int mu = (int)((i >> 5) & 3);
+        const int s = (int)(i >> 7) * W + lane;
         if (DIR == 0) {
-            cx<T> m[9];
+            T c[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+            if (s < g.V) {
+                cx<T> m[9];
 #pragma unroll
-            for (int k = 0; k < 9; k++) m[k] = ldc<T>(src + ((size_t)s * 4 + mu) * 9 + k);
-            T c[8];
-            ta_compact(m, (T)1, c);
+                for (int k = 0; k < 9; k++) m[k] = ldc<T>(src + ((size_t)s * 4 + mu) * 9 + k);
+                ta_compact(m, (T)1, c);
+            }
+            typename Vec2<T>::type* b = mom_at(dst, s, mu);
 #pragma unroll
             for (int q = 0; q < 4; q++) {
                 typename Vec2<T>::type v;
                 v.x = c[2 * q];
                 v.y = c[2 * q + 1];
-                dst[(size_t)(4 * mu + q) * Vs + s] = v;
+                b[q * W] = v;
             }
-        } else {
+        } else if (s < g.V) {
             T c[8];
+            const typename Vec2<T>::type* b = mom_at(src, s, mu);
 #pragma unroll
             for (int q = 0; q < 4; q++) {
-                typename Vec2<T>::type v = __ldg(src + (size_t)(4 * mu + q) * Vs + s);
+                typename Vec2<T>::type v = __ldg(b + q * W);
                 c[2 * q] = v.x;
                 c[2 * q + 1] = v.y;
             }
@@ -601,15 +730,20 @@ __global__ void __launch_bounds__(256) momenta_reorder_kernel(int V, int Vs, con
     }
 }
 
+// unit gauge field (with the boundary sign folded in, as everywhere in the native layout)
 template <class T>
-__global__ void __launch_bounds__(256) unit_links_kernel(int V, int Vs, typename Vec2<T>::type* U) {
-    const size_t n = (size_t)36 * V;
+__global__ void __launch_bounds__(256) unit_links_kernel(Geom g, typename Vec2<T>::type* U) {
+    const size_t n = (size_t)36 * g.Vs;
     for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
-        const int k = (int)(i / V) % 9, s = (int)(i % V);
+        const int lane = (int)(i & 31);
+        const int k = (int)((i >> 5) % 36);
+        const int s = (int)((i >> 5) / 36) * W + lane;
+        const int ij = k % 9;
         typename Vec2<T>::type v;
-        v.x = (k == 0 || k == 4 || k == 8) ? 1 : 0;
+        v.x = 0;
         v.y = 0;
-        U[(i / V) * (size_t)Vs + s] = v;
+        if (s < g.V && (ij == 0 || ij == 4 || ij == 8)) v.x = (T)link_sign(g, s, k / 9);
+        U[i] = v;
     }
 }
 

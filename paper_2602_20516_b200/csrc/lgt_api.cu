@@ -6,6 +6,7 @@
 #include <cstring>
 #include <new>
 #include <string>
+#include <vector>
 
 #include "../../include/lgt.h"
 #include "kernels.cuh"
@@ -27,7 +28,7 @@ struct lgt_ctx {
     void* P = nullptr;    // native momenta [16][Vs] pairs
     void* phi = nullptr;  // native pseudofermion
     bool has_phi = false;
-    void* ws[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};  // x, r, p, t, q, b
+    void* ws[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};  // x, r, p, t, (spare), b
     void* F = nullptr;      // compact force buffer for the canonical-output calls (lazy)
     void* stage = nullptr;  // canonical staging buffer for *_host calls and conversions (lazy)
     size_t stage_bytes = 0;
@@ -39,6 +40,11 @@ struct lgt_ctx {
     double* h_scal = nullptr;  // pinned
     int red_blocks = 0;
     long launches = 0;
+    // optional CUDA-event timing of every launch, by kernel class (lgt_timing_*)
+    bool timing = false;
+    std::vector<cudaEvent_t> ev_pool;
+    size_t ev_used = 0;
+    std::vector<int> ev_class;  // class of the launch bracketed by events (2i, 2i+1)
     std::string err;
 };
 
@@ -63,9 +69,28 @@ int fail(lgt_ctx* c, int code, const char* what, cudaError_t e = cudaSuccess) {
         if (e_ != cudaSuccess) return fail(c, (e_ == cudaErrorMemoryAllocation) ? LGT_ENOMEM : LGT_ECUDA, #call, e_); \
     } while (0)
 
-#define LAUNCH(c, kern, grid, block, ...)                           \
+cudaEvent_t timing_event(lgt_ctx* c) {
+    if (c->ev_used == c->ev_pool.size()) {
+        cudaEvent_t e = nullptr;
+        if (cudaEventCreate(&e) != cudaSuccess) return nullptr;
+        c->ev_pool.push_back(e);
+    }
+    return c->ev_pool[c->ev_used++];
+}
+
+#define LAUNCH(c, kclass, kern, grid, block, ...)                   \
     do {                                                            \
+        cudaEvent_t e0_ = nullptr, e1_ = nullptr;                   \
+        if ((c)->timing) {                                          \
+            e0_ = timing_event(c);                                  \
+            e1_ = timing_event(c);                                  \
+            if (e0_ && e1_) {                                       \
+                (c)->ev_class.push_back(kclass);                    \
+                cudaEventRecord(e0_, (c)->stream);                  \
+            }                                                       \
+        }                                                           \
         kern<<<(grid), (block), 0, (c)->stream>>>(__VA_ARGS__);     \
+        if (e0_ && e1_) cudaEventRecord(e1_, (c)->stream);          \
         (c)->launches++;                                            \
         cudaError_t e_ = cudaGetLastError();                        \
         if (e_ != cudaSuccess) return fail((c), LGT_ECUDA, #kern, e_); \
@@ -111,51 +136,62 @@ template <class T> struct Ops {
     typedef typename Vec2<T>::type T2;
 
     static int to_native(lgt_ctx* c, const void* src, void* dst, int ncomp) {
-        size_t n = (size_t)c->g.V * ncomp;
-        LAUNCH(c, (reorder_kernel<T, 0>), stream_blocks(c, n), 256, c->g.V, c->g.Vs, ncomp, (const T2*)src, (T2*)dst);
+        size_t n = (size_t)c->g.Vs * ncomp;
+        if (ncomp == 36)
+            LAUNCH(c, LGT_K_OTHER, (reorder_kernel<T, 0, 36, 1>), stream_blocks(c, n), 256, c->g, (const T2*)src, (T2*)dst);
+        else
+            LAUNCH(c, LGT_K_OTHER, (reorder_kernel<T, 0, 12, 0>), stream_blocks(c, n), 256, c->g, (const T2*)src, (T2*)dst);
         return LGT_OK;
     }
     static int from_native(lgt_ctx* c, const void* src, void* dst, int ncomp) {
-        size_t n = (size_t)c->g.V * ncomp;
-        LAUNCH(c, (reorder_kernel<T, 1>), stream_blocks(c, n), 256, c->g.V, c->g.Vs, ncomp, (const T2*)src, (T2*)dst);
+        size_t n = (size_t)c->g.Vs * ncomp;
+        if (ncomp == 36)
+            LAUNCH(c, LGT_K_OTHER, (reorder_kernel<T, 1, 36, 1>), stream_blocks(c, n), 256, c->g, (const T2*)src, (T2*)dst);
+        else
+            LAUNCH(c, LGT_K_OTHER, (reorder_kernel<T, 1, 12, 0>), stream_blocks(c, n), 256, c->g, (const T2*)src, (T2*)dst);
         return LGT_OK;
     }
     static int momenta_to_native(lgt_ctx* c, const void* src, void* dst) {
-        LAUNCH(c, (momenta_reorder_kernel<T, 0>), stream_blocks(c, (size_t)4 * c->g.V), 256, c->g.V, c->g.Vs, (const T2*)src, (T2*)dst);
+        LAUNCH(c, LGT_K_OTHER, (momenta_reorder_kernel<T, 0>), stream_blocks(c, (size_t)4 * c->g.Vs), 256, c->g, (const T2*)src, (T2*)dst);
         return LGT_OK;
     }
     static int momenta_from_native(lgt_ctx* c, const void* src, void* dst) {
-        LAUNCH(c, (momenta_reorder_kernel<T, 1>), stream_blocks(c, (size_t)4 * c->g.V), 256, c->g.V, c->g.Vs, (const T2*)src, (T2*)dst);
+        LAUNCH(c, LGT_K_OTHER, (momenta_reorder_kernel<T, 1>), stream_blocks(c, (size_t)4 * c->g.Vs), 256, c->g, (const T2*)src, (T2*)dst);
         return LGT_OK;
     }
     static int unit_links(lgt_ctx* c) {
-        LAUNCH(c, (unit_links_kernel<T>), stream_blocks(c, (size_t)36 * c->g.V), 256, c->g.V, c->g.Vs, (T2*)c->U);
+        LAUNCH(c, LGT_K_OTHER, (unit_links_kernel<T>), stream_blocks(c, (size_t)36 * c->g.Vs), 256, c->g, (T2*)c->U);
         return LGT_OK;
     }
 
-    // mode 0: plain; 1: CG "t = D p" (+ pAp, alpha); 2: CG "q = D^dag t"
-    static int dslash(lgt_ctx* c, const void* in, void* out, int dagger, int mode) {
-        const int grid = site_blocks(c, 128);
+    // mode 0: out = D in / D^dag in; 1: CG "t = D p" (+ pAp, alpha); 2: CG "q = D^dag t" fused with the x, r update
+    static int dslash(lgt_ctx* c, const void* in, void* out, int dagger, int mode, void* r = nullptr) {
+        const int grid = (c->g.Vs + 127) / 128;
         const T kappa = (T)c->kappa;
+#define DSLASH_ARGS c->g, (const T2*)c->U, (const T2*)in, (T2*)out, kappa, c->st, c->partials, (T2*)r
         if (mode == 0) {
             if (dagger)
-                LAUNCH(c, (dslash_kernel<T, 1, 0>), grid, 128, c->g, (const T2*)c->U, (const T2*)in, (T2*)out, kappa, c->st, c->partials, c->counter);
+                LAUNCH(c, LGT_K_DSLASH, (dslash_kernel<T, 1, 0>), grid, 128, DSLASH_ARGS);
             else
-                LAUNCH(c, (dslash_kernel<T, 0, 0>), grid, 128, c->g, (const T2*)c->U, (const T2*)in, (T2*)out, kappa, c->st, c->partials, c->counter);
+                LAUNCH(c, LGT_K_DSLASH, (dslash_kernel<T, 0, 0>), grid, 128, DSLASH_ARGS);
         } else if (mode == 1) {
-            LAUNCH(c, (dslash_kernel<T, 0, 1>), grid, 128, c->g, (const T2*)c->U, (const T2*)in, (T2*)out, kappa, c->st, c->partials, c->counter);
+            LAUNCH(c, LGT_K_DSLASH, (dslash_kernel<T, 0, 1>), grid, 128, DSLASH_ARGS);
         } else {
-            LAUNCH(c, (dslash_kernel<T, 1, 2>), grid, 128, c->g, (const T2*)c->U, (const T2*)in, (T2*)out, kappa, c->st, c->partials, c->counter);
+            LAUNCH(c, LGT_K_DSLASH_R, (dslash_kernel<T, 1, 2>), grid, 128, DSLASH_ARGS);
         }
+#undef DSLASH_ARGS
         return LGT_OK;
     }
 
     // CG on D^dag D (reading A-10): b, x native; y (optional) receives D x.
+    // Per iteration: t = D p (+ |t|^2) | alpha | q = D^dag t fused with r -= alpha q (+ |r|^2) | beta, stop test |
+    // x += alpha p, p = r + beta p.
     static int cg(lgt_ctx* c, const void* b, void* x, void* y, double tol, int max_iter, int* iters, double* rel) {
-        T2 *r = (T2*)c->ws[1], *p = (T2*)c->ws[2], *t = (T2*)c->ws[3], *q = (T2*)c->ws[4];
+        T2 *r = (T2*)c->ws[1], *p = (T2*)c->ws[2], *t = (T2*)c->ws[3];
         const size_t n = (size_t)12 * c->g.Vs;
         const int nb = stream_blocks(c, n);
-        LAUNCH(c, (cg_init_kernel<T>), nb, 256, n, (const T2*)b, (T2*)x, r, p, c->st, tol * tol, max_iter, c->partials, c->counter);
+        const int ngrid = (c->g.Vs + 127) / 128;  // blocks (= partials) of the stencil kernels
+        LAUNCH(c, LGT_K_CG_BLAS, (cg_init_kernel<T>), nb, 256, n, (const T2*)b, (T2*)x, r, p, c->st, tol * tol, max_iter, c->partials, c->counter);
         int rc;
         int launched = 0;
         for (;;) {
@@ -168,9 +204,10 @@ template <class T> struct Ops {
             if (chunk <= 0) chunk = 1;
             for (int i = 0; i < chunk; i++) {
                 if ((rc = dslash(c, p, t, 0, 1)) != LGT_OK) return rc;
-                if ((rc = dslash(c, t, q, 1, 2)) != LGT_OK) return rc;
-                LAUNCH(c, (cg_update_xr_kernel<T>), nb, 256, n, (T2*)x, r, (const T2*)p, (const T2*)q, c->st, c->partials, c->counter);
-                LAUNCH(c, (cg_update_p_kernel<T>), nb, 256, n, p, (const T2*)r, c->st);
+                LAUNCH(c, LGT_K_CG_BLAS, (cg_scalars_kernel<1>), 1, 1024, ngrid, c->partials, c->st);
+                if ((rc = dslash(c, t, nullptr, 1, 2, r)) != LGT_OK) return rc;
+                LAUNCH(c, LGT_K_CG_BLAS, (cg_scalars_kernel<2>), 1, 1024, ngrid, c->partials, c->st);
+                LAUNCH(c, LGT_K_CG_BLAS, (cg_update_xp_kernel<T>), nb, 256, n, (T2*)x, p, (const T2*)r, c->st, launched + i + 1);
             }
             launched += chunk;
         }
@@ -183,37 +220,37 @@ template <class T> struct Ops {
     }
 
     static int fermion_force(lgt_ctx* c, const void* X, const void* Y, void* P, int acc, double eps) {
-        dim3 grid(site_blocks(c, 128), 4);
+        const int grid = c->g.Vs / 32;
         if (acc)
-            LAUNCH(c, (fermion_force_kernel<T, 1>), grid, 128, c->g, (const T2*)c->U, (const T2*)X, (const T2*)Y, (T2*)P, (T)c->kappa, (T)eps);
+            LAUNCH(c, LGT_K_FERMION_FORCE, (fermion_force_kernel<T, 1>), grid, 128, c->g, (const T2*)c->U, (const T2*)X, (const T2*)Y, (T2*)P, (T)c->kappa, (T)eps);
         else
-            LAUNCH(c, (fermion_force_kernel<T, 0>), grid, 128, c->g, (const T2*)c->U, (const T2*)X, (const T2*)Y, (T2*)P, (T)c->kappa, (T)eps);
+            LAUNCH(c, LGT_K_FERMION_FORCE, (fermion_force_kernel<T, 0>), grid, 128, c->g, (const T2*)c->U, (const T2*)X, (const T2*)Y, (T2*)P, (T)c->kappa, (T)eps);
         return LGT_OK;
     }
     static int gauge_force(lgt_ctx* c, void* P, int acc, double eps) {
-        dim3 grid(site_blocks(c, 128), 4);
+        const int grid = c->g.Vs / 32;
         if (acc)
-            LAUNCH(c, (gauge_force_kernel<T, 1>), grid, 128, c->g, (const T2*)c->U, (T2*)P, (T)(c->beta / 6.0), (T)eps);
+            LAUNCH(c, LGT_K_GAUGE_FORCE, (gauge_force_kernel<T, 1>), grid, 128, c->g, (const T2*)c->U, (T2*)P, (T)(c->beta / 6.0), (T)eps);
         else
-            LAUNCH(c, (gauge_force_kernel<T, 0>), grid, 128, c->g, (const T2*)c->U, (T2*)P, (T)(c->beta / 6.0), (T)eps);
+            LAUNCH(c, LGT_K_GAUGE_FORCE, (gauge_force_kernel<T, 0>), grid, 128, c->g, (const T2*)c->U, (T2*)P, (T)(c->beta / 6.0), (T)eps);
         return LGT_OK;
     }
     static int link_update(lgt_ctx* c, double eps) {
-        dim3 grid(site_blocks(c, 128), 4);
-        LAUNCH(c, (link_update_kernel<T>), grid, 128, c->g, (T2*)c->U, (const T2*)c->P, (T)eps);
+        const int grid = c->g.Vs / 32;
+        LAUNCH(c, LGT_K_LINK_UPDATE, (link_update_kernel<T>), grid, 128, c->g, (T2*)c->U, (const T2*)c->P, (T)eps);
         return LGT_OK;
     }
     static int plaquette_sum(lgt_ctx* c, double* dev_result) {
-        LAUNCH(c, (plaquette_kernel<T>), site_blocks(c, 128), 128, c->g, (const T2*)c->U, dev_result, c->partials, c->counter);
+        LAUNCH(c, LGT_K_OTHER, (plaquette_kernel<T>), site_blocks(c, 128), 128, c->g, (const T2*)c->U, dev_result, c->partials, c->counter);
         return LGT_OK;
     }
     static int kinetic(lgt_ctx* c, double* dev_result) {
-        LAUNCH(c, (kinetic_kernel<T>), stream_blocks(c, (size_t)4 * c->g.V), 256, c->g, (const T2*)c->P, dev_result, c->partials, c->counter);
+        LAUNCH(c, LGT_K_OTHER, (kinetic_kernel<T>), stream_blocks(c, (size_t)4 * c->g.Vs), 256, c->g, (const T2*)c->P, dev_result, c->partials, c->counter);
         return LGT_OK;
     }
     static int redot(lgt_ctx* c, const void* a, const void* b, double* dev_result) {
         const size_t n = (size_t)12 * c->g.Vs;
-        LAUNCH(c, (redot_kernel<T>), stream_blocks(c, n), 256, n, (const T2*)a, (const T2*)b, dev_result, c->partials, c->counter);
+        LAUNCH(c, LGT_K_OTHER, (redot_kernel<T>), stream_blocks(c, n), 256, n, (const T2*)a, (const T2*)b, dev_result, c->partials, c->counter);
         return LGT_OK;
     }
 };
@@ -311,7 +348,7 @@ int lgt_create(lgt_ctx** out, const int dims[4], double beta, double kappa, cons
         stride *= dims[m];
     }
     c->g.V = (int)V;
-    c->g.Vs = (int)V;
+    c->g.Vs = (int)((V + 31) / 32 * 32);
     int sms = 148;
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device);
     c->red_blocks = sms * 8;
@@ -325,7 +362,7 @@ int lgt_create(lgt_ctx** out, const int dims[4], double beta, double kappa, cons
     alloc(&c->P, mom_bytes(c));
     alloc(&c->phi, spinor_bytes(c));
     for (int i = 0; i < 6; i++) alloc(&c->ws[i], spinor_bytes(c));
-    size_t npart = (size_t)site_blocks(c, 128) + c->red_blocks + 64;
+    size_t npart = (size_t)(c->g.Vs / 32) + c->red_blocks + 64;
     alloc((void**)&c->partials, npart * sizeof(double));
     alloc((void**)&c->counter, sizeof(unsigned));
     alloc((void**)&c->st, sizeof(CgState));
@@ -338,6 +375,7 @@ int lgt_create(lgt_ctx** out, const int dims[4], double beta, double kappa, cons
                   cudaMemsetAsync(c->st, 0, sizeof(CgState), c->stream) == cudaSuccess &&
                   cudaMemsetAsync(c->P, 0, mom_bytes(c), c->stream) == cudaSuccess &&
                   cudaMemsetAsync(c->phi, 0, spinor_bytes(c), c->stream) == cudaSuccess;
+        for (int i = 0; i < 6 && ok; i++) ok = cudaMemsetAsync(c->ws[i], 0, spinor_bytes(c), c->stream) == cudaSuccess;
         if (!ok) rc = fail(nullptr, LGT_ECUDA, "lgt_create: cudaMemsetAsync failed");
     }
     if (rc == LGT_OK) {
@@ -369,7 +407,38 @@ int lgt_destroy(lgt_ctx* c) {
     cudaFree(c->scal);
     if (c->h_st) cudaFreeHost(c->h_st);
     if (c->h_scal) cudaFreeHost(c->h_scal);
+    for (cudaEvent_t e : c->ev_pool) cudaEventDestroy(e);
     delete c;
+    return LGT_OK;
+}
+
+int lgt_timing_enable(lgt_ctx* c, int enable) {
+    CHECK_CTX(c);
+    c->timing = enable != 0;
+    return LGT_OK;
+}
+int lgt_timing_reset(lgt_ctx* c) {
+    CHECK_CTX(c);
+    CU(cudaStreamSynchronize(c->stream));
+    c->ev_used = 0;
+    c->ev_class.clear();
+    return LGT_OK;
+}
+int lgt_timing_read(lgt_ctx* c, int kernel_class, double* ms_total, long* launches) {
+    CHECK_CTX(c);
+    if (kernel_class < 0 || kernel_class >= LGT_K_COUNT) return fail(c, LGT_EINVAL, "lgt_timing_read: bad kernel class");
+    CU(cudaStreamSynchronize(c->stream));
+    double total = 0.0;
+    long n = 0;
+    for (size_t i = 0; i < c->ev_class.size(); i++) {
+        if (c->ev_class[i] != kernel_class) continue;
+        float ms = 0.f;
+        CU(cudaEventElapsedTime(&ms, c->ev_pool[2 * i], c->ev_pool[2 * i + 1]));
+        total += ms;
+        n++;
+    }
+    if (ms_total) *ms_total = total;
+    if (launches) *launches = n;
     return LGT_OK;
 }
 

@@ -49,6 +49,9 @@ SYMBOLS = {
     "lgt_fermion_force_native": (_i, [_vp, _vp, _vp, _d]),
     "lgt_gauge_force_accumulate": (_i, [_vp, _d]),
     "lgt_cg_native": (_i, [_vp, _vp, _vp, _vp, _d, _i, _ip, _dp]),
+    "lgt_timing_enable": (_i, [_vp, _i]),
+    "lgt_timing_reset": (_i, [_vp]),
+    "lgt_timing_read": (_i, [_vp, _i, _dp, _lp]),
     "lgt_launch_count": (_l, [_vp]),
     "lgt_stream": (_vp, [_vp]),
 }
@@ -245,6 +248,35 @@ def lgt_cg_native(ctx, b, x, y, tol, max_iter):
     rc = _check(ctx, lib().lgt_cg_native(ctx, _ptr(b), _ptr(x), _ptr(y), tol, max_iter, C.byref(it), C.byref(rel)),
                 allow=(LGT_ENOCONV,))
     return it.value, rel.value, rc == LGT_OK
+
+
+(LGT_K_DSLASH, LGT_K_CG_BLAS, LGT_K_FERMION_FORCE, LGT_K_GAUGE_FORCE, LGT_K_LINK_UPDATE, LGT_K_OTHER,
+ LGT_K_DSLASH_R) = range(7)
+KERNEL_CLASSES = ("dslash", "cg_blas1", "fermion_force", "gauge_force", "link_update", "other", "dslash_dag_fused_r")
+
+
+def lgt_timing_enable(ctx, enable=True):
+    return _check(ctx, lib().lgt_timing_enable(ctx, int(bool(enable))))
+
+
+def lgt_timing_reset(ctx):
+    return _check(ctx, lib().lgt_timing_reset(ctx))
+
+
+def lgt_timing_read(ctx, kernel_class):
+    """Returns (ms_total, launches) of one kernel class since the last reset."""
+    ms, n = C.c_double(), C.c_long()
+    _check(ctx, lib().lgt_timing_read(ctx, int(kernel_class), C.byref(ms), C.byref(n)))
+    return ms.value, n.value
+
+
+def lgt_stream(ctx):
+    return lib().lgt_stream(ctx)
+
+
+def lgt_last_error(ctx):
+    msg = lib().lgt_last_error(ctx)
+    return msg.decode() if msg else ""
 
 
 def lgt_launch_count(ctx):
