@@ -114,20 +114,15 @@ def make_inputs(cfg):
 
 # ------------------------------------------------------------------------------------------------ our arm
 def run_ours(args):
-    import numpy as np
     import torch
-    import torch.distributed as dist
 
-    from paper_2602_20516_b200 import lgt, synth
+    from paper_2602_20516_b200 import dist, lgt, synth
 
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
+    rank, world, local = dist.env_rank_world()
     if not torch.cuda.is_available():
         raise RuntimeError("bench.py needs a CUDA device: the product path has no CPU fallback")
     torch.cuda.set_device(local)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    dist.init("nccl", torch.device("cuda", local))
     lgt.lib()
 
     cfg = dict(synth.CONFIGS[args.config])
@@ -162,8 +157,7 @@ def run_ours(args):
         return it
 
     def barrier():
-        if world > 1:
-            dist.barrier()
+        dist.barrier()
         torch.cuda.synchronize()
 
     reset_state()
@@ -208,13 +202,8 @@ def run_ours(args):
     d2h = hU_out.numel() * 16 + hP_out.numel() * 16
 
     # ---- max over ranks, aggregate
-    stats = torch.tensor([elapsed_ms, e2e_s], dtype=torch.float64, device="cuda")
-    sums = torch.tensor([total_reals, total_flops, e2e_reals, launches], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(stats, op=dist.ReduceOp.MAX)
-        dist.all_reduce(sums, op=dist.ReduceOp.SUM)
-    elapsed_ms, e2e_s = stats.tolist()
-    total_reals, total_flops, e2e_reals, launches_all = sums.tolist()
+    (elapsed_ms, e2e_s), (total_reals, total_flops, e2e_reals, launches_all) = dist.aggregate(
+        [elapsed_ms, e2e_s], [total_reals, total_flops, e2e_reals, launches], device="cuda")
 
     # ---- the metric's two kernels in isolation (inputs exceed L2: links 604 MB, spinors 201 MB each)
     kernels = {}
@@ -261,8 +250,7 @@ def run_ours(args):
 
     if rank != 0:
         lat.close()
-        if world > 1:
-            dist.destroy_process_group()
+        dist.shutdown()
         return
 
     peak, peak_src = measured_peaks()
@@ -315,8 +303,7 @@ def run_ours(args):
     if world == 1 and not args.skip_cpu_baseline:
         out["cpu_baseline"] = cpu_baseline(cfg, sample_iters=args.cpu_sample_iters)
     lat.close()
-    if world > 1:
-        dist.destroy_process_group()
+    dist.shutdown()
     print(json.dumps(out), flush=True)
 
 
@@ -352,11 +339,11 @@ def cpu_baseline(cfg, sample_iters, steps=1, warmup=0):
 
 
 def run_reference(args):
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
+    from paper_2602_20516_b200 import dist, synth
+
+    rank, world, _ = dist.env_rank_world()
     if rank != 0:
         return
-    from paper_2602_20516_b200 import synth
 
     cfg = dict(synth.CONFIGS[args.config])
     if args.lattice:

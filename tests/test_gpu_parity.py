@@ -286,3 +286,109 @@ def test_error_paths(lgt):
     x, it, rel, ok = lat.cg(np.zeros_like(b), 1e-13, 10)
     assert ok and it == 0 and not x.any()
     lat.close()
+
+
+# ------------------------------------------------------------------------------------------------ full sizes
+def _sample_sites(V, n, seed):
+    rng = np.random.default_rng(seed)
+    # first / last sites (all boundaries), plus a random sample
+    return np.unique(np.concatenate([[0, 1, 31, 32, V - 1, V - 32, V // 2], rng.integers(0, V, n)]))
+
+
+def test_config3_full_size_kernels_sampled(lgt):
+    """configs[3] (32^4, the bench workload): Dslash, fermion force and gauge force at full size in the launch
+    shapes bench.py times, compared on sampled sites / links that the oracle computes one by one."""
+    c = synth.CONFIGS[3]
+    dims, beta, kappa, bc = c["dims"], c["beta"], c["kappa"], c["bc"]
+    V = synth.volume(dims)
+    U = synth.config_links(3)
+    X = synth.gaussian_spinor(dims, 11)
+    Y = synth.gaussian_spinor(dims, 12)
+    sites = _sample_sites(V, 200, 13)
+    lat = lgt.Lattice(dims, beta, kappa, bc)
+    lat.set_links(U)
+    for dag in (False, True):
+        out = lat.dslash(X, dagger=dag)
+        ref = oracle.dslash_sites(dims, kappa, bc, U, X, sites, dagger=dag)
+        assert site_rel_err(out[sites], ref) < TOL64
+    F, _ = lat.fermion_force(X, Y)
+    G = lat.gauge_force()
+    worst_f = worst_g = 0.0
+    for s in sites[:60]:
+        for mu in range(4):
+            rf = oracle.fermion_force_link(dims, kappa, bc, U, X, Y, int(s), mu)
+            rg = oracle.gauge_force_link(dims, beta, U, int(s), mu)
+            worst_f = max(worst_f, np.linalg.norm(F[s, mu] - rf) / np.linalg.norm(rf))
+            worst_g = max(worst_g, np.linalg.norm(G[s, mu] - rg) / np.linalg.norm(rg))
+    assert worst_f < TOL64 and worst_g < TOL64, (worst_f, worst_g)
+    # fp32 variant of the same lattice (configs[3]: "also run as an fp32 Dslash and force variant")
+    lat.close()
+    U32, X32, Y32 = round32(U), round32(X), round32(Y)
+    lat = lgt.Lattice(dims, beta, kappa, bc, precision=lgt.LGT_F32)
+    lat.set_links(U32)
+    out = lat.dslash(X32).astype(np.complex128)
+    assert site_rel_err(out[sites], oracle.dslash_sites(dims, kappa, bc, U32, X32, sites)) < TOL32
+    F32, _ = lat.fermion_force(X32, Y32)
+    worst = 0.0
+    for s in sites[:40]:
+        for mu in range(4):
+            rf = oracle.fermion_force_link(dims, kappa, bc, U32, X32, Y32, int(s), mu)
+            worst = max(worst, np.linalg.norm(F32[s, mu].astype(np.complex128) - rf) / np.linalg.norm(rf))
+    assert worst < TOL32, worst
+    lat.close()
+
+
+def test_config3_full_size_md_step(lgt):
+    """configs[3]: one full MD step at 32^4 exactly as bench.py runs it (kick(dt) then drift(dt), CG to 1e-12):
+    CG iteration count identical to the oracle's, momenta and links per link within 1e-11."""
+    c = synth.CONFIGS[3]
+    dims, beta, kappa, bc, tol, dt = c["dims"], c["beta"], c["kappa"], c["bc"], c["cg_tol"], c["dt"]
+    V = synth.volume(dims)
+    U = synth.config_links(3)
+    P = synth.gaussian_momenta(dims, c["seed_mom"])
+    eta = synth.gaussian_spinor(dims, c["seed_eta"])
+    phi = oracle.dslash(dims, kappa, bc, U, eta, dagger=True)
+    lat = lgt.Lattice(dims, beta, kappa, bc)
+    lat.set_links(U)
+    lat.set_momenta(P)
+    lat.set_pseudofermion(phi)
+    it = lgt.lgt_md_kick(lat.ctx, dt, tol, 10 * V)
+    lgt.lgt_md_drift(lat.ctx, dt)
+    P1, U1 = lat.get_momenta(), lat.get_links()
+    lat.close()
+    P_ref, it_ref, ok = oracle.kick(dims, beta, kappa, bc, U, phi, P, dt, tol, 10 * V)
+    U_ref = oracle.drift(dims, dt, P_ref, U)
+    assert ok and it == it_ref, (it, it_ref)
+    assert link_rel_err(P1, P_ref)[0] < TOL64
+    assert np.abs(U1 - U_ref).max() < 1e-13
+
+
+def test_config4_largest_lattice_sampled(lgt):
+    """configs[4] shape (48^3 x 96, the largest single-GPU working set, Lx not a multiple of the 32-site layout block):
+    Dslash and fermion force on sampled sites.  The links are a periodic tiling of a seeded 24^4 warm field (a valid
+    SU(3) configuration of the full size that takes seconds, not minutes, to make on the host)."""
+    import torch
+
+    dims, kappa, bc = (48, 48, 48, 96), 0.12, BC
+    free, _ = torch.cuda.mem_get_info()
+    if free < 40e9:
+        pytest.skip("needs about 40 GB of device memory")
+    V = synth.volume(dims)
+    small = synth.warm_links((24, 24, 24, 24), 0.3, 1401).reshape(24, 24, 24, 24, 4, 3, 3)
+    U = np.tile(small, (4, 2, 2, 2, 1, 1, 1)).reshape(V, 4, 3, 3)
+    X = synth.gaussian_spinor(dims, 1402)
+    Y = synth.gaussian_spinor(dims, 1403)
+    sites = _sample_sites(V, 100, 5)
+    lat = lgt.Lattice(dims, 5.6, kappa, bc)
+    lat.set_links(U)
+    out = lat.dslash(X)
+    assert site_rel_err(out[sites], oracle.dslash_sites(dims, kappa, bc, U, X, sites)) < TOL64
+    del out
+    F, _ = lat.fermion_force(X, Y)
+    worst = 0.0
+    for s in sites[:40]:
+        for mu in range(4):
+            rf = oracle.fermion_force_link(dims, kappa, bc, U, X, Y, int(s), mu)
+            worst = max(worst, np.linalg.norm(F[s, mu] - rf) / np.linalg.norm(rf))
+    assert worst < TOL64, worst
+    lat.close()
