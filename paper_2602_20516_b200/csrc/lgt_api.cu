@@ -220,7 +220,7 @@ template <class T> struct Ops {
     }
 
     static int fermion_force(lgt_ctx* c, const void* X, const void* Y, void* P, int acc, double eps) {
-        const int grid = c->g.Vs / 32;
+        const int grid = (c->g.Vs + 127) / 128;
         if (acc)
             LAUNCH(c, LGT_K_FERMION_FORCE, (fermion_force_kernel<T, 1>), grid, 128, c->g, (const T2*)c->U, (const T2*)X, (const T2*)Y, (T2*)P, (T)c->kappa, (T)eps);
         else
