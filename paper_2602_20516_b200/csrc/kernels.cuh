@@ -458,8 +458,10 @@ __global__ void __launch_bounds__(128, 1) fermion_force_kernel(Geom g, const typ
 // One thread per link (s, mu), warp w of the block = direction mu:
 //   V = sum_{nu != mu} [U_nu(s+mu) U_mu^dag(s+nu) U_nu^dag(s) + U_nu^dag(s+mu-nu) U_mu^dag(s-nu) U_nu(s-nu)],
 //   F = (beta/6) P_su(3)[U_mu(s) V]; ACC: Pi -= eps F.
+// Bound by fp64 FMA issue and load latency, not HBM (fp64 pipe 48 % busy, DRAM 20 %, profiles/r01c_forces.md);
+// two blocks per SM (~246 registers) let the compiler batch the 18 link loads: 680 us against 775 us at 174 registers.
 template <class T, int ACC>
-__global__ void __launch_bounds__(128) gauge_force_kernel(Geom g, const typename Vec2<T>::type* __restrict__ U,
+__global__ void __launch_bounds__(128, 2) gauge_force_kernel(Geom g, const typename Vec2<T>::type* __restrict__ U,
                                                           typename Vec2<T>::type* __restrict__ P, T beta_over_6, T eps) {
     const int s = blockIdx.x * W + (threadIdx.x & 31);
     if (s >= g.V) return;

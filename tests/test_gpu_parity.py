@@ -124,6 +124,26 @@ def test_cg_and_fermion_force_configs(lgt, cfg):
     lat.close()
 
 
+@pytest.mark.parametrize("dims", [(4, 3, 5, 6), (6, 2, 1, 10), (3, 3, 3, 3), (8, 8, 8, 8)])
+def test_fermion_force_ragged_shapes(lgt, dims):
+    """Force kernel alone on shapes that do not fill a 128-site block, with extents of 1 and 2 (forward and
+    backward neighbour coincide) and every boundary-sign pattern: rounding-level agreement per link."""
+    kappa = 0.12
+    U = synth.warm_links(dims, 0.3, 21)
+    X = synth.gaussian_spinor(dims, 22)
+    Y = synth.gaussian_spinor(dims, 23)
+    for bc in (BC, (1, 1, 1, 1), (-1, -1, 1, -1)):
+        lat = lgt.Lattice(dims, 5.6, kappa, bc)
+        lat.set_links(U)
+        F, _ = lat.fermion_force(X, Y)
+        e, plain = link_rel_err(F, oracle.fermion_force(dims, kappa, bc, U, X, Y))
+        assert e < 1e-13, (dims, bc, e, plain)
+        # traceless anti-Hermitian output (Eq. 7 of the paper, PAPER.md:109)
+        assert np.abs(F + F.conj().swapaxes(-1, -2)).max() < 1e-15
+        assert np.abs(np.trace(F, axis1=-2, axis2=-1)).max() < 1e-15
+        lat.close()
+
+
 def test_fermion_force_fp32(lgt):
     dims, kappa = (8, 8, 8, 8), 0.12
     U = round32(synth.warm_links(dims, 0.3, 3))
