@@ -25,7 +25,22 @@ struct Geom {
     int V;          // sites
     int Vs;         // sites padded to a multiple of 32
     int bc[4];      // fermion boundary signs (used by the layout conversion only)
+    // block swizzle of the site-per-thread stencil kernels (0 = lexicographic): blocks sweep all time slices of
+    // a slab of swz_Z z-planes before moving to the next slab, so that the t neighbours stay in L2 on big lattices
+    int swz_Z;
+    int swz_cxy;    // 128-site chunks per xy plane
 };
+
+// lexicographic 128-site chunk handled by block b
+__device__ __forceinline__ int swizzled_chunk(const Geom& g, int b) {
+    if (g.swz_Z == 0) return b;
+    const int cslab = g.swz_cxy * g.swz_Z;
+    const int per_slab = cslab * g.L[3];
+    const int slab = b / per_slab, rem = b - slab * per_slab;
+    const int t = rem / cslab, j = rem - t * cslab;
+    const int z = slab * g.swz_Z + j / g.swz_cxy;
+    return (t * g.L[2] + z) * g.swz_cxy + j % g.swz_cxy;
+}
 
 // CG recurrence scalars, resident on the device so that iterations need no host round trip.
 struct CgState {
@@ -244,7 +259,7 @@ __global__ void __launch_bounds__(128, 1) dslash_kernel(Geom g, const typename V
                                                         typename Vec2<T>::type* __restrict__ out, T kappa, CgState* st,
                                                         double* partials, typename Vec2<T>::type* __restrict__ r) {
     const int done = (MODE != 0) ? st->done : 0;
-    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    const int s = swizzled_chunk(g, blockIdx.x) * blockDim.x + threadIdx.x;
     double nrm = 0.0;
     if (s < g.V) {
         if (MODE == 2) {
@@ -442,7 +457,7 @@ __global__ void __launch_bounds__(128, 1) fermion_force_kernel(Geom g, const typ
                                                                const typename Vec2<T>::type* __restrict__ X,
                                                                const typename Vec2<T>::type* __restrict__ Y,
                                                                typename Vec2<T>::type* __restrict__ P, T kappa, T eps) {
-    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    const int s = swizzled_chunk(g, blockIdx.x) * blockDim.x + threadIdx.x;
     if (s >= g.V) return;
     const Site c = site_coords(g, s);
     cx<T> Xs[12], Ys[12];

@@ -263,6 +263,21 @@ int read_scalars(lgt_ctx* c, int n) {
     return LGT_OK;
 }
 
+// Automatic block swizzle: off while one time slice of links + spinors (48 complex numbers per site) stays well
+// inside L2 together with its successor; else the largest divisor Z of Lz whose slab slice does.
+// Measured (fp64 Dslash): 48^3 x 96 2347 -> 2030 us, 64^4 3715 -> 3219 us; 32^4 is faster without (191 vs 198 us).
+int auto_swizzle(const lgt_ctx* c) {
+    const double limit = 28e6;  // bytes of one slab slice
+    const double site_bytes = 48.0 * (double)c->esize;
+    const long long xy = (long long)c->g.L[0] * c->g.L[1];
+    if (xy % 128 != 0) return 0;
+    if ((double)xy * c->g.L[2] * site_bytes <= limit) return 0;
+    int best = 0;
+    for (int Z = 1; Z <= c->g.L[2]; Z++)
+        if (c->g.L[2] % Z == 0 && (double)xy * Z * site_bytes <= limit) best = Z;
+    return best;
+}
+
 bool fermions_on(const lgt_ctx* c) { return c->kappa != 0.0 && c->has_phi; }
 
 // Pi -= eps (F^g + F^f)
@@ -349,6 +364,8 @@ int lgt_create(lgt_ctx** out, const int dims[4], double beta, double kappa, cons
     }
     c->g.V = (int)V;
     c->g.Vs = (int)((V + 31) / 32 * 32);
+    c->g.swz_cxy = (int)(((long long)dims[0] * dims[1]) / 128);
+    c->g.swz_Z = auto_swizzle(c);
     int sms = 148;
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device);
     c->red_blocks = sms * 8;
@@ -443,6 +460,20 @@ int lgt_timing_read(lgt_ctx* c, int kernel_class, double* ms_total, long* launch
 }
 
 long lgt_launch_count(const lgt_ctx* c) { return c ? c->launches : 0; }
+int lgt_set_block_swizzle(lgt_ctx* c, int z_planes, int* in_effect) {
+    CHECK_CTX(c);
+    if (z_planes < 0) {
+        c->g.swz_Z = auto_swizzle(c);
+    } else if (z_planes == 0) {
+        c->g.swz_Z = 0;
+    } else {
+        if (c->g.L[2] % z_planes != 0 || ((long long)c->g.L[0] * c->g.L[1]) % 128 != 0)
+            return fail(c, LGT_EINVAL, "lgt_set_block_swizzle: Z must divide Lz and Lx*Ly must be a multiple of 128");
+        c->g.swz_Z = z_planes;
+    }
+    if (in_effect) *in_effect = c->g.swz_Z;
+    return LGT_OK;
+}
 void* lgt_stream(const lgt_ctx* c) { return c ? (void*)c->stream : nullptr; }
 long lgt_native_spinor_bytes(const lgt_ctx* c) { return c ? (long)spinor_bytes(c) : 0; }
 

@@ -54,6 +54,7 @@ SYMBOLS = {
     "lgt_timing_read": (_i, [_vp, _i, _dp, _lp]),
     "lgt_launch_count": (_l, [_vp]),
     "lgt_stream": (_vp, [_vp]),
+    "lgt_set_block_swizzle": (_i, [_vp, _i, _ip]),
 }
 
 _lib = None
@@ -281,6 +282,14 @@ def lgt_last_error(ctx):
 
 def lgt_launch_count(ctx):
     return lib().lgt_launch_count(ctx)
+
+
+def lgt_set_block_swizzle(ctx, z_planes=-1):
+    """Block traversal order of the Dslash kernels (0 lexicographic, Z > 0 slabs of Z z-planes, < 0 automatic).
+    Returns the value in effect."""
+    out = C.c_int(0)
+    _check(ctx, lib().lgt_set_block_swizzle(ctx, int(z_planes), C.byref(out)))
+    return out.value
 
 
 # ---- convenience wrapper -----------------------------------------------------------------------

@@ -57,6 +57,32 @@ def test_dslash_fp64(lgt, dims, dag):
         lat.close()
 
 
+@pytest.mark.parametrize("dims,zs", [((16, 8, 8, 6), (1, 2, 4, 8)), ((32, 4, 6, 3), (1, 3, 6)), ((8, 16, 4, 5), (2, 4))])
+def test_dslash_block_swizzle(lgt, dims, zs):
+    """The slab-by-slab block order (lgt_set_block_swizzle) is a pure relabelling of blocks: D, D^dag and a whole CG
+    solve must be bitwise what the lexicographic order gives, and equal to the oracle."""
+    U = synth.warm_links(dims, 0.3, 17)
+    psi = synth.gaussian_spinor(dims, 18)
+    lat = lgt.Lattice(dims, 5.6, 0.12, BC)
+    lat.set_links(U)
+    assert lgt.lgt_set_block_swizzle(lat.ctx, 0) == 0
+    base = [lat.dslash(psi, dagger=d) for d in (False, True)]
+    x0, it0, _, ok0 = lat.cg(psi, 1e-10, 2000)
+    for d in (False, True):
+        assert site_rel_err(base[d], oracle.dslash(dims, 0.12, BC, U, psi, dagger=d)) < TOL64
+    for z in zs:
+        assert lgt.lgt_set_block_swizzle(lat.ctx, z) == z
+        for d in (False, True):
+            assert np.array_equal(lat.dslash(psi, dagger=d), base[d])
+        x, it, _, ok = lat.cg(psi, 1e-10, 2000)
+        assert ok and ok0 and it == it0
+        assert np.abs(x - x0).max() <= 1e-13 * np.abs(x0).max()  # block partials are summed in another order
+    with pytest.raises(lgt.LgtError):
+        lgt.lgt_set_block_swizzle(lat.ctx, 5 if dims[2] % 5 else 7)
+    assert lgt.lgt_set_block_swizzle(lat.ctx, -1) == 0  # small lattice: automatic choice is "off"
+    lat.close()
+
+
 @pytest.mark.parametrize("dims", [(4, 3, 5, 6), (16, 16, 16, 16)])
 def test_dslash_fp32(lgt, dims):
     U = round32(synth.warm_links(dims, 0.3, 7))
@@ -401,6 +427,7 @@ def test_config4_largest_lattice_sampled(lgt):
     sites = _sample_sites(V, 100, 5)
     lat = lgt.Lattice(dims, 5.6, kappa, bc)
     lat.set_links(U)
+    assert lgt.lgt_set_block_swizzle(lat.ctx, -1) > 0  # one time slice exceeds the L2 budget: slab order is on
     out = lat.dslash(X)
     assert site_rel_err(out[sites], oracle.dslash_sites(dims, kappa, bc, U, X, sites)) < TOL64
     del out
