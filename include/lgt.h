@@ -41,6 +41,7 @@ typedef struct lgt_ctx lgt_ctx; /* opaque */
 
 enum { LGT_OK = 0, LGT_EINVAL = -1, LGT_ENOMEM = -2, LGT_ECUDA = -3, LGT_ENOCONV = -4, LGT_ESTATE = -5 };
 enum { LGT_F64 = 0, LGT_F32 = 1 };
+enum { LGT_SOLVER_CG = 0, LGT_SOLVER_MIXED_CG = 1 };
 
 /* ---- lifetime -------------------------------------------------------------------------- */
 
@@ -95,6 +96,20 @@ int lgt_dslash(lgt_ctx* ctx, const void* in, void* out, int dagger);
  * iters, rel_resid (= |r|/|b|) may be NULL.  Returns LGT_ENOCONV if the cap was hit (x holds the
  * last iterate). */
 int lgt_cg(lgt_ctx* ctx, const void* b, void* x, double tol, int max_iter, int* iters, double* rel_resid);
+
+/* Mixed-precision variant (LGT_F64 handles only).  Same system, same x0 = 0, same answer to
+ * tolerance: defect correction x <- x + e where e ~ (D^dag D)^-1 r comes from a CG run entirely in fp32 on the
+ * residual scaled to unit norm, to relative residual max(inner_tol, tol |b| / (4 |r|)); then r = b - D^dag D x in
+ * fp64.  Stops when the TRUE residual satisfies |r| <= tol |b| (so rel_resid is a true, not a recurrence, residual).
+ * inner_iters = fp32 CG iterations in total (capped by max_iter), outer_cycles = corrections; any may be NULL.
+ * LGT_ENOCONV if the cap (or 40 cycles) was hit; x then holds the last iterate. */
+int lgt_cg_mixed(lgt_ctx* ctx, const void* b, void* x, double tol, int max_iter, double inner_tol,
+                 int* inner_iters, int* outer_cycles, double* rel_resid);
+/* Chooses the solver used wherever the library solves the pseudofermion system itself (lgt_action, lgt_fermion_force
+ * with X = Y = NULL, lgt_md_*): LGT_SOLVER_CG (default; the plain CG of lgt_cg, iteration counts identical to the
+ * oracle's in fp64) or LGT_SOLVER_MIXED_CG with the given inner_tol (ignored for LGT_SOLVER_CG).  cg_iters outputs
+ * then count fp32 iterations. */
+int lgt_set_solver(lgt_ctx* ctx, int solver, double inner_tol);
 
 /* ---- A4, A5: forces (PAPER.md:105-109 Eq. 7; :425 Eq. S3.12; :462-506 S4) ----------------- */
 /* F^g_mu(x) = (beta/6) P_su(3)[ U_mu(x) V_mu(x) ], V = sum of the six staples. F: [V][4][3][3]. */

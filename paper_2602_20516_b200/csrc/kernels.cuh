@@ -668,6 +668,43 @@ __global__ void __launch_bounds__(256) kinetic_kernel(Geom g, const typename Vec
     block_reduce_finalize(acc, partials, counter, [result](double sum) { *result = sum; });
 }
 
+// ---------------------------------------------------------------------------- mixed-precision solver helpers
+// (fp32 inner CG inside an fp64 defect-correction loop.)  All are one pass over n complex numbers.
+// dst = (float)(scale * src)
+__global__ void __launch_bounds__(256) down_convert_kernel(size_t n, const double2* __restrict__ src, float2* __restrict__ dst,
+                                                           double scale) {
+    for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+        double2 v = __ldg(src + i);
+        float2 o;
+        o.x = (float)(scale * v.x);
+        o.y = (float)(scale * v.y);
+        dst[i] = o;
+    }
+}
+// x += a * (double)e
+__global__ void __launch_bounds__(256) up_axpy_kernel(size_t n, double2* __restrict__ x, const float2* __restrict__ e, double a) {
+    for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+        float2 ev = __ldg(e + i);
+        double2 xv = x[i];
+        xv.x = fma(a, (double)ev.x, xv.x);
+        xv.y = fma(a, (double)ev.y, xv.y);
+        x[i] = xv;
+    }
+}
+// r = b - q, result = |r|^2 (fixed-order sum)
+__global__ void __launch_bounds__(256) residual_kernel(size_t n, const double2* __restrict__ b, const double2* __restrict__ q,
+                                                       double2* __restrict__ r, double* result, double* partials, unsigned* counter) {
+    double acc = 0.0;
+    for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+        double2 bv = __ldg(b + i), qv = __ldg(q + i);
+        bv.x -= qv.x;
+        bv.y -= qv.y;
+        r[i] = bv;
+        acc += bv.x * bv.x + bv.y * bv.y;
+    }
+    block_reduce_finalize(acc, partials, counter, [result](double sum) { *result = sum; });
+}
+
 // ---------------------------------------------------------------------------- layout conversion
 __device__ __forceinline__ int link_sign(const Geom& g, int s, int mu) {
     if (g.bc[mu] > 0) return 1;

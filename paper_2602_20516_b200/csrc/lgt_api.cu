@@ -29,6 +29,13 @@ struct lgt_ctx {
     void* phi = nullptr;  // native pseudofermion
     bool has_phi = false;
     void* ws[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};  // x, r, p, t, (spare), b
+    // mixed-precision solver (LGT_F64 handles only, lazy): fp32 copy of the links, five fp32 spinor workspaces
+    void* U32 = nullptr;
+    bool u32_valid = false;
+    void* ws32[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};  // b, e, r, p, t
+    int solver = LGT_SOLVER_CG;
+    double inner_tol = 1e-5;
+    int last_outer = 0;
     void* F = nullptr;      // compact force buffer for the canonical-output calls (lazy)
     void* stage = nullptr;  // canonical staging buffer for *_host calls and conversions (lazy)
     size_t stage_bytes = 0;
@@ -160,15 +167,16 @@ template <class T> struct Ops {
         return LGT_OK;
     }
     static int unit_links(lgt_ctx* c) {
+        c->u32_valid = false;
         LAUNCH(c, LGT_K_OTHER, (unit_links_kernel<T>), stream_blocks(c, (size_t)36 * c->g.Vs), 256, c->g, (T2*)c->U);
         return LGT_OK;
     }
 
     // mode 0: out = D in / D^dag in; 1: CG "t = D p" (+ pAp, alpha); 2: CG "q = D^dag t" fused with the x, r update
-    static int dslash(lgt_ctx* c, const void* in, void* out, int dagger, int mode, void* r = nullptr) {
+    static int dslash(lgt_ctx* c, const void* U, const void* in, void* out, int dagger, int mode, void* r = nullptr) {
         const int grid = (c->g.Vs + 127) / 128;
         const T kappa = (T)c->kappa;
-#define DSLASH_ARGS c->g, (const T2*)c->U, (const T2*)in, (T2*)out, kappa, c->st, c->partials, (T2*)r
+#define DSLASH_ARGS c->g, (const T2*)U, (const T2*)in, (T2*)out, kappa, c->st, c->partials, (T2*)r
         if (mode == 0) {
             if (dagger)
                 LAUNCH(c, LGT_K_DSLASH, (dslash_kernel<T, 1, 0>), grid, 128, DSLASH_ARGS);
@@ -186,8 +194,10 @@ template <class T> struct Ops {
     // CG on D^dag D (reading A-10): b, x native; y (optional) receives D x.
     // Per iteration: t = D p (+ |t|^2) | alpha | q = D^dag t fused with r -= alpha q (+ |r|^2) | beta, stop test |
     // x += alpha p, p = r + beta p.
-    static int cg(lgt_ctx* c, const void* b, void* x, void* y, double tol, int max_iter, int* iters, double* rel) {
-        T2 *r = (T2*)c->ws[1], *p = (T2*)c->ws[2], *t = (T2*)c->ws[3];
+    // U: native links of precision T; wr, wp, wt: three native spinor workspaces of precision T.
+    static int cg(lgt_ctx* c, const void* U, void* wr, void* wp, void* wt, const void* b, void* x, void* y, double tol,
+                  int max_iter, int* iters, double* rel) {
+        T2 *r = (T2*)wr, *p = (T2*)wp, *t = (T2*)wt;
         const size_t n = (size_t)12 * c->g.Vs;
         const int nb = stream_blocks(c, n);
         const int ngrid = (c->g.Vs + 127) / 128;  // blocks (= partials) of the stencil kernels
@@ -203,9 +213,9 @@ template <class T> struct Ops {
             if (chunk > 8) chunk = 8;
             if (chunk <= 0) chunk = 1;
             for (int i = 0; i < chunk; i++) {
-                if ((rc = dslash(c, p, t, 0, 1)) != LGT_OK) return rc;
+                if ((rc = dslash(c, U, p, t, 0, 1)) != LGT_OK) return rc;
                 LAUNCH(c, LGT_K_CG_BLAS, (cg_scalars_kernel<1>), 1, 1024, ngrid, c->partials, c->st);
-                if ((rc = dslash(c, t, nullptr, 1, 2, r)) != LGT_OK) return rc;
+                if ((rc = dslash(c, U, t, nullptr, 1, 2, r)) != LGT_OK) return rc;
                 LAUNCH(c, LGT_K_CG_BLAS, (cg_scalars_kernel<2>), 1, 1024, ngrid, c->partials, c->st);
                 LAUNCH(c, LGT_K_CG_BLAS, (cg_update_xp_kernel<T>), nb, 256, n, (T2*)x, p, (const T2*)r, c->st, launched + i + 1);
             }
@@ -214,7 +224,7 @@ template <class T> struct Ops {
         const CgState& h = *c->h_st;
         if (iters) *iters = h.iter;
         if (rel) *rel = (h.bb > 0.0) ? sqrt(h.rr / h.bb) : 0.0;
-        if (y && (rc = dslash(c, x, y, 0, 0)) != LGT_OK) return rc;
+        if (y && (rc = dslash(c, U, x, y, 0, 0)) != LGT_OK) return rc;
         if (h.rr > h.tol2 * h.bb) return fail(c, LGT_ENOCONV, "CG did not reach the tolerance within max_iter");
         return LGT_OK;
     }
@@ -237,6 +247,7 @@ template <class T> struct Ops {
     }
     static int link_update(lgt_ctx* c, double eps) {
         const int grid = c->g.Vs / 32;
+        c->u32_valid = false;
         LAUNCH(c, LGT_K_LINK_UPDATE, (link_update_kernel<T>), grid, 128, c->g, (T2*)c->U, (const T2*)c->P, (T)eps);
         return LGT_OK;
     }
@@ -278,6 +289,75 @@ int auto_swizzle(const lgt_ctx* c) {
     return best;
 }
 
+// Mixed-precision solve of (D^dag D) x = b on an fp64 handle:
+// defect correction x <- x + e, e ~ (D^dag D)^-1 r from a CG run entirely in fp32 (fp32 links, fp32 vectors, the
+// same fused kernels instantiated for float) on the residual scaled to unit norm, then r = b - D^dag D x in fp64.
+// Stops on the TRUE fp64 residual |r| <= tol |b|.  iters = fp32 CG iterations in total; outer = correction cycles.
+// After the loop t = D x (fp64) is what the last residual evaluation left behind, so y = D x costs nothing.
+int cg_mixed(lgt_ctx* c, const void* b, void* x, void* y, double tol, int max_iter, int* iters, double* rel) {
+    if (c->prec != LGT_F64) return fail(c, LGT_ESTATE, "mixed-precision CG needs an LGT_F64 handle");
+    typedef Ops<double> O64;
+    typedef Ops<float> O32;
+    const size_t n = (size_t)12 * c->g.Vs;
+    if (!c->U32) {
+        CU(cudaMalloc(&c->U32, (size_t)36 * c->g.Vs * sizeof(float2)));
+        for (int i = 0; i < 5; i++) CU(cudaMalloc(&c->ws32[i], n * sizeof(float2)));
+        c->u32_valid = false;
+    }
+    const int nb = stream_blocks(c, n);
+    if (!c->u32_valid) {
+        const size_t nu = (size_t)36 * c->g.Vs;
+        LAUNCH(c, LGT_K_OTHER, down_convert_kernel, stream_blocks(c, nu), 256, nu, (const double2*)c->U, (float2*)c->U32, 1.0);
+        c->u32_valid = true;
+    }
+    double2 *r = (double2*)c->ws[1], *q = (double2*)c->ws[2];
+    double2* t = (double2*)(y ? y : c->ws[3]);
+    float2 *b32 = (float2*)c->ws32[0], *e32 = (float2*)c->ws32[1];
+    int rc, total = 0, outer = 0, conv = LGT_OK;
+    CU(cudaMemsetAsync(x, 0, n * sizeof(double2), c->stream));
+    CU(cudaMemsetAsync(t, 0, n * sizeof(double2), c->stream));
+    CU(cudaMemcpyAsync(r, b, n * sizeof(double2), cudaMemcpyDeviceToDevice, c->stream));
+    if ((rc = O64::redot(c, b, b, c->scal + 3)) != LGT_OK) return rc;
+    CU(cudaMemcpyAsync(c->h_scal + 3, c->scal + 3, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    const double bb = c->h_scal[3];
+    double rr = bb;
+    while (bb > 0.0 && rr > tol * tol * bb) {
+        if (total >= max_iter || outer >= 40) {
+            conv = LGT_ENOCONV;
+            break;
+        }
+        const double scale = 1.0 / sqrt(rr);
+        LAUNCH(c, LGT_K_CG_BLAS, down_convert_kernel, nb, 256, n, (const double2*)r, b32, scale);
+        // the inner solve need not go below what the outer tolerance still asks for
+        double eps = 0.25 * tol * sqrt(bb / rr);
+        if (eps < c->inner_tol) eps = c->inner_tol;
+        int it = 0;
+        rc = O32::cg(c, c->U32, c->ws32[2], c->ws32[3], c->ws32[4], b32, e32, nullptr, eps, max_iter - total, &it, nullptr);
+        if (rc != LGT_OK && rc != LGT_ENOCONV) return rc;
+        total += it;
+        outer++;
+        LAUNCH(c, LGT_K_CG_BLAS, up_axpy_kernel, nb, 256, n, (double2*)x, (const float2*)e32, 1.0 / scale);
+        if ((rc = O64::dslash(c, c->U, x, t, 0, 0)) != LGT_OK) return rc;
+        if ((rc = O64::dslash(c, c->U, t, q, 1, 0)) != LGT_OK) return rc;
+        LAUNCH(c, LGT_K_CG_BLAS, residual_kernel, nb, 256, n, (const double2*)b, (const double2*)q, r, c->scal + 3, c->partials, c->counter);
+        CU(cudaMemcpyAsync(c->h_scal + 3, c->scal + 3, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+        CU(cudaStreamSynchronize(c->stream));
+        rr = c->h_scal[3];
+    }
+    c->last_outer = outer;
+    if (iters) *iters = total;
+    if (rel) *rel = bb > 0.0 ? sqrt(rr / bb) : 0.0;
+    if (conv != LGT_OK) return fail(c, LGT_ENOCONV, "mixed-precision CG did not reach the tolerance");
+    return LGT_OK;
+}
+
+// the handle's solver for the pseudofermion system: plain fp64/fp32 CG, or the mixed-precision one
+int solve(lgt_ctx* c, const void* b, void* x, void* y, double tol, int max_iter, int* iters, double* rel) {
+    if (c->solver == LGT_SOLVER_MIXED_CG && c->prec == LGT_F64) return cg_mixed(c, b, x, y, tol, max_iter, iters, rel);
+    return DISPATCH(c, cg, c, c->U, c->ws[1], c->ws[2], c->ws[3], b, x, y, tol, max_iter, iters, rel);
+}
+
 bool fermions_on(const lgt_ctx* c) { return c->kappa != 0.0 && c->has_phi; }
 
 // Pi -= eps (F^g + F^f)
@@ -285,7 +365,7 @@ int kick(lgt_ctx* c, double eps, double tol, int max_iter, int* cg_iters) {
     int rc, it = 0, conv = LGT_OK;
     if ((rc = DISPATCH(c, gauge_force, c, c->P, 1, eps)) != LGT_OK) return rc;
     if (fermions_on(c)) {
-        rc = DISPATCH(c, cg, c, c->phi, c->ws[0], c->ws[3], tol, max_iter, &it, nullptr);
+        rc = solve(c, c->phi, c->ws[0], c->ws[3], tol, max_iter, &it, nullptr);
         if (rc == LGT_ENOCONV) conv = rc;
         else if (rc != LGT_OK) return rc;
         if ((rc = DISPATCH(c, fermion_force, c, c->ws[0], c->ws[3], c->P, 1, eps)) != LGT_OK) return rc;
@@ -300,7 +380,7 @@ int hamiltonian(lgt_ctx* c, double tol, int max_iter, double* S_g, double* S_F, 
     if ((rc = DISPATCH(c, kinetic, c, c->scal + 1)) != LGT_OK) return rc;
     bool ferm = fermions_on(c) && S_F != nullptr;
     if (ferm) {
-        rc = DISPATCH(c, cg, c, c->phi, c->ws[0], nullptr, tol, max_iter, &it, nullptr);
+        rc = solve(c, c->phi, c->ws[0], nullptr, tol, max_iter, &it, nullptr);
         if (rc == LGT_ENOCONV) conv = rc;
         else if (rc != LGT_OK) return rc;
         if ((rc = DISPATCH(c, redot, c, c->phi, c->ws[0], c->scal + 2)) != LGT_OK) return rc;
@@ -417,6 +497,8 @@ int lgt_destroy(lgt_ctx* c) {
     cudaFree(c->phi);
     for (int i = 0; i < 6; i++) cudaFree(c->ws[i]);
     cudaFree(c->F);
+    cudaFree(c->U32);
+    for (int i = 0; i < 5; i++) cudaFree(c->ws32[i]);
     cudaFree(c->stage);
     cudaFree(c->partials);
     cudaFree(c->counter);
@@ -481,6 +563,7 @@ long lgt_native_spinor_bytes(const lgt_ctx* c) { return c ? (long)spinor_bytes(c
 int lgt_set_links(lgt_ctx* c, const void* U) {
     CHECK_CTX(c);
     if (!U) return fail(c, LGT_EINVAL, "lgt_set_links: null pointer");
+    c->u32_valid = false;
     return DISPATCH(c, to_native, c, U, c->U, 36);
 }
 int lgt_get_links(lgt_ctx* c, void* U) {
@@ -567,14 +650,14 @@ int lgt_spinor_from_native(lgt_ctx* c, const void* native, void* canonical) {
 int lgt_dslash_native(lgt_ctx* c, const void* in, void* out, int dagger) {
     CHECK_CTX(c);
     if (!in || !out || in == out) return fail(c, LGT_EINVAL, "lgt_dslash_native: in and out must be distinct non-null buffers");
-    return DISPATCH(c, dslash, c, in, out, dagger ? 1 : 0, 0);
+    return DISPATCH(c, dslash, c, c->U, in, out, dagger ? 1 : 0, 0);
 }
 int lgt_dslash(lgt_ctx* c, const void* in, void* out, int dagger) {
     CHECK_CTX(c);
     if (!in || !out || in == out) return fail(c, LGT_EINVAL, "lgt_dslash: in and out must be distinct non-null buffers");
     int rc;
     if ((rc = DISPATCH(c, to_native, c, in, c->ws[3], 12)) != LGT_OK) return rc;
-    if ((rc = DISPATCH(c, dslash, c, c->ws[3], c->ws[4], dagger ? 1 : 0, 0)) != LGT_OK) return rc;
+    if ((rc = DISPATCH(c, dslash, c, c->U, c->ws[3], c->ws[4], dagger ? 1 : 0, 0)) != LGT_OK) return rc;
     return DISPATCH(c, from_native, c, c->ws[4], out, 12);
 }
 
@@ -583,7 +666,7 @@ int lgt_cg_native(lgt_ctx* c, const void* b, void* x, void* y, double tol, int m
     CHECK_CTX(c);
     if (!b || !x || b == x) return fail(c, LGT_EINVAL, "lgt_cg_native: bad pointers");
     if (!(tol >= 0.0) || max_iter < 0) return fail(c, LGT_EINVAL, "lgt_cg_native: bad tol / max_iter");
-    return DISPATCH(c, cg, c, b, x, y, tol, max_iter, iters, rel_resid);
+    return DISPATCH(c, cg, c, c->U, c->ws[1], c->ws[2], c->ws[3], b, x, y, tol, max_iter, iters, rel_resid);
 }
 int lgt_cg(lgt_ctx* c, const void* b, void* x, double tol, int max_iter, int* iters, double* rel_resid) {
     CHECK_CTX(c);
@@ -591,7 +674,34 @@ int lgt_cg(lgt_ctx* c, const void* b, void* x, double tol, int max_iter, int* it
     if (!(tol >= 0.0) || max_iter < 0) return fail(c, LGT_EINVAL, "lgt_cg: bad tol / max_iter");
     int rc;
     if ((rc = DISPATCH(c, to_native, c, b, c->ws[5], 12)) != LGT_OK) return rc;
-    int conv = DISPATCH(c, cg, c, c->ws[5], c->ws[0], nullptr, tol, max_iter, iters, rel_resid);
+    int conv = DISPATCH(c, cg, c, c->U, c->ws[1], c->ws[2], c->ws[3], c->ws[5], c->ws[0], nullptr, tol, max_iter, iters, rel_resid);
+    if (conv != LGT_OK && conv != LGT_ENOCONV) return conv;
+    if ((rc = DISPATCH(c, from_native, c, c->ws[0], x, 12)) != LGT_OK) return rc;
+    return conv;
+}
+
+int lgt_set_solver(lgt_ctx* c, int solver, double inner_tol) {
+    CHECK_CTX(c);
+    if (solver != LGT_SOLVER_CG && solver != LGT_SOLVER_MIXED_CG) return fail(c, LGT_EINVAL, "lgt_set_solver: unknown solver");
+    if (solver == LGT_SOLVER_MIXED_CG && c->prec != LGT_F64) return fail(c, LGT_EINVAL, "lgt_set_solver: mixed precision needs an LGT_F64 handle");
+    if (solver == LGT_SOLVER_MIXED_CG && !(inner_tol > 0.0 && inner_tol < 1.0)) return fail(c, LGT_EINVAL, "lgt_set_solver: inner_tol must be in (0, 1)");
+    c->solver = solver;
+    if (solver == LGT_SOLVER_MIXED_CG) c->inner_tol = inner_tol;
+    return LGT_OK;
+}
+int lgt_cg_mixed(lgt_ctx* c, const void* b, void* x, double tol, int max_iter, double inner_tol, int* inner_iters, int* outer_cycles,
+                 double* rel_resid) {
+    CHECK_CTX(c);
+    if (!b || !x) return fail(c, LGT_EINVAL, "lgt_cg_mixed: null pointer");
+    if (!(tol >= 0.0) || max_iter < 0 || !(inner_tol > 0.0 && inner_tol < 1.0)) return fail(c, LGT_EINVAL, "lgt_cg_mixed: bad tol / max_iter / inner_tol");
+    if (c->prec != LGT_F64) return fail(c, LGT_EINVAL, "lgt_cg_mixed: needs an LGT_F64 handle");
+    int rc;
+    if ((rc = DISPATCH(c, to_native, c, b, c->ws[5], 12)) != LGT_OK) return rc;
+    const double keep = c->inner_tol;
+    c->inner_tol = inner_tol;
+    int conv = cg_mixed(c, c->ws[5], c->ws[0], nullptr, tol, max_iter, inner_iters, rel_resid);
+    c->inner_tol = keep;
+    if (outer_cycles) *outer_cycles = c->last_outer;
     if (conv != LGT_OK && conv != LGT_ENOCONV) return conv;
     if ((rc = DISPATCH(c, from_native, c, c->ws[0], x, 12)) != LGT_OK) return rc;
     return conv;
@@ -621,7 +731,7 @@ int lgt_fermion_force(lgt_ctx* c, const void* X, const void* Y, void* F, double 
         if ((rc = DISPATCH(c, to_native, c, Y, c->ws[3], 12)) != LGT_OK) return rc;
     } else {
         if (!c->has_phi) return fail(c, LGT_ESTATE, "lgt_fermion_force: no pseudofermion set");
-        conv = DISPATCH(c, cg, c, c->phi, c->ws[0], c->ws[3], tol, max_iter, &it, nullptr);
+        conv = solve(c, c->phi, c->ws[0], c->ws[3], tol, max_iter, &it, nullptr);
         if (conv != LGT_OK && conv != LGT_ENOCONV) return conv;
     }
     if (cg_iters) *cg_iters = it;

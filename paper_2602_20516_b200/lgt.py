@@ -13,6 +13,7 @@ LIB_PATH = os.path.join(_HERE, "liblgt.so")
 
 LGT_OK, LGT_EINVAL, LGT_ENOMEM, LGT_ECUDA, LGT_ENOCONV, LGT_ESTATE = 0, -1, -2, -3, -4, -5
 LGT_F64, LGT_F32 = 0, 1
+LGT_SOLVER_CG, LGT_SOLVER_MIXED_CG = 0, 1
 
 # every symbol include/lgt.h declares: (restype, argtypes)
 _vp, _i, _d, _l = C.c_void_p, C.c_int, C.c_double, C.c_long
@@ -55,6 +56,8 @@ SYMBOLS = {
     "lgt_launch_count": (_l, [_vp]),
     "lgt_stream": (_vp, [_vp]),
     "lgt_set_block_swizzle": (_i, [_vp, _i, _ip]),
+    "lgt_cg_mixed": (_i, [_vp, _vp, _vp, _d, _i, _d, _ip, _ip, _dp]),
+    "lgt_set_solver": (_i, [_vp, _i, _d]),
 }
 
 _lib = None
@@ -182,6 +185,18 @@ def lgt_cg(ctx, b, x, tol, max_iter):
     it, rel = C.c_int(), C.c_double()
     rc = _check(ctx, lib().lgt_cg(ctx, _ptr(b), _ptr(x), tol, max_iter, C.byref(it), C.byref(rel)), allow=(LGT_ENOCONV,))
     return it.value, rel.value, rc == LGT_OK
+
+
+def lgt_cg_mixed(ctx, b, x, tol, max_iter, inner_tol=1e-5):
+    """Mixed-precision defect-correction CG.  Returns (inner_iters, outer_cycles, true_rel_resid, converged)."""
+    it, outer, rel = C.c_int(), C.c_int(), C.c_double()
+    rc = _check(ctx, lib().lgt_cg_mixed(ctx, _ptr(b), _ptr(x), tol, max_iter, inner_tol, C.byref(it), C.byref(outer),
+                                        C.byref(rel)), allow=(LGT_ENOCONV,))
+    return it.value, outer.value, rel.value, rc == LGT_OK
+
+
+def lgt_set_solver(ctx, solver, inner_tol=1e-5):
+    return _check(ctx, lib().lgt_set_solver(ctx, int(solver), float(inner_tol)))
 
 
 def lgt_gauge_force(ctx, F):
@@ -361,6 +376,11 @@ class Lattice:
         x = self.empty(self.V, 4, 3)
         it, rel, ok = lgt_cg(self.ctx, self.to_device(b), x, tol, max_iter)
         return x.cpu().numpy(), it, rel, ok
+
+    def cg_mixed(self, b, tol, max_iter, inner_tol=1e-5):
+        x = self.empty(self.V, 4, 3)
+        it, outer, rel, ok = lgt_cg_mixed(self.ctx, self.to_device(b), x, tol, max_iter, inner_tol)
+        return x.cpu().numpy(), it, outer, rel, ok
 
     def gauge_force(self):
         F = self.empty(self.V, 4, 3, 3)

@@ -150,6 +150,65 @@ def test_cg_and_fermion_force_configs(lgt, cfg):
     lat.close()
 
 
+@pytest.mark.parametrize("cfg,dims", [(0, None), (2, None), (2, (6, 10, 4, 8))])
+def test_mixed_precision_cg(lgt, cfg, dims):
+    """fp32 inner CG inside an fp64 defect-correction loop.  The solution of a linear system is unique,
+    so the reference is the oracle's fp64 CG solution and the TRUE residual taken with the oracle's D; iteration
+    counts are this solver's own (reading A-25) and are only bounded here.  Then the whole fermion kick
+    through the mixed solver against the oracle force (1e-11 per link)."""
+    c = synth.CONFIGS[cfg]
+    dims = dims or c["dims"]
+    # Solved to 1e-13 on both sides: with plain CG the two sides stop the same recurrence at the same iteration and
+    # their solution errors cancel in the comparison; here the stopping rules differ (recurrence residual in the
+    # oracle, true residual in the mixed solver), the errors are independent, and at 1e-12 the per-link force
+    # difference is 1.5e-11 - 2.1e-11 (measured), just above the 1e-11 bar.
+    kappa, bc, tol = c["kappa"], c["bc"], 1e-13
+    V = synth.volume(dims)
+    U = synth.warm_links(dims, c["eps"], c["seed_links"])
+    eta = synth.gaussian_spinor(dims, c["seed_eta"])
+    phi = oracle.dslash(dims, kappa, bc, U, eta, dagger=True)
+    X_ref, it_ref, _, ok_ref = oracle.cg(dims, kappa, bc, U, phi, tol, 10 * V)
+    Y_ref = oracle.dslash(dims, kappa, bc, U, X_ref)
+    F_ref = oracle.fermion_force(dims, kappa, bc, U, X_ref, Y_ref)
+    assert ok_ref
+
+    lat = lgt.Lattice(dims, 5.5, kappa, bc)
+    lat.set_links(U)
+    X, inner, outer, rel, ok = lat.cg_mixed(phi, tol, 10 * V, inner_tol=1e-5)
+    assert ok and rel <= tol
+    assert 2 <= outer <= 8 and inner <= 2 * it_ref, (inner, outer, it_ref)
+    # true residual with the oracle's operator
+    AX = oracle.dslash(dims, kappa, bc, U, oracle.dslash(dims, kappa, bc, U, X), dagger=True)
+    true_rel = np.linalg.norm(phi - AX) / np.linalg.norm(phi)
+    assert true_rel <= 1.05 * tol, true_rel
+    assert site_rel_err(X, X_ref) < 1e-9
+    # a looser inner tolerance costs more cycles but reaches the same answer
+    X2, inner2, outer2, rel2, ok2 = lat.cg_mixed(phi, tol, 10 * V, inner_tol=1e-3)
+    assert ok2 and rel2 <= tol and outer2 > outer
+    assert site_rel_err(X2, X_ref) < 1e-9
+    # the fermion force and action through the handle's solver switch
+    lat.set_pseudofermion(phi)
+    lgt.lgt_set_solver(lat.ctx, lgt.LGT_SOLVER_MIXED_CG, 1e-5)
+    F, it2 = lat.fermion_force(None, None, tol=tol, max_iter=10 * V)
+    assert it2 == inner
+    e, plain = link_rel_err(F, F_ref)
+    assert e < TOL64, (e, plain)
+    _, S_F, _, _ = lgt.lgt_action(lat.ctx, tol, 10 * V)
+    n2 = np.sum(np.abs(eta) ** 2)
+    assert abs(S_F - n2) < 1e-11 * n2  # pin P6: S_F = |eta|^2
+    lgt.lgt_set_solver(lat.ctx, lgt.LGT_SOLVER_CG)
+    F, it3 = lat.fermion_force(None, None, tol=tol, max_iter=10 * V)
+    assert it3 == it_ref
+    # cap reached: LGT_ENOCONV, reported as not converged
+    _, inner4, _, rel4, ok4 = lat.cg_mixed(phi, tol, 5, inner_tol=1e-5)
+    assert not ok4 and inner4 == 5 and rel4 > tol
+    lat.close()
+    lat32 = lgt.Lattice(dims, 5.5, kappa, bc, precision=lgt.LGT_F32)
+    with pytest.raises(lgt.LgtError):
+        lgt.lgt_set_solver(lat32.ctx, lgt.LGT_SOLVER_MIXED_CG, 1e-5)
+    lat32.close()
+
+
 @pytest.mark.parametrize("dims", [(4, 3, 5, 6), (6, 2, 1, 10), (3, 3, 3, 3), (8, 8, 8, 8)])
 def test_fermion_force_ragged_shapes(lgt, dims):
     """Force kernel alone on shapes that do not fill a 128-site block, with extents of 1 and 2 (forward and
