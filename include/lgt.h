@@ -42,6 +42,7 @@ typedef struct lgt_ctx lgt_ctx; /* opaque */
 enum { LGT_OK = 0, LGT_EINVAL = -1, LGT_ENOMEM = -2, LGT_ECUDA = -3, LGT_ENOCONV = -4, LGT_ESTATE = -5 };
 enum { LGT_F64 = 0, LGT_F32 = 1 };
 enum { LGT_SOLVER_CG = 0, LGT_SOLVER_MIXED_CG = 1 };
+enum { LGT_ACTION_FULL = 0, LGT_ACTION_EO = 1 };
 
 /* ---- lifetime -------------------------------------------------------------------------- */
 
@@ -110,6 +111,25 @@ int lgt_cg_mixed(lgt_ctx* ctx, const void* b, void* x, double tol, int max_iter,
  * oracle's in fp64) or LGT_SOLVER_MIXED_CG with the given inner_tol (ignored for LGT_SOLVER_CG).  cg_iters outputs
  * then count fp32 iterations. */
 int lgt_set_solver(lgt_ctx* ctx, int solver, double inner_tol);
+
+/* ---- even/odd (Schur) preconditioning (every extent of the lattice must be even) ---------- */
+/* With sites split by parity p = (x+y+z+t) mod 2, D = [[1, -kappa H_eo], [-kappa H_oe, 1]] and
+ *   M = 1 - kappa^2 H_eo H_oe   (acts on even sites),   det D = det M,
+ * so phi_e^dag (M^dag M)^-1 phi_e is a pseudofermion action for the same two-flavour determinant as
+ * phi^dag (D^dag D)^-1 phi, with a better conditioned solve on half the sites.
+ * lgt_eo_mhat: out = M in (dagger != 0: M^dag in) on the even sites of canonical full-size spinors; odd sites of
+ *   `in` are ignored and odd sites of `out` are set to zero.
+ * lgt_eo_cg: solves (M^dag M) x_e = b_e by the same CG recurrence and stop rule as lgt_cg (x0 = 0, recurrence
+ *   residual, iters = applications of M^dag M); canonical full-size spinors, odd sites ignored / zeroed. */
+int lgt_eo_mhat(lgt_ctx* ctx, const void* in, void* out, int dagger);
+int lgt_eo_cg(lgt_ctx* ctx, const void* b, void* x, double tol, int max_iter, int* iters, double* rel_resid);
+/* Chooses the pseudofermion action used by lgt_action, lgt_fermion_force (X = Y = NULL) and lgt_md_*:
+ *   LGT_ACTION_FULL (default): S_F = phi^dag (D^dag D)^-1 phi, the paper's form;
+ *   LGT_ACTION_EO: S_F = phi_e^dag (M^dag M)^-1 phi_e (only the even sites of the pseudofermion are used).  Its force
+ *     is the same fused per-link kernel applied to X = (X_e, kappa H_oe X_e), Y = (Y_e, kappa H_oe^dag Y_e) with
+ *     X_e = (M^dag M)^-1 phi_e, Y_e = M X_e (DESIGN.md derives this from S3.12).
+ * LGT_EINVAL if an extent is odd. */
+int lgt_set_fermion_action(lgt_ctx* ctx, int action);
 
 /* ---- A4, A5: forces (PAPER.md:105-109 Eq. 7; :425 Eq. S3.12; :462-506 S4) ----------------- */
 /* F^g_mu(x) = (beta/6) P_su(3)[ U_mu(x) V_mu(x) ], V = sum of the six staples. F: [V][4][3][3]. */

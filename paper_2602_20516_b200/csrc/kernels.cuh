@@ -29,6 +29,8 @@ struct Geom {
     // a slab of swz_Z z-planes before moving to the next slab, so that the t neighbours stay in L2 on big lattices
     int swz_Z;
     int swz_cxy;    // 128-site chunks per xy plane
+    int Vh;         // sites of one parity (V / 2; even/odd fields need every extent even)
+    int Vhs;        // Vh padded to a multiple of 32
 };
 
 // lexicographic 128-site chunk handled by block b
@@ -666,6 +668,155 @@ __global__ void __launch_bounds__(256) kinetic_kernel(Geom g, const typename Vec
         acc += d0 * d0 + d1 * d1 + d2 * d2 + 2.0 * off;
     }
     block_reduce_finalize(acc, partials, counter, [result](double sum) { *result = sum; });
+}
+
+// ---------------------------------------------------------------------------- even/odd (checkerboard) fields
+// SURVEY 8(f)1.  Parity p = (x+y+z+t) & 1, checkerboard index c = s >> 1 of the lexicographic site s (Lx even, so
+// the two sites 2c, 2c+1 of a pair have opposite parity).  A half field holds the Vh sites of one parity in the same
+// blocked layout as a full field: spinor half[blk][12][32], links half[blk][4][9][32] with blk = c / 32; the
+// helpers spinor_at / link_at apply unchanged to a half-field base pointer.
+__device__ __forceinline__ Site cb_coords(const Geom& g, int p, int c, int& s) {
+    Site cs;
+    const int Lxh = g.L[0] >> 1;
+    const int xh = c % Lxh;
+    int r = c / Lxh;
+    cs.x[1] = r % g.L[1];
+    r /= g.L[1];
+    cs.x[2] = r % g.L[2];
+    cs.x[3] = r / g.L[2];
+    const int odd = (cs.x[1] + cs.x[2] + cs.x[3] + p) & 1;
+    cs.x[0] = 2 * xh + odd;
+    s = 2 * c + odd;
+    return cs;
+}
+
+// acc += (1 + SG gamma_MU) U_MU(s) in(s+MU): link of the output site's parity (Up), spinor of the other parity
+template <int MU, int SG, class T>
+__device__ __forceinline__ void hop_fwd_cb(const Geom& g, const typename Vec2<T>::type* Up, const typename Vec2<T>::type* in,
+                                           const Site& cs, int s, int c, cx<T> acc[12]) {
+    const int cn = nbr_fwd(g, cs, s, MU) >> 1;
+    cx<T> p[12], h[6], u[9], w[6];
+    load_spinor<T>(in, cn, p);
+    load_link<T>(Up, MU, c, u);
+    spin_project<MU, SG>(p, h);
+    su3_mul_half(u, h, w);
+    spin_reconstruct_add<MU, SG>(w, acc);
+}
+// acc += (1 + SG gamma_MU) U_MU^dag(s-MU) in(s-MU): link and spinor of the other parity (Uq, in)
+template <int MU, int SG, class T>
+__device__ __forceinline__ void hop_bwd_cb(const Geom& g, const typename Vec2<T>::type* Uq, const typename Vec2<T>::type* in,
+                                           const Site& cs, int s, cx<T> acc[12]) {
+    const int cn = nbr_bwd(g, cs, s, MU) >> 1;
+    cx<T> p[12], h[6], u[9], w[6];
+    load_spinor<T>(in, cn, p);
+    load_link<T>(Uq, MU, cn, u);
+    spin_project<MU, SG>(p, h);
+    su3_dag_mul_half(u, h, w);
+    spin_reconstruct_add<MU, SG>(w, acc);
+}
+
+// One parity of the hopping term H = sum_mu [(1 - gamma) U psi(x+mu) + (1 + gamma) U^dag psi(x-mu)] (D = 1 - kappa H),
+// one thread per output site of parity p; DAG: gamma -> -gamma.   val = self - kap * (H in)  (self == nullptr: 0).
+//   MODE 0: out = val.                            MODE 3: the same inside CG (returns at once when converged)
+//   MODE 1: out = val, block partials of |val|^2  (second half of M p, feeds alpha)
+//   MODE 2: r -= alpha val, block partials of |r|^2 (second half of M^dag u fused with the residual update)
+// With kap = -kappa and no self this is the odd half "t_o = kappa H_oe p_e"; with kap = +kappa and self = p_e the
+// even half "p_e - kappa H_eo t_o" of the Schur complement M = 1 - kappa^2 H_eo H_oe.
+template <class T, int DAG, int MODE>
+__global__ void __launch_bounds__(128, 1) hop_cb_kernel(Geom g, int p, const typename Vec2<T>::type* __restrict__ Up,
+                                                        const typename Vec2<T>::type* __restrict__ Uq,
+                                                        const typename Vec2<T>::type* __restrict__ in,
+                                                        const typename Vec2<T>::type* __restrict__ self,
+                                                        typename Vec2<T>::type* __restrict__ out, T kap, CgState* st,
+                                                        double* partials, typename Vec2<T>::type* __restrict__ r) {
+    const int done = (MODE != 0) ? st->done : 0;
+    const int c = blockIdx.x * blockDim.x + threadIdx.x;
+    double nrm = 0.0;
+    if (c < g.Vh) {
+        if (MODE == 2) {
+            const typename Vec2<T>::type* br = spinor_at(r, c);
+#pragma unroll
+            for (int k = 0; k < 12; k++) asm volatile("prefetch.global.L2 [%0];" ::"l"(br + k * W));
+        }
+        int s;
+        const Site cs = cb_coords(g, p, c, s);
+        cx<T> acc[12];
+#pragma unroll
+        for (int k = 0; k < 12; k++) acc[k] = mk<T>(0, 0);
+        constexpr int F = DAG ? +1 : -1;
+        hop_fwd_cb<0, F, T>(g, Up, in, cs, s, c, acc);
+        if (MODE != 0 && done) return;  // uniform over the grid
+        hop_bwd_cb<0, -F, T>(g, Uq, in, cs, s, acc);
+        hop_fwd_cb<1, F, T>(g, Up, in, cs, s, c, acc);
+        hop_bwd_cb<1, -F, T>(g, Uq, in, cs, s, acc);
+        hop_fwd_cb<2, F, T>(g, Up, in, cs, s, c, acc);
+        hop_bwd_cb<2, -F, T>(g, Uq, in, cs, s, acc);
+        hop_fwd_cb<3, F, T>(g, Up, in, cs, s, c, acc);
+        hop_bwd_cb<3, -F, T>(g, Uq, in, cs, s, acc);
+        if (MODE == 2) {
+            const T alpha = (T)st->alpha;
+            const typename Vec2<T>::type* bi = spinor_at(self, c);
+            typename Vec2<T>::type* br = spinor_at(r, c);
+#pragma unroll
+            for (int k = 0; k < 12; k++) {
+                cx<T> sv = ldc<T>(bi + k * W);
+                cx<T> q = mk<T>(fma(-kap, acc[k].re, sv.re), fma(-kap, acc[k].im, sv.im));
+                cx<T> rv = ldc_rw<T>(br + k * W);
+                rv.re = fma(-alpha, q.re, rv.re);
+                rv.im = fma(-alpha, q.im, rv.im);
+                stc<T>(br + k * W, rv);
+                nrm += (double)rv.re * (double)rv.re + (double)rv.im * (double)rv.im;
+            }
+        } else {
+            typename Vec2<T>::type* bo = spinor_at(out, c);
+#pragma unroll
+            for (int k = 0; k < 12; k++) {
+                cx<T> sv = mk<T>(0, 0);
+                if (self) sv = ldc<T>(spinor_at(self, c) + k * W);
+                cx<T> o = mk<T>(fma(-kap, acc[k].re, sv.re), fma(-kap, acc[k].im, sv.im));
+                stc<T>(bo + k * W, o);
+                if (MODE == 1) nrm += (double)o.re * (double)o.re + (double)o.im * (double)o.im;
+            }
+        }
+    } else {
+        if (MODE != 0 && done) return;
+        if (c < g.Vhs && MODE != 2) {
+            typename Vec2<T>::type* bo = spinor_at(out, c);
+#pragma unroll
+            for (int k = 0; k < 12; k++) stc<T>(bo + k * W, mk<T>(0, 0));
+        }
+    }
+    if (MODE == 1 || MODE == 2) block_partial(nrm, partials);
+}
+
+// full field (lexicographic blocked layout) <-> two half fields.  DIR 0: split, DIR 1: merge.  NCOMP 12 or 36.
+// half = [parity][Vhs * NCOMP]; padding lanes of the halves are zeroed on split.
+template <class T, int DIR, int NCOMP>
+__global__ void __launch_bounds__(256) eo_reorder_kernel(Geom g, typename Vec2<T>::type* __restrict__ full,
+                                                         typename Vec2<T>::type* __restrict__ half) {
+    const size_t n = (size_t)2 * g.Vhs * NCOMP;
+    for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+        // i enumerates the half-field order (parity, blk, k, lane)
+        const int p = (int)(i / ((size_t)g.Vhs * NCOMP));
+        const size_t j = i - (size_t)p * g.Vhs * NCOMP;
+        const int lane = (int)(j & 31);
+        const int k = (int)((j >> 5) % NCOMP);
+        const int c = (int)((j >> 5) / NCOMP) * W + lane;
+        if (c < g.Vh) {
+            int s;
+            cb_coords(g, p, c, s);
+            typename Vec2<T>::type* f = full + ((size_t)(s >> 5) * (NCOMP * W) + (size_t)k * W + (s & 31));
+            if (DIR == 0)
+                half[i] = *f;
+            else
+                *f = half[i];
+        } else if (DIR == 0) {
+            typename Vec2<T>::type z;
+            z.x = 0;
+            z.y = 0;
+            half[i] = z;
+        }
+    }
 }
 
 // ---------------------------------------------------------------------------- mixed-precision solver helpers

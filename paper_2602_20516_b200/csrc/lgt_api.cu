@@ -33,6 +33,11 @@ struct lgt_ctx {
     void* U32 = nullptr;
     bool u32_valid = false;
     void* ws32[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};  // b, e, r, p, t
+    // even/odd preconditioned action (lazy): checkerboard copy of the links, eight half spinor fields
+    int action = LGT_ACTION_FULL;
+    void* Ucb = nullptr;
+    bool ucb_valid = false;
+    void* eo = nullptr;  // Xe, Xo, Ye, Yo, be, re, pe, to: 8 x 12 * Vhs complex
     int solver = LGT_SOLVER_CG;
     double inner_tol = 1e-5;
     int last_outer = 0;
@@ -168,6 +173,7 @@ template <class T> struct Ops {
     }
     static int unit_links(lgt_ctx* c) {
         c->u32_valid = false;
+        c->ucb_valid = false;
         LAUNCH(c, LGT_K_OTHER, (unit_links_kernel<T>), stream_blocks(c, (size_t)36 * c->g.Vs), 256, c->g, (T2*)c->U);
         return LGT_OK;
     }
@@ -248,6 +254,7 @@ template <class T> struct Ops {
     static int link_update(lgt_ctx* c, double eps) {
         const int grid = c->g.Vs / 32;
         c->u32_valid = false;
+        c->ucb_valid = false;
         LAUNCH(c, LGT_K_LINK_UPDATE, (link_update_kernel<T>), grid, 128, c->g, (T2*)c->U, (const T2*)c->P, (T)eps);
         return LGT_OK;
     }
@@ -259,10 +266,115 @@ template <class T> struct Ops {
         LAUNCH(c, LGT_K_OTHER, (kinetic_kernel<T>), stream_blocks(c, (size_t)4 * c->g.Vs), 256, c->g, (const T2*)c->P, dev_result, c->partials, c->counter);
         return LGT_OK;
     }
-    static int redot(lgt_ctx* c, const void* a, const void* b, double* dev_result) {
-        const size_t n = (size_t)12 * c->g.Vs;
+    static int redot(lgt_ctx* c, const void* a, const void* b, double* dev_result, size_t n = 0) {
+        if (n == 0) n = (size_t)12 * c->g.Vs;
         LAUNCH(c, LGT_K_OTHER, (redot_kernel<T>), stream_blocks(c, n), 256, n, (const T2*)a, (const T2*)b, dev_result, c->partials, c->counter);
         return LGT_OK;
+    }
+
+    // ---- even/odd preconditioning
+    static T2* eo_field(lgt_ctx* c, int i) { return (T2*)c->eo + (size_t)i * 12 * c->g.Vhs; }
+    static const T2* links_cb(lgt_ctx* c, int p) { return (const T2*)c->Ucb + (size_t)p * 36 * c->g.Vhs; }
+    static int eo_ensure(lgt_ctx* c) {
+        if (!c->Ucb) {
+            CU(cudaMalloc(&c->Ucb, (size_t)2 * 36 * c->g.Vhs * sizeof(T2)));
+            c->ucb_valid = false;
+        }
+        if (!c->eo) {
+            CU(cudaMalloc(&c->eo, (size_t)8 * 12 * c->g.Vhs * sizeof(T2)));
+            CU(cudaMemsetAsync(c->eo, 0, (size_t)8 * 12 * c->g.Vhs * sizeof(T2), c->stream));
+        }
+        if (!c->ucb_valid) {
+            const size_t n = (size_t)2 * 36 * c->g.Vhs;
+            LAUNCH(c, LGT_K_OTHER, (eo_reorder_kernel<T, 0, 36>), stream_blocks(c, n), 256, c->g, (T2*)c->U, (T2*)c->Ucb);
+            c->ucb_valid = true;
+        }
+        return LGT_OK;
+    }
+    // full native spinor -> (even, odd) halves at eo fields (ie, ie + 1), or back
+    static int eo_split(lgt_ctx* c, const void* full, T2* halves) {
+        const size_t n = (size_t)2 * 12 * c->g.Vhs;
+        LAUNCH(c, LGT_K_OTHER, (eo_reorder_kernel<T, 0, 12>), stream_blocks(c, n), 256, c->g, (T2*)full, halves);
+        return LGT_OK;
+    }
+    static int eo_merge(lgt_ctx* c, T2* halves, void* full) {
+        const size_t n = (size_t)2 * 12 * c->g.Vhs;
+        LAUNCH(c, LGT_K_OTHER, (eo_reorder_kernel<T, 1, 12>), stream_blocks(c, n), 256, c->g, (T2*)full, halves);
+        return LGT_OK;
+    }
+    // out (parity p) = self - kap * H in (in of parity 1 - p); mode as in hop_cb_kernel
+    static int hop(lgt_ctx* c, int p, const T2* in, const T2* self, T2* out, int dagger, int mode, double kap, T2* r = nullptr) {
+        const int grid = (c->g.Vhs + 127) / 128;
+#define HOP_ARGS c->g, p, links_cb(c, p), links_cb(c, 1 - p), in, self, out, (T)kap, c->st, c->partials, r
+        if (mode == 0) {
+            if (dagger) LAUNCH(c, LGT_K_DSLASH, (hop_cb_kernel<T, 1, 0>), grid, 128, HOP_ARGS);
+            else LAUNCH(c, LGT_K_DSLASH, (hop_cb_kernel<T, 0, 0>), grid, 128, HOP_ARGS);
+        } else if (mode == 3) {
+            if (dagger) LAUNCH(c, LGT_K_DSLASH, (hop_cb_kernel<T, 1, 3>), grid, 128, HOP_ARGS);
+            else LAUNCH(c, LGT_K_DSLASH, (hop_cb_kernel<T, 0, 3>), grid, 128, HOP_ARGS);
+        } else if (mode == 1) {
+            LAUNCH(c, LGT_K_DSLASH, (hop_cb_kernel<T, 0, 1>), grid, 128, HOP_ARGS);
+        } else {
+            LAUNCH(c, LGT_K_DSLASH_R, (hop_cb_kernel<T, 1, 2>), grid, 128, HOP_ARGS);
+        }
+#undef HOP_ARGS
+        return LGT_OK;
+    }
+    // out_e = M in_e (dagger: M^dag in_e), M = 1 - kappa^2 H_eo H_oe; scratch_o receives kappa H_oe in_e
+    static int eo_mhat(lgt_ctx* c, const T2* in_e, T2* out_e, T2* scratch_o, int dagger) {
+        int rc;
+        if ((rc = hop(c, 1, in_e, nullptr, scratch_o, dagger, 0, -c->kappa)) != LGT_OK) return rc;
+        return hop(c, 0, scratch_o, in_e, out_e, dagger, 0, c->kappa);
+    }
+    // CG on M^dag M x_e = b_e, x0 = 0, same recurrence and stop rule as cg(); u_e, t_o are scratch half fields.
+    static int eo_cg(lgt_ctx* c, const T2* b, T2* x, T2* r, T2* p, T2* u, T2* t, double tol, int max_iter, int* iters, double* rel) {
+        const size_t n = (size_t)12 * c->g.Vhs;
+        const int nb = stream_blocks(c, n);
+        const int ngrid = (c->g.Vhs + 127) / 128;
+        LAUNCH(c, LGT_K_CG_BLAS, (cg_init_kernel<T>), nb, 256, n, b, x, r, p, c->st, tol * tol, max_iter, c->partials, c->counter);
+        int rc, launched = 0;
+        for (;;) {
+            CU(cudaMemcpyAsync(c->h_st, c->st, sizeof(CgState), cudaMemcpyDeviceToHost, c->stream));
+            CU(cudaStreamSynchronize(c->stream));
+            if (c->h_st->done) break;
+            int chunk = max_iter - launched;
+            if (chunk > 8) chunk = 8;
+            if (chunk <= 0) chunk = 1;
+            for (int i = 0; i < chunk; i++) {
+                if ((rc = hop(c, 1, p, nullptr, t, 0, 3, -c->kappa)) != LGT_OK) return rc;   // t_o = kappa H_oe p
+                if ((rc = hop(c, 0, t, p, u, 0, 1, c->kappa)) != LGT_OK) return rc;          // u = M p, |u|^2
+                LAUNCH(c, LGT_K_CG_BLAS, (cg_scalars_kernel<1>), 1, 1024, ngrid, c->partials, c->st);
+                if ((rc = hop(c, 1, u, nullptr, t, 1, 3, -c->kappa)) != LGT_OK) return rc;   // t_o = kappa H^dag_oe u
+                if ((rc = hop(c, 0, t, u, nullptr, 1, 2, c->kappa, r)) != LGT_OK) return rc; // r -= alpha M^dag u
+                LAUNCH(c, LGT_K_CG_BLAS, (cg_scalars_kernel<2>), 1, 1024, ngrid, c->partials, c->st);
+                LAUNCH(c, LGT_K_CG_BLAS, (cg_update_xp_kernel<T>), nb, 256, n, x, p, (const T2*)r, c->st, launched + i + 1);
+            }
+            launched += chunk;
+        }
+        const CgState& h = *c->h_st;
+        if (iters) *iters = h.iter;
+        if (rel) *rel = (h.bb > 0.0) ? sqrt(h.rr / h.bb) : 0.0;
+        if (h.rr > h.tol2 * h.bb) return fail(c, LGT_ENOCONV, "even/odd CG did not reach the tolerance within max_iter");
+        return LGT_OK;
+    }
+    // Even/odd action: X_e = (M^dag M)^-1 phi_e, Y_e = M X_e, X_o = kappa H_oe X_e, Y_o = kappa H^dag_oe Y_e, merged into
+    // the full fields X, Y (native) that the fused force kernel takes; Re <phi_e, X_e> to dev_SF if not null.
+    static int eo_solve_xy(lgt_ctx* c, void* X, void* Y, double tol, int max_iter, int* iters, double* dev_SF) {
+        int rc, conv;
+        if ((rc = eo_ensure(c)) != LGT_OK) return rc;
+        T2 *Xe = eo_field(c, 0), *Xo = eo_field(c, 1), *Ye = eo_field(c, 2), *Yo = eo_field(c, 3);
+        T2 *be = eo_field(c, 4), *re = eo_field(c, 5), *pe = eo_field(c, 6), *to = eo_field(c, 7);
+        if ((rc = eo_split(c, c->phi, be)) != LGT_OK) return rc;  // (be, re) receive (phi_e, phi_o); re is overwritten next
+        conv = eo_cg(c, be, Xe, re, pe, Ye, to, tol, max_iter, iters, nullptr);
+        if (conv != LGT_OK && conv != LGT_ENOCONV) return conv;
+        if (dev_SF && (rc = redot(c, be, Xe, dev_SF, (size_t)12 * c->g.Vhs)) != LGT_OK) return rc;
+        if (X && Y) {
+            if ((rc = eo_mhat(c, Xe, Ye, Xo, 0)) != LGT_OK) return rc;                  // Y_e = M X_e, X_o = kappa H_oe X_e
+            if ((rc = hop(c, 1, Ye, nullptr, Yo, 1, 0, -c->kappa)) != LGT_OK) return rc;  // Y_o = kappa H^dag_oe Y_e
+            if ((rc = eo_merge(c, Xe, X)) != LGT_OK) return rc;
+            if ((rc = eo_merge(c, Ye, Y)) != LGT_OK) return rc;
+        }
+        return conv;
     }
 };
 
@@ -352,10 +464,22 @@ int cg_mixed(lgt_ctx* c, const void* b, void* x, void* y, double tol, int max_it
     return LGT_OK;
 }
 
-// the handle's solver for the pseudofermion system: plain fp64/fp32 CG, or the mixed-precision one
-int solve(lgt_ctx* c, const void* b, void* x, void* y, double tol, int max_iter, int* iters, double* rel) {
-    if (c->solver == LGT_SOLVER_MIXED_CG && c->prec == LGT_F64) return cg_mixed(c, b, x, y, tol, max_iter, iters, rel);
-    return DISPATCH(c, cg, c, c->U, c->ws[1], c->ws[2], c->ws[3], b, x, y, tol, max_iter, iters, rel);
+// X = ws[0], Y = ws[3] (full native fields, as the fused force kernel takes them) for the handle's fermion action and
+// solver; dev_SF (may be null) receives S_F on the device.  y == false: only X (and S_F) are wanted.
+//   LGT_ACTION_FULL: X = (D^dag D)^-1 phi, Y = D X, S_F = Re <phi, X>   (plain or mixed-precision CG)
+//   LGT_ACTION_EO:   X_e = (M^dag M)^-1 phi_e, ...  (Ops::eo_solve_xy), S_F = Re <phi_e, X_e>
+int solve(lgt_ctx* c, bool y, double tol, int max_iter, int* iters, double* dev_SF) {
+    int rc, conv;
+    if (c->action == LGT_ACTION_EO)
+        return DISPATCH(c, eo_solve_xy, c, y ? c->ws[0] : nullptr, y ? c->ws[3] : nullptr, tol, max_iter, iters, dev_SF);
+    void* Y = y ? c->ws[3] : nullptr;
+    if (c->solver == LGT_SOLVER_MIXED_CG && c->prec == LGT_F64)
+        conv = cg_mixed(c, c->phi, c->ws[0], Y, tol, max_iter, iters, nullptr);
+    else
+        conv = DISPATCH(c, cg, c, c->U, c->ws[1], c->ws[2], c->ws[3], c->phi, c->ws[0], Y, tol, max_iter, iters, nullptr);
+    if (conv != LGT_OK && conv != LGT_ENOCONV) return conv;
+    if (dev_SF && (rc = DISPATCH(c, redot, c, c->phi, c->ws[0], dev_SF, 0)) != LGT_OK) return rc;
+    return conv;
 }
 
 bool fermions_on(const lgt_ctx* c) { return c->kappa != 0.0 && c->has_phi; }
@@ -365,7 +489,7 @@ int kick(lgt_ctx* c, double eps, double tol, int max_iter, int* cg_iters) {
     int rc, it = 0, conv = LGT_OK;
     if ((rc = DISPATCH(c, gauge_force, c, c->P, 1, eps)) != LGT_OK) return rc;
     if (fermions_on(c)) {
-        rc = solve(c, c->phi, c->ws[0], c->ws[3], tol, max_iter, &it, nullptr);
+        rc = solve(c, true, tol, max_iter, &it, nullptr);
         if (rc == LGT_ENOCONV) conv = rc;
         else if (rc != LGT_OK) return rc;
         if ((rc = DISPATCH(c, fermion_force, c, c->ws[0], c->ws[3], c->P, 1, eps)) != LGT_OK) return rc;
@@ -380,10 +504,9 @@ int hamiltonian(lgt_ctx* c, double tol, int max_iter, double* S_g, double* S_F, 
     if ((rc = DISPATCH(c, kinetic, c, c->scal + 1)) != LGT_OK) return rc;
     bool ferm = fermions_on(c) && S_F != nullptr;
     if (ferm) {
-        rc = solve(c, c->phi, c->ws[0], nullptr, tol, max_iter, &it, nullptr);
+        rc = solve(c, false, tol, max_iter, &it, c->scal + 2);
         if (rc == LGT_ENOCONV) conv = rc;
         else if (rc != LGT_OK) return rc;
-        if ((rc = DISPATCH(c, redot, c, c->phi, c->ws[0], c->scal + 2)) != LGT_OK) return rc;
     }
     if ((rc = read_scalars(c, 3)) != LGT_OK) return rc;
     if (S_g) *S_g = c->beta * (6.0 * (double)c->g.V - c->h_scal[0]);
@@ -393,6 +516,39 @@ int hamiltonian(lgt_ctx* c, double tol, int max_iter, double* S_g, double* S_F, 
     return conv;
 }
 
+}  // namespace
+
+namespace {
+int eo_check(lgt_ctx* c, const char* what) {
+    for (int m = 0; m < 4; m++)
+        if (c->g.L[m] % 2) return fail(c, LGT_EINVAL, what);
+    return LGT_OK;
+}
+template <class T> int eo_mhat_canonical(lgt_ctx* c, const void* in, void* out, int dagger) {
+    typedef Ops<T> O;
+    int rc;
+    if ((rc = O::eo_ensure(c)) != LGT_OK) return rc;
+    if ((rc = O::to_native(c, in, c->ws[5], 12)) != LGT_OK) return rc;
+    if ((rc = O::eo_split(c, c->ws[5], O::eo_field(c, 4))) != LGT_OK) return rc;          // fields 4, 5 = (in_e, in_o)
+    if ((rc = O::eo_mhat(c, O::eo_field(c, 4), O::eo_field(c, 2), O::eo_field(c, 7), dagger)) != LGT_OK) return rc;
+    CU(cudaMemsetAsync(O::eo_field(c, 3), 0, (size_t)12 * c->g.Vhs * sizeof(typename O::T2), c->stream));  // odd part of out = 0
+    if ((rc = O::eo_merge(c, O::eo_field(c, 2), c->ws[5])) != LGT_OK) return rc;
+    return O::from_native(c, c->ws[5], out, 12);
+}
+template <class T> int eo_cg_canonical(lgt_ctx* c, const void* b, void* x, double tol, int max_iter, int* iters, double* rel) {
+    typedef Ops<T> O;
+    int rc;
+    if ((rc = O::eo_ensure(c)) != LGT_OK) return rc;
+    if ((rc = O::to_native(c, b, c->ws[5], 12)) != LGT_OK) return rc;
+    if ((rc = O::eo_split(c, c->ws[5], O::eo_field(c, 4))) != LGT_OK) return rc;
+    int conv = O::eo_cg(c, O::eo_field(c, 4), O::eo_field(c, 0), O::eo_field(c, 5), O::eo_field(c, 6), O::eo_field(c, 2),
+                        O::eo_field(c, 7), tol, max_iter, iters, rel);
+    if (conv != LGT_OK && conv != LGT_ENOCONV) return conv;
+    CU(cudaMemsetAsync(O::eo_field(c, 1), 0, (size_t)12 * c->g.Vhs * sizeof(typename O::T2), c->stream));  // odd part of x = 0
+    if ((rc = O::eo_merge(c, O::eo_field(c, 0), c->ws[5])) != LGT_OK) return rc;
+    if ((rc = O::from_native(c, c->ws[5], x, 12)) != LGT_OK) return rc;
+    return conv;
+}
 }  // namespace
 
 #define CHECK_CTX(c) \
@@ -444,6 +600,8 @@ int lgt_create(lgt_ctx** out, const int dims[4], double beta, double kappa, cons
     }
     c->g.V = (int)V;
     c->g.Vs = (int)((V + 31) / 32 * 32);
+    c->g.Vh = (int)(V / 2);
+    c->g.Vhs = (c->g.Vh + 31) / 32 * 32;
     c->g.swz_cxy = (int)(((long long)dims[0] * dims[1]) / 128);
     c->g.swz_Z = auto_swizzle(c);
     int sms = 148;
@@ -498,6 +656,8 @@ int lgt_destroy(lgt_ctx* c) {
     for (int i = 0; i < 6; i++) cudaFree(c->ws[i]);
     cudaFree(c->F);
     cudaFree(c->U32);
+    cudaFree(c->Ucb);
+    cudaFree(c->eo);
     for (int i = 0; i < 5; i++) cudaFree(c->ws32[i]);
     cudaFree(c->stage);
     cudaFree(c->partials);
@@ -564,6 +724,7 @@ int lgt_set_links(lgt_ctx* c, const void* U) {
     CHECK_CTX(c);
     if (!U) return fail(c, LGT_EINVAL, "lgt_set_links: null pointer");
     c->u32_valid = false;
+    c->ucb_valid = false;
     return DISPATCH(c, to_native, c, U, c->U, 36);
 }
 int lgt_get_links(lgt_ctx* c, void* U) {
@@ -680,6 +841,32 @@ int lgt_cg(lgt_ctx* c, const void* b, void* x, double tol, int max_iter, int* it
     return conv;
 }
 
+int lgt_set_fermion_action(lgt_ctx* c, int action) {
+    CHECK_CTX(c);
+    if (action != LGT_ACTION_FULL && action != LGT_ACTION_EO) return fail(c, LGT_EINVAL, "lgt_set_fermion_action: unknown action");
+    if (action == LGT_ACTION_EO)
+        for (int m = 0; m < 4; m++)
+            if (c->g.L[m] % 2) return fail(c, LGT_EINVAL, "lgt_set_fermion_action: the even/odd action needs every extent even");
+    c->action = action;
+    return LGT_OK;
+}
+int lgt_eo_mhat(lgt_ctx* c, const void* in, void* out, int dagger) {
+    CHECK_CTX(c);
+    if (!in || !out || in == out) return fail(c, LGT_EINVAL, "lgt_eo_mhat: in and out must be distinct non-null buffers");
+    int rc = eo_check(c, "lgt_eo_mhat: every extent must be even");
+    if (rc != LGT_OK) return rc;
+    return c->prec == LGT_F64 ? eo_mhat_canonical<double>(c, in, out, dagger ? 1 : 0) : eo_mhat_canonical<float>(c, in, out, dagger ? 1 : 0);
+}
+int lgt_eo_cg(lgt_ctx* c, const void* b, void* x, double tol, int max_iter, int* iters, double* rel_resid) {
+    CHECK_CTX(c);
+    if (!b || !x) return fail(c, LGT_EINVAL, "lgt_eo_cg: null pointer");
+    if (!(tol >= 0.0) || max_iter < 0) return fail(c, LGT_EINVAL, "lgt_eo_cg: bad tol / max_iter");
+    int rc = eo_check(c, "lgt_eo_cg: every extent must be even");
+    if (rc != LGT_OK) return rc;
+    return c->prec == LGT_F64 ? eo_cg_canonical<double>(c, b, x, tol, max_iter, iters, rel_resid)
+                              : eo_cg_canonical<float>(c, b, x, tol, max_iter, iters, rel_resid);
+}
+
 int lgt_set_solver(lgt_ctx* c, int solver, double inner_tol) {
     CHECK_CTX(c);
     if (solver != LGT_SOLVER_CG && solver != LGT_SOLVER_MIXED_CG) return fail(c, LGT_EINVAL, "lgt_set_solver: unknown solver");
@@ -731,7 +918,7 @@ int lgt_fermion_force(lgt_ctx* c, const void* X, const void* Y, void* F, double 
         if ((rc = DISPATCH(c, to_native, c, Y, c->ws[3], 12)) != LGT_OK) return rc;
     } else {
         if (!c->has_phi) return fail(c, LGT_ESTATE, "lgt_fermion_force: no pseudofermion set");
-        conv = solve(c, c->phi, c->ws[0], c->ws[3], tol, max_iter, &it, nullptr);
+        conv = solve(c, true, tol, max_iter, &it, nullptr);
         if (conv != LGT_OK && conv != LGT_ENOCONV) return conv;
     }
     if (cg_iters) *cg_iters = it;

@@ -14,6 +14,7 @@ LIB_PATH = os.path.join(_HERE, "liblgt.so")
 LGT_OK, LGT_EINVAL, LGT_ENOMEM, LGT_ECUDA, LGT_ENOCONV, LGT_ESTATE = 0, -1, -2, -3, -4, -5
 LGT_F64, LGT_F32 = 0, 1
 LGT_SOLVER_CG, LGT_SOLVER_MIXED_CG = 0, 1
+LGT_ACTION_FULL, LGT_ACTION_EO = 0, 1
 
 # every symbol include/lgt.h declares: (restype, argtypes)
 _vp, _i, _d, _l = C.c_void_p, C.c_int, C.c_double, C.c_long
@@ -58,6 +59,9 @@ SYMBOLS = {
     "lgt_set_block_swizzle": (_i, [_vp, _i, _ip]),
     "lgt_cg_mixed": (_i, [_vp, _vp, _vp, _d, _i, _d, _ip, _ip, _dp]),
     "lgt_set_solver": (_i, [_vp, _i, _d]),
+    "lgt_eo_mhat": (_i, [_vp, _vp, _vp, _i]),
+    "lgt_eo_cg": (_i, [_vp, _vp, _vp, _d, _i, _ip, _dp]),
+    "lgt_set_fermion_action": (_i, [_vp, _i]),
 }
 
 _lib = None
@@ -193,6 +197,21 @@ def lgt_cg_mixed(ctx, b, x, tol, max_iter, inner_tol=1e-5):
     rc = _check(ctx, lib().lgt_cg_mixed(ctx, _ptr(b), _ptr(x), tol, max_iter, inner_tol, C.byref(it), C.byref(outer),
                                         C.byref(rel)), allow=(LGT_ENOCONV,))
     return it.value, outer.value, rel.value, rc == LGT_OK
+
+
+def lgt_eo_mhat(ctx, src, dst, dagger=False):
+    return _check(ctx, lib().lgt_eo_mhat(ctx, _ptr(src), _ptr(dst), int(bool(dagger))))
+
+
+def lgt_eo_cg(ctx, b, x, tol, max_iter):
+    """CG on M^dag M (even sites).  Returns (iters, rel_resid, converged)."""
+    it, rel = C.c_int(), C.c_double()
+    rc = _check(ctx, lib().lgt_eo_cg(ctx, _ptr(b), _ptr(x), tol, max_iter, C.byref(it), C.byref(rel)), allow=(LGT_ENOCONV,))
+    return it.value, rel.value, rc == LGT_OK
+
+
+def lgt_set_fermion_action(ctx, action):
+    return _check(ctx, lib().lgt_set_fermion_action(ctx, int(action)))
 
 
 def lgt_set_solver(ctx, solver, inner_tol=1e-5):
@@ -375,6 +394,16 @@ class Lattice:
     def cg(self, b, tol, max_iter):
         x = self.empty(self.V, 4, 3)
         it, rel, ok = lgt_cg(self.ctx, self.to_device(b), x, tol, max_iter)
+        return x.cpu().numpy(), it, rel, ok
+
+    def eo_mhat(self, psi, dagger=False):
+        out = self.empty(self.V, 4, 3)
+        lgt_eo_mhat(self.ctx, self.to_device(psi), out, dagger)
+        return out.cpu().numpy()
+
+    def eo_cg(self, b, tol, max_iter):
+        x = self.empty(self.V, 4, 3)
+        it, rel, ok = lgt_eo_cg(self.ctx, self.to_device(b), x, tol, max_iter)
         return x.cpu().numpy(), it, rel, ok
 
     def cg_mixed(self, b, tol, max_iter, inner_tol=1e-5):

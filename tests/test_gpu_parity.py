@@ -6,6 +6,7 @@ import numpy as np
 import pytest
 
 import oracle
+from oracle import evenodd as oeo
 from paper_2602_20516_b200 import synth
 from lattice_util import link_rel_err
 
@@ -207,6 +208,110 @@ def test_mixed_precision_cg(lgt, cfg, dims):
     with pytest.raises(lgt.LgtError):
         lgt.lgt_set_solver(lat32.ctx, lgt.LGT_SOLVER_MIXED_CG, 1e-5)
     lat32.close()
+
+
+EO_DIMS = [(4, 4, 4, 4), (2, 2, 2, 2), (6, 10, 4, 8), (16, 4, 2, 6), (8, 8, 8, 8)]
+
+
+@pytest.mark.parametrize("dims", EO_DIMS)
+def test_eo_schur_operator(lgt, dims):
+    """M = 1 - kappa^2 H_eo H_oe and M^dag on the even sites against the oracle's definition
+    (oracle/evenodd.py), fp64 and fp32, periodic and antiperiodic boundaries; odd sites of the output are zero."""
+    U = synth.warm_links(dims, 0.3, 27)
+    psi = synth.gaussian_spinor(dims, 28)
+    odd = oeo.parity(dims) == 1
+    for bc in (BC, (1, 1, 1, 1), (-1, 1, -1, -1)):
+        lat = lgt.Lattice(dims, 5.6, 0.12, bc)
+        lat.set_links(U)
+        for dag in (False, True):
+            out = lat.eo_mhat(psi, dagger=dag)
+            ref = oeo.mhat(dims, 0.12, bc, U, psi, dagger=dag)
+            assert not out[odd].any()
+            assert site_rel_err(out[~odd], ref[~odd]) < TOL64
+        lat.close()
+    lat = lgt.Lattice(dims, 5.6, 0.12, BC, precision=lgt.LGT_F32)
+    U32, psi32 = round32(U), round32(psi)
+    lat.set_links(U32)
+    out = lat.eo_mhat(psi32).astype(np.complex128)
+    assert site_rel_err(out[~odd], oeo.mhat(dims, 0.12, BC, U32, psi32)[~odd]) < TOL32
+    lat.close()
+
+
+@pytest.mark.parametrize("dims,kappa", [((4, 4, 4, 4), 0.10), ((8, 8, 8, 8), 0.12), ((6, 10, 4, 8), 0.12)])
+def test_eo_cg_force_and_action(lgt, dims, kappa):
+    """CG on M^dag M: iteration count identical to the oracle's, solution, then the even/odd action and its per-link
+    force through lgt_set_fermion_action (reconstruction X_o = kappa H_oe X_e, Y_o = kappa H_oe^dag Y_e on the GPU),
+    the closed form S = |eta_e|^2, and one kick of the momenta."""
+    V = synth.volume(dims)
+    tol, beta = 1e-12, 5.5
+    U = synth.warm_links(dims, 0.3, 37)
+    eta = oeo.keep(synth.gaussian_spinor(dims, 38), dims, 0)
+    phi = oeo.mhat(dims, kappa, BC, U, eta, dagger=True) + oeo.keep(synth.gaussian_spinor(dims, 39), dims, 1)  # odd part must be ignored
+    X_ref, it_ref, rel_ref, ok_ref = oeo.cg(dims, kappa, BC, U, phi, tol, 10 * V)
+    F_ref, _, _ = oeo.fermion_force(dims, kappa, BC, U, phi, tol, 10 * V)
+    assert ok_ref
+
+    lat = lgt.Lattice(dims, beta, kappa, BC)
+    lat.set_links(U)
+    X, it, rel, ok = lat.eo_cg(phi, tol, 10 * V)
+    assert ok and it == it_ref, (it, it_ref, rel, rel_ref)
+    even = oeo.parity(dims) == 0
+    assert not X[~even].any()
+    assert site_rel_err(X[even], X_ref[even]) < 1e-9
+    lat.set_pseudofermion(phi)
+    lgt.lgt_set_fermion_action(lat.ctx, lgt.LGT_ACTION_EO)
+    F, it2 = lat.fermion_force(None, None, tol=tol, max_iter=10 * V)
+    assert it2 == it_ref
+    e, plain = link_rel_err(F, F_ref)
+    assert e < TOL64, (e, plain)
+    S_g, S_F, K, _ = lgt.lgt_action(lat.ctx, tol, 10 * V)
+    n2 = np.sum(np.abs(eta) ** 2)
+    assert abs(S_F - n2) < 1e-11 * n2
+    # one kick: Pi -= eps (F^g + F^eo)
+    P0 = synth.gaussian_momenta(dims, 40)
+    lat.set_momenta(P0)
+    its = lgt.lgt_md_kick(lat.ctx, 0.05, tol, 10 * V)
+    assert its == it_ref
+    P_ref = P0 - 0.05 * (oracle.gauge_force(dims, beta, U) + F_ref)
+    assert link_rel_err(lat.get_momenta(), P_ref)[0] < TOL64
+    # the full action is untouched by the switch back
+    lgt.lgt_set_fermion_action(lat.ctx, lgt.LGT_ACTION_FULL)
+    _, S_full, _, _ = lgt.lgt_action(lat.ctx, tol, 10 * V)
+    S_full_ref, _, _, _ = oracle.fermion_action(dims, kappa, BC, U, phi, tol, 10 * V)
+    assert abs(S_full - S_full_ref) < 1e-10 * abs(S_full_ref)
+    lat.close()
+
+
+def test_eo_leapfrog_conserves_energy(lgt):
+    """Leapfrog with the even/odd action on 8^4: |dH| ~ dt^2 and exact reversibility (pin P7 on this action)."""
+    dims, beta, kappa = (8, 8, 8, 8), 5.6, 0.12
+    U0 = synth.warm_links(dims, 0.3, 47)
+    P0 = synth.gaussian_momenta(dims, 48)
+    phi = synth.gaussian_spinor(dims, 49)
+    lat = lgt.Lattice(dims, beta, kappa, BC)
+    lgt.lgt_set_fermion_action(lat.ctx, lgt.LGT_ACTION_EO)
+    lat.set_pseudofermion(phi)
+    dH = []
+    for n, dt in ((8, 0.02), (16, 0.01)):
+        lat.set_links(U0)
+        lat.set_momenta(P0)
+        H0, H1, _ = lgt.lgt_md_trajectory(lat.ctx, n, dt, 1e-13, 20000)
+        dH.append(abs(H1 - H0))
+    assert dH[0] < 5.0 and 3.5 < dH[0] / dH[1] < 4.5, dH
+    lat.set_momenta(-lat.get_momenta())
+    lgt.lgt_md_trajectory(lat.ctx, 16, 0.01, 1e-13, 20000)
+    assert np.abs(lat.get_links() - U0).max() < 1e-10
+    lat.close()
+
+
+def test_eo_refuses_odd_extents(lgt):
+    lat = lgt.Lattice((4, 3, 4, 4), 5.5, 0.1, BC)
+    with pytest.raises(lgt.LgtError) as e:
+        lgt.lgt_set_fermion_action(lat.ctx, lgt.LGT_ACTION_EO)
+    assert e.value.code == lgt.LGT_EINVAL
+    with pytest.raises(lgt.LgtError):
+        lat.eo_mhat(synth.gaussian_spinor((4, 3, 4, 4), 1))
+    lat.close()
 
 
 @pytest.mark.parametrize("dims", [(4, 3, 5, 6), (6, 2, 1, 10), (3, 3, 3, 3), (8, 8, 8, 8)])
