@@ -573,6 +573,49 @@ def test_config3_full_size_md_step(lgt):
     assert np.abs(U1 - U_ref).max() < 1e-13
 
 
+def test_config3_full_size_solver_variants(lgt):
+    """configs[3] at full size for the two SURVEY 8(f)1 solver variants, as bench.py's `extras` runs them, checked by
+    properties the oracle can evaluate in seconds at 32^4: the TRUE residual of the returned solution taken with the
+    oracle's D (mixed precision), resp. with the oracle's M (even/odd), and the even/odd force on sampled links
+    against the oracle's per-link force evaluated on the GPU's reconstructed X, Y."""
+    c = synth.CONFIGS[3]
+    dims, beta, kappa, bc, tol = c["dims"], c["beta"], c["kappa"], c["bc"], c["cg_tol"]
+    V = synth.volume(dims)
+    U = synth.config_links(3)
+    eta = synth.gaussian_spinor(dims, c["seed_eta"])
+    phi = oracle.dslash(dims, kappa, bc, U, eta, dagger=True)
+    nphi = np.linalg.norm(phi)
+    lat = lgt.Lattice(dims, beta, kappa, bc)
+    lat.set_links(U)
+    X, inner, outer, rel, ok = lat.cg_mixed(phi, tol, 10 * V)
+    assert ok and rel <= tol and outer <= 6 and inner < 400, (inner, outer, rel)
+    AX = oracle.dslash(dims, kappa, bc, U, oracle.dslash(dims, kappa, bc, U, X), dagger=True)
+    assert np.linalg.norm(phi - AX) / nphi <= 1.05 * tol
+    # phi = D^dag eta  =>  X = D^-1 eta, so D X = eta (pin P6) also holds for the mixed solver's X
+    assert site_rel_err(oracle.dslash(dims, kappa, bc, U, X), eta) < 1e-9
+    del AX
+    Xe, it, rel, ok = lat.eo_cg(phi, tol, 10 * V)
+    assert ok and 20 < it < 159, it  # fewer iterations than the unpreconditioned solve (159)
+    even = oeo.parity(dims) == 0
+    r = oeo.keep(phi, dims, 0) - oeo.mhat(dims, kappa, bc, U, oeo.mhat(dims, kappa, bc, U, Xe), dagger=True)
+    assert np.linalg.norm(r) / np.linalg.norm(phi[even]) <= 3 * tol  # recurrence vs true residual
+    # force through the action switch, sampled links; X, Y rebuilt by the oracle from the GPU's X_e
+    lat.set_pseudofermion(phi)
+    lgt.lgt_set_fermion_action(lat.ctx, lgt.LGT_ACTION_EO)
+    F, it2 = lat.fermion_force(None, None, tol=tol, max_iter=10 * V)
+    assert it2 == it
+    Ye = oeo.mhat(dims, kappa, bc, U, Xe)
+    Xf = Xe - oeo.keep(oracle.dslash(dims, kappa, bc, U, Xe), dims, 1)
+    Yf = Ye - oeo.keep(oracle.dslash(dims, kappa, bc, U, Ye, dagger=True), dims, 1)
+    worst = 0.0
+    for s_ in _sample_sites(V, 30, 9)[:24]:
+        for mu in range(4):
+            rf = oracle.fermion_force_link(dims, kappa, bc, U, Xf, Yf, int(s_), mu)
+            worst = max(worst, np.linalg.norm(F[s_, mu] - rf) / np.linalg.norm(rf))
+    assert worst < TOL64, worst
+    lat.close()
+
+
 def test_config4_largest_lattice_sampled(lgt):
     """configs[4] shape (48^3 x 96, the largest single-GPU working set, Lx not a multiple of the 32-site layout block):
     Dslash and fermion force on sampled sites.  The links are a periodic tiling of a seeded 24^4 warm field (a valid
