@@ -44,9 +44,19 @@ FLOPS = dict(dslash=1368, dslash_fused_r=1368 + 96, cg_update_xp=96, cg_iter=2 *
 NCU_TRAFFIC_BYTES = {"dslash_f64_32^4": 1019435008}  # profiles/r01b_ncu_full.md, dslash_kernel<double,0,1>
 
 
-def step_reals(cg_iters):
-    return (REALS["gauge_force"] + REALS["cg_init"] + cg_iters * REALS["cg_iter"] + REALS["dslash"]
-            + REALS["fermion_force"] + REALS["link_update"])
+# even/odd action, per site of the FULL lattice: a half-lattice hop reads 8 links + 1 spinor and writes 1 spinor per
+# output site, and there are V/2 output sites
+REALS_EO = dict(hop=(2 * (72 + 12 + 12)) // 2, hop_fused_r=(2 * (72 + 12 + 2 * 12)) // 2, update_xp=(2 * 5 * 12) // 2)
+REALS_EO["cg_iter"] = 3 * REALS_EO["hop"] + REALS_EO["hop_fused_r"] + REALS_EO["update_xp"]   # -> 3408 B fp64
+
+
+def step_reals(cg_iters, solver="cg", action="full"):
+    fixed = REALS["gauge_force"] + REALS["fermion_force"] + REALS["link_update"]
+    if action == "eo":  # CG on M^dag M, then Y_e = M X_e, X_o, Y_o (3 hops), split of phi and two merges (5 x 24 x 2)
+        return fixed + cg_iters * REALS_EO["cg_iter"] + 3 * REALS_EO["hop"] + 5 * 48
+    if solver == "mixed":  # fp32 iterations move half the bytes; about 4 fp64 defect-correction cycles of 2 Dslash + 3 BLAS-1
+        return fixed + cg_iters * REALS["cg_iter"] // 2 + 4 * (2 * REALS["dslash"] + 3 * 48)
+    return fixed + REALS["cg_init"] + cg_iters * REALS["cg_iter"] + REALS["dslash"]
 
 
 def step_flops(cg_iters):
@@ -201,6 +211,11 @@ def run_ours(args):
         dist.barrier()
         torch.cuda.synchronize()
 
+    if args.solver == "mixed":
+        lgt.lgt_set_solver(ctx, lgt.LGT_SOLVER_MIXED_CG, 1e-5)
+    if args.action == "eo":
+        lgt.lgt_set_fermion_action(ctx, lgt.LGT_ACTION_EO)
+    variant = args.solver != "cg" or args.action != "full"
     reset_state()
     for _ in range(args.warmup):
         md_step()
@@ -223,7 +238,7 @@ def run_ours(args):
     launches = lgt.lgt_launch_count(ctx) - launches0
     per_class = {name: lgt.lgt_timing_read(ctx, k) for k, name in enumerate(lgt.KERNEL_CLASSES)}
     lgt.lgt_timing_reset(ctx)
-    total_reals = sum(step_reals(i) for i in iters) * V
+    total_reals = sum(step_reals(i, args.solver, args.action) for i in iters) * V
     total_flops = sum(step_flops(i) for i in iters) * V
 
     # ---- end to end: host buffers in, host buffers out, through the C ABI, every step
@@ -238,13 +253,13 @@ def run_ours(args):
         lgt.lgt_get_momenta_host(ctx, hP_out)
     torch.cuda.synchronize()
     e2e_s = time.perf_counter() - t0
-    e2e_reals = sum(step_reals(i) for i in e2e_iters) * V
+    e2e_reals = sum(step_reals(i, args.solver, args.action) for i in e2e_iters) * V
     h2d = hU.numel() * 16 + hP.numel() * 16 + hphi.numel() * 16
     d2h = hU_out.numel() * 16 + hP_out.numel() * 16
 
     # ---- the same MD step with the mixed-precision solver; not the headline: `value` stays pure fp64
     extras = {}
-    if rank == 0 and not args.skip_extras:
+    if rank == 0 and not args.skip_extras and not variant:
         lgt.lgt_set_solver(ctx, lgt.LGT_SOLVER_MIXED_CG, 1e-5)
         reset_state()
         md_step()
@@ -339,7 +354,7 @@ def run_ours(args):
     peak, peak_src = measured_peaks()
     ds_ms, ds_n = per_class["dslash"]
     ds_avg_s = ds_ms / max(ds_n, 1) * 1e-3
-    ds_bytes = REALS["dslash"] * 8 * V
+    ds_bytes = (REALS_EO["hop"] if args.action == "eo" else REALS["dslash"]) * (4 if args.solver == "mixed" else 8) * V
     achieved = ds_bytes / ds_avg_s / 1e9 if ds_n else None
     shares = {name: round(ms / elapsed_ms, 4) for name, (ms, n) in per_class.items() if n}
     in_place = {}
@@ -367,19 +382,22 @@ def run_ours(args):
                                "fermion force] + drift(dt)" % (args.config, "x".join(map(str, dims))),
                    "beta": beta, "kappa": kappa, "bc": list(bc), "dt": dt, "cg_tol": tol,
                    "cg_iters_per_step": iters, "parallelism": "replicas x%d" % world,
+                   "solver": args.solver, "fermion_action": args.action,
                    "l2": "inputs exceed L2 (links 604 MB, each spinor 201 MB at 32^4)"},
         "gflops": round(total_flops / (elapsed_ms * 1e-3) / 1e9, 1),
         "clocks": clocks,
         "e2e": {"value": round(e2e_reals * 8 / e2e_s / 1e9, 1), "unit": "GB/s", "steps": k_e2e,
                 "ms_per_step": round(e2e_s / k_e2e * 1e3, 2), "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
         "gpu_launches": int(launches_all),
-        "roofline": {"kernel": "dslash_kernel<double> (inside CG, %d launches)" % ds_n, "bound": "hbm",
+        "roofline": {"kernel": ("hop_cb_kernel<double> (inside CG, %d launches)" if args.action == "eo" else
+                                "dslash_kernel<float> (inside the fp32 CG, %d launches)" if args.solver == "mixed" else
+                                "dslash_kernel<double> (inside CG, %d launches)") % ds_n, "bound": "hbm",
                      "achieved": round(achieved, 1) if achieved else None, "peak": peak, "unit": "GB/s",
                      "frac": round(achieved / peak, 4) if achieved else None,
                      "frac_of_nominal_8TBs": round(achieved / 8000.0, 4) if achieved else None,
                      "peak_source": peak_src, "avg_launch_us": round(ds_avg_s * 1e6, 2),
                      "algorithmic_bytes_per_launch": ds_bytes,
-                     "traffic": NCU_TRAFFIC_BYTES.get("dslash_f64_32^4") if tuple(dims) == (32, 32, 32, 32) else None,
+                     "traffic": NCU_TRAFFIC_BYTES.get("dslash_f64_32^4") if tuple(dims) == (32, 32, 32, 32) and not variant else None,
                      "share_of_step": shares, "kernels_in_place": in_place},
         "kernels": kernels,
         "extras": extras,
@@ -456,6 +474,10 @@ def main():
     ap.add_argument("--config", type=int, default=3, help="BASELINE.json configs index (3 = 32^4 MD step)")
     ap.add_argument("--lattice", type=int, nargs=4, default=None, help="override dims (debugging only)")
     ap.add_argument("--skip-cpu-baseline", action="store_true", help="profiling runs only: leave the oracle leg out")
+    ap.add_argument("--solver", default="cg", choices=["cg", "mixed"],
+                    help="non-default: time the step with the mixed-precision solver (not the headline configuration)")
+    ap.add_argument("--action", default="full", choices=["full", "eo"],
+                    help="non-default: time the step with the even/odd preconditioned action (not the headline configuration)")
     ap.add_argument("--skip-extras", action="store_true", help="profiling runs only: leave the non-headline solver arms out")
     ap.add_argument("--cpu-sample-iters", type=int, default=4, help="CG iterations in the oracle's bounded sample")
     args = ap.parse_args()
