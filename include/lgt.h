@@ -43,6 +43,7 @@ enum { LGT_OK = 0, LGT_EINVAL = -1, LGT_ENOMEM = -2, LGT_ECUDA = -3, LGT_ENOCONV
 enum { LGT_F64 = 0, LGT_F32 = 1 };
 enum { LGT_SOLVER_CG = 0, LGT_SOLVER_MIXED_CG = 1 };
 enum { LGT_ACTION_FULL = 0, LGT_ACTION_EO = 1 };
+enum { LGT_INT_LEAPFROG = 0, LGT_INT_OMELYAN = 1, LGT_INT_SEXTON_WEINGARTEN = 2 };
 
 /* ---- lifetime -------------------------------------------------------------------------- */
 
@@ -153,6 +154,32 @@ int lgt_md_step(lgt_ctx* ctx, double dt, double tol, int max_iter, int* cg_iters
  * evaluated before and after (either pointer may be NULL to skip that evaluation). */
 int lgt_md_trajectory(lgt_ctx* ctx, int nsteps, double dt, double tol, int max_iter,
                       double* H_initial, double* H_final, long* cg_iters);
+
+/* ---- HMC around the trajectory (leapfrog, Sexton-Weingarten with inner gauge steps) ---- */
+/* Integrator used by lgt_md_trajectory and lgt_hmc_trajectory (a step = dt, adjacent kicks merged; K = kick with both
+ * forces, Kg / Kf = gauge / fermion force only, D = drift):
+ *   LGT_INT_LEAPFROG (default):   K(dt/2) D(dt) K(dt/2)
+ *   LGT_INT_OMELYAN:              K(l dt) D(dt/2) K((1-2l) dt) D(dt/2) K(l dt), l = 0.1931833275037836 (2nd-order minimum norm)
+ *   LGT_INT_SEXTON_WEINGARTEN:    Kf(dt/2) [Kg(h/2) D(h) Kg(h/2)]^n_inner Kf(dt/2), h = dt / n_inner (n_inner >= 1; ignored else)
+ * lgt_md_step / lgt_md_kick / lgt_md_drift are not affected. */
+int lgt_set_integrator(lgt_ctx* ctx, int integrator, int n_inner);
+/* Heat baths from the counter-based generator Philox4x32-10, a pure function of (seed, trajectory, element) so that
+ * the oracle reproduces them (reading A-25: key = seed, counter = (element, draw, stream, trajectory)):
+ *   momenta:        Pi_mu(x) = sum_a pi^a tau^a, pi^a ~ N(0,1), weight exp(-K);
+ *   pseudofermion:  eta ~ exp(-eta^dag eta), then phi = D^dag eta (LGT_ACTION_FULL) or phi_e = M^dag eta_e, phi_o = 0
+ *                   (LGT_ACTION_EO), so that S_F = |eta|^2 (resp. |eta_e|^2), returned through eta_norm2 (may be NULL).
+ * LGT_ESTATE if kappa == 0. */
+int lgt_momentum_heatbath(lgt_ctx* ctx, unsigned long long seed, unsigned trajectory);
+int lgt_pseudofermion_heatbath(lgt_ctx* ctx, unsigned long long seed, unsigned trajectory, double* eta_norm2);
+/* The handle's pseudofermion in the canonical layout, [V][4][3] complex, device pointer.  LGT_ESTATE if none is set. */
+int lgt_get_pseudofermion(lgt_ctx* ctx, void* phi);
+/* One HMC trajectory: both heat baths (the pseudofermion one if kappa != 0), H_0 = K + S_g + |eta|^2, nsteps steps of
+ * the handle's integrator, H_1 = K + S_g + S_F (one more solve), Metropolis test "u < exp(-(H_1 - H_0))" with u the
+ * generator's stream-3 uniform of this trajectory; on rejection the links of the start are restored.  The momenta are
+ * left as integrated.  Outputs (any may be NULL): dH = H_1 - H_0, accepted = 0 / 1, cg_iters = solver iterations in
+ * total, H_initial = H_0.  LGT_ENOCONV if a solve hit max_iter (the trajectory is still completed). */
+int lgt_hmc_trajectory(lgt_ctx* ctx, int nsteps, double dt, double tol, int max_iter, unsigned long long seed,
+                       unsigned trajectory, double* dH, int* accepted, long* cg_iters, double* H_initial);
 
 /* ---- native-layout spinor fields (for callers that keep fields resident between calls) ---- */
 /* Bytes of one spinor field in the handle's internal layout and precision. */

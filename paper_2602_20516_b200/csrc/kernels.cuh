@@ -856,6 +856,91 @@ __global__ void __launch_bounds__(256) residual_kernel(size_t n, const double2* 
     block_reduce_finalize(acc, partials, counter, [result](double sum) { *result = sum; });
 }
 
+// ---------------------------------------------------------------------------- heat baths
+// Counter-based generator Philox4x32-10 (Salmon et al., SC'11), restated here; the draw map is DESIGN.md reading A-25:
+// key = (seed lo, seed hi), counter = (element, draw j, stream, trajectory); words x0..x3 -> two uniforms in (0,1)
+// with 53 random bits each -> one Box-Muller pair.  Always evaluated in double, whatever the handle's precision.
+__device__ __forceinline__ void philox4x32_10(unsigned c[4], unsigned k0, unsigned k1) {
+#pragma unroll
+    for (int round = 0; round < 10; round++) {
+        const unsigned hi0 = __umulhi(0xD2511F53u, c[0]), lo0 = 0xD2511F53u * c[0];
+        const unsigned hi1 = __umulhi(0xCD9E8D57u, c[2]), lo1 = 0xCD9E8D57u * c[2];
+        const unsigned n0 = hi1 ^ c[1] ^ k0, n2 = hi0 ^ c[3] ^ k1;
+        c[0] = n0;
+        c[1] = lo1;
+        c[2] = n2;
+        c[3] = lo0;
+        k0 += 0x9E3779B9u;
+        k1 += 0xBB67AE85u;
+    }
+}
+__device__ __forceinline__ void philox_uniforms(unsigned long long seed, unsigned traj, unsigned stream, unsigned element,
+                                                unsigned j, double& u1, double& u2) {
+    unsigned c[4] = {element, j, stream, traj};
+    philox4x32_10(c, (unsigned)(seed & 0xffffffffull), (unsigned)(seed >> 32));
+    const unsigned long long a = ((unsigned long long)c[1] << 32) | c[0], b = ((unsigned long long)c[3] << 32) | c[2];
+    u1 = ((double)(a >> 11) + 0.5) * 0x1p-53;
+    u2 = ((double)(b >> 11) + 0.5) * 0x1p-53;
+}
+__device__ __forceinline__ void philox_gaussian_pair(unsigned long long seed, unsigned traj, unsigned stream, unsigned element,
+                                                     unsigned j, double& g0, double& g1) {
+    double u1, u2, sn, cs;
+    philox_uniforms(seed, traj, stream, element, j, u1, u2);
+    const double rad = sqrt(-2.0 * log(u1));
+    sincos(6.283185307179586476925286766559 * u2, &sn, &cs);
+    g0 = rad * cs;
+    g1 = rad * sn;
+}
+
+// Pi_mu(s) = sum_a pi^a tau^a, pi^a ~ N(0,1) (stream 1, element = link 4 s + mu, draw j gives pi^(2j+1), pi^(2j+2)),
+// written in the compact 8-real form; padding lanes zero.
+template <class T>
+__global__ void __launch_bounds__(256) momentum_heatbath_kernel(Geom g, typename Vec2<T>::type* __restrict__ P,
+                                                                unsigned long long seed, unsigned traj) {
+    const size_t n = (size_t)4 * g.Vs;
+    for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+        const int lane = (int)(i & 31);
+        const int mu = (int)((i >> 5) & 3);
+        const int s = (int)(i >> 7) * W + lane;
+        double pi[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+        if (s < g.V) {
+#pragma unroll
+            for (int j = 0; j < 4; j++) philox_gaussian_pair(seed, traj, 1u, (unsigned)(4 * s + mu), (unsigned)j, pi[2 * j], pi[2 * j + 1]);
+        }
+        // tau^a = i lambda^a / 2:  Im Pi00 = (pi3 + pi8/sqrt3)/2, Im Pi11 = (-pi3 + pi8/sqrt3)/2,
+        // Pi01 = (pi2 + i pi1)/2, Pi02 = (pi5 + i pi4)/2, Pi12 = (pi7 + i pi6)/2      (pi1 = pi[0])
+        const double r3 = 0.57735026918962576450914878050196 * pi[7];
+        const double c[8] = {0.5 * (pi[2] + r3), 0.5 * (r3 - pi[2]), 0.5 * pi[1], 0.5 * pi[0],
+                             0.5 * pi[4],        0.5 * pi[3],        0.5 * pi[6], 0.5 * pi[5]};
+        typename Vec2<T>::type* b = mom_at(P, s, mu);
+#pragma unroll
+        for (int q = 0; q < 4; q++) {
+            typename Vec2<T>::type v;
+            v.x = (T)c[2 * q];
+            v.y = (T)c[2 * q + 1];
+            b[q * W] = v;
+        }
+    }
+}
+
+// eta(s)_k = (g0 + i g1) / sqrt 2 (stream 2, element = site s, draw j = component k = 3 alpha + a); native layout.
+template <class T>
+__global__ void __launch_bounds__(256) spinor_heatbath_kernel(Geom g, typename Vec2<T>::type* __restrict__ eta,
+                                                              unsigned long long seed, unsigned traj) {
+    const size_t n = (size_t)12 * g.Vs;
+    for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+        const int lane = (int)(i & 31);
+        const int k = (int)((i >> 5) % 12);
+        const int s = (int)((i >> 5) / 12) * W + lane;
+        double g0 = 0.0, g1 = 0.0;
+        if (s < g.V) philox_gaussian_pair(seed, traj, 2u, (unsigned)s, (unsigned)k, g0, g1);
+        typename Vec2<T>::type v;
+        v.x = (T)(0.70710678118654752440084436210485 * g0);
+        v.y = (T)(0.70710678118654752440084436210485 * g1);
+        eta[i] = v;
+    }
+}
+
 // ---------------------------------------------------------------------------- layout conversion
 __device__ __forceinline__ int link_sign(const Geom& g, int s, int mu) {
     if (g.bc[mu] > 0) return 1;

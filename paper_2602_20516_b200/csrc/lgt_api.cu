@@ -2,6 +2,7 @@
 // No torch, no host-side arithmetic on fields: every step of the path runs in the kernels of kernels.cuh.
 #include <cuda_runtime.h>
 
+#include <cmath>
 #include <cstdio>
 #include <cstring>
 #include <new>
@@ -39,6 +40,9 @@ struct lgt_ctx {
     bool ucb_valid = false;
     void* eo = nullptr;  // Xe, Xo, Ye, Yo, be, re, pe, to: 8 x 12 * Vhs complex
     int solver = LGT_SOLVER_CG;
+    int integrator = LGT_INT_LEAPFROG;
+    int n_inner = 1;        // gauge sub-steps per step of the Sexton-Weingarten integrator
+    void* Usave = nullptr;  // links at the start of an HMC trajectory (lazy)
     double inner_tol = 1e-5;
     int last_outer = 0;
     void* F = nullptr;      // compact force buffer for the canonical-output calls (lazy)
@@ -272,6 +276,31 @@ template <class T> struct Ops {
         return LGT_OK;
     }
 
+    static int momentum_heatbath(lgt_ctx* c, unsigned long long seed, unsigned traj) {
+        LAUNCH(c, LGT_K_OTHER, (momentum_heatbath_kernel<T>), stream_blocks(c, (size_t)4 * c->g.Vs), 256, c->g, (T2*)c->P, seed, traj);
+        return LGT_OK;
+    }
+    // eta ~ exp(-eta^dag eta) into ws[4]; phi = D^dag eta (full action) or phi_e = M^dag eta_e (even/odd action);
+    // S_F at the start of the trajectory, |eta|^2 resp. |eta_e|^2, to dev_SF0.
+    static int pseudofermion_heatbath(lgt_ctx* c, unsigned long long seed, unsigned traj, double* dev_SF0) {
+        int rc;
+        T2* eta = (T2*)c->ws[4];
+        LAUNCH(c, LGT_K_OTHER, (spinor_heatbath_kernel<T>), stream_blocks(c, (size_t)12 * c->g.Vs), 256, c->g, eta, seed, traj);
+        if (c->action == LGT_ACTION_EO) {
+            if ((rc = eo_ensure(c)) != LGT_OK) return rc;
+            if ((rc = eo_split(c, eta, eo_field(c, 4))) != LGT_OK) return rc;  // fields 4, 5 = (eta_e, eta_o)
+            if ((rc = eo_mhat(c, eo_field(c, 4), eo_field(c, 2), eo_field(c, 7), 1)) != LGT_OK) return rc;
+            CU(cudaMemsetAsync(eo_field(c, 3), 0, (size_t)12 * c->g.Vhs * sizeof(T2), c->stream));
+            if ((rc = eo_merge(c, eo_field(c, 2), c->phi)) != LGT_OK) return rc;
+            if (dev_SF0 && (rc = redot(c, eo_field(c, 4), eo_field(c, 4), dev_SF0, (size_t)12 * c->g.Vhs)) != LGT_OK) return rc;
+        } else {
+            if ((rc = dslash(c, c->U, eta, c->phi, 1, 0)) != LGT_OK) return rc;
+            if (dev_SF0 && (rc = redot(c, eta, eta, dev_SF0, 0)) != LGT_OK) return rc;
+        }
+        c->has_phi = true;
+        return LGT_OK;
+    }
+
     // ---- even/odd preconditioning
     static T2* eo_field(lgt_ctx* c, int i) { return (T2*)c->eo + (size_t)i * 12 * c->g.Vhs; }
     static const T2* links_cb(lgt_ctx* c, int p) { return (const T2*)c->Ucb + (size_t)p * 36 * c->g.Vhs; }
@@ -484,10 +513,29 @@ int solve(lgt_ctx* c, bool y, double tol, int max_iter, int* iters, double* dev_
 
 bool fermions_on(const lgt_ctx* c) { return c->kappa != 0.0 && c->has_phi; }
 
-// Pi -= eps (F^g + F^f)
-int kick(lgt_ctx* c, double eps, double tol, int max_iter, int* cg_iters) {
+// Metropolis uniform: Philox4x32-10 at counter (0, 0, stream 3, trajectory), first uniform (reading A-25)
+double metropolis_uniform(unsigned long long seed, unsigned traj) {
+    unsigned c[4] = {0u, 0u, 3u, traj};
+    unsigned k0 = (unsigned)(seed & 0xffffffffull), k1 = (unsigned)(seed >> 32);
+    for (int round = 0; round < 10; round++) {
+        const unsigned long long p0 = 0xD2511F53ull * c[0], p1 = 0xCD9E8D57ull * c[2];
+        const unsigned n0 = (unsigned)(p1 >> 32) ^ c[1] ^ k0, n2 = (unsigned)(p0 >> 32) ^ c[3] ^ k1;
+        c[0] = n0;
+        c[1] = (unsigned)p1;
+        c[2] = n2;
+        c[3] = (unsigned)p0;
+        k0 += 0x9E3779B9u;
+        k1 += 0xBB67AE85u;
+    }
+    const unsigned long long a = ((unsigned long long)c[1] << 32) | c[0];
+    return ((double)(a >> 11) + 0.5) * 0x1p-53;
+}
+
+// Pi -= eps F^g
+int kick_gauge(lgt_ctx* c, double eps) { return DISPATCH(c, gauge_force, c, c->P, 1, eps); }
+// Pi -= eps F^f (solve, then the fused force kernel); nothing if there are no fermions
+int kick_fermion(lgt_ctx* c, double eps, double tol, int max_iter, int* cg_iters) {
     int rc, it = 0, conv = LGT_OK;
-    if ((rc = DISPATCH(c, gauge_force, c, c->P, 1, eps)) != LGT_OK) return rc;
     if (fermions_on(c)) {
         rc = solve(c, true, tol, max_iter, &it, nullptr);
         if (rc == LGT_ENOCONV) conv = rc;
@@ -495,6 +543,59 @@ int kick(lgt_ctx* c, double eps, double tol, int max_iter, int* cg_iters) {
         if ((rc = DISPATCH(c, fermion_force, c, c->ws[0], c->ws[3], c->P, 1, eps)) != LGT_OK) return rc;
     }
     if (cg_iters) *cg_iters = it;
+    return conv;
+}
+// Pi -= eps (F^g + F^f)
+int kick(lgt_ctx* c, double eps, double tol, int max_iter, int* cg_iters) {
+    int rc;
+    if ((rc = kick_gauge(c, eps)) != LGT_OK) return rc;
+    return kick_fermion(c, eps, tol, max_iter, cg_iters);
+}
+
+// MD trajectory of nsteps steps of size dt with the handle's integrator, adjacent kicks merged (include/lgt.h).
+int integrate(lgt_ctx* c, int nsteps, double dt, double tol, int max_iter, long* cg_iters) {
+    int rc, it = 0, conv = LGT_OK;
+    long total = 0;
+#define STEP(call)                           \
+    do {                                     \
+        it = 0;                              \
+        rc = (call);                         \
+        if (rc == LGT_ENOCONV) conv = rc;    \
+        else if (rc != LGT_OK) return rc;    \
+        total += it;                         \
+    } while (0)
+#define DRIFT(eps) STEP(DISPATCH(c, link_update, c, (eps)))
+    if (nsteps > 0 && c->integrator == LGT_INT_LEAPFROG) {
+        STEP(kick(c, 0.5 * dt, tol, max_iter, &it));
+        for (int n = 0; n < nsteps; n++) {
+            DRIFT(dt);
+            STEP(kick(c, (n == nsteps - 1) ? 0.5 * dt : dt, tol, max_iter, &it));
+        }
+    } else if (nsteps > 0 && c->integrator == LGT_INT_OMELYAN) {
+        const double lam = 0.1931833275037836;
+        STEP(kick(c, lam * dt, tol, max_iter, &it));
+        for (int n = 0; n < nsteps; n++) {
+            DRIFT(0.5 * dt);
+            STEP(kick(c, (1.0 - 2.0 * lam) * dt, tol, max_iter, &it));
+            DRIFT(0.5 * dt);
+            STEP(kick(c, (n == nsteps - 1) ? lam * dt : 2.0 * lam * dt, tol, max_iter, &it));
+        }
+    } else if (nsteps > 0) {  // Sexton-Weingarten: fermion force outside, m gauge leapfrog steps inside
+        const int m = c->n_inner;
+        const double h = dt / m;
+        STEP(kick_fermion(c, 0.5 * dt, tol, max_iter, &it));
+        for (int n = 0; n < nsteps; n++) {
+            STEP(kick_gauge(c, 0.5 * h));
+            for (int i = 0; i < m; i++) {
+                DRIFT(h);
+                STEP(kick_gauge(c, (i == m - 1) ? 0.5 * h : h));
+            }
+            STEP(kick_fermion(c, (n == nsteps - 1) ? 0.5 * dt : dt, tol, max_iter, &it));
+        }
+    }
+#undef DRIFT
+#undef STEP
+    if (cg_iters) *cg_iters = total;
     return conv;
 }
 
@@ -657,6 +758,7 @@ int lgt_destroy(lgt_ctx* c) {
     cudaFree(c->F);
     cudaFree(c->U32);
     cudaFree(c->Ucb);
+    cudaFree(c->Usave);
     cudaFree(c->eo);
     for (int i = 0; i < 5; i++) cudaFree(c->ws32[i]);
     cudaFree(c->stage);
@@ -964,17 +1066,8 @@ int lgt_md_trajectory(lgt_ctx* c, int nsteps, double dt, double tol, int max_ite
         if (rc == LGT_ENOCONV) conv = rc; else if (rc != LGT_OK) return rc;
         *H_initial = k + sg + sf;
     }
-    if (nsteps > 0) {
-        rc = kick(c, 0.5 * dt, tol, max_iter, &it);
-        if (rc == LGT_ENOCONV) conv = rc; else if (rc != LGT_OK) return rc;
-        total += it;
-        for (int n = 0; n < nsteps; n++) {
-            if ((rc = DISPATCH(c, link_update, c, dt)) != LGT_OK) return rc;
-            rc = kick(c, (n == nsteps - 1) ? 0.5 * dt : dt, tol, max_iter, &it);
-            if (rc == LGT_ENOCONV) conv = rc; else if (rc != LGT_OK) return rc;
-            total += it;
-        }
-    }
+    rc = integrate(c, nsteps, dt, tol, max_iter, &total);
+    if (rc == LGT_ENOCONV) conv = rc; else if (rc != LGT_OK) return rc;
     if (H_final) {
         rc = hamiltonian(c, tol, max_iter, &sg, &sf, &k, &it);
         if (rc == LGT_ENOCONV) conv = rc; else if (rc != LGT_OK) return rc;
@@ -982,6 +1075,74 @@ int lgt_md_trajectory(lgt_ctx* c, int nsteps, double dt, double tol, int max_ite
     }
     if (cg_iters) *cg_iters = total;
     CU(cudaStreamSynchronize(c->stream));
+    return conv;
+}
+
+// ---- HMC around the MD trajectory
+int lgt_set_integrator(lgt_ctx* c, int integrator, int n_inner) {
+    CHECK_CTX(c);
+    if (integrator != LGT_INT_LEAPFROG && integrator != LGT_INT_OMELYAN && integrator != LGT_INT_SEXTON_WEINGARTEN)
+        return fail(c, LGT_EINVAL, "lgt_set_integrator: unknown integrator");
+    if (integrator == LGT_INT_SEXTON_WEINGARTEN && n_inner < 1) return fail(c, LGT_EINVAL, "lgt_set_integrator: n_inner must be >= 1");
+    c->integrator = integrator;
+    c->n_inner = integrator == LGT_INT_SEXTON_WEINGARTEN ? n_inner : 1;
+    return LGT_OK;
+}
+int lgt_momentum_heatbath(lgt_ctx* c, unsigned long long seed, unsigned trajectory) {
+    CHECK_CTX(c);
+    return DISPATCH(c, momentum_heatbath, c, seed, trajectory);
+}
+int lgt_pseudofermion_heatbath(lgt_ctx* c, unsigned long long seed, unsigned trajectory, double* eta_norm2) {
+    CHECK_CTX(c);
+    if (c->kappa == 0.0) return fail(c, LGT_ESTATE, "lgt_pseudofermion_heatbath: kappa == 0, no fermions on this handle");
+    int rc = DISPATCH(c, pseudofermion_heatbath, c, seed, trajectory, c->scal + 4);
+    if (rc != LGT_OK) return rc;
+    if (eta_norm2) {
+        if ((rc = read_scalars(c, 5)) != LGT_OK) return rc;
+        *eta_norm2 = c->h_scal[4];
+    }
+    return LGT_OK;
+}
+int lgt_get_pseudofermion(lgt_ctx* c, void* phi) {
+    CHECK_CTX(c);
+    if (!phi) return fail(c, LGT_EINVAL, "lgt_get_pseudofermion: null pointer");
+    if (!c->has_phi) return fail(c, LGT_ESTATE, "lgt_get_pseudofermion: no pseudofermion set");
+    return DISPATCH(c, from_native, c, c->phi, phi, 12);
+}
+int lgt_hmc_trajectory(lgt_ctx* c, int nsteps, double dt, double tol, int max_iter, unsigned long long seed, unsigned trajectory,
+                       double* dH, int* accepted, long* cg_iters, double* H_initial) {
+    CHECK_CTX(c);
+    if (nsteps < 0) return fail(c, LGT_EINVAL, "lgt_hmc_trajectory: nsteps < 0");
+    int rc, it = 0, conv = LGT_OK;
+    long total = 0;
+    const bool ferm = c->kappa != 0.0;
+    if (!c->Usave) CU(cudaMalloc(&c->Usave, links_bytes(c)));
+    if ((rc = DISPATCH(c, momentum_heatbath, c, seed, trajectory)) != LGT_OK) return rc;
+    if (ferm && (rc = DISPATCH(c, pseudofermion_heatbath, c, seed, trajectory, c->scal + 4)) != LGT_OK) return rc;
+    CU(cudaMemcpyAsync(c->Usave, c->U, links_bytes(c), cudaMemcpyDeviceToDevice, c->stream));
+    if ((rc = DISPATCH(c, plaquette_sum, c, c->scal + 0)) != LGT_OK) return rc;
+    if ((rc = DISPATCH(c, kinetic, c, c->scal + 1)) != LGT_OK) return rc;
+    if ((rc = read_scalars(c, 5)) != LGT_OK) return rc;
+    // S_F at the start is |eta|^2 exactly (phi = D^dag eta), no solve needed
+    const double H0 = c->h_scal[1] + c->beta * (6.0 * (double)c->g.V - c->h_scal[0]) + (ferm ? c->h_scal[4] : 0.0);
+    rc = integrate(c, nsteps, dt, tol, max_iter, &total);
+    if (rc == LGT_ENOCONV) conv = rc; else if (rc != LGT_OK) return rc;
+    double sg, sf, k;
+    rc = hamiltonian(c, tol, max_iter, &sg, &sf, &k, &it);
+    if (rc == LGT_ENOCONV) conv = rc; else if (rc != LGT_OK) return rc;
+    total += it;
+    const double d = (k + sg + sf) - H0;
+    const bool acc = metropolis_uniform(seed, trajectory) < exp(-d);
+    if (!acc) {
+        CU(cudaMemcpyAsync(c->U, c->Usave, links_bytes(c), cudaMemcpyDeviceToDevice, c->stream));
+        c->u32_valid = false;
+        c->ucb_valid = false;
+    }
+    CU(cudaStreamSynchronize(c->stream));
+    if (dH) *dH = d;
+    if (accepted) *accepted = acc ? 1 : 0;
+    if (cg_iters) *cg_iters = total;
+    if (H_initial) *H_initial = H0;
     return conv;
 }
 

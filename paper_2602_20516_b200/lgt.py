@@ -15,6 +15,7 @@ LGT_OK, LGT_EINVAL, LGT_ENOMEM, LGT_ECUDA, LGT_ENOCONV, LGT_ESTATE = 0, -1, -2, 
 LGT_F64, LGT_F32 = 0, 1
 LGT_SOLVER_CG, LGT_SOLVER_MIXED_CG = 0, 1
 LGT_ACTION_FULL, LGT_ACTION_EO = 0, 1
+LGT_INT_LEAPFROG, LGT_INT_OMELYAN, LGT_INT_SEXTON_WEINGARTEN = 0, 1, 2
 
 # every symbol include/lgt.h declares: (restype, argtypes)
 _vp, _i, _d, _l = C.c_void_p, C.c_int, C.c_double, C.c_long
@@ -62,6 +63,11 @@ SYMBOLS = {
     "lgt_eo_mhat": (_i, [_vp, _vp, _vp, _i]),
     "lgt_eo_cg": (_i, [_vp, _vp, _vp, _d, _i, _ip, _dp]),
     "lgt_set_fermion_action": (_i, [_vp, _i]),
+    "lgt_set_integrator": (_i, [_vp, _i, _i]),
+    "lgt_momentum_heatbath": (_i, [_vp, C.c_ulonglong, C.c_uint]),
+    "lgt_pseudofermion_heatbath": (_i, [_vp, C.c_ulonglong, C.c_uint, _dp]),
+    "lgt_get_pseudofermion": (_i, [_vp, _vp]),
+    "lgt_hmc_trajectory": (_i, [_vp, _i, _d, _d, _i, C.c_ulonglong, C.c_uint, _dp, _ip, _lp, _dp]),
 }
 
 _lib = None
@@ -252,6 +258,33 @@ def lgt_md_trajectory(ctx, nsteps, dt, tol=1e-12, max_iter=100000, measure=True)
                                         C.byref(h0) if measure else None, C.byref(h1) if measure else None,
                                         C.byref(its)))
     return h0.value, h1.value, its.value
+
+
+def lgt_set_integrator(ctx, integrator, n_inner=1):
+    _check(ctx, lib().lgt_set_integrator(ctx, integrator, n_inner))
+
+
+def lgt_momentum_heatbath(ctx, seed, trajectory):
+    _check(ctx, lib().lgt_momentum_heatbath(ctx, seed, trajectory))
+
+
+def lgt_pseudofermion_heatbath(ctx, seed, trajectory):
+    """Returns |eta|^2 (= S_F at the start of the trajectory)."""
+    n2 = C.c_double()
+    _check(ctx, lib().lgt_pseudofermion_heatbath(ctx, seed, trajectory, C.byref(n2)))
+    return n2.value
+
+
+def lgt_get_pseudofermion(ctx, phi):
+    _check(ctx, lib().lgt_get_pseudofermion(ctx, _ptr(phi)))
+
+
+def lgt_hmc_trajectory(ctx, nsteps, dt, seed, trajectory, tol=1e-12, max_iter=100000):
+    """Returns (dH, accepted, cg_iters, H_initial, converged)."""
+    dH, acc, its, H0 = C.c_double(), C.c_int(), C.c_long(), C.c_double()
+    rc = _check(ctx, lib().lgt_hmc_trajectory(ctx, nsteps, dt, tol, max_iter, seed, trajectory, C.byref(dH), C.byref(acc),
+                                              C.byref(its), C.byref(H0)), allow=(LGT_ENOCONV,))
+    return dH.value, bool(acc.value), its.value, H0.value, rc == LGT_OK
 
 
 def lgt_native_spinor_bytes(ctx):

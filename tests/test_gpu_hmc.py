@@ -1,0 +1,168 @@
+"""GPU parity for the HMC layer: heat baths, integrators, Metropolis through the C ABI against
+oracle/hmc.py on the same (seed, trajectory).  Gaussians agree to libm rounding (both sides run the same
+counter-based generator in double), integrator end states to the base tolerance 1e-11.
+"""
+import numpy as np
+import pytest
+
+import oracle
+from oracle import evenodd as oeo
+from oracle import hmc as ohmc
+from paper_2602_20516_b200 import synth
+from lattice_util import link_rel_err
+
+pytestmark = pytest.mark.gpu
+
+BC = (1, 1, 1, -1)
+TOL64 = 1e-11
+
+
+@pytest.fixture(scope="module")
+def lgt():
+    import torch
+
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device; the product path has no CPU fallback")
+    from paper_2602_20516_b200 import lgt as m
+
+    m.lib()
+    return m
+
+
+@pytest.mark.parametrize("dims", [(4, 4, 4, 4), (4, 3, 5, 6), (8, 8, 8, 8)])
+def test_heatbaths_match_oracle(lgt, dims):
+    kappa, seed, traj = 0.11, 0x1234567890ABCDEF, 5
+    U = synth.warm_links(dims, 0.25, 77)
+    lat = lgt.Lattice(dims, 5.5, kappa, BC)
+    lat.set_links(U)
+    lgt.lgt_momentum_heatbath(lat.ctx, seed, traj)
+    P_ref, _ = ohmc.momentum_heatbath(dims, seed, traj)
+    P = lat.get_momenta()
+    assert np.abs(P - P_ref).max() < 2e-15 * max(1.0, np.abs(P_ref).max())
+    n2 = lgt.lgt_pseudofermion_heatbath(lat.ctx, seed, traj)
+    eta = ohmc.pseudofermion_noise(dims, seed, traj)
+    assert abs(n2 - np.sum(np.abs(eta) ** 2)) < 1e-13 * n2
+    phi = lat.empty(synth.volume(dims), 4, 3)
+    lgt.lgt_get_pseudofermion(lat.ctx, phi)
+    phi_ref = oracle.dslash(dims, kappa, BC, U, eta, dagger=True)
+    assert np.abs(phi.cpu().numpy() - phi_ref).max() < 1e-13
+    # other trajectory number: other field
+    lgt.lgt_momentum_heatbath(lat.ctx, seed, traj + 1)
+    assert np.abs(lat.get_momenta() - P_ref).max() > 0.1
+    lat.close()
+
+
+def test_heatbath_even_odd_and_fp32(lgt):
+    dims, kappa, seed, traj = (4, 4, 6, 8), 0.12, 99, 2
+    U = synth.warm_links(dims, 0.25, 78)
+    lat = lgt.Lattice(dims, 5.5, kappa, BC)
+    lat.set_links(U)
+    lgt.lgt_set_fermion_action(lat.ctx, lgt.LGT_ACTION_EO)
+    n2 = lgt.lgt_pseudofermion_heatbath(lat.ctx, seed, traj)
+    eta = ohmc.pseudofermion_noise(dims, seed, traj)
+    eta_e = oeo.keep(eta, dims, 0)
+    assert abs(n2 - np.sum(np.abs(eta_e) ** 2)) < 1e-13 * n2
+    phi = lat.empty(synth.volume(dims), 4, 3)
+    lgt.lgt_get_pseudofermion(lat.ctx, phi)
+    assert np.abs(phi.cpu().numpy() - oeo.mhat(dims, kappa, BC, U, eta_e, dagger=True)).max() < 1e-13
+    # S_F of the even/odd action at the start equals |eta_e|^2
+    _, S_F, _, _ = lgt.lgt_action(lat.ctx, 1e-13, 5000)
+    assert abs(S_F - n2) < 1e-10 * n2
+    lat.close()
+    lat32 = lgt.Lattice(dims, 5.5, kappa, BC, lgt.LGT_F32)
+    lgt.lgt_momentum_heatbath(lat32.ctx, seed, traj)
+    P_ref, _ = ohmc.momentum_heatbath(dims, seed, traj)
+    assert np.abs(lat32.get_momenta() - P_ref).max() < 1e-6
+    lat32.close()
+
+
+@pytest.mark.parametrize("integ,m", [("omelyan", 1), ("sw", 3), ("sw", 1)])
+def test_integrators_match_oracle(lgt, integ, m):
+    dims, beta, kappa = (4, 4, 4, 4), 5.5, 0.10
+    U0 = synth.warm_links(dims, 0.2, 1001)
+    P0 = synth.gaussian_momenta(dims, 5)
+    phi = oracle.dslash(dims, kappa, BC, U0, synth.gaussian_spinor(dims, 6), dagger=True)
+    lat = lgt.Lattice(dims, beta, kappa, BC)
+    lat.set_links(U0)
+    lat.set_momenta(P0)
+    lat.set_pseudofermion(phi)
+    code = lgt.LGT_INT_OMELYAN if integ == "omelyan" else lgt.LGT_INT_SEXTON_WEINGARTEN
+    ocode = ohmc.OMELYAN if integ == "omelyan" else ohmc.SEXTON_WEINGARTEN
+    lgt.lgt_set_integrator(lat.ctx, code, m)
+    H0, H1, its = lgt.lgt_md_trajectory(lat.ctx, 3, 0.04, tol=1e-13, max_iter=5000)
+    U_ref, P_ref, its_ref = ohmc.integrate(dims, beta, kappa, BC, U0, phi, P0, 3, 0.04, ocode, n_inner=m, tol=1e-13, max_iter=5000)
+    assert its == its_ref
+    assert np.abs(lat.get_links() - U_ref).max() < 1e-12
+    assert link_rel_err(lat.get_momenta(), P_ref)[0] < TOL64
+    dH_ref = (oracle.hamiltonian(dims, beta, kappa, BC, U_ref, phi, P_ref, 1e-13, 5000)[0]
+              - oracle.hamiltonian(dims, beta, kappa, BC, U0, phi, P0, 1e-13, 5000)[0])
+    assert abs((H1 - H0) - dH_ref) < 1e-9 * abs(H0)
+    # back to leapfrog: lgt_md_trajectory is the pinned oracle trajectory again
+    lgt.lgt_set_integrator(lat.ctx, lgt.LGT_INT_LEAPFROG)
+    lat.set_links(U0)
+    lat.set_momenta(P0)
+    lgt.lgt_md_trajectory(lat.ctx, 2, 0.04, tol=1e-13, max_iter=5000, measure=False)
+    U_lf, P_lf, _, _ = oracle.trajectory(dims, beta, kappa, BC, U0, phi, P0, 2, 0.04, tol=1e-13, max_iter=5000)
+    assert np.abs(lat.get_links() - U_lf).max() < 1e-12 and link_rel_err(lat.get_momenta(), P_lf)[0] < TOL64
+    with pytest.raises(lgt.LgtError):
+        lgt.lgt_set_integrator(lat.ctx, 7)
+    with pytest.raises(lgt.LgtError):
+        lgt.lgt_set_integrator(lat.ctx, lgt.LGT_INT_SEXTON_WEINGARTEN, 0)
+    lat.close()
+
+
+def test_hmc_trajectories_match_oracle(lgt):
+    """Three consecutive trajectories with fermions, and coarse gauge-only ones that get rejected: dH, the decision
+    (away from the threshold) and the links after the test agree with the oracle."""
+    dims, beta, kappa, seed = (4, 4, 4, 4), 5.5, 0.10, 20260220516
+    U = synth.warm_links(dims, 0.2, 1001)
+    lat = lgt.Lattice(dims, beta, kappa, BC)
+    lat.set_links(U)
+    lgt.lgt_set_integrator(lat.ctx, lgt.LGT_INT_OMELYAN)
+    for traj in range(3):
+        dH, acc, its, H0, ok = lgt.lgt_hmc_trajectory(lat.ctx, 4, 0.03, seed, traj, tol=1e-13, max_iter=5000)
+        ref = ohmc.hmc_trajectory(dims, beta, kappa, BC, U, seed, traj, 4, 0.03, ohmc.OMELYAN, tol=1e-13, max_iter=5000)
+        assert ok and abs(H0 - ref["H0"]) < 1e-12 * abs(ref["H0"])
+        assert abs(dH - ref["dH"]) < 1e-9 * abs(ref["H0"])
+        if abs(ref["u"] - np.exp(-ref["dH"])) > 1e-6:
+            assert acc == ref["accepted"]
+            assert np.abs(lat.get_links() - ref["U"]).max() < 1e-11
+        U = lat.get_links()
+    lat.close()
+    lat = lgt.Lattice(dims, beta, 0.0, BC)
+    U = synth.warm_links(dims, 0.2, 1001)
+    lat.set_links(U)
+    seen = set()
+    for traj in range(6):
+        dH, acc, _, _, _ = lgt.lgt_hmc_trajectory(lat.ctx, 1, 0.1, 7, traj)
+        ref = ohmc.hmc_trajectory(dims, beta, 0.0, BC, U, 7, traj, 1, 0.1)
+        assert abs(dH - ref["dH"]) < 1e-9 * abs(ref["H0"]) and acc == ref["accepted"]
+        assert np.abs(lat.get_links() - ref["U"]).max() < 1e-11
+        if not acc:
+            assert np.array_equal(lat.get_links(), U)  # restored bit for bit
+        seen.add(acc)
+        U = lat.get_links()
+    assert seen == {True, False}
+    with pytest.raises(lgt.LgtError):
+        lgt.lgt_pseudofermion_heatbath(lat.ctx, 1, 0)  # kappa == 0
+    lat.close()
+
+
+def test_hmc_even_odd_mixed_acceptance(lgt):
+    """8^4 with the even/odd action and the Sexton-Weingarten integrator: dH small, exp(-dH) averages to about 1 over a
+    few trajectories (Creutz identity, loose), plaquette stays a plaquette."""
+    dims, beta, kappa = (8, 8, 8, 8), 5.6, 0.12
+    lat = lgt.Lattice(dims, beta, kappa, BC)
+    lat.set_links(synth.warm_links(dims, 0.3, 11))
+    lgt.lgt_set_fermion_action(lat.ctx, lgt.LGT_ACTION_EO)
+    lgt.lgt_set_integrator(lat.ctx, lgt.LGT_INT_SEXTON_WEINGARTEN, 4)
+    dHs, accs = [], []
+    for traj in range(6):
+        dH, acc, its, H0, ok = lgt.lgt_hmc_trajectory(lat.ctx, 10, 0.02, 31337, traj, tol=1e-10, max_iter=5000)
+        assert ok and its > 0
+        dHs.append(dH)
+        accs.append(acc)
+    assert max(abs(d) for d in dHs) < 1.0 and sum(accs) >= 3
+    assert 0.3 < np.mean(np.exp(-np.array(dHs))) < 3.0
+    assert 0.3 < lgt.lgt_plaquette(lat.ctx) < 1.0
+    lat.close()
