@@ -181,6 +181,18 @@ int lgt_get_pseudofermion(lgt_ctx* ctx, void* phi);
 int lgt_hmc_trajectory(lgt_ctx* ctx, int nsteps, double dt, double tol, int max_iter, unsigned long long seed,
                        unsigned trajectory, double* dH, int* accepted, long* cg_iters, double* H_initial);
 
+/* ---- stout smearing of the fermions' links (rho = 0.3; ref. [6] PAPER.md:196) ---- */
+/* With n_levels > 0 the Dirac operator everywhere in the library (lgt_dslash*, lgt_cg*, lgt_eo_*, lgt_action's S_F,
+ * lgt_fermion_force, the heat bath, lgt_md_*, lgt_hmc_trajectory) is built on the smeared links U^(n):
+ *     U^(k+1)_mu(x) = exp(A) U^(k)_mu(x),   A = -rho P_su(3)[ U^(k)_mu(x) V^(k)_mu(x) ],  V = sum of the six staples
+ * (ref. [6]'s exp(iQ) U with Omega = C U^dag, C = rho V^dag), U^(0) = the handle's links; the gauge action stays on
+ * U^(0).  The fermion force is then the force with respect to U^(0): the force with respect to U^(n) pulled back level
+ * by level with the closed Cayley-Hamilton form of d exp.  lgt_fermion_force with given
+ * X, Y expects them to belong to D[U^(n)].  n_levels = 0 (default) switches smearing off; at most 8 levels.
+ * lgt_get_smeared_links: U^(n) in the canonical layout, [V][4][3][3], device pointer. */
+int lgt_set_smearing(lgt_ctx* ctx, int n_levels, double rho);
+int lgt_get_smeared_links(lgt_ctx* ctx, void* U);
+
 /* ---- native-layout spinor fields (for callers that keep fields resident between calls) ---- */
 /* Bytes of one spinor field in the handle's internal layout and precision. */
 long lgt_native_spinor_bytes(const lgt_ctx* ctx);

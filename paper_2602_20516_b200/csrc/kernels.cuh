@@ -581,8 +581,9 @@ template <class T> __device__ __forceinline__ void exp_iQ(const cx<T> Q[9], cx<T
     E[8] = E[8] + f0;
 }
 
+// Uout may be U itself (the MD drift) or another buffer (a stout level: Uout = exp(A) U).
 template <class T>
-__global__ void __launch_bounds__(128) link_update_kernel(Geom g, typename Vec2<T>::type* __restrict__ U,
+__global__ void __launch_bounds__(128) link_update_kernel(Geom g, const typename Vec2<T>::type* U, typename Vec2<T>::type* Uout,
                                                           const typename Vec2<T>::type* __restrict__ P, T eps) {
     const int s = blockIdx.x * W + (threadIdx.x & 31);
     if (s >= g.V) return;
@@ -608,12 +609,263 @@ __global__ void __launch_bounds__(128) link_update_kernel(Geom g, typename Vec2<
     Q[7] = conj(Q[5]);
     cx<T> E[9], u[9], r[9];
     exp_iQ(Q, E);
-    typename Vec2<T>::type* ub = link_at(U, s, mu);
+    const typename Vec2<T>::type* ub = link_at(U, s, mu);
+    typename Vec2<T>::type* uo = link_at(Uout, s, mu);
 #pragma unroll
     for (int k = 0; k < 9; k++) u[k] = ldc_rw<T>(ub + k * W);
     mul_nn(E, u, r);
 #pragma unroll
-    for (int k = 0; k < 9; k++) stc<T>(ub + k * W, r[k]);
+    for (int k = 0; k < 9; k++) stc<T>(uo + k * W, r[k]);
+}
+
+// ---------------------------------------------------------------------------- stout smearing
+// One level: U'_mu(x) = exp(A) U, A = -rho P_su(3)[U V] (gauge_force_kernel with scale -rho writes A in the compact form,
+// link_update_kernel applies it).  The force recursion of the paper's ref. [6] in our conventions
+// (DESIGN.md "Stout smearing"): with F' the force with respect to U', E = exp(A) = exp(iQ), Q = -iA,
+//   F = E^dag F' E  +  force of W[U] = 2 rho sum Re tr[U V G],   G = P_su(3)[-i Gamma],
+//   Gamma = tr(B1 M) Q + tr(B2 M) Q^2 + f1 M + f2 (Q M + M Q),   M = E^dag F',
+// from d exp(iQ) = tr(Q dQ) B1 + tr(Q^2 dQ) B2 + f1 dQ + f2 (dQ Q + Q dQ), B_i = b_i0 + b_i1 Q + b_i2 Q^2.
+
+// f_j and b_ij of exp(iQ) for traceless Hermitian Q (Q2 = Q^2); returns false when |Q| is so small that the closed
+// forms lose digits to cancellation (c1 = tr Q^2 / 2 < 5e-3) -- the caller then uses the commutator series.
+template <class T>
+__device__ __forceinline__ bool stout_coefficients(const cx<T> Q[9], const cx<T> Q2[9], cx<T> f[3], cx<T> b1[3], cx<T> b2[3]) {
+    cx<T> d0 = Q[4] * Q[8] - Q[5] * Q[7];
+    cx<T> d1 = Q[3] * Q[8] - Q[5] * Q[6];
+    cx<T> d2 = Q[3] * Q[7] - Q[4] * Q[6];
+    T c0 = (Q[0] * d0 - Q[1] * d1 + Q[2] * d2).re;
+    const T c1 = (T)0.5 * (Q2[0].re + Q2[4].re + Q2[8].re);
+    if (!(c1 > (T)5e-3)) return false;
+    const bool neg = c0 < 0;
+    c0 = fabs(c0);
+    const T c1_3 = c1 * (T)(1.0 / 3.0);
+    const T ratio = c0 / (2 * c1_3 * sqrt(c1_3));
+    const T theta = acos(ratio > 1 ? (T)1 : ratio);
+    T st, ct;
+    sincos(theta * (T)(1.0 / 3.0), &st, &ct);
+    const T u = sqrt(c1_3) * ct, w = sqrt(c1) * st;
+    const T u2 = u * u, w2 = w * w;
+    T sw, cw;
+    sincos(w, &sw, &cw);
+    T xi0, xi1;
+    if (fabs(w) < (T)0.05) {
+        xi0 = 1 - w2 * (T)(1.0 / 6.0) * (1 - w2 * (T)(1.0 / 20.0) * (1 - w2 * (T)(1.0 / 42.0)));
+        xi1 = -(T)(1.0 / 3.0) + w2 * (T)(1.0 / 30.0) * (1 - w2 * (T)(1.0 / 28.0) * (1 - w2 * (T)(1.0 / 54.0)));
+    } else {
+        xi0 = sw / w;
+        xi1 = (cw - xi0) / w2;
+    }
+    T s2u, c2u, s1u, c1u;
+    sincos(2 * u, &s2u, &c2u);
+    sincos(u, &s1u, &c1u);
+    const cx<T> e2 = mk<T>(c2u, s2u), em = mk<T>(c1u, -s1u);
+    const T den = 9 * u2 - w2, inv = 1 / den, inv2 = (T)0.5 * inv * inv;
+    f[0] = inv * ((u2 - w2) * e2 + em * mk<T>(8 * u2 * cw, 2 * u * (3 * u2 + w2) * xi0));
+    f[1] = inv * ((2 * u) * e2 - em * mk<T>(2 * u * cw, -(3 * u2 - w2) * xi0));
+    f[2] = inv * (e2 - em * mk<T>(cw, 3 * u * xi0));
+    cx<T> r1[3], r2[3];
+    // r1^(0) = 2 (u + i (u^2 - w^2)) e2 + 2 em { 4u (2 - iu) cw + i [9u^2 + w^2 - iu (3u^2 + w^2)] xi0 }
+    r1[0] = (T)2 * (mk<T>(u, u2 - w2) * e2) +
+            (T)2 * (em * mk<T>(8 * u * cw + u * (3 * u2 + w2) * xi0, -4 * u2 * cw + (9 * u2 + w2) * xi0));
+    // r1^(1) = 2 (1 + 2iu) e2 + em { -2 (1 - iu) cw + i [6u + i (w^2 - 3u^2)] xi0 }
+    r1[1] = (T)2 * (mk<T>(1, 2 * u) * e2) + em * mk<T>(-2 * cw - (w2 - 3 * u2) * xi0, 2 * u * cw + 6 * u * xi0);
+    // r1^(2) = 2i e2 + i em [cw - 3 (1 - iu) xi0]
+    r1[2] = times_i((T)2 * e2) + times_i(em * mk<T>(cw - 3 * xi0, 3 * u * xi0));
+    // r2^(0) = -2 e2 + 2iu em [cw + (1 + 4iu) xi0 + 3u^2 xi1]
+    r2[0] = (T)-2 * e2 + (2 * u) * times_i(em * mk<T>(cw + xi0 + 3 * u2 * xi1, 4 * u * xi0));
+    // r2^(1) = -i em [cw + (1 + 2iu) xi0 - 3u^2 xi1]
+    r2[1] = times_mi(em * mk<T>(cw + xi0 - 3 * u2 * xi1, 2 * u * xi0));
+    // r2^(2) = em [xi0 - 3iu xi1]
+    r2[2] = em * mk<T>(xi0, -3 * u * xi1);
+#pragma unroll
+    for (int j = 0; j < 3; j++) {
+        b1[j] = inv2 * ((2 * u) * r1[j] + (3 * u2 - w2) * r2[j] - (2 * (15 * u2 + w2)) * f[j]);
+        b2[j] = inv2 * (r1[j] - (3 * u) * r2[j] - (24 * u) * f[j]);
+    }
+    if (neg) {  // c0 -> -c0: f_j -> (-1)^j f_j^*, b_1j -> (-1)^j b_1j^*, b_2j -> (-1)^(j+1) b_2j^*
+        f[0] = conj(f[0]);
+        f[1] = mk<T>(-f[1].re, f[1].im);
+        f[2] = conj(f[2]);
+        b1[0] = conj(b1[0]);
+        b1[1] = mk<T>(-b1[1].re, b1[1].im);
+        b1[2] = conj(b1[2]);
+        b2[0] = mk<T>(-b2[0].re, b2[0].im);
+        b2[1] = conj(b2[1]);
+        b2[2] = mk<T>(-b2[2].re, b2[2].im);
+    }
+    return true;
+}
+
+template <class T> __device__ __forceinline__ cx<T> trace_prod(const cx<T> a[9], const cx<T> b[9]) {
+    cx<T> t = mk<T>(0, 0);
+#pragma unroll
+    for (int i = 0; i < 3; i++)
+#pragma unroll
+        for (int j = 0; j < 3; j++) cfma(t, a[3 * i + j], b[3 * j + i]);
+    return t;
+}
+template <class T> __device__ __forceinline__ void load_compact(const typename Vec2<T>::type* P, int s, int mu, T c[8]) {
+    const typename Vec2<T>::type* b = mom_at(P, s, mu);
+#pragma unroll
+    for (int q = 0; q < 4; q++) {
+        typename Vec2<T>::type v = __ldg(b + q * W);
+        c[2 * q] = v.x;
+        c[2 * q + 1] = v.y;
+    }
+}
+template <class T> __device__ __forceinline__ void store_compact(typename Vec2<T>::type* P, int s, int mu, const T c[8]) {
+    typename Vec2<T>::type* b = mom_at(P, s, mu);
+#pragma unroll
+    for (int q = 0; q < 4; q++) {
+        typename Vec2<T>::type v;
+        v.x = c[2 * q];
+        v.y = c[2 * q + 1];
+        b[q * W] = v;
+    }
+}
+
+// Per link, local: F' -> E^dag F' E (in place in Fio) and G (module comment above).  A, Fio, G in the compact form.
+template <class T>
+__global__ void __launch_bounds__(128) stout_local_kernel(Geom g, const typename Vec2<T>::type* __restrict__ A,
+                                                          typename Vec2<T>::type* __restrict__ Fio,
+                                                          typename Vec2<T>::type* __restrict__ G) {
+    const int s = blockIdx.x * W + (threadIdx.x & 31);
+    if (s >= g.V) return;
+    const int mu = threadIdx.x >> 5;
+    T ca[8], cf[8];
+    load_compact<T>(A, s, mu, ca);
+    load_compact<T>(Fio, s, mu, cf);
+    cx<T> Am[9], Fp[9], Q[9], Q2[9], E[9], M[9], t[9];
+    compact_expand(ca, Am);
+    compact_expand(cf, Fp);
+#pragma unroll
+    for (int k = 0; k < 9; k++) Q[k] = times_mi(Am[k]);
+    mul_nn(Q, Q, Q2);
+    exp_iQ(Q, E);
+    mul_dn(E, Fp, M);  // M = E^dag F'
+    mul_nn(M, E, t);   // E^dag F' E
+    T out[8];
+    ta_compact(t, (T)1, out);
+    store_compact<T>(Fio, s, mu, out);
+    cx<T> f[3], b1[3], b2[3], Gm[9];
+    if (stout_coefficients(Q, Q2, f, b1, b2)) {
+        const cx<T> trM = M[0] + M[4] + M[8], trQM = trace_prod(Q, M), trQ2M = trace_prod(Q2, M);
+        const cx<T> tB1 = b1[0] * trM + b1[1] * trQM + b1[2] * trQ2M;
+        const cx<T> tB2 = b2[0] * trM + b2[1] * trQM + b2[2] * trQ2M;
+        cx<T> QM[9], MQ[9];
+        mul_nn(Q, M, QM);
+        mul_nn(M, Q, MQ);
+#pragma unroll
+        for (int k = 0; k < 9; k++) Gm[k] = times_mi(tB1 * Q[k] + tB2 * Q2[k] + f[1] * M[k] + f[2] * (QM[k] + MQ[k]));
+    } else {
+        // G = sum_k (-ad_A)^k F' / (k+1)!: |A| < 0.1 here, 12 terms are below rounding
+        cx<T> term[9];
+#pragma unroll
+        for (int k = 0; k < 9; k++) Gm[k] = term[k] = Fp[k];
+        for (int n = 1; n < 12; n++) {
+            cx<T> a1[9], a2[9];
+            mul_nn(Am, term, a1);
+            mul_nn(term, Am, a2);
+            const T sc = (T)-1 / (T)(n + 1);
+#pragma unroll
+            for (int k = 0; k < 9; k++) {
+                term[k] = sc * (a1[k] - a2[k]);
+                Gm[k] = Gm[k] + term[k];
+            }
+        }
+    }
+    ta_compact(Gm, (T)1, out);
+    store_compact<T>(G, s, mu, out);
+}
+
+template <class T> __device__ __forceinline__ void load_su3_compact(const typename Vec2<T>::type* P, int s, int mu, cx<T> m[9]) {
+    T c[8];
+    load_compact<T>(P, s, mu, c);
+    compact_expand(c, m);
+}
+
+// Per link: F_mu(s) = Fdir_mu(s) - rho P_su(3)[X], X = the sum over the six plaquettes through the link of the
+// plaquette started at s with G inserted in front of each of its four links in turn (minus sign in front of a link
+// that the loop traverses backwards).  ACC: Pi -= eps F, else F written (compact).
+template <class T, int ACC>
+__global__ void __launch_bounds__(128) stout_chain_kernel(Geom g, const typename Vec2<T>::type* __restrict__ U,
+                                                          const typename Vec2<T>::type* __restrict__ G,
+                                                          const typename Vec2<T>::type* __restrict__ Fdir,
+                                                          typename Vec2<T>::type* __restrict__ out, T rho, T eps) {
+    const int s = blockIdx.x * W + (threadIdx.x & 31);
+    if (s >= g.V) return;
+    const int mu = threadIdx.x >> 5;
+    const Site c = site_coords(g, s);
+    const int smu = nbr_fwd(g, c, s, mu);
+    cx<T> X[9], Ua[9], Ga[9];
+    mat_zero(X);
+    load_link<T>(U, mu, s, Ua);
+    load_su3_compact<T>(G, s, mu, Ga);
+    for (int nu = 0; nu < 4; nu++) {
+        if (nu == mu) continue;
+        cx<T> a[9], b[9], t1[9], t2[9], t3[9], gi[9];
+        {   // up: a = (s,mu), b = (s+mu,nu), c = (s+nu,mu), d = (s,nu):  P = Ua Ub Uc^dag Ud^dag
+            const int snu = nbr_fwd(g, c, s, nu);
+            load_link<T>(U, nu, smu, a);   // Ub
+            load_link<T>(U, mu, snu, b);   // Uc
+            mul_nd(a, b, t1);              // Ub Uc^dag
+            load_link<T>(U, nu, s, b);     // Ud
+            mul_nd(t1, b, t2);             // S = Ub Uc^dag Ud^dag
+            load_su3_compact<T>(G, smu, nu, gi);  // Gb
+            mul_nn(gi, t2, t3);            // Gb S
+            load_su3_compact<T>(G, s, nu, gi);    // Gd
+#pragma unroll
+            for (int k = 0; k < 9; k++) gi[k] = Ga[k] - gi[k];
+            mul_nn(t2, gi, a);             // S (Ga - Gd)
+#pragma unroll
+            for (int k = 0; k < 9; k++) t3[k] = t3[k] + a[k];
+            load_su3_compact<T>(G, snu, mu, gi);  // Gc
+            mul_nn(t1, gi, a);             // Ub Uc^dag Gc
+            mul_nd(a, b, t2);              // Ub Uc^dag Gc Ud^dag
+#pragma unroll
+            for (int k = 0; k < 9; k++) t3[k] = t3[k] - t2[k];
+            mul_nn(Ua, t3, a);             // Ua [Gb S + S (Ga - Gd) - Ub Uc^dag Gc Ud^dag]
+#pragma unroll
+            for (int k = 0; k < 9; k++) X[k] = X[k] + a[k];
+        }
+        {   // down: b' = (s+mu-nu,nu), c' = (s-nu,mu), d' = (s-nu,nu):  P' = Ua Ub'^dag Uc'^dag Ud'
+            const int sdn = nbr_bwd(g, c, s, nu);
+            Site cm = c;
+            cm.x[mu] = (c.x[mu] == g.L[mu] - 1) ? 0 : c.x[mu] + 1;
+            const int smudn = nbr_bwd(g, cm, smu, nu);
+            load_link<T>(U, nu, smudn, a);  // Ub'
+            load_link<T>(U, mu, sdn, b);    // Uc'
+            mul_nn(b, a, t1);               // Uc' Ub'  ->  (Ub'^dag Uc'^dag) = t1^dag
+            load_link<T>(U, nu, sdn, b);    // Ud'
+            load_su3_compact<T>(G, sdn, mu, gi);   // Gc'
+            load_su3_compact<T>(G, sdn, nu, t2);   // Gd'
+#pragma unroll
+            for (int k = 0; k < 9; k++) gi[k] = t2[k] - gi[k];  // Gd' - Gc'
+            mul_nn(gi, b, t2);              // (Gd' - Gc') Ud'
+            mul_dn(t1, t2, t3);             // Ub'^dag Uc'^dag (Gd' - Gc') Ud'
+            mul_dn(t1, b, t2);              // Ub'^dag Uc'^dag Ud'   (so that P' = Ua t2)
+            mul_nn(t2, Ga, gi);             // ... Ga
+#pragma unroll
+            for (int k = 0; k < 9; k++) t3[k] = t3[k] + gi[k];
+            // - Ub'^dag Gb' Uc'^dag Ud'
+            load_su3_compact<T>(G, smudn, nu, gi);  // Gb'
+            load_link<T>(U, mu, sdn, t1);   // Uc' again (t1 is free now)
+            mul_dn(t1, b, t2);              // Uc'^dag Ud'
+            mul_nn(gi, t2, t1);             // Gb' Uc'^dag Ud'
+            mul_dn(a, t1, t2);              // Ub'^dag Gb' Uc'^dag Ud'
+#pragma unroll
+            for (int k = 0; k < 9; k++) t3[k] = t3[k] - t2[k];
+            mul_nn(Ua, t3, a);
+#pragma unroll
+            for (int k = 0; k < 9; k++) X[k] = X[k] + a[k];
+        }
+    }
+    T fw[8], fd[8];
+    ta_compact(X, -rho, fw);
+    load_compact<T>(Fdir, s, mu, fd);
+#pragma unroll
+    for (int k = 0; k < 8; k++) fw[k] += fd[k];
+    store_force<T, ACC>(out, s, mu, fw, eps);
 }
 
 // ---------------------------------------------------------------------------- A1: actions

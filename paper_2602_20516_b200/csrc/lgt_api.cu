@@ -18,6 +18,8 @@ namespace {
 std::string g_create_error;
 }
 
+constexpr int LGT_MAX_SMEAR = 8;
+
 struct lgt_ctx {
     Geom g;
     double beta, kappa;
@@ -40,6 +42,16 @@ struct lgt_ctx {
     bool ucb_valid = false;
     void* eo = nullptr;  // Xe, Xo, Ye, Yo, be, re, pe, to: 8 x 12 * Vhs complex
     int solver = LGT_SOLVER_CG;
+    // stout smearing of the links the fermions see (lazy): Usm[k] = level k+1 links, Asm[k] = its exponents (compact)
+    int nsmear = 0;
+    double rho = 0.0;
+    void* Usm[LGT_MAX_SMEAR] = {};
+    void* Asm[LGT_MAX_SMEAR] = {};
+    bool usm_valid = false;
+    void* Uf = nullptr;  // links of the Dirac operator: U, or Usm[nsmear - 1]
+    void* F2 = nullptr;  // three more compact force buffers for the smearing recursion (lazy)
+    void* F3 = nullptr;
+    void* F4 = nullptr;
     int integrator = LGT_INT_LEAPFROG;
     int n_inner = 1;        // gauge sub-steps per step of the Sexton-Weingarten integrator
     void* Usave = nullptr;  // links at the start of an HMC trajectory (lazy)
@@ -177,6 +189,7 @@ template <class T> struct Ops {
     }
     static int unit_links(lgt_ctx* c) {
         c->u32_valid = false;
+    c->usm_valid = false;
         c->ucb_valid = false;
         LAUNCH(c, LGT_K_OTHER, (unit_links_kernel<T>), stream_blocks(c, (size_t)36 * c->g.Vs), 256, c->g, (T2*)c->U);
         return LGT_OK;
@@ -239,12 +252,70 @@ template <class T> struct Ops {
         return LGT_OK;
     }
 
+    // ---- stout smearing: the Dirac operator sees c->Uf
+    // Brings c->Uf up to date: the thin links, or level nsmear of U^(k+1) = exp(A^(k+1)) U^(k), A = -rho P_su(3)[U V].
+    static int ensure_fermion_links(lgt_ctx* c) {
+        if (c->nsmear == 0) {
+            c->Uf = c->U;
+            return LGT_OK;
+        }
+        const int grid = c->g.Vs / 32;
+        for (int k = 0; k < c->nsmear; k++) {
+            if (!c->Usm[k]) CU(cudaMalloc(&c->Usm[k], links_bytes(c)));
+            if (!c->Asm[k]) {
+                CU(cudaMalloc(&c->Asm[k], mom_bytes(c)));
+                CU(cudaMemsetAsync(c->Asm[k], 0, mom_bytes(c), c->stream));
+            }
+        }
+        if (!c->usm_valid) {
+            const T2* Uin = (const T2*)c->U;
+            for (int k = 0; k < c->nsmear; k++) {
+                if (c->g.Vs != c->g.V) CU(cudaMemsetAsync(c->Usm[k], 0, links_bytes(c), c->stream));  // padding lanes
+                LAUNCH(c, LGT_K_GAUGE_FORCE, (gauge_force_kernel<T, 0>), grid, 128, c->g, Uin, (T2*)c->Asm[k], (T)(-c->rho), (T)0);
+                LAUNCH(c, LGT_K_LINK_UPDATE, (link_update_kernel<T>), grid, 128, c->g, Uin, (T2*)c->Usm[k], (const T2*)c->Asm[k], (T)1);
+                Uin = (const T2*)c->Usm[k];
+            }
+            c->usm_valid = true;
+        }
+        c->Uf = c->Usm[c->nsmear - 1];
+        return LGT_OK;
+    }
+
+    // F^f from X, Y: Pi -= eps F (acc) or F written to P (compact).  With smearing, the force with respect to the
+    // smeared links is pulled back level by level (stout_local_kernel, stout_chain_kernel) to the thin links.
     static int fermion_force(lgt_ctx* c, const void* X, const void* Y, void* P, int acc, double eps) {
+        int rc;
+        if ((rc = ensure_fermion_links(c)) != LGT_OK) return rc;
         const int grid = (c->g.Vs + 127) / 128;
-        if (acc)
-            LAUNCH(c, LGT_K_FERMION_FORCE, (fermion_force_kernel<T, 1>), grid, 128, c->g, (const T2*)c->U, (const T2*)X, (const T2*)Y, (T2*)P, (T)c->kappa, (T)eps);
-        else
-            LAUNCH(c, LGT_K_FERMION_FORCE, (fermion_force_kernel<T, 0>), grid, 128, c->g, (const T2*)c->U, (const T2*)X, (const T2*)Y, (T2*)P, (T)c->kappa, (T)eps);
+        if (c->nsmear == 0) {
+            if (acc)
+                LAUNCH(c, LGT_K_FERMION_FORCE, (fermion_force_kernel<T, 1>), grid, 128, c->g, (const T2*)c->Uf, (const T2*)X, (const T2*)Y, (T2*)P, (T)c->kappa, (T)eps);
+            else
+                LAUNCH(c, LGT_K_FERMION_FORCE, (fermion_force_kernel<T, 0>), grid, 128, c->g, (const T2*)c->Uf, (const T2*)X, (const T2*)Y, (T2*)P, (T)c->kappa, (T)eps);
+            return LGT_OK;
+        }
+        if (!c->F2) {
+            CU(cudaMalloc(&c->F2, mom_bytes(c)));
+            CU(cudaMalloc(&c->F3, mom_bytes(c)));
+            CU(cudaMalloc(&c->F4, mom_bytes(c)));
+            CU(cudaMemsetAsync(c->F2, 0, mom_bytes(c), c->stream));
+            CU(cudaMemsetAsync(c->F3, 0, mom_bytes(c), c->stream));
+            CU(cudaMemsetAsync(c->F4, 0, mom_bytes(c), c->stream));
+        }
+        const int lgrid = c->g.Vs / 32;
+        T2 *Fa = (T2*)c->F3, *Fb = (T2*)c->F4, *G = (T2*)c->F2;  // P is never one of these
+        LAUNCH(c, LGT_K_FERMION_FORCE, (fermion_force_kernel<T, 0>), grid, 128, c->g, (const T2*)c->Uf, (const T2*)X, (const T2*)Y, Fa, (T)c->kappa, (T)0);
+        for (int k = c->nsmear - 1; k >= 0; k--) {
+            const T2* Uk = (const T2*)(k == 0 ? c->U : c->Usm[k - 1]);
+            LAUNCH(c, LGT_K_FERMION_FORCE, (stout_local_kernel<T>), lgrid, 128, c->g, (const T2*)c->Asm[k], Fa, G);
+            if (k == 0 && acc)
+                LAUNCH(c, LGT_K_FERMION_FORCE, (stout_chain_kernel<T, 1>), lgrid, 128, c->g, Uk, (const T2*)G, (const T2*)Fa, (T2*)P, (T)c->rho, (T)eps);
+            else
+                LAUNCH(c, LGT_K_FERMION_FORCE, (stout_chain_kernel<T, 0>), lgrid, 128, c->g, Uk, (const T2*)G, (const T2*)Fa, (k == 0 ? (T2*)P : Fb), (T)c->rho, (T)0);
+            T2* t = Fa;
+            Fa = Fb;
+            Fb = t;
+        }
         return LGT_OK;
     }
     static int gauge_force(lgt_ctx* c, void* P, int acc, double eps) {
@@ -258,8 +329,9 @@ template <class T> struct Ops {
     static int link_update(lgt_ctx* c, double eps) {
         const int grid = c->g.Vs / 32;
         c->u32_valid = false;
+    c->usm_valid = false;
         c->ucb_valid = false;
-        LAUNCH(c, LGT_K_LINK_UPDATE, (link_update_kernel<T>), grid, 128, c->g, (T2*)c->U, (const T2*)c->P, (T)eps);
+        LAUNCH(c, LGT_K_LINK_UPDATE, (link_update_kernel<T>), grid, 128, c->g, (const T2*)c->U, (T2*)c->U, (const T2*)c->P, (T)eps);
         return LGT_OK;
     }
     static int plaquette_sum(lgt_ctx* c, double* dev_result) {
@@ -284,6 +356,7 @@ template <class T> struct Ops {
     // S_F at the start of the trajectory, |eta|^2 resp. |eta_e|^2, to dev_SF0.
     static int pseudofermion_heatbath(lgt_ctx* c, unsigned long long seed, unsigned traj, double* dev_SF0) {
         int rc;
+        if ((rc = ensure_fermion_links(c)) != LGT_OK) return rc;
         T2* eta = (T2*)c->ws[4];
         LAUNCH(c, LGT_K_OTHER, (spinor_heatbath_kernel<T>), stream_blocks(c, (size_t)12 * c->g.Vs), 256, c->g, eta, seed, traj);
         if (c->action == LGT_ACTION_EO) {
@@ -294,7 +367,7 @@ template <class T> struct Ops {
             if ((rc = eo_merge(c, eo_field(c, 2), c->phi)) != LGT_OK) return rc;
             if (dev_SF0 && (rc = redot(c, eo_field(c, 4), eo_field(c, 4), dev_SF0, (size_t)12 * c->g.Vhs)) != LGT_OK) return rc;
         } else {
-            if ((rc = dslash(c, c->U, eta, c->phi, 1, 0)) != LGT_OK) return rc;
+            if ((rc = dslash(c, c->Uf, eta, c->phi, 1, 0)) != LGT_OK) return rc;
             if (dev_SF0 && (rc = redot(c, eta, eta, dev_SF0, 0)) != LGT_OK) return rc;
         }
         c->has_phi = true;
@@ -305,6 +378,8 @@ template <class T> struct Ops {
     static T2* eo_field(lgt_ctx* c, int i) { return (T2*)c->eo + (size_t)i * 12 * c->g.Vhs; }
     static const T2* links_cb(lgt_ctx* c, int p) { return (const T2*)c->Ucb + (size_t)p * 36 * c->g.Vhs; }
     static int eo_ensure(lgt_ctx* c) {
+        int rcf = ensure_fermion_links(c);
+        if (rcf != LGT_OK) return rcf;
         if (!c->Ucb) {
             CU(cudaMalloc(&c->Ucb, (size_t)2 * 36 * c->g.Vhs * sizeof(T2)));
             c->ucb_valid = false;
@@ -315,7 +390,7 @@ template <class T> struct Ops {
         }
         if (!c->ucb_valid) {
             const size_t n = (size_t)2 * 36 * c->g.Vhs;
-            LAUNCH(c, LGT_K_OTHER, (eo_reorder_kernel<T, 0, 36>), stream_blocks(c, n), 256, c->g, (T2*)c->U, (T2*)c->Ucb);
+            LAUNCH(c, LGT_K_OTHER, (eo_reorder_kernel<T, 0, 36>), stream_blocks(c, n), 256, c->g, (T2*)c->Uf, (T2*)c->Ucb);
             c->ucb_valid = true;
         }
         return LGT_OK;
@@ -439,6 +514,8 @@ int cg_mixed(lgt_ctx* c, const void* b, void* x, void* y, double tol, int max_it
     if (c->prec != LGT_F64) return fail(c, LGT_ESTATE, "mixed-precision CG needs an LGT_F64 handle");
     typedef Ops<double> O64;
     typedef Ops<float> O32;
+    int rcf = O64::ensure_fermion_links(c);
+    if (rcf != LGT_OK) return rcf;
     const size_t n = (size_t)12 * c->g.Vs;
     if (!c->U32) {
         CU(cudaMalloc(&c->U32, (size_t)36 * c->g.Vs * sizeof(float2)));
@@ -448,7 +525,7 @@ int cg_mixed(lgt_ctx* c, const void* b, void* x, void* y, double tol, int max_it
     const int nb = stream_blocks(c, n);
     if (!c->u32_valid) {
         const size_t nu = (size_t)36 * c->g.Vs;
-        LAUNCH(c, LGT_K_OTHER, down_convert_kernel, stream_blocks(c, nu), 256, nu, (const double2*)c->U, (float2*)c->U32, 1.0);
+        LAUNCH(c, LGT_K_OTHER, down_convert_kernel, stream_blocks(c, nu), 256, nu, (const double2*)c->Uf, (float2*)c->U32, 1.0);
         c->u32_valid = true;
     }
     double2 *r = (double2*)c->ws[1], *q = (double2*)c->ws[2];
@@ -479,8 +556,8 @@ int cg_mixed(lgt_ctx* c, const void* b, void* x, void* y, double tol, int max_it
         total += it;
         outer++;
         LAUNCH(c, LGT_K_CG_BLAS, up_axpy_kernel, nb, 256, n, (double2*)x, (const float2*)e32, 1.0 / scale);
-        if ((rc = O64::dslash(c, c->U, x, t, 0, 0)) != LGT_OK) return rc;
-        if ((rc = O64::dslash(c, c->U, t, q, 1, 0)) != LGT_OK) return rc;
+        if ((rc = O64::dslash(c, c->Uf, x, t, 0, 0)) != LGT_OK) return rc;
+        if ((rc = O64::dslash(c, c->Uf, t, q, 1, 0)) != LGT_OK) return rc;
         LAUNCH(c, LGT_K_CG_BLAS, residual_kernel, nb, 256, n, (const double2*)b, (const double2*)q, r, c->scal + 3, c->partials, c->counter);
         CU(cudaMemcpyAsync(c->h_scal + 3, c->scal + 3, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
         CU(cudaStreamSynchronize(c->stream));
@@ -502,10 +579,11 @@ int solve(lgt_ctx* c, bool y, double tol, int max_iter, int* iters, double* dev_
     if (c->action == LGT_ACTION_EO)
         return DISPATCH(c, eo_solve_xy, c, y ? c->ws[0] : nullptr, y ? c->ws[3] : nullptr, tol, max_iter, iters, dev_SF);
     void* Y = y ? c->ws[3] : nullptr;
+    if ((rc = DISPATCH(c, ensure_fermion_links, c)) != LGT_OK) return rc;
     if (c->solver == LGT_SOLVER_MIXED_CG && c->prec == LGT_F64)
         conv = cg_mixed(c, c->phi, c->ws[0], Y, tol, max_iter, iters, nullptr);
     else
-        conv = DISPATCH(c, cg, c, c->U, c->ws[1], c->ws[2], c->ws[3], c->phi, c->ws[0], Y, tol, max_iter, iters, nullptr);
+        conv = DISPATCH(c, cg, c, c->Uf, c->ws[1], c->ws[2], c->ws[3], c->phi, c->ws[0], Y, tol, max_iter, iters, nullptr);
     if (conv != LGT_OK && conv != LGT_ENOCONV) return conv;
     if (dev_SF && (rc = DISPATCH(c, redot, c, c->phi, c->ws[0], dev_SF, 0)) != LGT_OK) return rc;
     return conv;
@@ -759,6 +837,13 @@ int lgt_destroy(lgt_ctx* c) {
     cudaFree(c->U32);
     cudaFree(c->Ucb);
     cudaFree(c->Usave);
+    for (int i = 0; i < LGT_MAX_SMEAR; i++) {
+        cudaFree(c->Usm[i]);
+        cudaFree(c->Asm[i]);
+    }
+    cudaFree(c->F2);
+    cudaFree(c->F3);
+    cudaFree(c->F4);
     cudaFree(c->eo);
     for (int i = 0; i < 5; i++) cudaFree(c->ws32[i]);
     cudaFree(c->stage);
@@ -826,6 +911,7 @@ int lgt_set_links(lgt_ctx* c, const void* U) {
     CHECK_CTX(c);
     if (!U) return fail(c, LGT_EINVAL, "lgt_set_links: null pointer");
     c->u32_valid = false;
+    c->usm_valid = false;
     c->ucb_valid = false;
     return DISPATCH(c, to_native, c, U, c->U, 36);
 }
@@ -913,14 +999,17 @@ int lgt_spinor_from_native(lgt_ctx* c, const void* native, void* canonical) {
 int lgt_dslash_native(lgt_ctx* c, const void* in, void* out, int dagger) {
     CHECK_CTX(c);
     if (!in || !out || in == out) return fail(c, LGT_EINVAL, "lgt_dslash_native: in and out must be distinct non-null buffers");
-    return DISPATCH(c, dslash, c, c->U, in, out, dagger ? 1 : 0, 0);
+    int rcf = DISPATCH(c, ensure_fermion_links, c);
+    if (rcf != LGT_OK) return rcf;
+    return DISPATCH(c, dslash, c, c->Uf, in, out, dagger ? 1 : 0, 0);
 }
 int lgt_dslash(lgt_ctx* c, const void* in, void* out, int dagger) {
     CHECK_CTX(c);
     if (!in || !out || in == out) return fail(c, LGT_EINVAL, "lgt_dslash: in and out must be distinct non-null buffers");
     int rc;
+    if ((rc = DISPATCH(c, ensure_fermion_links, c)) != LGT_OK) return rc;
     if ((rc = DISPATCH(c, to_native, c, in, c->ws[3], 12)) != LGT_OK) return rc;
-    if ((rc = DISPATCH(c, dslash, c, c->U, c->ws[3], c->ws[4], dagger ? 1 : 0, 0)) != LGT_OK) return rc;
+    if ((rc = DISPATCH(c, dslash, c, c->Uf, c->ws[3], c->ws[4], dagger ? 1 : 0, 0)) != LGT_OK) return rc;
     return DISPATCH(c, from_native, c, c->ws[4], out, 12);
 }
 
@@ -929,15 +1018,18 @@ int lgt_cg_native(lgt_ctx* c, const void* b, void* x, void* y, double tol, int m
     CHECK_CTX(c);
     if (!b || !x || b == x) return fail(c, LGT_EINVAL, "lgt_cg_native: bad pointers");
     if (!(tol >= 0.0) || max_iter < 0) return fail(c, LGT_EINVAL, "lgt_cg_native: bad tol / max_iter");
-    return DISPATCH(c, cg, c, c->U, c->ws[1], c->ws[2], c->ws[3], b, x, y, tol, max_iter, iters, rel_resid);
+    int rcf = DISPATCH(c, ensure_fermion_links, c);
+    if (rcf != LGT_OK) return rcf;
+    return DISPATCH(c, cg, c, c->Uf, c->ws[1], c->ws[2], c->ws[3], b, x, y, tol, max_iter, iters, rel_resid);
 }
 int lgt_cg(lgt_ctx* c, const void* b, void* x, double tol, int max_iter, int* iters, double* rel_resid) {
     CHECK_CTX(c);
     if (!b || !x) return fail(c, LGT_EINVAL, "lgt_cg: null pointer");
     if (!(tol >= 0.0) || max_iter < 0) return fail(c, LGT_EINVAL, "lgt_cg: bad tol / max_iter");
     int rc;
+    if ((rc = DISPATCH(c, ensure_fermion_links, c)) != LGT_OK) return rc;
     if ((rc = DISPATCH(c, to_native, c, b, c->ws[5], 12)) != LGT_OK) return rc;
-    int conv = DISPATCH(c, cg, c, c->U, c->ws[1], c->ws[2], c->ws[3], c->ws[5], c->ws[0], nullptr, tol, max_iter, iters, rel_resid);
+    int conv = DISPATCH(c, cg, c, c->Uf, c->ws[1], c->ws[2], c->ws[3], c->ws[5], c->ws[0], nullptr, tol, max_iter, iters, rel_resid);
     if (conv != LGT_OK && conv != LGT_ENOCONV) return conv;
     if ((rc = DISPATCH(c, from_native, c, c->ws[0], x, 12)) != LGT_OK) return rc;
     return conv;
@@ -1136,6 +1228,7 @@ int lgt_hmc_trajectory(lgt_ctx* c, int nsteps, double dt, double tol, int max_it
     if (!acc) {
         CU(cudaMemcpyAsync(c->U, c->Usave, links_bytes(c), cudaMemcpyDeviceToDevice, c->stream));
         c->u32_valid = false;
+    c->usm_valid = false;
         c->ucb_valid = false;
     }
     CU(cudaStreamSynchronize(c->stream));
@@ -1144,6 +1237,26 @@ int lgt_hmc_trajectory(lgt_ctx* c, int nsteps, double dt, double tol, int max_it
     if (cg_iters) *cg_iters = total;
     if (H_initial) *H_initial = H0;
     return conv;
+}
+
+// ---- stout smearing
+int lgt_set_smearing(lgt_ctx* c, int n_levels, double rho) {
+    CHECK_CTX(c);
+    if (n_levels < 0 || n_levels > LGT_MAX_SMEAR) return fail(c, LGT_EINVAL, "lgt_set_smearing: n_levels must be in 0..8");
+    if (n_levels > 0 && !(rho >= 0.0)) return fail(c, LGT_EINVAL, "lgt_set_smearing: rho must be >= 0");
+    c->nsmear = n_levels;
+    c->rho = n_levels ? rho : 0.0;
+    c->usm_valid = false;
+    c->u32_valid = false;
+    c->ucb_valid = false;
+    return LGT_OK;
+}
+int lgt_get_smeared_links(lgt_ctx* c, void* U) {
+    CHECK_CTX(c);
+    if (!U) return fail(c, LGT_EINVAL, "lgt_get_smeared_links: null pointer");
+    int rc = DISPATCH(c, ensure_fermion_links, c);
+    if (rc != LGT_OK) return rc;
+    return DISPATCH(c, from_native, c, c->Uf, U, 36);
 }
 
 }  // extern "C"

@@ -63,6 +63,8 @@ SYMBOLS = {
     "lgt_eo_mhat": (_i, [_vp, _vp, _vp, _i]),
     "lgt_eo_cg": (_i, [_vp, _vp, _vp, _d, _i, _ip, _dp]),
     "lgt_set_fermion_action": (_i, [_vp, _i]),
+    "lgt_set_smearing": (_i, [_vp, _i, _d]),
+    "lgt_get_smeared_links": (_i, [_vp, _vp]),
     "lgt_set_integrator": (_i, [_vp, _i, _i]),
     "lgt_momentum_heatbath": (_i, [_vp, C.c_ulonglong, C.c_uint]),
     "lgt_pseudofermion_heatbath": (_i, [_vp, C.c_ulonglong, C.c_uint, _dp]),
@@ -258,6 +260,14 @@ def lgt_md_trajectory(ctx, nsteps, dt, tol=1e-12, max_iter=100000, measure=True)
                                         C.byref(h0) if measure else None, C.byref(h1) if measure else None,
                                         C.byref(its)))
     return h0.value, h1.value, its.value
+
+
+def lgt_set_smearing(ctx, n_levels, rho=0.0):
+    _check(ctx, lib().lgt_set_smearing(ctx, n_levels, rho))
+
+
+def lgt_get_smeared_links(ctx, U):
+    _check(ctx, lib().lgt_get_smeared_links(ctx, _ptr(U)))
 
 
 def lgt_set_integrator(ctx, integrator, n_inner=1):
