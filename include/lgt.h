@@ -193,6 +193,41 @@ int lgt_hmc_trajectory(lgt_ctx* ctx, int nsteps, double dt, double tol, int max_
 int lgt_set_smearing(lgt_ctx* ctx, int n_levels, double rho);
 int lgt_get_smeared_links(lgt_ctx* ctx, void* U);
 
+/* ---- one lattice on several GPUs: time-slab decomposition -------------- */
+/* The lattice dims = {Lx,Ly,Lz,Lt} is cut into nranks slabs of Lt / nranks time slices (Lt % nranks == 0 and
+ * Lx*Ly*Lz % 32 == 0, else LGT_EINVAL).  A group object holds this process's ranks: in production ONE rank per
+ * process (nlocal = 1, local_ranks = {rank}) and the exchange steps of the path -- the halo slices of the stencil
+ * kernels' input field before every Dslash / force launch, the link halo after every link change, and the sums of
+ * CG and of the actions -- go through NCCL (send/recv of whole time slices, all-reduce of 1-3 doubles) on the group's
+ * stream after lgt_dd_nccl_init.  With nlocal = nranks every rank lives in this process on ONE device and the same
+ * exchanges are plain device copies: the verification mode used by the tests (no rank ever waits on another).
+ * Field arguments are per-rank SLABS in the canonical layout of the slab's own Lt / nranks time slices
+ * ([V/nranks][...], global site order restricted to the slab), given as arrays of nlocal device pointers.
+ * State goes in and out through the rank handles: lgt_dd_rank(d, i) returns a handle on which ONLY lgt_set_links,
+ * lgt_get_links, lgt_set_momenta, lgt_get_momenta, lgt_set_pseudofermion, lgt_get_pseudofermion (+ _host forms),
+ * lgt_timing_* and lgt_launch_count may be called (slab arrays); everything else on it returns LGT_ESTATE.
+ * Plain CG on the full operator and the leapfrog; the solver variants, smearing and heat baths are single-GPU only. */
+typedef struct lgt_dd lgt_dd;
+int lgt_dd_create(lgt_dd** out, const int dims[4], int nranks, int nlocal, const int* local_ranks, double beta, double kappa,
+                  const int bc[4], int precision, int device, void* cuda_stream);
+int lgt_dd_destroy(lgt_dd* d);
+const char* lgt_dd_last_error(const lgt_dd* d);
+/* NCCL transport: rank 0 obtains a 128-byte id (HOST buffer), the caller broadcasts it to all processes (e.g. through
+ * torch.distributed), every process calls lgt_dd_nccl_init on its one-rank group.  libnccl.so.2 is opened at run time. */
+int lgt_dd_nccl_unique_id(void* id128);
+int lgt_dd_nccl_init(lgt_dd* d, const void* id128);
+int lgt_dd_local_ranks(const lgt_dd* d);
+lgt_ctx* lgt_dd_rank(lgt_dd* d, int local_index);
+/* The decomposed forms of lgt_dslash, lgt_cg, lgt_action, lgt_md_kick, lgt_md_drift, lgt_md_trajectory (leapfrog):
+ * same mathematics, same kernels on each slab's interior, sums taken over all ranks; scalar outputs are global. */
+int lgt_dd_dslash(lgt_dd* d, const void* const* in, void* const* out, int dagger);
+int lgt_dd_cg(lgt_dd* d, const void* const* b, void* const* x, double tol, int max_iter, int* iters, double* rel_resid);
+int lgt_dd_action(lgt_dd* d, double tol, int max_iter, double* S_g, double* S_F, double* K, int* cg_iters);
+int lgt_dd_md_kick(lgt_dd* d, double eps, double tol, int max_iter, int* cg_iters);
+int lgt_dd_md_drift(lgt_dd* d, double eps);
+int lgt_dd_md_trajectory(lgt_dd* d, int nsteps, double dt, double tol, int max_iter, double* H_initial, double* H_final,
+                         long* cg_iters);
+
 /* ---- native-layout spinor fields (for callers that keep fields resident between calls) ---- */
 /* Bytes of one spinor field in the handle's internal layout and precision. */
 long lgt_native_spinor_bytes(const lgt_ctx* ctx);

@@ -31,6 +31,12 @@ struct Geom {
     int swz_cxy;    // 128-site chunks per xy plane
     int Vh;         // sites of one parity (V / 2; even/odd fields need every extent even)
     int Vhs;        // Vh padded to a multiple of 32
+    // Sites the compute kernels own: [s_begin, s_end).  The whole lattice, or, on a time-slab of a decomposed lattice
+    // (lgt_dd_*), the interior slices 1 .. Lt_local of a local lattice whose slices 0 and
+    // Lt_local + 1 are ghost copies of the neighbour ranks' boundary slices.  s_begin is a multiple of 32.
+    int s_begin, s_end;
+    int t_off;      // global t of local slice 0 (0, or rank * Lt_local - 1 on a slab)
+    int Lt_glob;    // global time extent (for the fermion boundary sign of the t links)
 };
 
 // lexicographic 128-site chunk handled by block b
@@ -56,6 +62,7 @@ struct CgState {
     int max_iter;
     int done;
     int pad;
+    double tmp;    // decomposed lattice: this rank's part of a sum, then (after the all-reduce) the global sum
 };
 
 struct Site {
@@ -220,6 +227,74 @@ __global__ void __launch_bounds__(1024) cg_scalars_kernel(int n, const double* _
     }
 }
 
+// Decomposed lattice (lgt_dd_*): the CG scalar updates in two phases around an all-reduce over the ranks.
+//   cg_partial_sum_kernel: st->tmp = this rank's sum of n block partials (fixed order, as cg_scalars_kernel)
+//   [all-reduce of st->tmp]
+//   cg_apply_kernel<WHAT>: WHAT 0 after cg_init (rr = bb = tmp, stop test), 1: pAp, alpha; 2: beta, rr, count, stop test
+__global__ void __launch_bounds__(1024) cg_partial_sum_kernel(int n, const double* __restrict__ partials, CgState* st) {
+    if (st->done) return;
+    __shared__ double warp_sums[32];
+    double a16[16];
+#pragma unroll
+    for (int j = 0; j < 16; j++) a16[j] = 0.0;
+    for (int base = threadIdx.x; base < n; base += 16 * 1024) {
+#pragma unroll
+        for (int j = 0; j < 16; j++) {
+            const int i = base + j * 1024;
+            if (i < n) a16[j] += __ldcg(partials + i);
+        }
+    }
+#pragma unroll
+    for (int w = 8; w > 0; w >>= 1)
+#pragma unroll
+        for (int j = 0; j < w; j++) a16[j] += a16[j + w];
+    double v = a16[0];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+    if (lane == 0) warp_sums[warp] = v;
+    __syncthreads();
+    if (warp == 0) {
+        double sum = warp_sums[lane];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) sum += __shfl_down_sync(0xffffffffu, sum, o);
+        if (lane == 0) st->tmp = sum;
+    }
+}
+template <int WHAT> __global__ void cg_apply_kernel(CgState* st) {
+    const double sum = st->tmp;
+    if (WHAT == 0) {
+        st->rr = sum;
+        st->bb = sum;
+        st->done = (!(sum > st->tol2 * sum) || st->max_iter <= 0) ? 1 : 0;
+    } else if (st->done) {
+        return;
+    } else if (WHAT == 1) {
+        st->pAp = sum;
+        st->alpha = st->rr / sum;
+    } else {
+        st->beta = sum / st->rr;
+        st->rr = sum;
+        st->iter += 1;
+        st->done = (!(sum > st->tol2 * st->bb) || st->iter >= st->max_iter) ? 1 : 0;
+    }
+}
+// st->tmp = st->rr (the local |b|^2 that cg_init_kernel left there)
+__global__ void cg_rr_to_tmp_kernel(CgState* st) { st->tmp = st->rr; }
+
+// All-reduce (sum) of `count` doubles among up to 8 ranks that live in this process: every p[i] receives the sum,
+// added in rank order (so all ranks hold the same bits, as after an NCCL all-reduce).
+struct DdPtrs {
+    double* p[8];
+};
+__global__ void dd_local_allreduce_kernel(DdPtrs ptrs, int nranks, int count) {
+    for (int k = threadIdx.x; k < count; k += blockDim.x) {
+        double sum = 0.0;
+        for (int r = 0; r < nranks; r++) sum += ptrs.p[r][k];
+        for (int r = 0; r < nranks; r++) ptrs.p[r][k] = sum;
+    }
+}
+
 // ---------------------------------------------------------------------------- A2: Wilson-Dirac operator
 // Forward hop of direction MU: acc += (1 + SG gamma_MU) U_MU(s) psi(s+MU)          (boundary sign is in U)
 template <int MU, int SG, class T>
@@ -261,9 +336,9 @@ __global__ void __launch_bounds__(128, 1) dslash_kernel(Geom g, const typename V
                                                         typename Vec2<T>::type* __restrict__ out, T kappa, CgState* st,
                                                         double* partials, typename Vec2<T>::type* __restrict__ r) {
     const int done = (MODE != 0) ? st->done : 0;
-    const int s = swizzled_chunk(g, blockIdx.x) * blockDim.x + threadIdx.x;
+    const int s = g.s_begin + swizzled_chunk(g, blockIdx.x) * blockDim.x + threadIdx.x;
     double nrm = 0.0;
-    if (s < g.V) {
+    if (s < g.s_end) {
         if (MODE == 2) {
             // r is only needed by the epilogue: pull its lines into L2 now, without holding registers, so that the
             // read-modify-write at the end does not expose a full DRAM latency
@@ -459,8 +534,8 @@ __global__ void __launch_bounds__(128, 1) fermion_force_kernel(Geom g, const typ
                                                                const typename Vec2<T>::type* __restrict__ X,
                                                                const typename Vec2<T>::type* __restrict__ Y,
                                                                typename Vec2<T>::type* __restrict__ P, T kappa, T eps) {
-    const int s = swizzled_chunk(g, blockIdx.x) * blockDim.x + threadIdx.x;
-    if (s >= g.V) return;
+    const int s = g.s_begin + swizzled_chunk(g, blockIdx.x) * blockDim.x + threadIdx.x;
+    if (s >= g.s_end) return;
     const Site c = site_coords(g, s);
     cx<T> Xs[12], Ys[12];
     load_spinor<T>(X, s, Xs);
@@ -480,8 +555,8 @@ __global__ void __launch_bounds__(128, 1) fermion_force_kernel(Geom g, const typ
 template <class T, int ACC>
 __global__ void __launch_bounds__(128, 2) gauge_force_kernel(Geom g, const typename Vec2<T>::type* __restrict__ U,
                                                           typename Vec2<T>::type* __restrict__ P, T beta_over_6, T eps) {
-    const int s = blockIdx.x * W + (threadIdx.x & 31);
-    if (s >= g.V) return;
+    const int s = g.s_begin + blockIdx.x * W + (threadIdx.x & 31);
+    if (s >= g.s_end) return;
     const int mu = threadIdx.x >> 5;
     const Site c = site_coords(g, s);
     const int smu = nbr_fwd(g, c, s, mu);
@@ -585,8 +660,8 @@ template <class T> __device__ __forceinline__ void exp_iQ(const cx<T> Q[9], cx<T
 template <class T>
 __global__ void __launch_bounds__(128) link_update_kernel(Geom g, const typename Vec2<T>::type* U, typename Vec2<T>::type* Uout,
                                                           const typename Vec2<T>::type* __restrict__ P, T eps) {
-    const int s = blockIdx.x * W + (threadIdx.x & 31);
-    if (s >= g.V) return;
+    const int s = g.s_begin + blockIdx.x * W + (threadIdx.x & 31);
+    if (s >= g.s_end) return;
     const int mu = threadIdx.x >> 5;
     T c[8];
     const typename Vec2<T>::type* pb = mom_at(P, s, mu);
@@ -729,8 +804,8 @@ template <class T>
 __global__ void __launch_bounds__(128) stout_local_kernel(Geom g, const typename Vec2<T>::type* __restrict__ A,
                                                           typename Vec2<T>::type* __restrict__ Fio,
                                                           typename Vec2<T>::type* __restrict__ G) {
-    const int s = blockIdx.x * W + (threadIdx.x & 31);
-    if (s >= g.V) return;
+    const int s = g.s_begin + blockIdx.x * W + (threadIdx.x & 31);
+    if (s >= g.s_end) return;
     const int mu = threadIdx.x >> 5;
     T ca[8], cf[8];
     load_compact<T>(A, s, mu, ca);
@@ -792,8 +867,8 @@ __global__ void __launch_bounds__(128) stout_chain_kernel(Geom g, const typename
                                                           const typename Vec2<T>::type* __restrict__ G,
                                                           const typename Vec2<T>::type* __restrict__ Fdir,
                                                           typename Vec2<T>::type* __restrict__ out, T rho, T eps) {
-    const int s = blockIdx.x * W + (threadIdx.x & 31);
-    if (s >= g.V) return;
+    const int s = g.s_begin + blockIdx.x * W + (threadIdx.x & 31);
+    if (s >= g.s_end) return;
     const int mu = threadIdx.x >> 5;
     const Site c = site_coords(g, s);
     const int smu = nbr_fwd(g, c, s, mu);
@@ -873,9 +948,9 @@ __global__ void __launch_bounds__(128) stout_chain_kernel(Geom g, const typename
 template <class T>
 __global__ void __launch_bounds__(128) plaquette_kernel(Geom g, const typename Vec2<T>::type* __restrict__ U, double* result,
                                                         double* partials, unsigned* counter) {
-    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    const int s = g.s_begin + blockIdx.x * blockDim.x + threadIdx.x;
     double acc = 0.0;
-    if (s < g.V) {
+    if (s < g.s_end) {
         const Site c = site_coords(g, s);
         for (int mu = 0; mu < 4; mu++) {
             const int smu = nbr_fwd(g, c, s, mu);
@@ -905,8 +980,9 @@ template <class T>
 __global__ void __launch_bounds__(256) kinetic_kernel(Geom g, const typename Vec2<T>::type* __restrict__ P, double* result,
                                                       double* partials, unsigned* counter) {
     double acc = 0.0;
-    const size_t nlinks = (size_t)4 * g.Vs;
-    for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < nlinks; i += (size_t)gridDim.x * blockDim.x) {
+    // owned links only; s_end is V (padding lanes hold zeros) or a multiple of 32
+    const size_t nlinks = (size_t)4 * (g.s_end == g.V ? g.Vs : g.s_end);
+    for (size_t i = (size_t)4 * g.s_begin + blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < nlinks; i += (size_t)gridDim.x * blockDim.x) {
         // i = (blk * 4 + mu) * 32 + lane
         const typename Vec2<T>::type* b = P + (i >> 5) * (4 * W) + (i & 31);
         typename Vec2<T>::type d = __ldg(b);
@@ -1197,6 +1273,7 @@ __global__ void __launch_bounds__(256) spinor_heatbath_kernel(Geom g, typename V
 __device__ __forceinline__ int link_sign(const Geom& g, int s, int mu) {
     if (g.bc[mu] > 0) return 1;
     int x = (s / g.stride[mu]) % g.L[mu];
+    if (mu == 3) return ((x + g.t_off + g.Lt_glob) % g.Lt_glob == g.Lt_glob - 1) ? -1 : 1;
     return (x == g.L[mu] - 1) ? -1 : 1;
 }
 
@@ -1212,22 +1289,23 @@ __global__ void __launch_bounds__(256) reorder_kernel(Geom g, const typename Vec
         const int k = (int)((i >> 5) % NCOMP);
         const int s = (int)((i >> 5) / NCOMP) * W + lane;
         T sg = 1;
-        if (LINKS && s < g.V) sg = (T)link_sign(g, s, k / 9);
+        const bool own = s >= g.s_begin && s < g.s_end;  // the canonical buffer holds the owned sites only
+        if (LINKS && own) sg = (T)link_sign(g, s, k / 9);
         if (DIR == 0) {
             typename Vec2<T>::type v;
             v.x = 0;
             v.y = 0;
-            if (s < g.V) {
-                v = __ldg(src + (size_t)s * NCOMP + k);
+            if (own) {
+                v = __ldg(src + (size_t)(s - g.s_begin) * NCOMP + k);
                 v.x *= sg;
                 v.y *= sg;
             }
             dst[i] = v;
-        } else if (s < g.V) {
+        } else if (own) {
             typename Vec2<T>::type v = __ldg(src + i);
             v.x *= sg;
             v.y *= sg;
-            dst[(size_t)s * NCOMP + k] = v;
+            dst[(size_t)(s - g.s_begin) * NCOMP + k] = v;
         }
     }
 }
@@ -1244,10 +1322,10 @@ __global__ void __launch_bounds__(256) momenta_reorder_kernel(Geom g, const type
         const int s = (int)(i >> 7) * W + lane;
         if (DIR == 0) {
             T c[8] = {0, 0, 0, 0, 0, 0, 0, 0};
-            if (s < g.V) {
+            if (s >= g.s_begin && s < g.s_end) {  // the canonical buffer holds the owned sites only
                 cx<T> m[9];
 #pragma unroll
-                for (int k = 0; k < 9; k++) m[k] = ldc<T>(src + ((size_t)s * 4 + mu) * 9 + k);
+                for (int k = 0; k < 9; k++) m[k] = ldc<T>(src + ((size_t)(s - g.s_begin) * 4 + mu) * 9 + k);
                 ta_compact(m, (T)1, c);
             }
             typename Vec2<T>::type* b = mom_at(dst, s, mu);
@@ -1258,7 +1336,7 @@ __global__ void __launch_bounds__(256) momenta_reorder_kernel(Geom g, const type
                 v.y = c[2 * q + 1];
                 b[q * W] = v;
             }
-        } else if (s < g.V) {
+        } else if (s >= g.s_begin && s < g.s_end) {
             T c[8];
             const typename Vec2<T>::type* b = mom_at(src, s, mu);
 #pragma unroll
@@ -1270,7 +1348,7 @@ __global__ void __launch_bounds__(256) momenta_reorder_kernel(Geom g, const type
             cx<T> m[9];
             compact_expand(c, m);
 #pragma unroll
-            for (int k = 0; k < 9; k++) stc<T>(dst + ((size_t)s * 4 + mu) * 9 + k, m[k]);
+            for (int k = 0; k < 9; k++) stc<T>(dst + ((size_t)(s - g.s_begin) * 4 + mu) * 9 + k, m[k]);
         }
     }
 }

@@ -52,6 +52,8 @@ struct lgt_ctx {
     void* F2 = nullptr;  // three more compact force buffers for the smearing recursion (lazy)
     void* F3 = nullptr;
     void* F4 = nullptr;
+    // a time slab of a decomposed lattice (lgt_dd_*): the group's "link ghosts are current" flag, cleared on link changes
+    bool* dd_links_valid = nullptr;
     int integrator = LGT_INT_LEAPFROG;
     int n_inner = 1;        // gauge sub-steps per step of the Sexton-Weingarten integrator
     void* Usave = nullptr;  // links at the start of an HMC trajectory (lazy)
@@ -139,7 +141,9 @@ struct DeviceGuard {
 inline size_t spinor_bytes(const lgt_ctx* c) { return (size_t)12 * c->g.Vs * c->esize; }
 inline size_t links_bytes(const lgt_ctx* c) { return (size_t)36 * c->g.Vs * c->esize; }
 inline size_t mom_bytes(const lgt_ctx* c) { return (size_t)16 * c->g.Vs * c->esize; }
-inline int site_blocks(const lgt_ctx* c, int bs) { return (c->g.V + bs - 1) / bs; }
+// sites the compute kernels own (Geom::s_begin .. s_end), padding lanes included on an undivided lattice
+inline int own_sites(const lgt_ctx* c) { return (c->g.s_end == c->g.V ? c->g.Vs : c->g.s_end) - c->g.s_begin; }
+inline int site_blocks(const lgt_ctx* c, int bs) { return (own_sites(c) + bs - 1) / bs; }
 inline int stream_blocks(const lgt_ctx* c, size_t n) {
     size_t b = (n + 255) / 256;
     return (int)(b < (size_t)c->red_blocks ? (b ? b : 1) : c->red_blocks);
@@ -190,6 +194,7 @@ template <class T> struct Ops {
     static int unit_links(lgt_ctx* c) {
         c->u32_valid = false;
     c->usm_valid = false;
+    if (c->dd_links_valid) *c->dd_links_valid = false;
         c->ucb_valid = false;
         LAUNCH(c, LGT_K_OTHER, (unit_links_kernel<T>), stream_blocks(c, (size_t)36 * c->g.Vs), 256, c->g, (T2*)c->U);
         return LGT_OK;
@@ -197,7 +202,7 @@ template <class T> struct Ops {
 
     // mode 0: out = D in / D^dag in; 1: CG "t = D p" (+ pAp, alpha); 2: CG "q = D^dag t" fused with the x, r update
     static int dslash(lgt_ctx* c, const void* U, const void* in, void* out, int dagger, int mode, void* r = nullptr) {
-        const int grid = (c->g.Vs + 127) / 128;
+        const int grid = site_blocks(c, 128);
         const T kappa = (T)c->kappa;
 #define DSLASH_ARGS c->g, (const T2*)U, (const T2*)in, (T2*)out, kappa, c->st, c->partials, (T2*)r
         if (mode == 0) {
@@ -223,7 +228,7 @@ template <class T> struct Ops {
         T2 *r = (T2*)wr, *p = (T2*)wp, *t = (T2*)wt;
         const size_t n = (size_t)12 * c->g.Vs;
         const int nb = stream_blocks(c, n);
-        const int ngrid = (c->g.Vs + 127) / 128;  // blocks (= partials) of the stencil kernels
+        const int ngrid = site_blocks(c, 128);  // blocks (= partials) of the stencil kernels
         LAUNCH(c, LGT_K_CG_BLAS, (cg_init_kernel<T>), nb, 256, n, (const T2*)b, (T2*)x, r, p, c->st, tol * tol, max_iter, c->partials, c->counter);
         int rc;
         int launched = 0;
@@ -259,7 +264,7 @@ template <class T> struct Ops {
             c->Uf = c->U;
             return LGT_OK;
         }
-        const int grid = c->g.Vs / 32;
+        const int grid = site_blocks(c, 32);
         for (int k = 0; k < c->nsmear; k++) {
             if (!c->Usm[k]) CU(cudaMalloc(&c->Usm[k], links_bytes(c)));
             if (!c->Asm[k]) {
@@ -286,7 +291,7 @@ template <class T> struct Ops {
     static int fermion_force(lgt_ctx* c, const void* X, const void* Y, void* P, int acc, double eps) {
         int rc;
         if ((rc = ensure_fermion_links(c)) != LGT_OK) return rc;
-        const int grid = (c->g.Vs + 127) / 128;
+        const int grid = site_blocks(c, 128);
         if (c->nsmear == 0) {
             if (acc)
                 LAUNCH(c, LGT_K_FERMION_FORCE, (fermion_force_kernel<T, 1>), grid, 128, c->g, (const T2*)c->Uf, (const T2*)X, (const T2*)Y, (T2*)P, (T)c->kappa, (T)eps);
@@ -302,7 +307,7 @@ template <class T> struct Ops {
             CU(cudaMemsetAsync(c->F3, 0, mom_bytes(c), c->stream));
             CU(cudaMemsetAsync(c->F4, 0, mom_bytes(c), c->stream));
         }
-        const int lgrid = c->g.Vs / 32;
+        const int lgrid = site_blocks(c, 32);
         T2 *Fa = (T2*)c->F3, *Fb = (T2*)c->F4, *G = (T2*)c->F2;  // P is never one of these
         LAUNCH(c, LGT_K_FERMION_FORCE, (fermion_force_kernel<T, 0>), grid, 128, c->g, (const T2*)c->Uf, (const T2*)X, (const T2*)Y, Fa, (T)c->kappa, (T)0);
         for (int k = c->nsmear - 1; k >= 0; k--) {
@@ -319,7 +324,7 @@ template <class T> struct Ops {
         return LGT_OK;
     }
     static int gauge_force(lgt_ctx* c, void* P, int acc, double eps) {
-        const int grid = c->g.Vs / 32;
+        const int grid = site_blocks(c, 32);
         if (acc)
             LAUNCH(c, LGT_K_GAUGE_FORCE, (gauge_force_kernel<T, 1>), grid, 128, c->g, (const T2*)c->U, (T2*)P, (T)(c->beta / 6.0), (T)eps);
         else
@@ -327,9 +332,10 @@ template <class T> struct Ops {
         return LGT_OK;
     }
     static int link_update(lgt_ctx* c, double eps) {
-        const int grid = c->g.Vs / 32;
+        const int grid = site_blocks(c, 32);
         c->u32_valid = false;
     c->usm_valid = false;
+    if (c->dd_links_valid) *c->dd_links_valid = false;
         c->ucb_valid = false;
         LAUNCH(c, LGT_K_LINK_UPDATE, (link_update_kernel<T>), grid, 128, c->g, (const T2*)c->U, (T2*)c->U, (const T2*)c->P, (T)eps);
         return LGT_OK;
@@ -733,6 +739,9 @@ template <class T> int eo_cg_canonical(lgt_ctx* c, const void* b, void* x, doubl
 #define CHECK_CTX(c) \
     if (!(c)) return LGT_EINVAL; \
     DeviceGuard guard_((c)->device)
+// calls that need neighbours or global sums are wrong on one time slab of a decomposed lattice: use lgt_dd_*
+#define NOT_SLAB(c) \
+    if ((c)->dd_links_valid) return fail((c), LGT_ESTATE, "this handle is a time slab of a decomposed lattice: use the lgt_dd_* call")
 
 extern "C" {
 
@@ -783,6 +792,10 @@ int lgt_create(lgt_ctx** out, const int dims[4], double beta, double kappa, cons
     c->g.Vhs = (c->g.Vh + 31) / 32 * 32;
     c->g.swz_cxy = (int)(((long long)dims[0] * dims[1]) / 128);
     c->g.swz_Z = auto_swizzle(c);
+    c->g.s_begin = 0;
+    c->g.s_end = c->g.V;
+    c->g.t_off = 0;
+    c->g.Lt_glob = c->g.L[3];
     int sms = 148;
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device);
     c->red_blocks = sms * 8;
@@ -891,6 +904,7 @@ int lgt_timing_read(lgt_ctx* c, int kernel_class, double* ms_total, long* launch
 long lgt_launch_count(const lgt_ctx* c) { return c ? c->launches : 0; }
 int lgt_set_block_swizzle(lgt_ctx* c, int z_planes, int* in_effect) {
     CHECK_CTX(c);
+    NOT_SLAB(c);
     if (z_planes < 0) {
         c->g.swz_Z = auto_swizzle(c);
     } else if (z_planes == 0) {
@@ -912,6 +926,7 @@ int lgt_set_links(lgt_ctx* c, const void* U) {
     if (!U) return fail(c, LGT_EINVAL, "lgt_set_links: null pointer");
     c->u32_valid = false;
     c->usm_valid = false;
+    if (c->dd_links_valid) *c->dd_links_valid = false;
     c->ucb_valid = false;
     return DISPATCH(c, to_native, c, U, c->U, 36);
 }
@@ -973,10 +988,12 @@ HOST_SET(lgt_set_pseudofermion_host, lgt_set_pseudofermion, (size_t)12 * c->g.V 
 // ---- actions
 int lgt_action(lgt_ctx* c, double tol, int max_iter, double* S_g, double* S_F, double* K, int* cg_iters) {
     CHECK_CTX(c);
+    NOT_SLAB(c);
     return hamiltonian(c, tol, max_iter, S_g, S_F, K, cg_iters);
 }
 int lgt_plaquette(lgt_ctx* c, double* plaq) {
     CHECK_CTX(c);
+    NOT_SLAB(c);
     if (!plaq) return fail(c, LGT_EINVAL, "lgt_plaquette: null pointer");
     int rc = DISPATCH(c, plaquette_sum, c, c->scal + 0);
     if (rc != LGT_OK) return rc;
@@ -998,6 +1015,7 @@ int lgt_spinor_from_native(lgt_ctx* c, const void* native, void* canonical) {
 }
 int lgt_dslash_native(lgt_ctx* c, const void* in, void* out, int dagger) {
     CHECK_CTX(c);
+    NOT_SLAB(c);
     if (!in || !out || in == out) return fail(c, LGT_EINVAL, "lgt_dslash_native: in and out must be distinct non-null buffers");
     int rcf = DISPATCH(c, ensure_fermion_links, c);
     if (rcf != LGT_OK) return rcf;
@@ -1005,6 +1023,7 @@ int lgt_dslash_native(lgt_ctx* c, const void* in, void* out, int dagger) {
 }
 int lgt_dslash(lgt_ctx* c, const void* in, void* out, int dagger) {
     CHECK_CTX(c);
+    NOT_SLAB(c);
     if (!in || !out || in == out) return fail(c, LGT_EINVAL, "lgt_dslash: in and out must be distinct non-null buffers");
     int rc;
     if ((rc = DISPATCH(c, ensure_fermion_links, c)) != LGT_OK) return rc;
@@ -1016,6 +1035,7 @@ int lgt_dslash(lgt_ctx* c, const void* in, void* out, int dagger) {
 // ---- solver
 int lgt_cg_native(lgt_ctx* c, const void* b, void* x, void* y, double tol, int max_iter, int* iters, double* rel_resid) {
     CHECK_CTX(c);
+    NOT_SLAB(c);
     if (!b || !x || b == x) return fail(c, LGT_EINVAL, "lgt_cg_native: bad pointers");
     if (!(tol >= 0.0) || max_iter < 0) return fail(c, LGT_EINVAL, "lgt_cg_native: bad tol / max_iter");
     int rcf = DISPATCH(c, ensure_fermion_links, c);
@@ -1024,6 +1044,7 @@ int lgt_cg_native(lgt_ctx* c, const void* b, void* x, void* y, double tol, int m
 }
 int lgt_cg(lgt_ctx* c, const void* b, void* x, double tol, int max_iter, int* iters, double* rel_resid) {
     CHECK_CTX(c);
+    NOT_SLAB(c);
     if (!b || !x) return fail(c, LGT_EINVAL, "lgt_cg: null pointer");
     if (!(tol >= 0.0) || max_iter < 0) return fail(c, LGT_EINVAL, "lgt_cg: bad tol / max_iter");
     int rc;
@@ -1037,6 +1058,7 @@ int lgt_cg(lgt_ctx* c, const void* b, void* x, double tol, int max_iter, int* it
 
 int lgt_set_fermion_action(lgt_ctx* c, int action) {
     CHECK_CTX(c);
+    NOT_SLAB(c);
     if (action != LGT_ACTION_FULL && action != LGT_ACTION_EO) return fail(c, LGT_EINVAL, "lgt_set_fermion_action: unknown action");
     if (action == LGT_ACTION_EO)
         for (int m = 0; m < 4; m++)
@@ -1046,6 +1068,7 @@ int lgt_set_fermion_action(lgt_ctx* c, int action) {
 }
 int lgt_eo_mhat(lgt_ctx* c, const void* in, void* out, int dagger) {
     CHECK_CTX(c);
+    NOT_SLAB(c);
     if (!in || !out || in == out) return fail(c, LGT_EINVAL, "lgt_eo_mhat: in and out must be distinct non-null buffers");
     int rc = eo_check(c, "lgt_eo_mhat: every extent must be even");
     if (rc != LGT_OK) return rc;
@@ -1053,6 +1076,7 @@ int lgt_eo_mhat(lgt_ctx* c, const void* in, void* out, int dagger) {
 }
 int lgt_eo_cg(lgt_ctx* c, const void* b, void* x, double tol, int max_iter, int* iters, double* rel_resid) {
     CHECK_CTX(c);
+    NOT_SLAB(c);
     if (!b || !x) return fail(c, LGT_EINVAL, "lgt_eo_cg: null pointer");
     if (!(tol >= 0.0) || max_iter < 0) return fail(c, LGT_EINVAL, "lgt_eo_cg: bad tol / max_iter");
     int rc = eo_check(c, "lgt_eo_cg: every extent must be even");
@@ -1063,6 +1087,7 @@ int lgt_eo_cg(lgt_ctx* c, const void* b, void* x, double tol, int max_iter, int*
 
 int lgt_set_solver(lgt_ctx* c, int solver, double inner_tol) {
     CHECK_CTX(c);
+    NOT_SLAB(c);
     if (solver != LGT_SOLVER_CG && solver != LGT_SOLVER_MIXED_CG) return fail(c, LGT_EINVAL, "lgt_set_solver: unknown solver");
     if (solver == LGT_SOLVER_MIXED_CG && c->prec != LGT_F64) return fail(c, LGT_EINVAL, "lgt_set_solver: mixed precision needs an LGT_F64 handle");
     if (solver == LGT_SOLVER_MIXED_CG && !(inner_tol > 0.0 && inner_tol < 1.0)) return fail(c, LGT_EINVAL, "lgt_set_solver: inner_tol must be in (0, 1)");
@@ -1073,6 +1098,7 @@ int lgt_set_solver(lgt_ctx* c, int solver, double inner_tol) {
 int lgt_cg_mixed(lgt_ctx* c, const void* b, void* x, double tol, int max_iter, double inner_tol, int* inner_iters, int* outer_cycles,
                  double* rel_resid) {
     CHECK_CTX(c);
+    NOT_SLAB(c);
     if (!b || !x) return fail(c, LGT_EINVAL, "lgt_cg_mixed: null pointer");
     if (!(tol >= 0.0) || max_iter < 0 || !(inner_tol > 0.0 && inner_tol < 1.0)) return fail(c, LGT_EINVAL, "lgt_cg_mixed: bad tol / max_iter / inner_tol");
     if (c->prec != LGT_F64) return fail(c, LGT_EINVAL, "lgt_cg_mixed: needs an LGT_F64 handle");
@@ -1091,6 +1117,7 @@ int lgt_cg_mixed(lgt_ctx* c, const void* b, void* x, double tol, int max_iter, d
 // ---- forces
 int lgt_gauge_force(lgt_ctx* c, void* F) {
     CHECK_CTX(c);
+    NOT_SLAB(c);
     if (!F) return fail(c, LGT_EINVAL, "lgt_gauge_force: null pointer");
     int rc;
     if ((rc = ensure_force_buf(c)) != LGT_OK) return rc;
@@ -1099,10 +1126,12 @@ int lgt_gauge_force(lgt_ctx* c, void* F) {
 }
 int lgt_gauge_force_accumulate(lgt_ctx* c, double eps) {
     CHECK_CTX(c);
+    NOT_SLAB(c);
     return DISPATCH(c, gauge_force, c, c->P, 1, eps);
 }
 int lgt_fermion_force(lgt_ctx* c, const void* X, const void* Y, void* F, double tol, int max_iter, int* cg_iters) {
     CHECK_CTX(c);
+    NOT_SLAB(c);
     if (!F) return fail(c, LGT_EINVAL, "lgt_fermion_force: null pointer");
     if ((X == nullptr) != (Y == nullptr)) return fail(c, LGT_EINVAL, "lgt_fermion_force: give both X and Y or neither");
     int rc, conv = LGT_OK, it = 0;
@@ -1122,6 +1151,7 @@ int lgt_fermion_force(lgt_ctx* c, const void* X, const void* Y, void* F, double 
 }
 int lgt_fermion_force_native(lgt_ctx* c, const void* X, const void* Y, double eps) {
     CHECK_CTX(c);
+    NOT_SLAB(c);
     if (!X || !Y) return fail(c, LGT_EINVAL, "lgt_fermion_force_native: null pointer");
     return DISPATCH(c, fermion_force, c, X, Y, c->P, 1, eps);
 }
@@ -1129,14 +1159,17 @@ int lgt_fermion_force_native(lgt_ctx* c, const void* X, const void* Y, double ep
 // ---- molecular dynamics
 int lgt_md_kick(lgt_ctx* c, double eps, double tol, int max_iter, int* cg_iters) {
     CHECK_CTX(c);
+    NOT_SLAB(c);
     return kick(c, eps, tol, max_iter, cg_iters);
 }
 int lgt_md_drift(lgt_ctx* c, double eps) {
     CHECK_CTX(c);
+    NOT_SLAB(c);
     return DISPATCH(c, link_update, c, eps);
 }
 int lgt_md_step(lgt_ctx* c, double dt, double tol, int max_iter, int* cg_iters) {
     CHECK_CTX(c);
+    NOT_SLAB(c);
     int rc, it1 = 0, it2 = 0, conv = LGT_OK;
     rc = kick(c, 0.5 * dt, tol, max_iter, &it1);
     if (rc == LGT_ENOCONV) conv = rc; else if (rc != LGT_OK) return rc;
@@ -1149,6 +1182,7 @@ int lgt_md_step(lgt_ctx* c, double dt, double tol, int max_iter, int* cg_iters) 
 int lgt_md_trajectory(lgt_ctx* c, int nsteps, double dt, double tol, int max_iter, double* H_initial, double* H_final,
                       long* cg_iters) {
     CHECK_CTX(c);
+    NOT_SLAB(c);
     if (nsteps < 0) return fail(c, LGT_EINVAL, "lgt_md_trajectory: nsteps < 0");
     int rc, it = 0, conv = LGT_OK;
     long total = 0;
@@ -1182,10 +1216,12 @@ int lgt_set_integrator(lgt_ctx* c, int integrator, int n_inner) {
 }
 int lgt_momentum_heatbath(lgt_ctx* c, unsigned long long seed, unsigned trajectory) {
     CHECK_CTX(c);
+    NOT_SLAB(c);
     return DISPATCH(c, momentum_heatbath, c, seed, trajectory);
 }
 int lgt_pseudofermion_heatbath(lgt_ctx* c, unsigned long long seed, unsigned trajectory, double* eta_norm2) {
     CHECK_CTX(c);
+    NOT_SLAB(c);
     if (c->kappa == 0.0) return fail(c, LGT_ESTATE, "lgt_pseudofermion_heatbath: kappa == 0, no fermions on this handle");
     int rc = DISPATCH(c, pseudofermion_heatbath, c, seed, trajectory, c->scal + 4);
     if (rc != LGT_OK) return rc;
@@ -1204,6 +1240,7 @@ int lgt_get_pseudofermion(lgt_ctx* c, void* phi) {
 int lgt_hmc_trajectory(lgt_ctx* c, int nsteps, double dt, double tol, int max_iter, unsigned long long seed, unsigned trajectory,
                        double* dH, int* accepted, long* cg_iters, double* H_initial) {
     CHECK_CTX(c);
+    NOT_SLAB(c);
     if (nsteps < 0) return fail(c, LGT_EINVAL, "lgt_hmc_trajectory: nsteps < 0");
     int rc, it = 0, conv = LGT_OK;
     long total = 0;
@@ -1229,6 +1266,7 @@ int lgt_hmc_trajectory(lgt_ctx* c, int nsteps, double dt, double tol, int max_it
         CU(cudaMemcpyAsync(c->U, c->Usave, links_bytes(c), cudaMemcpyDeviceToDevice, c->stream));
         c->u32_valid = false;
     c->usm_valid = false;
+    if (c->dd_links_valid) *c->dd_links_valid = false;
         c->ucb_valid = false;
     }
     CU(cudaStreamSynchronize(c->stream));
@@ -1242,17 +1280,20 @@ int lgt_hmc_trajectory(lgt_ctx* c, int nsteps, double dt, double tol, int max_it
 // ---- stout smearing
 int lgt_set_smearing(lgt_ctx* c, int n_levels, double rho) {
     CHECK_CTX(c);
+    NOT_SLAB(c);
     if (n_levels < 0 || n_levels > LGT_MAX_SMEAR) return fail(c, LGT_EINVAL, "lgt_set_smearing: n_levels must be in 0..8");
     if (n_levels > 0 && !(rho >= 0.0)) return fail(c, LGT_EINVAL, "lgt_set_smearing: rho must be >= 0");
     c->nsmear = n_levels;
     c->rho = n_levels ? rho : 0.0;
     c->usm_valid = false;
+    if (c->dd_links_valid) *c->dd_links_valid = false;
     c->u32_valid = false;
     c->ucb_valid = false;
     return LGT_OK;
 }
 int lgt_get_smeared_links(lgt_ctx* c, void* U) {
     CHECK_CTX(c);
+    NOT_SLAB(c);
     if (!U) return fail(c, LGT_EINVAL, "lgt_get_smeared_links: null pointer");
     int rc = DISPATCH(c, ensure_fermion_links, c);
     if (rc != LGT_OK) return rc;
@@ -1260,3 +1301,5 @@ int lgt_get_smeared_links(lgt_ctx* c, void* U) {
 }
 
 }  // extern "C"
+
+#include "lgt_dd.cuh"

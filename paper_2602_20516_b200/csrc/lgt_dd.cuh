@@ -1,0 +1,488 @@
+// lgt_dd.cuh -- the MD step on a lattice decomposed into time slabs, one slab per rank (include/lgt.h "lgt_dd_*",
+// SURVEY.md 8(e)).  Included by lgt_api.cu; uses its handle, launch macro and Ops<T>.
+//
+// A rank's slab is an ordinary handle on the local lattice (Lx, Ly, Lz, Lt_local + 2): slices 0 and Lt_local + 1
+// are ghost copies of the neighbour ranks' boundary slices, and Geom::s_begin / s_end restrict every compute kernel
+// to the interior.  Because t is the slowest index and Lx Ly Lz is a multiple of 32, a time slice of any native field
+// is one contiguous run, so a halo exchange is two sends and two receives per rank and field, with no packing kernel.
+// The same driver serves two transports: NCCL send/recv + all-reduce between processes (one rank per process), and
+// plain device copies between ranks that live in this process (the single-GPU verification mode: all ranks of the
+// group on one device and one stream, stepped in lockstep, nothing ever waits on another rank).
+#pragma once
+#include <dlfcn.h>
+
+namespace {
+
+// ---- NCCL through dlopen: no link-time dependency, and the process's already loaded libnccl.so.2 (torch's) is reused
+struct NcclApi {
+    typedef struct { char internal[128]; } UniqueId;
+    void* lib = nullptr;
+    int (*GetUniqueId)(UniqueId*) = nullptr;
+    int (*CommInitRank)(void**, int, UniqueId, int) = nullptr;
+    int (*CommDestroy)(void*) = nullptr;
+    int (*GroupStart)() = nullptr;
+    int (*GroupEnd)() = nullptr;
+    int (*Send)(const void*, size_t, int, int, void*, cudaStream_t) = nullptr;
+    int (*Recv)(void*, size_t, int, int, void*, cudaStream_t) = nullptr;
+    int (*AllReduce)(const void*, void*, size_t, int, int, void*, cudaStream_t) = nullptr;
+    const char* (*GetErrorString)(int) = nullptr;
+    bool load() {
+        if (lib) return true;
+        lib = dlopen("libnccl.so.2", RTLD_NOW | RTLD_GLOBAL);
+        if (!lib) lib = dlopen("libnccl.so", RTLD_NOW | RTLD_GLOBAL);
+        if (!lib) return false;
+#define NCCL_SYM(name) *(void**)(&name) = dlsym(lib, "nccl" #name)
+        NCCL_SYM(GetUniqueId);
+        NCCL_SYM(CommInitRank);
+        NCCL_SYM(CommDestroy);
+        NCCL_SYM(GroupStart);
+        NCCL_SYM(GroupEnd);
+        NCCL_SYM(Send);
+        NCCL_SYM(Recv);
+        NCCL_SYM(AllReduce);
+        NCCL_SYM(GetErrorString);
+#undef NCCL_SYM
+        return GetUniqueId && CommInitRank && CommDestroy && GroupStart && GroupEnd && Send && Recv && AllReduce;
+    }
+};
+NcclApi g_nccl;
+constexpr int NCCL_CHAR = 0, NCCL_DOUBLE = 8, NCCL_SUM = 0;  // ncclDataType_t / ncclRedOp_t values of nccl.h
+
+std::string g_dd_create_error;
+
+}  // namespace
+
+struct lgt_dd {
+    int nranks = 0;
+    std::vector<lgt_ctx*> rk;   // this process's ranks
+    std::vector<int> rank_of;   // their global rank numbers
+    int Lt_loc = 0;
+    int V3 = 0;
+    int prec = LGT_F64;
+    int device = 0;
+    cudaStream_t stream = nullptr;
+    bool links_ghost_valid = false;
+    void* comm = nullptr;  // ncclComm_t; null: every rank is local
+    std::string err;
+};
+
+namespace {
+
+int dd_fail(lgt_dd* d, int code, const char* what, const char* detail = nullptr) {
+    std::string m = what;
+    if (detail && *detail) m += std::string(": ") + detail;
+    if (d) d->err = m;
+    else g_dd_create_error = m;
+    return code;
+}
+#define DD_CU(call)                                                                        \
+    do {                                                                                   \
+        cudaError_t e_ = (call);                                                           \
+        if (e_ != cudaSuccess) return dd_fail(d, LGT_ECUDA, #call, cudaGetErrorString(e_)); \
+    } while (0)
+#define DD_NCCL(call)                                                                                              \
+    do {                                                                                                           \
+        int r_ = (call);                                                                                           \
+        if (r_ != 0) return dd_fail(d, LGT_ECUDA, #call, g_nccl.GetErrorString ? g_nccl.GetErrorString(r_) : ""); \
+    } while (0)
+// a failing rank-level call: carry its message up
+#define DD_RK(i, call)                                                     \
+    do {                                                                   \
+        int rc_ = (call);                                                  \
+        if (rc_ != LGT_OK) return dd_fail(d, rc_, d->rk[i]->err.c_str()); \
+    } while (0)
+
+int dd_local_index(const lgt_dd* d, int rank) {
+    for (size_t i = 0; i < d->rank_of.size(); i++)
+        if (d->rank_of[i] == rank) return (int)i;
+    return -1;
+}
+
+// Halo exchange of one native field per local rank: base[i] points to the field of local rank i, `per_site` = complex
+// (or pair) elements per site (12 spinor, 36 links, 16 compact momenta).  Rank r's first interior slice goes to the
+// upper ghost slice of rank r - 1, its last interior slice to the lower ghost slice of rank r + 1 (periodic in ranks).
+int dd_exchange(lgt_dd* d, void* const* base, int per_site) {
+    const size_t esize = d->prec == LGT_F64 ? 16 : 8;
+    const size_t slice = (size_t)d->V3 * per_site * esize;
+    const int n = (int)d->rk.size();
+    if (!d->comm) {
+        for (int i = 0; i < n; i++) {
+            const int r = d->rank_of[i];
+            const int dn = dd_local_index(d, (r + d->nranks - 1) % d->nranks), up = dd_local_index(d, (r + 1) % d->nranks);
+            char* mine = (char*)base[i];
+            DD_CU(cudaMemcpyAsync((char*)base[dn] + (size_t)(d->Lt_loc + 1) * slice, mine + slice, slice, cudaMemcpyDeviceToDevice, d->stream));
+            DD_CU(cudaMemcpyAsync((char*)base[up], mine + (size_t)d->Lt_loc * slice, slice, cudaMemcpyDeviceToDevice, d->stream));
+        }
+        return LGT_OK;
+    }
+    // one rank per process; sends and receives to the same peer pair up in the order they are issued
+    const int r = d->rank_of[0];
+    const int dn = (r + d->nranks - 1) % d->nranks, up = (r + 1) % d->nranks;
+    char* mine = (char*)base[0];
+    DD_NCCL(g_nccl.GroupStart());
+    DD_NCCL(g_nccl.Send(mine + slice, slice, NCCL_CHAR, dn, d->comm, d->stream));
+    DD_NCCL(g_nccl.Send(mine + (size_t)d->Lt_loc * slice, slice, NCCL_CHAR, up, d->comm, d->stream));
+    DD_NCCL(g_nccl.Recv(mine + (size_t)(d->Lt_loc + 1) * slice, slice, NCCL_CHAR, up, d->comm, d->stream));
+    DD_NCCL(g_nccl.Recv(mine, slice, NCCL_CHAR, dn, d->comm, d->stream));
+    DD_NCCL(g_nccl.GroupEnd());
+    return LGT_OK;
+}
+
+// Sum of `count` doubles over all ranks, in place at ptr[i] of every local rank (device memory).
+int dd_allreduce(lgt_dd* d, double* const* ptr, int count) {
+    if (!d->comm) {
+        DdPtrs p;
+        for (size_t i = 0; i < 8; i++) p.p[i] = i < d->rk.size() ? ptr[i] : nullptr;
+        dd_local_allreduce_kernel<<<1, 32, 0, d->stream>>>(p, (int)d->rk.size(), count);
+        DD_CU(cudaGetLastError());
+        return LGT_OK;
+    }
+    DD_NCCL(g_nccl.AllReduce(ptr[0], ptr[0], (size_t)count, NCCL_DOUBLE, NCCL_SUM, d->comm, d->stream));
+    return LGT_OK;
+}
+
+int dd_exchange_links(lgt_dd* d) {
+    if (d->links_ghost_valid) return LGT_OK;
+    std::vector<void*> u;
+    for (lgt_ctx* c : d->rk) u.push_back(c->U);
+    int rc = dd_exchange(d, u.data(), 36);
+    if (rc == LGT_OK) d->links_ghost_valid = true;
+    return rc;
+}
+
+}  // namespace
+
+namespace {
+
+// The driver: every step loops over the local ranks (one in production, all of them in the single-GPU verification
+// mode), then does the step's communication, so that both transports run the same sequence of launches.
+template <class T> struct DdOps {
+    typedef typename Vec2<T>::type T2;
+    typedef Ops<T> O;
+
+    static size_t spinor_off(const lgt_ctx* c) { return (size_t)12 * c->g.s_begin; }
+    static size_t spinor_n(const lgt_ctx* c) { return (size_t)12 * own_sites(c); }
+
+    static int exchange_spinor(lgt_dd* d, int ws_index_or_phi /* 0..5: ws[i], 6: phi */) {
+        std::vector<void*> f;
+        for (lgt_ctx* c : d->rk) f.push_back(ws_index_or_phi == 6 ? c->phi : c->ws[ws_index_or_phi]);
+        return dd_exchange(d, f.data(), 12);
+    }
+    static int allreduce_tmp(lgt_dd* d) {
+        std::vector<double*> p;
+        for (lgt_ctx* c : d->rk) p.push_back(&c->st->tmp);
+        return dd_allreduce(d, p.data(), 1);
+    }
+
+    // out = D in (or D^dag in) on the fields ws[in], ws[out] of every rank
+    static int dslash(lgt_dd* d, int in, int out, int dagger) {
+        int rc;
+        if ((rc = dd_exchange_links(d)) != LGT_OK) return rc;
+        if ((rc = exchange_spinor(d, in)) != LGT_OK) return rc;
+        for (size_t i = 0; i < d->rk.size(); i++) {
+            lgt_ctx* c = d->rk[i];
+            DD_RK(i, O::dslash(c, c->U, in == 6 ? c->phi : c->ws[in], c->ws[out], dagger, 0));
+        }
+        return LGT_OK;
+    }
+
+    // CG on D^dag D, b = ws[ib] (or phi for ib == 6), x = ws[0], workspaces r, p, t = ws[1..3]; leaves Y = D x in ws[3]
+    // if want_y.  Same recurrence, stop rule and fused kernels as Ops::cg; every sum is all-reduced over the ranks.
+    static int cg(lgt_dd* d, int ib, bool want_y, double tol, int max_iter, int* iters, double* rel) {
+        int rc;
+        if ((rc = dd_exchange_links(d)) != LGT_OK) return rc;
+        const int n = (int)d->rk.size();
+        for (int i = 0; i < n; i++) {
+            lgt_ctx* c = d->rk[i];
+            const size_t off = spinor_off(c), cnt = spinor_n(c);
+            const T2* b = (const T2*)(ib == 6 ? c->phi : c->ws[ib]) + off;
+            LAUNCH(c, LGT_K_CG_BLAS, (cg_init_kernel<T>), stream_blocks(c, cnt), 256, cnt, b, (T2*)c->ws[0] + off, (T2*)c->ws[1] + off,
+                   (T2*)c->ws[2] + off, c->st, tol * tol, max_iter, c->partials, c->counter);
+            LAUNCH(c, LGT_K_CG_BLAS, cg_rr_to_tmp_kernel, 1, 1, c->st);
+        }
+        if ((rc = allreduce_tmp(d)) != LGT_OK) return rc;
+        for (int i = 0; i < n; i++) LAUNCH(d->rk[i], LGT_K_CG_BLAS, (cg_apply_kernel<0>), 1, 1, d->rk[i]->st);
+        lgt_ctx* c0 = d->rk[0];
+        int launched = 0;
+        for (;;) {
+            DD_CU(cudaMemcpyAsync(c0->h_st, c0->st, sizeof(CgState), cudaMemcpyDeviceToHost, d->stream));
+            DD_CU(cudaStreamSynchronize(d->stream));
+            if (c0->h_st->done) break;
+            int chunk = max_iter - launched;
+            if (chunk > 8) chunk = 8;
+            if (chunk <= 0) chunk = 1;
+            for (int it = 0; it < chunk; it++) {
+                if ((rc = exchange_spinor(d, 2)) != LGT_OK) return rc;  // p
+                for (int i = 0; i < n; i++) {
+                    lgt_ctx* c = d->rk[i];
+                    DD_RK(i, O::dslash(c, c->U, c->ws[2], c->ws[3], 0, 1));  // t = D p, partials of |t|^2
+                    LAUNCH(c, LGT_K_CG_BLAS, cg_partial_sum_kernel, 1, 1024, site_blocks(c, 128), c->partials, c->st);
+                }
+                if ((rc = allreduce_tmp(d)) != LGT_OK) return rc;
+                for (int i = 0; i < n; i++) LAUNCH(d->rk[i], LGT_K_CG_BLAS, (cg_apply_kernel<1>), 1, 1, d->rk[i]->st);
+                if ((rc = exchange_spinor(d, 3)) != LGT_OK) return rc;  // t
+                for (int i = 0; i < n; i++) {
+                    lgt_ctx* c = d->rk[i];
+                    DD_RK(i, O::dslash(c, c->U, c->ws[3], nullptr, 1, 2, c->ws[1]));  // r -= alpha D^dag t, partials of |r|^2
+                    LAUNCH(c, LGT_K_CG_BLAS, cg_partial_sum_kernel, 1, 1024, site_blocks(c, 128), c->partials, c->st);
+                }
+                if ((rc = allreduce_tmp(d)) != LGT_OK) return rc;
+                for (int i = 0; i < n; i++) {
+                    lgt_ctx* c = d->rk[i];
+                    const size_t off = spinor_off(c), cnt = spinor_n(c);
+                    LAUNCH(c, LGT_K_CG_BLAS, (cg_apply_kernel<2>), 1, 1, c->st);
+                    LAUNCH(c, LGT_K_CG_BLAS, (cg_update_xp_kernel<T>), stream_blocks(c, cnt), 256, cnt, (T2*)c->ws[0] + off, (T2*)c->ws[2] + off,
+                           (const T2*)c->ws[1] + off, c->st, launched + it + 1);
+                }
+            }
+            launched += chunk;
+        }
+        const CgState& h = *c0->h_st;
+        if (iters) *iters = h.iter;
+        if (rel) *rel = (h.bb > 0.0) ? sqrt(h.rr / h.bb) : 0.0;
+        if (want_y && (rc = dslash(d, 0, 3, 0)) != LGT_OK) return rc;
+        if (h.rr > h.tol2 * h.bb) return dd_fail(d, LGT_ENOCONV, "CG did not reach the tolerance within max_iter");
+        return LGT_OK;
+    }
+
+    // Pi -= eps (F^g + F^f) on every rank
+    static int kick(lgt_dd* d, double eps, double tol, int max_iter, int* cg_iters) {
+        int rc, it = 0, conv = LGT_OK;
+        if ((rc = dd_exchange_links(d)) != LGT_OK) return rc;
+        for (size_t i = 0; i < d->rk.size(); i++) DD_RK(i, O::gauge_force(d->rk[i], d->rk[i]->P, 1, eps));
+        if (fermions_on(d->rk[0])) {
+            rc = cg(d, 6, true, tol, max_iter, &it, nullptr);
+            if (rc == LGT_ENOCONV) conv = rc;
+            else if (rc != LGT_OK) return rc;
+            if ((rc = exchange_spinor(d, 0)) != LGT_OK) return rc;  // X(x + mu)
+            if ((rc = exchange_spinor(d, 3)) != LGT_OK) return rc;  // Y(x + mu)
+            for (size_t i = 0; i < d->rk.size(); i++) {
+                lgt_ctx* c = d->rk[i];
+                c->Uf = c->U;
+                DD_RK(i, O::fermion_force(c, c->ws[0], c->ws[3], c->P, 1, eps));
+            }
+        }
+        if (cg_iters) *cg_iters = it;
+        return conv;
+    }
+
+    static int drift(lgt_dd* d, double eps) {
+        for (size_t i = 0; i < d->rk.size(); i++) DD_RK(i, O::link_update(d->rk[i], eps));
+        d->links_ghost_valid = false;
+        return dd_exchange_links(d);
+    }
+
+    // S_g, S_F, K summed over the ranks (device slots scal[0..2] of every rank, one all-reduce of three doubles)
+    static int action(lgt_dd* d, double tol, int max_iter, double* S_g, double* S_F, double* K, int* cg_iters) {
+        int rc, it = 0, conv = LGT_OK;
+        if ((rc = dd_exchange_links(d)) != LGT_OK) return rc;
+        const bool ferm = fermions_on(d->rk[0]) && S_F != nullptr;
+        if (ferm) {
+            rc = cg(d, 6, false, tol, max_iter, &it, nullptr);
+            if (rc == LGT_ENOCONV) conv = rc;
+            else if (rc != LGT_OK) return rc;
+        }
+        std::vector<double*> slots;
+        for (size_t i = 0; i < d->rk.size(); i++) {
+            lgt_ctx* c = d->rk[i];
+            DD_RK(i, O::plaquette_sum(c, c->scal + 0));
+            DD_RK(i, O::kinetic(c, c->scal + 1));
+            if (ferm) {
+                const size_t off = spinor_off(c);
+                LAUNCH(c, LGT_K_OTHER, (redot_kernel<T>), stream_blocks(c, spinor_n(c)), 256, spinor_n(c), (const T2*)c->phi + off,
+                       (const T2*)c->ws[0] + off, c->scal + 2, c->partials, c->counter);
+            } else {
+                DD_CU(cudaMemsetAsync(c->scal + 2, 0, sizeof(double), d->stream));
+            }
+            slots.push_back(c->scal);
+        }
+        if ((rc = dd_allreduce(d, slots.data(), 3)) != LGT_OK) return rc;
+        lgt_ctx* c0 = d->rk[0];
+        DD_CU(cudaMemcpyAsync(c0->h_scal, c0->scal, 3 * sizeof(double), cudaMemcpyDeviceToHost, d->stream));
+        DD_CU(cudaStreamSynchronize(d->stream));
+        const double sites = (double)d->V3 * d->Lt_loc * d->nranks;
+        if (S_g) *S_g = c0->beta * (6.0 * sites - c0->h_scal[0]);
+        if (K) *K = c0->h_scal[1];
+        if (S_F) *S_F = ferm ? c0->h_scal[2] : 0.0;
+        if (cg_iters) *cg_iters = it;
+        return conv;
+    }
+};
+
+#define DD_DISPATCH(d, fn, ...) ((d)->prec == LGT_F64 ? DdOps<double>::fn(__VA_ARGS__) : DdOps<float>::fn(__VA_ARGS__))
+
+}  // namespace
+
+#define CHECK_DD(d)               \
+    if (!(d)) return LGT_EINVAL;  \
+    DeviceGuard guard_((d)->device)
+
+extern "C" {
+
+const char* lgt_dd_last_error(const lgt_dd* d) { return d ? d->err.c_str() : g_dd_create_error.c_str(); }
+
+int lgt_dd_destroy(lgt_dd* d) {
+    if (!d) return LGT_OK;
+    DeviceGuard guard(d->device);
+    cudaStreamSynchronize(d->stream);
+    if (d->comm && g_nccl.CommDestroy) g_nccl.CommDestroy(d->comm);
+    for (lgt_ctx* c : d->rk) lgt_destroy(c);
+    delete d;
+    return LGT_OK;
+}
+
+int lgt_dd_create(lgt_dd** out, const int dims[4], int nranks, int nlocal, const int* local_ranks, double beta, double kappa,
+                  const int bc[4], int precision, int device, void* cuda_stream) {
+    lgt_dd* d = nullptr;
+    if (!out || !dims || !bc || !local_ranks) return dd_fail(nullptr, LGT_EINVAL, "lgt_dd_create: null argument");
+    *out = nullptr;
+    if (nranks < 1 || nlocal < 1 || nlocal > nranks || nlocal > 8) return dd_fail(nullptr, LGT_EINVAL, "lgt_dd_create: need 1 <= nlocal <= min(nranks, 8)");
+    if (nlocal != nranks && nlocal != 1) return dd_fail(nullptr, LGT_EINVAL, "lgt_dd_create: either every rank is local or exactly one is");
+    for (int m = 0; m < 4; m++)
+        if (dims[m] < 1) return dd_fail(nullptr, LGT_EINVAL, "lgt_dd_create: dims must be >= 1");
+    if (dims[3] % nranks != 0) return dd_fail(nullptr, LGT_EINVAL, "lgt_dd_create: Lt must be a multiple of the number of ranks");
+    const long long V3 = (long long)dims[0] * dims[1] * dims[2];
+    if (V3 % 32 != 0) return dd_fail(nullptr, LGT_EINVAL, "lgt_dd_create: Lx*Ly*Lz must be a multiple of 32 (a time slice is then one contiguous run)");
+    for (int i = 0; i < nlocal; i++) {
+        if (local_ranks[i] < 0 || local_ranks[i] >= nranks) return dd_fail(nullptr, LGT_EINVAL, "lgt_dd_create: bad local rank number");
+        for (int j = 0; j < i; j++)
+            if (local_ranks[j] == local_ranks[i]) return dd_fail(nullptr, LGT_EINVAL, "lgt_dd_create: duplicate local rank number");
+    }
+    d = new lgt_dd();
+    d->nranks = nranks;
+    d->Lt_loc = dims[3] / nranks;
+    d->V3 = (int)V3;
+    d->prec = precision;
+    d->device = device;
+    d->stream = (cudaStream_t)cuda_stream;
+    const int ldims[4] = {dims[0], dims[1], dims[2], d->Lt_loc + 2};
+    for (int i = 0; i < nlocal; i++) {
+        lgt_ctx* c = nullptr;
+        int rc = lgt_create(&c, ldims, beta, kappa, bc, precision, device, cuda_stream);
+        if (rc != LGT_OK) {
+            g_dd_create_error = std::string("lgt_dd_create: ") + lgt_last_error(nullptr);
+            lgt_dd_destroy(d);
+            return rc;
+        }
+        c->g.s_begin = d->V3;
+        c->g.s_end = c->g.V - d->V3;
+        c->g.t_off = local_ranks[i] * d->Lt_loc - 1;
+        c->g.Lt_glob = dims[3];
+        c->g.swz_Z = 0;
+        c->dd_links_valid = &d->links_ghost_valid;
+        d->rk.push_back(c);
+        d->rank_of.push_back(local_ranks[i]);
+        // the unit field again, now with the boundary sign at the right global time slice
+        rc = precision == LGT_F64 ? Ops<double>::unit_links(c) : Ops<float>::unit_links(c);
+        if (rc != LGT_OK) {
+            g_dd_create_error = "lgt_dd_create: " + c->err;
+            lgt_dd_destroy(d);
+            return rc;
+        }
+    }
+    d->links_ghost_valid = true;  // the unit field fills the ghost slices too
+    *out = d;
+    return LGT_OK;
+}
+
+int lgt_dd_nccl_unique_id(void* id128) {
+    if (!id128) return LGT_EINVAL;
+    if (!g_nccl.load()) return dd_fail(nullptr, LGT_ECUDA, "lgt_dd_nccl_unique_id: libnccl.so.2 not found");
+    NcclApi::UniqueId id;
+    if (g_nccl.GetUniqueId(&id) != 0) return dd_fail(nullptr, LGT_ECUDA, "ncclGetUniqueId failed");
+    memcpy(id128, &id, sizeof id);
+    return LGT_OK;
+}
+int lgt_dd_nccl_init(lgt_dd* d, const void* id128) {
+    CHECK_DD(d);
+    if (!id128) return dd_fail(d, LGT_EINVAL, "lgt_dd_nccl_init: null id");
+    if (d->rk.size() != 1) return dd_fail(d, LGT_ESTATE, "lgt_dd_nccl_init: the NCCL transport serves one rank per process");
+    if (d->comm) return dd_fail(d, LGT_ESTATE, "lgt_dd_nccl_init: already initialised");
+    if (!g_nccl.load()) return dd_fail(d, LGT_ECUDA, "lgt_dd_nccl_init: libnccl.so.2 not found");
+    NcclApi::UniqueId id;
+    memcpy(&id, id128, sizeof id);
+    DD_NCCL(g_nccl.CommInitRank(&d->comm, d->nranks, id, d->rank_of[0]));
+    d->links_ghost_valid = false;
+    return LGT_OK;
+}
+
+int lgt_dd_local_ranks(const lgt_dd* d) { return d ? (int)d->rk.size() : 0; }
+lgt_ctx* lgt_dd_rank(lgt_dd* d, int local_index) {
+    if (!d || local_index < 0 || local_index >= (int)d->rk.size()) return nullptr;
+    return d->rk[local_index];
+}
+
+int lgt_dd_dslash(lgt_dd* d, const void* const* in, void* const* out, int dagger) {
+    CHECK_DD(d);
+    if (!in || !out) return dd_fail(d, LGT_EINVAL, "lgt_dd_dslash: null pointer");
+    for (size_t i = 0; i < d->rk.size(); i++) {
+        if (!in[i] || !out[i] || in[i] == out[i]) return dd_fail(d, LGT_EINVAL, "lgt_dd_dslash: in and out must be distinct non-null buffers");
+        DD_RK(i, DISPATCH(d->rk[i], to_native, d->rk[i], in[i], d->rk[i]->ws[4], 12));
+    }
+    int rc = DD_DISPATCH(d, dslash, d, 4, 5, dagger ? 1 : 0);
+    if (rc != LGT_OK) return rc;
+    for (size_t i = 0; i < d->rk.size(); i++) DD_RK(i, DISPATCH(d->rk[i], from_native, d->rk[i], d->rk[i]->ws[5], out[i], 12));
+    return LGT_OK;
+}
+int lgt_dd_cg(lgt_dd* d, const void* const* b, void* const* x, double tol, int max_iter, int* iters, double* rel_resid) {
+    CHECK_DD(d);
+    if (!b || !x) return dd_fail(d, LGT_EINVAL, "lgt_dd_cg: null pointer");
+    if (!(tol >= 0.0) || max_iter < 0) return dd_fail(d, LGT_EINVAL, "lgt_dd_cg: bad tol / max_iter");
+    for (size_t i = 0; i < d->rk.size(); i++) {
+        if (!b[i] || !x[i]) return dd_fail(d, LGT_EINVAL, "lgt_dd_cg: null pointer");
+        DD_RK(i, DISPATCH(d->rk[i], to_native, d->rk[i], b[i], d->rk[i]->ws[5], 12));
+    }
+    int conv = DD_DISPATCH(d, cg, d, 5, false, tol, max_iter, iters, rel_resid);
+    if (conv != LGT_OK && conv != LGT_ENOCONV) return conv;
+    for (size_t i = 0; i < d->rk.size(); i++) DD_RK(i, DISPATCH(d->rk[i], from_native, d->rk[i], d->rk[i]->ws[0], x[i], 12));
+    return conv;
+}
+int lgt_dd_action(lgt_dd* d, double tol, int max_iter, double* S_g, double* S_F, double* K, int* cg_iters) {
+    CHECK_DD(d);
+    return DD_DISPATCH(d, action, d, tol, max_iter, S_g, S_F, K, cg_iters);
+}
+int lgt_dd_md_kick(lgt_dd* d, double eps, double tol, int max_iter, int* cg_iters) {
+    CHECK_DD(d);
+    return DD_DISPATCH(d, kick, d, eps, tol, max_iter, cg_iters);
+}
+int lgt_dd_md_drift(lgt_dd* d, double eps) {
+    CHECK_DD(d);
+    return DD_DISPATCH(d, drift, d, eps);
+}
+int lgt_dd_md_trajectory(lgt_dd* d, int nsteps, double dt, double tol, int max_iter, double* H_initial, double* H_final, long* cg_iters) {
+    CHECK_DD(d);
+    if (nsteps < 0) return dd_fail(d, LGT_EINVAL, "lgt_dd_md_trajectory: nsteps < 0");
+    int rc, it = 0, conv = LGT_OK;
+    long total = 0;
+    double sg, sf, k;
+#define DD_STEP(call)                      \
+    do {                                   \
+        it = 0;                            \
+        rc = (call);                       \
+        if (rc == LGT_ENOCONV) conv = rc;  \
+        else if (rc != LGT_OK) return rc;  \
+    } while (0)
+    if (H_initial) {
+        DD_STEP(DD_DISPATCH(d, action, d, tol, max_iter, &sg, &sf, &k, &it));
+        *H_initial = k + sg + sf;
+    }
+    if (nsteps > 0) {
+        DD_STEP(DD_DISPATCH(d, kick, d, 0.5 * dt, tol, max_iter, &it));
+        total += it;
+        for (int n = 0; n < nsteps; n++) {
+            DD_STEP(DD_DISPATCH(d, drift, d, dt));
+            DD_STEP(DD_DISPATCH(d, kick, d, (n == nsteps - 1) ? 0.5 * dt : dt, tol, max_iter, &it));
+            total += it;
+        }
+    }
+    if (H_final) {
+        DD_STEP(DD_DISPATCH(d, action, d, tol, max_iter, &sg, &sf, &k, &it));
+        *H_final = k + sg + sf;
+    }
+#undef DD_STEP
+    if (cg_iters) *cg_iters = total;
+    DD_CU(cudaStreamSynchronize(d->stream));
+    return conv;
+}
+
+}  // extern "C"

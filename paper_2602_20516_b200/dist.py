@@ -1,8 +1,11 @@
-"""Multi-GPU plumbing for bench.py: one process per GPU, N independent replicas of the path.
+"""Multi-GPU plumbing: one process per GPU.
 
-The MD step of one lattice does not shard without a halo exchange (not built),
-so N > 1 runs N independent lattices -- "replicas only", weak scaling, no data-path collective.
-torch.distributed is used for the barrier around the timed region and for two tiny reductions:
+Two ways to use N GPUs:
+  replicas   N independent lattices, no data-path collective (bench.py's default for N > 1, weak scaling);
+  decomposed ONE lattice cut into N time slabs (lgt_dd_*): halo slices and the CG / action sums travel over the
+             library's own NCCL communicator; this module only carries the 128-byte NCCL id from rank 0 to the
+             others and says which rows of a canonical array belong to which rank.
+torch.distributed is used for that broadcast, for the barrier around the timed region and for two tiny reductions:
 the MAX over ranks of the device time and the SUM over ranks of the work done.
 """
 import os
@@ -43,6 +46,49 @@ def aggregate(times, sums, device="cpu"):
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         dist.all_reduce(s, op=dist.ReduceOp.SUM)
     return t.tolist(), s.tolist()
+
+
+def slab_rows(dims, nranks, rank):
+    """Row range [lo, hi) of a canonical field [V, ...] (site s = x + Lx*(y + Ly*(z + Lz*t)), t slowest) owned by
+    `rank` when the lattice is cut into nranks slabs of Lt / nranks time slices."""
+    Lx, Ly, Lz, Lt = [int(d) for d in dims]
+    if nranks < 1 or Lt % nranks:
+        raise ValueError("Lt must be a multiple of the number of ranks")
+    if not 0 <= rank < nranks:
+        raise ValueError("bad rank")
+    per = Lx * Ly * Lz * (Lt // nranks)
+    return rank * per, (rank + 1) * per
+
+
+def broadcast_bytes(data, nbytes, src=0, device="cpu"):
+    """Rank `src` passes `data` (bytes of length nbytes), everybody returns the same bytes.  Identity without a group."""
+    import torch
+    import torch.distributed as dist
+
+    if not (dist.is_available() and dist.is_initialized()):
+        return bytes(data)
+    if dist.get_rank() == src:
+        t = torch.tensor(list(bytes(data)), dtype=torch.uint8, device=device)
+        assert t.numel() == nbytes
+    else:
+        t = torch.zeros(nbytes, dtype=torch.uint8, device=device)
+    dist.broadcast(t, src=src)
+    return bytes(t.cpu().tolist())
+
+
+def decomposed_lattice(dims, beta, kappa, bc, precision=None, local_device=0, stream=None):
+    """This process's slab of ONE lattice shared by all ranks of the default process group: a DecomposedLattice with one
+    local rank whose NCCL communicator is initialised from an id that rank 0 creates and broadcasts here."""
+    from . import lgt
+
+    rank, world, _ = env_rank_world()
+    dd = lgt.DecomposedLattice(dims, world, [rank], beta, kappa, bc, lgt.LGT_F64 if precision is None else precision,
+                               local_device, stream)
+    if world > 1:
+        ident = lgt.lgt_dd_nccl_unique_id() if rank == 0 else None
+        ident = broadcast_bytes(ident, 128, src=0, device="cuda:%d" % local_device)
+        lgt.lgt_dd_nccl_init(dd.d, ident)
+    return dd
 
 
 def throughput(units_total, time_max_s):

@@ -63,6 +63,19 @@ SYMBOLS = {
     "lgt_eo_mhat": (_i, [_vp, _vp, _vp, _i]),
     "lgt_eo_cg": (_i, [_vp, _vp, _vp, _d, _i, _ip, _dp]),
     "lgt_set_fermion_action": (_i, [_vp, _i]),
+    "lgt_dd_create": (_i, [C.POINTER(_vp), _ip, _i, _i, _ip, _d, _d, _ip, _i, _i, _vp]),
+    "lgt_dd_destroy": (_i, [_vp]),
+    "lgt_dd_last_error": (C.c_char_p, [_vp]),
+    "lgt_dd_nccl_unique_id": (_i, [_vp]),
+    "lgt_dd_nccl_init": (_i, [_vp, _vp]),
+    "lgt_dd_local_ranks": (_i, [_vp]),
+    "lgt_dd_rank": (_vp, [_vp, _i]),
+    "lgt_dd_dslash": (_i, [_vp, C.POINTER(_vp), C.POINTER(_vp), _i]),
+    "lgt_dd_cg": (_i, [_vp, C.POINTER(_vp), C.POINTER(_vp), _d, _i, _ip, _dp]),
+    "lgt_dd_action": (_i, [_vp, _d, _i, _dp, _dp, _dp, _ip]),
+    "lgt_dd_md_kick": (_i, [_vp, _d, _d, _i, _ip]),
+    "lgt_dd_md_drift": (_i, [_vp, _d]),
+    "lgt_dd_md_trajectory": (_i, [_vp, _i, _d, _d, _i, _dp, _dp, _lp]),
     "lgt_set_smearing": (_i, [_vp, _i, _d]),
     "lgt_get_smeared_links": (_i, [_vp, _vp]),
     "lgt_set_integrator": (_i, [_vp, _i, _i]),
@@ -369,6 +382,95 @@ def lgt_set_block_swizzle(ctx, z_planes=-1):
     return out.value
 
 
+# ---- decomposed lattice (lgt_dd_*) -----------------------------------------------------------------
+def _dd_check(d, rc, allow=()):
+    if rc != LGT_OK and rc not in allow:
+        msg = lib().lgt_dd_last_error(d)
+        raise LgtError(rc, msg.decode() if msg else "")
+    return rc
+
+
+def _ptr_array(items):
+    return (_vp * len(items))(*[_ptr(t) for t in items])
+
+
+def lgt_dd_create(dims, nranks, local_ranks, beta, kappa, bc, precision=LGT_F64, device=0, stream=None):
+    h = _vp()
+    d4 = (C.c_int * 4)(*[int(x) for x in dims])
+    b4 = (C.c_int * 4)(*[int(x) for x in bc])
+    lr = (C.c_int * len(local_ranks))(*[int(r) for r in local_ranks])
+    rc = lib().lgt_dd_create(C.byref(h), d4, nranks, len(local_ranks), lr, beta, kappa, b4, precision, device, stream)
+    _dd_check(None, rc)
+    return h
+
+
+def lgt_dd_destroy(d):
+    lib().lgt_dd_destroy(d)
+
+
+def lgt_dd_last_error(d):
+    msg = lib().lgt_dd_last_error(d)
+    return msg.decode() if msg else ""
+
+
+def lgt_dd_nccl_unique_id():
+    """128 bytes (rank 0 calls this, everybody receives them by a broadcast)."""
+    buf = C.create_string_buffer(128)
+    _dd_check(None, lib().lgt_dd_nccl_unique_id(buf))
+    return bytes(buf.raw)
+
+
+def lgt_dd_nccl_init(d, id128):
+    _dd_check(d, lib().lgt_dd_nccl_init(d, C.c_char_p(bytes(id128))))
+
+
+def lgt_dd_local_ranks(d):
+    return lib().lgt_dd_local_ranks(d)
+
+
+def lgt_dd_rank(d, local_index):
+    h = lib().lgt_dd_rank(d, local_index)
+    if not h:
+        raise LgtError(LGT_EINVAL, "lgt_dd_rank: bad local index")
+    return _vp(h)
+
+
+def lgt_dd_dslash(d, ins, outs, dagger=False):
+    _dd_check(d, lib().lgt_dd_dslash(d, _ptr_array(ins), _ptr_array(outs), int(bool(dagger))))
+
+
+def lgt_dd_cg(d, bs, xs, tol, max_iter):
+    """Returns (iters, rel_resid, converged)."""
+    it, rel = C.c_int(), C.c_double()
+    rc = _dd_check(d, lib().lgt_dd_cg(d, _ptr_array(bs), _ptr_array(xs), tol, max_iter, C.byref(it), C.byref(rel)), allow=(LGT_ENOCONV,))
+    return it.value, rel.value, rc == LGT_OK
+
+
+def lgt_dd_action(d, tol=1e-12, max_iter=100000):
+    """Returns (S_g, S_F, K, cg_iters), global values."""
+    sg, sf, k, it = C.c_double(), C.c_double(), C.c_double(), C.c_int()
+    _dd_check(d, lib().lgt_dd_action(d, tol, max_iter, C.byref(sg), C.byref(sf), C.byref(k), C.byref(it)))
+    return sg.value, sf.value, k.value, it.value
+
+
+def lgt_dd_md_kick(d, eps, tol=1e-12, max_iter=100000):
+    it = C.c_int()
+    _dd_check(d, lib().lgt_dd_md_kick(d, eps, tol, max_iter, C.byref(it)))
+    return it.value
+
+
+def lgt_dd_md_drift(d, eps):
+    _dd_check(d, lib().lgt_dd_md_drift(d, eps))
+
+
+def lgt_dd_md_trajectory(d, nsteps, dt, tol=1e-12, max_iter=100000, measure=True):
+    """Returns (H_initial, H_final, cg_iters)."""
+    h0, h1, its = C.c_double(), C.c_double(), C.c_long()
+    _dd_check(d, lib().lgt_dd_md_trajectory(d, nsteps, dt, tol, max_iter, C.byref(h0) if measure else None,
+                                            C.byref(h1) if measure else None, C.byref(its)))
+    return h0.value, h1.value, its.value
+
+
 # ---- convenience wrapper -----------------------------------------------------------------------
 class Lattice:
     """A handle plus torch buffers in the canonical layout.  numpy in / numpy out helpers for tests."""
@@ -464,3 +566,81 @@ class Lattice:
         it = lgt_fermion_force(self.ctx, None if X is None else self.to_device(X),
                                None if Y is None else self.to_device(Y), F, tol, max_iter)
         return F.cpu().numpy(), it
+
+
+class DecomposedLattice:
+    """A group of time slabs (lgt_dd_*) with numpy in / numpy out helpers.  `local_ranks` = all ranks: the
+    single-device verification mode; one rank: the production mode (call nccl_init with the broadcast id)."""
+
+    def __init__(self, dims, nranks, local_ranks, beta, kappa, bc, precision=LGT_F64, device=0, stream=None):
+        import torch
+
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_2602_20516_b200 needs a CUDA device (there is no CPU fallback)")
+        self.torch = torch
+        self.dims = tuple(int(d) for d in dims)
+        self.nranks, self.local_ranks = int(nranks), [int(r) for r in local_ranks]
+        self.V = self.dims[0] * self.dims[1] * self.dims[2] * self.dims[3]
+        self.Vloc = self.V // self.nranks
+        self.cdtype = torch.complex128 if precision == LGT_F64 else torch.complex64
+        self.device = torch.device("cuda", device)
+        self.d = lgt_dd_create(dims, nranks, local_ranks, beta, kappa, bc, precision, device, stream)
+        self.ranks = [lgt_dd_rank(self.d, i) for i in range(len(self.local_ranks))]
+
+    def close(self):
+        if self.d is not None:
+            lgt_dd_destroy(self.d)
+            self.d = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def slab(self, a, rank):
+        """Rows of a global canonical array [V, ...] that belong to `rank` (t is the slowest index)."""
+        return a[rank * self.Vloc:(rank + 1) * self.Vloc]
+
+    def _up(self, a, rank):
+        return self.torch.from_numpy(self.slab(a, rank)).to(self.cdtype).to(self.device).contiguous()
+
+    def _scatter(self, a, setter):
+        for i, r in enumerate(self.local_ranks):
+            setter(self.ranks[i], self._up(a, r))
+
+    def _gather(self, getter, *shape):
+        """Local slabs as a list of numpy arrays in local-rank order."""
+        out = []
+        for i in range(len(self.local_ranks)):
+            t = self.torch.empty((self.Vloc,) + shape, dtype=self.cdtype, device=self.device)
+            getter(self.ranks[i], t)
+            out.append(t.cpu().numpy())
+        return out
+
+    def set_links(self, U):
+        self._scatter(U, lgt_set_links)
+
+    def set_momenta(self, P):
+        self._scatter(P, lgt_set_momenta)
+
+    def set_pseudofermion(self, phi):
+        self._scatter(phi, lgt_set_pseudofermion)
+
+    def get_links(self):
+        return self._gather(lgt_get_links, 4, 3, 3)
+
+    def get_momenta(self):
+        return self._gather(lgt_get_momenta, 4, 3, 3)
+
+    def dslash(self, psi, dagger=False):
+        ins = [self._up(psi, r) for r in self.local_ranks]
+        outs = [self.torch.empty_like(t) for t in ins]
+        lgt_dd_dslash(self.d, ins, outs, dagger)
+        return [t.cpu().numpy() for t in outs]
+
+    def cg(self, b, tol, max_iter):
+        bs = [self._up(b, r) for r in self.local_ranks]
+        xs = [self.torch.empty_like(t) for t in bs]
+        it, rel, ok = lgt_dd_cg(self.d, bs, xs, tol, max_iter)
+        return [t.cpu().numpy() for t in xs], it, rel, ok

@@ -19,8 +19,11 @@ WORKER = textwrap.dedent("""
     times, sums = dist.aggregate([10.0 * (rank + 1), 1.0], [100.0 * (rank + 1), 7.0])
     cfg = dict(synth.CONFIGS[0]); cfg["seed_links"] += 100 * rank
     U = synth.config_links(cfg)
+    # decomposed mode: the id travels from rank 0, the slabs tile the lattice
+    ident = dist.broadcast_bytes(bytes(range(128)) if rank == 0 else None, 128, src=0)
+    lo, hi = dist.slab_rows((4, 4, 2, 8), world, rank)
     print(json.dumps({"rank": rank, "times": times, "sums": sums, "u00": [U[0,0,0,0].real, U[0,0,0,0].imag],
-                      "value": dist.throughput(sums[0], times[0] * 1e-3)}))
+                      "value": dist.throughput(sums[0], times[0] * 1e-3), "id": list(ident), "rows": [lo, hi]}))
     dist.shutdown()
 """) % ROOT
 
@@ -55,6 +58,8 @@ def test_two_rank_aggregation_gloo(tmp_path):
         assert o["sums"] == [300.0, 14.0]  # SUM over ranks
         assert abs(o["value"] - 300.0 / 20e-3) < 1e-9
     assert outs[0]["u00"] != outs[1]["u00"]  # replicas are independent lattices
+    assert outs[0]["id"] == outs[1]["id"] == list(range(128))
+    assert sorted(o["rows"] for o in outs) == [[0, 128], [128, 256]]
 
 
 def test_single_process_identity():
@@ -64,3 +69,9 @@ def test_single_process_identity():
     t, s = dist.aggregate([3.0], [5.0])
     assert t == [3.0] and s == [5.0]
     assert dist.env_rank_world()[1] >= 1
+    assert dist.broadcast_bytes(b"abc", 3) == b"abc"
+    rows = [dist.slab_rows((4, 4, 4, 12), 3, r) for r in range(3)]
+    assert rows == [(0, 256), (256, 512), (512, 768)]
+    import pytest
+    with pytest.raises(ValueError):
+        dist.slab_rows((4, 4, 4, 10), 3, 0)

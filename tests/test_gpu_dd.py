@@ -1,0 +1,136 @@
+"""GPU parity for the time-slab decomposition (lgt_dd_*): all ranks of the group live on the one GPU and are
+stepped in lockstep with device copies as the exchange (no rank waits on another), so the decomposed kernels, halo
+logic, global sums and boundary signs are verified against the oracle on the undivided lattice; the NCCL transport
+is exercised with one rank (send/recv to itself through the same code path).
+"""
+import numpy as np
+import pytest
+
+import oracle
+from paper_2602_20516_b200 import synth
+from lattice_util import link_rel_err
+
+pytestmark = pytest.mark.gpu
+
+BC = (1, 1, 1, -1)
+TOL64 = 1e-11
+
+
+@pytest.fixture(scope="module")
+def lgt():
+    import torch
+
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device; the product path has no CPU fallback")
+    from paper_2602_20516_b200 import lgt as m
+
+    m.lib()
+    return m
+
+
+def cat(slabs):
+    return np.concatenate(slabs, axis=0)
+
+
+@pytest.mark.parametrize("dims,nranks", [((4, 4, 2, 8), 1), ((4, 4, 2, 8), 2), ((4, 4, 2, 8), 4), ((8, 4, 4, 6), 3),
+                                         ((4, 4, 2, 8), 8), ((8, 8, 8, 8), 2)])
+def test_dd_dslash_matches_oracle_and_single_handle(lgt, dims, nranks):
+    kappa = 0.12
+    U = synth.warm_links(dims, 0.3, 501)
+    psi = synth.gaussian_spinor(dims, 502)
+    dd = lgt.DecomposedLattice(dims, nranks, list(range(nranks)), 5.5, kappa, BC)
+    dd.set_links(U)
+    one = lgt.Lattice(dims, 5.5, kappa, BC)
+    one.set_links(U)
+    for dag in (False, True):
+        out = cat(dd.dslash(psi, dagger=dag))
+        assert np.abs(out - oracle.dslash(dims, kappa, BC, U, psi, dagger=dag)).max() < 1e-12
+        assert np.array_equal(out, one.dslash(psi, dagger=dag))  # same kernel, same order of operations per site
+    assert np.array_equal(cat(dd.get_links()), U)
+    # a slab handle refuses the single-lattice calls
+    with pytest.raises(lgt.LgtError) as e:
+        lgt.lgt_plaquette(dd.ranks[0])
+    assert e.value.code == lgt.LGT_ESTATE
+    dd.close()
+    one.close()
+
+
+@pytest.mark.parametrize("nranks", [2, 4])
+def test_dd_cg(lgt, nranks):
+    dims, kappa = (4, 4, 4, 8), 0.12
+    U = synth.warm_links(dims, 0.3, 511)
+    b = oracle.dslash(dims, kappa, BC, U, synth.gaussian_spinor(dims, 512), dagger=True)
+    x_ref, it_ref, _, ok = oracle.cg(dims, kappa, BC, U, b, 1e-12, 5000)
+    assert ok
+    dd = lgt.DecomposedLattice(dims, nranks, list(range(nranks)), 5.5, kappa, BC)
+    dd.set_links(U)
+    xs, it, rel, ok = dd.cg(b, 1e-12, 5000)
+    assert ok and it == it_ref and rel <= 1e-12
+    x = cat(xs)
+    assert np.linalg.norm(x - x_ref) < 1e-10 * np.linalg.norm(x_ref)
+    dd.close()
+
+
+@pytest.mark.parametrize("nranks", [2, 4])
+def test_dd_md_trajectory(lgt, nranks):
+    """Leapfrog with both forces on the decomposed lattice against the oracle's trajectory on the undivided one."""
+    dims, beta, kappa = (4, 4, 2, 8), 5.6, 0.11
+    U0 = synth.warm_links(dims, 0.25, 521)
+    P0 = synth.gaussian_momenta(dims, 522)
+    phi = oracle.dslash(dims, kappa, BC, U0, synth.gaussian_spinor(dims, 523), dagger=True)
+    dd = lgt.DecomposedLattice(dims, nranks, list(range(nranks)), beta, kappa, BC)
+    dd.set_links(U0)
+    dd.set_momenta(P0)
+    dd.set_pseudofermion(phi)
+    S_g, S_F, K, _ = lgt.lgt_dd_action(dd.d, 1e-13, 5000)
+    H_ref, K_ref, Sg_ref, SF_ref = oracle.hamiltonian(dims, beta, kappa, BC, U0, phi, P0, 1e-13, 5000)
+    assert abs(S_g - Sg_ref) < 1e-11 * abs(Sg_ref) and abs(S_F - SF_ref) < 1e-10 * abs(SF_ref) and abs(K - K_ref) < 1e-12 * K_ref
+    H0, H1, its = lgt.lgt_dd_md_trajectory(dd.d, 3, 0.03, tol=1e-13, max_iter=5000)
+    U_ref, P_ref, its_ref, ok = oracle.trajectory(dims, beta, kappa, BC, U0, phi, P0, 3, 0.03, tol=1e-13, max_iter=5000)
+    assert ok and its == its_ref
+    assert np.abs(cat(dd.get_links()) - U_ref).max() < 1e-12
+    assert link_rel_err(cat(dd.get_momenta()), P_ref)[0] < TOL64
+    H1_ref = oracle.hamiltonian(dims, beta, kappa, BC, U_ref, phi, P_ref, 1e-13, 5000)[0]
+    assert abs((H1 - H0) - (H1_ref - H_ref)) < 1e-9 * abs(H_ref)
+    # kick and drift on their own
+    dd.set_links(U0)
+    dd.set_momenta(P0)
+    lgt.lgt_dd_md_kick(dd.d, 0.05, 1e-13, 5000)
+    P1, _, _ = oracle.kick(dims, beta, kappa, BC, U0, phi, P0, 0.05, 1e-13, 5000)
+    assert link_rel_err(cat(dd.get_momenta()), P1)[0] < TOL64
+    lgt.lgt_dd_md_drift(dd.d, 0.05)
+    assert np.abs(cat(dd.get_links()) - oracle.drift(dims, 0.05, P1, U0)).max() < 1e-13
+    dd.close()
+
+
+def test_dd_nccl_transport_one_rank(lgt):
+    """The NCCL code path (send/recv of the halo slices to itself, all-reduce of the sums) with a single rank."""
+    dims, kappa = (4, 4, 2, 8), 0.12
+    U = synth.warm_links(dims, 0.3, 531)
+    b = oracle.dslash(dims, kappa, BC, U, synth.gaussian_spinor(dims, 532), dagger=True)
+    dd = lgt.DecomposedLattice(dims, 1, [0], 5.5, kappa, BC)
+    lgt.lgt_dd_nccl_init(dd.d, lgt.lgt_dd_nccl_unique_id())
+    dd.set_links(U)
+    assert np.abs(cat(dd.dslash(b)) - oracle.dslash(dims, kappa, BC, U, b)).max() < 1e-12
+    x_ref, it_ref, _, _ = oracle.cg(dims, kappa, BC, U, b, 1e-12, 5000)
+    xs, it, rel, ok = dd.cg(b, 1e-12, 5000)
+    assert ok and it == it_ref and np.linalg.norm(cat(xs) - x_ref) < 1e-10 * np.linalg.norm(x_ref)
+    with pytest.raises(lgt.LgtError):
+        lgt.lgt_dd_nccl_init(dd.d, lgt.lgt_dd_nccl_unique_id())  # already initialised
+    dd.close()
+
+
+def test_dd_argument_checks(lgt):
+    with pytest.raises(lgt.LgtError):
+        lgt.lgt_dd_create((4, 4, 2, 8), 3, [0, 1, 2], 5.5, 0.1, BC)  # Lt not divisible
+    with pytest.raises(lgt.LgtError):
+        lgt.lgt_dd_create((4, 3, 2, 8), 2, [0, 1], 5.5, 0.1, BC)  # time slice not a multiple of 32 sites
+    with pytest.raises(lgt.LgtError):
+        lgt.lgt_dd_create((4, 4, 2, 8), 4, [0, 1], 5.5, 0.1, BC)  # neither all local nor one local
+    with pytest.raises(lgt.LgtError):
+        lgt.lgt_dd_create((4, 4, 2, 8), 2, [0, 0], 5.5, 0.1, BC)
+    d = lgt.lgt_dd_create((4, 4, 2, 8), 2, [0, 1], 5.5, 0.1, BC)
+    assert lgt.lgt_dd_local_ranks(d) == 2
+    with pytest.raises(lgt.LgtError):
+        lgt.lgt_dd_nccl_init(d, b"\0" * 128)  # NCCL serves one rank per process
+    lgt.lgt_dd_destroy(d)
