@@ -298,6 +298,38 @@ def run_ours(args):
             "hop_fused_r_avg_us": round(hopr_ms / max(hopr_n, 1) * 1e3, 2),
             "note": "S_F = phi_e^dag (M^dag M)^-1 phi_e, CG on the Schur complement to the same 1e-12"}
         lgt.lgt_set_fermion_action(ctx, lgt.LGT_ACTION_FULL)
+        # the decomposed path (lgt_dd_*) on this one GPU: 1 and 4 time slabs in one process, halo exchange by device copies
+        import numpy as np
+        U_np, P_np, phi_np = hU.numpy(), hP.numpy(), hphi.numpy()
+        for nr in (1, 4):
+            if dims[3] % nr or (dims[0] * dims[1] * dims[2]) % 32:
+                continue
+            dd = lgt.DecomposedLattice(dims, nr, list(range(nr)), beta, kappa, bc, lgt.LGT_F64, local, stream)
+
+            def dd_reset():
+                dd.set_links(U_np)
+                dd.set_momenta(P_np)
+                dd.set_pseudofermion(phi_np)
+
+            def dd_step():
+                it = lgt.lgt_dd_md_kick(dd.d, dt, tol, max_iter)
+                lgt.lgt_dd_md_drift(dd.d, dt)
+                return it
+
+            dd_reset()
+            dd_step()
+            dd_reset()
+            torch.cuda.synchronize()
+            a.record()
+            dd_iters = [dd_step() for _ in range(2)]
+            b.record()
+            torch.cuda.synchronize()
+            extras["decomposed_%d_slabs_one_gpu" % nr] = {
+                "ms_per_step": round(a.elapsed_time(b) / 2, 3), "cg_iters_per_step": dd_iters,
+                "note": "same MD step through lgt_dd_* with %d time slab(s) resident on this GPU: the cost of the ghost "
+                        "slices, halo copies and split reductions, not a multi-GPU number" % nr}
+            dd.close()
+            del dd
 
     # ---- max over ranks, aggregate
     (elapsed_ms, e2e_s), (total_reals, total_flops, e2e_reals, launches_all) = dist.aggregate(
@@ -440,6 +472,107 @@ def cpu_baseline(cfg, sample_iters, steps=1, warmup=0):
                       % ("x".join(map(str, cfg["dims"])), sample_iters, sample_iters)}
 
 
+# ------------------------------------------------------------------------------------------------ one lattice on N GPUs
+def run_decomposed(args):
+    """--parallelism dd: ONE configs[3] lattice cut into N time slabs (lgt_dd_*), strong scaling.  The same MD step, the
+    same byte accounting for the whole lattice; halo slices and CG sums go over the library's NCCL communicator.
+    Verified on one GPU only (all slabs in one process, and NCCL with a single rank): DESIGN.md "Multi-GPU"."""
+    import torch
+
+    from paper_2602_20516_b200 import dist, lgt, synth
+
+    rank, world, local = dist.env_rank_world()
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dist.init("nccl", torch.device("cuda", local))
+    lgt.lib()
+    cfg = dict(synth.CONFIGS[args.config])
+    if args.lattice:
+        cfg["dims"] = tuple(args.lattice)
+    dims, beta, kappa, bc = cfg["dims"], cfg["beta"], cfg["kappa"], cfg["bc"]
+    tol, dt = cfg.get("cg_tol", 1e-12), cfg.get("dt", 0.01)
+    V = synth.volume(dims)
+    max_iter = 10 * V
+    U, P, eta = make_inputs(cfg)  # every rank draws the same global fields and keeps its slab
+    stream = torch.cuda.current_stream().cuda_stream
+    dd = dist.decomposed_lattice(dims, beta, kappa, bc, lgt.LGT_F64, local, stream)
+    lo, hi = dist.slab_rows(dims, world, rank)
+    hU, hP = torch.from_numpy(U[lo:hi].copy()).pin_memory(), torch.from_numpy(P[lo:hi].copy()).pin_memory()
+    ctx = dd.ranks[0]
+    lgt.lgt_set_links_host(ctx, hU)
+    d_eta = torch.from_numpy(eta[lo:hi].copy()).cuda()
+    d_phi = torch.empty_like(d_eta)
+    lgt.lgt_dd_dslash(dd.d, [d_eta], [d_phi], True)
+    hphi = d_phi.cpu().pin_memory()
+    hU_out, hP_out = torch.empty_like(hU), torch.empty_like(hP)
+    del U, P, eta, d_eta
+
+    def reset_state():
+        lgt.lgt_set_links_host(ctx, hU)
+        lgt.lgt_set_momenta_host(ctx, hP)
+        lgt.lgt_set_pseudofermion_host(ctx, hphi)
+
+    def md_step():
+        it = lgt.lgt_dd_md_kick(dd.d, dt, tol, max_iter)
+        lgt.lgt_dd_md_drift(dd.d, dt)
+        return it
+
+    def barrier():
+        dist.barrier()
+        torch.cuda.synchronize()
+
+    reset_state()
+    for _ in range(args.warmup):
+        md_step()
+    sampler = ClockSampler(local)
+    launches0 = lgt.lgt_launch_count(ctx)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    sampler.start()
+    barrier()
+    e0.record()
+    iters = [md_step() for _ in range(args.steps)]
+    e1.record()
+    barrier()
+    clocks = sampler.stop()
+    elapsed_ms = e0.elapsed_time(e1)
+    launches = lgt.lgt_launch_count(ctx) - launches0
+    k_e2e = max(1, min(args.steps, 3))
+    barrier()
+    t0 = time.perf_counter()
+    e2e_iters = []
+    for _ in range(k_e2e):
+        reset_state()
+        e2e_iters.append(md_step())
+        lgt.lgt_get_links_host(ctx, hU_out)
+        lgt.lgt_get_momenta_host(ctx, hP_out)
+    torch.cuda.synchronize()
+    e2e_s = time.perf_counter() - t0
+    (elapsed_ms, e2e_s), (launches_all,) = dist.aggregate([elapsed_ms, e2e_s], [launches], device="cuda")
+    if rank == 0:
+        total_reals = sum(step_reals(i) for i in iters) * V  # the whole lattice: strong scaling
+        e2e_reals = sum(step_reals(i) for i in e2e_iters) * V
+        out = {
+            "metric": METRIC, "value": round(total_reals * 8 / (elapsed_ms * 1e-3) / 1e9, 1), "unit": "GB/s", "n_gpus": world,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": round(elapsed_ms / args.steps, 3),
+            "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": "configs[%d]: ONE %s SU(3) lattice in %d time slabs, one MD step = kick(dt) + drift(dt), "
+                                   "CG 1e-12" % (args.config, "x".join(map(str, dims)), world),
+                       "beta": beta, "kappa": kappa, "bc": list(bc), "dt": dt, "cg_tol": tol, "cg_iters_per_step": iters,
+                       "parallelism": "dd%d (time slabs, NCCL halo exchange + all-reduce)" % world,
+                       "l2": "inputs exceed L2 at 32^4 up to 8 slabs (links 604 MB / N per rank)"},
+            "clocks": clocks,
+            "e2e": {"value": round(e2e_reals * 8 / e2e_s / 1e9, 1), "unit": "GB/s", "steps": k_e2e,
+                    "ms_per_step": round(e2e_s / k_e2e * 1e3, 2),
+                    "h2d_bytes_per_step": (hU.numel() + hP.numel() + hphi.numel()) * 16 * world,
+                    "d2h_bytes_per_step": (hU_out.numel() + hP_out.numel()) * 16 * world},
+            "gpu_launches": int(launches_all),
+        }
+        print(json.dumps(out), flush=True)
+    dd.close()
+    dist.shutdown()
+
+
 def run_reference(args):
     from paper_2602_20516_b200 import dist, synth
 
@@ -479,12 +612,17 @@ def main():
     ap.add_argument("--action", default="full", choices=["full", "eo"],
                     help="non-default: time the step with the even/odd preconditioned action (not the headline configuration)")
     ap.add_argument("--skip-extras", action="store_true", help="profiling runs only: leave the non-headline solver arms out")
+    ap.add_argument("--parallelism", default="replicas", choices=["replicas", "dd"],
+                    help="N > 1: 'replicas' = N independent lattices (default, weak scaling); 'dd' = ONE lattice cut into N "
+                         "time slabs with NCCL halo exchange (lgt_dd_*, strong scaling; verified on one GPU only, DESIGN.md)")
     ap.add_argument("--cpu-sample-iters", type=int, default=4, help="CG iterations in the oracle's bounded sample")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3  # timing rule: at least 3 warm-up steps
     if args.impl == "reference":
         run_reference(args)
+    elif args.parallelism == "dd":
+        run_decomposed(args)
     else:
         run_ours(args)
 

@@ -979,11 +979,11 @@ int lgt_set_pseudofermion(lgt_ctx* c, const void* phi) {
         CU(cudaStreamSynchronize(c->stream));                                                       \
         return LGT_OK;                                                                              \
     }
-HOST_SET(lgt_set_links_host, lgt_set_links, (size_t)36 * c->g.V * c->esize)
-HOST_GET(lgt_get_links_host, lgt_get_links, (size_t)36 * c->g.V * c->esize)
-HOST_SET(lgt_set_momenta_host, lgt_set_momenta, (size_t)36 * c->g.V * c->esize)
-HOST_GET(lgt_get_momenta_host, lgt_get_momenta, (size_t)36 * c->g.V * c->esize)
-HOST_SET(lgt_set_pseudofermion_host, lgt_set_pseudofermion, (size_t)12 * c->g.V * c->esize)
+HOST_SET(lgt_set_links_host, lgt_set_links, (size_t)36 * (c->g.s_end - c->g.s_begin) * c->esize)
+HOST_GET(lgt_get_links_host, lgt_get_links, (size_t)36 * (c->g.s_end - c->g.s_begin) * c->esize)
+HOST_SET(lgt_set_momenta_host, lgt_set_momenta, (size_t)36 * (c->g.s_end - c->g.s_begin) * c->esize)
+HOST_GET(lgt_get_momenta_host, lgt_get_momenta, (size_t)36 * (c->g.s_end - c->g.s_begin) * c->esize)
+HOST_SET(lgt_set_pseudofermion_host, lgt_set_pseudofermion, (size_t)12 * (c->g.s_end - c->g.s_begin) * c->esize)
 
 // ---- actions
 int lgt_action(lgt_ctx* c, double tol, int max_iter, double* S_g, double* S_F, double* K, int* cg_iters) {
