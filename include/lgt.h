@@ -110,7 +110,8 @@ int lgt_cg_mixed(lgt_ctx* ctx, const void* b, void* x, double tol, int max_iter,
 /* Chooses the solver used wherever the library solves the pseudofermion system itself (lgt_action, lgt_fermion_force
  * with X = Y = NULL, lgt_md_*): LGT_SOLVER_CG (default; the plain CG of lgt_cg, iteration counts identical to the
  * oracle's in fp64) or LGT_SOLVER_MIXED_CG with the given inner_tol (ignored for LGT_SOLVER_CG).  cg_iters outputs
- * then count fp32 iterations. */
+ * then count fp32 iterations.  Combines with LGT_ACTION_EO: fp32 CG on the Schur complement M^dag M inside the same
+ * fp64 defect correction on the true residual (the fastest configuration of the MD step, bench.py "extras"). */
 int lgt_set_solver(lgt_ctx* ctx, int solver, double inner_tol);
 
 /* ---- even/odd (Schur) preconditioning (every extent of the lattice must be even) ---------- */

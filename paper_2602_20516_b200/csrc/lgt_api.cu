@@ -41,6 +41,10 @@ struct lgt_ctx {
     void* Ucb = nullptr;
     bool ucb_valid = false;
     void* eo = nullptr;  // Xe, Xo, Ye, Yo, be, re, pe, to: 8 x 12 * Vhs complex
+    // mixed-precision solve of the even/odd system (LGT_F64 handles, lazy): fp32 checkerboard links, six fp32 half fields
+    void* Ucb32 = nullptr;
+    bool ucb32_valid = false;
+    void* eo32 = nullptr;  // b, e, r, p, u, t
     int solver = LGT_SOLVER_CG;
     // stout smearing of the links the fermions see (lazy): Usm[k] = level k+1 links, Asm[k] = its exponents (compact)
     int nsmear = 0;
@@ -164,6 +168,8 @@ int ensure_force_buf(lgt_ctx* c) {
     return LGT_OK;
 }
 
+int eo_cg_mixed(lgt_ctx* c, void* b, void* x, void* r, void* q, void* u, void* t_o, double tol, int max_iter, int* iters);
+
 template <class T> struct Ops {
     typedef typename Vec2<T>::type T2;
 
@@ -196,6 +202,7 @@ template <class T> struct Ops {
     c->usm_valid = false;
     if (c->dd_links_valid) *c->dd_links_valid = false;
         c->ucb_valid = false;
+    c->ucb32_valid = false;
         LAUNCH(c, LGT_K_OTHER, (unit_links_kernel<T>), stream_blocks(c, (size_t)36 * c->g.Vs), 256, c->g, (T2*)c->U);
         return LGT_OK;
     }
@@ -337,6 +344,7 @@ template <class T> struct Ops {
     c->usm_valid = false;
     if (c->dd_links_valid) *c->dd_links_valid = false;
         c->ucb_valid = false;
+    c->ucb32_valid = false;
         LAUNCH(c, LGT_K_LINK_UPDATE, (link_update_kernel<T>), grid, 128, c->g, (const T2*)c->U, (T2*)c->U, (const T2*)c->P, (T)eps);
         return LGT_OK;
     }
@@ -381,14 +389,17 @@ template <class T> struct Ops {
     }
 
     // ---- even/odd preconditioning
-    static T2* eo_field(lgt_ctx* c, int i) { return (T2*)c->eo + (size_t)i * 12 * c->g.Vhs; }
-    static const T2* links_cb(lgt_ctx* c, int p) { return (const T2*)c->Ucb + (size_t)p * 36 * c->g.Vhs; }
+    // Ops<float> on an LGT_F64 handle (the fp32 inner solve of the mixed-precision solver) works on the fp32 copies
+    static bool fp32_on_f64(const lgt_ctx* c) { return sizeof(T) == 4 && c->prec == LGT_F64; }
+    static T2* eo_field(lgt_ctx* c, int i) { return (T2*)(fp32_on_f64(c) ? c->eo32 : c->eo) + (size_t)i * 12 * c->g.Vhs; }
+    static const T2* links_cb(lgt_ctx* c, int p) { return (const T2*)(fp32_on_f64(c) ? c->Ucb32 : c->Ucb) + (size_t)p * 36 * c->g.Vhs; }
     static int eo_ensure(lgt_ctx* c) {
         int rcf = ensure_fermion_links(c);
         if (rcf != LGT_OK) return rcf;
         if (!c->Ucb) {
             CU(cudaMalloc(&c->Ucb, (size_t)2 * 36 * c->g.Vhs * sizeof(T2)));
             c->ucb_valid = false;
+    c->ucb32_valid = false;
         }
         if (!c->eo) {
             CU(cudaMalloc(&c->eo, (size_t)8 * 12 * c->g.Vhs * sizeof(T2)));
@@ -475,7 +486,10 @@ template <class T> struct Ops {
         T2 *Xe = eo_field(c, 0), *Xo = eo_field(c, 1), *Ye = eo_field(c, 2), *Yo = eo_field(c, 3);
         T2 *be = eo_field(c, 4), *re = eo_field(c, 5), *pe = eo_field(c, 6), *to = eo_field(c, 7);
         if ((rc = eo_split(c, c->phi, be)) != LGT_OK) return rc;  // (be, re) receive (phi_e, phi_o); re is overwritten next
-        conv = eo_cg(c, be, Xe, re, pe, Ye, to, tol, max_iter, iters, nullptr);
+        if (c->solver == LGT_SOLVER_MIXED_CG && c->prec == LGT_F64 && sizeof(T) == 8)
+            conv = eo_cg_mixed(c, be, Xe, re, pe, Ye, to, tol, max_iter, iters);
+        else
+            conv = eo_cg(c, be, Xe, re, pe, Ye, to, tol, max_iter, iters, nullptr);
         if (conv != LGT_OK && conv != LGT_ENOCONV) return conv;
         if (dev_SF && (rc = redot(c, be, Xe, dev_SF, (size_t)12 * c->g.Vhs)) != LGT_OK) return rc;
         if (X && Y) {
@@ -493,6 +507,63 @@ template <class T> struct Ops {
 int read_scalars(lgt_ctx* c, int n) {
     CU(cudaMemcpyAsync(c->h_scal, c->scal, sizeof(double) * n, cudaMemcpyDeviceToHost, c->stream));
     CU(cudaStreamSynchronize(c->stream));
+    return LGT_OK;
+}
+
+// Mixed-precision solve of (M^dag M) x_e = b_e on an fp64 handle: the defect correction of cg_mixed() with the even/odd
+// operator -- fp32 CG on the Schur complement (fp32 checkerboard links and half fields) inside, true fp64 residual
+// r = b - M^dag M x outside, stop on |r| <= tol |b|.  b, x, r, q, u: fp64 even half fields; t_o: an odd scratch field.
+int eo_cg_mixed(lgt_ctx* c, void* b, void* x, void* r, void* q, void* u, void* t_o, double tol, int max_iter, int* iters) {
+    typedef Ops<double> O64;
+    typedef Ops<float> O32;
+    const size_t n = (size_t)12 * c->g.Vhs;
+    if (!c->Ucb32) {
+        CU(cudaMalloc(&c->Ucb32, (size_t)2 * 36 * c->g.Vhs * sizeof(float2)));
+        CU(cudaMalloc(&c->eo32, (size_t)6 * n * sizeof(float2)));
+        CU(cudaMemsetAsync(c->eo32, 0, (size_t)6 * n * sizeof(float2), c->stream));
+        c->ucb32_valid = false;
+    }
+    const int nb = stream_blocks(c, n);
+    if (!c->ucb32_valid) {
+        const size_t nu = (size_t)2 * 36 * c->g.Vhs;
+        LAUNCH(c, LGT_K_OTHER, down_convert_kernel, stream_blocks(c, nu), 256, nu, (const double2*)c->Ucb, (float2*)c->Ucb32, 1.0);
+        c->ucb32_valid = true;
+    }
+    float2 *b32 = O32::eo_field(c, 0), *e32 = O32::eo_field(c, 1), *r32 = O32::eo_field(c, 2), *p32 = O32::eo_field(c, 3),
+           *u32 = O32::eo_field(c, 4), *t32 = O32::eo_field(c, 5);
+    int rc, total = 0, outer = 0, conv = LGT_OK;
+    CU(cudaMemsetAsync(x, 0, n * sizeof(double2), c->stream));
+    CU(cudaMemcpyAsync(r, b, n * sizeof(double2), cudaMemcpyDeviceToDevice, c->stream));
+    if ((rc = O64::redot(c, b, b, c->scal + 3, n)) != LGT_OK) return rc;
+    CU(cudaMemcpyAsync(c->h_scal + 3, c->scal + 3, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    const double bb = c->h_scal[3];
+    double rr = bb;
+    while (bb > 0.0 && rr > tol * tol * bb) {
+        if (total >= max_iter || outer >= 40) {
+            conv = LGT_ENOCONV;
+            break;
+        }
+        const double scale = 1.0 / sqrt(rr);
+        LAUNCH(c, LGT_K_CG_BLAS, down_convert_kernel, nb, 256, n, (const double2*)r, b32, scale);
+        double eps = 0.25 * tol * sqrt(bb / rr);
+        if (eps < c->inner_tol) eps = c->inner_tol;
+        int it = 0;
+        rc = O32::eo_cg(c, b32, e32, r32, p32, u32, t32, eps, max_iter - total, &it, nullptr);
+        if (rc != LGT_OK && rc != LGT_ENOCONV) return rc;
+        total += it;
+        outer++;
+        LAUNCH(c, LGT_K_CG_BLAS, up_axpy_kernel, nb, 256, n, (double2*)x, (const float2*)e32, 1.0 / scale);
+        if ((rc = O64::eo_mhat(c, (const double2*)x, (double2*)u, (double2*)t_o, 0)) != LGT_OK) return rc;
+        if ((rc = O64::eo_mhat(c, (const double2*)u, (double2*)q, (double2*)t_o, 1)) != LGT_OK) return rc;
+        LAUNCH(c, LGT_K_CG_BLAS, residual_kernel, nb, 256, n, (const double2*)b, (const double2*)q, (double2*)r, c->scal + 3, c->partials, c->counter);
+        CU(cudaMemcpyAsync(c->h_scal + 3, c->scal + 3, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+        CU(cudaStreamSynchronize(c->stream));
+        rr = c->h_scal[3];
+    }
+    c->last_outer = outer;
+    if (iters) *iters = total;
+    if (conv != LGT_OK) return fail(c, LGT_ENOCONV, "mixed-precision even/odd CG did not reach the tolerance");
     return LGT_OK;
 }
 
@@ -858,6 +929,8 @@ int lgt_destroy(lgt_ctx* c) {
     cudaFree(c->F3);
     cudaFree(c->F4);
     cudaFree(c->eo);
+    cudaFree(c->Ucb32);
+    cudaFree(c->eo32);
     for (int i = 0; i < 5; i++) cudaFree(c->ws32[i]);
     cudaFree(c->stage);
     cudaFree(c->partials);
@@ -928,6 +1001,7 @@ int lgt_set_links(lgt_ctx* c, const void* U) {
     c->usm_valid = false;
     if (c->dd_links_valid) *c->dd_links_valid = false;
     c->ucb_valid = false;
+    c->ucb32_valid = false;
     return DISPATCH(c, to_native, c, U, c->U, 36);
 }
 int lgt_get_links(lgt_ctx* c, void* U) {
@@ -1268,6 +1342,7 @@ int lgt_hmc_trajectory(lgt_ctx* c, int nsteps, double dt, double tol, int max_it
     c->usm_valid = false;
     if (c->dd_links_valid) *c->dd_links_valid = false;
         c->ucb_valid = false;
+    c->ucb32_valid = false;
     }
     CU(cudaStreamSynchronize(c->stream));
     if (dH) *dH = d;
@@ -1289,6 +1364,7 @@ int lgt_set_smearing(lgt_ctx* c, int n_levels, double rho) {
     if (c->dd_links_valid) *c->dd_links_valid = false;
     c->u32_valid = false;
     c->ucb_valid = false;
+    c->ucb32_valid = false;
     return LGT_OK;
 }
 int lgt_get_smeared_links(lgt_ctx* c, void* U) {

@@ -282,6 +282,35 @@ def test_eo_cg_force_and_action(lgt, dims, kappa):
     lat.close()
 
 
+def test_eo_mixed_precision_solver(lgt):
+    """Even/odd action with the mixed-precision solver (fp32 CG on the Schur complement, fp64 defect correction on the
+    true residual): same force and action as the oracle's fp64 solve, and through a links change (stale fp32 copies)."""
+    dims, kappa, tol = (8, 8, 8, 8), 0.12, 1e-12
+    V = synth.volume(dims)
+    U = synth.warm_links(dims, 0.3, 47)
+    phi = oeo.mhat(dims, kappa, BC, U, oeo.keep(synth.gaussian_spinor(dims, 48), dims, 0), dagger=True)
+    F_ref, it_ref, _ = oeo.fermion_force(dims, kappa, BC, U, phi, tol, 10 * V)
+    lat = lgt.Lattice(dims, 5.5, kappa, BC)
+    lat.set_links(U)
+    lat.set_pseudofermion(phi)
+    lgt.lgt_set_fermion_action(lat.ctx, lgt.LGT_ACTION_EO)
+    lgt.lgt_set_solver(lat.ctx, lgt.LGT_SOLVER_MIXED_CG, 1e-5)
+    F, it = lat.fermion_force(None, None, tol=tol, max_iter=10 * V)
+    assert 0 < it < 2 * it_ref + 20  # fp32 iterations in total
+    e, plain = link_rel_err(F, F_ref)
+    assert e < 1e-10, (e, plain)
+    _, S_F, _, _ = lgt.lgt_action(lat.ctx, tol, 10 * V)
+    S_ref = oeo.action(dims, kappa, BC, U, phi, tol, 10 * V)[0]
+    assert abs(S_F - S_ref) < 1e-11 * abs(S_ref)
+    # new links: the fp32 checkerboard copy must follow
+    U2 = synth.warm_links(dims, 0.25, 49)
+    lat.set_links(U2)
+    F2, _ = lat.fermion_force(None, None, tol=tol, max_iter=10 * V)
+    F2_ref, _, _ = oeo.fermion_force(dims, kappa, BC, U2, phi, tol, 10 * V)
+    assert link_rel_err(F2, F2_ref)[0] < 1e-10
+    lat.close()
+
+
 def test_eo_leapfrog_conserves_energy(lgt):
     """Leapfrog with the even/odd action on 8^4: |dH| ~ dt^2 and exact reversibility (pin P7 on this action)."""
     dims, beta, kappa = (8, 8, 8, 8), 5.6, 0.12
