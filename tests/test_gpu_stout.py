@@ -181,3 +181,31 @@ def test_smearing_with_solver_variants_and_fp32(lgt):
     F32, _ = lat32.fermion_force(X.astype(np.complex64), Y.astype(np.complex64))
     assert link_rel_err(F32.astype(np.complex128), F_ref)[0] < 2e-4  # fp32 inputs and a deeper chain than the thin force
     lat32.close()
+
+
+def test_paper_second_hmc_setup(lgt):
+    """6^4, Wilson fermions on stout links (rho = 0.3), Sexton-Weingarten with 10 inner gauge steps.
+    A few HMC trajectories from a warm start: |dH| small and shrinking like dt^2 between two step sizes on the same
+    (seed, trajectory), trajectories accepted, links stay SU(3)."""
+    dims, beta, kappa = (6, 6, 6, 6), 5.6, 0.11
+    U0 = synth.warm_links(dims, 0.25, 451)
+    lat = lgt.Lattice(dims, beta, kappa, BC)
+    lgt.lgt_set_smearing(lat.ctx, 1, RHO)
+    lgt.lgt_set_integrator(lat.ctx, lgt.LGT_INT_SEXTON_WEINGARTEN, 10)
+    dH = {}
+    for nsteps, dt in ((5, 0.04), (10, 0.02)):
+        lat.set_links(U0)
+        d, acc, its, H0, ok = lgt.lgt_hmc_trajectory(lat.ctx, nsteps, dt, 451, 0, tol=1e-11, max_iter=5000)
+        assert ok and its > 0
+        dH[nsteps] = d
+    assert abs(dH[5]) < 1.0 and 2.5 < dH[5] / dH[10] < 6.0, dH
+    lat.set_links(U0)
+    accs = []
+    for traj in range(4):
+        d, acc, _, _, ok = lgt.lgt_hmc_trajectory(lat.ctx, 10, 0.02, 452, traj, tol=1e-11, max_iter=5000)
+        assert ok and abs(d) < 0.5
+        accs.append(acc)
+    assert sum(accs) >= 3
+    U = lat.get_links()
+    assert np.abs(U @ U.conj().swapaxes(-1, -2) - np.eye(3)).max() < 1e-12
+    lat.close()
