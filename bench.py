@@ -41,7 +41,7 @@ FLOPS = dict(dslash=1368, dslash_fused_r=1368 + 96, cg_update_xp=96, cg_iter=2 *
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel from the ncu --set full capture
 # summarised in profiles/ (None until captured for the current kernel).
-NCU_TRAFFIC_BYTES = {"dslash_f64_32^4": 1019435008}  # profiles/r01b_ncu_full.md, dslash_kernel<double,0,1>
+NCU_TRAFFIC_BYTES = {"dslash_f64_32^4": 1020500000}  # profiles/r01e_ncu_cg.md, dslash_kernel<double,0,1>: 1.0205 GB
 
 
 # even/odd action, per site of the FULL lattice: a half-lattice hop reads 8 links + 1 spinor and writes 1 spinor per
@@ -50,8 +50,12 @@ REALS_EO = dict(hop=(2 * (72 + 12 + 12)) // 2, hop_fused_r=(2 * (72 + 12 + 2 * 1
 REALS_EO["cg_iter"] = 3 * REALS_EO["hop"] + REALS_EO["hop_fused_r"] + REALS_EO["update_xp"]   # -> 3408 B fp64
 
 
-def step_reals(cg_iters, solver="cg", action="full"):
-    fixed = REALS["gauge_force"] + REALS["fermion_force"] + REALS["link_update"]
+# one stout level, forward (staples -> A, exp(A) U -> U') and backward (local: A, F' rw, G; chain: U, G, Fdir, out rw)
+REALS_STOUT_LEVEL = (2 * 36 + 32) + (32 + 2 * 2 * 36) + (32 + 2 * 32 + 32) + (2 * 36 + 32 + 32 + 2 * 32)
+
+
+def step_reals(cg_iters, solver="cg", action="full", smear=0):
+    fixed = REALS["gauge_force"] + REALS["fermion_force"] + REALS["link_update"] + smear * REALS_STOUT_LEVEL
     if action == "eo":  # CG on M^dag M, then Y_e = M X_e, X_o, Y_o (3 hops), split of phi and two merges (5 x 24 x 2)
         return fixed + cg_iters * REALS_EO["cg_iter"] + 3 * REALS_EO["hop"] + 5 * 48
     if solver == "mixed":  # fp32 iterations move half the bytes; about 4 fp64 defect-correction cycles of 2 Dslash + 3 BLAS-1
@@ -189,6 +193,8 @@ def run_ours(args):
     stream = torch.cuda.current_stream().cuda_stream
     lat = lgt.Lattice(dims, beta, kappa, bc, lgt.LGT_F64, local, stream)
     ctx = lat.ctx
+    if args.smear:
+        lgt.lgt_set_smearing(ctx, args.smear, 0.3)  # rho = 0.3
     hU, hP = torch.from_numpy(U).pin_memory(), torch.from_numpy(P).pin_memory()
     d_eta, d_phi = lat.to_device(eta), lat.empty(V, 4, 3)
     lgt.lgt_set_links_host(ctx, hU)
@@ -215,7 +221,7 @@ def run_ours(args):
         lgt.lgt_set_solver(ctx, lgt.LGT_SOLVER_MIXED_CG, 1e-5)
     if args.action == "eo":
         lgt.lgt_set_fermion_action(ctx, lgt.LGT_ACTION_EO)
-    variant = args.solver != "cg" or args.action != "full"
+    variant = args.solver != "cg" or args.action != "full" or args.smear > 0
     reset_state()
     for _ in range(args.warmup):
         md_step()
@@ -238,7 +244,7 @@ def run_ours(args):
     launches = lgt.lgt_launch_count(ctx) - launches0
     per_class = {name: lgt.lgt_timing_read(ctx, k) for k, name in enumerate(lgt.KERNEL_CLASSES)}
     lgt.lgt_timing_reset(ctx)
-    total_reals = sum(step_reals(i, args.solver, args.action) for i in iters) * V
+    total_reals = sum(step_reals(i, args.solver, args.action, args.smear) for i in iters) * V
     total_flops = sum(step_flops(i) for i in iters) * V
 
     # ---- end to end: host buffers in, host buffers out, through the C ABI, every step
@@ -253,7 +259,7 @@ def run_ours(args):
         lgt.lgt_get_momenta_host(ctx, hP_out)
     torch.cuda.synchronize()
     e2e_s = time.perf_counter() - t0
-    e2e_reals = sum(step_reals(i, args.solver, args.action) for i in e2e_iters) * V
+    e2e_reals = sum(step_reals(i, args.solver, args.action, args.smear) for i in e2e_iters) * V
     h2d = hU.numel() * 16 + hP.numel() * 16 + hphi.numel() * 16
     d2h = hU_out.numel() * 16 + hP_out.numel() * 16
 
@@ -319,6 +325,7 @@ def run_ours(args):
             if dims[3] % nr or (dims[0] * dims[1] * dims[2]) % 32:
                 continue
             dd = lgt.DecomposedLattice(dims, nr, list(range(nr)), beta, kappa, bc, lgt.LGT_F64, local, stream)
+            lgt.lgt_dd_set_halo_mode(dd.d, lgt.LGT_DD_PUSH)  # halos stored by the Dslash kernels themselves
 
             def dd_reset():
                 dd.set_links(U_np)
@@ -340,8 +347,8 @@ def run_ours(args):
             torch.cuda.synchronize()
             extras["decomposed_%d_slabs_one_gpu" % nr] = {
                 "ms_per_step": round(a.elapsed_time(b) / 2, 3), "cg_iters_per_step": dd_iters,
-                "note": "same MD step through lgt_dd_* with %d time slab(s) resident on this GPU: the cost of the ghost "
-                        "slices, halo copies and split reductions, not a multi-GPU number" % nr}
+                "note": "same MD step through lgt_dd_* (LGT_DD_PUSH) with %d time slab(s) resident on this GPU: the cost of the "
+                        "ghost slices, pushed halos and split reductions, not a multi-GPU number" % nr}
             dd.close()
             del dd
 
@@ -460,7 +467,7 @@ def run_ours(args):
                                "fermion force] + drift(dt)" % (args.config, "x".join(map(str, dims))),
                    "beta": beta, "kappa": kappa, "bc": list(bc), "dt": dt, "cg_tol": tol,
                    "cg_iters_per_step": iters, "parallelism": "replicas x%d" % world,
-                   "solver": args.solver, "fermion_action": args.action,
+                   "solver": args.solver, "fermion_action": args.action, "stout_levels": args.smear,
                    "l2": "inputs exceed L2 (links 604 MB, each spinor 201 MB at 32^4)"},
         "gflops": round(total_flops / (elapsed_ms * 1e-3) / 1e9, 1),
         "clocks": clocks,
@@ -542,7 +549,7 @@ def run_decomposed(args):
     max_iter = 10 * V
     U, P, eta = make_inputs(cfg)  # every rank draws the same global fields and keeps its slab
     stream = torch.cuda.current_stream().cuda_stream
-    dd = dist.decomposed_lattice(dims, beta, kappa, bc, lgt.LGT_F64, local, stream)
+    dd = dist.decomposed_lattice(dims, beta, kappa, bc, lgt.LGT_F64, local, stream, halo=args.halo)
     lo, hi = dist.slab_rows(dims, world, rank)
     hU, hP = torch.from_numpy(U[lo:hi].copy()).pin_memory(), torch.from_numpy(P[lo:hi].copy()).pin_memory()
     ctx = dd.ranks[0]
@@ -605,7 +612,7 @@ def run_decomposed(args):
             "config": {"workload": "configs[%d]: ONE %s SU(3) lattice in %d time slabs, one MD step = kick(dt) + drift(dt), "
                                    "CG 1e-12" % (args.config, "x".join(map(str, dims)), world),
                        "beta": beta, "kappa": kappa, "bc": list(bc), "dt": dt, "cg_tol": tol, "cg_iters_per_step": iters,
-                       "parallelism": "dd%d (time slabs, NCCL halo exchange + all-reduce)" % world,
+                       "parallelism": "dd%d (time slabs, halo %s, NCCL all-reduce)" % (world, args.halo),
                        "l2": "inputs exceed L2 at 32^4 up to 8 slabs (links 604 MB / N per rank)"},
             "clocks": clocks,
             "e2e": {"value": round(e2e_reals * 8 / e2e_s / 1e9, 1), "unit": "GB/s", "steps": k_e2e,
@@ -657,6 +664,11 @@ def main():
                     help="non-default: time the step with the mixed-precision solver (not the headline configuration)")
     ap.add_argument("--action", default="full", choices=["full", "eo"],
                     help="non-default: time the step with the even/odd preconditioned action (not the headline configuration)")
+    ap.add_argument("--halo", default="exchange", choices=["exchange", "push"],
+                    help="--parallelism dd: NCCL send/recv of the halo slices, or halos stored into the neighbours' ghost "
+                         "slices by the Dslash kernels (CUDA IPC between processes)")
+    ap.add_argument("--smear", type=int, default=0,
+                    help="non-default: the fermions see this many levels of stout-smeared links (rho = 0.3); not the headline")
     ap.add_argument("--skip-extras", action="store_true", help="profiling runs only: leave the non-headline solver arms out")
     ap.add_argument("--parallelism", default="replicas", choices=["replicas", "dd"],
                     help="N > 1: 'replicas' = N independent lattices (default, weak scaling); 'dd' = ONE lattice cut into N "

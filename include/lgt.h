@@ -217,6 +217,20 @@ const char* lgt_dd_last_error(const lgt_dd* d);
  * torch.distributed), every process calls lgt_dd_nccl_init on its one-rank group.  libnccl.so.2 is opened at run time. */
 int lgt_dd_nccl_unique_id(void* id128);
 int lgt_dd_nccl_init(lgt_dd* d, const void* id128);
+/* How the halo slices of the CG fields travel:
+ *   LGT_DD_EXCHANGE (default): a separate exchange (NCCL send/recv, or device copies between local ranks) before
+ *     every Dslash;
+ *   LGT_DD_PUSH: fused into the producing kernels -- the Dslash kernels of the CG loop store the results of a slab's
+ *     first / last interior slice straight into the neighbour's ghost slice (peer memory), the ghost slices of the
+ *     search direction follow by local arithmetic, and the all-reduce that follows each Dslash anyway is the barrier:
+ *     no separate transfer inside the iteration.  Same iterates bit for bit.  Between processes the neighbours'
+ *     buffers are mapped with CUDA IPC: every rank exports 128 bytes (lgt_dd_ipc_export, HOST buffer), the caller
+ *     all-gathers them, every rank imports the handles of ranks r-1 and r+1 (lgt_dd_ipc_import), then switches mode.
+ *     Ranks that share a process need no import.  LGT_ESTATE if a neighbour's buffers are not reachable. */
+enum { LGT_DD_EXCHANGE = 0, LGT_DD_PUSH = 1 };
+int lgt_dd_set_halo_mode(lgt_dd* d, int mode);
+int lgt_dd_ipc_export(lgt_dd* d, void* handles128);
+int lgt_dd_ipc_import(lgt_dd* d, const void* lo_handles128, const void* hi_handles128);
 int lgt_dd_local_ranks(const lgt_dd* d);
 lgt_ctx* lgt_dd_rank(lgt_dd* d, int local_index);
 /* The decomposed forms of lgt_dslash, lgt_cg, lgt_action, lgt_md_kick, lgt_md_drift, lgt_md_trajectory (leapfrog):

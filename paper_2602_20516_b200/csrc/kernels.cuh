@@ -330,11 +330,28 @@ __device__ __forceinline__ void hop_bwd(const Geom& g, const typename Vec2<T>::t
 //           (cg_scalars_kernel<2> finishes beta, the iteration count and the stop test).  q never touches HBM.
 // In the CG modes the convergence flag is loaded first but tested only after the first hop's loads are in
 // flight, so that its latency is not paid at the head of every block.
-template <class T, int DAG, int MODE>
+// PUSH (time slab of a decomposed lattice, CG modes): a site of the slab's first / last interior time slice also stores
+// its result -- t in MODE 1, the updated r in MODE 2 -- straight into the ghost slice of the neighbour rank's copy of
+// that field (peer memory: NVLink stores, or the other slab's buffer when the ranks share a device), so the halo
+// transfer rides inside the producing kernel and the all-reduce that follows it anyway is the barrier.
+template <class T> struct PushTo {
+    typename Vec2<T>::type* lo = nullptr;  // the field of rank r - 1 (its upper ghost slice receives our first interior slice)
+    typename Vec2<T>::type* hi = nullptr;  // the field of rank r + 1 (its lower ghost slice receives our last interior slice)
+    int lt_loc = 0;                        // interior time slices per slab
+};
+template <class T, int PUSH>
+__device__ __forceinline__ void push_halo(const Geom& g, const PushTo<T>& to, int s, int k, cx<T> v) {
+    if (!PUSH) return;
+    const int V3 = g.stride[3];
+    if (s < 2 * V3) stc<T>(spinor_at(to.lo, s + to.lt_loc * V3) + k * W, v);
+    if (s >= to.lt_loc * V3) stc<T>(spinor_at(to.hi, s - to.lt_loc * V3) + k * W, v);
+}
+
+template <class T, int DAG, int MODE, int PUSH = 0>
 __global__ void __launch_bounds__(128, 1) dslash_kernel(Geom g, const typename Vec2<T>::type* __restrict__ U,
                                                         const typename Vec2<T>::type* __restrict__ in,
                                                         typename Vec2<T>::type* __restrict__ out, T kappa, CgState* st,
-                                                        double* partials, typename Vec2<T>::type* __restrict__ r) {
+                                                        double* partials, typename Vec2<T>::type* __restrict__ r, PushTo<T> push) {
     const int done = (MODE != 0) ? st->done : 0;
     const int s = g.s_begin + swizzled_chunk(g, blockIdx.x) * blockDim.x + threadIdx.x;
     double nrm = 0.0;
@@ -372,6 +389,7 @@ __global__ void __launch_bounds__(128, 1) dslash_kernel(Geom g, const typename V
                 rv.re = fma(-alpha, q.re, rv.re);
                 rv.im = fma(-alpha, q.im, rv.im);
                 stc<T>(br + k * W, rv);
+                push_halo<T, PUSH>(g, push, s, k, rv);
                 nrm += (double)rv.re * (double)rv.re + (double)rv.im * (double)rv.im;
             }
         } else {
@@ -381,12 +399,13 @@ __global__ void __launch_bounds__(128, 1) dslash_kernel(Geom g, const typename V
                 cx<T> pv = ldc<T>(bi + k * W);
                 cx<T> o = mk<T>(fma(-kappa, acc[k].re, pv.re), fma(-kappa, acc[k].im, pv.im));
                 stc<T>(bo + k * W, o);
+                push_halo<T, PUSH>(g, push, s, k, o);
                 if (MODE == 1) nrm += (double)o.re * (double)o.re + (double)o.im * (double)o.im;
             }
         }
     } else {
         if (MODE != 0 && done) return;
-        if (s < g.Vs && MODE != 2) {
+        if (s >= g.V && s < g.Vs && MODE != 2) {  // padding lanes only, never a ghost slice
             typename Vec2<T>::type* bo = spinor_at(out, s);
 #pragma unroll
             for (int k = 0; k < 12; k++) stc<T>(bo + k * W, mk<T>(0, 0));
@@ -448,6 +467,23 @@ __global__ void __launch_bounds__(256) cg_update_xp_kernel(size_t n, typename Ve
             pv.y = fma(beta, pv.y, rv.y);
             p[i] = pv;
         }
+    }
+}
+
+// Decomposed lattice with pushed halos: the ghost slices of p follow the owner's update p = r + beta p from the ghost
+// copy of r (bitwise the owner's arithmetic), so p never travels.  n complex numbers from each of the two ghost slices.
+template <class T>
+__global__ void __launch_bounds__(256) cg_update_p_ghost_kernel(size_t n, size_t hi_offset, typename Vec2<T>::type* __restrict__ p,
+                                                                const typename Vec2<T>::type* __restrict__ r, const CgState* st,
+                                                                int iteration) {
+    if (st->iter != iteration || st->done) return;
+    const T beta = (T)st->beta;
+    for (size_t j = blockIdx.x * (size_t)blockDim.x + threadIdx.x; j < 2 * n; j += (size_t)gridDim.x * blockDim.x) {
+        const size_t i = j < n ? j : hi_offset + (j - n);
+        typename Vec2<T>::type pv = p[i], rv = __ldg(r + i);
+        pv.x = fma(beta, pv.x, rv.x);
+        pv.y = fma(beta, pv.y, rv.y);
+        p[i] = pv;
     }
 }
 

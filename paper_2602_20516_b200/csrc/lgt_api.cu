@@ -208,10 +208,19 @@ template <class T> struct Ops {
     }
 
     // mode 0: out = D in / D^dag in; 1: CG "t = D p" (+ pAp, alpha); 2: CG "q = D^dag t" fused with the x, r update
-    static int dslash(lgt_ctx* c, const void* U, const void* in, void* out, int dagger, int mode, void* r = nullptr) {
+    static int dslash(lgt_ctx* c, const void* U, const void* in, void* out, int dagger, int mode, void* r = nullptr,
+                      const PushTo<T>* push = nullptr) {
         const int grid = site_blocks(c, 128);
         const T kappa = (T)c->kappa;
-#define DSLASH_ARGS c->g, (const T2*)U, (const T2*)in, (T2*)out, kappa, c->st, c->partials, (T2*)r
+#define DSLASH_ARGS c->g, (const T2*)U, (const T2*)in, (T2*)out, kappa, c->st, c->partials, (T2*)r, PushTo<T>()
+        if (push && mode == 1) {
+            LAUNCH(c, LGT_K_DSLASH, (dslash_kernel<T, 0, 1, 1>), grid, 128, c->g, (const T2*)U, (const T2*)in, (T2*)out, kappa, c->st, c->partials, (T2*)r, *push);
+            return LGT_OK;
+        }
+        if (push && mode == 2) {
+            LAUNCH(c, LGT_K_DSLASH_R, (dslash_kernel<T, 1, 2, 1>), grid, 128, c->g, (const T2*)U, (const T2*)in, (T2*)out, kappa, c->st, c->partials, (T2*)r, *push);
+            return LGT_OK;
+        }
         if (mode == 0) {
             if (dagger)
                 LAUNCH(c, LGT_K_DSLASH, (dslash_kernel<T, 1, 0>), grid, 128, DSLASH_ARGS);

@@ -63,6 +63,11 @@ struct lgt_dd {
     cudaStream_t stream = nullptr;
     bool links_ghost_valid = false;
     void* comm = nullptr;  // ncclComm_t; null: every rank is local
+    // LGT_DD_PUSH: halos of the CG fields t (ws[3]) and r (ws[1]) are stored into the neighbours' ghost slices by the
+    // producing kernels.  Neighbours in other processes: their buffers mapped through CUDA IPC, [field r, t][lo, hi].
+    int halo_mode = 0;
+    void* ipc_peer[2][2] = {{nullptr, nullptr}, {nullptr, nullptr}};
+    bool ipc_open[2][2] = {{false, false}, {false, false}};
     std::string err;
 };
 
@@ -202,6 +207,31 @@ template <class T> struct DdOps {
         }
         if ((rc = allreduce_tmp(d)) != LGT_OK) return rc;
         for (int i = 0; i < n; i++) LAUNCH(d->rk[i], LGT_K_CG_BLAS, (cg_apply_kernel<0>), 1, 1, d->rk[i]->st);
+        const bool push = d->halo_mode == LGT_DD_PUSH;
+        std::vector<PushTo<T>> push_t(n), push_r(n);
+        if (push) {
+            // r = p = b on the ghost slices too (one ordinary exchange of b); from here on p's ghosts follow by local
+            // arithmetic and the ghosts of t and r are written by the neighbours' Dslash kernels
+            if ((rc = exchange_spinor(d, ib)) != LGT_OK) return rc;
+            const size_t slice = (size_t)12 * d->V3, hi = (size_t)(d->Lt_loc + 1) * slice;
+            for (int i = 0; i < n; i++) {
+                lgt_ctx* c = d->rk[i];
+                const T2* b = (const T2*)(ib == 6 ? c->phi : c->ws[ib]);
+                for (int f = 1; f <= 2; f++) {
+                    DD_CU(cudaMemcpyAsync((T2*)c->ws[f], b, slice * sizeof(T2), cudaMemcpyDeviceToDevice, d->stream));
+                    DD_CU(cudaMemcpyAsync((T2*)c->ws[f] + hi, b + hi, slice * sizeof(T2), cudaMemcpyDeviceToDevice, d->stream));
+                }
+                const int r = d->rank_of[i];
+                const int dn = dd_local_index(d, (r + d->nranks - 1) % d->nranks), up = dd_local_index(d, (r + 1) % d->nranks);
+                push_r[i].lo = (T2*)(dn >= 0 ? d->rk[dn]->ws[1] : d->ipc_peer[0][0]);
+                push_r[i].hi = (T2*)(up >= 0 ? d->rk[up]->ws[1] : d->ipc_peer[0][1]);
+                push_t[i].lo = (T2*)(dn >= 0 ? d->rk[dn]->ws[3] : d->ipc_peer[1][0]);
+                push_t[i].hi = (T2*)(up >= 0 ? d->rk[up]->ws[3] : d->ipc_peer[1][1]);
+                push_r[i].lt_loc = push_t[i].lt_loc = d->Lt_loc;
+                if (!push_r[i].lo || !push_r[i].hi || !push_t[i].lo || !push_t[i].hi)
+                    return dd_fail(d, LGT_ESTATE, "LGT_DD_PUSH: the neighbours' buffers are not mapped (lgt_dd_ipc_import)");
+            }
+        }
         lgt_ctx* c0 = d->rk[0];
         int launched = 0;
         for (;;) {
@@ -212,18 +242,18 @@ template <class T> struct DdOps {
             if (chunk > 8) chunk = 8;
             if (chunk <= 0) chunk = 1;
             for (int it = 0; it < chunk; it++) {
-                if ((rc = exchange_spinor(d, 2)) != LGT_OK) return rc;  // p
+                if (!push && (rc = exchange_spinor(d, 2)) != LGT_OK) return rc;  // p
                 for (int i = 0; i < n; i++) {
                     lgt_ctx* c = d->rk[i];
-                    DD_RK(i, O::dslash(c, c->U, c->ws[2], c->ws[3], 0, 1));  // t = D p, partials of |t|^2
+                    DD_RK(i, O::dslash(c, c->U, c->ws[2], c->ws[3], 0, 1, nullptr, push ? &push_t[i] : nullptr));  // t = D p, partials of |t|^2
                     LAUNCH(c, LGT_K_CG_BLAS, cg_partial_sum_kernel, 1, 1024, site_blocks(c, 128), c->partials, c->st);
                 }
                 if ((rc = allreduce_tmp(d)) != LGT_OK) return rc;
                 for (int i = 0; i < n; i++) LAUNCH(d->rk[i], LGT_K_CG_BLAS, (cg_apply_kernel<1>), 1, 1, d->rk[i]->st);
-                if ((rc = exchange_spinor(d, 3)) != LGT_OK) return rc;  // t
+                if (!push && (rc = exchange_spinor(d, 3)) != LGT_OK) return rc;  // t
                 for (int i = 0; i < n; i++) {
                     lgt_ctx* c = d->rk[i];
-                    DD_RK(i, O::dslash(c, c->U, c->ws[3], nullptr, 1, 2, c->ws[1]));  // r -= alpha D^dag t, partials of |r|^2
+                    DD_RK(i, O::dslash(c, c->U, c->ws[3], nullptr, 1, 2, c->ws[1], push ? &push_r[i] : nullptr));  // r -= alpha D^dag t, partials of |r|^2
                     LAUNCH(c, LGT_K_CG_BLAS, cg_partial_sum_kernel, 1, 1024, site_blocks(c, 128), c->partials, c->st);
                 }
                 if ((rc = allreduce_tmp(d)) != LGT_OK) return rc;
@@ -233,6 +263,11 @@ template <class T> struct DdOps {
                     LAUNCH(c, LGT_K_CG_BLAS, (cg_apply_kernel<2>), 1, 1, c->st);
                     LAUNCH(c, LGT_K_CG_BLAS, (cg_update_xp_kernel<T>), stream_blocks(c, cnt), 256, cnt, (T2*)c->ws[0] + off, (T2*)c->ws[2] + off,
                            (const T2*)c->ws[1] + off, c->st, launched + it + 1);
+                    if (push) {
+                        const size_t slice = (size_t)12 * d->V3;
+                        LAUNCH(c, LGT_K_CG_BLAS, (cg_update_p_ghost_kernel<T>), stream_blocks(c, 2 * slice), 256, slice,
+                               (size_t)(d->Lt_loc + 1) * slice, (T2*)c->ws[2], (const T2*)c->ws[1], c->st, launched + it + 1);
+                    }
                 }
             }
             launched += chunk;
@@ -326,6 +361,9 @@ int lgt_dd_destroy(lgt_dd* d) {
     DeviceGuard guard(d->device);
     cudaStreamSynchronize(d->stream);
     if (d->comm && g_nccl.CommDestroy) g_nccl.CommDestroy(d->comm);
+    for (int f = 0; f < 2; f++)
+        for (int sd = 0; sd < 2; sd++)
+            if (d->ipc_open[f][sd]) cudaIpcCloseMemHandle(d->ipc_peer[f][sd]);
     for (lgt_ctx* c : d->rk) lgt_destroy(c);
     delete d;
     return LGT_OK;
@@ -403,6 +441,50 @@ int lgt_dd_nccl_init(lgt_dd* d, const void* id128) {
     memcpy(&id, id128, sizeof id);
     DD_NCCL(g_nccl.CommInitRank(&d->comm, d->nranks, id, d->rank_of[0]));
     d->links_ghost_valid = false;
+    return LGT_OK;
+}
+
+int lgt_dd_set_halo_mode(lgt_dd* d, int mode) {
+    CHECK_DD(d);
+    if (mode != LGT_DD_EXCHANGE && mode != LGT_DD_PUSH) return dd_fail(d, LGT_EINVAL, "lgt_dd_set_halo_mode: unknown mode");
+    if (mode == LGT_DD_PUSH && d->rk.size() != (size_t)d->nranks && d->nranks > 1)
+        for (int f = 0; f < 2; f++)
+            for (int s = 0; s < 2; s++)
+                if (!d->ipc_peer[f][s]) return dd_fail(d, LGT_ESTATE, "lgt_dd_set_halo_mode: LGT_DD_PUSH needs the neighbours' buffers (lgt_dd_ipc_import)");
+    d->halo_mode = mode;
+    return LGT_OK;
+}
+// 2 x 64 bytes: the CUDA IPC handles of this rank's r and t fields (ws[1], ws[3])
+int lgt_dd_ipc_export(lgt_dd* d, void* handles128) {
+    CHECK_DD(d);
+    if (!handles128) return dd_fail(d, LGT_EINVAL, "lgt_dd_ipc_export: null pointer");
+    if (d->rk.size() != 1) return dd_fail(d, LGT_ESTATE, "lgt_dd_ipc_export: one rank per process");
+    static_assert(sizeof(cudaIpcMemHandle_t) == 64, "CUDA IPC handle size");
+    cudaIpcMemHandle_t h[2];
+    DD_CU(cudaIpcGetMemHandle(&h[0], d->rk[0]->ws[1]));
+    DD_CU(cudaIpcGetMemHandle(&h[1], d->rk[0]->ws[3]));
+    memcpy(handles128, h, sizeof h);
+    return LGT_OK;
+}
+int lgt_dd_ipc_import(lgt_dd* d, const void* lo_handles128, const void* hi_handles128) {
+    CHECK_DD(d);
+    if (!lo_handles128 || !hi_handles128) return dd_fail(d, LGT_EINVAL, "lgt_dd_ipc_import: null pointer");
+    if (d->rk.size() != 1 || d->nranks < 2) return dd_fail(d, LGT_ESTATE, "lgt_dd_ipc_import: for one rank per process and at least two ranks");
+    if (d->ipc_peer[0][0]) return dd_fail(d, LGT_ESTATE, "lgt_dd_ipc_import: already imported");
+    cudaIpcMemHandle_t lo[2], hi[2];
+    memcpy(lo, lo_handles128, sizeof lo);
+    memcpy(hi, hi_handles128, sizeof hi);
+    const bool same_peer = d->nranks == 2;  // both neighbours are the one other rank: map its buffers once
+    for (int f = 0; f < 2; f++) {
+        DD_CU(cudaIpcOpenMemHandle(&d->ipc_peer[f][0], lo[f], cudaIpcMemLazyEnablePeerAccess));
+        d->ipc_open[f][0] = true;
+        if (same_peer) {
+            d->ipc_peer[f][1] = d->ipc_peer[f][0];
+        } else {
+            DD_CU(cudaIpcOpenMemHandle(&d->ipc_peer[f][1], hi[f], cudaIpcMemLazyEnablePeerAccess));
+            d->ipc_open[f][1] = true;
+        }
+    }
     return LGT_OK;
 }
 

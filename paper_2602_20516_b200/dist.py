@@ -76,9 +76,25 @@ def broadcast_bytes(data, nbytes, src=0, device="cpu"):
     return bytes(t.cpu().tolist())
 
 
-def decomposed_lattice(dims, beta, kappa, bc, precision=None, local_device=0, stream=None):
+def allgather_bytes(data, nbytes, device="cpu"):
+    """Every rank passes nbytes bytes; returns the list of all ranks' bytes in rank order."""
+    import torch
+    import torch.distributed as dist
+
+    if not (dist.is_available() and dist.is_initialized()):
+        return [bytes(data)]
+    mine = torch.tensor(list(bytes(data)), dtype=torch.uint8, device=device)
+    assert mine.numel() == nbytes
+    out = [torch.zeros(nbytes, dtype=torch.uint8, device=device) for _ in range(dist.get_world_size())]
+    dist.all_gather(out, mine)
+    return [bytes(t.cpu().tolist()) for t in out]
+
+
+def decomposed_lattice(dims, beta, kappa, bc, precision=None, local_device=0, stream=None, halo="exchange"):
     """This process's slab of ONE lattice shared by all ranks of the default process group: a DecomposedLattice with one
-    local rank whose NCCL communicator is initialised from an id that rank 0 creates and broadcasts here."""
+    local rank whose NCCL communicator is initialised from an id that rank 0 creates and broadcasts here.
+    halo = "push": the neighbours' CG buffers are mapped through CUDA IPC (handles all-gathered here) and the halo
+    slices travel inside the Dslash kernels (lgt.LGT_DD_PUSH)."""
     from . import lgt
 
     rank, world, _ = env_rank_world()
@@ -88,6 +104,11 @@ def decomposed_lattice(dims, beta, kappa, bc, precision=None, local_device=0, st
         ident = lgt.lgt_dd_nccl_unique_id() if rank == 0 else None
         ident = broadcast_bytes(ident, 128, src=0, device="cuda:%d" % local_device)
         lgt.lgt_dd_nccl_init(dd.d, ident)
+        if halo == "push":
+            handles = allgather_bytes(lgt.lgt_dd_ipc_export(dd.d), 128, device="cuda:%d" % local_device)
+            lgt.lgt_dd_ipc_import(dd.d, handles[(rank - 1) % world], handles[(rank + 1) % world])
+    if halo == "push":
+        lgt.lgt_dd_set_halo_mode(dd.d, lgt.LGT_DD_PUSH)
     return dd
 
 

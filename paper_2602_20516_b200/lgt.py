@@ -16,6 +16,7 @@ LGT_F64, LGT_F32 = 0, 1
 LGT_SOLVER_CG, LGT_SOLVER_MIXED_CG = 0, 1
 LGT_ACTION_FULL, LGT_ACTION_EO = 0, 1
 LGT_INT_LEAPFROG, LGT_INT_OMELYAN, LGT_INT_SEXTON_WEINGARTEN = 0, 1, 2
+LGT_DD_EXCHANGE, LGT_DD_PUSH = 0, 1
 
 # every symbol include/lgt.h declares: (restype, argtypes)
 _vp, _i, _d, _l = C.c_void_p, C.c_int, C.c_double, C.c_long
@@ -68,6 +69,9 @@ SYMBOLS = {
     "lgt_dd_last_error": (C.c_char_p, [_vp]),
     "lgt_dd_nccl_unique_id": (_i, [_vp]),
     "lgt_dd_nccl_init": (_i, [_vp, _vp]),
+    "lgt_dd_set_halo_mode": (_i, [_vp, _i]),
+    "lgt_dd_ipc_export": (_i, [_vp, _vp]),
+    "lgt_dd_ipc_import": (_i, [_vp, _vp, _vp]),
     "lgt_dd_local_ranks": (_i, [_vp]),
     "lgt_dd_rank": (_vp, [_vp, _i]),
     "lgt_dd_dslash": (_i, [_vp, C.POINTER(_vp), C.POINTER(_vp), _i]),
@@ -422,6 +426,21 @@ def lgt_dd_nccl_unique_id():
 
 def lgt_dd_nccl_init(d, id128):
     _dd_check(d, lib().lgt_dd_nccl_init(d, C.c_char_p(bytes(id128))))
+
+
+def lgt_dd_set_halo_mode(d, mode):
+    _dd_check(d, lib().lgt_dd_set_halo_mode(d, mode))
+
+
+def lgt_dd_ipc_export(d):
+    """128 bytes: the CUDA IPC handles of this rank's r and t fields."""
+    buf = C.create_string_buffer(128)
+    _dd_check(d, lib().lgt_dd_ipc_export(d, buf))
+    return bytes(buf.raw)
+
+
+def lgt_dd_ipc_import(d, lo_handles, hi_handles):
+    _dd_check(d, lib().lgt_dd_ipc_import(d, C.c_char_p(bytes(lo_handles)), C.c_char_p(bytes(hi_handles))))
 
 
 def lgt_dd_local_ranks(d):

@@ -22,6 +22,8 @@ WORKER = textwrap.dedent("""
     # decomposed mode: the id travels from rank 0, the slabs tile the lattice
     ident = dist.broadcast_bytes(bytes(range(128)) if rank == 0 else None, 128, src=0)
     lo, hi = dist.slab_rows((4, 4, 2, 8), world, rank)
+    gathered = dist.allgather_bytes(bytes([rank + 1] * 16), 16)
+    assert gathered == [bytes([1] * 16), bytes([2] * 16)]
     print(json.dumps({"rank": rank, "times": times, "sums": sums, "u00": [U[0,0,0,0].real, U[0,0,0,0].imag],
                       "value": dist.throughput(sums[0], times[0] * 1e-3), "id": list(ident), "rows": [lo, hi]}))
     dist.shutdown()
@@ -70,6 +72,7 @@ def test_single_process_identity():
     assert t == [3.0] and s == [5.0]
     assert dist.env_rank_world()[1] >= 1
     assert dist.broadcast_bytes(b"abc", 3) == b"abc"
+    assert dist.allgather_bytes(b"xy", 2) == [b"xy"]
     rows = [dist.slab_rows((4, 4, 4, 12), 3, r) for r in range(3)]
     assert rows == [(0, 256), (256, 512), (512, 768)]
     import pytest

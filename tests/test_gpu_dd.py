@@ -178,3 +178,33 @@ def test_dd_full_size_dslash_four_slabs(lgt):
     V3 = dims[0] * dims[1] * dims[2]
     sites = np.array([0, 5, V3 * 8 - 1, V3 * 8, V3 * 16 + 77, V3 * 24 - 3, V - V3 + 9, V - 1], dtype=np.int64)
     assert np.abs(out[sites] - oracle.dslash_sites(dims, kappa, bc, U, psi, sites)).max() < 1e-12
+
+
+@pytest.mark.parametrize("nranks", [1, 2, 4, 8])
+def test_dd_pushed_halos_are_bitwise_the_exchanged_ones(lgt, nranks):
+    """LGT_DD_PUSH: the Dslash kernels of the CG loop store their boundary slices into the neighbours' ghost slices and
+    the ghosts of p follow by local arithmetic; no separate transfer inside the iteration.  Same iterates bit for bit
+    as with the separate exchange, the oracle's iteration count, and the MD trajectory on top of it."""
+    dims, beta, kappa = (4, 4, 2, 8), 5.6, 0.12
+    U = synth.warm_links(dims, 0.3, 561)
+    P0 = synth.gaussian_momenta(dims, 562)
+    b = oracle.dslash(dims, kappa, BC, U, synth.gaussian_spinor(dims, 563), dagger=True)
+    x_ref, it_ref, _, ok = oracle.cg(dims, kappa, BC, U, b, 1e-12, 5000)
+    res = {}
+    for mode in (lgt.LGT_DD_EXCHANGE, lgt.LGT_DD_PUSH):
+        dd = lgt.DecomposedLattice(dims, nranks, list(range(nranks)), beta, kappa, BC)
+        lgt.lgt_dd_set_halo_mode(dd.d, mode)
+        dd.set_links(U)
+        xs, it, rel, ok = dd.cg(b, 1e-12, 5000)
+        assert ok and it == it_ref
+        dd.set_momenta(P0)
+        dd.set_pseudofermion(b)
+        H0, H1, its = lgt.lgt_dd_md_trajectory(dd.d, 2, 0.03, tol=1e-13, max_iter=5000)
+        res[mode] = (cat(xs), cat(dd.get_links()), cat(dd.get_momenta()), H1 - H0, its)
+        dd.close()
+    ex, pu = res[lgt.LGT_DD_EXCHANGE], res[lgt.LGT_DD_PUSH]
+    assert np.array_equal(ex[0], pu[0]) and np.array_equal(ex[1], pu[1]) and np.array_equal(ex[2], pu[2])
+    assert ex[3] == pu[3] and ex[4] == pu[4]
+    assert np.linalg.norm(pu[0] - x_ref) < 1e-10 * np.linalg.norm(x_ref)
+    U_ref, P_ref, its_ref, _ = oracle.trajectory(dims, beta, kappa, BC, U, b, P0, 2, 0.03, tol=1e-13, max_iter=5000)
+    assert pu[4] == its_ref and np.abs(pu[1] - U_ref).max() < 1e-12 and link_rel_err(pu[2], P_ref)[0] < TOL64
