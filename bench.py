@@ -673,7 +673,7 @@ def main():
     ap.add_argument("--parallelism", default="replicas", choices=["replicas", "dd"],
                     help="N > 1: 'replicas' = N independent lattices (default, weak scaling); 'dd' = ONE lattice cut into N "
                          "time slabs with NCCL halo exchange (lgt_dd_*, strong scaling; verified on one GPU only, DESIGN.md)")
-    ap.add_argument("--cpu-sample-iters", type=int, default=4, help="CG iterations in the oracle's bounded sample")
+    ap.add_argument("--cpu-sample-iters", type=int, default=20, help="CG iterations in the oracle's bounded sample")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3  # timing rule: at least 3 warm-up steps
