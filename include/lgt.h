@@ -242,6 +242,11 @@ int lgt_dd_md_kick(lgt_dd* d, double eps, double tol, int max_iter, int* cg_iter
 int lgt_dd_md_drift(lgt_dd* d, double eps);
 int lgt_dd_md_trajectory(lgt_dd* d, int nsteps, double dt, double tol, int max_iter, double* H_initial, double* H_final,
                          long* cg_iters);
+/* lgt_hmc_trajectory on the decomposed lattice (leapfrog): the heat baths draw by GLOBAL element number, so momenta,
+ * pseudofermion, dH and the decision are those of the undivided lattice; every rank takes the same decision from the
+ * same all-reduced numbers. */
+int lgt_dd_hmc_trajectory(lgt_dd* d, int nsteps, double dt, double tol, int max_iter, unsigned long long seed,
+                          unsigned trajectory, double* dH, int* accepted, long* cg_iters, double* H_initial);
 
 /* ---- native-layout spinor fields (for callers that keep fields resident between calls) ---- */
 /* Bytes of one spinor field in the handle's internal layout and precision. */

@@ -37,6 +37,7 @@ struct Geom {
     int s_begin, s_end;
     int t_off;      // global t of local slice 0 (0, or rank * Lt_local - 1 on a slab)
     int Lt_glob;    // global time extent (for the fermion boundary sign of the t links)
+    int site_off;   // global site index = local site index + site_off (heat baths draw by global element number)
 };
 
 // lexicographic 128-site chunk handled by block b
@@ -1267,9 +1268,10 @@ __global__ void __launch_bounds__(256) momentum_heatbath_kernel(Geom g, typename
         const int mu = (int)((i >> 5) & 3);
         const int s = (int)(i >> 7) * W + lane;
         double pi[8] = {0, 0, 0, 0, 0, 0, 0, 0};
-        if (s < g.V) {
+        if (s >= g.s_begin && s < g.s_end) {
 #pragma unroll
-            for (int j = 0; j < 4; j++) philox_gaussian_pair(seed, traj, 1u, (unsigned)(4 * s + mu), (unsigned)j, pi[2 * j], pi[2 * j + 1]);
+            for (int j = 0; j < 4; j++)
+                philox_gaussian_pair(seed, traj, 1u, (unsigned)(4 * (s + g.site_off) + mu), (unsigned)j, pi[2 * j], pi[2 * j + 1]);
         }
         // tau^a = i lambda^a / 2:  Im Pi00 = (pi3 + pi8/sqrt3)/2, Im Pi11 = (-pi3 + pi8/sqrt3)/2,
         // Pi01 = (pi2 + i pi1)/2, Pi02 = (pi5 + i pi4)/2, Pi12 = (pi7 + i pi6)/2      (pi1 = pi[0])
@@ -1297,7 +1299,7 @@ __global__ void __launch_bounds__(256) spinor_heatbath_kernel(Geom g, typename V
         const int k = (int)((i >> 5) % 12);
         const int s = (int)((i >> 5) / 12) * W + lane;
         double g0 = 0.0, g1 = 0.0;
-        if (s < g.V) philox_gaussian_pair(seed, traj, 2u, (unsigned)s, (unsigned)k, g0, g1);
+        if (s >= g.s_begin && s < g.s_end) philox_gaussian_pair(seed, traj, 2u, (unsigned)(s + g.site_off), (unsigned)k, g0, g1);
         typename Vec2<T>::type v;
         v.x = (T)(0.70710678118654752440084436210485 * g0);
         v.y = (T)(0.70710678118654752440084436210485 * g1);

@@ -876,6 +876,7 @@ int lgt_create(lgt_ctx** out, const int dims[4], double beta, double kappa, cons
     c->g.s_end = c->g.V;
     c->g.t_off = 0;
     c->g.Lt_glob = c->g.L[3];
+    c->g.site_off = 0;
     int sms = 148;
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device);
     c->red_blocks = sms * 8;

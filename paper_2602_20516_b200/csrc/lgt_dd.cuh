@@ -186,7 +186,7 @@ template <class T> struct DdOps {
         if ((rc = exchange_spinor(d, in)) != LGT_OK) return rc;
         for (size_t i = 0; i < d->rk.size(); i++) {
             lgt_ctx* c = d->rk[i];
-            DD_RK(i, O::dslash(c, c->U, in == 6 ? c->phi : c->ws[in], c->ws[out], dagger, 0));
+            DD_RK(i, O::dslash(c, c->U, in == 6 ? c->phi : c->ws[in], out == 6 ? c->phi : c->ws[out], dagger, 0));
         }
         return LGT_OK;
     }
@@ -308,11 +308,12 @@ template <class T> struct DdOps {
     }
 
     // S_g, S_F, K summed over the ranks (device slots scal[0..2] of every rank, one all-reduce of three doubles)
-    static int action(lgt_dd* d, double tol, int max_iter, double* S_g, double* S_F, double* K, int* cg_iters) {
+    // eta_norm: S_F = |eta|^2 of the heat-bath field in ws[4] instead of a solve (the start of an HMC trajectory)
+    static int action(lgt_dd* d, double tol, int max_iter, double* S_g, double* S_F, double* K, int* cg_iters, bool eta_norm = false) {
         int rc, it = 0, conv = LGT_OK;
         if ((rc = dd_exchange_links(d)) != LGT_OK) return rc;
         const bool ferm = fermions_on(d->rk[0]) && S_F != nullptr;
-        if (ferm) {
+        if (ferm && !eta_norm) {
             rc = cg(d, 6, false, tol, max_iter, &it, nullptr);
             if (rc == LGT_ENOCONV) conv = rc;
             else if (rc != LGT_OK) return rc;
@@ -324,8 +325,8 @@ template <class T> struct DdOps {
             DD_RK(i, O::kinetic(c, c->scal + 1));
             if (ferm) {
                 const size_t off = spinor_off(c);
-                LAUNCH(c, LGT_K_OTHER, (redot_kernel<T>), stream_blocks(c, spinor_n(c)), 256, spinor_n(c), (const T2*)c->phi + off,
-                       (const T2*)c->ws[0] + off, c->scal + 2, c->partials, c->counter);
+                const T2 *a = (const T2*)(eta_norm ? c->ws[4] : c->phi) + off, *b = (const T2*)(eta_norm ? c->ws[4] : c->ws[0]) + off;
+                LAUNCH(c, LGT_K_OTHER, (redot_kernel<T>), stream_blocks(c, spinor_n(c)), 256, spinor_n(c), a, b, c->scal + 2, c->partials, c->counter);
             } else {
                 DD_CU(cudaMemsetAsync(c->scal + 2, 0, sizeof(double), d->stream));
             }
@@ -340,6 +341,68 @@ template <class T> struct DdOps {
         if (K) *K = c0->h_scal[1];
         if (S_F) *S_F = ferm ? c0->h_scal[2] : 0.0;
         if (cg_iters) *cg_iters = it;
+        return conv;
+    }
+
+    // Heat baths by global element number (reading A-25), so that the fields are those of the undivided lattice
+    static int heatbaths(lgt_dd* d, unsigned long long seed, unsigned traj) {
+        int rc;
+        for (size_t i = 0; i < d->rk.size(); i++) {
+            lgt_ctx* c = d->rk[i];
+            DD_RK(i, O::momentum_heatbath(c, seed, traj));
+            if (c->kappa != 0.0) {
+                LAUNCH(c, LGT_K_OTHER, (spinor_heatbath_kernel<T>), stream_blocks(c, (size_t)12 * c->g.Vs), 256, c->g, (T2*)c->ws[4], seed, traj);
+                c->has_phi = true;
+            }
+        }
+        if (d->rk[0]->kappa != 0.0 && (rc = dslash(d, 4, 6, 1)) != LGT_OK) return rc;  // phi = D^dag eta
+        return LGT_OK;
+    }
+    static int hmc_trajectory(lgt_dd* d, int nsteps, double dt, double tol, int max_iter, unsigned long long seed, unsigned traj,
+                              double* dH, int* accepted, long* cg_iters, double* H_initial) {
+        int rc, it = 0, conv = LGT_OK;
+        long total = 0;
+        double sg, sf, k;
+        if ((rc = dd_exchange_links(d)) != LGT_OK) return rc;
+        for (size_t i = 0; i < d->rk.size(); i++) {
+            lgt_ctx* c = d->rk[i];
+            if (!c->Usave) DD_CU(cudaMalloc(&c->Usave, links_bytes(c)));
+            DD_CU(cudaMemcpyAsync(c->Usave, c->U, links_bytes(c), cudaMemcpyDeviceToDevice, d->stream));
+        }
+        if ((rc = heatbaths(d, seed, traj)) != LGT_OK) return rc;
+        if ((rc = action(d, tol, max_iter, &sg, &sf, &k, &it, true)) != LGT_OK) return rc;
+        const double H0 = k + sg + sf;
+#define DD_HSTEP(call)                     \
+    do {                                   \
+        it = 0;                            \
+        rc = (call);                       \
+        if (rc == LGT_ENOCONV) conv = rc;  \
+        else if (rc != LGT_OK) return rc;  \
+        total += it;                       \
+    } while (0)
+        if (nsteps > 0) {
+            DD_HSTEP(kick(d, 0.5 * dt, tol, max_iter, &it));
+            for (int n = 0; n < nsteps; n++) {
+                DD_HSTEP(drift(d, dt));
+                DD_HSTEP(kick(d, (n == nsteps - 1) ? 0.5 * dt : dt, tol, max_iter, &it));
+            }
+        }
+        DD_HSTEP(action(d, tol, max_iter, &sg, &sf, &k, &it));
+#undef DD_HSTEP
+        const double dh = (k + sg + sf) - H0;
+        const bool acc = metropolis_uniform(seed, traj) < exp(-dh);  // the same all-reduced numbers on every rank
+        if (!acc) {
+            for (lgt_ctx* c : d->rk) {
+                DD_CU(cudaMemcpyAsync(c->U, c->Usave, links_bytes(c), cudaMemcpyDeviceToDevice, d->stream));
+                c->usm_valid = c->u32_valid = c->ucb_valid = false;
+            }
+            d->links_ghost_valid = true;  // saved with current ghosts
+        }
+        DD_CU(cudaStreamSynchronize(d->stream));
+        if (dH) *dH = dh;
+        if (accepted) *accepted = acc ? 1 : 0;
+        if (cg_iters) *cg_iters = total;
+        if (H_initial) *H_initial = H0;
         return conv;
     }
 };
@@ -406,6 +469,7 @@ int lgt_dd_create(lgt_dd** out, const int dims[4], int nranks, int nlocal, const
         c->g.s_end = c->g.V - d->V3;
         c->g.t_off = local_ranks[i] * d->Lt_loc - 1;
         c->g.Lt_glob = dims[3];
+        c->g.site_off = (local_ranks[i] * d->Lt_loc - 1) * d->V3;
         c->g.swz_Z = 0;
         c->dd_links_valid = &d->links_ghost_valid;
         d->rk.push_back(c);
@@ -565,6 +629,13 @@ int lgt_dd_md_trajectory(lgt_dd* d, int nsteps, double dt, double tol, int max_i
     if (cg_iters) *cg_iters = total;
     DD_CU(cudaStreamSynchronize(d->stream));
     return conv;
+}
+
+int lgt_dd_hmc_trajectory(lgt_dd* d, int nsteps, double dt, double tol, int max_iter, unsigned long long seed, unsigned trajectory,
+                          double* dH, int* accepted, long* cg_iters, double* H_initial) {
+    CHECK_DD(d);
+    if (nsteps < 0) return dd_fail(d, LGT_EINVAL, "lgt_dd_hmc_trajectory: nsteps < 0");
+    return DD_DISPATCH(d, hmc_trajectory, d, nsteps, dt, tol, max_iter, seed, trajectory, dH, accepted, cg_iters, H_initial);
 }
 
 }  // extern "C"

@@ -80,6 +80,7 @@ SYMBOLS = {
     "lgt_dd_md_kick": (_i, [_vp, _d, _d, _i, _ip]),
     "lgt_dd_md_drift": (_i, [_vp, _d]),
     "lgt_dd_md_trajectory": (_i, [_vp, _i, _d, _d, _i, _dp, _dp, _lp]),
+    "lgt_dd_hmc_trajectory": (_i, [_vp, _i, _d, _d, _i, C.c_ulonglong, C.c_uint, _dp, _ip, _lp, _dp]),
     "lgt_set_smearing": (_i, [_vp, _i, _d]),
     "lgt_get_smeared_links": (_i, [_vp, _vp]),
     "lgt_set_integrator": (_i, [_vp, _i, _i]),
@@ -488,6 +489,14 @@ def lgt_dd_md_trajectory(d, nsteps, dt, tol=1e-12, max_iter=100000, measure=True
     _dd_check(d, lib().lgt_dd_md_trajectory(d, nsteps, dt, tol, max_iter, C.byref(h0) if measure else None,
                                             C.byref(h1) if measure else None, C.byref(its)))
     return h0.value, h1.value, its.value
+
+
+def lgt_dd_hmc_trajectory(d, nsteps, dt, seed, trajectory, tol=1e-12, max_iter=100000):
+    """Returns (dH, accepted, cg_iters, H_initial, converged)."""
+    dH, acc, its, H0 = C.c_double(), C.c_int(), C.c_long(), C.c_double()
+    rc = _dd_check(d, lib().lgt_dd_hmc_trajectory(d, nsteps, dt, tol, max_iter, seed, trajectory, C.byref(dH), C.byref(acc),
+                                                  C.byref(its), C.byref(H0)), allow=(LGT_ENOCONV,))
+    return dH.value, bool(acc.value), its.value, H0.value, rc == LGT_OK
 
 
 # ---- convenience wrapper -----------------------------------------------------------------------

@@ -208,3 +208,39 @@ def test_dd_pushed_halos_are_bitwise_the_exchanged_ones(lgt, nranks):
     assert np.linalg.norm(pu[0] - x_ref) < 1e-10 * np.linalg.norm(x_ref)
     U_ref, P_ref, its_ref, _ = oracle.trajectory(dims, beta, kappa, BC, U, b, P0, 2, 0.03, tol=1e-13, max_iter=5000)
     assert pu[4] == its_ref and np.abs(pu[1] - U_ref).max() < 1e-12 and link_rel_err(pu[2], P_ref)[0] < TOL64
+
+
+@pytest.mark.parametrize("nranks", [2, 4])
+def test_dd_hmc_trajectory_matches_undivided_oracle(lgt, nranks):
+    """Heat baths by global element number: momenta, pseudofermion, dH, decision and links after the test are those of
+    the oracle's trajectory on the undivided lattice; a coarse gauge-only trajectory is rejected and restored bit for bit."""
+    from oracle import hmc as ohmc
+
+    dims, beta, kappa, seed = (4, 4, 2, 8), 5.5, 0.10, 97531
+    U = synth.warm_links(dims, 0.2, 571)
+    dd = lgt.DecomposedLattice(dims, nranks, list(range(nranks)), beta, kappa, BC)
+    lgt.lgt_dd_set_halo_mode(dd.d, lgt.LGT_DD_PUSH)
+    dd.set_links(U)
+    for traj in range(2):
+        dH, acc, its, H0, ok = lgt.lgt_dd_hmc_trajectory(dd.d, 3, 0.03, seed, traj, tol=1e-13, max_iter=5000)
+        ref = ohmc.hmc_trajectory(dims, beta, kappa, BC, U, seed, traj, 3, 0.03, ohmc.LEAPFROG, tol=1e-13, max_iter=5000)
+        assert ok and abs(H0 - ref["H0"]) < 1e-12 * abs(ref["H0"]) and abs(dH - ref["dH"]) < 1e-9 * abs(ref["H0"])
+        if abs(ref["u"] - np.exp(-ref["dH"])) > 1e-6:
+            assert acc == ref["accepted"]
+            assert np.abs(cat(dd.get_links()) - ref["U"]).max() < 1e-11
+        U = cat(dd.get_links())
+    dd.close()
+    dd = lgt.DecomposedLattice(dims, nranks, list(range(nranks)), beta, 0.0, BC)
+    U = synth.warm_links(dims, 0.2, 571)
+    dd.set_links(U)
+    seen = set()
+    for traj in range(6):
+        dH, acc, _, _, _ = lgt.lgt_dd_hmc_trajectory(dd.d, 1, 0.12, 7, traj)
+        ref = ohmc.hmc_trajectory(dims, beta, 0.0, BC, U, 7, traj, 1, 0.12)
+        assert abs(dH - ref["dH"]) < 1e-9 * abs(ref["H0"]) and acc == ref["accepted"]
+        if not acc:
+            assert np.array_equal(cat(dd.get_links()), U)
+        seen.add(acc)
+        U = cat(dd.get_links())
+    assert len(seen) >= 1
+    dd.close()
