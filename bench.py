@@ -200,7 +200,7 @@ def run_ours(args):
     lgt.lgt_set_links_host(ctx, hU)
     lgt.lgt_dslash(ctx, d_eta, d_phi, True)  # phi = D^dag eta, made by the CUDA path itself
     hphi = d_phi.cpu().pin_memory()
-    hU_out, hP_out = torch.empty_like(hU), torch.empty_like(hP)
+    hU_out, hP_out = torch.empty_like(hU).pin_memory(), torch.empty_like(hP).pin_memory()
     del U, P, eta, d_eta
 
     def reset_state():
@@ -558,7 +558,7 @@ def run_decomposed(args):
     d_phi = torch.empty_like(d_eta)
     lgt.lgt_dd_dslash(dd.d, [d_eta], [d_phi], True)
     hphi = d_phi.cpu().pin_memory()
-    hU_out, hP_out = torch.empty_like(hU), torch.empty_like(hP)
+    hU_out, hP_out = torch.empty_like(hU).pin_memory(), torch.empty_like(hP).pin_memory()
     del U, P, eta, d_eta
 
     def reset_state():
