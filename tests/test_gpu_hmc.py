@@ -166,3 +166,23 @@ def test_hmc_even_odd_mixed_acceptance(lgt):
     assert 0.3 < np.mean(np.exp(-np.array(dHs))) < 3.0
     assert 0.3 < lgt.lgt_plaquette(lat.ctx) < 1.0
     lat.close()
+
+
+def test_pure_gauge_hmc_reproduces_the_known_plaquette(lgt):
+    """End-to-end physics check of heat bath + integrator + Metropolis on the GPU: SU(3) Wilson gauge action at
+    beta = 6.0 thermalises to the textbook mean plaquette 0.5937 (8^4 is within 1e-3 of the infinite-volume value)."""
+    dims, beta = (8, 8, 8, 8), 6.0
+    lat = lgt.Lattice(dims, beta, 0.0, (1, 1, 1, 1))
+    lat.set_links(synth.warm_links(dims, 0.3, 601))
+    lgt.lgt_set_integrator(lat.ctx, lgt.LGT_INT_OMELYAN)
+    plaq, accs, dHs = [], [], []
+    for traj in range(140):  # the white-noise warm start is far from equilibrium: fine steps (trajectory length 1)
+        dH, acc, _, _, _ = lgt.lgt_hmc_trajectory(lat.ctx, 25, 0.04, 4242, traj)
+        accs.append(acc)
+        dHs.append(dH)
+        plaq.append(lgt.lgt_plaquette(lat.ctx))
+    tail = np.array(plaq[60:])
+    assert np.mean(accs[60:]) > 0.7, np.mean(accs)
+    assert abs(np.mean(np.exp(-np.array(dHs[60:]))) - 1.0) < 0.15  # <exp(-dH)> = 1
+    assert abs(tail.mean() - 0.5937) < 0.004, (tail.mean(), tail.std())
+    lat.close()
