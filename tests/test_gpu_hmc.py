@@ -186,3 +186,26 @@ def test_pure_gauge_hmc_reproduces_the_known_plaquette(lgt):
     assert abs(np.mean(np.exp(-np.array(dHs[60:]))) - 1.0) < 0.15  # <exp(-dH)> = 1
     assert abs(tail.mean() - 0.5937) < 0.004, (tail.mean(), tail.std())
     lat.close()
+
+
+def test_heatbaths_full_size_sampled(lgt):
+    """configs[3]'s 32^4 lattice: the heat-bath kernels in their production launch shape, sampled links and sites against
+    the oracle's generator evaluated at exactly those elements; K / dof and |eta|^2 / dof as global checks."""
+    c = synth.CONFIGS[3]
+    dims, seed, traj = c["dims"], 0xABCDEF0123, 17
+    V = synth.volume(dims)
+    lat = lgt.Lattice(dims, c["beta"], c["kappa"], c["bc"])
+    lgt.lgt_momentum_heatbath(lat.ctx, seed, traj)
+    P = lat.get_momenta().reshape(4 * V, 3, 3)
+    links = np.array([0, 1, 127, 128, 4 * 31 + 3, 4 * (V // 2) + 2, 4 * V - 1, 4 * (V - 33)], dtype=np.uint64)
+    g0, g1 = ohmc.gaussian_pairs(seed, traj, ohmc.STREAM_MOMENTA, links[:, None], np.arange(4, dtype=np.uint64)[None, :])
+    pi = np.empty((len(links), 8))
+    pi[:, 0::2], pi[:, 1::2] = g0, g1
+    tau = np.array([oracle.generator(a) for a in range(8)])
+    ref = np.einsum("na,aij->nij", pi, tau)
+    assert np.abs(P[links.astype(np.int64)] - ref).max() < 1e-14
+    _, _, K, _ = lgt.lgt_action(lat.ctx)
+    assert abs(K / (4 * V * 8) - 0.5) < 5 * np.sqrt(0.5 / (32 * V))
+    n2 = lgt.lgt_pseudofermion_heatbath(lat.ctx, seed, traj)
+    assert abs(n2 / (12 * V) - 1.0) < 5 / np.sqrt(12 * V)
+    lat.close()

@@ -209,3 +209,24 @@ def test_paper_second_hmc_setup(lgt):
     U = lat.get_links()
     assert np.abs(U @ U.conj().swapaxes(-1, -2) - np.eye(3)).max() < 1e-12
     lat.close()
+
+
+def test_smeared_force_16x16x16x16(lgt):
+    """configs[2]'s lattice (several hundred blocks per kernel, ragged nothing): one stout level, X and Y given, so that
+    the pull-back kernels alone are compared per link with the oracle at a size well beyond one tile."""
+    c = synth.CONFIGS[2]
+    dims, kappa, bc = c["dims"], c["kappa"], c["bc"]
+    U = synth.config_links(2)
+    U1, A = ost.smear(dims, RHO, U)
+    X = synth.gaussian_spinor(dims, 461)
+    Y = synth.gaussian_spinor(dims, 462)
+    Fp = oracle.fermion_force(dims, kappa, bc, U1, X, Y)
+    F_ref = ost.pull_back(dims, RHO, U, A, Fp)[0]
+    lat = lgt.Lattice(dims, 5.6, kappa, bc)
+    lat.set_links(U)
+    lgt.lgt_set_smearing(lat.ctx, 1, RHO)
+    assert np.abs(smeared_links(lgt, lat, synth.volume(dims)) - U1).max() < 1e-13
+    F, _ = lat.fermion_force(X, Y)
+    err, plain = link_rel_err(F, F_ref)
+    assert err < TOL64, (err, plain)
+    lat.close()
