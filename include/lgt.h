@@ -284,7 +284,7 @@ int lgt_timing_read(lgt_ctx* ctx, int kernel_class, double* ms_total, long* laun
 long lgt_launch_count(const lgt_ctx* ctx);
 /* The stream the handle enqueues on (cudaStream_t as void*). */
 void* lgt_stream(const lgt_ctx* ctx);
-/* Block traversal order of the Dslash kernels (results are bitwise independent of it).  z_planes = 0: lexicographic;
+/* Block traversal order of the Dslash, fermion-force and staple kernels (results are bitwise independent of it).  z_planes = 0: lexicographic;
  * z_planes = Z > 0: blocks sweep all time slices of a slab of Z z-planes before the next slab, which keeps the
  * t neighbours of a site in L2 when one time slice of links + spinors no longer fits;
  * z_planes < 0: automatic (the default chosen by lgt_create).  LGT_EINVAL if Z does not divide Lz or Lx*Ly is

@@ -592,7 +592,9 @@ __global__ void __launch_bounds__(128, 1) fermion_force_kernel(Geom g, const typ
 template <class T, int ACC>
 __global__ void __launch_bounds__(128, 2) gauge_force_kernel(Geom g, const typename Vec2<T>::type* __restrict__ U,
                                                           typename Vec2<T>::type* __restrict__ P, T beta_over_6, T eps) {
-    const int s = g.s_begin + blockIdx.x * W + (threadIdx.x & 31);
+    // same slab-by-slab block order as the Dslash kernels on lattices whose time slice exceeds L2 (four 32-site blocks
+    // per 128-site chunk)
+    const int s = g.s_begin + (swizzled_chunk(g, blockIdx.x >> 2) * 4 + (blockIdx.x & 3)) * W + (threadIdx.x & 31);
     if (s >= g.s_end) return;
     const int mu = threadIdx.x >> 5;
     const Site c = site_coords(g, s);

@@ -69,12 +69,14 @@ def test_dslash_block_swizzle(lgt, dims, zs):
     assert lgt.lgt_set_block_swizzle(lat.ctx, 0) == 0
     base = [lat.dslash(psi, dagger=d) for d in (False, True)]
     x0, it0, _, ok0 = lat.cg(psi, 1e-10, 2000)
+    Fg0 = lat.gauge_force()
     for d in (False, True):
         assert site_rel_err(base[d], oracle.dslash(dims, 0.12, BC, U, psi, dagger=d)) < TOL64
     for z in zs:
         assert lgt.lgt_set_block_swizzle(lat.ctx, z) == z
         for d in (False, True):
             assert np.array_equal(lat.dslash(psi, dagger=d), base[d])
+        assert np.array_equal(lat.gauge_force(), Fg0)  # the staple kernel walks its blocks in the same order
         x, it, _, ok = lat.cg(psi, 1e-10, 2000)
         assert ok and ok0 and it == it0
         assert np.abs(x - x0).max() <= 1e-13 * np.abs(x0).max()  # block partials are summed in another order
