@@ -207,7 +207,7 @@ int lgt_get_smeared_links(lgt_ctx* ctx, void* U);
  * State goes in and out through the rank handles: lgt_dd_rank(d, i) returns a handle on which ONLY lgt_set_links,
  * lgt_get_links, lgt_set_momenta, lgt_get_momenta, lgt_set_pseudofermion, lgt_get_pseudofermion (+ _host forms),
  * lgt_timing_* and lgt_launch_count may be called (slab arrays); everything else on it returns LGT_ESTATE.
- * Plain CG on the full operator and the leapfrog; the solver variants, smearing and heat baths are single-GPU only. */
+ * Full operator (plain or mixed-precision CG) and the leapfrog; the even/odd action and smearing are single-GPU only. */
 typedef struct lgt_dd lgt_dd;
 int lgt_dd_create(lgt_dd** out, const int dims[4], int nranks, int nlocal, const int* local_ranks, double beta, double kappa,
                   const int bc[4], int precision, int device, void* cuda_stream);
@@ -238,6 +238,10 @@ lgt_ctx* lgt_dd_rank(lgt_dd* d, int local_index);
 int lgt_dd_dslash(lgt_dd* d, const void* const* in, void* const* out, int dagger);
 int lgt_dd_cg(lgt_dd* d, const void* const* b, void* const* x, double tol, int max_iter, int* iters, double* rel_resid);
 int lgt_dd_action(lgt_dd* d, double tol, int max_iter, double* S_g, double* S_F, double* K, int* cg_iters);
+/* lgt_set_solver for the solves inside lgt_dd_action / lgt_dd_md_* / lgt_dd_hmc_trajectory: LGT_SOLVER_MIXED_CG runs the
+ * decomposed CG in fp32 (fp32 copies of the links incl. ghost slices) inside an fp64 defect correction on the true,
+ * all-reduced residual.  lgt_dd_cg itself is always the plain CG. */
+int lgt_dd_set_solver(lgt_dd* d, int solver, double inner_tol);
 int lgt_dd_md_kick(lgt_dd* d, double eps, double tol, int max_iter, int* cg_iters);
 int lgt_dd_md_drift(lgt_dd* d, double eps);
 int lgt_dd_md_trajectory(lgt_dd* d, int nsteps, double dt, double tol, int max_iter, double* H_initial, double* H_final,

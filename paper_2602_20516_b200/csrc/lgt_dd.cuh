@@ -106,8 +106,8 @@ int dd_local_index(const lgt_dd* d, int rank) {
 // Halo exchange of one native field per local rank: base[i] points to the field of local rank i, `per_site` = complex
 // (or pair) elements per site (12 spinor, 36 links, 16 compact momenta).  Rank r's first interior slice goes to the
 // upper ghost slice of rank r - 1, its last interior slice to the lower ghost slice of rank r + 1 (periodic in ranks).
-int dd_exchange(lgt_dd* d, void* const* base, int per_site) {
-    const size_t esize = d->prec == LGT_F64 ? 16 : 8;
+int dd_exchange(lgt_dd* d, void* const* base, int per_site, size_t esize = 0) {
+    if (!esize) esize = d->prec == LGT_F64 ? 16 : 8;
     const size_t slice = (size_t)d->V3 * per_site * esize;
     const int n = (int)d->rk.size();
     if (!d->comm) {
@@ -159,6 +159,9 @@ int dd_exchange_links(lgt_dd* d) {
 
 namespace {
 
+// (D^dag D) x = b with the group's solver (plain CG, or the mixed-precision defect correction on LGT_F64 groups)
+int dd_solve(lgt_dd* d, int ib, bool want_y, double tol, int max_iter, int* iters);
+
 // The driver: every step loops over the local ranks (one in production, all of them in the single-GPU verification
 // mode), then does the step's communication, so that both transports run the same sequence of launches.
 template <class T> struct DdOps {
@@ -168,10 +171,28 @@ template <class T> struct DdOps {
     static size_t spinor_off(const lgt_ctx* c) { return (size_t)12 * c->g.s_begin; }
     static size_t spinor_n(const lgt_ctx* c) { return (size_t)12 * own_sites(c); }
 
-    static int exchange_spinor(lgt_dd* d, int ws_index_or_phi /* 0..5: ws[i], 6: phi */) {
+    // Field k of a rank in precision T: 0..5 = ws[k], 6 = phi, 7 = links.  DdOps<float> on an LGT_F64 group is the fp32
+    // inner solve of the mixed-precision solver and works on the rank's fp32 copies: links U32 and
+    // ws32 = {b, e, r, p, t} standing for the roles ws[5] (b), ws[0] (x), ws[1] (r), ws[2] (p), ws[3] (t).
+    static bool fp32_on_f64(const lgt_ctx* c) { return sizeof(T) == 4 && c->prec == LGT_F64; }
+    static void* fld(lgt_ctx* c, int k) {
+        if (fp32_on_f64(c)) {
+            switch (k) {
+                case 0: return c->ws32[1];
+                case 1: return c->ws32[2];
+                case 2: return c->ws32[3];
+                case 3: return c->ws32[4];
+                case 5: return c->ws32[0];
+                case 7: return c->U32;
+                default: return nullptr;
+            }
+        }
+        return k == 6 ? c->phi : k == 7 ? c->U : c->ws[k];
+    }
+    static int exchange_spinor(lgt_dd* d, int k) {
         std::vector<void*> f;
-        for (lgt_ctx* c : d->rk) f.push_back(ws_index_or_phi == 6 ? c->phi : c->ws[ws_index_or_phi]);
-        return dd_exchange(d, f.data(), 12);
+        for (lgt_ctx* c : d->rk) f.push_back(fld(c, k));
+        return dd_exchange(d, f.data(), 12, sizeof(T2));
     }
     static int allreduce_tmp(lgt_dd* d) {
         std::vector<double*> p;
@@ -186,7 +207,7 @@ template <class T> struct DdOps {
         if ((rc = exchange_spinor(d, in)) != LGT_OK) return rc;
         for (size_t i = 0; i < d->rk.size(); i++) {
             lgt_ctx* c = d->rk[i];
-            DD_RK(i, O::dslash(c, c->U, in == 6 ? c->phi : c->ws[in], out == 6 ? c->phi : c->ws[out], dagger, 0));
+            DD_RK(i, O::dslash(c, fld(c, 7), fld(c, in), fld(c, out), dagger, 0));
         }
         return LGT_OK;
     }
@@ -200,14 +221,16 @@ template <class T> struct DdOps {
         for (int i = 0; i < n; i++) {
             lgt_ctx* c = d->rk[i];
             const size_t off = spinor_off(c), cnt = spinor_n(c);
-            const T2* b = (const T2*)(ib == 6 ? c->phi : c->ws[ib]) + off;
-            LAUNCH(c, LGT_K_CG_BLAS, (cg_init_kernel<T>), stream_blocks(c, cnt), 256, cnt, b, (T2*)c->ws[0] + off, (T2*)c->ws[1] + off,
-                   (T2*)c->ws[2] + off, c->st, tol * tol, max_iter, c->partials, c->counter);
+            const T2* b = (const T2*)fld(c, ib) + off;
+            LAUNCH(c, LGT_K_CG_BLAS, (cg_init_kernel<T>), stream_blocks(c, cnt), 256, cnt, b, (T2*)fld(c, 0) + off, (T2*)fld(c, 1) + off,
+                   (T2*)fld(c, 2) + off, c->st, tol * tol, max_iter, c->partials, c->counter);
             LAUNCH(c, LGT_K_CG_BLAS, cg_rr_to_tmp_kernel, 1, 1, c->st);
         }
         if ((rc = allreduce_tmp(d)) != LGT_OK) return rc;
         for (int i = 0; i < n; i++) LAUNCH(d->rk[i], LGT_K_CG_BLAS, (cg_apply_kernel<0>), 1, 1, d->rk[i]->st);
-        const bool push = d->halo_mode == LGT_DD_PUSH;
+        // pushed halos need the neighbours' buffers of THIS precision: always there for local neighbours, mapped through
+        // IPC only for the handle's own precision
+        const bool push = d->halo_mode == LGT_DD_PUSH && (d->rk.size() == (size_t)d->nranks || !fp32_on_f64(d->rk[0]));
         std::vector<PushTo<T>> push_t(n), push_r(n);
         if (push) {
             // r = p = b on the ghost slices too (one ordinary exchange of b); from here on p's ghosts follow by local
@@ -216,17 +239,17 @@ template <class T> struct DdOps {
             const size_t slice = (size_t)12 * d->V3, hi = (size_t)(d->Lt_loc + 1) * slice;
             for (int i = 0; i < n; i++) {
                 lgt_ctx* c = d->rk[i];
-                const T2* b = (const T2*)(ib == 6 ? c->phi : c->ws[ib]);
+                const T2* b = (const T2*)fld(c, ib);
                 for (int f = 1; f <= 2; f++) {
-                    DD_CU(cudaMemcpyAsync((T2*)c->ws[f], b, slice * sizeof(T2), cudaMemcpyDeviceToDevice, d->stream));
-                    DD_CU(cudaMemcpyAsync((T2*)c->ws[f] + hi, b + hi, slice * sizeof(T2), cudaMemcpyDeviceToDevice, d->stream));
+                    DD_CU(cudaMemcpyAsync((T2*)fld(c, f), b, slice * sizeof(T2), cudaMemcpyDeviceToDevice, d->stream));
+                    DD_CU(cudaMemcpyAsync((T2*)fld(c, f) + hi, b + hi, slice * sizeof(T2), cudaMemcpyDeviceToDevice, d->stream));
                 }
                 const int r = d->rank_of[i];
                 const int dn = dd_local_index(d, (r + d->nranks - 1) % d->nranks), up = dd_local_index(d, (r + 1) % d->nranks);
-                push_r[i].lo = (T2*)(dn >= 0 ? d->rk[dn]->ws[1] : d->ipc_peer[0][0]);
-                push_r[i].hi = (T2*)(up >= 0 ? d->rk[up]->ws[1] : d->ipc_peer[0][1]);
-                push_t[i].lo = (T2*)(dn >= 0 ? d->rk[dn]->ws[3] : d->ipc_peer[1][0]);
-                push_t[i].hi = (T2*)(up >= 0 ? d->rk[up]->ws[3] : d->ipc_peer[1][1]);
+                push_r[i].lo = (T2*)(dn >= 0 ? fld(d->rk[dn], 1) : d->ipc_peer[0][0]);
+                push_r[i].hi = (T2*)(up >= 0 ? fld(d->rk[up], 1) : d->ipc_peer[0][1]);
+                push_t[i].lo = (T2*)(dn >= 0 ? fld(d->rk[dn], 3) : d->ipc_peer[1][0]);
+                push_t[i].hi = (T2*)(up >= 0 ? fld(d->rk[up], 3) : d->ipc_peer[1][1]);
                 push_r[i].lt_loc = push_t[i].lt_loc = d->Lt_loc;
                 if (!push_r[i].lo || !push_r[i].hi || !push_t[i].lo || !push_t[i].hi)
                     return dd_fail(d, LGT_ESTATE, "LGT_DD_PUSH: the neighbours' buffers are not mapped (lgt_dd_ipc_import)");
@@ -245,7 +268,7 @@ template <class T> struct DdOps {
                 if (!push && (rc = exchange_spinor(d, 2)) != LGT_OK) return rc;  // p
                 for (int i = 0; i < n; i++) {
                     lgt_ctx* c = d->rk[i];
-                    DD_RK(i, O::dslash(c, c->U, c->ws[2], c->ws[3], 0, 1, nullptr, push ? &push_t[i] : nullptr));  // t = D p, partials of |t|^2
+                    DD_RK(i, O::dslash(c, fld(c, 7), fld(c, 2), fld(c, 3), 0, 1, nullptr, push ? &push_t[i] : nullptr));  // t = D p, partials of |t|^2
                     LAUNCH(c, LGT_K_CG_BLAS, cg_partial_sum_kernel, 1, 1024, site_blocks(c, 128), c->partials, c->st);
                 }
                 if ((rc = allreduce_tmp(d)) != LGT_OK) return rc;
@@ -253,7 +276,7 @@ template <class T> struct DdOps {
                 if (!push && (rc = exchange_spinor(d, 3)) != LGT_OK) return rc;  // t
                 for (int i = 0; i < n; i++) {
                     lgt_ctx* c = d->rk[i];
-                    DD_RK(i, O::dslash(c, c->U, c->ws[3], nullptr, 1, 2, c->ws[1], push ? &push_r[i] : nullptr));  // r -= alpha D^dag t, partials of |r|^2
+                    DD_RK(i, O::dslash(c, fld(c, 7), fld(c, 3), nullptr, 1, 2, fld(c, 1), push ? &push_r[i] : nullptr));  // r -= alpha D^dag t, partials of |r|^2
                     LAUNCH(c, LGT_K_CG_BLAS, cg_partial_sum_kernel, 1, 1024, site_blocks(c, 128), c->partials, c->st);
                 }
                 if ((rc = allreduce_tmp(d)) != LGT_OK) return rc;
@@ -261,12 +284,12 @@ template <class T> struct DdOps {
                     lgt_ctx* c = d->rk[i];
                     const size_t off = spinor_off(c), cnt = spinor_n(c);
                     LAUNCH(c, LGT_K_CG_BLAS, (cg_apply_kernel<2>), 1, 1, c->st);
-                    LAUNCH(c, LGT_K_CG_BLAS, (cg_update_xp_kernel<T>), stream_blocks(c, cnt), 256, cnt, (T2*)c->ws[0] + off, (T2*)c->ws[2] + off,
-                           (const T2*)c->ws[1] + off, c->st, launched + it + 1);
+                    LAUNCH(c, LGT_K_CG_BLAS, (cg_update_xp_kernel<T>), stream_blocks(c, cnt), 256, cnt, (T2*)fld(c, 0) + off, (T2*)fld(c, 2) + off,
+                           (const T2*)fld(c, 1) + off, c->st, launched + it + 1);
                     if (push) {
                         const size_t slice = (size_t)12 * d->V3;
                         LAUNCH(c, LGT_K_CG_BLAS, (cg_update_p_ghost_kernel<T>), stream_blocks(c, 2 * slice), 256, slice,
-                               (size_t)(d->Lt_loc + 1) * slice, (T2*)c->ws[2], (const T2*)c->ws[1], c->st, launched + it + 1);
+                               (size_t)(d->Lt_loc + 1) * slice, (T2*)fld(c, 2), (const T2*)fld(c, 1), c->st, launched + it + 1);
                     }
                 }
             }
@@ -286,7 +309,7 @@ template <class T> struct DdOps {
         if ((rc = dd_exchange_links(d)) != LGT_OK) return rc;
         for (size_t i = 0; i < d->rk.size(); i++) DD_RK(i, O::gauge_force(d->rk[i], d->rk[i]->P, 1, eps));
         if (fermions_on(d->rk[0])) {
-            rc = cg(d, 6, true, tol, max_iter, &it, nullptr);
+            rc = dd_solve(d, 6, true, tol, max_iter, &it);
             if (rc == LGT_ENOCONV) conv = rc;
             else if (rc != LGT_OK) return rc;
             if ((rc = exchange_spinor(d, 0)) != LGT_OK) return rc;  // X(x + mu)
@@ -314,7 +337,7 @@ template <class T> struct DdOps {
         if ((rc = dd_exchange_links(d)) != LGT_OK) return rc;
         const bool ferm = fermions_on(d->rk[0]) && S_F != nullptr;
         if (ferm && !eta_norm) {
-            rc = cg(d, 6, false, tol, max_iter, &it, nullptr);
+            rc = dd_solve(d, 6, false, tol, max_iter, &it);
             if (rc == LGT_ENOCONV) conv = rc;
             else if (rc != LGT_OK) return rc;
         }
@@ -408,6 +431,96 @@ template <class T> struct DdOps {
 };
 
 #define DD_DISPATCH(d, fn, ...) ((d)->prec == LGT_F64 ? DdOps<double>::fn(__VA_ARGS__) : DdOps<float>::fn(__VA_ARGS__))
+
+// Mixed-precision solve on a decomposed lattice: the defect correction of cg_mixed() with every rank's fp32 copies
+// (links incl. ghost slices, five spinor buffers) and the decomposed fp32 CG inside; true fp64 residual, all-reduced.
+// b = field ib, x = ws[0]; r, q, t = ws[1], ws[2], ws[3]; leaves Y = D x in ws[3].
+int dd_cg_mixed(lgt_dd* d, int ib, bool want_y, double tol, int max_iter, int* iters) {
+    typedef DdOps<double> D64;
+    typedef DdOps<float> D32;
+    int rc;
+    if ((rc = dd_exchange_links(d)) != LGT_OK) return rc;
+    const int n = (int)d->rk.size();
+    std::vector<double*> slot;
+    for (int i = 0; i < n; i++) {
+        lgt_ctx* c = d->rk[i];
+        const size_t nfull = (size_t)12 * c->g.Vs, nu = (size_t)36 * c->g.Vs;
+        if (!c->U32) {
+            DD_CU(cudaMalloc(&c->U32, nu * sizeof(float2)));
+            for (int k = 0; k < 5; k++) {
+                DD_CU(cudaMalloc(&c->ws32[k], nfull * sizeof(float2)));
+                DD_CU(cudaMemsetAsync(c->ws32[k], 0, nfull * sizeof(float2), d->stream));
+            }
+            c->u32_valid = false;
+        }
+        if (!c->u32_valid) {  // ghost slices included: the links were exchanged above
+            LAUNCH(c, LGT_K_OTHER, down_convert_kernel, stream_blocks(c, nu), 256, nu, (const double2*)c->U, (float2*)c->U32, 1.0);
+            c->u32_valid = true;
+        }
+        const size_t off = D64::spinor_off(c), cnt = D64::spinor_n(c);
+        const double2* b = (const double2*)D64::fld(c, ib);
+        DD_CU(cudaMemsetAsync(c->ws[0], 0, nfull * sizeof(double2), d->stream));
+        DD_CU(cudaMemsetAsync(c->ws[3], 0, nfull * sizeof(double2), d->stream));
+        DD_CU(cudaMemcpyAsync(c->ws[1], b, nfull * sizeof(double2), cudaMemcpyDeviceToDevice, d->stream));
+        LAUNCH(c, LGT_K_OTHER, (redot_kernel<double>), stream_blocks(c, cnt), 256, cnt, b + off, b + off, c->scal + 3, c->partials, c->counter);
+        slot.push_back(c->scal + 3);
+    }
+    lgt_ctx* c0 = d->rk[0];
+    auto read_sum = [&](double& out) -> int {
+        int r2 = dd_allreduce(d, slot.data(), 1);
+        if (r2 != LGT_OK) return r2;
+        DD_CU(cudaMemcpyAsync(c0->h_scal + 3, c0->scal + 3, sizeof(double), cudaMemcpyDeviceToHost, d->stream));
+        DD_CU(cudaStreamSynchronize(d->stream));
+        out = c0->h_scal[3];
+        return LGT_OK;
+    };
+    double bb = 0.0;
+    if ((rc = read_sum(bb)) != LGT_OK) return rc;
+    double rr = bb;
+    int total = 0, outer = 0, conv = LGT_OK;
+    while (bb > 0.0 && rr > tol * tol * bb) {
+        if (total >= max_iter || outer >= 40) {
+            conv = LGT_ENOCONV;
+            break;
+        }
+        const double scale = 1.0 / sqrt(rr);
+        for (int i = 0; i < n; i++) {
+            lgt_ctx* c = d->rk[i];
+            const size_t nfull = (size_t)12 * c->g.Vs;
+            LAUNCH(c, LGT_K_CG_BLAS, down_convert_kernel, stream_blocks(c, nfull), 256, nfull, (const double2*)c->ws[1], (float2*)c->ws32[0], scale);
+        }
+        double eps = 0.25 * tol * sqrt(bb / rr);
+        if (eps < c0->inner_tol) eps = c0->inner_tol;
+        int it = 0;
+        rc = D32::cg(d, 5, false, eps, max_iter - total, &it, nullptr);
+        if (rc != LGT_OK && rc != LGT_ENOCONV) return rc;
+        total += it;
+        outer++;
+        for (int i = 0; i < n; i++) {
+            lgt_ctx* c = d->rk[i];
+            const size_t off = D64::spinor_off(c), cnt = D64::spinor_n(c);
+            LAUNCH(c, LGT_K_CG_BLAS, up_axpy_kernel, stream_blocks(c, cnt), 256, cnt, (double2*)c->ws[0] + off, (const float2*)c->ws32[1] + off, 1.0 / scale);
+        }
+        if ((rc = D64::dslash(d, 0, 3, 0)) != LGT_OK) return rc;  // t = D x
+        if ((rc = D64::dslash(d, 3, 2, 1)) != LGT_OK) return rc;  // q = D^dag t
+        for (int i = 0; i < n; i++) {
+            lgt_ctx* c = d->rk[i];
+            const size_t off = D64::spinor_off(c), cnt = D64::spinor_n(c);
+            LAUNCH(c, LGT_K_CG_BLAS, residual_kernel, stream_blocks(c, cnt), 256, cnt, (const double2*)D64::fld(c, ib) + off,
+                   (const double2*)c->ws[2] + off, (double2*)c->ws[1] + off, c->scal + 3, c->partials, c->counter);
+        }
+        if ((rc = read_sum(rr)) != LGT_OK) return rc;
+    }
+    (void)want_y;  // Y = D x is what the last residual evaluation left in ws[3]
+    if (iters) *iters = total;
+    if (conv != LGT_OK) return dd_fail(d, LGT_ENOCONV, "mixed-precision CG did not reach the tolerance");
+    return LGT_OK;
+}
+
+int dd_solve(lgt_dd* d, int ib, bool want_y, double tol, int max_iter, int* iters) {
+    if (d->prec == LGT_F64 && d->rk[0]->solver == LGT_SOLVER_MIXED_CG) return dd_cg_mixed(d, ib, want_y, tol, max_iter, iters);
+    return DD_DISPATCH(d, cg, d, ib, want_y, tol, max_iter, iters, nullptr);
+}
 
 }  // namespace
 
@@ -629,6 +742,18 @@ int lgt_dd_md_trajectory(lgt_dd* d, int nsteps, double dt, double tol, int max_i
     if (cg_iters) *cg_iters = total;
     DD_CU(cudaStreamSynchronize(d->stream));
     return conv;
+}
+
+int lgt_dd_set_solver(lgt_dd* d, int solver, double inner_tol) {
+    CHECK_DD(d);
+    if (solver != LGT_SOLVER_CG && solver != LGT_SOLVER_MIXED_CG) return dd_fail(d, LGT_EINVAL, "lgt_dd_set_solver: unknown solver");
+    if (solver == LGT_SOLVER_MIXED_CG && d->prec != LGT_F64) return dd_fail(d, LGT_EINVAL, "lgt_dd_set_solver: mixed precision needs an LGT_F64 group");
+    if (solver == LGT_SOLVER_MIXED_CG && !(inner_tol > 0.0 && inner_tol < 1.0)) return dd_fail(d, LGT_EINVAL, "lgt_dd_set_solver: inner_tol must be in (0, 1)");
+    for (lgt_ctx* c : d->rk) {
+        c->solver = solver;
+        if (solver == LGT_SOLVER_MIXED_CG) c->inner_tol = inner_tol;
+    }
+    return LGT_OK;
 }
 
 int lgt_dd_hmc_trajectory(lgt_dd* d, int nsteps, double dt, double tol, int max_iter, unsigned long long seed, unsigned trajectory,

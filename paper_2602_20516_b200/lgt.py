@@ -77,6 +77,7 @@ SYMBOLS = {
     "lgt_dd_dslash": (_i, [_vp, C.POINTER(_vp), C.POINTER(_vp), _i]),
     "lgt_dd_cg": (_i, [_vp, C.POINTER(_vp), C.POINTER(_vp), _d, _i, _ip, _dp]),
     "lgt_dd_action": (_i, [_vp, _d, _i, _dp, _dp, _dp, _ip]),
+    "lgt_dd_set_solver": (_i, [_vp, _i, _d]),
     "lgt_dd_md_kick": (_i, [_vp, _d, _d, _i, _ip]),
     "lgt_dd_md_drift": (_i, [_vp, _d]),
     "lgt_dd_md_trajectory": (_i, [_vp, _i, _d, _d, _i, _dp, _dp, _lp]),
@@ -471,6 +472,10 @@ def lgt_dd_action(d, tol=1e-12, max_iter=100000):
     sg, sf, k, it = C.c_double(), C.c_double(), C.c_double(), C.c_int()
     _dd_check(d, lib().lgt_dd_action(d, tol, max_iter, C.byref(sg), C.byref(sf), C.byref(k), C.byref(it)))
     return sg.value, sf.value, k.value, it.value
+
+
+def lgt_dd_set_solver(d, solver, inner_tol=1e-5):
+    _dd_check(d, lib().lgt_dd_set_solver(d, solver, inner_tol))
 
 
 def lgt_dd_md_kick(d, eps, tol=1e-12, max_iter=100000):

@@ -244,3 +244,34 @@ def test_dd_hmc_trajectory_matches_undivided_oracle(lgt, nranks):
         U = cat(dd.get_links())
     assert len(seen) >= 1
     dd.close()
+
+
+@pytest.mark.parametrize("nranks,mode", [(2, "exchange"), (4, "push"), (1, "push")])
+def test_dd_mixed_precision_solver(lgt, nranks, mode):
+    """lgt_dd_set_solver(MIXED): decomposed fp32 CG inside the fp64 defect correction; kick, drift and action agree with
+    the oracle's fp64 results on the undivided lattice, also after the links moved (fp32 copies refreshed)."""
+    dims, beta, kappa = (4, 4, 4, 8), 5.6, 0.12
+    U0 = synth.warm_links(dims, 0.3, 581)
+    P0 = synth.gaussian_momenta(dims, 582)
+    phi = oracle.dslash(dims, kappa, BC, U0, synth.gaussian_spinor(dims, 583), dagger=True)
+    dd = lgt.DecomposedLattice(dims, nranks, list(range(nranks)), beta, kappa, BC)
+    lgt.lgt_dd_set_halo_mode(dd.d, lgt.LGT_DD_PUSH if mode == "push" else lgt.LGT_DD_EXCHANGE)
+    lgt.lgt_dd_set_solver(dd.d, lgt.LGT_SOLVER_MIXED_CG, 1e-5)
+    dd.set_links(U0)
+    dd.set_momenta(P0)
+    dd.set_pseudofermion(phi)
+    it = lgt.lgt_dd_md_kick(dd.d, 0.05, 1e-12, 5000)
+    P1, it_ref, _ = oracle.kick(dims, beta, kappa, BC, U0, phi, P0, 0.05, 1e-12, 5000)
+    assert 0 < it < 2 * it_ref + 20
+    assert link_rel_err(cat(dd.get_momenta()), P1)[0] < 1e-10
+    lgt.lgt_dd_md_drift(dd.d, 0.05)
+    U1 = oracle.drift(dims, 0.05, P1, U0)
+    lgt.lgt_dd_md_kick(dd.d, 0.05, 1e-12, 5000)
+    P2, _, _ = oracle.kick(dims, beta, kappa, BC, U1, phi, P1, 0.05, 1e-12, 5000)
+    assert link_rel_err(cat(dd.get_momenta()), P2)[0] < 1e-10
+    _, S_F, _, _ = lgt.lgt_dd_action(dd.d, 1e-12, 5000)
+    S_ref = oracle.fermion_action(dims, kappa, BC, U1, phi, 1e-12, 5000)[0]
+    assert abs(S_F - S_ref) < 1e-10 * abs(S_ref)
+    with pytest.raises(lgt.LgtError):
+        lgt.lgt_dd_set_solver(dd.d, 5, 1e-5)
+    dd.close()
