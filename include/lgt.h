@@ -207,7 +207,7 @@ int lgt_get_smeared_links(lgt_ctx* ctx, void* U);
  * State goes in and out through the rank handles: lgt_dd_rank(d, i) returns a handle on which ONLY lgt_set_links,
  * lgt_get_links, lgt_set_momenta, lgt_get_momenta, lgt_set_pseudofermion, lgt_get_pseudofermion (+ _host forms),
  * lgt_timing_* and lgt_launch_count may be called (slab arrays); everything else on it returns LGT_ESTATE.
- * Full operator (plain or mixed-precision CG) and the leapfrog; the even/odd action and smearing are single-GPU only. */
+ * Full operator (plain or mixed-precision CG) or even/odd action, leapfrog; smearing is single-GPU only. */
 typedef struct lgt_dd lgt_dd;
 int lgt_dd_create(lgt_dd** out, const int dims[4], int nranks, int nlocal, const int* local_ranks, double beta, double kappa,
                   const int bc[4], int precision, int device, void* cuda_stream);
@@ -242,6 +242,10 @@ int lgt_dd_action(lgt_dd* d, double tol, int max_iter, double* S_g, double* S_F,
  * decomposed CG in fp32 (fp32 copies of the links incl. ghost slices) inside an fp64 defect correction on the true,
  * all-reduced residual.  lgt_dd_cg itself is always the plain CG. */
 int lgt_dd_set_solver(lgt_dd* d, int solver, double inner_tol);
+/* lgt_set_fermion_action for the decomposed lattice: LGT_ACTION_EO runs CG on the Schur complement with the half fields'
+ * ghost slices exchanged before every hop (plain fp64 / fp32 CG; the mixed solver applies to LGT_ACTION_FULL only).
+ * Needs even extents, an even number of time slices per slab and Lx*Ly*Lz % 64 == 0, else LGT_EINVAL. */
+int lgt_dd_set_fermion_action(lgt_dd* d, int action);
 int lgt_dd_md_kick(lgt_dd* d, double eps, double tol, int max_iter, int* cg_iters);
 int lgt_dd_md_drift(lgt_dd* d, double eps);
 int lgt_dd_md_trajectory(lgt_dd* d, int nsteps, double dt, double tol, int max_iter, double* H_initial, double* H_final,

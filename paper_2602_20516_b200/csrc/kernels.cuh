@@ -38,6 +38,7 @@ struct Geom {
     int t_off;      // global t of local slice 0 (0, or rank * Lt_local - 1 on a slab)
     int Lt_glob;    // global time extent (for the fermion boundary sign of the t links)
     int site_off;   // global site index = local site index + site_off (heat baths draw by global element number)
+    int h_begin, h_end;  // the owned range of checkerboard indices of a half field (s_begin / 2, s_end / 2)
 };
 
 // lexicographic 128-site chunk handled by block b
@@ -1097,9 +1098,9 @@ __global__ void __launch_bounds__(128, 1) hop_cb_kernel(Geom g, int p, const typ
                                                         typename Vec2<T>::type* __restrict__ out, T kap, CgState* st,
                                                         double* partials, typename Vec2<T>::type* __restrict__ r) {
     const int done = (MODE != 0) ? st->done : 0;
-    const int c = blockIdx.x * blockDim.x + threadIdx.x;
+    const int c = g.h_begin + blockIdx.x * blockDim.x + threadIdx.x;
     double nrm = 0.0;
-    if (c < g.Vh) {
+    if (c < g.h_end) {
         if (MODE == 2) {
             const typename Vec2<T>::type* br = spinor_at(r, c);
 #pragma unroll
@@ -1147,7 +1148,7 @@ __global__ void __launch_bounds__(128, 1) hop_cb_kernel(Geom g, int p, const typ
         }
     } else {
         if (MODE != 0 && done) return;
-        if (c < g.Vhs && MODE != 2) {
+        if (c >= g.Vh && c < g.Vhs && MODE != 2) {  // padding lanes only, never a ghost slice
             typename Vec2<T>::type* bo = spinor_at(out, c);
 #pragma unroll
             for (int k = 0; k < 12; k++) stc<T>(bo + k * W, mk<T>(0, 0));

@@ -148,6 +148,8 @@ inline size_t mom_bytes(const lgt_ctx* c) { return (size_t)16 * c->g.Vs * c->esi
 // sites the compute kernels own (Geom::s_begin .. s_end), padding lanes included on an undivided lattice
 inline int own_sites(const lgt_ctx* c) { return (c->g.s_end == c->g.V ? c->g.Vs : c->g.s_end) - c->g.s_begin; }
 inline int site_blocks(const lgt_ctx* c, int bs) { return (own_sites(c) + bs - 1) / bs; }
+// the same for one parity of a checkerboarded field
+inline int own_half_sites(const lgt_ctx* c) { return (c->g.h_end == c->g.Vh ? c->g.Vhs : c->g.h_end) - c->g.h_begin; }
 inline int stream_blocks(const lgt_ctx* c, size_t n) {
     size_t b = (n + 255) / 256;
     return (int)(b < (size_t)c->red_blocks ? (b ? b : 1) : c->red_blocks);
@@ -434,7 +436,7 @@ template <class T> struct Ops {
     }
     // out (parity p) = self - kap * H in (in of parity 1 - p); mode as in hop_cb_kernel
     static int hop(lgt_ctx* c, int p, const T2* in, const T2* self, T2* out, int dagger, int mode, double kap, T2* r = nullptr) {
-        const int grid = (c->g.Vhs + 127) / 128;
+        const int grid = (own_half_sites(c) + 127) / 128;
 #define HOP_ARGS c->g, p, links_cb(c, p), links_cb(c, 1 - p), in, self, out, (T)kap, c->st, c->partials, r
         if (mode == 0) {
             if (dagger) LAUNCH(c, LGT_K_DSLASH, (hop_cb_kernel<T, 1, 0>), grid, 128, HOP_ARGS);
@@ -460,7 +462,7 @@ template <class T> struct Ops {
     static int eo_cg(lgt_ctx* c, const T2* b, T2* x, T2* r, T2* p, T2* u, T2* t, double tol, int max_iter, int* iters, double* rel) {
         const size_t n = (size_t)12 * c->g.Vhs;
         const int nb = stream_blocks(c, n);
-        const int ngrid = (c->g.Vhs + 127) / 128;
+        const int ngrid = (own_half_sites(c) + 127) / 128;
         LAUNCH(c, LGT_K_CG_BLAS, (cg_init_kernel<T>), nb, 256, n, b, x, r, p, c->st, tol * tol, max_iter, c->partials, c->counter);
         int rc, launched = 0;
         for (;;) {
@@ -877,6 +879,8 @@ int lgt_create(lgt_ctx** out, const int dims[4], double beta, double kappa, cons
     c->g.t_off = 0;
     c->g.Lt_glob = c->g.L[3];
     c->g.site_off = 0;
+    c->g.h_begin = 0;
+    c->g.h_end = c->g.Vh;
     int sms = 148;
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device);
     c->red_blocks = sms * 8;

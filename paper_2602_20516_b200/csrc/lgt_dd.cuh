@@ -309,7 +309,7 @@ template <class T> struct DdOps {
         if ((rc = dd_exchange_links(d)) != LGT_OK) return rc;
         for (size_t i = 0; i < d->rk.size(); i++) DD_RK(i, O::gauge_force(d->rk[i], d->rk[i]->P, 1, eps));
         if (fermions_on(d->rk[0])) {
-            rc = dd_solve(d, 6, true, tol, max_iter, &it);
+            rc = d->rk[0]->action == LGT_ACTION_EO ? eo_solve(d, true, tol, max_iter, &it, false) : dd_solve(d, 6, true, tol, max_iter, &it);
             if (rc == LGT_ENOCONV) conv = rc;
             else if (rc != LGT_OK) return rc;
             if ((rc = exchange_spinor(d, 0)) != LGT_OK) return rc;  // X(x + mu)
@@ -336,8 +336,9 @@ template <class T> struct DdOps {
         int rc, it = 0, conv = LGT_OK;
         if ((rc = dd_exchange_links(d)) != LGT_OK) return rc;
         const bool ferm = fermions_on(d->rk[0]) && S_F != nullptr;
+        const bool eo = d->rk[0]->action == LGT_ACTION_EO;
         if (ferm && !eta_norm) {
-            rc = dd_solve(d, 6, false, tol, max_iter, &it);
+            rc = eo ? eo_solve(d, false, tol, max_iter, &it, true) : dd_solve(d, 6, false, tol, max_iter, &it);
             if (rc == LGT_ENOCONV) conv = rc;
             else if (rc != LGT_OK) return rc;
         }
@@ -346,7 +347,13 @@ template <class T> struct DdOps {
             lgt_ctx* c = d->rk[i];
             DD_RK(i, O::plaquette_sum(c, c->scal + 0));
             DD_RK(i, O::kinetic(c, c->scal + 1));
-            if (ferm) {
+            if (ferm && eo) {
+                if (eta_norm) {  // |eta_e|^2; after a solve eo_solve() has left Re <phi_e, X_e> in the slot already
+                    const size_t off = half_off(c), cnt = half_n(c);
+                    LAUNCH(c, LGT_K_OTHER, (redot_kernel<T>), stream_blocks(c, cnt), 256, cnt, (const T2*)hB(c) + off, (const T2*)hB(c) + off,
+                           c->scal + 2, c->partials, c->counter);
+                }
+            } else if (ferm) {
                 const size_t off = spinor_off(c);
                 const T2 *a = (const T2*)(eta_norm ? c->ws[4] : c->phi) + off, *b = (const T2*)(eta_norm ? c->ws[4] : c->ws[0]) + off;
                 LAUNCH(c, LGT_K_OTHER, (redot_kernel<T>), stream_blocks(c, spinor_n(c)), 256, spinor_n(c), a, b, c->scal + 2, c->partials, c->counter);
@@ -367,6 +374,118 @@ template <class T> struct DdOps {
         return conv;
     }
 
+    // ---- even/odd preconditioned action on the slabs.  A rank's LOCAL parity (x + y + z + t_local) differs from the global
+    // one by t_off, so the globally even sites are the local parity pe = t_off & 1; everything else is Ops<T>'s even/odd
+    // code with (pe, 1 - pe) in place of (0, 1), the input half field's ghost slices exchanged before every hop and the
+    // CG sums all-reduced.  Half fields have V3 / 2 sites per time slice, so their slices are contiguous runs too.
+    static int pe_of(const lgt_ctx* c) { return c->g.t_off & 1; }
+    static T2* E(lgt_ctx* c, int k) { return O::eo_field(c, k + pe_of(c)); }      // globally even member of the pair (k, k+1)
+    static T2* Od(lgt_ctx* c, int k) { return O::eo_field(c, k + 1 - pe_of(c)); }  // globally odd member
+    typedef T2* (*HalfSel)(lgt_ctx*);
+    static int exchange_half(lgt_dd* d, HalfSel sel) {
+        std::vector<void*> f;
+        for (lgt_ctx* c : d->rk) f.push_back(sel(c));
+        return dd_exchange(d, f.data(), 6, sizeof(T2));  // 12 components x V3 / 2 sites per slice
+    }
+    static T2* hXe(lgt_ctx* c) { return E(c, 0); }
+    static T2* hXo(lgt_ctx* c) { return Od(c, 0); }
+    static T2* hYe(lgt_ctx* c) { return E(c, 2); }
+    static T2* hP(lgt_ctx* c) { return O::eo_field(c, 6); }
+    static T2* hT(lgt_ctx* c) { return O::eo_field(c, 7); }
+    static size_t half_off(const lgt_ctx* c) { return (size_t)12 * c->g.h_begin; }
+    static size_t half_n(const lgt_ctx* c) { return (size_t)12 * (c->g.h_end - c->g.h_begin); }
+    // one hop on every rank, after the exchange of its input field
+    static int hop_all(lgt_dd* d, bool to_even, HalfSel in, HalfSel self, HalfSel out, int dagger, int mode, bool plus_kappa, HalfSel r = nullptr) {
+        int rc;
+        if ((rc = exchange_half(d, in)) != LGT_OK) return rc;
+        for (size_t i = 0; i < d->rk.size(); i++) {
+            lgt_ctx* c = d->rk[i];
+            const int p = to_even ? pe_of(c) : 1 - pe_of(c);
+            DD_RK(i, O::hop(c, p, in(c), self ? self(c) : nullptr, out ? out(c) : nullptr, dagger, mode, plus_kappa ? c->kappa : -c->kappa,
+                            r ? r(c) : nullptr));
+        }
+        return LGT_OK;
+    }
+    static T2* hB(lgt_ctx* c) { return E(c, 4); }
+    static T2* hR(lgt_ctx* c) { return Od(c, 4); }  // the odd half of the split source is free: CG residual
+
+    // X_e = (M^dag M)^-1 phi_e on every rank; then, if want_xy, the full fields X = ws[0], Y = ws[3] of the force kernel
+    static int eo_solve(lgt_dd* d, bool want_xy, double tol, int max_iter, int* iters, bool sf_to_slot2) {
+        int rc;
+        if ((rc = dd_exchange_links(d)) != LGT_OK) return rc;
+        const int n = (int)d->rk.size();
+        for (int i = 0; i < n; i++) {
+            lgt_ctx* c = d->rk[i];
+            DD_RK(i, O::eo_ensure(c));
+            DD_RK(i, O::eo_split(c, c->phi, O::eo_field(c, 4)));
+            const size_t off = half_off(c), cnt = half_n(c);
+            LAUNCH(c, LGT_K_CG_BLAS, (cg_init_kernel<T>), stream_blocks(c, cnt), 256, cnt, (const T2*)hB(c) + off, hXe(c) + off, hR(c) + off,
+                   hP(c) + off, c->st, tol * tol, max_iter, c->partials, c->counter);
+            LAUNCH(c, LGT_K_CG_BLAS, cg_rr_to_tmp_kernel, 1, 1, c->st);
+        }
+        if ((rc = allreduce_tmp(d)) != LGT_OK) return rc;
+        for (int i = 0; i < n; i++) LAUNCH(d->rk[i], LGT_K_CG_BLAS, (cg_apply_kernel<0>), 1, 1, d->rk[i]->st);
+        lgt_ctx* c0 = d->rk[0];
+        int launched = 0;
+        auto sum_and = [&](int what) -> int {
+            for (int i = 0; i < n; i++) {
+                lgt_ctx* c = d->rk[i];
+                LAUNCH(c, LGT_K_CG_BLAS, cg_partial_sum_kernel, 1, 1024, (own_half_sites(c) + 127) / 128, c->partials, c->st);
+            }
+            int r2 = allreduce_tmp(d);
+            if (r2 != LGT_OK) return r2;
+            for (int i = 0; i < n; i++) {
+                if (what == 1) LAUNCH(d->rk[i], LGT_K_CG_BLAS, (cg_apply_kernel<1>), 1, 1, d->rk[i]->st);
+                else LAUNCH(d->rk[i], LGT_K_CG_BLAS, (cg_apply_kernel<2>), 1, 1, d->rk[i]->st);
+            }
+            return LGT_OK;
+        };
+        for (;;) {
+            DD_CU(cudaMemcpyAsync(c0->h_st, c0->st, sizeof(CgState), cudaMemcpyDeviceToHost, d->stream));
+            DD_CU(cudaStreamSynchronize(d->stream));
+            if (c0->h_st->done) break;
+            int chunk = max_iter - launched;
+            if (chunk > 8) chunk = 8;
+            if (chunk <= 0) chunk = 1;
+            for (int it = 0; it < chunk; it++) {
+                if ((rc = hop_all(d, false, hP, nullptr, hT, 0, 3, false)) != LGT_OK) return rc;  // t_o = kappa H_oe p
+                if ((rc = hop_all(d, true, hT, hP, hYe, 0, 1, true)) != LGT_OK) return rc;         // u = M p, |u|^2
+                if ((rc = sum_and(1)) != LGT_OK) return rc;
+                if ((rc = hop_all(d, false, hYe, nullptr, hT, 1, 3, false)) != LGT_OK) return rc;  // t_o = kappa H_oe^dag u
+                if ((rc = hop_all(d, true, hT, hYe, nullptr, 1, 2, true, hR)) != LGT_OK) return rc;  // r -= alpha M^dag u
+                if ((rc = sum_and(2)) != LGT_OK) return rc;
+                for (int i = 0; i < n; i++) {
+                    lgt_ctx* c = d->rk[i];
+                    const size_t off = half_off(c), cnt = half_n(c);
+                    LAUNCH(c, LGT_K_CG_BLAS, (cg_update_xp_kernel<T>), stream_blocks(c, cnt), 256, cnt, hXe(c) + off, hP(c) + off,
+                           (const T2*)hR(c) + off, c->st, launched + it + 1);
+                }
+            }
+            launched += chunk;
+        }
+        const CgState h = *c0->h_st;
+        if (iters) *iters = h.iter;
+        if (sf_to_slot2)
+            for (int i = 0; i < n; i++) {
+                lgt_ctx* c = d->rk[i];
+                const size_t off = half_off(c), cnt = half_n(c);
+                LAUNCH(c, LGT_K_OTHER, (redot_kernel<T>), stream_blocks(c, cnt), 256, cnt, (const T2*)hB(c) + off, (const T2*)hXe(c) + off,
+                       c->scal + 2, c->partials, c->counter);
+            }
+        if (want_xy) {
+            if ((rc = hop_all(d, false, hXe, nullptr, hXo, 0, 0, false)) != LGT_OK) return rc;  // X_o = kappa H_oe X_e
+            if ((rc = hop_all(d, true, hXo, hXe, hYe, 0, 0, true)) != LGT_OK) return rc;        // Y_e = M X_e
+            if ((rc = hop_all(d, false, hYe, nullptr, [](lgt_ctx* c) { return Od(c, 2); }, 1, 0, false)) != LGT_OK) return rc;  // Y_o
+            for (int i = 0; i < n; i++) {
+                lgt_ctx* c = d->rk[i];
+                DD_RK(i, O::eo_merge(c, O::eo_field(c, 0), c->ws[0]));
+                DD_RK(i, O::eo_merge(c, O::eo_field(c, 2), c->ws[3]));
+            }
+        }
+        if (h.rr > h.tol2 * h.bb) return dd_fail(d, LGT_ENOCONV, "even/odd CG did not reach the tolerance within max_iter");
+        return LGT_OK;
+    }
+
     // Heat baths by global element number (reading A-25), so that the fields are those of the undivided lattice
     static int heatbaths(lgt_dd* d, unsigned long long seed, unsigned traj) {
         int rc;
@@ -378,7 +497,22 @@ template <class T> struct DdOps {
                 c->has_phi = true;
             }
         }
-        if (d->rk[0]->kappa != 0.0 && (rc = dslash(d, 4, 6, 1)) != LGT_OK) return rc;  // phi = D^dag eta
+        if (d->rk[0]->kappa == 0.0) return LGT_OK;
+        if (d->rk[0]->action != LGT_ACTION_EO) return dslash(d, 4, 6, 1);  // phi = D^dag eta
+        // even/odd action: phi_e = M^dag eta_e, phi_o = 0; eta_e stays in the even member of fields (4, 5) for |eta_e|^2
+        if ((rc = dd_exchange_links(d)) != LGT_OK) return rc;
+        for (size_t i = 0; i < d->rk.size(); i++) {
+            lgt_ctx* c = d->rk[i];
+            DD_RK(i, O::eo_ensure(c));
+            DD_RK(i, O::eo_split(c, c->ws[4], O::eo_field(c, 4)));
+        }
+        if ((rc = hop_all(d, false, hB, nullptr, hT, 1, 0, false)) != LGT_OK) return rc;
+        if ((rc = hop_all(d, true, hT, hB, hYe, 1, 0, true)) != LGT_OK) return rc;
+        for (size_t i = 0; i < d->rk.size(); i++) {
+            lgt_ctx* c = d->rk[i];
+            DD_CU(cudaMemsetAsync(Od(c, 2), 0, (size_t)12 * c->g.Vhs * sizeof(T2), d->stream));
+            DD_RK(i, O::eo_merge(c, O::eo_field(c, 2), c->phi));
+        }
         return LGT_OK;
     }
     static int hmc_trajectory(lgt_dd* d, int nsteps, double dt, double tol, int max_iter, unsigned long long seed, unsigned traj,
@@ -583,6 +717,8 @@ int lgt_dd_create(lgt_dd** out, const int dims[4], int nranks, int nlocal, const
         c->g.t_off = local_ranks[i] * d->Lt_loc - 1;
         c->g.Lt_glob = dims[3];
         c->g.site_off = (local_ranks[i] * d->Lt_loc - 1) * d->V3;
+        c->g.h_begin = d->V3 / 2;
+        c->g.h_end = c->g.Vh - d->V3 / 2;
         c->g.swz_Z = 0;
         c->dd_links_valid = &d->links_ghost_valid;
         d->rk.push_back(c);
@@ -744,6 +880,18 @@ int lgt_dd_md_trajectory(lgt_dd* d, int nsteps, double dt, double tol, int max_i
     return conv;
 }
 
+int lgt_dd_set_fermion_action(lgt_dd* d, int action) {
+    CHECK_DD(d);
+    if (action != LGT_ACTION_FULL && action != LGT_ACTION_EO) return dd_fail(d, LGT_EINVAL, "lgt_dd_set_fermion_action: unknown action");
+    if (action == LGT_ACTION_EO) {
+        const Geom& g = d->rk[0]->g;
+        if (g.L[0] % 2 || g.L[1] % 2 || g.L[2] % 2 || d->Lt_loc % 2 || d->V3 % 64)
+            return dd_fail(d, LGT_EINVAL, "lgt_dd_set_fermion_action: the even/odd action needs even extents, an even number of time slices "
+                                          "per slab and Lx*Ly*Lz a multiple of 64");
+    }
+    for (lgt_ctx* c : d->rk) c->action = action;
+    return LGT_OK;
+}
 int lgt_dd_set_solver(lgt_dd* d, int solver, double inner_tol) {
     CHECK_DD(d);
     if (solver != LGT_SOLVER_CG && solver != LGT_SOLVER_MIXED_CG) return dd_fail(d, LGT_EINVAL, "lgt_dd_set_solver: unknown solver");

@@ -78,6 +78,7 @@ SYMBOLS = {
     "lgt_dd_cg": (_i, [_vp, C.POINTER(_vp), C.POINTER(_vp), _d, _i, _ip, _dp]),
     "lgt_dd_action": (_i, [_vp, _d, _i, _dp, _dp, _dp, _ip]),
     "lgt_dd_set_solver": (_i, [_vp, _i, _d]),
+    "lgt_dd_set_fermion_action": (_i, [_vp, _i]),
     "lgt_dd_md_kick": (_i, [_vp, _d, _d, _i, _ip]),
     "lgt_dd_md_drift": (_i, [_vp, _d]),
     "lgt_dd_md_trajectory": (_i, [_vp, _i, _d, _d, _i, _dp, _dp, _lp]),
@@ -476,6 +477,10 @@ def lgt_dd_action(d, tol=1e-12, max_iter=100000):
 
 def lgt_dd_set_solver(d, solver, inner_tol=1e-5):
     _dd_check(d, lib().lgt_dd_set_solver(d, solver, inner_tol))
+
+
+def lgt_dd_set_fermion_action(d, action):
+    _dd_check(d, lib().lgt_dd_set_fermion_action(d, action))
 
 
 def lgt_dd_md_kick(d, eps, tol=1e-12, max_iter=100000):

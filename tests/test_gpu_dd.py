@@ -275,3 +275,49 @@ def test_dd_mixed_precision_solver(lgt, nranks, mode):
     with pytest.raises(lgt.LgtError):
         lgt.lgt_dd_set_solver(dd.d, 5, 1e-5)
     dd.close()
+
+
+@pytest.mark.parametrize("nranks", [1, 2, 4])
+def test_dd_even_odd_action(lgt, nranks):
+    """The even/odd action on slabs (local parity = global parity shifted by the slab's time offset): iteration count,
+    kick and S_F against the oracle's even/odd mode on the undivided lattice; an HMC trajectory against the
+    (oracle-verified) single-GPU even/odd trajectory with the same seed."""
+    from oracle import evenodd as oeo
+
+    dims, beta, kappa, tol = (4, 4, 4, 8), 5.6, 0.12, 1e-12
+    V = synth.volume(dims)
+    U0 = synth.warm_links(dims, 0.3, 591)
+    P0 = synth.gaussian_momenta(dims, 592)
+    phi = oeo.mhat(dims, kappa, BC, U0, oeo.keep(synth.gaussian_spinor(dims, 593), dims, 0), dagger=True)
+    F_ref, it_ref, _ = oeo.fermion_force(dims, kappa, BC, U0, phi, tol, 10 * V)
+    dd = lgt.DecomposedLattice(dims, nranks, list(range(nranks)), beta, kappa, BC)
+    lgt.lgt_dd_set_fermion_action(dd.d, lgt.LGT_ACTION_EO)
+    dd.set_links(U0)
+    dd.set_momenta(P0)
+    dd.set_pseudofermion(phi)
+    it = lgt.lgt_dd_md_kick(dd.d, 0.05, tol, 10 * V)
+    assert it == it_ref
+    P_ref = P0 - 0.05 * (oracle.gauge_force(dims, beta, U0) + F_ref)
+    assert link_rel_err(cat(dd.get_momenta()), P_ref)[0] < TOL64
+    _, S_F, _, _ = lgt.lgt_dd_action(dd.d, tol, 10 * V)
+    S_ref = oeo.action(dims, kappa, BC, U0, phi, tol, 10 * V)[0]
+    assert abs(S_F - S_ref) < 1e-11 * abs(S_ref)
+    # HMC with the even/odd action: same (seed, trajectory) on one undivided handle
+    one = lgt.Lattice(dims, beta, kappa, BC)
+    lgt.lgt_set_fermion_action(one.ctx, lgt.LGT_ACTION_EO)
+    one.set_links(U0)
+    dd.set_links(U0)
+    for traj in range(2):
+        a = lgt.lgt_hmc_trajectory(one.ctx, 3, 0.03, 1357, traj, tol=1e-13, max_iter=5000)
+        b = lgt.lgt_dd_hmc_trajectory(dd.d, 3, 0.03, 1357, traj, tol=1e-13, max_iter=5000)
+        assert abs(a[3] - b[3]) < 1e-12 * abs(a[3]) and abs(a[0] - b[0]) < 1e-9 * abs(a[3])
+        assert a[1] == b[1] and a[2] == b[2]
+        assert np.abs(cat(dd.get_links()) - one.get_links()).max() < 1e-11
+    one.close()
+    dd.close()
+    with pytest.raises(lgt.LgtError):
+        bad = lgt.lgt_dd_create((4, 4, 2, 8), 2, [0, 1], beta, kappa, BC)  # 32 sites per time slice: not a multiple of 64
+        try:
+            lgt.lgt_dd_set_fermion_action(bad, lgt.LGT_ACTION_EO)
+        finally:
+            lgt.lgt_dd_destroy(bad)
