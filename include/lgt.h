@@ -207,7 +207,7 @@ int lgt_get_smeared_links(lgt_ctx* ctx, void* U);
  * State goes in and out through the rank handles: lgt_dd_rank(d, i) returns a handle on which ONLY lgt_set_links,
  * lgt_get_links, lgt_set_momenta, lgt_get_momenta, lgt_set_pseudofermion, lgt_get_pseudofermion (+ _host forms),
  * lgt_timing_* and lgt_launch_count may be called (slab arrays); everything else on it returns LGT_ESTATE.
- * Full operator (plain or mixed-precision CG) or even/odd action, leapfrog; smearing is single-GPU only. */
+ * Full operator (plain or mixed-precision CG) or even/odd action, stout-smeared fermion links, leapfrog. */
 typedef struct lgt_dd lgt_dd;
 int lgt_dd_create(lgt_dd** out, const int dims[4], int nranks, int nlocal, const int* local_ranks, double beta, double kappa,
                   const int bc[4], int precision, int device, void* cuda_stream);
@@ -246,6 +246,10 @@ int lgt_dd_set_solver(lgt_dd* d, int solver, double inner_tol);
  * ghost slices exchanged before every hop (plain fp64 / fp32 CG; the mixed solver applies to LGT_ACTION_FULL only).
  * Needs even extents, an even number of time slices per slab and Lx*Ly*Lz % 64 == 0, else LGT_EINVAL. */
 int lgt_dd_set_fermion_action(lgt_dd* d, int action);
+/* lgt_set_smearing for the decomposed lattice: every level's links are built on the slabs' interiors and their ghost
+ * slices exchanged before the next level; in the force recursion the ghost slices of G are exchanged before each
+ * chain kernel. */
+int lgt_dd_set_smearing(lgt_dd* d, int n_levels, double rho);
 int lgt_dd_md_kick(lgt_dd* d, double eps, double tol, int max_iter, int* cg_iters);
 int lgt_dd_md_drift(lgt_dd* d, double eps);
 int lgt_dd_md_trajectory(lgt_dd* d, int nsteps, double dt, double tol, int max_iter, double* H_initial, double* H_final,

@@ -277,12 +277,7 @@ template <class T> struct Ops {
 
     // ---- stout smearing: the Dirac operator sees c->Uf
     // Brings c->Uf up to date: the thin links, or level nsmear of U^(k+1) = exp(A^(k+1)) U^(k), A = -rho P_su(3)[U V].
-    static int ensure_fermion_links(lgt_ctx* c) {
-        if (c->nsmear == 0) {
-            c->Uf = c->U;
-            return LGT_OK;
-        }
-        const int grid = site_blocks(c, 32);
+    static int smear_alloc(lgt_ctx* c) {
         for (int k = 0; k < c->nsmear; k++) {
             if (!c->Usm[k]) CU(cudaMalloc(&c->Usm[k], links_bytes(c)));
             if (!c->Asm[k]) {
@@ -290,14 +285,27 @@ template <class T> struct Ops {
                 CU(cudaMemsetAsync(c->Asm[k], 0, mom_bytes(c), c->stream));
             }
         }
-        if (!c->usm_valid) {
-            const T2* Uin = (const T2*)c->U;
-            for (int k = 0; k < c->nsmear; k++) {
-                if (c->g.Vs != c->g.V) CU(cudaMemsetAsync(c->Usm[k], 0, links_bytes(c), c->stream));  // padding lanes
-                LAUNCH(c, LGT_K_GAUGE_FORCE, (gauge_force_kernel<T, 0>), grid, 128, c->g, Uin, (T2*)c->Asm[k], (T)(-c->rho), (T)0);
-                LAUNCH(c, LGT_K_LINK_UPDATE, (link_update_kernel<T>), grid, 128, c->g, Uin, (T2*)c->Usm[k], (const T2*)c->Asm[k], (T)1);
-                Uin = (const T2*)c->Usm[k];
-            }
+        return LGT_OK;
+    }
+    // level k + 1 from level k (the owned sites; on a slab the caller exchanges the ghost slices of the result)
+    static int smear_level(lgt_ctx* c, int k) {
+        const int grid = site_blocks(c, 32);
+        const T2* Uin = (const T2*)(k == 0 ? c->U : c->Usm[k - 1]);
+        if (c->g.Vs != c->g.V) CU(cudaMemsetAsync(c->Usm[k], 0, links_bytes(c), c->stream));  // padding lanes
+        LAUNCH(c, LGT_K_GAUGE_FORCE, (gauge_force_kernel<T, 0>), grid, 128, c->g, Uin, (T2*)c->Asm[k], (T)(-c->rho), (T)0);
+        LAUNCH(c, LGT_K_LINK_UPDATE, (link_update_kernel<T>), grid, 128, c->g, Uin, (T2*)c->Usm[k], (const T2*)c->Asm[k], (T)1);
+        return LGT_OK;
+    }
+    static int ensure_fermion_links(lgt_ctx* c) {
+        if (c->nsmear == 0) {
+            c->Uf = c->U;
+            return LGT_OK;
+        }
+        int rc;
+        if ((rc = smear_alloc(c)) != LGT_OK) return rc;
+        if (!c->usm_valid && !c->dd_links_valid) {  // on a slab the group driver interleaves the levels with halo exchanges
+            for (int k = 0; k < c->nsmear; k++)
+                if ((rc = smear_level(c, k)) != LGT_OK) return rc;
             c->usm_valid = true;
         }
         c->Uf = c->Usm[c->nsmear - 1];

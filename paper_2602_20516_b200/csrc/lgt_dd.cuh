@@ -183,11 +183,11 @@ template <class T> struct DdOps {
                 case 2: return c->ws32[3];
                 case 3: return c->ws32[4];
                 case 5: return c->ws32[0];
-                case 7: return c->U32;
+                case 7: return c->U32;  // fp32 copy of the fermions' links
                 default: return nullptr;
             }
         }
-        return k == 6 ? c->phi : k == 7 ? c->U : c->ws[k];
+        return k == 6 ? c->phi : k == 7 ? c->Uf : c->ws[k];
     }
     static int exchange_spinor(lgt_dd* d, int k) {
         std::vector<void*> f;
@@ -200,10 +200,84 @@ template <class T> struct DdOps {
         return dd_allreduce(d, p.data(), 1);
     }
 
+    // Thin-link ghosts current, then the fermions' links c->Uf of every rank: the thin links, or the stout levels built
+    // in lockstep with a halo exchange of each level's result (the next level's staples reach into the ghost slices).
+    static int fermion_links(lgt_dd* d) {
+        int rc;
+        if ((rc = dd_exchange_links(d)) != LGT_OK) return rc;
+        const int nsm = d->rk[0]->nsmear;
+        bool valid = true;
+        for (size_t i = 0; i < d->rk.size(); i++) {
+            DD_RK(i, O::ensure_fermion_links(d->rk[i]));  // allocation and c->Uf; computes nothing on a slab
+            valid = valid && d->rk[i]->usm_valid;
+        }
+        if (nsm == 0 || valid) return LGT_OK;
+        for (int k = 0; k < nsm; k++) {
+            std::vector<void*> u;
+            for (size_t i = 0; i < d->rk.size(); i++) {
+                DD_RK(i, O::smear_level(d->rk[i], k));
+                u.push_back(d->rk[i]->Usm[k]);
+            }
+            if ((rc = dd_exchange(d, u.data(), 36, sizeof(T2))) != LGT_OK) return rc;
+        }
+        for (lgt_ctx* c : d->rk) c->usm_valid = true;
+        return LGT_OK;
+    }
+    // Pi -= eps F^f from X = ws[0], Y = ws[3] (ghost slices current): the fused kernel, or with smearing the force with
+    // respect to U^(n) pulled back level by level as in Ops::fermion_force, G's ghost slices exchanged before each chain
+    static int fermion_force(lgt_dd* d, double eps) {
+        int rc;
+        const int nsm = d->rk[0]->nsmear;
+        if (nsm == 0) {
+            for (size_t i = 0; i < d->rk.size(); i++) DD_RK(i, O::fermion_force(d->rk[i], d->rk[i]->ws[0], d->rk[i]->ws[3], d->rk[i]->P, 1, eps));
+            return LGT_OK;
+        }
+        const size_t nr = d->rk.size();
+        std::vector<T2*> Fa(nr), Fb(nr);
+        for (size_t i = 0; i < nr; i++) {
+            lgt_ctx* c = d->rk[i];
+            if (!c->F2) {
+                DD_CU(cudaMalloc(&c->F2, mom_bytes(c)));
+                DD_CU(cudaMalloc(&c->F3, mom_bytes(c)));
+                DD_CU(cudaMalloc(&c->F4, mom_bytes(c)));
+                DD_CU(cudaMemsetAsync(c->F2, 0, mom_bytes(c), d->stream));
+                DD_CU(cudaMemsetAsync(c->F3, 0, mom_bytes(c), d->stream));
+                DD_CU(cudaMemsetAsync(c->F4, 0, mom_bytes(c), d->stream));
+            }
+            Fa[i] = (T2*)c->F3;
+            Fb[i] = (T2*)c->F4;
+            LAUNCH(c, LGT_K_FERMION_FORCE, (fermion_force_kernel<T, 0>), site_blocks(c, 128), 128, c->g, (const T2*)c->Uf, (const T2*)c->ws[0],
+                   (const T2*)c->ws[3], Fa[i], (T)c->kappa, (T)0);
+        }
+        for (int k = nsm - 1; k >= 0; k--) {
+            std::vector<void*> g;
+            for (size_t i = 0; i < nr; i++) {
+                lgt_ctx* c = d->rk[i];
+                LAUNCH(c, LGT_K_FERMION_FORCE, (stout_local_kernel<T>), site_blocks(c, 32), 128, c->g, (const T2*)c->Asm[k], Fa[i], (T2*)c->F2);
+                g.push_back(c->F2);
+            }
+            if ((rc = dd_exchange(d, g.data(), 16, sizeof(T2))) != LGT_OK) return rc;
+            for (size_t i = 0; i < nr; i++) {
+                lgt_ctx* c = d->rk[i];
+                const T2* Uk = (const T2*)(k == 0 ? c->U : c->Usm[k - 1]);
+                if (k == 0)
+                    LAUNCH(c, LGT_K_FERMION_FORCE, (stout_chain_kernel<T, 1>), site_blocks(c, 32), 128, c->g, Uk, (const T2*)c->F2, (const T2*)Fa[i],
+                           (T2*)c->P, (T)c->rho, (T)eps);
+                else
+                    LAUNCH(c, LGT_K_FERMION_FORCE, (stout_chain_kernel<T, 0>), site_blocks(c, 32), 128, c->g, Uk, (const T2*)c->F2, (const T2*)Fa[i],
+                           Fb[i], (T)c->rho, (T)0);
+                T2* t = Fa[i];
+                Fa[i] = Fb[i];
+                Fb[i] = t;
+            }
+        }
+        return LGT_OK;
+    }
+
     // out = D in (or D^dag in) on the fields ws[in], ws[out] of every rank
     static int dslash(lgt_dd* d, int in, int out, int dagger) {
         int rc;
-        if ((rc = dd_exchange_links(d)) != LGT_OK) return rc;
+        if ((rc = fermion_links(d)) != LGT_OK) return rc;
         if ((rc = exchange_spinor(d, in)) != LGT_OK) return rc;
         for (size_t i = 0; i < d->rk.size(); i++) {
             lgt_ctx* c = d->rk[i];
@@ -216,7 +290,7 @@ template <class T> struct DdOps {
     // if want_y.  Same recurrence, stop rule and fused kernels as Ops::cg; every sum is all-reduced over the ranks.
     static int cg(lgt_dd* d, int ib, bool want_y, double tol, int max_iter, int* iters, double* rel) {
         int rc;
-        if ((rc = dd_exchange_links(d)) != LGT_OK) return rc;
+        if (!fp32_on_f64(d->rk[0]) && (rc = fermion_links(d)) != LGT_OK) return rc;  // (the mixed driver has done it in fp64)
         const int n = (int)d->rk.size();
         for (int i = 0; i < n; i++) {
             lgt_ctx* c = d->rk[i];
@@ -314,11 +388,7 @@ template <class T> struct DdOps {
             else if (rc != LGT_OK) return rc;
             if ((rc = exchange_spinor(d, 0)) != LGT_OK) return rc;  // X(x + mu)
             if ((rc = exchange_spinor(d, 3)) != LGT_OK) return rc;  // Y(x + mu)
-            for (size_t i = 0; i < d->rk.size(); i++) {
-                lgt_ctx* c = d->rk[i];
-                c->Uf = c->U;
-                DD_RK(i, O::fermion_force(c, c->ws[0], c->ws[3], c->P, 1, eps));
-            }
+            if ((rc = fermion_force(d, eps)) != LGT_OK) return rc;
         }
         if (cg_iters) *cg_iters = it;
         return conv;
@@ -412,7 +482,7 @@ template <class T> struct DdOps {
     // X_e = (M^dag M)^-1 phi_e on every rank; then, if want_xy, the full fields X = ws[0], Y = ws[3] of the force kernel
     static int eo_solve(lgt_dd* d, bool want_xy, double tol, int max_iter, int* iters, bool sf_to_slot2) {
         int rc;
-        if ((rc = dd_exchange_links(d)) != LGT_OK) return rc;
+        if ((rc = fermion_links(d)) != LGT_OK) return rc;
         const int n = (int)d->rk.size();
         for (int i = 0; i < n; i++) {
             lgt_ctx* c = d->rk[i];
@@ -500,7 +570,7 @@ template <class T> struct DdOps {
         if (d->rk[0]->kappa == 0.0) return LGT_OK;
         if (d->rk[0]->action != LGT_ACTION_EO) return dslash(d, 4, 6, 1);  // phi = D^dag eta
         // even/odd action: phi_e = M^dag eta_e, phi_o = 0; eta_e stays in the even member of fields (4, 5) for |eta_e|^2
-        if ((rc = dd_exchange_links(d)) != LGT_OK) return rc;
+        if ((rc = fermion_links(d)) != LGT_OK) return rc;
         for (size_t i = 0; i < d->rk.size(); i++) {
             lgt_ctx* c = d->rk[i];
             DD_RK(i, O::eo_ensure(c));
@@ -573,7 +643,7 @@ int dd_cg_mixed(lgt_dd* d, int ib, bool want_y, double tol, int max_iter, int* i
     typedef DdOps<double> D64;
     typedef DdOps<float> D32;
     int rc;
-    if ((rc = dd_exchange_links(d)) != LGT_OK) return rc;
+    if ((rc = D64::fermion_links(d)) != LGT_OK) return rc;
     const int n = (int)d->rk.size();
     std::vector<double*> slot;
     for (int i = 0; i < n; i++) {
@@ -588,7 +658,7 @@ int dd_cg_mixed(lgt_dd* d, int ib, bool want_y, double tol, int max_iter, int* i
             c->u32_valid = false;
         }
         if (!c->u32_valid) {  // ghost slices included: the links were exchanged above
-            LAUNCH(c, LGT_K_OTHER, down_convert_kernel, stream_blocks(c, nu), 256, nu, (const double2*)c->U, (float2*)c->U32, 1.0);
+            LAUNCH(c, LGT_K_OTHER, down_convert_kernel, stream_blocks(c, nu), 256, nu, (const double2*)c->Uf, (float2*)c->U32, 1.0);
             c->u32_valid = true;
         }
         const size_t off = D64::spinor_off(c), cnt = D64::spinor_n(c);
@@ -890,6 +960,17 @@ int lgt_dd_set_fermion_action(lgt_dd* d, int action) {
                                           "per slab and Lx*Ly*Lz a multiple of 64");
     }
     for (lgt_ctx* c : d->rk) c->action = action;
+    return LGT_OK;
+}
+int lgt_dd_set_smearing(lgt_dd* d, int n_levels, double rho) {
+    CHECK_DD(d);
+    if (n_levels < 0 || n_levels > LGT_MAX_SMEAR) return dd_fail(d, LGT_EINVAL, "lgt_dd_set_smearing: n_levels must be in 0..8");
+    if (n_levels > 0 && !(rho >= 0.0)) return dd_fail(d, LGT_EINVAL, "lgt_dd_set_smearing: rho must be >= 0");
+    for (lgt_ctx* c : d->rk) {
+        c->nsmear = n_levels;
+        c->rho = n_levels ? rho : 0.0;
+        c->usm_valid = c->u32_valid = c->ucb_valid = c->ucb32_valid = false;
+    }
     return LGT_OK;
 }
 int lgt_dd_set_solver(lgt_dd* d, int solver, double inner_tol) {

@@ -321,3 +321,44 @@ def test_dd_even_odd_action(lgt, nranks):
             lgt.lgt_dd_set_fermion_action(bad, lgt.LGT_ACTION_EO)
         finally:
             lgt.lgt_dd_destroy(bad)
+
+
+@pytest.mark.parametrize("nranks,levels", [(2, 1), (4, 2), (1, 2)])
+def test_dd_stout_smearing(lgt, nranks, levels):
+    """Stout-smeared fermions on slabs: every level's ghost slices are exchanged before the next level, G's before each
+    chain kernel.  Dslash on the smeared links and the kick (gauge force on thin links + pulled-back fermion force)
+    against the oracle on the undivided lattice; with the even/odd action on top for one case."""
+    from oracle import stout as ost
+
+    dims, beta, kappa, rho = (4, 4, 4, 8), 5.6, 0.11, 0.3
+    U0 = synth.warm_links(dims, 0.25, 601)
+    P0 = synth.gaussian_momenta(dims, 602)
+    Un = ost.smear_levels(dims, rho, levels, U0)[0][-1]
+    psi = synth.gaussian_spinor(dims, 603)
+    phi = oracle.dslash(dims, kappa, BC, Un, psi, dagger=True)
+    dd = lgt.DecomposedLattice(dims, nranks, list(range(nranks)), beta, kappa, BC)
+    lgt.lgt_dd_set_smearing(dd.d, levels, rho)
+    lgt.lgt_dd_set_halo_mode(dd.d, lgt.LGT_DD_PUSH)
+    dd.set_links(U0)
+    assert np.abs(cat(dd.dslash(psi)) - oracle.dslash(dims, kappa, BC, Un, psi)).max() < 1e-12
+    dd.set_momenta(P0)
+    dd.set_pseudofermion(phi)
+    it = lgt.lgt_dd_md_kick(dd.d, 0.05, 1e-13, 5000)
+    Ff, it_ref, ok = ost.fermion_force(dims, kappa, BC, U0, phi, levels, rho, 1e-13, 5000)
+    assert ok and it == it_ref
+    P_ref = P0 - 0.05 * (oracle.gauge_force(dims, beta, U0) + Ff)
+    assert link_rel_err(cat(dd.get_momenta()), P_ref)[0] < TOL64
+    # after a drift the smeared links follow the new thin links
+    lgt.lgt_dd_md_drift(dd.d, 0.05)
+    U1 = oracle.drift(dims, 0.05, P_ref, U0)
+    assert np.abs(cat(dd.dslash(psi)) - oracle.dslash(dims, kappa, BC, ost.smear_levels(dims, rho, levels, U1)[0][-1], psi)).max() < 1e-11
+    if levels == 1:
+        from oracle import evenodd as oeo
+        lgt.lgt_dd_set_fermion_action(dd.d, lgt.LGT_ACTION_EO)
+        dd.set_links(U0)
+        dd.set_momenta(P0)
+        Xe, Ye, _, _ = oeo.solve_xy(dims, kappa, BC, Un, phi, 1e-13, 5000)
+        Feo = ost.pull_back(dims, rho, U0, ost.smear(dims, rho, U0)[1], oracle.fermion_force(dims, kappa, BC, Un, Xe, Ye))[0]
+        lgt.lgt_dd_md_kick(dd.d, 0.05, 1e-13, 5000)
+        assert link_rel_err(cat(dd.get_momenta()), P0 - 0.05 * (oracle.gauge_force(dims, beta, U0) + Feo))[0] < TOL64
+    dd.close()
