@@ -207,7 +207,7 @@ int lgt_get_smeared_links(lgt_ctx* ctx, void* U);
  * State goes in and out through the rank handles: lgt_dd_rank(d, i) returns a handle on which ONLY lgt_set_links,
  * lgt_get_links, lgt_set_momenta, lgt_get_momenta, lgt_set_pseudofermion, lgt_get_pseudofermion (+ _host forms),
  * lgt_timing_* and lgt_launch_count may be called (slab arrays); everything else on it returns LGT_ESTATE.
- * Full operator (plain or mixed-precision CG) or even/odd action, stout-smeared fermion links, leapfrog. */
+ * Full operator (plain or mixed-precision CG) or even/odd action, stout-smeared fermion links, all three integrators. */
 typedef struct lgt_dd lgt_dd;
 int lgt_dd_create(lgt_dd** out, const int dims[4], int nranks, int nlocal, const int* local_ranks, double beta, double kappa,
                   const int bc[4], int precision, int device, void* cuda_stream);
@@ -233,7 +233,7 @@ int lgt_dd_ipc_export(lgt_dd* d, void* handles128);
 int lgt_dd_ipc_import(lgt_dd* d, const void* lo_handles128, const void* hi_handles128);
 int lgt_dd_local_ranks(const lgt_dd* d);
 lgt_ctx* lgt_dd_rank(lgt_dd* d, int local_index);
-/* The decomposed forms of lgt_dslash, lgt_cg, lgt_action, lgt_md_kick, lgt_md_drift, lgt_md_trajectory (leapfrog):
+/* The decomposed forms of lgt_dslash, lgt_cg, lgt_action, lgt_md_kick, lgt_md_drift, lgt_md_trajectory:
  * same mathematics, same kernels on each slab's interior, sums taken over all ranks; scalar outputs are global. */
 int lgt_dd_dslash(lgt_dd* d, const void* const* in, void* const* out, int dagger);
 int lgt_dd_cg(lgt_dd* d, const void* const* b, void* const* x, double tol, int max_iter, int* iters, double* rel_resid);
@@ -250,11 +250,13 @@ int lgt_dd_set_fermion_action(lgt_dd* d, int action);
  * slices exchanged before the next level; in the force recursion the ghost slices of G are exchanged before each
  * chain kernel. */
 int lgt_dd_set_smearing(lgt_dd* d, int n_levels, double rho);
+/* lgt_set_integrator for lgt_dd_md_trajectory and lgt_dd_hmc_trajectory (the same kick / drift sequences). */
+int lgt_dd_set_integrator(lgt_dd* d, int integrator, int n_inner);
 int lgt_dd_md_kick(lgt_dd* d, double eps, double tol, int max_iter, int* cg_iters);
 int lgt_dd_md_drift(lgt_dd* d, double eps);
 int lgt_dd_md_trajectory(lgt_dd* d, int nsteps, double dt, double tol, int max_iter, double* H_initial, double* H_final,
                          long* cg_iters);
-/* lgt_hmc_trajectory on the decomposed lattice (leapfrog): the heat baths draw by GLOBAL element number, so momenta,
+/* lgt_hmc_trajectory on the decomposed lattice: the heat baths draw by GLOBAL element number, so momenta,
  * pseudofermion, dH and the decision are those of the undivided lattice; every rank takes the same decision from the
  * same all-reduced numbers. */
 int lgt_dd_hmc_trajectory(lgt_dd* d, int nsteps, double dt, double tol, int max_iter, unsigned long long seed,

@@ -726,8 +726,10 @@ int kick(lgt_ctx* c, double eps, double tol, int max_iter, int* cg_iters) {
     return kick_fermion(c, eps, tol, max_iter, cg_iters);
 }
 
-// MD trajectory of nsteps steps of size dt with the handle's integrator, adjacent kicks merged (include/lgt.h).
-int integrate(lgt_ctx* c, int nsteps, double dt, double tol, int max_iter, long* cg_iters) {
+// MD trajectory of nsteps steps of size dt, adjacent kicks merged (include/lgt.h "lgt_set_integrator").  S supplies the
+// moves: kick(eps, &it) with both forces, kick_gauge(eps), kick_fermion(eps, &it), drift(eps) -- one handle, or all slabs
+// of a decomposed lattice in lockstep.
+template <class S> int integrate_with(S& s, int integrator, int n_inner, int nsteps, double dt, long* cg_iters) {
     int rc, it = 0, conv = LGT_OK;
     long total = 0;
 #define STEP(call)                           \
@@ -738,39 +740,50 @@ int integrate(lgt_ctx* c, int nsteps, double dt, double tol, int max_iter, long*
         else if (rc != LGT_OK) return rc;    \
         total += it;                         \
     } while (0)
-#define DRIFT(eps) STEP(DISPATCH(c, link_update, c, (eps)))
-    if (nsteps > 0 && c->integrator == LGT_INT_LEAPFROG) {
-        STEP(kick(c, 0.5 * dt, tol, max_iter, &it));
+    if (nsteps > 0 && integrator == LGT_INT_LEAPFROG) {
+        STEP(s.kick(0.5 * dt, &it));
         for (int n = 0; n < nsteps; n++) {
-            DRIFT(dt);
-            STEP(kick(c, (n == nsteps - 1) ? 0.5 * dt : dt, tol, max_iter, &it));
+            STEP(s.drift(dt));
+            STEP(s.kick((n == nsteps - 1) ? 0.5 * dt : dt, &it));
         }
-    } else if (nsteps > 0 && c->integrator == LGT_INT_OMELYAN) {
+    } else if (nsteps > 0 && integrator == LGT_INT_OMELYAN) {
         const double lam = 0.1931833275037836;
-        STEP(kick(c, lam * dt, tol, max_iter, &it));
+        STEP(s.kick(lam * dt, &it));
         for (int n = 0; n < nsteps; n++) {
-            DRIFT(0.5 * dt);
-            STEP(kick(c, (1.0 - 2.0 * lam) * dt, tol, max_iter, &it));
-            DRIFT(0.5 * dt);
-            STEP(kick(c, (n == nsteps - 1) ? lam * dt : 2.0 * lam * dt, tol, max_iter, &it));
+            STEP(s.drift(0.5 * dt));
+            STEP(s.kick((1.0 - 2.0 * lam) * dt, &it));
+            STEP(s.drift(0.5 * dt));
+            STEP(s.kick((n == nsteps - 1) ? lam * dt : 2.0 * lam * dt, &it));
         }
     } else if (nsteps > 0) {  // Sexton-Weingarten: fermion force outside, m gauge leapfrog steps inside
-        const int m = c->n_inner;
+        const int m = n_inner;
         const double h = dt / m;
-        STEP(kick_fermion(c, 0.5 * dt, tol, max_iter, &it));
+        STEP(s.kick_fermion(0.5 * dt, &it));
         for (int n = 0; n < nsteps; n++) {
-            STEP(kick_gauge(c, 0.5 * h));
+            STEP(s.kick_gauge(0.5 * h));
             for (int i = 0; i < m; i++) {
-                DRIFT(h);
-                STEP(kick_gauge(c, (i == m - 1) ? 0.5 * h : h));
+                STEP(s.drift(h));
+                STEP(s.kick_gauge((i == m - 1) ? 0.5 * h : h));
             }
-            STEP(kick_fermion(c, (n == nsteps - 1) ? 0.5 * dt : dt, tol, max_iter, &it));
+            STEP(s.kick_fermion((n == nsteps - 1) ? 0.5 * dt : dt, &it));
         }
     }
-#undef DRIFT
 #undef STEP
     if (cg_iters) *cg_iters = total;
     return conv;
+}
+struct HandleMoves {
+    lgt_ctx* c;
+    double tol;
+    int max_iter;
+    int kick(double eps, int* it) { return ::kick(c, eps, tol, max_iter, it); }
+    int kick_gauge(double eps) { return ::kick_gauge(c, eps); }
+    int kick_fermion(double eps, int* it) { return ::kick_fermion(c, eps, tol, max_iter, it); }
+    int drift(double eps) { return DISPATCH(c, link_update, c, eps); }
+};
+int integrate(lgt_ctx* c, int nsteps, double dt, double tol, int max_iter, long* cg_iters) {
+    HandleMoves m{c, tol, max_iter};
+    return integrate_with(m, c->integrator, c->n_inner, nsteps, dt, cg_iters);
 }
 
 int hamiltonian(lgt_ctx* c, double tol, int max_iter, double* S_g, double* S_F, double* K, int* cg_iters) {

@@ -377,11 +377,16 @@ template <class T> struct DdOps {
         return LGT_OK;
     }
 
-    // Pi -= eps (F^g + F^f) on every rank
-    static int kick(lgt_dd* d, double eps, double tol, int max_iter, int* cg_iters) {
-        int rc, it = 0, conv = LGT_OK;
+    // Pi -= eps F^g on every rank
+    static int kick_gauge(lgt_dd* d, double eps) {
+        int rc;
         if ((rc = dd_exchange_links(d)) != LGT_OK) return rc;
         for (size_t i = 0; i < d->rk.size(); i++) DD_RK(i, O::gauge_force(d->rk[i], d->rk[i]->P, 1, eps));
+        return LGT_OK;
+    }
+    // Pi -= eps F^f on every rank (solve, halo of X and Y, force kernels); nothing without fermions
+    static int kick_fermion(lgt_dd* d, double eps, double tol, int max_iter, int* cg_iters) {
+        int rc, it = 0, conv = LGT_OK;
         if (fermions_on(d->rk[0])) {
             rc = d->rk[0]->action == LGT_ACTION_EO ? eo_solve(d, true, tol, max_iter, &it, false) : dd_solve(d, 6, true, tol, max_iter, &it);
             if (rc == LGT_ENOCONV) conv = rc;
@@ -392,6 +397,12 @@ template <class T> struct DdOps {
         }
         if (cg_iters) *cg_iters = it;
         return conv;
+    }
+    // Pi -= eps (F^g + F^f) on every rank
+    static int kick(lgt_dd* d, double eps, double tol, int max_iter, int* cg_iters) {
+        int rc;
+        if ((rc = kick_gauge(d, eps)) != LGT_OK) return rc;
+        return kick_fermion(d, eps, tol, max_iter, cg_iters);
     }
 
     static int drift(lgt_dd* d, double eps) {
@@ -556,6 +567,20 @@ template <class T> struct DdOps {
         return LGT_OK;
     }
 
+    struct Moves {
+        lgt_dd* d;
+        double tol;
+        int max_iter;
+        int kick(double eps, int* it) { return DdOps::kick(d, eps, tol, max_iter, it); }
+        int kick_gauge(double eps) { return DdOps::kick_gauge(d, eps); }
+        int kick_fermion(double eps, int* it) { return DdOps::kick_fermion(d, eps, tol, max_iter, it); }
+        int drift(double eps) { return DdOps::drift(d, eps); }
+    };
+    static int integrate(lgt_dd* d, int nsteps, double dt, double tol, int max_iter, long* cg_iters) {
+        Moves m{d, tol, max_iter};
+        return integrate_with(m, d->rk[0]->integrator, d->rk[0]->n_inner, nsteps, dt, cg_iters);
+    }
+
     // Heat baths by global element number (reading A-25), so that the fields are those of the undivided lattice
     static int heatbaths(lgt_dd* d, unsigned long long seed, unsigned traj) {
         int rc;
@@ -599,29 +624,20 @@ template <class T> struct DdOps {
         if ((rc = heatbaths(d, seed, traj)) != LGT_OK) return rc;
         if ((rc = action(d, tol, max_iter, &sg, &sf, &k, &it, true)) != LGT_OK) return rc;
         const double H0 = k + sg + sf;
-#define DD_HSTEP(call)                     \
-    do {                                   \
-        it = 0;                            \
-        rc = (call);                       \
-        if (rc == LGT_ENOCONV) conv = rc;  \
-        else if (rc != LGT_OK) return rc;  \
-        total += it;                       \
-    } while (0)
-        if (nsteps > 0) {
-            DD_HSTEP(kick(d, 0.5 * dt, tol, max_iter, &it));
-            for (int n = 0; n < nsteps; n++) {
-                DD_HSTEP(drift(d, dt));
-                DD_HSTEP(kick(d, (n == nsteps - 1) ? 0.5 * dt : dt, tol, max_iter, &it));
-            }
-        }
-        DD_HSTEP(action(d, tol, max_iter, &sg, &sf, &k, &it));
-#undef DD_HSTEP
+        rc = integrate(d, nsteps, dt, tol, max_iter, &total);
+        if (rc == LGT_ENOCONV) conv = rc;
+        else if (rc != LGT_OK) return rc;
+        it = 0;
+        rc = action(d, tol, max_iter, &sg, &sf, &k, &it);
+        if (rc == LGT_ENOCONV) conv = rc;
+        else if (rc != LGT_OK) return rc;
+        total += it;
         const double dh = (k + sg + sf) - H0;
         const bool acc = metropolis_uniform(seed, traj) < exp(-dh);  // the same all-reduced numbers on every rank
         if (!acc) {
             for (lgt_ctx* c : d->rk) {
                 DD_CU(cudaMemcpyAsync(c->U, c->Usave, links_bytes(c), cudaMemcpyDeviceToDevice, d->stream));
-                c->usm_valid = c->u32_valid = c->ucb_valid = false;
+                c->usm_valid = c->u32_valid = c->ucb_valid = c->ucb32_valid = false;
             }
             d->links_ghost_valid = true;  // saved with current ghosts
         }
@@ -931,15 +947,9 @@ int lgt_dd_md_trajectory(lgt_dd* d, int nsteps, double dt, double tol, int max_i
         DD_STEP(DD_DISPATCH(d, action, d, tol, max_iter, &sg, &sf, &k, &it));
         *H_initial = k + sg + sf;
     }
-    if (nsteps > 0) {
-        DD_STEP(DD_DISPATCH(d, kick, d, 0.5 * dt, tol, max_iter, &it));
-        total += it;
-        for (int n = 0; n < nsteps; n++) {
-            DD_STEP(DD_DISPATCH(d, drift, d, dt));
-            DD_STEP(DD_DISPATCH(d, kick, d, (n == nsteps - 1) ? 0.5 * dt : dt, tol, max_iter, &it));
-            total += it;
-        }
-    }
+    rc = DD_DISPATCH(d, integrate, d, nsteps, dt, tol, max_iter, &total);
+    if (rc == LGT_ENOCONV) conv = rc;
+    else if (rc != LGT_OK) return rc;
     if (H_final) {
         DD_STEP(DD_DISPATCH(d, action, d, tol, max_iter, &sg, &sf, &k, &it));
         *H_final = k + sg + sf;
@@ -960,6 +970,17 @@ int lgt_dd_set_fermion_action(lgt_dd* d, int action) {
                                           "per slab and Lx*Ly*Lz a multiple of 64");
     }
     for (lgt_ctx* c : d->rk) c->action = action;
+    return LGT_OK;
+}
+int lgt_dd_set_integrator(lgt_dd* d, int integrator, int n_inner) {
+    CHECK_DD(d);
+    if (integrator != LGT_INT_LEAPFROG && integrator != LGT_INT_OMELYAN && integrator != LGT_INT_SEXTON_WEINGARTEN)
+        return dd_fail(d, LGT_EINVAL, "lgt_dd_set_integrator: unknown integrator");
+    if (integrator == LGT_INT_SEXTON_WEINGARTEN && n_inner < 1) return dd_fail(d, LGT_EINVAL, "lgt_dd_set_integrator: n_inner must be >= 1");
+    for (lgt_ctx* c : d->rk) {
+        c->integrator = integrator;
+        c->n_inner = integrator == LGT_INT_SEXTON_WEINGARTEN ? n_inner : 1;
+    }
     return LGT_OK;
 }
 int lgt_dd_set_smearing(lgt_dd* d, int n_levels, double rho) {

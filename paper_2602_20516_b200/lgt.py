@@ -80,6 +80,7 @@ SYMBOLS = {
     "lgt_dd_set_solver": (_i, [_vp, _i, _d]),
     "lgt_dd_set_fermion_action": (_i, [_vp, _i]),
     "lgt_dd_set_smearing": (_i, [_vp, _i, _d]),
+    "lgt_dd_set_integrator": (_i, [_vp, _i, _i]),
     "lgt_dd_md_kick": (_i, [_vp, _d, _d, _i, _ip]),
     "lgt_dd_md_drift": (_i, [_vp, _d]),
     "lgt_dd_md_trajectory": (_i, [_vp, _i, _d, _d, _i, _dp, _dp, _lp]),
@@ -478,6 +479,10 @@ def lgt_dd_action(d, tol=1e-12, max_iter=100000):
 
 def lgt_dd_set_solver(d, solver, inner_tol=1e-5):
     _dd_check(d, lib().lgt_dd_set_solver(d, solver, inner_tol))
+
+
+def lgt_dd_set_integrator(d, integrator, n_inner=1):
+    _dd_check(d, lib().lgt_dd_set_integrator(d, integrator, n_inner))
 
 
 def lgt_dd_set_smearing(d, n_levels, rho=0.0):

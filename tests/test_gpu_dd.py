@@ -362,3 +362,29 @@ def test_dd_stout_smearing(lgt, nranks, levels):
         lgt.lgt_dd_md_kick(dd.d, 0.05, 1e-13, 5000)
         assert link_rel_err(cat(dd.get_momenta()), P0 - 0.05 * (oracle.gauge_force(dims, beta, U0) + Feo))[0] < TOL64
     dd.close()
+
+
+@pytest.mark.parametrize("integ,m", [("omelyan", 1), ("sw", 3)])
+def test_dd_integrators(lgt, integ, m):
+    """Omelyan and Sexton-Weingarten on two slabs against the oracle's integrators on the undivided lattice."""
+    from oracle import hmc as ohmc
+
+    dims, beta, kappa = (4, 4, 2, 8), 5.5, 0.10
+    U0 = synth.warm_links(dims, 0.2, 611)
+    P0 = synth.gaussian_momenta(dims, 612)
+    phi = oracle.dslash(dims, kappa, BC, U0, synth.gaussian_spinor(dims, 613), dagger=True)
+    dd = lgt.DecomposedLattice(dims, 2, [0, 1], beta, kappa, BC)
+    dd.set_links(U0)
+    dd.set_momenta(P0)
+    dd.set_pseudofermion(phi)
+    code = lgt.LGT_INT_OMELYAN if integ == "omelyan" else lgt.LGT_INT_SEXTON_WEINGARTEN
+    ocode = ohmc.OMELYAN if integ == "omelyan" else ohmc.SEXTON_WEINGARTEN
+    lgt.lgt_dd_set_integrator(dd.d, code, m)
+    H0, H1, its = lgt.lgt_dd_md_trajectory(dd.d, 3, 0.04, tol=1e-13, max_iter=5000)
+    U_ref, P_ref, its_ref = ohmc.integrate(dims, beta, kappa, BC, U0, phi, P0, 3, 0.04, ocode, n_inner=m, tol=1e-13, max_iter=5000)
+    assert its == its_ref
+    assert np.abs(cat(dd.get_links()) - U_ref).max() < 1e-12
+    assert link_rel_err(cat(dd.get_momenta()), P_ref)[0] < TOL64
+    with pytest.raises(lgt.LgtError):
+        lgt.lgt_dd_set_integrator(dd.d, 9, 1)
+    dd.close()
