@@ -243,7 +243,8 @@ int lgt_dd_action(lgt_dd* d, double tol, int max_iter, double* S_g, double* S_F,
  * all-reduced residual.  lgt_dd_cg itself is always the plain CG. */
 int lgt_dd_set_solver(lgt_dd* d, int solver, double inner_tol);
 /* lgt_set_fermion_action for the decomposed lattice: LGT_ACTION_EO runs CG on the Schur complement with the half fields'
- * ghost slices exchanged before every hop (plain fp64 / fp32 CG; the mixed solver applies to LGT_ACTION_FULL only).
+ * ghost slices exchanged before every hop; with LGT_SOLVER_MIXED_CG the decomposed fp32 CG on the Schur complement runs
+ * inside the fp64 defect correction.
  * Needs even extents, an even number of time slices per slab and Lx*Ly*Lz % 64 == 0, else LGT_EINVAL. */
 int lgt_dd_set_fermion_action(lgt_dd* d, int action);
 /* lgt_set_smearing for the decomposed lattice: every level's links are built on the slabs' interiors and their ghost

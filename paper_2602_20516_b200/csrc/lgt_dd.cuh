@@ -161,6 +161,8 @@ namespace {
 
 // (D^dag D) x = b with the group's solver (plain CG, or the mixed-precision defect correction on LGT_F64 groups)
 int dd_solve(lgt_dd* d, int ib, bool want_y, double tol, int max_iter, int* iters);
+// mixed-precision form of the even/odd solve (defined after the driver)
+int dd_eo_cg_mixed(lgt_dd* d, double tol, int max_iter, int* iters);
 
 // The driver: every step loops over the local ranks (one in production, all of them in the single-GPU verification
 // mode), then does the step's communication, so that both transports run the same sequence of launches.
@@ -491,17 +493,20 @@ template <class T> struct DdOps {
     static T2* hR(lgt_ctx* c) { return Od(c, 4); }  // the odd half of the split source is free: CG residual
 
     // X_e = (M^dag M)^-1 phi_e on every rank; then, if want_xy, the full fields X = ws[0], Y = ws[3] of the force kernel
-    static int eo_solve(lgt_dd* d, bool want_xy, double tol, int max_iter, int* iters, bool sf_to_slot2) {
+    // the k-th half field of this precision's set (for DdOps<float> on an LGT_F64 group: the fp32 set b, e, r, p, u, t)
+    template <int K> static T2* F(lgt_ctx* c) { return O::eo_field(c, K); }
+    // CG on M^dag M over the globally even sites of every rank: x = 0 start, the recurrence, stop rule and fused kernels
+    // of Ops::eo_cg, input ghost slices exchanged before every hop, sums all-reduced.  B, X, R, P, U: even half fields,
+    // Tt: an odd scratch field.  Returns the final recurrence state through *state.
+    static int eo_cg_loop(lgt_dd* d, HalfSel B, HalfSel X, HalfSel R, HalfSel P, HalfSel Uu, HalfSel Tt, double tol, int max_iter,
+                          CgState* state) {
         int rc;
-        if ((rc = fermion_links(d)) != LGT_OK) return rc;
         const int n = (int)d->rk.size();
         for (int i = 0; i < n; i++) {
             lgt_ctx* c = d->rk[i];
-            DD_RK(i, O::eo_ensure(c));
-            DD_RK(i, O::eo_split(c, c->phi, O::eo_field(c, 4)));
             const size_t off = half_off(c), cnt = half_n(c);
-            LAUNCH(c, LGT_K_CG_BLAS, (cg_init_kernel<T>), stream_blocks(c, cnt), 256, cnt, (const T2*)hB(c) + off, hXe(c) + off, hR(c) + off,
-                   hP(c) + off, c->st, tol * tol, max_iter, c->partials, c->counter);
+            LAUNCH(c, LGT_K_CG_BLAS, (cg_init_kernel<T>), stream_blocks(c, cnt), 256, cnt, (const T2*)B(c) + off, X(c) + off, R(c) + off,
+                   P(c) + off, c->st, tol * tol, max_iter, c->partials, c->counter);
             LAUNCH(c, LGT_K_CG_BLAS, cg_rr_to_tmp_kernel, 1, 1, c->st);
         }
         if ((rc = allreduce_tmp(d)) != LGT_OK) return rc;
@@ -529,22 +534,46 @@ template <class T> struct DdOps {
             if (chunk > 8) chunk = 8;
             if (chunk <= 0) chunk = 1;
             for (int it = 0; it < chunk; it++) {
-                if ((rc = hop_all(d, false, hP, nullptr, hT, 0, 3, false)) != LGT_OK) return rc;  // t_o = kappa H_oe p
-                if ((rc = hop_all(d, true, hT, hP, hYe, 0, 1, true)) != LGT_OK) return rc;         // u = M p, |u|^2
+                if ((rc = hop_all(d, false, P, nullptr, Tt, 0, 3, false)) != LGT_OK) return rc;   // t_o = kappa H_oe p
+                if ((rc = hop_all(d, true, Tt, P, Uu, 0, 1, true)) != LGT_OK) return rc;           // u = M p, |u|^2
                 if ((rc = sum_and(1)) != LGT_OK) return rc;
-                if ((rc = hop_all(d, false, hYe, nullptr, hT, 1, 3, false)) != LGT_OK) return rc;  // t_o = kappa H_oe^dag u
-                if ((rc = hop_all(d, true, hT, hYe, nullptr, 1, 2, true, hR)) != LGT_OK) return rc;  // r -= alpha M^dag u
+                if ((rc = hop_all(d, false, Uu, nullptr, Tt, 1, 3, false)) != LGT_OK) return rc;  // t_o = kappa H_oe^dag u
+                if ((rc = hop_all(d, true, Tt, Uu, nullptr, 1, 2, true, R)) != LGT_OK) return rc;  // r -= alpha M^dag u
                 if ((rc = sum_and(2)) != LGT_OK) return rc;
                 for (int i = 0; i < n; i++) {
                     lgt_ctx* c = d->rk[i];
                     const size_t off = half_off(c), cnt = half_n(c);
-                    LAUNCH(c, LGT_K_CG_BLAS, (cg_update_xp_kernel<T>), stream_blocks(c, cnt), 256, cnt, hXe(c) + off, hP(c) + off,
-                           (const T2*)hR(c) + off, c->st, launched + it + 1);
+                    LAUNCH(c, LGT_K_CG_BLAS, (cg_update_xp_kernel<T>), stream_blocks(c, cnt), 256, cnt, X(c) + off, P(c) + off,
+                           (const T2*)R(c) + off, c->st, launched + it + 1);
                 }
             }
             launched += chunk;
         }
-        const CgState h = *c0->h_st;
+        *state = *c0->h_st;
+        return LGT_OK;
+    }
+
+    // X_e = (M^dag M)^-1 phi_e on every rank; then, if want_xy, the full fields X = ws[0], Y = ws[3] of the force kernel
+    static int eo_solve(lgt_dd* d, bool want_xy, double tol, int max_iter, int* iters, bool sf_to_slot2) {
+        int rc;
+        if ((rc = fermion_links(d)) != LGT_OK) return rc;
+        const int n = (int)d->rk.size();
+        for (int i = 0; i < n; i++) {
+            lgt_ctx* c = d->rk[i];
+            DD_RK(i, O::eo_ensure(c));
+            DD_RK(i, O::eo_split(c, c->phi, O::eo_field(c, 4)));
+        }
+        CgState h;
+        memset(&h, 0, sizeof h);
+        bool converged = true;
+        if (d->prec == LGT_F64 && sizeof(T) == 8 && d->rk[0]->solver == LGT_SOLVER_MIXED_CG) {
+            rc = dd_eo_cg_mixed(d, tol, max_iter, &h.iter);
+            if (rc == LGT_ENOCONV) converged = false;
+            else if (rc != LGT_OK) return rc;
+        } else {
+            if ((rc = eo_cg_loop(d, hB, hXe, hR, hP, hYe, hT, tol, max_iter, &h)) != LGT_OK) return rc;
+            converged = !(h.rr > h.tol2 * h.bb);
+        }
         if (iters) *iters = h.iter;
         if (sf_to_slot2)
             for (int i = 0; i < n; i++) {
@@ -563,7 +592,7 @@ template <class T> struct DdOps {
                 DD_RK(i, O::eo_merge(c, O::eo_field(c, 2), c->ws[3]));
             }
         }
-        if (h.rr > h.tol2 * h.bb) return dd_fail(d, LGT_ENOCONV, "even/odd CG did not reach the tolerance within max_iter");
+        if (!converged) return dd_fail(d, LGT_ENOCONV, "even/odd CG did not reach the tolerance within max_iter");
         return LGT_OK;
     }
 
@@ -734,6 +763,90 @@ int dd_cg_mixed(lgt_dd* d, int ib, bool want_y, double tol, int max_iter, int* i
     (void)want_y;  // Y = D x is what the last residual evaluation left in ws[3]
     if (iters) *iters = total;
     if (conv != LGT_OK) return dd_fail(d, LGT_ENOCONV, "mixed-precision CG did not reach the tolerance");
+    return LGT_OK;
+}
+
+// (M^dag M) x_e = phi_e on the slabs in mixed precision: eo_cg_mixed()'s defect correction with the decomposed fp32 CG
+// inside and the all-reduced true fp64 residual outside.  fp64 half fields: b = even of (4,5), x = even of (0,1),
+// r = odd of (4,5), q = field 6, u = even of (2,3), t = field 7 (the assignment of DdOps<double>::eo_solve).
+int dd_eo_cg_mixed(lgt_dd* d, double tol, int max_iter, int* iters) {
+    typedef DdOps<double> D64;
+    typedef DdOps<float> D32;
+    int rc;
+    const int n = (int)d->rk.size();
+    std::vector<double*> slot;
+    for (int i = 0; i < n; i++) {
+        lgt_ctx* c = d->rk[i];
+        const size_t nh = (size_t)12 * c->g.Vhs, nu = (size_t)2 * 36 * c->g.Vhs;
+        if (!c->Ucb32) {
+            DD_CU(cudaMalloc(&c->Ucb32, nu * sizeof(float2)));
+            DD_CU(cudaMalloc(&c->eo32, 6 * nh * sizeof(float2)));
+            DD_CU(cudaMemsetAsync(c->eo32, 0, 6 * nh * sizeof(float2), d->stream));
+            c->ucb32_valid = false;
+        }
+        if (!c->ucb32_valid) {
+            LAUNCH(c, LGT_K_OTHER, down_convert_kernel, stream_blocks(c, nu), 256, nu, (const double2*)c->Ucb, (float2*)c->Ucb32, 1.0);
+            c->ucb32_valid = true;
+        }
+        const size_t off = D64::half_off(c), cnt = D64::half_n(c);
+        DD_CU(cudaMemsetAsync(D64::hXe(c), 0, nh * sizeof(double2), d->stream));
+        DD_CU(cudaMemcpyAsync(D64::hR(c), D64::hB(c), nh * sizeof(double2), cudaMemcpyDeviceToDevice, d->stream));
+        LAUNCH(c, LGT_K_OTHER, (redot_kernel<double>), stream_blocks(c, cnt), 256, cnt, (const double2*)D64::hB(c) + off,
+               (const double2*)D64::hB(c) + off, c->scal + 3, c->partials, c->counter);
+        slot.push_back(c->scal + 3);
+    }
+    lgt_ctx* c0 = d->rk[0];
+    auto read_sum = [&](double& out) -> int {
+        int r2 = dd_allreduce(d, slot.data(), 1);
+        if (r2 != LGT_OK) return r2;
+        DD_CU(cudaMemcpyAsync(c0->h_scal + 3, c0->scal + 3, sizeof(double), cudaMemcpyDeviceToHost, d->stream));
+        DD_CU(cudaStreamSynchronize(d->stream));
+        out = c0->h_scal[3];
+        return LGT_OK;
+    };
+    double bb = 0.0;
+    if ((rc = read_sum(bb)) != LGT_OK) return rc;
+    double rr = bb;
+    int total = 0, outer = 0, conv = LGT_OK;
+    while (bb > 0.0 && rr > tol * tol * bb) {
+        if (total >= max_iter || outer >= 40) {
+            conv = LGT_ENOCONV;
+            break;
+        }
+        const double scale = 1.0 / sqrt(rr);
+        for (int i = 0; i < n; i++) {
+            lgt_ctx* c = d->rk[i];
+            const size_t nh = (size_t)12 * c->g.Vhs;
+            LAUNCH(c, LGT_K_CG_BLAS, down_convert_kernel, stream_blocks(c, nh), 256, nh, (const double2*)D64::hR(c), D32::template F<0>(c), scale);
+        }
+        double eps = 0.25 * tol * sqrt(bb / rr);
+        if (eps < c0->inner_tol) eps = c0->inner_tol;
+        CgState st32;
+        rc = D32::eo_cg_loop(d, D32::template F<0>, D32::template F<1>, D32::template F<2>, D32::template F<3>, D32::template F<4>,
+                             D32::template F<5>, eps, max_iter - total, &st32);
+        if (rc != LGT_OK) return rc;
+        total += st32.iter;
+        outer++;
+        for (int i = 0; i < n; i++) {
+            lgt_ctx* c = d->rk[i];
+            const size_t off = D64::half_off(c), cnt = D64::half_n(c);
+            LAUNCH(c, LGT_K_CG_BLAS, up_axpy_kernel, stream_blocks(c, cnt), 256, cnt, (double2*)D64::hXe(c) + off,
+                   (const float2*)D32::template F<1>(c) + off, 1.0 / scale);
+        }
+        if ((rc = D64::hop_all(d, false, D64::hXe, nullptr, D64::hT, 0, 0, false)) != LGT_OK) return rc;  // u = M x
+        if ((rc = D64::hop_all(d, true, D64::hT, D64::hXe, D64::hYe, 0, 0, true)) != LGT_OK) return rc;
+        if ((rc = D64::hop_all(d, false, D64::hYe, nullptr, D64::hT, 1, 0, false)) != LGT_OK) return rc;  // q = M^dag u
+        if ((rc = D64::hop_all(d, true, D64::hT, D64::hYe, D64::hP, 1, 0, true)) != LGT_OK) return rc;
+        for (int i = 0; i < n; i++) {
+            lgt_ctx* c = d->rk[i];
+            const size_t off = D64::half_off(c), cnt = D64::half_n(c);
+            LAUNCH(c, LGT_K_CG_BLAS, residual_kernel, stream_blocks(c, cnt), 256, cnt, (const double2*)D64::hB(c) + off,
+                   (const double2*)D64::hP(c) + off, (double2*)D64::hR(c) + off, c->scal + 3, c->partials, c->counter);
+        }
+        if ((rc = read_sum(rr)) != LGT_OK) return rc;
+    }
+    if (iters) *iters = total;
+    if (conv != LGT_OK) return dd_fail(d, LGT_ENOCONV, "mixed-precision even/odd CG did not reach the tolerance");
     return LGT_OK;
 }
 

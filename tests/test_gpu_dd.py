@@ -388,3 +388,37 @@ def test_dd_integrators(lgt, integ, m):
     with pytest.raises(lgt.LgtError):
         lgt.lgt_dd_set_integrator(dd.d, 9, 1)
     dd.close()
+
+
+@pytest.mark.parametrize("nranks", [2, 4])
+def test_dd_even_odd_mixed_precision(lgt, nranks):
+    """The fastest configuration on slabs: even/odd action with the mixed-precision solver (decomposed fp32 CG on the Schur
+    complement inside the fp64 defect correction); kick and action against the oracle's fp64 even/odd mode."""
+    from oracle import evenodd as oeo
+
+    dims, beta, kappa, tol = (4, 4, 4, 8), 5.6, 0.12, 1e-12
+    V = synth.volume(dims)
+    U0 = synth.warm_links(dims, 0.3, 621)
+    P0 = synth.gaussian_momenta(dims, 622)
+    phi = oeo.mhat(dims, kappa, BC, U0, oeo.keep(synth.gaussian_spinor(dims, 623), dims, 0), dagger=True)
+    F_ref, it_ref, _ = oeo.fermion_force(dims, kappa, BC, U0, phi, tol, 10 * V)
+    dd = lgt.DecomposedLattice(dims, nranks, list(range(nranks)), beta, kappa, BC)
+    lgt.lgt_dd_set_fermion_action(dd.d, lgt.LGT_ACTION_EO)
+    lgt.lgt_dd_set_solver(dd.d, lgt.LGT_SOLVER_MIXED_CG, 1e-5)
+    dd.set_links(U0)
+    dd.set_momenta(P0)
+    dd.set_pseudofermion(phi)
+    it = lgt.lgt_dd_md_kick(dd.d, 0.05, tol, 10 * V)
+    assert 0 < it < 2 * it_ref + 20
+    P1 = P0 - 0.05 * (oracle.gauge_force(dims, beta, U0) + F_ref)
+    assert link_rel_err(cat(dd.get_momenta()), P1)[0] < 1e-10
+    _, S_F, _, _ = lgt.lgt_dd_action(dd.d, tol, 10 * V)
+    S_ref = oeo.action(dims, kappa, BC, U0, phi, tol, 10 * V)[0]
+    assert abs(S_F - S_ref) < 1e-10 * abs(S_ref)
+    # after a drift the fp32 checkerboard links follow
+    lgt.lgt_dd_md_drift(dd.d, 0.05)
+    U1 = oracle.drift(dims, 0.05, P1, U0)
+    lgt.lgt_dd_md_kick(dd.d, 0.05, tol, 10 * V)
+    F1, _, _ = oeo.fermion_force(dims, kappa, BC, U1, phi, tol, 10 * V)
+    assert link_rel_err(cat(dd.get_momenta()), P1 - 0.05 * (oracle.gauge_force(dims, beta, U1) + F1))[0] < 1e-10
+    dd.close()
