@@ -550,6 +550,12 @@ def run_decomposed(args):
     U, P, eta = make_inputs(cfg)  # every rank draws the same global fields and keeps its slab
     stream = torch.cuda.current_stream().cuda_stream
     dd = dist.decomposed_lattice(dims, beta, kappa, bc, lgt.LGT_F64, local, stream, halo=args.halo)
+    if args.action == "eo":
+        lgt.lgt_dd_set_fermion_action(dd.d, lgt.LGT_ACTION_EO)
+    if args.solver == "mixed":
+        lgt.lgt_dd_set_solver(dd.d, lgt.LGT_SOLVER_MIXED_CG, 1e-5)
+    if args.smear:
+        lgt.lgt_dd_set_smearing(dd.d, args.smear, 0.3)
     lo, hi = dist.slab_rows(dims, world, rank)
     hU, hP = torch.from_numpy(U[lo:hi].copy()).pin_memory(), torch.from_numpy(P[lo:hi].copy()).pin_memory()
     ctx = dd.ranks[0]
@@ -603,8 +609,8 @@ def run_decomposed(args):
     e2e_s = time.perf_counter() - t0
     (elapsed_ms, e2e_s), (launches_all,) = dist.aggregate([elapsed_ms, e2e_s], [launches], device="cuda")
     if rank == 0:
-        total_reals = sum(step_reals(i) for i in iters) * V  # the whole lattice: strong scaling
-        e2e_reals = sum(step_reals(i) for i in e2e_iters) * V
+        total_reals = sum(step_reals(i, args.solver, args.action, args.smear) for i in iters) * V  # the whole lattice: strong scaling
+        e2e_reals = sum(step_reals(i, args.solver, args.action, args.smear) for i in e2e_iters) * V
         out = {
             "metric": METRIC, "value": round(total_reals * 8 / (elapsed_ms * 1e-3) / 1e9, 1), "unit": "GB/s", "n_gpus": world,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": round(elapsed_ms / args.steps, 3),
@@ -613,6 +619,7 @@ def run_decomposed(args):
                                    "CG 1e-12" % (args.config, "x".join(map(str, dims)), world),
                        "beta": beta, "kappa": kappa, "bc": list(bc), "dt": dt, "cg_tol": tol, "cg_iters_per_step": iters,
                        "parallelism": "dd%d (time slabs, halo %s, NCCL all-reduce)" % (world, args.halo),
+                       "solver": args.solver, "fermion_action": args.action, "stout_levels": args.smear,
                        "l2": "inputs exceed L2 at 32^4 up to 8 slabs (links 604 MB / N per rank)"},
             "clocks": clocks,
             "e2e": {"value": round(e2e_reals * 8 / e2e_s / 1e9, 1), "unit": "GB/s", "steps": k_e2e,
