@@ -1090,13 +1090,23 @@ __device__ __forceinline__ void hop_bwd_cb(const Geom& g, const typename Vec2<T>
 //   MODE 2: r -= alpha val, block partials of |r|^2 (second half of M^dag u fused with the residual update)
 // With kap = -kappa and no self this is the odd half "t_o = kappa H_oe p_e"; with kap = +kappa and self = p_e the
 // even half "p_e - kappa H_eo t_o" of the Schur complement M = 1 - kappa^2 H_eo H_oe.
-template <class T, int DAG, int MODE>
+// PUSH (time slab, CG modes 1 and 2): as in dslash_kernel, a site of the slab's first / last interior slice also stores
+// its result (u in MODE 1, the updated r in MODE 2) into the neighbour rank's ghost slice of that half field.
+template <class T, int PUSH>
+__device__ __forceinline__ void push_halo_half(const Geom& g, const PushTo<T>& to, int c, int k, cx<T> v) {
+    if (!PUSH) return;
+    const int V3h = g.stride[3] >> 1;
+    if (c < 2 * V3h) stc<T>(spinor_at(to.lo, c + to.lt_loc * V3h) + k * W, v);
+    if (c >= to.lt_loc * V3h) stc<T>(spinor_at(to.hi, c - to.lt_loc * V3h) + k * W, v);
+}
+
+template <class T, int DAG, int MODE, int PUSH = 0>
 __global__ void __launch_bounds__(128, 1) hop_cb_kernel(Geom g, int p, const typename Vec2<T>::type* __restrict__ Up,
                                                         const typename Vec2<T>::type* __restrict__ Uq,
                                                         const typename Vec2<T>::type* __restrict__ in,
                                                         const typename Vec2<T>::type* __restrict__ self,
                                                         typename Vec2<T>::type* __restrict__ out, T kap, CgState* st,
-                                                        double* partials, typename Vec2<T>::type* __restrict__ r) {
+                                                        double* partials, typename Vec2<T>::type* __restrict__ r, PushTo<T> push) {
     const int done = (MODE != 0) ? st->done : 0;
     const int c = g.h_begin + blockIdx.x * blockDim.x + threadIdx.x;
     double nrm = 0.0;
@@ -1133,6 +1143,7 @@ __global__ void __launch_bounds__(128, 1) hop_cb_kernel(Geom g, int p, const typ
                 rv.re = fma(-alpha, q.re, rv.re);
                 rv.im = fma(-alpha, q.im, rv.im);
                 stc<T>(br + k * W, rv);
+                push_halo_half<T, PUSH>(g, push, c, k, rv);
                 nrm += (double)rv.re * (double)rv.re + (double)rv.im * (double)rv.im;
             }
         } else {
@@ -1143,6 +1154,7 @@ __global__ void __launch_bounds__(128, 1) hop_cb_kernel(Geom g, int p, const typ
                 if (self) sv = ldc<T>(spinor_at(self, c) + k * W);
                 cx<T> o = mk<T>(fma(-kap, acc[k].re, sv.re), fma(-kap, acc[k].im, sv.im));
                 stc<T>(bo + k * W, o);
+                push_halo_half<T, PUSH>(g, push, c, k, o);
                 if (MODE == 1) nrm += (double)o.re * (double)o.re + (double)o.im * (double)o.im;
             }
         }

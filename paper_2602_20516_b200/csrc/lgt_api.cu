@@ -443,9 +443,20 @@ template <class T> struct Ops {
         return LGT_OK;
     }
     // out (parity p) = self - kap * H in (in of parity 1 - p); mode as in hop_cb_kernel
-    static int hop(lgt_ctx* c, int p, const T2* in, const T2* self, T2* out, int dagger, int mode, double kap, T2* r = nullptr) {
+    static int hop(lgt_ctx* c, int p, const T2* in, const T2* self, T2* out, int dagger, int mode, double kap, T2* r = nullptr,
+                   const PushTo<T>* push = nullptr) {
         const int grid = (own_half_sites(c) + 127) / 128;
-#define HOP_ARGS c->g, p, links_cb(c, p), links_cb(c, 1 - p), in, self, out, (T)kap, c->st, c->partials, r
+        if (push && mode == 1) {
+            LAUNCH(c, LGT_K_DSLASH, (hop_cb_kernel<T, 0, 1, 1>), grid, 128, c->g, p, links_cb(c, p), links_cb(c, 1 - p), in, self, out, (T)kap,
+                   c->st, c->partials, r, *push);
+            return LGT_OK;
+        }
+        if (push && mode == 2) {
+            LAUNCH(c, LGT_K_DSLASH_R, (hop_cb_kernel<T, 1, 2, 1>), grid, 128, c->g, p, links_cb(c, p), links_cb(c, 1 - p), in, self, out, (T)kap,
+                   c->st, c->partials, r, *push);
+            return LGT_OK;
+        }
+#define HOP_ARGS c->g, p, links_cb(c, p), links_cb(c, 1 - p), in, self, out, (T)kap, c->st, c->partials, r, PushTo<T>()
         if (mode == 0) {
             if (dagger) LAUNCH(c, LGT_K_DSLASH, (hop_cb_kernel<T, 1, 0>), grid, 128, HOP_ARGS);
             else LAUNCH(c, LGT_K_DSLASH, (hop_cb_kernel<T, 0, 0>), grid, 128, HOP_ARGS);

@@ -478,16 +478,32 @@ template <class T> struct DdOps {
     static size_t half_off(const lgt_ctx* c) { return (size_t)12 * c->g.h_begin; }
     static size_t half_n(const lgt_ctx* c) { return (size_t)12 * (c->g.h_end - c->g.h_begin); }
     // one hop on every rank, after the exchange of its input field
-    static int hop_all(lgt_dd* d, bool to_even, HalfSel in, HalfSel self, HalfSel out, int dagger, int mode, bool plus_kappa, HalfSel r = nullptr) {
+    // push: the result's boundary slices are stored into the neighbours' ghost slices by the kernel (modes 1, 2);
+    // input_current: the input's ghost slices are already up to date (pushed, or maintained locally), no exchange
+    static int hop_all(lgt_dd* d, bool to_even, HalfSel in, HalfSel self, HalfSel out, int dagger, int mode, bool plus_kappa, HalfSel r = nullptr,
+                       const std::vector<PushTo<T>>* push = nullptr, bool input_current = false) {
         int rc;
-        if ((rc = exchange_half(d, in)) != LGT_OK) return rc;
+        if (!input_current && (rc = exchange_half(d, in)) != LGT_OK) return rc;
         for (size_t i = 0; i < d->rk.size(); i++) {
             lgt_ctx* c = d->rk[i];
             const int p = to_even ? pe_of(c) : 1 - pe_of(c);
             DD_RK(i, O::hop(c, p, in(c), self ? self(c) : nullptr, out ? out(c) : nullptr, dagger, mode, plus_kappa ? c->kappa : -c->kappa,
-                            r ? r(c) : nullptr));
+                            r ? r(c) : nullptr, push ? &(*push)[i] : nullptr));
         }
         return LGT_OK;
+    }
+    // where rank i's kernels push the boundary slices of the half field `sel` (neighbours in this process only)
+    static bool push_targets(lgt_dd* d, HalfSel sel, std::vector<PushTo<T>>& to) {
+        to.resize(d->rk.size());
+        for (size_t i = 0; i < d->rk.size(); i++) {
+            const int r = d->rank_of[i];
+            const int dn = dd_local_index(d, (r + d->nranks - 1) % d->nranks), up = dd_local_index(d, (r + 1) % d->nranks);
+            if (dn < 0 || up < 0) return false;
+            to[i].lo = sel(d->rk[dn]);
+            to[i].hi = sel(d->rk[up]);
+            to[i].lt_loc = d->Lt_loc;
+        }
+        return true;
     }
     static T2* hB(lgt_ctx* c) { return E(c, 4); }
     static T2* hR(lgt_ctx* c) { return Od(c, 4); }  // the odd half of the split source is free: CG residual
@@ -511,6 +527,23 @@ template <class T> struct DdOps {
         }
         if ((rc = allreduce_tmp(d)) != LGT_OK) return rc;
         for (int i = 0; i < n; i++) LAUNCH(d->rk[i], LGT_K_CG_BLAS, (cg_apply_kernel<0>), 1, 1, d->rk[i]->st);
+        // LGT_DD_PUSH (neighbours in this process; between processes the half fields are not IPC-mapped and the exchange
+        // stays): u and r are pushed by the hops that produce them, each followed by an all-reduce that is the barrier; p's
+        // ghost slices follow by local arithmetic; the two odd intermediates t have no collective behind them and are
+        // exchanged as before.
+        std::vector<PushTo<T>> push_u, push_r;
+        const bool push = d->halo_mode == LGT_DD_PUSH && push_targets(d, Uu, push_u) && push_targets(d, R, push_r);
+        if (push) {
+            if ((rc = exchange_half(d, B)) != LGT_OK) return rc;  // r = p = b on the ghost slices too
+            const size_t slice = (size_t)6 * d->V3, hi = (size_t)(d->Lt_loc + 1) * slice;
+            for (int i = 0; i < n; i++) {
+                lgt_ctx* c = d->rk[i];
+                for (HalfSel f : {R, P}) {
+                    DD_CU(cudaMemcpyAsync(f(c), B(c), slice * sizeof(T2), cudaMemcpyDeviceToDevice, d->stream));
+                    DD_CU(cudaMemcpyAsync(f(c) + hi, B(c) + hi, slice * sizeof(T2), cudaMemcpyDeviceToDevice, d->stream));
+                }
+            }
+        }
         lgt_ctx* c0 = d->rk[0];
         int launched = 0;
         auto sum_and = [&](int what) -> int {
@@ -534,17 +567,22 @@ template <class T> struct DdOps {
             if (chunk > 8) chunk = 8;
             if (chunk <= 0) chunk = 1;
             for (int it = 0; it < chunk; it++) {
-                if ((rc = hop_all(d, false, P, nullptr, Tt, 0, 3, false)) != LGT_OK) return rc;   // t_o = kappa H_oe p
-                if ((rc = hop_all(d, true, Tt, P, Uu, 0, 1, true)) != LGT_OK) return rc;           // u = M p, |u|^2
+                if ((rc = hop_all(d, false, P, nullptr, Tt, 0, 3, false, nullptr, nullptr, push)) != LGT_OK) return rc;  // t_o = kappa H_oe p
+                if ((rc = hop_all(d, true, Tt, P, Uu, 0, 1, true, nullptr, push ? &push_u : nullptr)) != LGT_OK) return rc;  // u = M p, |u|^2
                 if ((rc = sum_and(1)) != LGT_OK) return rc;
-                if ((rc = hop_all(d, false, Uu, nullptr, Tt, 1, 3, false)) != LGT_OK) return rc;  // t_o = kappa H_oe^dag u
-                if ((rc = hop_all(d, true, Tt, Uu, nullptr, 1, 2, true, R)) != LGT_OK) return rc;  // r -= alpha M^dag u
+                if ((rc = hop_all(d, false, Uu, nullptr, Tt, 1, 3, false, nullptr, nullptr, push)) != LGT_OK) return rc;  // t_o = kappa H_oe^dag u
+                if ((rc = hop_all(d, true, Tt, Uu, nullptr, 1, 2, true, R, push ? &push_r : nullptr)) != LGT_OK) return rc;  // r -= alpha M^dag u
                 if ((rc = sum_and(2)) != LGT_OK) return rc;
                 for (int i = 0; i < n; i++) {
                     lgt_ctx* c = d->rk[i];
                     const size_t off = half_off(c), cnt = half_n(c);
                     LAUNCH(c, LGT_K_CG_BLAS, (cg_update_xp_kernel<T>), stream_blocks(c, cnt), 256, cnt, X(c) + off, P(c) + off,
                            (const T2*)R(c) + off, c->st, launched + it + 1);
+                    if (push) {
+                        const size_t slice = (size_t)6 * d->V3;
+                        LAUNCH(c, LGT_K_CG_BLAS, (cg_update_p_ghost_kernel<T>), stream_blocks(c, 2 * slice), 256, slice,
+                               (size_t)(d->Lt_loc + 1) * slice, P(c), (const T2*)R(c), c->st, launched + it + 1);
+                    }
                 }
             }
             launched += chunk;

@@ -422,3 +422,36 @@ def test_dd_even_odd_mixed_precision(lgt, nranks):
     F1, _, _ = oeo.fermion_force(dims, kappa, BC, U1, phi, tol, 10 * V)
     assert link_rel_err(cat(dd.get_momenta()), P1 - 0.05 * (oracle.gauge_force(dims, beta, U1) + F1))[0] < 1e-10
     dd.close()
+
+
+@pytest.mark.parametrize("nranks", [1, 2, 4])
+def test_dd_even_odd_pushed_halos(lgt, nranks):
+    """LGT_DD_PUSH under the even/odd action: u and r are pushed by the hops that produce them, p's ghost slices follow by
+    local arithmetic, the odd intermediates are still exchanged.  Bitwise the exchanged results, the oracle's count."""
+    from oracle import evenodd as oeo
+
+    dims, beta, kappa, tol = (4, 4, 4, 8), 5.6, 0.12, 1e-12
+    V = synth.volume(dims)
+    U0 = synth.warm_links(dims, 0.3, 631)
+    P0 = synth.gaussian_momenta(dims, 632)
+    phi = oeo.mhat(dims, kappa, BC, U0, oeo.keep(synth.gaussian_spinor(dims, 633), dims, 0), dagger=True)
+    _, it_ref, _ = oeo.fermion_force(dims, kappa, BC, U0, phi, tol, 10 * V)
+    res = {}
+    for mode in (lgt.LGT_DD_EXCHANGE, lgt.LGT_DD_PUSH):
+        dd = lgt.DecomposedLattice(dims, nranks, list(range(nranks)), beta, kappa, BC)
+        lgt.lgt_dd_set_fermion_action(dd.d, lgt.LGT_ACTION_EO)
+        lgt.lgt_dd_set_halo_mode(dd.d, mode)
+        dd.set_links(U0)
+        dd.set_momenta(P0)
+        dd.set_pseudofermion(phi)
+        H0, H1, its = lgt.lgt_dd_md_trajectory(dd.d, 2, 0.03, tol=tol, max_iter=10 * V)
+        res[mode] = (cat(dd.get_links()), cat(dd.get_momenta()), H1 - H0, its)
+        if mode == lgt.LGT_DD_PUSH:
+            lgt.lgt_dd_set_solver(dd.d, lgt.LGT_SOLVER_MIXED_CG, 1e-5)  # the fp32 inner solve pushes too
+            dd.set_links(U0)
+            dd.set_momenta(P0)
+            lgt.lgt_dd_md_trajectory(dd.d, 2, 0.03, tol=tol, max_iter=10 * V, measure=False)
+            assert link_rel_err(cat(dd.get_momenta()), res[mode][1])[0] < 1e-9
+        dd.close()
+    ex, pu = res[lgt.LGT_DD_EXCHANGE], res[lgt.LGT_DD_PUSH]
+    assert np.array_equal(ex[0], pu[0]) and np.array_equal(ex[1], pu[1]) and ex[2] == pu[2] and ex[3] == pu[3]
