@@ -332,22 +332,17 @@ __device__ __forceinline__ void hop_bwd(const Geom& g, const typename Vec2<T>::t
 //           (cg_scalars_kernel<2> finishes beta, the iteration count and the stop test).  q never touches HBM.
 // In the CG modes the convergence flag is loaded first but tested only after the first hop's loads are in
 // flight, so that its latency is not paid at the head of every block.
-// PUSH (time slab of a decomposed lattice, CG modes): a site of the slab's first / last interior time slice also stores
-// its result -- t in MODE 1, the updated r in MODE 2 -- straight into the ghost slice of the neighbour rank's copy of
-// that field (peer memory: NVLink stores, or the other slab's buffer when the ranks share a device), so the halo
-// transfer rides inside the producing kernel and the all-reduce that follows it anyway is the barrier.
+// PUSH (time slab of a decomposed lattice, CG modes): the launch covers one boundary time slice of the slab and every
+// site also stores its result -- t in MODE 1, the updated r in MODE 2 -- straight into the ghost slice of the
+// neighbour rank's copy of that field (peer memory: NVLink stores, or the other slab's buffer when the ranks share a
+// device), so the halo transfer rides inside the producing kernel and the all-reduce that follows it anyway is the
+// barrier.  PUSH 1: one target (field a, site offset da); PUSH 2: two (a slab of a single time slice feeds both
+// neighbours).  The bulk of the slab runs the PUSH 0 kernel: compiled in, the extra stores cost the big kernel ~25 %.
 template <class T> struct PushTo {
-    typename Vec2<T>::type* lo = nullptr;  // the field of rank r - 1 (its upper ghost slice receives our first interior slice)
-    typename Vec2<T>::type* hi = nullptr;  // the field of rank r + 1 (its lower ghost slice receives our last interior slice)
-    int lt_loc = 0;                        // interior time slices per slab
+    typename Vec2<T>::type* a = nullptr;
+    typename Vec2<T>::type* b = nullptr;
+    int da = 0, db = 0;
 };
-template <class T, int PUSH>
-__device__ __forceinline__ void push_halo(const Geom& g, const PushTo<T>& to, int s, int k, cx<T> v) {
-    if (!PUSH) return;
-    const int V3 = g.stride[3];
-    if (s < 2 * V3) stc<T>(spinor_at(to.lo, s + to.lt_loc * V3) + k * W, v);
-    if (s >= to.lt_loc * V3) stc<T>(spinor_at(to.hi, s - to.lt_loc * V3) + k * W, v);
-}
 
 template <class T, int DAG, int MODE, int PUSH = 0>
 __global__ void __launch_bounds__(128, 1) dslash_kernel(Geom g, const typename Vec2<T>::type* __restrict__ U,
@@ -391,7 +386,8 @@ __global__ void __launch_bounds__(128, 1) dslash_kernel(Geom g, const typename V
                 rv.re = fma(-alpha, q.re, rv.re);
                 rv.im = fma(-alpha, q.im, rv.im);
                 stc<T>(br + k * W, rv);
-                push_halo<T, PUSH>(g, push, s, k, rv);
+                if (PUSH >= 1) stc<T>(spinor_at(push.a, s + push.da) + k * W, rv);
+                if (PUSH == 2) stc<T>(spinor_at(push.b, s + push.db) + k * W, rv);
                 nrm += (double)rv.re * (double)rv.re + (double)rv.im * (double)rv.im;
             }
         } else {
@@ -401,7 +397,8 @@ __global__ void __launch_bounds__(128, 1) dslash_kernel(Geom g, const typename V
                 cx<T> pv = ldc<T>(bi + k * W);
                 cx<T> o = mk<T>(fma(-kappa, acc[k].re, pv.re), fma(-kappa, acc[k].im, pv.im));
                 stc<T>(bo + k * W, o);
-                push_halo<T, PUSH>(g, push, s, k, o);
+                if (PUSH >= 1) stc<T>(spinor_at(push.a, s + push.da) + k * W, o);
+                if (PUSH == 2) stc<T>(spinor_at(push.b, s + push.db) + k * W, o);
                 if (MODE == 1) nrm += (double)o.re * (double)o.re + (double)o.im * (double)o.im;
             }
         }
@@ -1090,16 +1087,7 @@ __device__ __forceinline__ void hop_bwd_cb(const Geom& g, const typename Vec2<T>
 //   MODE 2: r -= alpha val, block partials of |r|^2 (second half of M^dag u fused with the residual update)
 // With kap = -kappa and no self this is the odd half "t_o = kappa H_oe p_e"; with kap = +kappa and self = p_e the
 // even half "p_e - kappa H_eo t_o" of the Schur complement M = 1 - kappa^2 H_eo H_oe.
-// PUSH (time slab, CG modes 1 and 2): as in dslash_kernel, a site of the slab's first / last interior slice also stores
-// its result (u in MODE 1, the updated r in MODE 2) into the neighbour rank's ghost slice of that half field.
-template <class T, int PUSH>
-__device__ __forceinline__ void push_halo_half(const Geom& g, const PushTo<T>& to, int c, int k, cx<T> v) {
-    if (!PUSH) return;
-    const int V3h = g.stride[3] >> 1;
-    if (c < 2 * V3h) stc<T>(spinor_at(to.lo, c + to.lt_loc * V3h) + k * W, v);
-    if (c >= to.lt_loc * V3h) stc<T>(spinor_at(to.hi, c - to.lt_loc * V3h) + k * W, v);
-}
-
+// PUSH (time slab, CG modes 1 and 2): as in dslash_kernel, for the half field the launch produces (u in MODE 1, r in MODE 2).
 template <class T, int DAG, int MODE, int PUSH = 0>
 __global__ void __launch_bounds__(128, 1) hop_cb_kernel(Geom g, int p, const typename Vec2<T>::type* __restrict__ Up,
                                                         const typename Vec2<T>::type* __restrict__ Uq,
@@ -1143,7 +1131,8 @@ __global__ void __launch_bounds__(128, 1) hop_cb_kernel(Geom g, int p, const typ
                 rv.re = fma(-alpha, q.re, rv.re);
                 rv.im = fma(-alpha, q.im, rv.im);
                 stc<T>(br + k * W, rv);
-                push_halo_half<T, PUSH>(g, push, c, k, rv);
+                if (PUSH >= 1) stc<T>(spinor_at(push.a, c + push.da) + k * W, rv);
+                if (PUSH == 2) stc<T>(spinor_at(push.b, c + push.db) + k * W, rv);
                 nrm += (double)rv.re * (double)rv.re + (double)rv.im * (double)rv.im;
             }
         } else {
@@ -1154,7 +1143,8 @@ __global__ void __launch_bounds__(128, 1) hop_cb_kernel(Geom g, int p, const typ
                 if (self) sv = ldc<T>(spinor_at(self, c) + k * W);
                 cx<T> o = mk<T>(fma(-kap, acc[k].re, sv.re), fma(-kap, acc[k].im, sv.im));
                 stc<T>(bo + k * W, o);
-                push_halo_half<T, PUSH>(g, push, c, k, o);
+                if (PUSH >= 1) stc<T>(spinor_at(push.a, c + push.da) + k * W, o);
+                if (PUSH == 2) stc<T>(spinor_at(push.b, c + push.db) + k * W, o);
                 if (MODE == 1) nrm += (double)o.re * (double)o.re + (double)o.im * (double)o.im;
             }
         }

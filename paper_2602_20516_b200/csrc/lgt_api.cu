@@ -215,14 +215,18 @@ template <class T> struct Ops {
         const int grid = site_blocks(c, 128);
         const T kappa = (T)c->kappa;
 #define DSLASH_ARGS c->g, (const T2*)U, (const T2*)in, (T2*)out, kappa, c->st, c->partials, (T2*)r, PushTo<T>()
-        if (push && mode == 1) {
-            LAUNCH(c, LGT_K_DSLASH, (dslash_kernel<T, 0, 1, 1>), grid, 128, c->g, (const T2*)U, (const T2*)in, (T2*)out, kappa, c->st, c->partials, (T2*)r, *push);
+#define DSLASH_PUSH_ARGS c->g, (const T2*)U, (const T2*)in, (T2*)out, kappa, c->st, c->partials, (T2*)r, *push
+        if (push && mode == 1) {  // one target, or two when push->b is set
+            if (push->b) LAUNCH(c, LGT_K_DSLASH, (dslash_kernel<T, 0, 1, 2>), grid, 128, DSLASH_PUSH_ARGS);
+            else LAUNCH(c, LGT_K_DSLASH, (dslash_kernel<T, 0, 1, 1>), grid, 128, DSLASH_PUSH_ARGS);
             return LGT_OK;
         }
         if (push && mode == 2) {
-            LAUNCH(c, LGT_K_DSLASH_R, (dslash_kernel<T, 1, 2, 1>), grid, 128, c->g, (const T2*)U, (const T2*)in, (T2*)out, kappa, c->st, c->partials, (T2*)r, *push);
+            if (push->b) LAUNCH(c, LGT_K_DSLASH_R, (dslash_kernel<T, 1, 2, 2>), grid, 128, DSLASH_PUSH_ARGS);
+            else LAUNCH(c, LGT_K_DSLASH_R, (dslash_kernel<T, 1, 2, 1>), grid, 128, DSLASH_PUSH_ARGS);
             return LGT_OK;
         }
+#undef DSLASH_PUSH_ARGS
         if (mode == 0) {
             if (dagger)
                 LAUNCH(c, LGT_K_DSLASH, (dslash_kernel<T, 1, 0>), grid, 128, DSLASH_ARGS);
@@ -446,16 +450,18 @@ template <class T> struct Ops {
     static int hop(lgt_ctx* c, int p, const T2* in, const T2* self, T2* out, int dagger, int mode, double kap, T2* r = nullptr,
                    const PushTo<T>* push = nullptr) {
         const int grid = (own_half_sites(c) + 127) / 128;
+#define HOP_PUSH_ARGS c->g, p, links_cb(c, p), links_cb(c, 1 - p), in, self, out, (T)kap, c->st, c->partials, r, *push
         if (push && mode == 1) {
-            LAUNCH(c, LGT_K_DSLASH, (hop_cb_kernel<T, 0, 1, 1>), grid, 128, c->g, p, links_cb(c, p), links_cb(c, 1 - p), in, self, out, (T)kap,
-                   c->st, c->partials, r, *push);
+            if (push->b) LAUNCH(c, LGT_K_DSLASH, (hop_cb_kernel<T, 0, 1, 2>), grid, 128, HOP_PUSH_ARGS);
+            else LAUNCH(c, LGT_K_DSLASH, (hop_cb_kernel<T, 0, 1, 1>), grid, 128, HOP_PUSH_ARGS);
             return LGT_OK;
         }
         if (push && mode == 2) {
-            LAUNCH(c, LGT_K_DSLASH_R, (hop_cb_kernel<T, 1, 2, 1>), grid, 128, c->g, p, links_cb(c, p), links_cb(c, 1 - p), in, self, out, (T)kap,
-                   c->st, c->partials, r, *push);
+            if (push->b) LAUNCH(c, LGT_K_DSLASH_R, (hop_cb_kernel<T, 1, 2, 2>), grid, 128, HOP_PUSH_ARGS);
+            else LAUNCH(c, LGT_K_DSLASH_R, (hop_cb_kernel<T, 1, 2, 1>), grid, 128, HOP_PUSH_ARGS);
             return LGT_OK;
         }
+#undef HOP_PUSH_ARGS
 #define HOP_ARGS c->g, p, links_cb(c, p), links_cb(c, 1 - p), in, self, out, (T)kap, c->st, c->partials, r, PushTo<T>()
         if (mode == 0) {
             if (dagger) LAUNCH(c, LGT_K_DSLASH, (hop_cb_kernel<T, 1, 0>), grid, 128, HOP_ARGS);

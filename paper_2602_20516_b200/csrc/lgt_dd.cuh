@@ -164,6 +164,13 @@ int dd_solve(lgt_dd* d, int ib, bool want_y, double tol, int max_iter, int* iter
 // mixed-precision form of the even/odd solve (defined after the driver)
 int dd_eo_cg_mixed(lgt_dd* d, double tol, int max_iter, int* iters);
 
+// Where a rank's boundary slices of one field go: the same field of rank r - 1 (its upper ghost slice receives our first
+// interior slice) and of rank r + 1 (its lower ghost slice receives our last interior slice).
+template <class T> struct Neighbours {
+    typename Vec2<T>::type* lo = nullptr;
+    typename Vec2<T>::type* hi = nullptr;
+};
+
 // The driver: every step loops over the local ranks (one in production, all of them in the single-GPU verification
 // mode), then does the step's communication, so that both transports run the same sequence of launches.
 template <class T> struct DdOps {
@@ -200,6 +207,52 @@ template <class T> struct DdOps {
         std::vector<double*> p;
         for (lgt_ctx* c : d->rk) p.push_back(&c->st->tmp);
         return dd_allreduce(d, p.data(), 1);
+    }
+
+    // A pushing stencil launch over the owned range [*begin, *end) of a field with `slice` sites per time slice (a
+    // multiple of 128): the two boundary slices first, each with the PUSH kernel and its one target -- the halo stores
+    // are then in flight while the bulk computes -- then the interior with the ordinary kernel.  Block partials land
+    // where one launch over the whole range would put them, so the sums are unchanged bit for bit.
+    // `launch(push)` issues the kernel for the range currently set in c->g / c->partials (push == nullptr: no push).
+    template <class Launch>
+    static int split_launch(lgt_ctx* c, int* begin, int* end, int slice, int lt_loc, const Neighbours<T>& nb, Launch launch) {
+        const int b0 = *begin, e0 = *end;
+        double* const part0 = c->partials;
+        int rc;
+        PushTo<T> to;
+        if (lt_loc == 1) {  // the one slice feeds both neighbours
+            to.a = nb.lo;
+            to.da = slice;
+            to.b = nb.hi;
+            to.db = -slice;
+            return launch(&to);
+        }
+        *end = b0 + slice;  // first interior slice -> upper ghost slice of rank r - 1
+        to.a = nb.lo;
+        to.da = lt_loc * slice;
+        rc = launch(&to);
+        if (rc == LGT_OK) {
+            *begin = e0 - slice;  // last interior slice -> lower ghost slice of rank r + 1
+            *end = e0;
+            c->partials = part0 + (e0 - slice - b0) / 128;
+            to.a = nb.hi;
+            to.da = -lt_loc * slice;
+            rc = launch(&to);
+        }
+        if (rc == LGT_OK && lt_loc > 2) {
+            *begin = b0 + slice;  // the bulk
+            *end = e0 - slice;
+            c->partials = part0 + slice / 128;
+            rc = launch(nullptr);
+        }
+        *begin = b0;
+        *end = e0;
+        c->partials = part0;
+        return rc;
+    }
+    static int dslash_pushing(lgt_dd* d, lgt_ctx* c, const void* in, void* out, int dagger, int mode, void* r, const Neighbours<T>& nb) {
+        return split_launch(c, &c->g.s_begin, &c->g.s_end, d->V3, d->Lt_loc, nb,
+                            [&](const PushTo<T>* push) { return O::dslash(c, fld(c, 7), in, out, dagger, mode, r, push); });
     }
 
     // Thin-link ghosts current, then the fermions' links c->Uf of every rank: the thin links, or the stout levels built
@@ -306,8 +359,8 @@ template <class T> struct DdOps {
         for (int i = 0; i < n; i++) LAUNCH(d->rk[i], LGT_K_CG_BLAS, (cg_apply_kernel<0>), 1, 1, d->rk[i]->st);
         // pushed halos need the neighbours' buffers of THIS precision: always there for local neighbours, mapped through
         // IPC only for the handle's own precision
-        const bool push = d->halo_mode == LGT_DD_PUSH && (d->rk.size() == (size_t)d->nranks || !fp32_on_f64(d->rk[0]));
-        std::vector<PushTo<T>> push_t(n), push_r(n);
+        const bool push = d->halo_mode == LGT_DD_PUSH && d->V3 % 128 == 0 && (d->rk.size() == (size_t)d->nranks || !fp32_on_f64(d->rk[0]));
+        std::vector<Neighbours<T>> push_t(n), push_r(n);
         if (push) {
             // r = p = b on the ghost slices too (one ordinary exchange of b); from here on p's ghosts follow by local
             // arithmetic and the ghosts of t and r are written by the neighbours' Dslash kernels
@@ -326,7 +379,6 @@ template <class T> struct DdOps {
                 push_r[i].hi = (T2*)(up >= 0 ? fld(d->rk[up], 1) : d->ipc_peer[0][1]);
                 push_t[i].lo = (T2*)(dn >= 0 ? fld(d->rk[dn], 3) : d->ipc_peer[1][0]);
                 push_t[i].hi = (T2*)(up >= 0 ? fld(d->rk[up], 3) : d->ipc_peer[1][1]);
-                push_r[i].lt_loc = push_t[i].lt_loc = d->Lt_loc;
                 if (!push_r[i].lo || !push_r[i].hi || !push_t[i].lo || !push_t[i].hi)
                     return dd_fail(d, LGT_ESTATE, "LGT_DD_PUSH: the neighbours' buffers are not mapped (lgt_dd_ipc_import)");
             }
@@ -344,7 +396,8 @@ template <class T> struct DdOps {
                 if (!push && (rc = exchange_spinor(d, 2)) != LGT_OK) return rc;  // p
                 for (int i = 0; i < n; i++) {
                     lgt_ctx* c = d->rk[i];
-                    DD_RK(i, O::dslash(c, fld(c, 7), fld(c, 2), fld(c, 3), 0, 1, nullptr, push ? &push_t[i] : nullptr));  // t = D p, partials of |t|^2
+                    if (push) DD_RK(i, dslash_pushing(d, c, fld(c, 2), fld(c, 3), 0, 1, nullptr, push_t[i]));
+                    else DD_RK(i, O::dslash(c, fld(c, 7), fld(c, 2), fld(c, 3), 0, 1));  // t = D p, partials of |t|^2
                     LAUNCH(c, LGT_K_CG_BLAS, cg_partial_sum_kernel, 1, 1024, site_blocks(c, 128), c->partials, c->st);
                 }
                 if ((rc = allreduce_tmp(d)) != LGT_OK) return rc;
@@ -352,7 +405,8 @@ template <class T> struct DdOps {
                 if (!push && (rc = exchange_spinor(d, 3)) != LGT_OK) return rc;  // t
                 for (int i = 0; i < n; i++) {
                     lgt_ctx* c = d->rk[i];
-                    DD_RK(i, O::dslash(c, fld(c, 7), fld(c, 3), nullptr, 1, 2, fld(c, 1), push ? &push_r[i] : nullptr));  // r -= alpha D^dag t, partials of |r|^2
+                    if (push) DD_RK(i, dslash_pushing(d, c, fld(c, 3), nullptr, 1, 2, fld(c, 1), push_r[i]));
+                    else DD_RK(i, O::dslash(c, fld(c, 7), fld(c, 3), nullptr, 1, 2, fld(c, 1)));  // r -= alpha D^dag t, partials of |r|^2
                     LAUNCH(c, LGT_K_CG_BLAS, cg_partial_sum_kernel, 1, 1024, site_blocks(c, 128), c->partials, c->st);
                 }
                 if ((rc = allreduce_tmp(d)) != LGT_OK) return rc;
@@ -481,19 +535,24 @@ template <class T> struct DdOps {
     // push: the result's boundary slices are stored into the neighbours' ghost slices by the kernel (modes 1, 2);
     // input_current: the input's ghost slices are already up to date (pushed, or maintained locally), no exchange
     static int hop_all(lgt_dd* d, bool to_even, HalfSel in, HalfSel self, HalfSel out, int dagger, int mode, bool plus_kappa, HalfSel r = nullptr,
-                       const std::vector<PushTo<T>>* push = nullptr, bool input_current = false) {
+                       const std::vector<Neighbours<T>>* push = nullptr, bool input_current = false) {
         int rc;
         if (!input_current && (rc = exchange_half(d, in)) != LGT_OK) return rc;
         for (size_t i = 0; i < d->rk.size(); i++) {
             lgt_ctx* c = d->rk[i];
             const int p = to_even ? pe_of(c) : 1 - pe_of(c);
-            DD_RK(i, O::hop(c, p, in(c), self ? self(c) : nullptr, out ? out(c) : nullptr, dagger, mode, plus_kappa ? c->kappa : -c->kappa,
-                            r ? r(c) : nullptr, push ? &(*push)[i] : nullptr));
+            const double kap = plus_kappa ? c->kappa : -c->kappa;
+            if (push)
+                DD_RK(i, split_launch(c, &c->g.h_begin, &c->g.h_end, d->V3 / 2, d->Lt_loc, (*push)[i], [&](const PushTo<T>* to) {
+                          return O::hop(c, p, in(c), self ? self(c) : nullptr, out ? out(c) : nullptr, dagger, mode, kap, r ? r(c) : nullptr, to);
+                      }));
+            else
+                DD_RK(i, O::hop(c, p, in(c), self ? self(c) : nullptr, out ? out(c) : nullptr, dagger, mode, kap, r ? r(c) : nullptr));
         }
         return LGT_OK;
     }
     // where rank i's kernels push the boundary slices of the half field `sel` (neighbours in this process only)
-    static bool push_targets(lgt_dd* d, HalfSel sel, std::vector<PushTo<T>>& to) {
+    static bool push_targets(lgt_dd* d, HalfSel sel, std::vector<Neighbours<T>>& to) {
         to.resize(d->rk.size());
         for (size_t i = 0; i < d->rk.size(); i++) {
             const int r = d->rank_of[i];
@@ -501,7 +560,6 @@ template <class T> struct DdOps {
             if (dn < 0 || up < 0) return false;
             to[i].lo = sel(d->rk[dn]);
             to[i].hi = sel(d->rk[up]);
-            to[i].lt_loc = d->Lt_loc;
         }
         return true;
     }
@@ -531,8 +589,8 @@ template <class T> struct DdOps {
         // stays): u and r are pushed by the hops that produce them, each followed by an all-reduce that is the barrier; p's
         // ghost slices follow by local arithmetic; the two odd intermediates t have no collective behind them and are
         // exchanged as before.
-        std::vector<PushTo<T>> push_u, push_r;
-        const bool push = d->halo_mode == LGT_DD_PUSH && push_targets(d, Uu, push_u) && push_targets(d, R, push_r);
+        std::vector<Neighbours<T>> push_u, push_r;
+        const bool push = d->halo_mode == LGT_DD_PUSH && (d->V3 / 2) % 128 == 0 && push_targets(d, Uu, push_u) && push_targets(d, R, push_r);
         if (push) {
             if ((rc = exchange_half(d, B)) != LGT_OK) return rc;  // r = p = b on the ghost slices too
             const size_t slice = (size_t)6 * d->V3, hi = (size_t)(d->Lt_loc + 1) * slice;

@@ -184,8 +184,10 @@ def test_dd_full_size_dslash_four_slabs(lgt):
 def test_dd_pushed_halos_are_bitwise_the_exchanged_ones(lgt, nranks):
     """LGT_DD_PUSH: the Dslash kernels of the CG loop store their boundary slices into the neighbours' ghost slices and
     the ghosts of p follow by local arithmetic; no separate transfer inside the iteration.  Same iterates bit for bit
-    as with the separate exchange, the oracle's iteration count, and the MD trajectory on top of it."""
-    dims, beta, kappa = (4, 4, 2, 8), 5.6, 0.12
+    as with the separate exchange, the oracle's iteration count, and the MD trajectory on top of it.  Time slices of 128
+    sites, so that the boundary slices run the pushing kernel and the bulk the ordinary one (8 slabs: one slice per slab
+    feeds both neighbours; 4 slabs: no bulk)."""
+    dims, beta, kappa = (8, 4, 4, 8), 5.6, 0.12
     U = synth.warm_links(dims, 0.3, 561)
     P0 = synth.gaussian_momenta(dims, 562)
     b = oracle.dslash(dims, kappa, BC, U, synth.gaussian_spinor(dims, 563), dagger=True)
@@ -427,10 +429,11 @@ def test_dd_even_odd_mixed_precision(lgt, nranks):
 @pytest.mark.parametrize("nranks", [1, 2, 4])
 def test_dd_even_odd_pushed_halos(lgt, nranks):
     """LGT_DD_PUSH under the even/odd action: u and r are pushed by the hops that produce them, p's ghost slices follow by
-    local arithmetic, the odd intermediates are still exchanged.  Bitwise the exchanged results, the oracle's count."""
+    local arithmetic, the odd intermediates are still exchanged.  Bitwise the exchanged results, the oracle's count.
+    Half-field time slices of 128 sites (boundary / bulk split of the pushing hops)."""
     from oracle import evenodd as oeo
 
-    dims, beta, kappa, tol = (4, 4, 4, 8), 5.6, 0.12, 1e-12
+    dims, beta, kappa, tol = (8, 8, 4, 8), 5.6, 0.12, 1e-12
     V = synth.volume(dims)
     U0 = synth.warm_links(dims, 0.3, 631)
     P0 = synth.gaussian_momenta(dims, 632)
