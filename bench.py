@@ -321,11 +321,11 @@ def run_ours(args):
         # the decomposed path (lgt_dd_*) on this one GPU: 1 and 4 time slabs in one process, halo exchange by device copies
         import numpy as np
         U_np, P_np, phi_np = hU.numpy(), hP.numpy(), hphi.numpy()
-        for nr in (1, 4):
+        for nr, halo in ((1, "exchange"), (1, "push"), (4, "exchange")):
             if dims[3] % nr or (dims[0] * dims[1] * dims[2]) % 32:
                 continue
             dd = lgt.DecomposedLattice(dims, nr, list(range(nr)), beta, kappa, bc, lgt.LGT_F64, local, stream)
-            lgt.lgt_dd_set_halo_mode(dd.d, lgt.LGT_DD_PUSH)  # halos stored by the Dslash kernels themselves
+            lgt.lgt_dd_set_halo_mode(dd.d, lgt.LGT_DD_PUSH if halo == "push" else lgt.LGT_DD_EXCHANGE)
 
             def dd_reset():
                 dd.set_links(U_np)
@@ -345,10 +345,10 @@ def run_ours(args):
             dd_iters = [dd_step() for _ in range(2)]
             b.record()
             torch.cuda.synchronize()
-            extras["decomposed_%d_slabs_one_gpu" % nr] = {
+            extras["decomposed_%d_slabs_%s_one_gpu" % (nr, halo)] = {
                 "ms_per_step": round(a.elapsed_time(b) / 2, 3), "cg_iters_per_step": dd_iters,
-                "note": "same MD step through lgt_dd_* (LGT_DD_PUSH) with %d time slab(s) resident on this GPU: the cost of the "
-                        "ghost slices, pushed halos and split reductions, not a multi-GPU number" % nr}
+                "note": "same MD step through lgt_dd_* with %d time slab(s) resident on this GPU, halo mode %s: the cost of the "
+                        "ghost slices, halo traffic and split reductions, not a multi-GPU number" % (nr, halo)}
             dd.close()
             del dd
 
