@@ -41,7 +41,7 @@ FLOPS = dict(dslash=1368, dslash_fused_r=1368 + 96, cg_update_xp=96, cg_iter=2 *
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel from the ncu --set full capture
 # summarised in profiles/ (None until captured for the current kernel).
-NCU_TRAFFIC_BYTES = {"dslash_f64_32^4": 1020500000}  # profiles/r01e_ncu_cg.md, dslash_kernel<double,0,1>: 1.0205 GB
+NCU_TRAFFIC_BYTES = {"dslash_f64_32^4": 1019771616}  # profiles/r01f_ncu_cg.md, dslash_kernel<double,0,1,0>: 1.0198 GB
 
 
 # even/odd action, per site of the FULL lattice: a half-lattice hop reads 8 links + 1 spinor and writes 1 spinor per
