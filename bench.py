@@ -384,6 +384,28 @@ def run_ours(args):
                     "so this is context (PAPER.md:143-148), not a like-for-like ratio"}
         lat24.close()
 
+    # ---- the whole method end to end on the paper's other lattice size: HMC trajectories at 16^4 with everything on
+    if rank == 0 and not args.skip_extras and not variant:
+        d16 = (16, 16, 16, 16)
+        lat16 = lgt.Lattice(d16, beta, kappa, bc, lgt.LGT_F64, local, stream)
+        lat16.set_links(synth.warm_links(d16, 0.3, 1601))
+        lgt.lgt_set_fermion_action(lat16.ctx, lgt.LGT_ACTION_EO)
+        lgt.lgt_set_solver(lat16.ctx, lgt.LGT_SOLVER_MIXED_CG, 1e-5)
+        lgt.lgt_set_smearing(lat16.ctx, 1, 0.3)
+        lgt.lgt_set_integrator(lat16.ctx, lgt.LGT_INT_SEXTON_WEINGARTEN, 10)
+        lgt.lgt_hmc_trajectory(lat16.ctx, 10, 0.02, 16, 0, tol=1e-10)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        res16 = [lgt.lgt_hmc_trajectory(lat16.ctx, 10, 0.02, 16, t, tol=1e-10) for t in range(1, 5)]
+        torch.cuda.synchronize()
+        extras["hmc_trajectory_16^4"] = {
+            "ms_per_trajectory": round((time.perf_counter() - t0) / 4 * 1e3, 2), "md_steps": 10, "dt": 0.02,
+            "dH": [round(r[0], 4) for r in res16], "accepted": [bool(r[1]) for r in res16], "cg_iters": [r[2] for r in res16],
+            "plaquette": round(lgt.lgt_plaquette(lat16.ctx), 5),
+            "note": "heat baths, even/odd action, mixed-precision solver (true residual 1e-10), one stout level rho = 0.3, "
+                    "Sexton-Weingarten with 10 inner gauge steps, Metropolis: the paper's second HMC set-up (PAPER.md:154-156) at 16^4"}
+        lat16.close()
+
     # ---- max over ranks, aggregate
     (elapsed_ms, e2e_s), (total_reals, total_flops, e2e_reals, launches_all) = dist.aggregate(
         [elapsed_ms, e2e_s], [total_reals, total_flops, e2e_reals, launches], device="cuda")

@@ -865,7 +865,7 @@ template <class T> int eo_cg_canonical(lgt_ctx* c, const void* b, void* x, doubl
 
 extern "C" {
 
-const char* lgt_version(void) { return "lgt-b200 0.1 (sm_100a)"; }
+const char* lgt_version(void) { return "lgt-b200 0.2 (sm_100a)"; }
 
 const char* lgt_last_error(const lgt_ctx* c) { return c ? c->err.c_str() : g_create_error.c_str(); }
 
