@@ -63,7 +63,7 @@ struct CgState {
     int iter;
     int max_iter;
     int done;
-    int pad;
+    int fresh;     // set by the beta step of an iteration that really ran, cleared by the next alpha step: "x, p update due"
     double tmp;    // decomposed lattice: this rank's part of a sum, then (after the all-reduce) the global sum
 };
 
@@ -189,7 +189,10 @@ __device__ __forceinline__ void block_partial(double v, double* partials) {
 //   WHAT 2 (after r -= alpha q):   beta = sum / rr, rr = sum, iteration count, convergence flag
 template <int WHAT>
 __global__ void __launch_bounds__(1024) cg_scalars_kernel(int n, const double* __restrict__ partials, CgState* st) {
-    if (st->done) return;
+    const int done = st->done;
+    __syncthreads();
+    if (WHAT == 1 && threadIdx.x == 0) st->fresh = 0;  // every block of the previous x, p update has read it: kernels are ordered
+    if (done) return;
     __shared__ double warp_sums[32];
     double a16[16];
 #pragma unroll
@@ -223,6 +226,7 @@ __global__ void __launch_bounds__(1024) cg_scalars_kernel(int n, const double* _
                 st->beta = sum / st->rr;
                 st->rr = sum;
                 st->iter += 1;
+                st->fresh = 1;
                 st->done = (!(sum > st->tol2 * st->bb) || st->iter >= st->max_iter) ? 1 : 0;
             }
         }
@@ -269,15 +273,19 @@ template <int WHAT> __global__ void cg_apply_kernel(CgState* st) {
         st->rr = sum;
         st->bb = sum;
         st->done = (!(sum > st->tol2 * sum) || st->max_iter <= 0) ? 1 : 0;
+        st->fresh = 0;
     } else if (st->done) {
+        if (WHAT == 1) st->fresh = 0;
         return;
     } else if (WHAT == 1) {
+        st->fresh = 0;
         st->pAp = sum;
         st->alpha = st->rr / sum;
     } else {
         st->beta = sum / st->rr;
         st->rr = sum;
         st->iter += 1;
+        st->fresh = 1;
         st->done = (!(sum > st->tol2 * st->bb) || st->iter >= st->max_iter) ? 1 : 0;
     }
 }
@@ -440,19 +448,20 @@ __global__ void __launch_bounds__(256) cg_init_kernel(size_t n, const typename V
         st->tol2 = tol2;
         st->iter = 0;
         st->max_iter = max_iter;
+        st->fresh = 0;
         st->done = (!(sum > tol2 * sum) || max_iter <= 0) ? 1 : 0;
     });
 }
 
-// CG step 3 of iteration `iteration`: x += alpha p, then (unless converged) p = r + beta p.  One pass over x, p, r.
-// Runs only if step 2 of the same iteration ran (st->iter == iteration), so launches enqueued past convergence
-// do nothing and the last x update is never lost.
+// CG step 3: x += alpha p, then (unless converged) p = r + beta p.  One pass over x, p, r.
+// Runs only if step 2 of the same iteration ran (st->fresh), so launches enqueued past convergence do nothing and
+// the last x update is never lost; no argument changes from launch to launch, so a chunk of iterations can be replayed
+// as a CUDA graph.
 template <class T>
 __global__ void __launch_bounds__(256) cg_update_xp_kernel(size_t n, typename Vec2<T>::type* __restrict__ x,
                                                            typename Vec2<T>::type* __restrict__ p,
-                                                           const typename Vec2<T>::type* __restrict__ r, const CgState* st,
-                                                           int iteration) {
-    if (st->iter != iteration) return;
+                                                           const typename Vec2<T>::type* __restrict__ r, const CgState* st) {
+    if (!st->fresh) return;
     const T alpha = (T)st->alpha, beta = (T)st->beta;
     const bool done = st->done != 0;
     for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
@@ -473,9 +482,8 @@ __global__ void __launch_bounds__(256) cg_update_xp_kernel(size_t n, typename Ve
 // copy of r (bitwise the owner's arithmetic), so p never travels.  n complex numbers from each of the two ghost slices.
 template <class T>
 __global__ void __launch_bounds__(256) cg_update_p_ghost_kernel(size_t n, size_t hi_offset, typename Vec2<T>::type* __restrict__ p,
-                                                                const typename Vec2<T>::type* __restrict__ r, const CgState* st,
-                                                                int iteration) {
-    if (st->iter != iteration || st->done) return;
+                                                                const typename Vec2<T>::type* __restrict__ r, const CgState* st) {
+    if (!st->fresh || st->done) return;
     const T beta = (T)st->beta;
     for (size_t j = blockIdx.x * (size_t)blockDim.x + threadIdx.x; j < 2 * n; j += (size_t)gridDim.x * blockDim.x) {
         const size_t i = j < n ? j : hi_offset + (j - n);

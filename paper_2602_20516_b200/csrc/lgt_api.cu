@@ -267,7 +267,7 @@ template <class T> struct Ops {
                 LAUNCH(c, LGT_K_CG_BLAS, (cg_scalars_kernel<1>), 1, 1024, ngrid, c->partials, c->st);
                 if ((rc = dslash(c, U, t, nullptr, 1, 2, r)) != LGT_OK) return rc;
                 LAUNCH(c, LGT_K_CG_BLAS, (cg_scalars_kernel<2>), 1, 1024, ngrid, c->partials, c->st);
-                LAUNCH(c, LGT_K_CG_BLAS, (cg_update_xp_kernel<T>), nb, 256, n, (T2*)x, p, (const T2*)r, c->st, launched + i + 1);
+                LAUNCH(c, LGT_K_CG_BLAS, (cg_update_xp_kernel<T>), nb, 256, n, (T2*)x, p, (const T2*)r, c->st);
             }
             launched += chunk;
         }
@@ -504,7 +504,7 @@ template <class T> struct Ops {
                 if ((rc = hop(c, 1, u, nullptr, t, 1, 3, -c->kappa)) != LGT_OK) return rc;   // t_o = kappa H^dag_oe u
                 if ((rc = hop(c, 0, t, u, nullptr, 1, 2, c->kappa, r)) != LGT_OK) return rc; // r -= alpha M^dag u
                 LAUNCH(c, LGT_K_CG_BLAS, (cg_scalars_kernel<2>), 1, 1024, ngrid, c->partials, c->st);
-                LAUNCH(c, LGT_K_CG_BLAS, (cg_update_xp_kernel<T>), nb, 256, n, x, p, (const T2*)r, c->st, launched + i + 1);
+                LAUNCH(c, LGT_K_CG_BLAS, (cg_update_xp_kernel<T>), nb, 256, n, x, p, (const T2*)r, c->st);
             }
             launched += chunk;
         }
