@@ -79,6 +79,17 @@ struct lgt_ctx {
     std::vector<cudaEvent_t> ev_pool;
     size_t ev_used = 0;
     std::vector<int> ev_class;  // class of the launch bracketed by events (2i, 2i+1)
+    // CUDA graphs of one chunk (8 iterations) of the CG loops, keyed by the buffers the chunk touches (lazy)
+    struct ChunkGraph {
+        int kind;
+        const void* key[7];
+        int swz;
+        cudaGraphExec_t exec;
+        int launches;
+    };
+    std::vector<ChunkGraph> graphs;
+    cudaStream_t capture_stream = nullptr;
+    bool graphs_ok = true;
     std::string err;
 };
 
@@ -172,6 +183,63 @@ int ensure_force_buf(lgt_ctx* c) {
 
 int eo_cg_mixed(lgt_ctx* c, void* b, void* x, void* r, void* q, void* u, void* t_o, double tol, int max_iter, int* iters);
 
+// One chunk of CG iterations as a CUDA graph: the kernels of a chunk have no argument that changes from chunk to chunk
+// (the scalars, the stop flag and the "update due" flag live on the device), so the first chunk on a given set of buffers
+// is captured -- on a side stream, since the handle's stream may be the legacy default stream, which cannot capture --
+// and every later one is a single cudaGraphLaunch on the handle's stream.  This takes the per-launch host cost out of
+// the loop, which is what bounds small lattices (16^4: 7 launches of 3-10 us of work each per iteration).  Falls back to
+// plain launches while per-kernel timing is on, or if capture is not possible.
+template <class Body> int chunk_graph(lgt_ctx* c, int kind, const void* const (&key)[7], Body body) {
+    if (c->timing || !c->graphs_ok) return body();
+    for (const lgt_ctx::ChunkGraph& g : c->graphs)
+        if (g.kind == kind && g.swz == c->g.swz_Z && memcmp(g.key, key, sizeof key) == 0) {
+            CU(cudaGraphLaunch(g.exec, c->stream));
+            c->launches += g.launches;
+            return LGT_OK;
+        }
+    if (!c->capture_stream && cudaStreamCreateWithFlags(&c->capture_stream, cudaStreamNonBlocking) != cudaSuccess) {
+        c->graphs_ok = false;
+        cudaGetLastError();
+        return body();
+    }
+    cudaStream_t user = c->stream;
+    const long l0 = c->launches;
+    if (cudaStreamBeginCapture(c->capture_stream, cudaStreamCaptureModeThreadLocal) != cudaSuccess) {
+        c->graphs_ok = false;
+        cudaGetLastError();
+        return body();
+    }
+    c->stream = c->capture_stream;
+    const int rc = body();
+    c->stream = user;
+    cudaGraph_t graph = nullptr;
+    cudaError_t e = cudaStreamEndCapture(c->capture_stream, &graph);
+    const int nl = (int)(c->launches - l0);
+    c->launches = l0;
+    cudaGraphExec_t exec = nullptr;
+    if (rc == LGT_OK && e == cudaSuccess && graph) e = cudaGraphInstantiate(&exec, graph, 0);
+    if (graph) cudaGraphDestroy(graph);
+    if (rc != LGT_OK || e != cudaSuccess || !exec) {
+        c->graphs_ok = false;
+        cudaGetLastError();
+        return body();
+    }
+    lgt_ctx::ChunkGraph g;
+    g.kind = kind;
+    memcpy(g.key, key, sizeof key);
+    g.swz = c->g.swz_Z;
+    g.exec = exec;
+    g.launches = nl;
+    if (c->graphs.size() >= 16) {  // buffers keep changing (caller-owned x): do not hoard
+        cudaGraphExecDestroy(c->graphs.front().exec);
+        c->graphs.erase(c->graphs.begin());
+    }
+    c->graphs.push_back(g);
+    CU(cudaGraphLaunch(exec, c->stream));
+    c->launches += nl;
+    return LGT_OK;
+}
+
 template <class T> struct Ops {
     typedef typename Vec2<T>::type T2;
 
@@ -262,13 +330,19 @@ template <class T> struct Ops {
             int chunk = max_iter - launched;
             if (chunk > 8) chunk = 8;
             if (chunk <= 0) chunk = 1;
-            for (int i = 0; i < chunk; i++) {
-                if ((rc = dslash(c, U, p, t, 0, 1)) != LGT_OK) return rc;
-                LAUNCH(c, LGT_K_CG_BLAS, (cg_scalars_kernel<1>), 1, 1024, ngrid, c->partials, c->st);
-                if ((rc = dslash(c, U, t, nullptr, 1, 2, r)) != LGT_OK) return rc;
-                LAUNCH(c, LGT_K_CG_BLAS, (cg_scalars_kernel<2>), 1, 1024, ngrid, c->partials, c->st);
-                LAUNCH(c, LGT_K_CG_BLAS, (cg_update_xp_kernel<T>), nb, 256, n, (T2*)x, p, (const T2*)r, c->st);
-            }
+            auto body = [&]() -> int {
+                int r2;
+                for (int i = 0; i < chunk; i++) {
+                    if ((r2 = dslash(c, U, p, t, 0, 1)) != LGT_OK) return r2;
+                    LAUNCH(c, LGT_K_CG_BLAS, (cg_scalars_kernel<1>), 1, 1024, ngrid, c->partials, c->st);
+                    if ((r2 = dslash(c, U, t, nullptr, 1, 2, r)) != LGT_OK) return r2;
+                    LAUNCH(c, LGT_K_CG_BLAS, (cg_scalars_kernel<2>), 1, 1024, ngrid, c->partials, c->st);
+                    LAUNCH(c, LGT_K_CG_BLAS, (cg_update_xp_kernel<T>), nb, 256, n, (T2*)x, p, (const T2*)r, c->st);
+                }
+                return LGT_OK;
+            };
+            const void* const key[7] = {U, x, r, p, t, nullptr, (const void*)sizeof(T)};
+            if ((rc = (chunk == 8 ? chunk_graph(c, 0, key, body) : body())) != LGT_OK) return rc;
             launched += chunk;
         }
         const CgState& h = *c->h_st;
@@ -497,15 +571,21 @@ template <class T> struct Ops {
             int chunk = max_iter - launched;
             if (chunk > 8) chunk = 8;
             if (chunk <= 0) chunk = 1;
-            for (int i = 0; i < chunk; i++) {
-                if ((rc = hop(c, 1, p, nullptr, t, 0, 3, -c->kappa)) != LGT_OK) return rc;   // t_o = kappa H_oe p
-                if ((rc = hop(c, 0, t, p, u, 0, 1, c->kappa)) != LGT_OK) return rc;          // u = M p, |u|^2
-                LAUNCH(c, LGT_K_CG_BLAS, (cg_scalars_kernel<1>), 1, 1024, ngrid, c->partials, c->st);
-                if ((rc = hop(c, 1, u, nullptr, t, 1, 3, -c->kappa)) != LGT_OK) return rc;   // t_o = kappa H^dag_oe u
-                if ((rc = hop(c, 0, t, u, nullptr, 1, 2, c->kappa, r)) != LGT_OK) return rc; // r -= alpha M^dag u
-                LAUNCH(c, LGT_K_CG_BLAS, (cg_scalars_kernel<2>), 1, 1024, ngrid, c->partials, c->st);
-                LAUNCH(c, LGT_K_CG_BLAS, (cg_update_xp_kernel<T>), nb, 256, n, x, p, (const T2*)r, c->st);
-            }
+            auto body = [&]() -> int {
+                int r2;
+                for (int i = 0; i < chunk; i++) {
+                    if ((r2 = hop(c, 1, p, nullptr, t, 0, 3, -c->kappa)) != LGT_OK) return r2;   // t_o = kappa H_oe p
+                    if ((r2 = hop(c, 0, t, p, u, 0, 1, c->kappa)) != LGT_OK) return r2;          // u = M p, |u|^2
+                    LAUNCH(c, LGT_K_CG_BLAS, (cg_scalars_kernel<1>), 1, 1024, ngrid, c->partials, c->st);
+                    if ((r2 = hop(c, 1, u, nullptr, t, 1, 3, -c->kappa)) != LGT_OK) return r2;   // t_o = kappa H^dag_oe u
+                    if ((r2 = hop(c, 0, t, u, nullptr, 1, 2, c->kappa, r)) != LGT_OK) return r2; // r -= alpha M^dag u
+                    LAUNCH(c, LGT_K_CG_BLAS, (cg_scalars_kernel<2>), 1, 1024, ngrid, c->partials, c->st);
+                    LAUNCH(c, LGT_K_CG_BLAS, (cg_update_xp_kernel<T>), nb, 256, n, x, p, (const T2*)r, c->st);
+                }
+                return LGT_OK;
+            };
+            const void* const key[7] = {links_cb(c, 0), x, r, p, u, t, (const void*)sizeof(T)};
+            if ((rc = (chunk == 8 ? chunk_graph(c, 1, key, body) : body())) != LGT_OK) return rc;
             launched += chunk;
         }
         const CgState& h = *c->h_st;
@@ -992,6 +1072,8 @@ int lgt_destroy(lgt_ctx* c) {
     if (c->h_st) cudaFreeHost(c->h_st);
     if (c->h_scal) cudaFreeHost(c->h_scal);
     for (cudaEvent_t e : c->ev_pool) cudaEventDestroy(e);
+    for (const lgt_ctx::ChunkGraph& g : c->graphs) cudaGraphExecDestroy(g.exec);
+    if (c->capture_stream) cudaStreamDestroy(c->capture_stream);
     delete c;
     return LGT_OK;
 }
