@@ -677,3 +677,34 @@ def test_config4_largest_lattice_sampled(lgt):
             worst = max(worst, np.linalg.norm(F[s, mu] - rf) / np.linalg.norm(rf))
     assert worst < TOL64, worst
     lat.close()
+
+
+def test_cg_graph_replay_is_bitwise_the_plain_launches(lgt):
+    """The CG chunks run as CUDA graphs; with per-kernel timing on they fall back to plain launches.  Same kernels, same
+    order: solution, iteration count and the even/odd force must be bit-identical, and repeated solves reuse the graph."""
+    dims, kappa = (8, 8, 8, 8), 0.12
+    V = synth.volume(dims)
+    U = synth.warm_links(dims, 0.3, 71)
+    b = oracle.dslash(dims, kappa, BC, U, synth.gaussian_spinor(dims, 72), dagger=True)
+    lat = lgt.Lattice(dims, 5.6, kappa, BC)
+    lat.set_links(U)
+    lat.set_pseudofermion(b)
+    out = {}
+    for timing in (False, True, False):
+        lgt.lgt_timing_enable(lat.ctx, timing)
+        n0 = lgt.lgt_launch_count(lat.ctx)
+        x, it, rel, ok = lat.cg(b, 1e-12, 10 * V)
+        launches = lgt.lgt_launch_count(lat.ctx) - n0
+        lgt.lgt_set_fermion_action(lat.ctx, lgt.LGT_ACTION_EO)
+        F, it_eo = lat.fermion_force(None, None, tol=1e-12, max_iter=10 * V)
+        lgt.lgt_set_fermion_action(lat.ctx, lgt.LGT_ACTION_FULL)
+        out.setdefault("runs", []).append((x, it, F, it_eo, launches))
+    lgt.lgt_timing_enable(lat.ctx, False)
+    lgt.lgt_timing_reset(lat.ctx)
+    ref = out["runs"][1]  # plain launches
+    for run in (out["runs"][0], out["runs"][2]):
+        assert run[1] == ref[1] and run[3] == ref[3] and run[4] == ref[4]  # counts incl. the kernels inside the graphs
+        assert np.array_equal(run[0], ref[0]) and np.array_equal(run[2], ref[2])
+    x_ref, it_ref, _, _ = oracle.cg(dims, kappa, BC, U, b, 1e-12, 10 * V)
+    assert ref[1] == it_ref
+    lat.close()
