@@ -188,6 +188,33 @@ def test_pure_gauge_hmc_reproduces_the_known_plaquette(lgt):
     lat.close()
 
 
+def test_dynamical_hmc_creutz_identity_with_every_option(lgt):
+    """Exactness of the whole chain with fermions: even/odd action + mixed-precision solver + one stout level +
+    Sexton-Weingarten.  If any force (the smeared pull-back included) disagreed with the action that Metropolis
+    evaluates, or the solver tolerance leaked into dH, <exp(-dH)> would drift from 1 (Creutz) and acceptance would
+    collapse; reversibility errors show the same way."""
+    dims, beta, kappa = (8, 8, 8, 8), 5.6, 0.12
+    lat = lgt.Lattice(dims, beta, kappa, BC)
+    lat.set_links(synth.warm_links(dims, 0.3, 9))
+    lgt.lgt_set_fermion_action(lat.ctx, lgt.LGT_ACTION_EO)
+    lgt.lgt_set_solver(lat.ctx, lgt.LGT_SOLVER_MIXED_CG, 1e-5)
+    lgt.lgt_set_smearing(lat.ctx, 1, 0.3)
+    lgt.lgt_set_integrator(lat.ctx, lgt.LGT_INT_SEXTON_WEINGARTEN, 10)
+    dHs, accs = [], []
+    for traj in range(160):
+        dH, acc, its, _, ok = lgt.lgt_hmc_trajectory(lat.ctx, 10, 0.1, 90210, traj, tol=1e-10, max_iter=5000)
+        assert ok and np.isfinite(dH)
+        dHs.append(dH)
+        accs.append(acc)
+    e = np.exp(-np.array(dHs[60:]))
+    sigma = e.std() / np.sqrt(len(e))
+    assert np.mean(accs[60:]) > 0.6, np.mean(accs[60:])
+    assert abs(e.mean() - 1.0) < max(4 * sigma, 0.05), (e.mean(), sigma)
+    U = lat.get_links()
+    assert np.abs(U @ U.conj().swapaxes(-1, -2) - np.eye(3)).max() < 1e-12
+    lat.close()
+
+
 def test_heatbaths_full_size_sampled(lgt):
     """configs[3]'s 32^4 lattice: the heat-bath kernels in their production launch shape, sampled links and sites against
     the oracle's generator evaluated at exactly those elements; K / dof and |eta|^2 / dof as global checks."""
