@@ -69,6 +69,15 @@ def link_rel_err(F, F_ref):
     return float(floored.max()), float(plain.max())
 
 
+def link_rel_quantiles(F, F_ref, qs=(0.5, 0.9, 0.99, 0.999, 1.0)):
+    """The distribution behind the paper's Fig. 2: plain Eq. 8 over all links, no floor, at the
+    cumulative fractions qs."""
+    d = np.sqrt(np.sum(np.abs(F - F_ref) ** 2, axis=(-1, -2))).ravel()
+    n = np.sqrt(np.sum(np.abs(F_ref) ** 2, axis=(-1, -2))).ravel()
+    assert (n > 0).all()
+    return [float(v) for v in np.quantile(d / n, qs)]
+
+
 def numpy_dslash(U, psi, dims, kappa, bc, gam, dag=False):
     """Second, vectorised statement of the Wilson-Dirac operator of BASELINE.json configs[0]
     (np.roll shifts, einsum products); used to cross-check the oracle's indexing."""

@@ -8,7 +8,7 @@ import pytest
 import oracle
 from oracle import evenodd as oeo
 from paper_2602_20516_b200 import synth
-from lattice_util import link_rel_err
+from lattice_util import link_rel_err, link_rel_quantiles
 
 pytestmark = pytest.mark.gpu
 
@@ -144,6 +144,17 @@ def test_cg_and_fermion_force_configs(lgt, cfg):
     assert it2 == it_ref
     e, plain = link_rel_err(F, F_ref)
     assert e < TOL64, (e, plain)
+    if cfg == 2:
+        # the paper's own accuracy figure (Fig. 2: Eq. 8 over every link of a 16^4 lattice, "uniform
+        # agreement at the level of 1e-9 ... no visible outliers"), here GPU against oracle: the whole distribution
+        # sits at double-precision rounding (measured: median 9e-16, 99.9 % 3e-15, max 6e-15) with a short tail
+        q50, q90, q99, q999, qmax = link_rel_quantiles(F, F_ref)
+        print("Eq. 8 distribution, 16^4, GPU CG + force vs oracle: median %.2e 90%% %.2e 99%% %.2e 99.9%% %.2e max %.2e"
+              % (q50, q90, q99, q999, qmax))
+        assert qmax < 1e-13 and q50 < 1e-14 and qmax < 30 * q50
+        k50, _, _, _, kmax = link_rel_quantiles(F_shared, F_ref)
+        print("  force kernel alone (shared X, Y): median %.2e max %.2e" % (k50, kmax))
+        assert kmax < 1e-14
     # closed forms (pin P6): S_F = |eta|^2
     S_g, S_F, K, _ = lgt.lgt_action(lat.ctx, tol, 10 * V)
     n2 = np.sum(np.abs(eta) ** 2)
