@@ -215,6 +215,46 @@ def test_dynamical_hmc_creutz_identity_with_every_option(lgt):
     lat.close()
 
 
+@pytest.mark.parametrize("setup", ["8^4 leapfrog", "6^4 stout rho=0.3 Sexton-Weingarten 10"])
+def test_fig3_step_size_scaling(lgt, setup):
+    """The paper's dynamical validation (Fig. 3): Wilson-fermion HMC at 8^4 without smearing and at 6^4
+    with one stout level (rho = 0.3) under Sexton-Weingarten with 10 inner steps; dH must fall like dt^2 at fixed
+    trajectory length.  After a short thermalisation every measured configuration is evolved from the same links with
+    the same (seed, trajectory) heat bath at dt, dt/2, dt/4, so the ratio is taken configuration by configuration."""
+    if setup.startswith("8"):
+        dims, smear, integ, m, n0 = (8, 8, 8, 8), 0, lgt.LGT_INT_LEAPFROG, 1, 32
+    else:  # the gauge force sits on the inner level, so the outer step can be four times coarser
+        dims, smear, integ, m, n0 = (6, 6, 6, 6), 1, lgt.LGT_INT_SEXTON_WEINGARTEN, 10, 8
+    lat = lgt.Lattice(dims, 5.6, 0.12, BC)
+    lat.set_links(synth.warm_links(dims, 0.3, 33))
+    if smear:
+        lgt.lgt_set_smearing(lat.ctx, smear, 0.3)
+    lgt.lgt_set_integrator(lat.ctx, integ, m)
+    seed = 20516
+    for traj in range(30):
+        _, _, _, _, ok = lgt.lgt_hmc_trajectory(lat.ctx, 10, 0.05, seed, traj, tol=1e-10, max_iter=5000)
+        assert ok
+    steps = tuple((n0 * k, 1.0 / (n0 * k)) for k in (1, 2, 4))
+    dH = {n: [] for n, _ in steps}
+    accs = []
+    for traj in range(30, 42):
+        U = lat.get_links()
+        for n, dt in steps:
+            lat.set_links(U)
+            d, acc, _, _, ok = lgt.lgt_hmc_trajectory(lat.ctx, n, dt, seed, traj, tol=1e-12, max_iter=5000)
+            assert ok
+            dH[n].append(d)
+        accs.append(acc)  # the chain goes on from the finest step's outcome
+    a = {n: np.mean(np.abs(dH[n])) for n in dH}
+    a0, a1, a2 = (a[n0 * k] for k in (1, 2, 4))
+    print("%s: <|dH|> at dt = 1/%d, 1/%d, 1/%d: %.3e %.3e %.3e, ratios %.2f %.2f, acceptance at the finest %.2f"
+          % (setup, n0, 2 * n0, 4 * n0, a0, a1, a2, a0 / a1, a1 / a2, np.mean(accs)))
+    assert a0 < 1.0
+    assert 3.0 < a0 / a1 < 5.5 and 3.3 < a1 / a2 < 4.7, a
+    assert np.mean(accs) >= 0.75
+    lat.close()
+
+
 def test_heatbaths_full_size_sampled(lgt):
     """configs[3]'s 32^4 lattice: the heat-bath kernels in their production launch shape, sampled links and sites against
     the oracle's generator evaluated at exactly those elements; K / dof and |eta|^2 / dof as global checks."""
