@@ -526,7 +526,33 @@ def oracle_step(oracle, cfg, U, P, phi, sample_iters):
     return time.perf_counter() - t0, it
 
 
-def cpu_baseline(cfg, sample_iters, steps=1, warmup=0):
+def oracle_kernels(oracle, cfg, U, eta, phi):
+    """The metric's two named kernels on the oracle alone: one Dslash and one fermion force on given
+    spinor fields, with all host threads and with one (the paper's CPU column is single-threaded)."""
+    dims, kappa, bc = cfg["dims"], cfg["kappa"], cfg["bc"]
+    V = 1
+    for d in dims:
+        V *= d
+    n_all, out = oracle.num_threads(), {}
+    try:
+        for threads in sorted({n_all, 1}, reverse=True):
+            oracle.set_num_threads(threads)
+            for name, fn in (("dslash", lambda: oracle.dslash(dims, kappa, bc, U, eta)),
+                             ("fermion_force", lambda: oracle.fermion_force(dims, kappa, bc, U, eta, phi))):
+                best = float("inf")
+                for _ in range(2):
+                    t0 = time.perf_counter()
+                    fn()
+                    best = min(best, time.perf_counter() - t0)
+                out["%s_%d_threads" % (name, threads)] = {"ms": round(best * 1e3, 1),
+                                                           "GB/s": round(REALS[name] * 8 * V / best / 1e9, 3),
+                                                           "GFLOP/s": round(FLOPS[name] * V / best / 1e9, 2)}
+    finally:
+        oracle.set_num_threads(n_all)
+    return out
+
+
+def cpu_baseline(cfg, sample_iters, steps=1, warmup=0, per_kernel=True):
     import oracle
     from paper_2602_20516_b200 import synth
 
@@ -541,7 +567,7 @@ def cpu_baseline(cfg, sample_iters, steps=1, warmup=0):
         t += dt_s
         reals += step_reals(it) * V
     return {"value": round(reals * 8 / t / 1e9, 3), "unit": "GB/s", "cores": oracle.num_threads(), "kind": "oracle",
-            "seconds_per_sample": round(t / steps, 2),
+            "seconds_per_sample": round(t / steps, 2), "kernels": oracle_kernels(oracle, cfg, U, eta, phi) if per_kernel else None,
             "sample": "same %s lattice and fields; one MD step with CG capped at %d iterations "
                       "(gauge force + %d x (2 Dslash + BLAS-1) + Y = D X + fermion force + drift), same byte accounting"
                       % ("x".join(map(str, cfg["dims"])), sample_iters, sample_iters)}
@@ -666,7 +692,7 @@ def run_reference(args):
     if args.lattice:
         cfg["dims"] = tuple(args.lattice)
     t0 = time.perf_counter()
-    base = cpu_baseline(cfg, args.cpu_sample_iters, steps=args.steps, warmup=args.warmup)
+    base = cpu_baseline(cfg, args.cpu_sample_iters, steps=args.steps, warmup=args.warmup, per_kernel=False)
     out = {
         "impl": "reference", "metric": METRIC, "value": base["value"], "unit": "GB/s", "n_gpus": world,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": round(base["seconds_per_sample"] * 1e3, 1),
