@@ -36,8 +36,10 @@ REALS = dict(
     fermion_force=2 * (36 + 12 + 12) + 2 * 32,  # U + X + Y + Pi (8 reals x 4 links) rw -> 1472 B
     gauge_force=2 * 36 + 2 * 32,             # U + Pi rw                         -> 1088 B
     link_update=32 + 2 * 2 * 36,             # Pi r + U rw                       -> 1408 B
+    plaquette=2 * 36,                        # U r (six planes per site)         -> 576 B
 )
-FLOPS = dict(dslash=1368, dslash_fused_r=1368 + 96, cg_update_xp=96, cg_iter=2 * 1368 + 192, fermion_force=2300, gauge_force=10900, link_update=3500)
+FLOPS = dict(dslash=1368, dslash_fused_r=1368 + 96, cg_update_xp=96, cg_iter=2 * 1368 + 192, fermion_force=2300, gauge_force=10900, link_update=3500,
+             plaquette=2600)
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel from the ncu --set full capture
 # summarised in profiles/ (None until captured for the current kernel).
@@ -439,7 +441,9 @@ def run_ours(args):
                 ("dslash_dagger", lambda: lgt.lgt_dslash_native(hctx, bufs[0], bufs[1], True), "dslash"),
                 ("fermion_force", lambda: lgt.lgt_fermion_force_native(hctx, bufs[0], bufs[2], 1e-3), "fermion_force"),
                 ("gauge_force", lambda: lgt.lgt_gauge_force_accumulate(hctx, 1e-3), "gauge_force"),
-                ("link_update", lambda: lgt.lgt_md_drift(hctx, 1e-6), "link_update")):
+                ("link_update", lambda: lgt.lgt_md_drift(hctx, 1e-6), "link_update"),
+                # S_g: plaquette kernel + fixed-order sum; the call reads its 8-byte result back, so this is call time
+                ("plaquette_action_call", lambda: lgt.lgt_plaquette(hctx), "plaquette")):
             t = time_kernel(fn)
             kernels[name + tag] = {"us": round(t * 1e6, 2), "GB/s": round(REALS[key] * real_bytes * V / t / 1e9, 1),
                                    "GFLOP/s": round(FLOPS[key] * V / t / 1e9, 1)}
