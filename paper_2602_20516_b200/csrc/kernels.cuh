@@ -943,10 +943,7 @@ __global__ void __launch_bounds__(128) stout_chain_kernel(Geom g, const typename
             mul_nn(t1, gi, a);             // Ub Uc^dag Gc
             mul_nd(a, b, t2);              // Ub Uc^dag Gc Ud^dag
 #pragma unroll
-            for (int k = 0; k < 9; k++) t3[k] = t3[k] - t2[k];
-            mul_nn(Ua, t3, a);             // Ua [Gb S + S (Ga - Gd) - Ub Uc^dag Gc Ud^dag]
-#pragma unroll
-            for (int k = 0; k < 9; k++) X[k] = X[k] + a[k];
+            for (int k = 0; k < 9; k++) X[k] = X[k] + (t3[k] - t2[k]);  // Gb S + S (Ga - Gd) - Ub Uc^dag Gc Ud^dag
         }
         {   // down: b' = (s+mu-nu,nu), c' = (s-nu,mu), d' = (s-nu,nu):  P' = Ua Ub'^dag Uc'^dag Ud'
             const int sdn = nbr_bwd(g, c, s, nu);
@@ -955,30 +952,31 @@ __global__ void __launch_bounds__(128) stout_chain_kernel(Geom g, const typename
             const int smudn = nbr_bwd(g, cm, smu, nu);
             load_link<T>(U, nu, smudn, a);  // Ub'
             load_link<T>(U, mu, sdn, b);    // Uc'
-            mul_nn(b, a, t1);               // Uc' Ub'  ->  (Ub'^dag Uc'^dag) = t1^dag
-            load_link<T>(U, nu, sdn, b);    // Ud'
+            load_link<T>(U, nu, sdn, t1);   // Ud'
+            mul_dn(b, t1, t2);              // W = Uc'^dag Ud'   (so that P' = Ua Ub'^dag W)
             load_su3_compact<T>(G, sdn, mu, gi);   // Gc'
-            load_su3_compact<T>(G, sdn, nu, t2);   // Gd'
+            load_su3_compact<T>(G, sdn, nu, t3);   // Gd'
 #pragma unroll
-            for (int k = 0; k < 9; k++) gi[k] = t2[k] - gi[k];  // Gd' - Gc'
-            mul_nn(gi, b, t2);              // (Gd' - Gc') Ud'
-            mul_dn(t1, t2, t3);             // Ub'^dag Uc'^dag (Gd' - Gc') Ud'
-            mul_dn(t1, b, t2);              // Ub'^dag Uc'^dag Ud'   (so that P' = Ua t2)
-            mul_nn(t2, Ga, gi);             // ... Ga
+            for (int k = 0; k < 9; k++) gi[k] = t3[k] - gi[k];  // Gd' - Gc'
+            mul_nn(gi, t1, t3);             // (Gd' - Gc') Ud'
+            mul_dn(b, t3, t1);              // Uc'^dag (Gd' - Gc') Ud'
+            mul_nn(t2, Ga, t3);             // W Ga
 #pragma unroll
-            for (int k = 0; k < 9; k++) t3[k] = t3[k] + gi[k];
-            // - Ub'^dag Gb' Uc'^dag Ud'
+            for (int k = 0; k < 9; k++) t1[k] = t1[k] + t3[k];
             load_su3_compact<T>(G, smudn, nu, gi);  // Gb'
-            load_link<T>(U, mu, sdn, t1);   // Uc' again (t1 is free now)
-            mul_dn(t1, b, t2);              // Uc'^dag Ud'
-            mul_nn(gi, t2, t1);             // Gb' Uc'^dag Ud'
-            mul_dn(a, t1, t2);              // Ub'^dag Gb' Uc'^dag Ud'
+            mul_nn(gi, t2, t3);             // Gb' W
 #pragma unroll
-            for (int k = 0; k < 9; k++) t3[k] = t3[k] - t2[k];
-            mul_nn(Ua, t3, a);
+            for (int k = 0; k < 9; k++) t1[k] = t1[k] - t3[k];
+            mul_dn(a, t1, t3);              // Ub'^dag [Uc'^dag (Gd' - Gc') Ud' + W Ga - Gb' W]
 #pragma unroll
-            for (int k = 0; k < 9; k++) X[k] = X[k] + a[k];
+            for (int k = 0; k < 9; k++) X[k] = X[k] + t3[k];
         }
+    }
+    {   // the link itself multiplies every term from the left: once, at the end
+        cx<T> t[9];
+        mul_nn(Ua, X, t);
+#pragma unroll
+        for (int k = 0; k < 9; k++) X[k] = t[k];
     }
     T fw[8], fd[8];
     ta_compact(X, -rho, fw);
