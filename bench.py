@@ -500,7 +500,8 @@ def run_ours(args):
         "e2e": {"value": round(e2e_reals * 8 / e2e_s / 1e9, 1), "unit": "GB/s", "steps": k_e2e,
                 "ms_per_step": round(e2e_s / k_e2e * 1e3, 2), "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
         "gpu_launches": int(launches_all),
-        "roofline": {"kernel": ("hop_cb_kernel<double> (inside CG, %d launches)" if args.action == "eo" else
+        "roofline": {"kernel": ("hop_cb_kernel<float> (mostly inside the fp32 CG, %d launches)" if args.action == "eo" and args.solver == "mixed" else
+                                "hop_cb_kernel<double> (inside CG, %d launches)" if args.action == "eo" else
                                 "dslash_kernel<float> (inside the fp32 CG, %d launches)" if args.solver == "mixed" else
                                 "dslash_kernel<double> (inside CG, %d launches)") % ds_n, "bound": "hbm",
                      "achieved": round(achieved, 1) if achieved else None, "peak": peak, "unit": "GB/s",
