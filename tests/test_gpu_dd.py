@@ -323,6 +323,12 @@ def test_dd_even_odd_action(lgt, nranks):
             lgt.lgt_dd_set_fermion_action(bad, lgt.LGT_ACTION_EO)
         finally:
             lgt.lgt_dd_destroy(bad)
+    with pytest.raises(lgt.LgtError):
+        bad = lgt.lgt_dd_create((4, 4, 4, 6), 2, [0, 1], beta, kappa, BC)  # three slices per slab: a slab would start at an odd time
+        try:
+            lgt.lgt_dd_set_fermion_action(bad, lgt.LGT_ACTION_EO)
+        finally:
+            lgt.lgt_dd_destroy(bad)
 
 
 @pytest.mark.parametrize("nranks,levels", [(2, 1), (4, 2), (1, 2)])
