@@ -999,8 +999,10 @@ __global__ void __launch_bounds__(128) plaquette_kernel(Geom g, const typename V
     double acc = 0.0;
     if (s < g.s_end) {
         const Site c = site_coords(g, s);
+#pragma unroll
         for (int mu = 0; mu < 4; mu++) {
             const int smu = nbr_fwd(g, c, s, mu);
+#pragma unroll
             for (int nu = mu + 1; nu < 4; nu++) {
                 const int snu = nbr_fwd(g, c, s, nu);
                 cx<T> a[9], b[9], t1[9], t2[9];
