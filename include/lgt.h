@@ -33,6 +33,7 @@
  */
 #ifndef LGT_H
 #define LGT_H
+#include <stddef.h>
 #ifdef __cplusplus
 extern "C" {
 #endif
@@ -217,6 +218,25 @@ const char* lgt_dd_last_error(const lgt_dd* d);
  * torch.distributed), every process calls lgt_dd_nccl_init on its one-rank group.  libnccl.so.2 is opened at run time. */
 int lgt_dd_nccl_unique_id(void* id128);
 int lgt_dd_nccl_init(lgt_dd* d, const void* id128);
+/* Host transport (MPI, gloo, ... -- and the two-processes-on-one-GPU test of the inter-process path): instead of NCCL
+ * the caller supplies two callbacks that move HOST memory between the processes; the library stages the time slices
+ * through pinned buffers and synchronises the group's stream around each call (correct, not fast).
+ *   sendrecv(user, send_buf, send_peer, recv_buf, recv_peer, nbytes): post the two sends (send_buf[k], nbytes bytes, to
+ *     rank send_peer[k]) and the two receives (recv_buf[k] from rank recv_peer[k]) IN INDEX ORDER and return when all four
+ *     have completed; messages between one pair of ranks must be matched in the order they were posted.  A rank may
+ *     be its own peer (nranks = 1), and both peers may be the same rank (nranks = 2).
+ *   allreduce(user, buf, count): replace buf[0..count) (count <= 8) by its sum over all ranks, the same bits on every rank.
+ * Both return 0 on success.  One rank per process; exclusive with lgt_dd_nccl_init (LGT_ESTATE). */
+typedef int (*lgt_dd_sendrecv_fn)(void* user, const void* const send_buf[2], const int send_peer[2], void* const recv_buf[2],
+                                  const int recv_peer[2], size_t nbytes);
+typedef int (*lgt_dd_allreduce_fn)(void* user, double* buf, int count);
+int lgt_dd_set_host_transport(lgt_dd* d, lgt_dd_sendrecv_fn sendrecv, lgt_dd_allreduce_fn allreduce, void* user);
+/* The halo plan every transport follows (host-only, no device needed): for rank `rank` of `nranks` slabs of lt_local time
+ * slices, plan = {send_peer[2], send_slice[2], recv_peer[2], recv_slice[2]} in issue order; slices are local time-slice
+ * numbers of the slab's (lt_local + 2)-slice field (0 and lt_local + 1 are the ghost slices).  Rank r's first interior
+ * slice goes to the upper ghost slice of rank r - 1, its last interior slice to the lower ghost slice of rank r + 1.
+ * A group that holds one of several ranks and has no transport yet returns LGT_ESTATE from every exchanging call. */
+int lgt_dd_halo_plan(int nranks, int rank, int lt_local, int plan[8]);
 /* How the halo slices of the CG fields travel:
  *   LGT_DD_EXCHANGE (default): a separate exchange (NCCL send/recv, or device copies between local ranks) before
  *     every Dslash;

@@ -5,9 +5,12 @@
 // are ghost copies of the neighbour ranks' boundary slices, and Geom::s_begin / s_end restrict every compute kernel
 // to the interior.  Because t is the slowest index and Lx Ly Lz is a multiple of 32, a time slice of any native field
 // is one contiguous run, so a halo exchange is two sends and two receives per rank and field, with no packing kernel.
-// The same driver serves two transports: NCCL send/recv + all-reduce between processes (one rank per process), and
-// plain device copies between ranks that live in this process (the single-GPU verification mode: all ranks of the
-// group on one device and one stream, stepped in lockstep, nothing ever waits on another rank).
+// The same driver serves three transports: NCCL send/recv + all-reduce between processes (one rank per process); a
+// caller-supplied HOST transport (two callbacks: a paired send/receive of host buffers and an all-reduce of host
+// doubles -- MPI, gloo, ...; slices are staged through pinned memory), also one rank per process; and plain device
+// copies between ranks that live in this process (all ranks of the group on one device and one stream, stepped in
+// lockstep, nothing ever waits on another rank).  All three issue the sends and receives of lgt_dd_halo_plan in the
+// same order.
 #pragma once
 #include <dlfcn.h>
 
@@ -62,7 +65,14 @@ struct lgt_dd {
     int device = 0;
     cudaStream_t stream = nullptr;
     bool links_ghost_valid = false;
-    void* comm = nullptr;  // ncclComm_t; null: every rank is local
+    void* comm = nullptr;  // ncclComm_t; null: host transport, or every rank is local
+    // host transport (lgt_dd_set_host_transport): callbacks + pinned staging (2 outgoing, 2 incoming slices; sums)
+    lgt_dd_sendrecv_fn host_sendrecv = nullptr;
+    lgt_dd_allreduce_fn host_allreduce = nullptr;
+    void* host_user = nullptr;
+    char* h_stage = nullptr;
+    size_t h_stage_bytes = 0;
+    double* h_sum = nullptr;
     // LGT_DD_PUSH: halos of the CG fields t (ws[3]) and r (ws[1]) are stored into the neighbours' ghost slices by the
     // producing kernels.  Neighbours in other processes: their buffers mapped through CUDA IPC, [field r, t][lo, hi].
     int halo_mode = 0;
@@ -103,46 +113,119 @@ int dd_local_index(const lgt_dd* d, int rank) {
     return -1;
 }
 
+// The halo plan of one rank (include/lgt.h "lgt_dd_halo_plan"): rank r's first interior slice (local slice 1) goes to
+// the upper ghost slice (Lt_loc + 1) of rank r - 1, its last interior slice (Lt_loc) to the lower ghost slice (0) of
+// rank r + 1, periodic in ranks.  Every transport issues the two sends and the two receives in THIS order; sends and
+// receives between one pair of ranks are matched in issue order (NCCL, MPI and gloo all guarantee that), which is what
+// makes nranks = 2 (both neighbours are the one other rank) and nranks = 1 (a rank is its own neighbour) come out right.
+struct HaloPlan {
+    int send_peer[2], send_slice[2], recv_peer[2], recv_slice[2];
+};
+HaloPlan halo_plan(int nranks, int rank, int lt_loc) {
+    HaloPlan p;
+    const int dn = (rank + nranks - 1) % nranks, up = (rank + 1) % nranks;
+    p.send_peer[0] = dn;
+    p.send_slice[0] = 1;
+    p.send_peer[1] = up;
+    p.send_slice[1] = lt_loc;
+    p.recv_peer[0] = up;
+    p.recv_slice[0] = lt_loc + 1;
+    p.recv_peer[1] = dn;
+    p.recv_slice[1] = 0;
+    return p;
+}
+
+// A group that owns fewer ranks than the lattice has needs a transport before anything can be exchanged or summed.
+int dd_need_transport(lgt_dd* d) {
+    if (d->rk.size() != (size_t)d->nranks && !d->comm && !d->host_sendrecv)
+        return dd_fail(d, LGT_ESTATE, "this group holds one of several ranks and has no transport yet: call lgt_dd_nccl_init or "
+                                      "lgt_dd_set_host_transport first");
+    return LGT_OK;
+}
+
+int dd_host_stage(lgt_dd* d, size_t bytes) {
+    if (d->h_stage_bytes >= bytes) return LGT_OK;
+    DD_CU(cudaStreamSynchronize(d->stream));
+    if (d->h_stage) cudaFreeHost(d->h_stage);
+    d->h_stage = nullptr;
+    d->h_stage_bytes = 0;
+    DD_CU(cudaMallocHost((void**)&d->h_stage, bytes));
+    d->h_stage_bytes = bytes;
+    return LGT_OK;
+}
+
 // Halo exchange of one native field per local rank: base[i] points to the field of local rank i, `per_site` = complex
-// (or pair) elements per site (12 spinor, 36 links, 16 compact momenta).  Rank r's first interior slice goes to the
-// upper ghost slice of rank r - 1, its last interior slice to the lower ghost slice of rank r + 1 (periodic in ranks).
+// (or pair) elements per site (12 spinor, 36 links, 16 compact momenta).
 int dd_exchange(lgt_dd* d, void* const* base, int per_site, size_t esize = 0) {
     if (!esize) esize = d->prec == LGT_F64 ? 16 : 8;
     const size_t slice = (size_t)d->V3 * per_site * esize;
     const int n = (int)d->rk.size();
-    if (!d->comm) {
+    int rc;
+    if ((rc = dd_need_transport(d)) != LGT_OK) return rc;
+    if (!d->comm && !d->host_sendrecv) {
         for (int i = 0; i < n; i++) {
-            const int r = d->rank_of[i];
-            const int dn = dd_local_index(d, (r + d->nranks - 1) % d->nranks), up = dd_local_index(d, (r + 1) % d->nranks);
+            const HaloPlan p = halo_plan(d->nranks, d->rank_of[i], d->Lt_loc);
             char* mine = (char*)base[i];
-            DD_CU(cudaMemcpyAsync((char*)base[dn] + (size_t)(d->Lt_loc + 1) * slice, mine + slice, slice, cudaMemcpyDeviceToDevice, d->stream));
-            DD_CU(cudaMemcpyAsync((char*)base[up], mine + (size_t)d->Lt_loc * slice, slice, cudaMemcpyDeviceToDevice, d->stream));
+            for (int k = 0; k < 2; k++) {
+                // my k-th send lands where the peer's plan receives from me in the same position: send 0 (to r - 1) is
+                // that rank's receive 0 (from its r + 1), send 1 (to r + 1) its receive 1
+                const int peer = dd_local_index(d, p.send_peer[k]);
+                if (peer < 0) return dd_fail(d, LGT_ESTATE, "dd_exchange: a neighbour rank is not in this process");
+                const HaloPlan q = halo_plan(d->nranks, p.send_peer[k], d->Lt_loc);
+                DD_CU(cudaMemcpyAsync((char*)base[peer] + (size_t)q.recv_slice[k] * slice, mine + (size_t)p.send_slice[k] * slice, slice,
+                                      cudaMemcpyDeviceToDevice, d->stream));
+            }
         }
         return LGT_OK;
     }
-    // one rank per process; sends and receives to the same peer pair up in the order they are issued
-    const int r = d->rank_of[0];
-    const int dn = (r + d->nranks - 1) % d->nranks, up = (r + 1) % d->nranks;
+    // one rank per process
+    const HaloPlan p = halo_plan(d->nranks, d->rank_of[0], d->Lt_loc);
     char* mine = (char*)base[0];
-    DD_NCCL(g_nccl.GroupStart());
-    DD_NCCL(g_nccl.Send(mine + slice, slice, NCCL_CHAR, dn, d->comm, d->stream));
-    DD_NCCL(g_nccl.Send(mine + (size_t)d->Lt_loc * slice, slice, NCCL_CHAR, up, d->comm, d->stream));
-    DD_NCCL(g_nccl.Recv(mine + (size_t)(d->Lt_loc + 1) * slice, slice, NCCL_CHAR, up, d->comm, d->stream));
-    DD_NCCL(g_nccl.Recv(mine, slice, NCCL_CHAR, dn, d->comm, d->stream));
-    DD_NCCL(g_nccl.GroupEnd());
+    if (d->comm) {
+        DD_NCCL(g_nccl.GroupStart());
+        for (int k = 0; k < 2; k++) DD_NCCL(g_nccl.Send(mine + (size_t)p.send_slice[k] * slice, slice, NCCL_CHAR, p.send_peer[k], d->comm, d->stream));
+        for (int k = 0; k < 2; k++) DD_NCCL(g_nccl.Recv(mine + (size_t)p.recv_slice[k] * slice, slice, NCCL_CHAR, p.recv_peer[k], d->comm, d->stream));
+        DD_NCCL(g_nccl.GroupEnd());
+        return LGT_OK;
+    }
+    // host transport: outgoing slices to pinned memory, the caller's paired send/receive, incoming slices back
+    if ((rc = dd_host_stage(d, 4 * slice)) != LGT_OK) return rc;
+    char* h = d->h_stage;
+    for (int k = 0; k < 2; k++)
+        DD_CU(cudaMemcpyAsync(h + k * slice, mine + (size_t)p.send_slice[k] * slice, slice, cudaMemcpyDeviceToHost, d->stream));
+    DD_CU(cudaStreamSynchronize(d->stream));  // also orders the previous exchange's upload before the buffers are reused
+    const void* const sb[2] = {h, h + slice};
+    void* const rb[2] = {h + 2 * slice, h + 3 * slice};
+    if (d->host_sendrecv(d->host_user, sb, p.send_peer, rb, p.recv_peer, slice) != 0)
+        return dd_fail(d, LGT_ECUDA, "dd_exchange: the host transport's send/receive callback failed");
+    for (int k = 0; k < 2; k++)
+        DD_CU(cudaMemcpyAsync(mine + (size_t)p.recv_slice[k] * slice, h + (2 + k) * slice, slice, cudaMemcpyHostToDevice, d->stream));
     return LGT_OK;
 }
 
 // Sum of `count` doubles over all ranks, in place at ptr[i] of every local rank (device memory).
 int dd_allreduce(lgt_dd* d, double* const* ptr, int count) {
-    if (!d->comm) {
-        DdPtrs p;
-        for (size_t i = 0; i < 8; i++) p.p[i] = i < d->rk.size() ? ptr[i] : nullptr;
-        dd_local_allreduce_kernel<<<1, 32, 0, d->stream>>>(p, (int)d->rk.size(), count);
-        DD_CU(cudaGetLastError());
+    int rc;
+    if ((rc = dd_need_transport(d)) != LGT_OK) return rc;
+    if (d->comm) {
+        DD_NCCL(g_nccl.AllReduce(ptr[0], ptr[0], (size_t)count, NCCL_DOUBLE, NCCL_SUM, d->comm, d->stream));
         return LGT_OK;
     }
-    DD_NCCL(g_nccl.AllReduce(ptr[0], ptr[0], (size_t)count, NCCL_DOUBLE, NCCL_SUM, d->comm, d->stream));
+    if (d->host_allreduce) {
+        if (count > 8) return dd_fail(d, LGT_EINVAL, "dd_allreduce: at most 8 doubles");
+        if (!d->h_sum) DD_CU(cudaMallocHost((void**)&d->h_sum, 8 * sizeof(double)));
+        DD_CU(cudaMemcpyAsync(d->h_sum, ptr[0], count * sizeof(double), cudaMemcpyDeviceToHost, d->stream));
+        DD_CU(cudaStreamSynchronize(d->stream));
+        if (d->host_allreduce(d->host_user, d->h_sum, count) != 0)
+            return dd_fail(d, LGT_ECUDA, "dd_allreduce: the host transport's all-reduce callback failed");
+        DD_CU(cudaMemcpyAsync(ptr[0], d->h_sum, count * sizeof(double), cudaMemcpyHostToDevice, d->stream));
+        DD_CU(cudaStreamSynchronize(d->stream));  // h_sum is reused by the next sum
+        return LGT_OK;
+    }
+    DdPtrs p;
+    for (size_t i = 0; i < 8; i++) p.p[i] = i < d->rk.size() ? ptr[i] : nullptr;
+    dd_local_allreduce_kernel<<<1, 32, 0, d->stream>>>(p, (int)d->rk.size(), count);
+    DD_CU(cudaGetLastError());
     return LGT_OK;
 }
 
@@ -969,8 +1052,34 @@ int lgt_dd_destroy(lgt_dd* d) {
     for (int f = 0; f < 2; f++)
         for (int sd = 0; sd < 2; sd++)
             if (d->ipc_open[f][sd]) cudaIpcCloseMemHandle(d->ipc_peer[f][sd]);
+    if (d->h_stage) cudaFreeHost(d->h_stage);
+    if (d->h_sum) cudaFreeHost(d->h_sum);
     for (lgt_ctx* c : d->rk) lgt_destroy(c);
     delete d;
+    return LGT_OK;
+}
+
+int lgt_dd_halo_plan(int nranks, int rank, int lt_local, int plan[8]) {
+    if (!plan || nranks < 1 || rank < 0 || rank >= nranks || lt_local < 1) return LGT_EINVAL;
+    const HaloPlan p = halo_plan(nranks, rank, lt_local);
+    for (int k = 0; k < 2; k++) {
+        plan[k] = p.send_peer[k];
+        plan[2 + k] = p.send_slice[k];
+        plan[4 + k] = p.recv_peer[k];
+        plan[6 + k] = p.recv_slice[k];
+    }
+    return LGT_OK;
+}
+
+int lgt_dd_set_host_transport(lgt_dd* d, lgt_dd_sendrecv_fn sendrecv, lgt_dd_allreduce_fn allreduce, void* user) {
+    CHECK_DD(d);
+    if (!sendrecv || !allreduce) return dd_fail(d, LGT_EINVAL, "lgt_dd_set_host_transport: null callback");
+    if (d->rk.size() != 1) return dd_fail(d, LGT_ESTATE, "lgt_dd_set_host_transport: the host transport serves one rank per process");
+    if (d->comm) return dd_fail(d, LGT_ESTATE, "lgt_dd_set_host_transport: this group already uses NCCL");
+    d->host_sendrecv = sendrecv;
+    d->host_allreduce = allreduce;
+    d->host_user = user;
+    d->links_ghost_valid = false;
     return LGT_OK;
 }
 
@@ -1044,6 +1153,7 @@ int lgt_dd_nccl_init(lgt_dd* d, const void* id128) {
     if (!id128) return dd_fail(d, LGT_EINVAL, "lgt_dd_nccl_init: null id");
     if (d->rk.size() != 1) return dd_fail(d, LGT_ESTATE, "lgt_dd_nccl_init: the NCCL transport serves one rank per process");
     if (d->comm) return dd_fail(d, LGT_ESTATE, "lgt_dd_nccl_init: already initialised");
+    if (d->host_sendrecv) return dd_fail(d, LGT_ESTATE, "lgt_dd_nccl_init: this group already uses a host transport");
     if (!g_nccl.load()) return dd_fail(d, LGT_ECUDA, "lgt_dd_nccl_init: libnccl.so.2 not found");
     NcclApi::UniqueId id;
     memcpy(&id, id128, sizeof id);

@@ -90,9 +90,54 @@ def allgather_bytes(data, nbytes, device="cpu"):
     return [bytes(t.cpu().tolist()) for t in out]
 
 
-def decomposed_lattice(dims, beta, kappa, bc, precision=None, local_device=0, stream=None, halo="exchange"):
+def host_sendrecv(send_bufs, send_peers, recv_bufs, recv_peers, group=None):
+    """The `sendrecv` callback of lgt_dd_set_host_transport over a torch.distributed group with CPU tensors (gloo):
+    the k-th send of a rank is the k-th receive of its peer (lgt_dd_halo_plan), so message k carries tag k and the
+    pairing does not depend on arrival order.  A rank that is its own peer copies."""
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+
+    me = dist.get_rank(group) if dist.is_available() and dist.is_initialized() else 0
+    reqs = []
+    for k in range(2):
+        if send_peers[k] == me:  # this rank is its own neighbour: its k-th send is its own k-th receive
+            assert recv_peers[k] == me
+            np.copyto(recv_bufs[k], send_bufs[k])
+        else:
+            reqs.append(dist.isend(torch.from_numpy(send_bufs[k]), send_peers[k], group=group, tag=k))
+    for k in range(2):
+        if recv_peers[k] != me:
+            reqs.append(dist.irecv(torch.from_numpy(recv_bufs[k]), recv_peers[k], group=group, tag=k))
+    for r in reqs:
+        r.wait()
+
+
+def host_allreduce(buf, group=None):
+    """The `allreduce` callback: all-gather, then the sum in rank order on every rank -- the same bits everywhere, and
+    the same bits as the in-process lockstep mode (dd_local_allreduce_kernel adds in rank order too)."""
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+
+    if not (dist.is_available() and dist.is_initialized()):
+        return
+    mine = torch.from_numpy(np.array(buf, dtype=np.float64))
+    parts = [torch.zeros_like(mine) for _ in range(dist.get_world_size(group))]
+    dist.all_gather(parts, mine, group=group)
+    total = np.zeros_like(buf)
+    for p in parts:
+        total = total + p.numpy()
+    buf[:] = total
+
+
+def decomposed_lattice(dims, beta, kappa, bc, precision=None, local_device=0, stream=None, halo="exchange", transport="nccl",
+                       host_group=None):
     """This process's slab of ONE lattice shared by all ranks of the default process group: a DecomposedLattice with one
-    local rank whose NCCL communicator is initialised from an id that rank 0 creates and broadcasts here.
+    local rank.  transport = "nccl": the library's own NCCL communicator, initialised from an id that rank 0 creates and
+    broadcasts here.  transport = "host": halo slices and sums travel through host memory over `host_group` (a gloo
+    group; the default group if None) -- for clusters without NCCL between the ranks and for running the inter-process
+    path with several processes on ONE GPU, which NCCL refuses.
     halo = "push": the neighbours' CG buffers are mapped through CUDA IPC (handles all-gathered here) and the halo
     slices travel inside the Dslash kernels (lgt.LGT_DD_PUSH)."""
     from . import lgt
@@ -100,13 +145,17 @@ def decomposed_lattice(dims, beta, kappa, bc, precision=None, local_device=0, st
     rank, world, _ = env_rank_world()
     dd = lgt.DecomposedLattice(dims, world, [rank], beta, kappa, bc, lgt.LGT_F64 if precision is None else precision,
                                local_device, stream)
-    if world > 1:
+    on_cpu = transport == "host"
+    if transport == "host":
+        lgt.lgt_dd_set_host_transport(dd.d, lambda sb, sp, rb, rp: host_sendrecv(sb, sp, rb, rp, host_group),
+                                      lambda buf: host_allreduce(buf, host_group))
+    elif world > 1:
         ident = lgt.lgt_dd_nccl_unique_id() if rank == 0 else None
         ident = broadcast_bytes(ident, 128, src=0, device="cuda:%d" % local_device)
         lgt.lgt_dd_nccl_init(dd.d, ident)
-        if halo == "push":
-            handles = allgather_bytes(lgt.lgt_dd_ipc_export(dd.d), 128, device="cuda:%d" % local_device)
-            lgt.lgt_dd_ipc_import(dd.d, handles[(rank - 1) % world], handles[(rank + 1) % world])
+    if world > 1 and halo == "push":
+        handles = allgather_bytes(lgt.lgt_dd_ipc_export(dd.d), 128, device="cpu" if on_cpu else "cuda:%d" % local_device)
+        lgt.lgt_dd_ipc_import(dd.d, handles[(rank - 1) % world], handles[(rank + 1) % world])
     if halo == "push":
         lgt.lgt_dd_set_halo_mode(dd.d, lgt.LGT_DD_PUSH)
     return dd

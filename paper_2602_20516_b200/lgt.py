@@ -69,6 +69,8 @@ SYMBOLS = {
     "lgt_dd_last_error": (C.c_char_p, [_vp]),
     "lgt_dd_nccl_unique_id": (_i, [_vp]),
     "lgt_dd_nccl_init": (_i, [_vp, _vp]),
+    "lgt_dd_set_host_transport": (_i, [_vp, _vp, _vp, _vp]),
+    "lgt_dd_halo_plan": (_i, [_i, _i, _i, _ip]),
     "lgt_dd_set_halo_mode": (_i, [_vp, _i]),
     "lgt_dd_ipc_export": (_i, [_vp, _vp]),
     "lgt_dd_ipc_import": (_i, [_vp, _vp, _vp]),
@@ -415,6 +417,7 @@ def lgt_dd_create(dims, nranks, local_ranks, beta, kappa, bc, precision=LGT_F64,
 
 def lgt_dd_destroy(d):
     lib().lgt_dd_destroy(d)
+    _host_transports.pop(getattr(d, "value", None), None)
 
 
 def lgt_dd_last_error(d):
@@ -431,6 +434,55 @@ def lgt_dd_nccl_unique_id():
 
 def lgt_dd_nccl_init(d, id128):
     _dd_check(d, lib().lgt_dd_nccl_init(d, C.c_char_p(bytes(id128))))
+
+
+SENDRECV_FN = C.CFUNCTYPE(_i, _vp, C.POINTER(_vp), _ip, C.POINTER(_vp), _ip, C.c_size_t)
+ALLREDUCE_FN = C.CFUNCTYPE(_i, _vp, _dp, _i)
+_host_transports = {}  # group address -> the ctypes callback objects (they must outlive the group)
+
+
+def lgt_dd_halo_plan(nranks, rank, lt_local):
+    """Host-only.  Returns (send_peer, send_slice, recv_peer, recv_slice), two entries each, in issue order."""
+    plan = (C.c_int * 8)()
+    rc = lib().lgt_dd_halo_plan(nranks, rank, lt_local, plan)
+    if rc != LGT_OK:
+        raise LgtError(rc, "lgt_dd_halo_plan: bad arguments")
+    v = list(plan)
+    return v[0:2], v[2:4], v[4:6], v[6:8]
+
+
+def lgt_dd_set_host_transport(d, sendrecv, allreduce):
+    """sendrecv(send_bufs, send_peers, recv_bufs, recv_peers): two numpy uint8 views each way over the library's pinned
+    staging memory; allreduce(buf): numpy float64 view, summed over the ranks in place.  Exceptions become error codes."""
+    import numpy as np
+
+    def view(addr, n, ctype, dtype):
+        return np.frombuffer((ctype * n).from_address(addr), dtype=dtype)
+
+    def c_sendrecv(user, sb, sp, rb, rp, nbytes):
+        try:
+            sendrecv([view(sb[k], nbytes, C.c_ubyte, np.uint8) for k in range(2)], [sp[0], sp[1]],
+                     [view(rb[k], nbytes, C.c_ubyte, np.uint8) for k in range(2)], [rp[0], rp[1]])
+            return 0
+        except Exception:  # never unwind through the C frames
+            import traceback
+
+            traceback.print_exc()
+            return 1
+
+    def c_allreduce(user, buf, count):
+        try:
+            allreduce(view(C.addressof(buf.contents), count, C.c_double, np.float64))
+            return 0
+        except Exception:
+            import traceback
+
+            traceback.print_exc()
+            return 1
+
+    fns = (SENDRECV_FN(c_sendrecv), ALLREDUCE_FN(c_allreduce))
+    _dd_check(d, lib().lgt_dd_set_host_transport(d, C.cast(fns[0], _vp), C.cast(fns[1], _vp), None))
+    _host_transports[d.value] = fns
 
 
 def lgt_dd_set_halo_mode(d, mode):

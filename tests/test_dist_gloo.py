@@ -78,3 +78,100 @@ def test_single_process_identity():
     import pytest
     with pytest.raises(ValueError):
         dist.slab_rows((4, 4, 4, 10), 3, 0)
+
+
+# ---- the halo plan and the host transport of the decomposed lattice (lgt_dd_halo_plan, lgt_dd_set_host_transport)
+def test_halo_plan_with_in_order_matching():
+    """The plan every transport follows, run through a model of what NCCL, MPI and gloo guarantee -- messages between one
+    pair of ranks are matched in the order they were posted -- for 1, 2 (both neighbours are the same peer), 3, 4 and 8
+    ranks: every ghost slice must receive exactly the slice SURVEY 8(e) says it mirrors."""
+    from collections import defaultdict, deque
+
+    from paper_2602_20516_b200 import lgt
+
+    lgt.lib()
+    for nranks in (1, 2, 3, 4, 8):
+        for lt in (1, 2, 5):
+            plans = [lgt.lgt_dd_halo_plan(nranks, r, lt) for r in range(nranks)]
+            # field[r][slice] = (owner rank, owner's local slice) of the data held there; ghosts start empty
+            field = [[None] + [(r, t) for t in range(1, lt + 1)] + [None] for r in range(nranks)]
+            wires = defaultdict(deque)  # (src, dst) -> messages in posting order
+            for r, (sp, ss, rp, rs) in enumerate(plans):
+                for k in range(2):
+                    assert 1 <= ss[k] <= lt and rs[k] in (0, lt + 1)  # interior slices go out, ghost slices come in
+                    wires[(r, sp[k])].append(field[r][ss[k]])
+            for r, (sp, ss, rp, rs) in enumerate(plans):
+                for k in range(2):
+                    field[r][rs[k]] = wires[(rp[k], r)].popleft()
+            assert all(not q for q in wires.values())
+            for r in range(nranks):
+                assert field[r][0] == ((r - 1) % nranks, lt)      # lower ghost = last interior slice of rank r - 1
+                assert field[r][lt + 1] == ((r + 1) % nranks, 1)  # upper ghost = first interior slice of rank r + 1
+    with __import__("pytest").raises(lgt.LgtError):
+        lgt.lgt_dd_halo_plan(2, 2, 4)
+
+
+HOST_TRANSPORT_WORKER = textwrap.dedent("""
+    import json, sys
+    import numpy as np
+    sys.path.insert(0, %r)
+    from paper_2602_20516_b200 import dist, lgt
+    rank, world = dist.init("gloo")
+    lgt.lib()
+    lt, nbytes = 3, 4096
+    sp, ss, rp, rs = lgt.lgt_dd_halo_plan(world, rank, lt)
+    # a slab of lt + 2 slices; slice t of rank r is filled with the byte 16 * r + t
+    slab = np.zeros((lt + 2, nbytes), dtype=np.uint8)
+    for t in range(1, lt + 1):
+        slab[t] = 16 * rank + t
+    for rep in range(3):  # repeated exchanges must not cross-match
+        recv = [np.zeros(nbytes, dtype=np.uint8) for _ in range(2)]
+        dist.host_sendrecv([slab[ss[0]].copy(), slab[ss[1]].copy()], sp, recv, rp)
+        slab[rs[0]], slab[rs[1]] = recv[0], recv[1]
+        assert (slab[0] == 16 * ((rank - 1) %% world) + lt).all() and (slab[lt + 1] == 16 * ((rank + 1) %% world) + 1).all()
+    buf = np.array([0.1 * (rank + 1), 1e-17 * (rank + 1), 3.0], dtype=np.float64)
+    dist.host_allreduce(buf)
+    print(json.dumps({"rank": rank, "sum": [x.hex() for x in buf.tolist()]}))
+    dist.shutdown()
+""") % ROOT
+
+
+def test_host_transport_gloo_world_sizes(tmp_path):
+    """dist.host_sendrecv / host_allreduce (the callbacks behind lgt_dd_set_host_transport) between 2 and 3 gloo ranks:
+    with two ranks both neighbours are the one other rank, and each ghost must still get the right slice; the sums
+    are bit-identical on every rank and equal the rank-ordered sum."""
+    import json
+
+    script = tmp_path / "ht_worker.py"
+    script.write_text(HOST_TRANSPORT_WORKER)
+    for world in (2, 3):
+        port = free_port()
+        procs = []
+        for r in range(world):
+            env = dict(os.environ, RANK=str(r), WORLD_SIZE=str(world), LOCAL_RANK=str(r), MASTER_ADDR="127.0.0.1",
+                       MASTER_PORT=str(port), CUDA_VISIBLE_DEVICES="")
+            procs.append(subprocess.Popen([sys.executable, str(script)], env=env, stdout=subprocess.PIPE,
+                                          stderr=subprocess.PIPE, text=True))
+        sums = []
+        for p in procs:
+            o, e = p.communicate(timeout=300)
+            assert p.returncode == 0, e[-2000:]
+            sums.append(json.loads(o.strip().splitlines()[-1])["sum"])
+        expect = [0.0, 0.0, 0.0]
+        for r in range(world):
+            expect = [a + b for a, b in zip(expect, [0.1 * (r + 1), 1e-17 * (r + 1), 3.0])]
+        assert all(s == [x.hex() for x in expect] for s in sums)
+
+
+def test_host_transport_single_rank_is_a_copy():
+    import numpy as np
+
+    from paper_2602_20516_b200 import dist
+
+    a, b = np.arange(8, dtype=np.uint8), np.arange(8, 16, dtype=np.uint8)
+    ra, rb = np.zeros(8, dtype=np.uint8), np.zeros(8, dtype=np.uint8)
+    dist.host_sendrecv([a, b], [0, 0], [ra, rb], [0, 0])
+    assert (ra == a).all() and (rb == b).all()
+    buf = np.array([1.5, 2.5])
+    dist.host_allreduce(buf)
+    assert buf.tolist() == [1.5, 2.5]

@@ -464,3 +464,44 @@ def test_dd_even_odd_pushed_halos(lgt, nranks):
         dd.close()
     ex, pu = res[lgt.LGT_DD_EXCHANGE], res[lgt.LGT_DD_PUSH]
     assert np.array_equal(ex[0], pu[0]) and np.array_equal(ex[1], pu[1]) and ex[2] == pu[2] and ex[3] == pu[3]
+
+
+@pytest.mark.parametrize("world", [2, 3])
+def test_dd_between_processes_on_one_gpu(lgt, world):
+    """The inter-process path of the decomposition executed by SEPARATE PROCESSES that share this one GPU: one rank per
+    process (lgt_dd_create with nlocal = 1), halo slices and sums over the host transport on gloo (NCCL refuses two ranks
+    on one device, so NCCL itself stays covered by the one-rank test above), CUDA-IPC export / all-gather / import and
+    LGT_DD_PUSH stores into the other process's buffers.  With two processes both neighbours of a rank are the same peer.
+    The worker (tests/dd_two_process_worker.py) asserts, on every rank: Dslash, CG iterates and a leapfrog trajectory
+    bit-identical to the in-process lockstep group and within 1e-11 / 1e-12 of the oracle on the undivided lattice, the
+    oracle's CG iteration counts, for the exchange and the push mode; the mixed solver and the even/odd action on top."""
+    import json
+    import os
+    import socket
+    import subprocess
+    import sys
+
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    s = socket.socket()
+    s.bind(("127.0.0.1", 0))
+    port = s.getsockname()[1]
+    s.close()
+    procs = []
+    for r in range(world):
+        env = dict(os.environ, RANK=str(r), WORLD_SIZE=str(world), LOCAL_RANK="0", MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+        procs.append(subprocess.Popen([sys.executable, os.path.join(root, "tests", "dd_two_process_worker.py")], env=env,
+                                      stdout=subprocess.PIPE, stderr=subprocess.PIPE, text=True))
+    outs = []
+    try:
+        for p in procs:
+            o, e = p.communicate(timeout=900)
+            assert p.returncode == 0, (o[-1500:], e[-3000:])
+            outs.append(json.loads(o.strip().splitlines()[-1]))
+    finally:
+        for p in procs:
+            if p.poll() is None:
+                p.kill()
+    assert sorted(o["rank"] for o in outs) == list(range(world))
+    for o in outs:
+        for halo in ("exchange", "push"):
+            assert o[halo]["cg_iters"] == o["cg_iters_oracle"] and o[halo]["launches"] > 0
