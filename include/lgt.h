@@ -301,11 +301,12 @@ int lgt_cg_native(lgt_ctx* ctx, const void* b, void* x, void* y, double tol, int
 
 /* ---- per-kernel timing (CUDA events on the handle's stream, used by bench.py's roofline line) ---- */
 enum { LGT_K_DSLASH = 0,        /* out = D in, D^dag in, and CG step "t = D p" (+ |t|^2) */
-       LGT_K_CG_BLAS = 1,       /* CG initialisation and the x, p update pass */
+       LGT_K_CG_BLAS = 1,       /* CG initialisation, the one-block scalar kernels, precision conversion */
        LGT_K_FERMION_FORCE = 2, LGT_K_GAUGE_FORCE = 3, LGT_K_LINK_UPDATE = 4,
        LGT_K_OTHER = 5,         /* layout conversion, actions */
        LGT_K_DSLASH_R = 6,      /* CG step "q = D^dag t, r -= alpha q" (+ |r|^2), q kept on chip */
-       LGT_K_COUNT = 7 };
+       LGT_K_CG_UPDATE = 7,     /* CG step "x += alpha p, p = r + beta p" (one pass over x, p, r) */
+       LGT_K_COUNT = 8 };
 /* While enabled, every kernel launch is bracketed by a pair of CUDA events. */
 int lgt_timing_enable(lgt_ctx* ctx, int enable);
 /* Forgets the recorded launches (synchronises the stream). */
@@ -313,6 +314,15 @@ int lgt_timing_reset(lgt_ctx* ctx);
 /* Synchronises, then returns the summed device time (ms) and the number of launches of one kernel class
  * recorded since the last reset.  Either output may be NULL. */
 int lgt_timing_read(lgt_ctx* ctx, int kernel_class, double* ms_total, long* launches);
+
+/* ---- measured roofline denominators ---- */
+/* Two microbenchmarks on the handle's device and stream, timed with CUDA events, `launches` timed launches each after
+ * two untimed ones: (1) the FMA peak of the handle's precision -- 8 independent FMA chains per thread at full occupancy,
+ * 2 flops per FMA, in TFLOP/s; (2) a plain copy of the handle's native link field to a scratch buffer, read + write
+ * bytes, in GB/s.  `best` = fastest launch (burst), `mean` = average (sustained: under the power cap the clock drops).
+ * Any output may be NULL (both of a pair NULL skips that benchmark). */
+int lgt_measure_peaks(lgt_ctx* ctx, int launches, double* fma_tflops_best, double* fma_tflops_mean, double* copy_gbs_best,
+                      double* copy_gbs_mean);
 
 /* ---- introspection -------------------------------------------------------------------------- */
 /* Number of kernels this handle has launched since creation (bench.py's gpu_launches). */

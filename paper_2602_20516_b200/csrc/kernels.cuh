@@ -1324,6 +1324,28 @@ __global__ void __launch_bounds__(256) spinor_heatbath_kernel(Geom g, typename V
     }
 }
 
+// ---------------------------------------------------------------------------- roofline denominators, measured
+// fp64 / fp32 FMA peak: PEAK_CHAINS independent dependent-FMA chains per thread (enough to cover the FMA latency at
+// full occupancy), nothing else in the loop.  2 flops per FMA.
+constexpr int PEAK_CHAINS = 8;
+template <class T> __global__ void __launch_bounds__(256) peak_fma_kernel(double* sink, int iters, T a, T b) {
+    T x[PEAK_CHAINS];
+#pragma unroll
+    for (int j = 0; j < PEAK_CHAINS; j++) x[j] = (T)(threadIdx.x + j) * (T)1e-3;
+    for (int i = 0; i < iters; i++) {
+#pragma unroll
+        for (int j = 0; j < PEAK_CHAINS; j++) x[j] = fma(x[j], a, b);
+    }
+    T s = 0;
+#pragma unroll
+    for (int j = 0; j < PEAK_CHAINS; j++) s += x[j];
+    if (s == (T)-1.2345) sink[blockIdx.x] = (double)s;  // never true; keeps the chains alive
+}
+// plain device copy, 16 bytes per thread per step
+__global__ void __launch_bounds__(256) peak_copy_kernel(const int4* __restrict__ src, int4* __restrict__ dst, size_t n) {
+    for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) dst[i] = __ldg(src + i);
+}
+
 // ---------------------------------------------------------------------------- layout conversion
 __device__ __forceinline__ int link_sign(const Geom& g, int s, int mu) {
     if (g.bc[mu] > 0) return 1;

@@ -337,7 +337,7 @@ template <class T> struct Ops {
                     LAUNCH(c, LGT_K_CG_BLAS, (cg_scalars_kernel<1>), 1, 1024, ngrid, c->partials, c->st);
                     if ((r2 = dslash(c, U, t, nullptr, 1, 2, r)) != LGT_OK) return r2;
                     LAUNCH(c, LGT_K_CG_BLAS, (cg_scalars_kernel<2>), 1, 1024, ngrid, c->partials, c->st);
-                    LAUNCH(c, LGT_K_CG_BLAS, (cg_update_xp_kernel<T>), nb, 256, n, (T2*)x, p, (const T2*)r, c->st);
+                    LAUNCH(c, LGT_K_CG_UPDATE, (cg_update_xp_kernel<T>), nb, 256, n, (T2*)x, p, (const T2*)r, c->st);
                 }
                 return LGT_OK;
             };
@@ -580,7 +580,7 @@ template <class T> struct Ops {
                     if ((r2 = hop(c, 1, u, nullptr, t, 1, 3, -c->kappa)) != LGT_OK) return r2;   // t_o = kappa H^dag_oe u
                     if ((r2 = hop(c, 0, t, u, nullptr, 1, 2, c->kappa, r)) != LGT_OK) return r2; // r -= alpha M^dag u
                     LAUNCH(c, LGT_K_CG_BLAS, (cg_scalars_kernel<2>), 1, 1024, ngrid, c->partials, c->st);
-                    LAUNCH(c, LGT_K_CG_BLAS, (cg_update_xp_kernel<T>), nb, 256, n, x, p, (const T2*)r, c->st);
+                    LAUNCH(c, LGT_K_CG_UPDATE, (cg_update_xp_kernel<T>), nb, 256, n, x, p, (const T2*)r, c->st);
                 }
                 return LGT_OK;
             };
@@ -1484,6 +1484,67 @@ int lgt_hmc_trajectory(lgt_ctx* c, int nsteps, double dt, double tol, int max_it
     if (cg_iters) *cg_iters = total;
     if (H_initial) *H_initial = H0;
     return conv;
+}
+
+// ---- measured roofline denominators ("the builder must microbenchmark" the fp64 FMA peak)
+int lgt_measure_peaks(lgt_ctx* c, int launches, double* fma_tflops_best, double* fma_tflops_mean, double* copy_gbs_best,
+                      double* copy_gbs_mean) {
+    CHECK_CTX(c);
+    if (launches < 1 || launches > 1000) return fail(c, LGT_EINVAL, "lgt_measure_peaks: launches must be in 1..1000");
+    int sms = 148;
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, c->device);
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    CU(cudaEventCreate(&e0));
+    CU(cudaEventCreate(&e1));
+    int rc = LGT_OK;
+    auto time_launches = [&](auto launch, double work_per_launch, double* best, double* mean) -> int {
+        double tb = 1e30, tsum = 0.0;
+        for (int i = -2; i < launches; i++) {  // two untimed launches first
+            CU(cudaEventRecord(e0, c->stream));
+            launch();
+            CU(cudaEventRecord(e1, c->stream));
+            CU(cudaEventSynchronize(e1));
+            CU(cudaGetLastError());
+            float ms = 0.f;
+            CU(cudaEventElapsedTime(&ms, e0, e1));
+            if (i < 0) continue;
+            tsum += ms;
+            if (ms < tb) tb = ms;
+        }
+        if (best) *best = work_per_launch / (tb * 1e-3);
+        if (mean) *mean = work_per_launch / (tsum / launches * 1e-3);
+        return LGT_OK;
+    };
+    if (fma_tflops_best || fma_tflops_mean) {
+        // every SM holds 8 blocks of 256 threads (64 warps: full occupancy), each thread PEAK_CHAINS independent chains
+        const int grid = sms * 8, iters = c->prec == LGT_F64 ? 4096 : 16384;
+        const double flops = 2.0 * PEAK_CHAINS * (double)iters * 256.0 * grid;
+        double* sink = c->partials;  // grid <= red_blocks + 64 doubles... one slot per block
+        if (c->prec == LGT_F64)
+            rc = time_launches([&]() { peak_fma_kernel<double><<<grid, 256, 0, c->stream>>>(sink, iters, 1.0000001, 1e-9); }, flops * 1e-12,
+                               fma_tflops_best, fma_tflops_mean);
+        else
+            rc = time_launches([&]() { peak_fma_kernel<float><<<grid, 256, 0, c->stream>>>(sink, iters, 1.0001f, 1e-6f); }, flops * 1e-12,
+                               fma_tflops_best, fma_tflops_mean);
+        c->launches += launches + 2;
+    }
+    if (rc == LGT_OK && (copy_gbs_best || copy_gbs_mean)) {
+        // a plain copy of the native link field (604 MB at 32^4 fp64, well beyond L2) into a scratch buffer
+        const size_t bytes = links_bytes(c);
+        void* dst = nullptr;
+        cudaError_t e = cudaMalloc(&dst, bytes);
+        if (e != cudaSuccess) rc = fail(c, LGT_ENOMEM, "lgt_measure_peaks: cudaMalloc", e);
+        else {
+            const size_t n16 = bytes / 16;
+            rc = time_launches([&]() { peak_copy_kernel<<<sms * 16, 256, 0, c->stream>>>((const int4*)c->U, (int4*)dst, n16); }, 2.0 * (double)bytes * 1e-9,
+                               copy_gbs_best, copy_gbs_mean);
+            c->launches += launches + 2;
+            cudaFree(dst);
+        }
+    }
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    return rc;
 }
 
 // ---- stout smearing

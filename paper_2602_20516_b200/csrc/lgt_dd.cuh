@@ -497,7 +497,7 @@ template <class T> struct DdOps {
                     lgt_ctx* c = d->rk[i];
                     const size_t off = spinor_off(c), cnt = spinor_n(c);
                     LAUNCH(c, LGT_K_CG_BLAS, (cg_apply_kernel<2>), 1, 1, c->st);
-                    LAUNCH(c, LGT_K_CG_BLAS, (cg_update_xp_kernel<T>), stream_blocks(c, cnt), 256, cnt, (T2*)fld(c, 0) + off, (T2*)fld(c, 2) + off,
+                    LAUNCH(c, LGT_K_CG_UPDATE, (cg_update_xp_kernel<T>), stream_blocks(c, cnt), 256, cnt, (T2*)fld(c, 0) + off, (T2*)fld(c, 2) + off,
                            (const T2*)fld(c, 1) + off, c->st);
                     if (push) {
                         const size_t slice = (size_t)12 * d->V3;
@@ -717,7 +717,7 @@ template <class T> struct DdOps {
                 for (int i = 0; i < n; i++) {
                     lgt_ctx* c = d->rk[i];
                     const size_t off = half_off(c), cnt = half_n(c);
-                    LAUNCH(c, LGT_K_CG_BLAS, (cg_update_xp_kernel<T>), stream_blocks(c, cnt), 256, cnt, X(c) + off, P(c) + off,
+                    LAUNCH(c, LGT_K_CG_UPDATE, (cg_update_xp_kernel<T>), stream_blocks(c, cnt), 256, cnt, X(c) + off, P(c) + off,
                            (const T2*)R(c) + off, c->st);
                     if (push) {
                         const size_t slice = (size_t)6 * d->V3;

@@ -56,6 +56,7 @@ SYMBOLS = {
     "lgt_timing_enable": (_i, [_vp, _i]),
     "lgt_timing_reset": (_i, [_vp]),
     "lgt_timing_read": (_i, [_vp, _i, _dp, _lp]),
+    "lgt_measure_peaks": (_i, [_vp, _i, _dp, _dp, _dp, _dp]),
     "lgt_launch_count": (_l, [_vp]),
     "lgt_stream": (_vp, [_vp]),
     "lgt_set_block_swizzle": (_i, [_vp, _i, _ip]),
@@ -353,8 +354,17 @@ def lgt_cg_native(ctx, b, x, y, tol, max_iter):
 
 
 (LGT_K_DSLASH, LGT_K_CG_BLAS, LGT_K_FERMION_FORCE, LGT_K_GAUGE_FORCE, LGT_K_LINK_UPDATE, LGT_K_OTHER,
- LGT_K_DSLASH_R) = range(7)
-KERNEL_CLASSES = ("dslash", "cg_blas1", "fermion_force", "gauge_force", "link_update", "other", "dslash_dag_fused_r")
+ LGT_K_DSLASH_R, LGT_K_CG_UPDATE) = range(8)
+KERNEL_CLASSES = ("dslash", "cg_scalars", "fermion_force", "gauge_force", "link_update", "other", "dslash_dag_fused_r", "cg_update_xp")
+
+
+def lgt_measure_peaks(ctx, launches=10, fma=True, copy=True):
+    """Returns {"fma_tflops_best", "fma_tflops_mean", "copy_gbs_best", "copy_gbs_mean"} (None where not measured)."""
+    v = [C.c_double() for _ in range(4)]
+    _check(ctx, lib().lgt_measure_peaks(ctx, launches, C.byref(v[0]) if fma else None, C.byref(v[1]) if fma else None,
+                                        C.byref(v[2]) if copy else None, C.byref(v[3]) if copy else None))
+    keys = ("fma_tflops_best", "fma_tflops_mean", "copy_gbs_best", "copy_gbs_mean")
+    return {k: (x.value if (fma if i < 2 else copy) else None) for i, (k, x) in enumerate(zip(keys, v))}
 
 
 def lgt_timing_enable(ctx, enable=True):

@@ -659,34 +659,70 @@ def test_config3_full_size_solver_variants(lgt):
 
 
 def test_config4_largest_lattice_sampled(lgt):
-    """configs[4] shape (48^3 x 96, the largest single-GPU working set, Lx not a multiple of the 32-site layout block):
-    Dslash and fermion force on sampled sites.  The links are a periodic tiling of a seeded 24^4 warm field (a valid
-    SU(3) configuration of the full size that takes seconds, not minutes, to make on the host)."""
+    """configs[4] (48^3 x 96, the largest single-GPU working set, Lx not a multiple of the 32-site layout block; fp64 and
+    fp32; "Dslash, CG on D^dag D to 1e-10, fermion force and gauge force"), in the launch shape bench.py's configs4 sweep
+    times: D and D^dag, both forces on sampled sites / links against the oracle's per-site routines; one CG solve to
+    1e-10 checked by its TRUE residual with the oracle's D (two full oracle Dslashes) and by D X = eta; the fp32 Dslash
+    and both fp32 forces at 2e-5.  The links are a periodic tiling of a seeded 24^4 warm field (a valid SU(3)
+    configuration of the full size that takes seconds, not minutes, to make on the host)."""
     import torch
 
-    dims, kappa, bc = (48, 48, 48, 96), 0.12, BC
+    dims, beta, kappa, bc = (48, 48, 48, 96), 5.6, 0.12, BC
     free, _ = torch.cuda.mem_get_info()
-    if free < 40e9:
-        pytest.skip("needs about 40 GB of device memory")
+    assert free > 40e9, "configs[4] needs about 40 GB of free device memory; found %.1f GB" % (free / 1e9)
     V = synth.volume(dims)
     small = synth.warm_links((24, 24, 24, 24), 0.3, 1401).reshape(24, 24, 24, 24, 4, 3, 3)
     U = np.tile(small, (4, 2, 2, 2, 1, 1, 1)).reshape(V, 4, 3, 3)
     X = synth.gaussian_spinor(dims, 1402)
     Y = synth.gaussian_spinor(dims, 1403)
-    sites = _sample_sites(V, 100, 5)
-    lat = lgt.Lattice(dims, 5.6, kappa, bc)
+    # sampled sites, plus the corners of the index range and sites next to the antiperiodic time boundary
+    sites = np.unique(np.concatenate([_sample_sites(V, 100, 5), np.array([0, 47, 48 * 48 - 1, V - 1, V - 48 ** 3, V - 48 ** 3 - 1], dtype=np.int64)]))
+    lat = lgt.Lattice(dims, beta, kappa, bc)
     lat.set_links(U)
-    assert lgt.lgt_set_block_swizzle(lat.ctx, -1) > 0  # one time slice exceeds the L2 budget: slab order is on
-    out = lat.dslash(X)
-    assert site_rel_err(out[sites], oracle.dslash_sites(dims, kappa, bc, U, X, sites)) < TOL64
-    del out
+    for dag in (False, True):
+        out = lat.dslash(X, dagger=dag)
+        assert site_rel_err(out[sites], oracle.dslash_sites(dims, kappa, bc, U, X, sites, dagger=dag)) < TOL64
+        del out
     F, _ = lat.fermion_force(X, Y)
-    worst = 0.0
+    G = lat.gauge_force()
+    worst_f = worst_g = 0.0
     for s in sites[:40]:
         for mu in range(4):
             rf = oracle.fermion_force_link(dims, kappa, bc, U, X, Y, int(s), mu)
-            worst = max(worst, np.linalg.norm(F[s, mu] - rf) / np.linalg.norm(rf))
-    assert worst < TOL64, worst
+            rg = oracle.gauge_force_link(dims, beta, U, int(s), mu)
+            worst_f = max(worst_f, np.linalg.norm(F[s, mu] - rf) / np.linalg.norm(rf))
+            worst_g = max(worst_g, np.linalg.norm(G[s, mu] - rg) / np.linalg.norm(rg))
+    assert worst_f < TOL64 and worst_g < TOL64, (worst_f, worst_g)
+    del F, G
+    # CG on D^dag D to 1e-10 with phi = D^dag eta: true residual by the oracle's operator, and D X = eta (pin P6)
+    eta = Y
+    phi = oracle.dslash(dims, kappa, bc, U, eta, dagger=True)
+    Xs, it, rel, ok = lat.cg(phi, 1e-10, 10 * V)
+    assert ok and rel <= 1e-10 and 50 < it < 400, (it, rel)
+    DX = oracle.dslash(dims, kappa, bc, U, Xs)
+    assert np.linalg.norm(phi - oracle.dslash(dims, kappa, bc, U, DX, dagger=True)) <= 1.05e-10 * np.linalg.norm(phi)
+    assert site_rel_err(DX, eta) < 1e-7
+    del DX, Xs, phi
+    lat.close()
+    # fp32 (2e-5): inputs rounded to fp32 first (reading A-21)
+    U32, X32, Y32 = round32(U), round32(X), round32(Y)
+    del U, X, Y
+    lat = lgt.Lattice(dims, beta, kappa, bc, precision=lgt.LGT_F32)
+    lat.set_links(U32)
+    for dag in (False, True):
+        out = lat.dslash(X32, dagger=dag).astype(np.complex128)
+        assert site_rel_err(out[sites], oracle.dslash_sites(dims, kappa, bc, U32, X32, sites, dagger=dag)) < TOL32
+        del out
+    F32, _ = lat.fermion_force(X32, Y32)
+    G32 = lat.gauge_force()
+    worst_f = worst_g = 0.0
+    for s in sites[:30]:
+        for mu in range(4):
+            rf = oracle.fermion_force_link(dims, kappa, bc, U32, X32, Y32, int(s), mu)
+            rg = oracle.gauge_force_link(dims, beta, U32, int(s), mu)
+            worst_f = max(worst_f, np.linalg.norm(F32[s, mu].astype(np.complex128) - rf) / np.linalg.norm(rf))
+            worst_g = max(worst_g, np.linalg.norm(G32[s, mu].astype(np.complex128) - rg) / np.linalg.norm(rg))
+    assert worst_f < TOL32 and worst_g < TOL32, (worst_f, worst_g)
     lat.close()
 
 
