@@ -69,6 +69,20 @@ REALS_EO["cg_iter"] = 3 * REALS_EO["hop"] + REALS_EO["hop_fused_r"] + REALS_EO["
 REALS_STOUT_LEVEL = (2 * 36 + 32) + (32 + 2 * 2 * 36) + (32 + 2 * 32 + 32) + (2 * 36 + 32 + 32 + 2 * 32)
 
 
+# lgt_set_kernel_variant: what each number means (include/lgt.h has the same list)
+VARIANT_NAMES = {
+    "dslash": ["one 128-site block per chunk (default)",
+               "persistent, next chunk's first two hops requested before the current chunk's last",
+               "persistent, forward links by bulk copy (TMA) into per-warp shared-memory slots one chunk ahead",
+               "256-thread blocks on 2 x 2 x 2 tiles of 32-site layout blocks",
+               "variant 0 + L2 prefetch for the block 2 x SMs further on",
+               "variant 0 with the z and t neighbours loaded past L1 (no_allocate)"],
+    "gauge_force": ["one 32-site layout block x 4 directions per 128-thread block (default)",
+                    "two layout blocks per 256-thread block",
+                    "four layout blocks per 512-thread block (128 registers)"],
+}
+
+
 def step_reals(cg_iters, solver="cg", action="full", smear=0):
     fixed = REALS["gauge_force"] + REALS["fermion_force"] + REALS["link_update"] + smear * REALS_STOUT_LEVEL
     if action == "eo":  # CG on M^dag M, then Y_e = M X_e, X_o, Y_o (3 hops), split of phi and two merges (5 x 24 x 2)
@@ -965,6 +979,73 @@ def run_peaks(args):
     print(json.dumps({"peaks": out}), flush=True)
 
 
+def run_kernel_variants(args):
+    """`--kernel-variants`: the alternative implementations kept in the library (lgt_set_kernel_variant) on the headline
+    lattice, one after another in one process: isolated launches (CUDA events, inputs exceed L2), one CG solve each, and
+    whether the results equal variant 0's bit for bit.  This is the command behind profiles/r02*_variants.md."""
+    import torch
+
+    from paper_2602_20516_b200 import lgt, synth
+
+    torch.cuda.set_device(0)
+    cfg = dict(synth.CONFIGS[args.config])
+    if args.lattice:
+        cfg["dims"] = tuple(args.lattice)
+    dims, kappa, bc = cfg["dims"], cfg["kappa"], cfg["bc"]
+    V = synth.volume(dims)
+    U, _, eta = make_inputs(cfg)
+    lat = lgt.Lattice(dims, cfg["beta"], kappa, bc, lgt.LGT_F64, 0, torch.cuda.current_stream().cuda_stream)
+    ctx = lat.ctx
+    lgt.lgt_set_links_host(ctx, torch.from_numpy(U).pin_memory())
+    nat = [lat.native_spinor() for _ in range(4)]
+    lgt.lgt_spinor_to_native(ctx, lat.to_device(eta), nat[0])
+    del U, eta
+    out = {"lattice": "x".join(map(str, dims)), "dtype": "f64", "kernel_class": args.variant_class, "variants": {}}
+    kclass = lgt.KERNEL_CLASSES.index(args.variant_class)
+    ref = {}
+    names = VARIANT_NAMES[args.variant_class]
+    only = [int(v) for v in args.only_variants.split(",")] if args.only_variants else range(len(names))
+    for v in only:
+        lgt.lgt_set_kernel_variant(ctx, kclass, v)
+        res = {"what": names[v]}
+        if args.variant_class == "dslash":
+            for dag in (False, True):
+                t = time_calls(lambda: lgt.lgt_dslash_native(ctx, nat[0], nat[1], dag), n=args.variant_launches,
+                               warm=min(5, args.variant_launches))
+                key = "dslash_dagger" if dag else "dslash"
+                res[key] = {"us": round(t * 1e6, 1), "GB/s": round(REALS["dslash"] * 8 * V / t / 1e9, 1)}
+                got = nat[1].clone()
+                res[key]["bitwise_variant0"] = bool(torch.equal(got, ref.setdefault(key, got)))
+            if args.variant_no_cg:  # ncu captures: the isolated launches only
+                out["variants"][str(v)] = res
+                continue
+            lgt.lgt_dslash_native(ctx, nat[0], nat[2], True)  # phi = D^dag eta
+            for _ in range(2):
+                torch.cuda.synchronize()
+                t0 = time.perf_counter()
+                it, rel, ok = lgt.lgt_cg_native(ctx, nat[2], nat[3], None, cfg.get("cg_tol", 1e-12), 10 * V)
+                torch.cuda.synchronize()
+                dt = time.perf_counter() - t0
+            got = nat[3].clone()
+            res["cg"] = {"iters": it, "converged": ok, "us_per_iter": round(dt * 1e6 / max(it, 1), 1),
+                         "bitwise_variant0": bool(torch.equal(got, ref.setdefault("x", got)))}
+        else:
+            lgt.lgt_set_momenta_host(ctx, torch.zeros((V, 4, 3, 3), dtype=torch.complex128).pin_memory())
+            t = time_calls(lambda: lgt.lgt_gauge_force_accumulate(ctx, 1e-3), n=args.variant_launches,
+                           warm=min(5, args.variant_launches))
+            res["gauge_force"] = {"us": round(t * 1e6, 1), "GB/s": round(REALS["gauge_force"] * 8 * V / t / 1e9, 1),
+                                  "GFLOP/s": round(FLOPS["gauge_force"] * V / t / 1e9, 1)}
+            lgt.lgt_set_momenta_host(ctx, torch.zeros((V, 4, 3, 3), dtype=torch.complex128).pin_memory())
+            lgt.lgt_gauge_force_accumulate(ctx, 1.0)
+            got = torch.empty((V, 4, 3, 3), dtype=torch.complex128, device="cuda")
+            lgt.lgt_get_momenta(ctx, got)
+            base = ref.setdefault("F", got)
+            res["gauge_force"]["max_abs_diff_variant0"] = float((got - base).abs().max())
+        out["variants"][str(v)] = res
+    lat.close()
+    print(json.dumps(out), flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -997,6 +1078,12 @@ def main():
                     help="N > 1: 'replicas' = N independent lattices (default, weak scaling, plus one guarded decomposed pass); "
                          "'dd' = ONE lattice cut into N time slabs (lgt_dd_*, strong scaling) as the headline")
     ap.add_argument("--cpu-sample-iters", type=int, default=20, help="CG iterations in the oracle's bounded sample")
+    ap.add_argument("--kernel-variants", action="store_true",
+                    help="time every implementation variant of one kernel class on the headline lattice (profiles/r02*_variants.md)")
+    ap.add_argument("--variant-class", default="dslash", choices=sorted(VARIANT_NAMES))
+    ap.add_argument("--only-variants", default="", help="comma-separated variant numbers (default: all)")
+    ap.add_argument("--variant-launches", type=int, default=20)
+    ap.add_argument("--variant-no-cg", action="store_true", help="--kernel-variants: isolated launches only (for ncu captures)")
     ap.add_argument("--peaks", action="store_true", help="print the measured fp64 / fp32 FMA and copy peaks and exit")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
@@ -1005,6 +1092,8 @@ def main():
         ap.error("--same-gpu needs --transport host (NCCL refuses two ranks on one device)")
     if args.peaks:
         run_peaks(args)
+    elif args.kernel_variants:
+        run_kernel_variants(args)
     elif args.impl == "reference":
         run_reference(args)
     elif args.parallelism == "dd":

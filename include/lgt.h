@@ -335,6 +335,21 @@ void* lgt_stream(const lgt_ctx* ctx);
  * z_planes < 0: automatic (the default chosen by lgt_create).  LGT_EINVAL if Z does not divide Lz or Lx*Ly is
  * not a multiple of 128.  Returns the value in effect through *in_effect (may be NULL). */
 int lgt_set_block_swizzle(lgt_ctx* ctx, int z_planes, int* in_effect);
+/* Implementation variant of one kernel class (LGT_K_*); every variant computes the same operation and
+ * the alternatives stay in the library so that each measurement in profiles/ can be repeated.
+ *   LGT_K_DSLASH (covers LGT_K_DSLASH_R; D and D^dag bitwise the same in every variant):
+ *     0 = one 128-site block per chunk (dslash_kernel; the default and, measured, the fastest);
+ *     1 = persistent software-pipelined kernel: one wave of blocks loops over the chunks with the next chunk's first
+ *         loads in flight during the current chunk's last hops;
+ *     2 = persistent, the forward links brought by bulk copy (cp.async.bulk + mbarrier) into per-warp shared-memory
+ *         slots one chunk ahead;
+ *     3 = 256-thread blocks on 2 x 2 x 2 tiles of 32-site layout blocks (needs Lx*Ly % 64 == 0, even Lz and Lt,
+ *         an undivided lattice; other shapes run variant 0; CG sums differ from variant 0 in rounding);
+ *     4 = variant 0 plus an L2 prefetch of the forward links and t+1 spinors of the block 2 x SMs further on;
+ *     5 = variant 0 with the z and t neighbours loaded past L1 (ld.global.nc.L1::no_allocate).
+ * variant < 0 only queries.  The value in effect is returned through *in_effect (may be NULL).
+ * LGT_EINVAL for an unknown class or variant. */
+int lgt_set_kernel_variant(lgt_ctx* ctx, int kernel_class, int variant, int* in_effect);
 
 #ifdef __cplusplus
 }

@@ -96,15 +96,15 @@ template <class P> __device__ __forceinline__ P* mom_at(P* Pm, int s, int mu) {
     return Pm + ((size_t)(s >> 5) * (16 * W) + mu * (4 * W) + (s & 31));
 }
 
-template <class T> __device__ __forceinline__ void load_link(const typename Vec2<T>::type* U, int mu, int s, cx<T> u[9]) {
+template <class T, int NA = 0> __device__ __forceinline__ void load_link(const typename Vec2<T>::type* U, int mu, int s, cx<T> u[9]) {
     const typename Vec2<T>::type* b = link_at(U, s, mu);
 #pragma unroll
-    for (int k = 0; k < 9; k++) u[k] = ldc<T>(b + k * W);
+    for (int k = 0; k < 9; k++) u[k] = NA ? ldc_na(b + k * W) : ldc<T>(b + k * W);
 }
-template <class T> __device__ __forceinline__ void load_spinor(const typename Vec2<T>::type* f, int s, cx<T> p[12]) {
+template <class T, int NA = 0> __device__ __forceinline__ void load_spinor(const typename Vec2<T>::type* f, int s, cx<T> p[12]) {
     const typename Vec2<T>::type* b = spinor_at(f, s);
 #pragma unroll
-    for (int k = 0; k < 12; k++) p[k] = ldc<T>(b + k * W);
+    for (int k = 0; k < 12; k++) p[k] = NA ? ldc_na(b + k * W) : ldc<T>(b + k * W);
 }
 
 // ---------------------------------------------------------------------------- deterministic reductions
@@ -307,25 +307,25 @@ __global__ void dd_local_allreduce_kernel(DdPtrs ptrs, int nranks, int count) {
 
 // ---------------------------------------------------------------------------- A2: Wilson-Dirac operator
 // Forward hop of direction MU: acc += (1 + SG gamma_MU) U_MU(s) psi(s+MU)          (boundary sign is in U)
-template <int MU, int SG, class T>
+template <int MU, int SG, class T, int NA = 0>
 __device__ __forceinline__ void hop_fwd(const Geom& g, const typename Vec2<T>::type* U, const typename Vec2<T>::type* in,
                                         const Site& c, int s, cx<T> acc[12]) {
     const int sn = nbr_fwd(g, c, s, MU);
     cx<T> p[12], h[6], u[9], w[6];
-    load_spinor<T>(in, sn, p);
-    load_link<T>(U, MU, s, u);
+    load_spinor<T, NA>(in, sn, p);
+    load_link<T, NA>(U, MU, s, u);
     spin_project<MU, SG>(p, h);
     su3_mul_half(u, h, w);
     spin_reconstruct_add<MU, SG>(w, acc);
 }
 // Backward hop: acc += (1 + SG gamma_MU) U_MU^dag(s-MU) psi(s-MU)
-template <int MU, int SG, class T>
+template <int MU, int SG, class T, int NA = 0>
 __device__ __forceinline__ void hop_bwd(const Geom& g, const typename Vec2<T>::type* U, const typename Vec2<T>::type* in,
                                         const Site& c, int s, cx<T> acc[12]) {
     const int sn = nbr_bwd(g, c, s, MU);
     cx<T> p[12], h[6], u[9], w[6];
-    load_spinor<T>(in, sn, p);
-    load_link<T>(U, MU, sn, u);
+    load_spinor<T, NA>(in, sn, p);
+    load_link<T, NA>(U, MU, sn, u);
     spin_project<MU, SG>(p, h);
     su3_dag_mul_half(u, h, w);
     spin_reconstruct_add<MU, SG>(w, acc);
@@ -352,13 +352,36 @@ template <class T> struct PushTo {
     int da = 0, db = 0;
 };
 
-template <class T, int DAG, int MODE, int PUSH = 0>
+// PF > 0 (variant 4): every thread first asks L2 for the lines the block PF positions further on in the grid will need
+// from DRAM first -- its forward links and its t+1 spinors -- so that those loads find their data in L2 (prefetches hold
+// no registers; PF = the number of co-resident blocks, i.e. the block that takes this block's place on the SM).
+template <class T, int DAG, int MODE, int PUSH = 0, int PFON = 0>
 __global__ void __launch_bounds__(128, 1) dslash_kernel(Geom g, const typename Vec2<T>::type* __restrict__ U,
                                                         const typename Vec2<T>::type* __restrict__ in,
                                                         typename Vec2<T>::type* __restrict__ out, T kappa, CgState* st,
-                                                        double* partials, typename Vec2<T>::type* __restrict__ r, PushTo<T> push) {
+                                                        double* partials, typename Vec2<T>::type* __restrict__ r, PushTo<T> push,
+                                                        int pf = 0) {
     const int done = (MODE != 0) ? st->done : 0;
     const int s = g.s_begin + swizzled_chunk(g, blockIdx.x) * blockDim.x + threadIdx.x;
+    if (PFON == 1 && blockIdx.x + pf < gridDim.x && !(MODE != 0 && done)) {
+        const int sp = g.s_begin + swizzled_chunk(g, blockIdx.x + pf) * blockDim.x + threadIdx.x;
+        if (sp < g.s_end) {
+            // one lane per 128-byte line: the warp's link block is 36 x 32 complex, its spinor block 12 x 32, both contiguous
+            const int lane = threadIdx.x & 31;
+            constexpr int CPL = 128 / (int)sizeof(typename Vec2<T>::type);  // complex numbers per line
+            const typename Vec2<T>::type* bu = link_at(U, sp - lane, 0);
+#pragma unroll
+            for (int j = 0; j < (36 * W / CPL + 31) / 32; j++)
+                if (lane + 32 * j < 36 * W / CPL) asm volatile("prefetch.global.L2 [%0];" ::"l"(bu + (lane + 32 * j) * CPL));
+            const int spt = sp - lane + g.stride[3];
+            if (spt < g.s_end) {
+                const typename Vec2<T>::type* bp = spinor_at(in, spt);
+#pragma unroll
+                for (int j = 0; j < (12 * W / CPL + 31) / 32; j++)
+                    if (lane + 32 * j < 12 * W / CPL) asm volatile("prefetch.global.L2 [%0];" ::"l"(bp + (lane + 32 * j) * CPL));
+            }
+        }
+    }
     double nrm = 0.0;
     if (s < g.s_end) {
         if (MODE == 2) {
@@ -373,15 +396,16 @@ __global__ void __launch_bounds__(128, 1) dslash_kernel(Geom g, const typename V
 #pragma unroll
         for (int k = 0; k < 12; k++) acc[k] = mk<T>(0, 0);
         constexpr int F = DAG ? +1 : -1;  // D: (1 - gamma) forward, (1 + gamma) backward; D^dag: swapped
+        constexpr int NA = (PFON == 2) ? 1 : 0;  // variant 5: z and t neighbours (no reuse inside the block) bypass L1
         hop_fwd<0, F, T>(g, U, in, c, s, acc);
         if (MODE != 0 && done) return;  // uniform over the grid
         hop_bwd<0, -F, T>(g, U, in, c, s, acc);
         hop_fwd<1, F, T>(g, U, in, c, s, acc);
         hop_bwd<1, -F, T>(g, U, in, c, s, acc);
-        hop_fwd<2, F, T>(g, U, in, c, s, acc);
-        hop_bwd<2, -F, T>(g, U, in, c, s, acc);
-        hop_fwd<3, F, T>(g, U, in, c, s, acc);
-        hop_bwd<3, -F, T>(g, U, in, c, s, acc);
+        hop_fwd<2, F, T, NA>(g, U, in, c, s, acc);
+        hop_bwd<2, -F, T, NA>(g, U, in, c, s, acc);
+        hop_fwd<3, F, T, NA>(g, U, in, c, s, acc);
+        hop_bwd<3, -F, T, NA>(g, U, in, c, s, acc);
         const typename Vec2<T>::type* bi = spinor_at(in, s);
         if (MODE == 2) {
             const T alpha = (T)st->alpha;
@@ -416,6 +440,377 @@ __global__ void __launch_bounds__(128, 1) dslash_kernel(Geom g, const typename V
             typename Vec2<T>::type* bo = spinor_at(out, s);
 #pragma unroll
             for (int k = 0; k < 12; k++) stc<T>(bo + k * W, mk<T>(0, 0));
+        }
+    }
+    if (MODE != 0) block_partial(nrm, partials);
+}
+
+// The same operator as a PERSISTENT, software-pipelined kernel (variant 1 of lgt_set_kernel_variant(LGT_K_DSLASH)).
+// dslash_kernel gives every 128-site chunk its own block, so each block starts with empty registers: it issues its
+// first loads, waits one full (loaded) memory latency with nothing to compute, and at its end computes its last hops
+// with nothing in flight -- with ~28 blocks per SM slot, that ramp is paid 28 times per launch.  Here the grid is one
+// wave of blocks (2 per SM), each looping over chunks blockIdx, blockIdx + gridDim, ..., and the operands of the first
+// two hops of the NEXT chunk are requested before the current chunk's last hops and epilogue are computed, so the memory
+// pipe never drains between chunks.  Same arithmetic in the same order per site and the same block partials at the
+// same indices as dslash_kernel: results are bitwise identical.
+template <int MU, int FWD, class T>
+__device__ __forceinline__ void hop_load(const Geom& g, const typename Vec2<T>::type* U, const typename Vec2<T>::type* in,
+                                         const Site& c, int s, cx<T> p[12], cx<T> u[9]) {
+    const int sn = FWD ? nbr_fwd(g, c, s, MU) : nbr_bwd(g, c, s, MU);
+    load_spinor<T>(in, sn, p);
+    load_link<T>(U, MU, FWD ? s : sn, u);
+}
+template <int MU, int SG, int FWD, class T>
+__device__ __forceinline__ void hop_compute(const cx<T> p[12], const cx<T> u[9], cx<T> acc[12]) {
+    cx<T> h[6], w[6];
+    spin_project<MU, SG>(p, h);
+    if (FWD) su3_mul_half(u, h, w);
+    else su3_dag_mul_half(u, h, w);
+    spin_reconstruct_add<MU, SG>(w, acc);
+}
+
+template <class T, int DAG, int MODE>
+__global__ void __launch_bounds__(128, 1) dslash_persistent_kernel(Geom g, const typename Vec2<T>::type* __restrict__ U,
+                                                                   const typename Vec2<T>::type* __restrict__ in,
+                                                                   typename Vec2<T>::type* __restrict__ out, T kappa, CgState* st,
+                                                                   double* partials, typename Vec2<T>::type* __restrict__ r,
+                                                                   int nchunks) {
+    if (MODE != 0 && st->done) return;  // uniform over the grid
+    int chunk = blockIdx.x;
+    if (chunk >= nchunks) return;
+    constexpr int F = DAG ? +1 : -1;  // D: (1 - gamma) forward, (1 + gamma) backward; D^dag: swapped
+    const int last = g.s_end - 1;
+    int s = g.s_begin + swizzled_chunk(g, chunk) * 128 + threadIdx.x;
+    int sl = s < last ? s : last;  // lanes past the end compute on a valid site and store nothing
+    Site c = site_coords(g, sl);
+    cx<T> pa[12], ua[9], pb[12], ub[9];
+    hop_load<0, 1, T>(g, U, in, c, sl, pa, ua);
+    hop_load<0, 0, T>(g, U, in, c, sl, pb, ub);
+    for (;;) {
+        if (MODE == 2 && s <= last) {
+            const typename Vec2<T>::type* br = spinor_at(r, s);
+#pragma unroll
+            for (int k = 0; k < 12; k++) asm volatile("prefetch.global.L2 [%0];" ::"l"(br + k * W));
+        }
+        // where the next chunk is (the last chunk re-requests its own sites: L1 hits, results unused); computed here so
+        // that no branch separates the loads below from the hops around them
+        const int nchunk = chunk + gridDim.x;
+        const bool more = nchunk < nchunks;
+        const int s2 = more ? g.s_begin + swizzled_chunk(g, nchunk) * 128 + threadIdx.x : s;
+        const int sl2 = s2 < last ? s2 : last;
+        const Site c2 = site_coords(g, sl2);
+        cx<T> acc[12];
+#pragma unroll
+        for (int k = 0; k < 12; k++) acc[k] = mk<T>(0, 0);
+        hop_compute<0, F, 1, T>(pa, ua, acc);
+        hop_compute<0, -F, 0, T>(pb, ub, acc);
+        hop_fwd<1, F, T>(g, U, in, c, sl, acc);
+        hop_bwd<1, -F, T>(g, U, in, c, sl, acc);
+        hop_fwd<2, F, T>(g, U, in, c, sl, acc);
+        hop_bwd<2, -F, T>(g, U, in, c, sl, acc);
+        // the next chunk's first two hops go out now
+        hop_load<0, 1, T>(g, U, in, c2, sl2, pa, ua);
+        hop_load<0, 0, T>(g, U, in, c2, sl2, pb, ub);
+        hop_fwd<3, F, T>(g, U, in, c, sl, acc);
+        hop_bwd<3, -F, T>(g, U, in, c, sl, acc);
+        double nrm = 0.0;
+        if (s <= last) {
+            const typename Vec2<T>::type* bi = spinor_at(in, s);
+            if (MODE == 2) {
+                const T alpha = (T)st->alpha;
+                typename Vec2<T>::type* br = spinor_at(r, s);
+#pragma unroll
+                for (int k = 0; k < 12; k++) {
+                    cx<T> tv = ldc<T>(bi + k * W);
+                    cx<T> q = mk<T>(fma(-kappa, acc[k].re, tv.re), fma(-kappa, acc[k].im, tv.im));
+                    cx<T> rv = ldc_rw<T>(br + k * W);
+                    rv.re = fma(-alpha, q.re, rv.re);
+                    rv.im = fma(-alpha, q.im, rv.im);
+                    stc<T>(br + k * W, rv);
+                    nrm += (double)rv.re * (double)rv.re + (double)rv.im * (double)rv.im;
+                }
+            } else {
+                typename Vec2<T>::type* bo = spinor_at(out, s);
+#pragma unroll
+                for (int k = 0; k < 12; k++) {
+                    cx<T> pv = ldc<T>(bi + k * W);
+                    cx<T> o = mk<T>(fma(-kappa, acc[k].re, pv.re), fma(-kappa, acc[k].im, pv.im));
+                    stc<T>(bo + k * W, o);
+                    if (MODE == 1) nrm += (double)o.re * (double)o.re + (double)o.im * (double)o.im;
+                }
+            }
+        } else if (s >= g.V && s < g.Vs && MODE != 2) {  // padding lanes only, never a ghost slice
+            typename Vec2<T>::type* bo = spinor_at(out, s);
+#pragma unroll
+            for (int k = 0; k < 12; k++) stc<T>(bo + k * W, mk<T>(0, 0));
+        }
+        if (MODE != 0) {
+            block_partial(nrm, partials + chunk - blockIdx.x);  // block_partial adds blockIdx.x
+            __syncthreads();  // the partial's shared scratch is reused by the next chunk
+        }
+        if (!more) break;
+        chunk = nchunk;
+        s = s2;
+        sl = sl2;
+        c = c2;
+    }
+}
+
+// Variant 2: the persistent kernel with the FORWARD LINKS brought in by the bulk-copy engine (TMA, cp.async.bulk) one
+// chunk ahead.  In the native layout the nine components of U_mu for the 32 sites of a warp are one contiguous run
+// (9 x 32 complex = 4.5 KB in fp64), so each warp owns four shared-memory slots, one per direction, each with its own
+// mbarrier: at the top of a chunk the warp waits (once) for its four slots, every forward hop reads its link from the
+// slot instead of from global memory, and as soon as all 32 lanes have read slot mu, lane 0 re-arms it with the link
+// block of the warp's NEXT chunk.  The forward links are 60 % of the kernel's compulsory DRAM bytes and each is used
+// exactly once: with them prefetched most of a chunk ahead and held in shared memory instead of in registers, the
+// loads the threads still issue themselves are the neighbour spinors and backward links, nearly all L2 hits.
+// Ordering without compiler barriers (which would cut the load batching the kernel lives on): the slot reads depend
+// on a zero the wait returns, and the re-arm depends on a warp vote over a value formed from every lane's reads.
+// Same arithmetic in the same order as dslash_kernel, same block partials: bitwise identical results.
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned bar, unsigned count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
+}
+// waits until the four consecutive barriers at `bar` have completed the phase of the given parity; returns 0
+__device__ __forceinline__ unsigned mbar_wait4(unsigned bar, unsigned parity) {
+    unsigned zero;
+    asm volatile(
+        "{\n"
+        ".reg .pred p0, p1, p2, p3;\n"
+        "W4_AGAIN:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p0, [%1], %2;\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p1, [%1+8], %2;\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p2, [%1+16], %2;\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p3, [%1+24], %2;\n"
+        "and.pred p0, p0, p1;\n"
+        "and.pred p2, p2, p3;\n"
+        "and.pred p0, p0, p2;\n"
+        "@p0 bra W4_DONE;\n"
+        "bra W4_AGAIN;\n"
+        "W4_DONE:\n"
+        "mov.u32 %0, 0;\n"
+        "}"
+        : "=r"(zero)
+        : "r"(bar), "r"(parity)
+        : "memory");
+    return zero;
+}
+// if `go`: arm the barrier with `bytes` and start the bulk copy global -> shared that completes on it.  `after` is a
+// value the copy must not overtake (the vote over the lanes' reads of the slot being overwritten).
+__device__ __forceinline__ void bulk_load_if(bool go, unsigned dst, const void* src, unsigned bytes, unsigned bar, unsigned after) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p, q;\n"
+        ".reg .b32 t;\n"
+        ".reg .b64 st;\n"
+        "or.b32 t, %5, 0x80000000;\n"
+        "setp.ne.b32 q, t, 0x12345678;\n"   // always true, but only known once `after` is
+        "setp.ne.and.b32 p, %0, 0, q;\n"
+        "@p fence.proxy.async.shared::cta;\n"
+        "@p mbarrier.arrive.expect_tx.shared::cta.b64 st, [%4], %3;\n"
+        "@p cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%1], [%2], %3, [%4];\n"
+        "}" ::"r"((unsigned)go),
+        "r"(dst), "l"(src), "r"(bytes), "r"(bar), "r"(after));
+}
+
+template <int MU, int SG, class T>
+__device__ __forceinline__ unsigned hop_fwd_slot(const Geom& g, const typename Vec2<T>::type* slot_lane,
+                                                 const typename Vec2<T>::type* in, const Site& c, int s, cx<T> acc[12]) {
+    const int sn = nbr_fwd(g, c, s, MU);
+    cx<T> p[12], h[6], u[9], w[6];
+    load_spinor<T>(in, sn, p);
+    unsigned seen = 0;
+#pragma unroll
+    for (int k = 0; k < 9; k++) {
+        const typename Vec2<T>::type v = slot_lane[k * W];
+        u[k] = mk<T>(v.x, v.y);
+        seen ^= (sizeof(T) == 8) ? (unsigned)__double2loint((double)v.x) : __float_as_uint((float)v.x);
+    }
+    spin_project<MU, SG>(p, h);
+    su3_mul_half(u, h, w);
+    spin_reconstruct_add<MU, SG>(w, acc);
+    return seen;
+}
+
+template <class T> constexpr int dslash_tma_smem_bytes() { return 4 * 4 * 9 * W * (int)sizeof(typename Vec2<T>::type) + 4 * 4 * 8; }
+
+template <class T, int DAG, int MODE>
+__global__ void __launch_bounds__(128, 1) dslash_tma_kernel(Geom g, const typename Vec2<T>::type* __restrict__ U,
+                                                            const typename Vec2<T>::type* __restrict__ in,
+                                                            typename Vec2<T>::type* __restrict__ out, T kappa, CgState* st,
+                                                            double* partials, typename Vec2<T>::type* __restrict__ r, int nchunks) {
+    typedef typename Vec2<T>::type T2;
+    extern __shared__ __align__(128) unsigned char dslash_smem[];
+    if (MODE != 0 && st->done) return;  // uniform over the grid
+    int chunk = blockIdx.x;
+    if (chunk >= nchunks) return;
+    constexpr int F = DAG ? +1 : -1;
+    constexpr unsigned SLOT_BYTES = 9 * W * sizeof(T2);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    T2* slots = reinterpret_cast<T2*>(dslash_smem) + warp * (4 * 9 * W);
+    const unsigned slots_u32 = smem_u32(slots);
+    const unsigned bars = smem_u32(dslash_smem + 4 * 4 * SLOT_BYTES) + warp * 32;
+    const int last = g.s_end - 1;
+    const int last_blk = last >> 5;
+    if (lane == 0) {
+#pragma unroll
+        for (int mu = 0; mu < 4; mu++) mbar_init(bars + 8 * mu, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncwarp();
+    int s = g.s_begin + swizzled_chunk(g, chunk) * 128 + threadIdx.x;
+    {
+        int blk = (s - lane) >> 5;
+        blk = blk < last_blk ? blk : last_blk;
+#pragma unroll
+        for (int mu = 0; mu < 4; mu++)
+            bulk_load_if(lane == 0, slots_u32 + mu * SLOT_BYTES, U + ((size_t)blk * 36 + mu * 9) * W, SLOT_BYTES, bars + 8 * mu, 0u);
+    }
+    unsigned parity = 0;
+    for (;;) {
+        const int sl = s < last ? s : last;  // lanes past the end compute on a valid site and store nothing
+        if (MODE == 2 && s <= last) {
+            const T2* br = spinor_at(r, s);
+#pragma unroll
+            for (int k = 0; k < 12; k++) asm volatile("prefetch.global.L2 [%0];" ::"l"(br + k * W));
+        }
+        const Site c = site_coords(g, sl);
+        const int nchunk = chunk + gridDim.x;
+        const bool more = nchunk < nchunks;
+        const int s2 = more ? g.s_begin + swizzled_chunk(g, nchunk) * 128 + threadIdx.x : s;
+        int blk2 = (s2 - lane) >> 5;
+        blk2 = blk2 < last_blk ? blk2 : last_blk;
+        const T2* next_links = U + (size_t)blk2 * 36 * W;
+        const bool issue = more && lane == 0;
+        const unsigned zero = mbar_wait4(bars, parity);
+        const T2* slot_lane = slots + lane + zero;
+        cx<T> acc[12];
+#pragma unroll
+        for (int k = 0; k < 12; k++) acc[k] = mk<T>(0, 0);
+        unsigned seen;
+        seen = hop_fwd_slot<0, F, T>(g, slot_lane + 0 * 9 * W, in, c, sl, acc);
+        bulk_load_if(issue, slots_u32 + 0 * SLOT_BYTES, next_links + 0 * 9 * W, SLOT_BYTES, bars + 0, __ballot_sync(0xffffffffu, seen != 0x9e3779b9u));
+        hop_bwd<0, -F, T>(g, U, in, c, sl, acc);
+        seen = hop_fwd_slot<1, F, T>(g, slot_lane + 1 * 9 * W, in, c, sl, acc);
+        bulk_load_if(issue, slots_u32 + 1 * SLOT_BYTES, next_links + 1 * 9 * W, SLOT_BYTES, bars + 8, __ballot_sync(0xffffffffu, seen != 0x9e3779b9u));
+        hop_bwd<1, -F, T>(g, U, in, c, sl, acc);
+        seen = hop_fwd_slot<2, F, T>(g, slot_lane + 2 * 9 * W, in, c, sl, acc);
+        bulk_load_if(issue, slots_u32 + 2 * SLOT_BYTES, next_links + 2 * 9 * W, SLOT_BYTES, bars + 16, __ballot_sync(0xffffffffu, seen != 0x9e3779b9u));
+        hop_bwd<2, -F, T>(g, U, in, c, sl, acc);
+        seen = hop_fwd_slot<3, F, T>(g, slot_lane + 3 * 9 * W, in, c, sl, acc);
+        bulk_load_if(issue, slots_u32 + 3 * SLOT_BYTES, next_links + 3 * 9 * W, SLOT_BYTES, bars + 24, __ballot_sync(0xffffffffu, seen != 0x9e3779b9u));
+        hop_bwd<3, -F, T>(g, U, in, c, sl, acc);
+        double nrm = 0.0;
+        if (s <= last) {
+            const T2* bi = spinor_at(in, s);
+            if (MODE == 2) {
+                const T alpha = (T)st->alpha;
+                T2* br = spinor_at(r, s);
+#pragma unroll
+                for (int k = 0; k < 12; k++) {
+                    cx<T> tv = ldc<T>(bi + k * W);
+                    cx<T> q = mk<T>(fma(-kappa, acc[k].re, tv.re), fma(-kappa, acc[k].im, tv.im));
+                    cx<T> rv = ldc_rw<T>(br + k * W);
+                    rv.re = fma(-alpha, q.re, rv.re);
+                    rv.im = fma(-alpha, q.im, rv.im);
+                    stc<T>(br + k * W, rv);
+                    nrm += (double)rv.re * (double)rv.re + (double)rv.im * (double)rv.im;
+                }
+            } else {
+                T2* bo = spinor_at(out, s);
+#pragma unroll
+                for (int k = 0; k < 12; k++) {
+                    cx<T> pv = ldc<T>(bi + k * W);
+                    cx<T> o = mk<T>(fma(-kappa, acc[k].re, pv.re), fma(-kappa, acc[k].im, pv.im));
+                    stc<T>(bo + k * W, o);
+                    if (MODE == 1) nrm += (double)o.re * (double)o.re + (double)o.im * (double)o.im;
+                }
+            }
+        } else if (s >= g.V && s < g.Vs && MODE != 2) {  // padding lanes only, never a ghost slice
+            T2* bo = spinor_at(out, s);
+#pragma unroll
+            for (int k = 0; k < 12; k++) stc<T>(bo + k * W, mk<T>(0, 0));
+        }
+        if (MODE != 0) {
+            block_partial(nrm, partials + chunk - blockIdx.x);
+            __syncthreads();  // the partial's shared scratch is reused by the next chunk
+        }
+        if (!more) break;
+        chunk = nchunk;
+        s = s2;
+        parity ^= 1u;
+    }
+}
+
+// Variant 3: 4-D site blocking by block-to-site mapping (the layout is unchanged).  dslash_kernel's block is 128
+// consecutive lexicographic sites (four x rows at 32^4), so of the nine spinors and eight links a site needs only the
+// x and most y neighbours are shared inside the block: L2 -> L1 traffic is 2.06 KB per site for 0.96 KB compulsory.
+// Here a block of 256 threads covers a 2 x 2 x 2 arrangement of 32-site layout blocks -- two consecutive ones (64
+// lexicographic sites), at z and z+1, at t and t+1 -- so that half of the z and t neighbours (spinors, and the
+// backward links) are shared through L1 as well: 1.56 KB per site when L1 holds the tile.  One block per SM at ~250
+// registers, i.e. the same 8 warps per SM as dslash_kernel.  Needs Lx*Ly % 64 == 0, even Lz and Lt and an undivided
+// lattice.  Per-site arithmetic identical to dslash_kernel; the block partials cover other site sets, so CG sums
+// differ from variant 0 in rounding only.
+__device__ __forceinline__ int tile_site(const Geom& g, int b, int tid) {
+    const int nsub = (g.L[0] * g.L[1]) >> 6;  // 64-site sub-chunks per xy plane
+    const int zh = g.L[2] >> 1;
+    const int j = b % nsub;
+    const int r = b / nsub;
+    const int zp = r % zh, tp = r / zh;
+    const int w = tid >> 5;
+    const int z = 2 * zp + ((w >> 1) & 1), t = 2 * tp + (w >> 2);
+    return (t * g.L[2] + z) * (g.L[0] * g.L[1]) + 64 * j + 32 * (w & 1) + (tid & 31);
+}
+
+template <class T, int DAG, int MODE>
+__global__ void __launch_bounds__(256, 1) dslash_tile_kernel(Geom g, const typename Vec2<T>::type* __restrict__ U,
+                                                             const typename Vec2<T>::type* __restrict__ in,
+                                                             typename Vec2<T>::type* __restrict__ out, T kappa, CgState* st,
+                                                             double* partials, typename Vec2<T>::type* __restrict__ r) {
+    const int done = (MODE != 0) ? st->done : 0;
+    const int s = tile_site(g, blockIdx.x, threadIdx.x);  // always a lattice site: V is a multiple of 256 here
+    double nrm = 0.0;
+    if (MODE == 2) {
+        const typename Vec2<T>::type* br = spinor_at(r, s);
+#pragma unroll
+        for (int k = 0; k < 12; k++) asm volatile("prefetch.global.L2 [%0];" ::"l"(br + k * W));
+    }
+    const Site c = site_coords(g, s);
+    cx<T> acc[12];
+#pragma unroll
+    for (int k = 0; k < 12; k++) acc[k] = mk<T>(0, 0);
+    constexpr int F = DAG ? +1 : -1;
+    hop_fwd<0, F, T>(g, U, in, c, s, acc);
+    if (MODE != 0 && done) return;  // uniform over the grid
+    hop_bwd<0, -F, T>(g, U, in, c, s, acc);
+    hop_fwd<1, F, T>(g, U, in, c, s, acc);
+    hop_bwd<1, -F, T>(g, U, in, c, s, acc);
+    hop_fwd<2, F, T>(g, U, in, c, s, acc);
+    hop_bwd<2, -F, T>(g, U, in, c, s, acc);
+    hop_fwd<3, F, T>(g, U, in, c, s, acc);
+    hop_bwd<3, -F, T>(g, U, in, c, s, acc);
+    const typename Vec2<T>::type* bi = spinor_at(in, s);
+    if (MODE == 2) {
+        const T alpha = (T)st->alpha;
+        typename Vec2<T>::type* br = spinor_at(r, s);
+#pragma unroll
+        for (int k = 0; k < 12; k++) {
+            cx<T> tv = ldc<T>(bi + k * W);
+            cx<T> q = mk<T>(fma(-kappa, acc[k].re, tv.re), fma(-kappa, acc[k].im, tv.im));
+            cx<T> rv = ldc_rw<T>(br + k * W);
+            rv.re = fma(-alpha, q.re, rv.re);
+            rv.im = fma(-alpha, q.im, rv.im);
+            stc<T>(br + k * W, rv);
+            nrm += (double)rv.re * (double)rv.re + (double)rv.im * (double)rv.im;
+        }
+    } else {
+        typename Vec2<T>::type* bo = spinor_at(out, s);
+#pragma unroll
+        for (int k = 0; k < 12; k++) {
+            cx<T> pv = ldc<T>(bi + k * W);
+            cx<T> o = mk<T>(fma(-kappa, acc[k].re, pv.re), fma(-kappa, acc[k].im, pv.im));
+            stc<T>(bo + k * W, o);
+            if (MODE == 1) nrm += (double)o.re * (double)o.re + (double)o.im * (double)o.im;
         }
     }
     if (MODE != 0) block_partial(nrm, partials);
@@ -597,14 +992,22 @@ __global__ void __launch_bounds__(128, 1) fermion_force_kernel(Geom g, const typ
 // two blocks per SM (~244 registers) let the compiler batch the 18 link loads: 680 us against 775 us at 174 registers;
 // the staple loop is written over the three nu != mu and fully unrolled (a loop over four with a skip is not, and keeps
 // the loads of one staple behind the arithmetic of the previous one): 756 -> 633 us at 32^4 fp64, same sums bit for bit.
-template <class T, int ACC>
-__global__ void __launch_bounds__(128, 2) gauge_force_kernel(Geom g, const typename Vec2<T>::type* __restrict__ U,
-                                                          typename Vec2<T>::type* __restrict__ P, T beta_over_6, T eps) {
+// ROWS (1, 2 or 4) = 32-site layout blocks per thread block (ROWS x 128 threads, warp = (block, direction)): the
+// neighbouring rows' links are then shared through L1 by more warps (variants of LGT_K_GAUGE_FORCE).
+// The direction stays a run-time value on purpose: dispatching the warp to a body with the direction as a template
+// constant (no indexed local Site array, 0 bytes of stack) was measured at 989 us against 606 us at 32^4 fp64 -- the
+// compiler then schedules each staple's loads behind the previous staple's arithmetic again.
+template <class T, int ACC, int ROWS = 1>
+__global__ void __launch_bounds__(128 * ROWS, ROWS == 1 ? 2 : 1)
+    gauge_force_kernel(Geom g, const typename Vec2<T>::type* __restrict__ U, typename Vec2<T>::type* __restrict__ P,
+                       T beta_over_6, T eps) {
     // same slab-by-slab block order as the Dslash kernels on lattices whose time slice exceeds L2 (four 32-site blocks
     // per 128-site chunk)
-    const int s = g.s_begin + (swizzled_chunk(g, blockIdx.x >> 2) * 4 + (blockIdx.x & 3)) * W + (threadIdx.x & 31);
+    constexpr int BPC = 4 / ROWS;  // thread blocks per 128-site chunk
+    const int s = g.s_begin +
+                  (swizzled_chunk(g, blockIdx.x / BPC) * 4 + (blockIdx.x % BPC) * ROWS + (threadIdx.x >> 7)) * W + (threadIdx.x & 31);
     if (s >= g.s_end) return;
-    const int mu = threadIdx.x >> 5;
+    const int mu = (threadIdx.x >> 5) & 3;
     const Site c = site_coords(g, s);
     const int smu = nbr_fwd(g, c, s, mu);
     cx<T> V[9];

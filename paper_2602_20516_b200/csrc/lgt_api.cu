@@ -4,6 +4,7 @@
 
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -73,6 +74,8 @@ struct lgt_ctx {
     CgState* h_st = nullptr;  // pinned
     double* h_scal = nullptr;  // pinned
     int red_blocks = 0;
+    int num_sms = 0;
+    int variant[LGT_K_COUNT] = {};  // kernel variant per class (lgt_set_kernel_variant)
     long launches = 0;
     // optional CUDA-event timing of every launch, by kernel class (lgt_timing_*)
     bool timing = false;
@@ -135,6 +138,31 @@ cudaEvent_t timing_event(lgt_ctx* c) {
             }                                                       \
         }                                                           \
         kern<<<(grid), (block), 0, (c)->stream>>>(__VA_ARGS__);     \
+        if (e0_ && e1_) cudaEventRecord(e1_, (c)->stream);          \
+        (c)->launches++;                                            \
+        cudaError_t e_ = cudaGetLastError();                        \
+        if (e_ != cudaSuccess) return fail((c), LGT_ECUDA, #kern, e_); \
+    } while (0)
+
+// the same with dynamic shared memory (opt-in above 48 KB, once per kernel instantiation)
+#define LAUNCH_SMEM(c, kclass, kern, grid, block, smem, ...)        \
+    do {                                                            \
+        static bool attr_set_ = false;                              \
+        if (!attr_set_) {                                           \
+            cudaError_t ea_ = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (smem)); \
+            if (ea_ != cudaSuccess) return fail((c), LGT_ECUDA, "cudaFuncSetAttribute " #kern, ea_); \
+            attr_set_ = true;                                       \
+        }                                                           \
+        cudaEvent_t e0_ = nullptr, e1_ = nullptr;                   \
+        if ((c)->timing) {                                          \
+            e0_ = timing_event(c);                                  \
+            e1_ = timing_event(c);                                  \
+            if (e0_ && e1_) {                                       \
+                (c)->ev_class.push_back(kclass);                    \
+                cudaEventRecord(e0_, (c)->stream);                  \
+            }                                                       \
+        }                                                           \
+        kern<<<(grid), (block), (smem), (c)->stream>>>(__VA_ARGS__); \
         if (e0_ && e1_) cudaEventRecord(e1_, (c)->stream);          \
         (c)->launches++;                                            \
         cudaError_t e_ = cudaGetLastError();                        \
@@ -277,6 +305,15 @@ template <class T> struct Ops {
         return LGT_OK;
     }
 
+    // dslash_tile_kernel's preconditions (an undivided lattice whose xy planes split into 64-site runs, even Lz, Lt)
+    static bool tile_ok(const lgt_ctx* c) {
+        const Geom& g = c->g;
+        return g.s_begin == 0 && g.s_end == g.V && (g.L[0] * g.L[1]) % 64 == 0 && g.L[2] % 2 == 0 && g.L[3] % 2 == 0;
+    }
+    // blocks (= partials) of the stencil kernels' CG modes
+    static int dslash_partials(const lgt_ctx* c) {
+        return (c->variant[LGT_K_DSLASH] == 3 && tile_ok(c)) ? c->g.V / 256 : site_blocks(c, 128);
+    }
     // mode 0: out = D in / D^dag in; 1: CG "t = D p" (+ pAp, alpha); 2: CG "q = D^dag t" fused with the x, r update
     static int dslash(lgt_ctx* c, const void* U, const void* in, void* out, int dagger, int mode, void* r = nullptr,
                       const PushTo<T>* push = nullptr) {
@@ -295,6 +332,80 @@ template <class T> struct Ops {
             return LGT_OK;
         }
 #undef DSLASH_PUSH_ARGS
+        if (c->variant[LGT_K_DSLASH] == 1) {  // persistent, software-pipelined: one wave of blocks loops over the chunks
+            const int pgrid = grid < 2 * c->num_sms ? grid : 2 * c->num_sms;
+#define DSLASH_PARGS c->g, (const T2*)U, (const T2*)in, (T2*)out, kappa, c->st, c->partials, (T2*)r, grid
+            if (mode == 0) {
+                if (dagger)
+                    LAUNCH(c, LGT_K_DSLASH, (dslash_persistent_kernel<T, 1, 0>), pgrid, 128, DSLASH_PARGS);
+                else
+                    LAUNCH(c, LGT_K_DSLASH, (dslash_persistent_kernel<T, 0, 0>), pgrid, 128, DSLASH_PARGS);
+            } else if (mode == 1) {
+                LAUNCH(c, LGT_K_DSLASH, (dslash_persistent_kernel<T, 0, 1>), pgrid, 128, DSLASH_PARGS);
+            } else {
+                LAUNCH(c, LGT_K_DSLASH_R, (dslash_persistent_kernel<T, 1, 2>), pgrid, 128, DSLASH_PARGS);
+            }
+            return LGT_OK;
+        }
+        if (c->variant[LGT_K_DSLASH] == 2) {  // persistent, forward links by bulk copy into per-warp shared-memory slots
+            const int pgrid = grid < 2 * c->num_sms ? grid : 2 * c->num_sms;
+            constexpr int smem = dslash_tma_smem_bytes<T>();
+            if (mode == 0) {
+                if (dagger)
+                    LAUNCH_SMEM(c, LGT_K_DSLASH, (dslash_tma_kernel<T, 1, 0>), pgrid, 128, smem, DSLASH_PARGS);
+                else
+                    LAUNCH_SMEM(c, LGT_K_DSLASH, (dslash_tma_kernel<T, 0, 0>), pgrid, 128, smem, DSLASH_PARGS);
+            } else if (mode == 1) {
+                LAUNCH_SMEM(c, LGT_K_DSLASH, (dslash_tma_kernel<T, 0, 1>), pgrid, 128, smem, DSLASH_PARGS);
+            } else {
+                LAUNCH_SMEM(c, LGT_K_DSLASH_R, (dslash_tma_kernel<T, 1, 2>), pgrid, 128, smem, DSLASH_PARGS);
+            }
+            return LGT_OK;
+        }
+#undef DSLASH_PARGS
+        if (c->variant[LGT_K_DSLASH] == 3 && tile_ok(c)) {  // 2 x 2 x 2 tiles of 32-site layout blocks per 256-thread block
+            const int tgrid = c->g.V / 256;
+#define DSLASH_TARGS c->g, (const T2*)U, (const T2*)in, (T2*)out, kappa, c->st, c->partials, (T2*)r
+            if (mode == 0) {
+                if (dagger)
+                    LAUNCH(c, LGT_K_DSLASH, (dslash_tile_kernel<T, 1, 0>), tgrid, 256, DSLASH_TARGS);
+                else
+                    LAUNCH(c, LGT_K_DSLASH, (dslash_tile_kernel<T, 0, 0>), tgrid, 256, DSLASH_TARGS);
+            } else if (mode == 1) {
+                LAUNCH(c, LGT_K_DSLASH, (dslash_tile_kernel<T, 0, 1>), tgrid, 256, DSLASH_TARGS);
+            } else {
+                LAUNCH(c, LGT_K_DSLASH_R, (dslash_tile_kernel<T, 1, 2>), tgrid, 256, DSLASH_TARGS);
+            }
+#undef DSLASH_TARGS
+            return LGT_OK;
+        }
+        if (c->variant[LGT_K_DSLASH] == 4) {  // variant 0 with an L2 prefetch for the block that will take this block's place
+            const int pf = 2 * c->num_sms;
+            if (mode == 0) {
+                if (dagger)
+                    LAUNCH(c, LGT_K_DSLASH, (dslash_kernel<T, 1, 0, 0, 1>), grid, 128, DSLASH_ARGS, pf);
+                else
+                    LAUNCH(c, LGT_K_DSLASH, (dslash_kernel<T, 0, 0, 0, 1>), grid, 128, DSLASH_ARGS, pf);
+            } else if (mode == 1) {
+                LAUNCH(c, LGT_K_DSLASH, (dslash_kernel<T, 0, 1, 0, 1>), grid, 128, DSLASH_ARGS, pf);
+            } else {
+                LAUNCH(c, LGT_K_DSLASH_R, (dslash_kernel<T, 1, 2, 0, 1>), grid, 128, DSLASH_ARGS, pf);
+            }
+            return LGT_OK;
+        }
+        if (c->variant[LGT_K_DSLASH] == 5) {  // variant 0 with the z and t neighbours loaded past L1
+            if (mode == 0) {
+                if (dagger)
+                    LAUNCH(c, LGT_K_DSLASH, (dslash_kernel<T, 1, 0, 0, 2>), grid, 128, DSLASH_ARGS, 0);
+                else
+                    LAUNCH(c, LGT_K_DSLASH, (dslash_kernel<T, 0, 0, 0, 2>), grid, 128, DSLASH_ARGS, 0);
+            } else if (mode == 1) {
+                LAUNCH(c, LGT_K_DSLASH, (dslash_kernel<T, 0, 1, 0, 2>), grid, 128, DSLASH_ARGS, 0);
+            } else {
+                LAUNCH(c, LGT_K_DSLASH_R, (dslash_kernel<T, 1, 2, 0, 2>), grid, 128, DSLASH_ARGS, 0);
+            }
+            return LGT_OK;
+        }
         if (mode == 0) {
             if (dagger)
                 LAUNCH(c, LGT_K_DSLASH, (dslash_kernel<T, 1, 0>), grid, 128, DSLASH_ARGS);
@@ -318,7 +429,7 @@ template <class T> struct Ops {
         T2 *r = (T2*)wr, *p = (T2*)wp, *t = (T2*)wt;
         const size_t n = (size_t)12 * c->g.Vs;
         const int nb = stream_blocks(c, n);
-        const int ngrid = site_blocks(c, 128);  // blocks (= partials) of the stencil kernels
+        const int ngrid = dslash_partials(c);  // blocks (= partials) of the stencil kernels
         LAUNCH(c, LGT_K_CG_BLAS, (cg_init_kernel<T>), nb, 256, n, (const T2*)b, (T2*)x, r, p, c->st, tol * tol, max_iter, c->partials, c->counter);
         int rc;
         int launched = 0;
@@ -429,6 +540,20 @@ template <class T> struct Ops {
     }
     static int gauge_force(lgt_ctx* c, void* P, int acc, double eps) {
         const int grid = site_blocks(c, 32);
+        const int v = c->variant[LGT_K_GAUGE_FORCE];
+        if (v == 1 || v == 2) {  // 2 / 4 layout blocks per thread block
+            const int rows = 2 * v, g4 = site_blocks(c, 128) * (4 / rows);
+#define GF_ARGS c->g, (const T2*)c->U, (T2*)P, (T)(c->beta / 6.0), (T)eps
+            if (v == 1) {
+                if (acc) LAUNCH(c, LGT_K_GAUGE_FORCE, (gauge_force_kernel<T, 1, 2>), g4, 256, GF_ARGS);
+                else LAUNCH(c, LGT_K_GAUGE_FORCE, (gauge_force_kernel<T, 0, 2>), g4, 256, GF_ARGS);
+            } else {
+                if (acc) LAUNCH(c, LGT_K_GAUGE_FORCE, (gauge_force_kernel<T, 1, 4>), g4, 512, GF_ARGS);
+                else LAUNCH(c, LGT_K_GAUGE_FORCE, (gauge_force_kernel<T, 0, 4>), g4, 512, GF_ARGS);
+            }
+#undef GF_ARGS
+            return LGT_OK;
+        }
         if (acc)
             LAUNCH(c, LGT_K_GAUGE_FORCE, (gauge_force_kernel<T, 1>), grid, 128, c->g, (const T2*)c->U, (T2*)P, (T)(c->beta / 6.0), (T)eps);
         else
@@ -1002,6 +1127,7 @@ int lgt_create(lgt_ctx** out, const int dims[4], double beta, double kappa, cons
     int sms = 148;
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device);
     c->red_blocks = sms * 8;
+    c->num_sms = sms;
     int rc = LGT_OK;
     auto alloc = [&](void** p, size_t bytes) {
         if (rc != LGT_OK) return;
@@ -1122,6 +1248,22 @@ int lgt_set_block_swizzle(lgt_ctx* c, int z_planes, int* in_effect) {
         c->g.swz_Z = z_planes;
     }
     if (in_effect) *in_effect = c->g.swz_Z;
+    return LGT_OK;
+}
+int lgt_set_kernel_variant(lgt_ctx* c, int kernel_class, int variant, int* in_effect) {
+    CHECK_CTX(c);
+    if (kernel_class < 0 || kernel_class >= LGT_K_COUNT) return fail(c, LGT_EINVAL, "lgt_set_kernel_variant: unknown kernel class");
+    if (variant >= 0) {
+        const int nvar = (kernel_class == LGT_K_DSLASH) ? 6 : (kernel_class == LGT_K_GAUGE_FORCE) ? 3 : 1;
+        if (variant >= nvar) return fail(c, LGT_EINVAL, "lgt_set_kernel_variant: this kernel class has no such variant");
+        if (c->variant[kernel_class] != variant) {
+            // captured CG chunks hold the old kernels
+            for (lgt_ctx::ChunkGraph& g : c->graphs) cudaGraphExecDestroy(g.exec);
+            c->graphs.clear();
+        }
+        c->variant[kernel_class] = variant;
+    }
+    if (in_effect) *in_effect = c->variant[kernel_class];
     return LGT_OK;
 }
 void* lgt_stream(const lgt_ctx* c) { return c ? (void*)c->stream : nullptr; }

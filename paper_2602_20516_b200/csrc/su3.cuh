@@ -60,6 +60,17 @@ template <class T> __device__ __forceinline__ cx<T> ldc(const typename Vec2<T>::
     typename Vec2<T>::type v = __ldg(p);
     return mk<T>(v.x, v.y);
 }
+// the same without allocating the line in L1 (data no other thread of the block will ask for)
+__device__ __forceinline__ cx<double> ldc_na(const double2* p) {
+    cx<double> r;
+    asm("ld.global.nc.L1::no_allocate.v2.f64 {%0, %1}, [%2];" : "=d"(r.re), "=d"(r.im) : "l"(p));
+    return r;
+}
+__device__ __forceinline__ cx<float> ldc_na(const float2* p) {
+    cx<float> r;
+    asm("ld.global.nc.L1::no_allocate.v2.f32 {%0, %1}, [%2];" : "=f"(r.re), "=f"(r.im) : "l"(p));
+    return r;
+}
 template <class T> __device__ __forceinline__ cx<T> ldc_rw(const typename Vec2<T>::type* p) {
     typename Vec2<T>::type v = *p;
     return mk<T>(v.x, v.y);

@@ -60,6 +60,7 @@ SYMBOLS = {
     "lgt_launch_count": (_l, [_vp]),
     "lgt_stream": (_vp, [_vp]),
     "lgt_set_block_swizzle": (_i, [_vp, _i, _ip]),
+    "lgt_set_kernel_variant": (_i, [_vp, _i, _i, _ip]),
     "lgt_cg_mixed": (_i, [_vp, _vp, _vp, _d, _i, _d, _ip, _ip, _dp]),
     "lgt_set_solver": (_i, [_vp, _i, _d]),
     "lgt_eo_mhat": (_i, [_vp, _vp, _vp, _i]),
@@ -400,6 +401,13 @@ def lgt_set_block_swizzle(ctx, z_planes=-1):
     Returns the value in effect."""
     out = C.c_int(0)
     _check(ctx, lib().lgt_set_block_swizzle(ctx, int(z_planes), C.byref(out)))
+    return out.value
+
+
+def lgt_set_kernel_variant(ctx, kernel_class, variant=-1):
+    """Implementation variant of one kernel class (variant < 0 only queries).  Returns the value in effect."""
+    out = C.c_int(0)
+    _check(ctx, lib().lgt_set_kernel_variant(ctx, int(kernel_class), int(variant), C.byref(out)))
     return out.value
 
 

@@ -86,6 +86,38 @@ def test_dslash_block_swizzle(lgt, dims, zs):
     lat.close()
 
 
+@pytest.mark.parametrize("dims", [(8, 8, 8, 8), (12, 10, 6, 8), (16, 16, 8, 4), (32, 4, 6, 3), (4, 3, 5, 6)])
+def test_dslash_kernel_variants(lgt, dims):
+    """Every implementation variant of the Dslash kernels kept in the library (lgt_set_kernel_variant; measured against
+    each other in profiles/r02a_dslash_variants.md) applies the same operator: D and D^dag bitwise equal to variant 0
+    (same per-site arithmetic in the same order) and equal to the oracle, a CG solve with the oracle's iteration count.
+    Shapes the tiled variant cannot take (odd Lz / Lt, xy planes that are no multiple of 64 sites) fall back to variant 0."""
+    U = synth.warm_links(dims, 0.3, 27)
+    psi = synth.gaussian_spinor(dims, 28)
+    lat = lgt.Lattice(dims, 5.6, 0.12, BC)
+    lat.set_links(U)
+    assert lgt.lgt_set_kernel_variant(lat.ctx, lgt.LGT_K_DSLASH) == 0
+    base = [lat.dslash(psi, dagger=d) for d in (False, True)]
+    for d in (False, True):
+        assert site_rel_err(base[d], oracle.dslash(dims, 0.12, BC, U, psi, dagger=d)) < TOL64
+    x0, it0, _, ok0 = lat.cg(psi, 1e-10, 2000)
+    _, it_ref, _, ok_ref = oracle.cg(dims, 0.12, BC, U, psi, 1e-10, 2000)
+    assert ok0 and ok_ref and it0 == it_ref
+    for v in (1, 2, 3, 4, 5):
+        assert lgt.lgt_set_kernel_variant(lat.ctx, lgt.LGT_K_DSLASH, v) == v
+        for d in (False, True):
+            assert np.array_equal(lat.dslash(psi, dagger=d), base[d]), (v, d)
+        x, it, _, ok = lat.cg(psi, 1e-10, 2000)
+        assert ok and it == it0, (v, it, it0)
+        assert np.abs(x - x0).max() <= 1e-13 * np.abs(x0).max()  # variant 3 sums other block partials
+    with pytest.raises(lgt.LgtError):
+        lgt.lgt_set_kernel_variant(lat.ctx, lgt.LGT_K_DSLASH, 6)
+    with pytest.raises(lgt.LgtError):
+        lgt.lgt_set_kernel_variant(lat.ctx, 99, 0)
+    assert lgt.lgt_set_kernel_variant(lat.ctx, lgt.LGT_K_DSLASH, 0) == 0
+    lat.close()
+
+
 @pytest.mark.parametrize("dims", [(4, 3, 5, 6), (16, 16, 16, 16)])
 def test_dslash_fp32(lgt, dims):
     U = round32(synth.warm_links(dims, 0.3, 7))
