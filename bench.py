@@ -76,7 +76,9 @@ VARIANT_NAMES = {
                "persistent, forward links by bulk copy (TMA) into per-warp shared-memory slots one chunk ahead",
                "256-thread blocks on 2 x 2 x 2 tiles of 32-site layout blocks",
                "variant 0 + L2 prefetch for the block 2 x SMs further on",
-               "variant 0 with the z and t neighbours loaded past L1 (no_allocate)"],
+               "variant 0 with the z and t neighbours loaded past L1 (no_allocate)",
+               "variant 0 with the DRAM-bound hops first (t+, z+, y+, x+, then the backward ones)",
+               "12-real links: rows 0, 1 read, row 2 rebuilt in registers (768 B per site)"],
     "gauge_force": ["one 32-site layout block x 4 directions per 128-thread block (default)",
                     "two layout blocks per 256-thread block",
                     "four layout blocks per 512-thread block (128 registers)"],

@@ -337,7 +337,7 @@ void* lgt_stream(const lgt_ctx* ctx);
 int lgt_set_block_swizzle(lgt_ctx* ctx, int z_planes, int* in_effect);
 /* Implementation variant of one kernel class (LGT_K_*); every variant computes the same operation and
  * the alternatives stay in the library so that each measurement in profiles/ can be repeated.
- *   LGT_K_DSLASH (covers LGT_K_DSLASH_R; D and D^dag bitwise the same in every variant):
+ *   LGT_K_DSLASH (covers LGT_K_DSLASH_R; D and D^dag bitwise the same in variants 0-5):
  *     0 = one 128-site block per chunk (dslash_kernel; the default and, measured, the fastest);
  *     1 = persistent software-pipelined kernel: one wave of blocks loops over the chunks with the next chunk's first
  *         loads in flight during the current chunk's last hops;
@@ -346,7 +346,18 @@ int lgt_set_block_swizzle(lgt_ctx* ctx, int z_planes, int* in_effect);
  *     3 = 256-thread blocks on 2 x 2 x 2 tiles of 32-site layout blocks (needs Lx*Ly % 64 == 0, even Lz and Lt,
  *         an undivided lattice; other shapes run variant 0; CG sums differ from variant 0 in rounding);
  *     4 = variant 0 plus an L2 prefetch of the forward links and t+1 spinors of the block 2 x SMs further on;
- *     5 = variant 0 with the z and t neighbours loaded past L1 (ld.global.nc.L1::no_allocate).
+ *     5 = variant 0 with the z and t neighbours loaded past L1 (ld.global.nc.L1::no_allocate);
+ *     6 = variant 0 with the hops reordered so that those whose operands come from DRAM go first (t+, z+, y+, x+, then
+ *         the backward ones); the eight contributions are summed in another order, so results agree to rounding only;
+ *     7 = 12-real links: rows 0 and 1 of every link are read and row 2 = sign * conj(row0 x row1) is
+ *         rebuilt in registers (768 instead of 960 compulsory bytes per site).  Exact for special unitary links; links
+ *         that have drifted from unitarity by delta change the operator by O(delta).
+ *   LGT_K_GAUGE_FORCE: 0 = one 32-site layout block x 4 directions per 128-thread block (default, fastest);
+ *     1 / 2 = two / four layout blocks per 256- / 512-thread block (more sharing through L1; measured slower).  Same sums bit for bit.
+ *   LGT_K_CG_BLAS: 0 = the CG scalar updates (alpha; beta, count, stop test) as one-block kernels between the stencil
+ *     kernels (default); 1 = fused into the stencil kernels: the block that finishes last forms the same fixed-order sum
+ *     and applies the update (two launches fewer per iteration, bitwise the same iterates; measured slower: the fence
+ *     and ticket at the end of every block cost more than the two short launches).
  * variant < 0 only queries.  The value in effect is returned through *in_effect (may be NULL).
  * LGT_EINVAL for an unknown class or variant. */
 int lgt_set_kernel_variant(lgt_ctx* ctx, int kernel_class, int variant, int* in_effect);

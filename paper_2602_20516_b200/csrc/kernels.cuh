@@ -101,6 +101,23 @@ template <class T, int NA = 0> __device__ __forceinline__ void load_link(const t
 #pragma unroll
     for (int k = 0; k < 9; k++) u[k] = NA ? ldc_na(b + k * W) : ldc<T>(b + k * W);
 }
+// 12-real link "compression": only rows 0 and 1 are read, row 2 = sign * conj(row0 x row1) for a special
+// unitary matrix; sign = the fermion boundary sign folded into the native link (det(-U) = -1).  Reads 2/3 of the link
+// bytes from the same 9-component layout (the three rows of row 2 are simply not touched).
+template <class T> __device__ __forceinline__ void load_link12(const typename Vec2<T>::type* U, int mu, int s, T sign, cx<T> u[9]) {
+    const typename Vec2<T>::type* b = link_at(U, s, mu);
+#pragma unroll
+    for (int k = 0; k < 6; k++) u[k] = ldc<T>(b + k * W);
+    u[6] = sign * conj(u[1] * u[5] - u[2] * u[4]);
+    u[7] = sign * conj(u[2] * u[3] - u[0] * u[5]);
+    u[8] = sign * conj(u[0] * u[4] - u[1] * u[3]);
+}
+// the boundary sign of link (site with coordinate x_mu = xmu, direction mu) as folded into the native layout
+__device__ __forceinline__ int folded_sign(const Geom& g, int mu, int xmu) {
+    if (g.bc[mu] > 0) return 1;
+    if (mu == 3) return ((xmu + g.t_off + g.Lt_glob) % g.Lt_glob == g.Lt_glob - 1) ? -1 : 1;
+    return (xmu == g.L[mu] - 1) ? -1 : 1;
+}
 template <class T, int NA = 0> __device__ __forceinline__ void load_spinor(const typename Vec2<T>::type* f, int s, cx<T> p[12]) {
     const typename Vec2<T>::type* b = spinor_at(f, s);
 #pragma unroll
@@ -184,6 +201,79 @@ __device__ __forceinline__ void block_partial(double v, double* partials) {
     }
 }
 
+// The sum of n block partials in ONE fixed order whatever the number of threads NT (a divisor of 1024, multiple of 32)
+// that forms it: 1024 virtual lanes, lane v adds partials[v + 1024 j + 16384 k] into sixteen accumulators j, folds them
+// pairwise (8, 4, 2, 1), the 32 lanes of a virtual warp fold by the shuffle tree, and one warp folds the 32 warp sums.
+// Thread t of NT stands for the virtual lanes t, t + NT, ...; since NT is a multiple of 32 each virtual warp lives in one
+// real warp with the same lane numbering.  Result valid in thread 0.  All NT threads of the block must call it.
+template <int NT> __device__ __forceinline__ double cg_fixed_sum(int n, const double* __restrict__ partials, double* warp_sums32) {
+    constexpr int Q = 1024 / NT;
+    const int lane = threadIdx.x & 31;
+#pragma unroll 1
+    for (int q = 0; q < Q; q++) {
+        const int v = threadIdx.x + NT * q;
+        double a16[16];
+#pragma unroll
+        for (int j = 0; j < 16; j++) a16[j] = 0.0;
+        for (int base = v; base < n; base += 16 * 1024) {
+#pragma unroll
+            for (int j = 0; j < 16; j++) {
+                const int i = base + j * 1024;
+                if (i < n) a16[j] += __ldcg(partials + i);
+            }
+        }
+#pragma unroll
+        for (int w = 8; w > 0; w >>= 1)
+#pragma unroll
+            for (int j = 0; j < w; j++) a16[j] += a16[j + w];
+        double x = a16[0];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) x += __shfl_down_sync(0xffffffffu, x, o);
+        if (lane == 0) warp_sums32[v >> 5] = x;
+    }
+    __syncthreads();
+    double sum = 0.0;
+    if (threadIdx.x < 32) {
+        sum = warp_sums32[lane];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) sum += __shfl_down_sync(0xffffffffu, sum, o);
+    }
+    return sum;
+}
+// The CG scalar updates (one thread).  WHAT 1 (after t = D p): pAp, alpha; WHAT 2 (after r -= alpha q): beta, rr, count, stop test
+template <int WHAT> __device__ __forceinline__ void cg_scalars_apply(CgState* st, double sum) {
+    if (WHAT == 1) {
+        st->pAp = sum;
+        st->alpha = st->rr / sum;
+    } else {
+        st->beta = sum / st->rr;
+        st->rr = sum;
+        st->iter += 1;
+        st->fresh = 1;
+        st->done = (!(sum > st->tol2 * st->bb) || st->iter >= st->max_iter) ? 1 : 0;
+    }
+}
+// Tail of a stencil kernel of the CG loop when the scalar update is FUSED into it (variant 1 of LGT_K_CG_BLAS): the block
+// that finishes last (ticket counter) forms the same fixed-order sum as cg_scalars_kernel and applies the same update --
+// bitwise the same scalars, two launches fewer per iteration.  Called by all 128 threads after block_partial.
+template <int WHAT> __device__ __forceinline__ void cg_fused_tail(CgState* st, const double* partials, unsigned* counter) {
+    __shared__ double tail_sums[32];
+    __shared__ bool tail_last;
+    if (threadIdx.x == 0) {
+        __threadfence();
+        tail_last = (atomicAdd(counter, 1u) == gridDim.x - 1);
+    }
+    __syncthreads();
+    if (!tail_last) return;
+    __threadfence();
+    const double sum = cg_fixed_sum<128>((int)gridDim.x, partials, tail_sums);
+    if (threadIdx.x == 0) {
+        *counter = 0u;
+        if (WHAT == 1) st->fresh = 0;
+        cg_scalars_apply<WHAT>(st, sum);
+    }
+}
+
 // One block of 1024 threads: sum of n block partials in a fixed order, then the CG scalar update.
 //   WHAT 1 (after t = D p):        pAp = sum, alpha = rr / pAp
 //   WHAT 2 (after r -= alpha q):   beta = sum / rr, rr = sum, iteration count, convergence flag
@@ -194,43 +284,8 @@ __global__ void __launch_bounds__(1024) cg_scalars_kernel(int n, const double* _
     if (WHAT == 1 && threadIdx.x == 0) st->fresh = 0;  // every block of the previous x, p update has read it: kernels are ordered
     if (done) return;
     __shared__ double warp_sums[32];
-    double a16[16];
-#pragma unroll
-    for (int j = 0; j < 16; j++) a16[j] = 0.0;
-    for (int base = threadIdx.x; base < n; base += 16 * 1024) {
-#pragma unroll
-        for (int j = 0; j < 16; j++) {
-            const int i = base + j * 1024;
-            if (i < n) a16[j] += __ldcg(partials + i);
-        }
-    }
-#pragma unroll
-    for (int w = 8; w > 0; w >>= 1)
-#pragma unroll
-        for (int j = 0; j < w; j++) a16[j] += a16[j + w];
-    double v = a16[0];
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
-    if (lane == 0) warp_sums[warp] = v;
-    __syncthreads();
-    if (warp == 0) {
-        double sum = warp_sums[lane];
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) sum += __shfl_down_sync(0xffffffffu, sum, o);
-        if (lane == 0) {
-            if (WHAT == 1) {
-                st->pAp = sum;
-                st->alpha = st->rr / sum;
-            } else {
-                st->beta = sum / st->rr;
-                st->rr = sum;
-                st->iter += 1;
-                st->fresh = 1;
-                st->done = (!(sum > st->tol2 * st->bb) || st->iter >= st->max_iter) ? 1 : 0;
-            }
-        }
-    }
+    const double sum = cg_fixed_sum<1024>(n, partials, warp_sums);
+    if (threadIdx.x == 0) cg_scalars_apply<WHAT>(st, sum);
 }
 
 // Decomposed lattice (lgt_dd_*): the CG scalar updates in two phases around an all-reduce over the ranks.
@@ -312,8 +367,9 @@ __device__ __forceinline__ void hop_fwd(const Geom& g, const typename Vec2<T>::t
                                         const Site& c, int s, cx<T> acc[12]) {
     const int sn = nbr_fwd(g, c, s, MU);
     cx<T> p[12], h[6], u[9], w[6];
-    load_spinor<T, NA>(in, sn, p);
-    load_link<T, NA>(U, MU, s, u);
+    load_spinor<T, NA == 1>(in, sn, p);
+    if (NA == 2) load_link12<T>(U, MU, s, (T)folded_sign(g, MU, c.x[MU]), u);
+    else load_link<T, NA == 1>(U, MU, s, u);
     spin_project<MU, SG>(p, h);
     su3_mul_half(u, h, w);
     spin_reconstruct_add<MU, SG>(w, acc);
@@ -324,8 +380,9 @@ __device__ __forceinline__ void hop_bwd(const Geom& g, const typename Vec2<T>::t
                                         const Site& c, int s, cx<T> acc[12]) {
     const int sn = nbr_bwd(g, c, s, MU);
     cx<T> p[12], h[6], u[9], w[6];
-    load_spinor<T, NA>(in, sn, p);
-    load_link<T, NA>(U, MU, sn, u);
+    load_spinor<T, NA == 1>(in, sn, p);
+    if (NA == 2) load_link12<T>(U, MU, sn, (T)folded_sign(g, MU, c.x[MU] == 0 ? g.L[MU] - 1 : c.x[MU] - 1), u);
+    else load_link<T, NA == 1>(U, MU, sn, u);
     spin_project<MU, SG>(p, h);
     su3_dag_mul_half(u, h, w);
     spin_reconstruct_add<MU, SG>(w, acc);
@@ -360,8 +417,10 @@ __global__ void __launch_bounds__(128, 1) dslash_kernel(Geom g, const typename V
                                                         const typename Vec2<T>::type* __restrict__ in,
                                                         typename Vec2<T>::type* __restrict__ out, T kappa, CgState* st,
                                                         double* partials, typename Vec2<T>::type* __restrict__ r, PushTo<T> push,
-                                                        int pf = 0) {
+                                                        int pf = 0, unsigned* fuse = nullptr) {
     const int done = (MODE != 0) ? st->done : 0;
+    // fused scalar update, launches past convergence: the "x, p update due" flag is cleared here instead of by cg_scalars_kernel<1>
+    if (MODE == 1 && fuse && done && blockIdx.x == 0 && threadIdx.x == 0) st->fresh = 0;
     const int s = g.s_begin + swizzled_chunk(g, blockIdx.x) * blockDim.x + threadIdx.x;
     if (PFON == 1 && blockIdx.x + pf < gridDim.x && !(MODE != 0 && done)) {
         const int sp = g.s_begin + swizzled_chunk(g, blockIdx.x + pf) * blockDim.x + threadIdx.x;
@@ -397,6 +456,30 @@ __global__ void __launch_bounds__(128, 1) dslash_kernel(Geom g, const typename V
         for (int k = 0; k < 12; k++) acc[k] = mk<T>(0, 0);
         constexpr int F = DAG ? +1 : -1;  // D: (1 - gamma) forward, (1 + gamma) backward; D^dag: swapped
         constexpr int NA = (PFON == 2) ? 1 : 0;  // variant 5: z and t neighbours (no reuse inside the block) bypass L1
+        if (PFON == 3) {
+            // variant 6: the hops whose operands come from DRAM first -- the forward links are first touched here, and
+            // so are the t+1 spinors -- so that the block's DRAM requests all leave in its first batch of loads
+            hop_fwd<3, F, T>(g, U, in, c, s, acc);
+            if (MODE != 0 && done) return;  // uniform over the grid
+            hop_fwd<2, F, T>(g, U, in, c, s, acc);
+            hop_fwd<1, F, T>(g, U, in, c, s, acc);
+            hop_fwd<0, F, T>(g, U, in, c, s, acc);
+            hop_bwd<0, -F, T>(g, U, in, c, s, acc);
+            hop_bwd<1, -F, T>(g, U, in, c, s, acc);
+            hop_bwd<2, -F, T>(g, U, in, c, s, acc);
+            hop_bwd<3, -F, T>(g, U, in, c, s, acc);
+        } else if (PFON == 4) {
+            // variant 7: 12-real links, third row rebuilt in registers
+            hop_fwd<0, F, T, 2>(g, U, in, c, s, acc);
+            if (MODE != 0 && done) return;  // uniform over the grid
+            hop_bwd<0, -F, T, 2>(g, U, in, c, s, acc);
+            hop_fwd<1, F, T, 2>(g, U, in, c, s, acc);
+            hop_bwd<1, -F, T, 2>(g, U, in, c, s, acc);
+            hop_fwd<2, F, T, 2>(g, U, in, c, s, acc);
+            hop_bwd<2, -F, T, 2>(g, U, in, c, s, acc);
+            hop_fwd<3, F, T, 2>(g, U, in, c, s, acc);
+            hop_bwd<3, -F, T, 2>(g, U, in, c, s, acc);
+        } else {
         hop_fwd<0, F, T>(g, U, in, c, s, acc);
         if (MODE != 0 && done) return;  // uniform over the grid
         hop_bwd<0, -F, T>(g, U, in, c, s, acc);
@@ -406,6 +489,7 @@ __global__ void __launch_bounds__(128, 1) dslash_kernel(Geom g, const typename V
         hop_bwd<2, -F, T, NA>(g, U, in, c, s, acc);
         hop_fwd<3, F, T, NA>(g, U, in, c, s, acc);
         hop_bwd<3, -F, T, NA>(g, U, in, c, s, acc);
+        }
         const typename Vec2<T>::type* bi = spinor_at(in, s);
         if (MODE == 2) {
             const T alpha = (T)st->alpha;
@@ -442,7 +526,10 @@ __global__ void __launch_bounds__(128, 1) dslash_kernel(Geom g, const typename V
             for (int k = 0; k < 12; k++) stc<T>(bo + k * W, mk<T>(0, 0));
         }
     }
-    if (MODE != 0) block_partial(nrm, partials);
+    if (MODE != 0) {
+        block_partial(nrm, partials);
+        if (fuse) cg_fused_tail<MODE>(st, partials, fuse);
+    }
 }
 
 // The same operator as a PERSISTENT, software-pipelined kernel (variant 1 of lgt_set_kernel_variant(LGT_K_DSLASH)).
@@ -1509,8 +1596,10 @@ __global__ void __launch_bounds__(128, 1) hop_cb_kernel(Geom g, int p, const typ
                                                         const typename Vec2<T>::type* __restrict__ in,
                                                         const typename Vec2<T>::type* __restrict__ self,
                                                         typename Vec2<T>::type* __restrict__ out, T kap, CgState* st,
-                                                        double* partials, typename Vec2<T>::type* __restrict__ r, PushTo<T> push) {
+                                                        double* partials, typename Vec2<T>::type* __restrict__ r, PushTo<T> push,
+                                                        unsigned* fuse = nullptr) {
     const int done = (MODE != 0) ? st->done : 0;
+    if (MODE == 1 && fuse && done && blockIdx.x == 0 && threadIdx.x == 0) st->fresh = 0;  // as in dslash_kernel
     const int c = g.h_begin + blockIdx.x * blockDim.x + threadIdx.x;
     double nrm = 0.0;
     if (c < g.h_end) {
@@ -1571,7 +1660,10 @@ __global__ void __launch_bounds__(128, 1) hop_cb_kernel(Geom g, int p, const typ
             for (int k = 0; k < 12; k++) stc<T>(bo + k * W, mk<T>(0, 0));
         }
     }
-    if (MODE == 1 || MODE == 2) block_partial(nrm, partials);
+    if (MODE == 1 || MODE == 2) {
+        block_partial(nrm, partials);
+        if (fuse) cg_fused_tail<MODE>(st, partials, fuse);
+    }
 }
 
 // full field (lexicographic blocked layout) <-> two half fields.  DIR 0: split, DIR 1: merge.  NCOMP 12 or 36.

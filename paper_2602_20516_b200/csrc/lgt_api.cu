@@ -209,6 +209,15 @@ int ensure_force_buf(lgt_ctx* c) {
     return LGT_OK;
 }
 
+// every copy derived from the links (fp32, checkerboard, smeared, the slabs' ghost slices) is stale after a link change
+inline void invalidate_link_copies(lgt_ctx* c) {
+    c->u32_valid = false;
+    c->usm_valid = false;
+    if (c->dd_links_valid) *c->dd_links_valid = false;
+    c->ucb_valid = false;
+    c->ucb32_valid = false;
+}
+
 int eo_cg_mixed(lgt_ctx* c, void* b, void* x, void* r, void* q, void* u, void* t_o, double tol, int max_iter, int* iters);
 
 // One chunk of CG iterations as a CUDA graph: the kernels of a chunk have no argument that changes from chunk to chunk
@@ -314,6 +323,13 @@ template <class T> struct Ops {
     static int dslash_partials(const lgt_ctx* c) {
         return (c->variant[LGT_K_DSLASH] == 3 && tile_ok(c)) ? c->g.V / 256 : site_blocks(c, 128);
     }
+    // Variant 1 of LGT_K_CG_BLAS: the scalar updates of the CG loop ride in the last block of the stencil kernels
+    // (cg_fused_tail) instead of two one-block launches per iteration.  Only the one-block-per-chunk kernels have the
+    // tail, and the slabs of a decomposed lattice split their sums around an all-reduce.
+    static unsigned* fuse_counter(const lgt_ctx* c) {
+        const int dv = c->variant[LGT_K_DSLASH];
+        return (c->variant[LGT_K_CG_BLAS] == 1 && !c->dd_links_valid && dv != 1 && dv != 2 && dv != 3) ? c->counter : nullptr;
+    }
     // mode 0: out = D in / D^dag in; 1: CG "t = D p" (+ pAp, alpha); 2: CG "q = D^dag t" fused with the x, r update
     static int dslash(lgt_ctx* c, const void* U, const void* in, void* out, int dagger, int mode, void* r = nullptr,
                       const PushTo<T>* push = nullptr) {
@@ -387,9 +403,35 @@ template <class T> struct Ops {
                 else
                     LAUNCH(c, LGT_K_DSLASH, (dslash_kernel<T, 0, 0, 0, 1>), grid, 128, DSLASH_ARGS, pf);
             } else if (mode == 1) {
-                LAUNCH(c, LGT_K_DSLASH, (dslash_kernel<T, 0, 1, 0, 1>), grid, 128, DSLASH_ARGS, pf);
+                LAUNCH(c, LGT_K_DSLASH, (dslash_kernel<T, 0, 1, 0, 1>), grid, 128, DSLASH_ARGS, pf, fuse_counter(c));
             } else {
-                LAUNCH(c, LGT_K_DSLASH_R, (dslash_kernel<T, 1, 2, 0, 1>), grid, 128, DSLASH_ARGS, pf);
+                LAUNCH(c, LGT_K_DSLASH_R, (dslash_kernel<T, 1, 2, 0, 1>), grid, 128, DSLASH_ARGS, pf, fuse_counter(c));
+            }
+            return LGT_OK;
+        }
+        if (c->variant[LGT_K_DSLASH] == 7) {  // 12-real links: rows 0 and 1 read, row 2 rebuilt in registers
+            if (mode == 0) {
+                if (dagger)
+                    LAUNCH(c, LGT_K_DSLASH, (dslash_kernel<T, 1, 0, 0, 4>), grid, 128, DSLASH_ARGS, 0);
+                else
+                    LAUNCH(c, LGT_K_DSLASH, (dslash_kernel<T, 0, 0, 0, 4>), grid, 128, DSLASH_ARGS, 0);
+            } else if (mode == 1) {
+                LAUNCH(c, LGT_K_DSLASH, (dslash_kernel<T, 0, 1, 0, 4>), grid, 128, DSLASH_ARGS, 0, fuse_counter(c));
+            } else {
+                LAUNCH(c, LGT_K_DSLASH_R, (dslash_kernel<T, 1, 2, 0, 4>), grid, 128, DSLASH_ARGS, 0, fuse_counter(c));
+            }
+            return LGT_OK;
+        }
+        if (c->variant[LGT_K_DSLASH] == 6) {  // variant 0 with the DRAM-bound hops (t+, z+, y+, x+) first
+            if (mode == 0) {
+                if (dagger)
+                    LAUNCH(c, LGT_K_DSLASH, (dslash_kernel<T, 1, 0, 0, 3>), grid, 128, DSLASH_ARGS, 0);
+                else
+                    LAUNCH(c, LGT_K_DSLASH, (dslash_kernel<T, 0, 0, 0, 3>), grid, 128, DSLASH_ARGS, 0);
+            } else if (mode == 1) {
+                LAUNCH(c, LGT_K_DSLASH, (dslash_kernel<T, 0, 1, 0, 3>), grid, 128, DSLASH_ARGS, 0, fuse_counter(c));
+            } else {
+                LAUNCH(c, LGT_K_DSLASH_R, (dslash_kernel<T, 1, 2, 0, 3>), grid, 128, DSLASH_ARGS, 0, fuse_counter(c));
             }
             return LGT_OK;
         }
@@ -400,9 +442,9 @@ template <class T> struct Ops {
                 else
                     LAUNCH(c, LGT_K_DSLASH, (dslash_kernel<T, 0, 0, 0, 2>), grid, 128, DSLASH_ARGS, 0);
             } else if (mode == 1) {
-                LAUNCH(c, LGT_K_DSLASH, (dslash_kernel<T, 0, 1, 0, 2>), grid, 128, DSLASH_ARGS, 0);
+                LAUNCH(c, LGT_K_DSLASH, (dslash_kernel<T, 0, 1, 0, 2>), grid, 128, DSLASH_ARGS, 0, fuse_counter(c));
             } else {
-                LAUNCH(c, LGT_K_DSLASH_R, (dslash_kernel<T, 1, 2, 0, 2>), grid, 128, DSLASH_ARGS, 0);
+                LAUNCH(c, LGT_K_DSLASH_R, (dslash_kernel<T, 1, 2, 0, 2>), grid, 128, DSLASH_ARGS, 0, fuse_counter(c));
             }
             return LGT_OK;
         }
@@ -412,9 +454,9 @@ template <class T> struct Ops {
             else
                 LAUNCH(c, LGT_K_DSLASH, (dslash_kernel<T, 0, 0>), grid, 128, DSLASH_ARGS);
         } else if (mode == 1) {
-            LAUNCH(c, LGT_K_DSLASH, (dslash_kernel<T, 0, 1>), grid, 128, DSLASH_ARGS);
+            LAUNCH(c, LGT_K_DSLASH, (dslash_kernel<T, 0, 1>), grid, 128, DSLASH_ARGS, 0, fuse_counter(c));
         } else {
-            LAUNCH(c, LGT_K_DSLASH_R, (dslash_kernel<T, 1, 2>), grid, 128, DSLASH_ARGS);
+            LAUNCH(c, LGT_K_DSLASH_R, (dslash_kernel<T, 1, 2>), grid, 128, DSLASH_ARGS, 0, fuse_counter(c));
         }
 #undef DSLASH_ARGS
         return LGT_OK;
@@ -430,6 +472,7 @@ template <class T> struct Ops {
         const size_t n = (size_t)12 * c->g.Vs;
         const int nb = stream_blocks(c, n);
         const int ngrid = dslash_partials(c);  // blocks (= partials) of the stencil kernels
+        const bool fused = fuse_counter(c) != nullptr;
         LAUNCH(c, LGT_K_CG_BLAS, (cg_init_kernel<T>), nb, 256, n, (const T2*)b, (T2*)x, r, p, c->st, tol * tol, max_iter, c->partials, c->counter);
         int rc;
         int launched = 0;
@@ -445,14 +488,14 @@ template <class T> struct Ops {
                 int r2;
                 for (int i = 0; i < chunk; i++) {
                     if ((r2 = dslash(c, U, p, t, 0, 1)) != LGT_OK) return r2;
-                    LAUNCH(c, LGT_K_CG_BLAS, (cg_scalars_kernel<1>), 1, 1024, ngrid, c->partials, c->st);
+                    if (!fused) LAUNCH(c, LGT_K_CG_BLAS, (cg_scalars_kernel<1>), 1, 1024, ngrid, c->partials, c->st);
                     if ((r2 = dslash(c, U, t, nullptr, 1, 2, r)) != LGT_OK) return r2;
-                    LAUNCH(c, LGT_K_CG_BLAS, (cg_scalars_kernel<2>), 1, 1024, ngrid, c->partials, c->st);
+                    if (!fused) LAUNCH(c, LGT_K_CG_BLAS, (cg_scalars_kernel<2>), 1, 1024, ngrid, c->partials, c->st);
                     LAUNCH(c, LGT_K_CG_UPDATE, (cg_update_xp_kernel<T>), nb, 256, n, (T2*)x, p, (const T2*)r, c->st);
                 }
                 return LGT_OK;
             };
-            const void* const key[7] = {U, x, r, p, t, nullptr, (const void*)sizeof(T)};
+            const void* const key[7] = {U, x, r, p, t, (const void*)(size_t)fused, (const void*)sizeof(T)};
             if ((rc = (chunk == 8 ? chunk_graph(c, 0, key, body) : body())) != LGT_OK) return rc;
             launched += chunk;
         }
@@ -669,9 +712,9 @@ template <class T> struct Ops {
             if (dagger) LAUNCH(c, LGT_K_DSLASH, (hop_cb_kernel<T, 1, 3>), grid, 128, HOP_ARGS);
             else LAUNCH(c, LGT_K_DSLASH, (hop_cb_kernel<T, 0, 3>), grid, 128, HOP_ARGS);
         } else if (mode == 1) {
-            LAUNCH(c, LGT_K_DSLASH, (hop_cb_kernel<T, 0, 1>), grid, 128, HOP_ARGS);
+            LAUNCH(c, LGT_K_DSLASH, (hop_cb_kernel<T, 0, 1>), grid, 128, HOP_ARGS, fuse_counter(c));
         } else {
-            LAUNCH(c, LGT_K_DSLASH_R, (hop_cb_kernel<T, 1, 2>), grid, 128, HOP_ARGS);
+            LAUNCH(c, LGT_K_DSLASH_R, (hop_cb_kernel<T, 1, 2>), grid, 128, HOP_ARGS, fuse_counter(c));
         }
 #undef HOP_ARGS
         return LGT_OK;
@@ -687,6 +730,7 @@ template <class T> struct Ops {
         const size_t n = (size_t)12 * c->g.Vhs;
         const int nb = stream_blocks(c, n);
         const int ngrid = (own_half_sites(c) + 127) / 128;
+        const bool fused = fuse_counter(c) != nullptr;
         LAUNCH(c, LGT_K_CG_BLAS, (cg_init_kernel<T>), nb, 256, n, b, x, r, p, c->st, tol * tol, max_iter, c->partials, c->counter);
         int rc, launched = 0;
         for (;;) {
@@ -701,15 +745,15 @@ template <class T> struct Ops {
                 for (int i = 0; i < chunk; i++) {
                     if ((r2 = hop(c, 1, p, nullptr, t, 0, 3, -c->kappa)) != LGT_OK) return r2;   // t_o = kappa H_oe p
                     if ((r2 = hop(c, 0, t, p, u, 0, 1, c->kappa)) != LGT_OK) return r2;          // u = M p, |u|^2
-                    LAUNCH(c, LGT_K_CG_BLAS, (cg_scalars_kernel<1>), 1, 1024, ngrid, c->partials, c->st);
+                    if (!fused) LAUNCH(c, LGT_K_CG_BLAS, (cg_scalars_kernel<1>), 1, 1024, ngrid, c->partials, c->st);
                     if ((r2 = hop(c, 1, u, nullptr, t, 1, 3, -c->kappa)) != LGT_OK) return r2;   // t_o = kappa H^dag_oe u
                     if ((r2 = hop(c, 0, t, u, nullptr, 1, 2, c->kappa, r)) != LGT_OK) return r2; // r -= alpha M^dag u
-                    LAUNCH(c, LGT_K_CG_BLAS, (cg_scalars_kernel<2>), 1, 1024, ngrid, c->partials, c->st);
+                    if (!fused) LAUNCH(c, LGT_K_CG_BLAS, (cg_scalars_kernel<2>), 1, 1024, ngrid, c->partials, c->st);
                     LAUNCH(c, LGT_K_CG_UPDATE, (cg_update_xp_kernel<T>), nb, 256, n, x, p, (const T2*)r, c->st);
                 }
                 return LGT_OK;
             };
-            const void* const key[7] = {links_cb(c, 0), x, r, p, u, t, (const void*)sizeof(T)};
+            const void* const key[7] = {links_cb(c, 0), x, r, p, u, t, (const void*)(sizeof(T) + 64 * (size_t)fused)};
             if ((rc = (chunk == 8 ? chunk_graph(c, 1, key, body) : body())) != LGT_OK) return rc;
             launched += chunk;
         }
@@ -951,6 +995,16 @@ int kick(lgt_ctx* c, double eps, double tol, int max_iter, int* cg_iters) {
 // MD trajectory of nsteps steps of size dt, adjacent kicks merged (include/lgt.h "lgt_set_integrator").  S supplies the
 // moves: kick(eps, &it) with both forces, kick_gauge(eps), kick_fermion(eps, &it), drift(eps) -- one handle, or all slabs
 // of a decomposed lattice in lockstep.
+// The gauge part of one Sexton-Weingarten step: m leapfrog steps of size h with the gauge force alone
+template <class S> int plain_inner_gauge_steps(S& s, double h, int m) {
+    int rc;
+    if ((rc = s.kick_gauge(0.5 * h)) != LGT_OK) return rc;
+    for (int i = 0; i < m; i++) {
+        if ((rc = s.drift(h)) != LGT_OK) return rc;
+        if ((rc = s.kick_gauge((i == m - 1) ? 0.5 * h : h)) != LGT_OK) return rc;
+    }
+    return LGT_OK;
+}
 template <class S> int integrate_with(S& s, int integrator, int n_inner, int nsteps, double dt, long* cg_iters) {
     int rc, it = 0, conv = LGT_OK;
     long total = 0;
@@ -982,11 +1036,7 @@ template <class S> int integrate_with(S& s, int integrator, int n_inner, int nst
         const double h = dt / m;
         STEP(s.kick_fermion(0.5 * dt, &it));
         for (int n = 0; n < nsteps; n++) {
-            STEP(s.kick_gauge(0.5 * h));
-            for (int i = 0; i < m; i++) {
-                STEP(s.drift(h));
-                STEP(s.kick_gauge((i == m - 1) ? 0.5 * h : h));
-            }
+            STEP(s.inner_gauge_steps(h, m));
             STEP(s.kick_fermion((n == nsteps - 1) ? 0.5 * dt : dt, &it));
         }
     }
@@ -1002,6 +1052,19 @@ struct HandleMoves {
     int kick_gauge(double eps) { return ::kick_gauge(c, eps); }
     int kick_fermion(double eps, int* it) { return ::kick_fermion(c, eps, tol, max_iter, it); }
     int drift(double eps) { return DISPATCH(c, link_update, c, eps); }
+    // The 2 m + 1 launches of the inner gauge loop have the same arguments in every outer step of a trajectory (and in
+    // every trajectory with the same dt and m), and on the paper's lattice sizes (6^4 - 16^4) each is a
+    // few microseconds of work: they are captured once as a CUDA graph and replayed with one launch, like the CG chunks.
+    int inner_gauge_steps(double h, int m) {
+        unsigned long long hbits;
+        memcpy(&hbits, &h, sizeof hbits);
+        const void* const key[7] = {c->U, c->P, (const void*)hbits, (const void*)(size_t)m,
+                                    (const void*)(size_t)c->variant[LGT_K_GAUGE_FORCE], nullptr, (const void*)c->esize};
+        HandleMoves& self = *this;
+        const int rc = chunk_graph(c, 2, key, [&]() -> int { return plain_inner_gauge_steps(self, h, m); });
+        invalidate_link_copies(c);  // the replayed link updates changed U behind the host-side flags
+        return rc;
+    }
 };
 int integrate(lgt_ctx* c, int nsteps, double dt, double tol, int max_iter, long* cg_iters) {
     HandleMoves m{c, tol, max_iter};
@@ -1254,7 +1317,7 @@ int lgt_set_kernel_variant(lgt_ctx* c, int kernel_class, int variant, int* in_ef
     CHECK_CTX(c);
     if (kernel_class < 0 || kernel_class >= LGT_K_COUNT) return fail(c, LGT_EINVAL, "lgt_set_kernel_variant: unknown kernel class");
     if (variant >= 0) {
-        const int nvar = (kernel_class == LGT_K_DSLASH) ? 6 : (kernel_class == LGT_K_GAUGE_FORCE) ? 3 : 1;
+        const int nvar = (kernel_class == LGT_K_DSLASH) ? 8 : (kernel_class == LGT_K_GAUGE_FORCE) ? 3 : (kernel_class == LGT_K_CG_BLAS) ? 2 : 1;
         if (variant >= nvar) return fail(c, LGT_EINVAL, "lgt_set_kernel_variant: this kernel class has no such variant");
         if (c->variant[kernel_class] != variant) {
             // captured CG chunks hold the old kernels

@@ -783,6 +783,7 @@ template <class T> struct DdOps {
         int kick_gauge(double eps) { return DdOps::kick_gauge(d, eps); }
         int kick_fermion(double eps, int* it) { return DdOps::kick_fermion(d, eps, tol, max_iter, it); }
         int drift(double eps) { return DdOps::drift(d, eps); }
+        int inner_gauge_steps(double h, int m) { return plain_inner_gauge_steps(*this, h, m); }  // exchanges in between: no graph
     };
     static int integrate(lgt_dd* d, int nsteps, double dt, double tol, int max_iter, long* cg_iters) {
         Moves m{d, tol, max_iter};

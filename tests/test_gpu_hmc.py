@@ -276,3 +276,30 @@ def test_heatbaths_full_size_sampled(lgt):
     n2 = lgt.lgt_pseudofermion_heatbath(lat.ctx, seed, traj)
     assert abs(n2 / (12 * V) - 1.0) < 5 / np.sqrt(12 * V)
     lat.close()
+
+
+def test_sexton_weingarten_inner_loop_graph_is_bitwise_the_plain_launches(lgt):
+    """The 2 m + 1 launches of the inner gauge loop of a Sexton-Weingarten step are replayed as one CUDA graph; with
+    per-kernel timing on they are plain launches.  Same kernels in the same order: links, momenta, CG counts and launch
+    counts must be identical, with fermions on the even/odd action (whose link copies the replay must invalidate) and
+    without, and a second trajectory must reuse the graph."""
+    dims = (8, 8, 8, 4)
+    U = synth.warm_links(dims, 0.3, 91)
+    P = synth.gaussian_momenta(dims, 92)
+    for kappa in (0.0, 0.12):
+        runs = []
+        for timing in (False, True):
+            lat = lgt.Lattice(dims, 5.6, kappa, BC)
+            lat.set_links(U)
+            lat.set_momenta(P)
+            if kappa:
+                lat.set_pseudofermion(oracle.dslash(dims, kappa, BC, U, synth.gaussian_spinor(dims, 93), dagger=True))
+                lgt.lgt_set_fermion_action(lat.ctx, lgt.LGT_ACTION_EO)
+            lgt.lgt_set_integrator(lat.ctx, lgt.LGT_INT_SEXTON_WEINGARTEN, 5)
+            lgt.lgt_timing_enable(lat.ctx, timing)
+            n0 = lgt.lgt_launch_count(lat.ctx)
+            its = [lgt.lgt_md_trajectory(lat.ctx, 3, 0.05, 1e-11, 5000, measure=False)[2] for _ in range(2)]
+            runs.append((lat.get_links(), lat.get_momenta(), its, lgt.lgt_launch_count(lat.ctx) - n0))
+            lat.close()
+        assert runs[0][2] == runs[1][2] and runs[0][3] == runs[1][3]
+        assert np.array_equal(runs[0][0], runs[1][0]) and np.array_equal(runs[0][1], runs[1][1])
