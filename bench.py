@@ -803,18 +803,23 @@ def decomposed_steps(args, rank, world, local, steps, warmup, with_e2e=True):
     max_iter = 10 * V
     U, P, eta = make_inputs(cfg)  # every rank draws the same global fields and keeps its slab
     stream = torch.cuda.current_stream().cuda_stream
-    dd = dist.decomposed_lattice(dims, beta, kappa, bc, lgt.LGT_F64, local, stream, halo=args.halo, transport=args.transport)
+    grid = tuple(args.grid) if args.grid else None
+    if grid is not None and grid[0] * grid[1] != world:
+        raise SystemExit("--grid PT PZ needs PT * PZ = the number of ranks")
+    dd = dist.decomposed_lattice(dims, beta, kappa, bc, lgt.LGT_F64, local, stream, halo=args.halo, transport=args.transport, grid=grid)
     if args.action == "eo":
         lgt.lgt_dd_set_fermion_action(dd.d, lgt.LGT_ACTION_EO)
     if args.solver == "mixed":
         lgt.lgt_dd_set_solver(dd.d, lgt.LGT_SOLVER_MIXED_CG, 1e-5)
     if args.smear:
         lgt.lgt_dd_set_smearing(dd.d, args.smear, 0.3)
-    lo, hi = dist.slab_rows(dims, world, rank)
-    hU, hP = torch.from_numpy(U[lo:hi].copy()).pin_memory(), torch.from_numpy(P[lo:hi].copy()).pin_memory()
+    import numpy as np
+
+    mine = (lambda a: np.ascontiguousarray(dd.slab(a, rank)))  # this rank's time slab, or its (t, z) block on a grid
+    hU, hP = torch.from_numpy(mine(U)).pin_memory(), torch.from_numpy(mine(P)).pin_memory()
     ctx = dd.ranks[0]
     lgt.lgt_set_links_host(ctx, hU)
-    d_eta = torch.from_numpy(eta[lo:hi].copy()).cuda()
+    d_eta = torch.from_numpy(mine(eta)).cuda()
     d_phi = torch.empty_like(d_eta)
     lgt.lgt_dd_dslash(dd.d, [d_eta], [d_phi], True)
     hphi = d_phi.cpu().pin_memory()
@@ -869,8 +874,9 @@ def decomposed_steps(args, rank, world, local, steps, warmup, with_e2e=True):
     total_reals = sum(step_reals(i, args.solver, args.action, args.smear) for i in iters) * V  # the whole lattice: strong scaling
     res = {"value": round(total_reals * 8 / (elapsed_ms * 1e-3) / 1e9, 1), "unit": "GB/s", "ms_per_step": round(elapsed_ms / steps, 3),
            "steps": steps, "cg_iters_per_step": iters, "gpu_launches": int(launches_all), "clocks": clocks,
-           "parallelism": "dd%d: ONE %s lattice in %d time slabs, halo %s, transport %s%s" %
-                          (world, "x".join(map(str, dims)), world, args.halo, args.transport, ", every rank on cuda:0" if args.same_gpu else "")}
+           "parallelism": "dd%d: ONE %s lattice in %s, halo %s, transport %s%s" %
+                          (world, "x".join(map(str, dims)), ("a %d x %d (t, z) grid" % grid) if grid else "%d time slabs" % world, args.halo,
+                           args.transport, ", every rank on cuda:0" if args.same_gpu else "")}
     if with_e2e:
         e2e_reals = sum(step_reals(i, args.solver, args.action, args.smear) for i in e2e_iters) * V
         res["e2e"] = {"value": round(e2e_reals * 8 / e2e_s / 1e9, 1), "unit": "GB/s", "steps": k_e2e, "ms_per_step": round(e2e_s / k_e2e * 1e3, 2),
@@ -1068,6 +1074,8 @@ def main():
                     help="decomposed lattice: the library's NCCL communicator, or gloo through host memory (lgt_dd_set_host_transport)")
     ap.add_argument("--same-gpu", action="store_true",
                     help="--parallelism dd --transport host only: every rank on cuda:0 (runs the inter-process path on a one-GPU box)")
+    ap.add_argument("--grid", type=int, nargs=2, default=None, metavar=("PT", "PZ"),
+                    help="--parallelism dd: two split directions (lgt_dd_create_grid), PT * PZ = ranks; default: time slabs")
     ap.add_argument("--nccl-debug", action="store_true", help="--parallelism dd: NCCL_DEBUG=INFO, so that the output shows every rank's communicator")
     ap.add_argument("--smear", type=int, default=0,
                     help="non-default: the fermions see this many levels of stout-smeared links (rho = 0.3); not the headline")

@@ -212,6 +212,16 @@ int lgt_get_smeared_links(lgt_ctx* ctx, void* U);
 typedef struct lgt_dd lgt_dd;
 int lgt_dd_create(lgt_dd** out, const int dims[4], int nranks, int nlocal, const int* local_ranks, double beta, double kappa,
                   const int bc[4], int precision, int device, void* cuda_stream);
+/* The same with TWO split directions ("first T, then Z"): grid = {Pt, Pz}, Pt * Pz ranks, rank = pt * Pz + pz
+ * owns the time slices [pt Lt/Pt, (pt+1) Lt/Pt) and the z planes [pz Lz/Pz, (pz+1) Lz/Pz); Lt % Pt == 0, Lz % Pz == 0 and
+ * Lx*Ly % 32 == 0, else LGT_EINVAL.  A rank's local lattice has two ghost time slices and two ghost z planes; the halo of a
+ * field travels first in t (whole local slices) and then in z (the boundary xy planes of every local slice, ghost slices
+ * included, which fills the corners the staples need), through the same three transports.  Slab arrays are the rank's
+ * block [Lt/Pt][Lz/Pz][Ly][Lx] in lexicographic order.  Full operator with plain or mixed-precision CG, stout smearing,
+ * all integrators and the HMC trajectory; LGT_DD_PUSH and the even/odd action are for time slabs only (LGT_EINVAL).
+ * grid = {nranks, 1} is a time-slab decomposition whose ranks are their own z neighbours. */
+int lgt_dd_create_grid(lgt_dd** out, const int dims[4], const int grid[2], int nlocal, const int* local_ranks, double beta,
+                       double kappa, const int bc[4], int precision, int device, void* cuda_stream);
 int lgt_dd_destroy(lgt_dd* d);
 const char* lgt_dd_last_error(const lgt_dd* d);
 /* NCCL transport: rank 0 obtains a 128-byte id (HOST buffer), the caller broadcasts it to all processes (e.g. through

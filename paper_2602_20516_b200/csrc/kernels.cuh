@@ -39,7 +39,34 @@ struct Geom {
     int Lt_glob;    // global time extent (for the fermion boundary sign of the t links)
     int site_off;   // global site index = local site index + site_off (heat baths draw by global element number)
     int h_begin, h_end;  // the owned range of checkerboard indices of a half field (s_begin / 2, s_end / 2)
+    // Second split direction of a decomposed lattice (lgt_dd_create_grid): the local lattice then also carries two ghost
+    // z planes (local z = 0 and L[2] - 1), the owned sites are those of [s_begin, s_end) with z in [z_lo, z_hi), and the
+    // boundary sign of the z links goes by the global z coordinate.  Undivided or time slabs only: z_lo = 0, z_hi = L[2].
+    int z_lo, z_hi;
+    int z_off;      // global z of local plane 0
+    int Lz_glob;    // global z extent
 };
+// Global lexicographic number of local site s (the heat baths draw by it): an offset on the undivided lattice and on a
+// time slab, from the coordinates on a grid rank.
+__device__ __forceinline__ unsigned global_site(const Geom& g, int s) {
+    if (g.z_hi - g.z_lo == g.L[2]) return (unsigned)(s + g.site_off);
+    const int xy = g.L[0] * g.L[1];
+    const int t = s / (xy * g.L[2]), r = s - t * (xy * g.L[2]);
+    const int z = r / xy, q = r - z * xy;
+    return (unsigned)(((t + g.t_off) * g.Lz_glob + (z + g.z_off)) * xy + q);
+}
+// owned by this rank's compute kernels (s already inside [s_begin, s_end))?
+__device__ __forceinline__ bool z_owned(const Geom& g, int z) { return z >= g.z_lo && z < g.z_hi; }
+__device__ __forceinline__ int z_of_site(const Geom& g, int s) { return (s / (g.L[0] * g.L[1])) % g.L[2]; }
+// position of an owned site in the rank's canonical slab array: the owned sites in lexicographic order
+__device__ __forceinline__ size_t canonical_index(const Geom& g, int s) {
+    if (g.z_hi - g.z_lo == g.L[2]) return (size_t)(s - g.s_begin);
+    const int xy = g.L[0] * g.L[1];
+    const int t = s / (xy * g.L[2]), r = s - t * (xy * g.L[2]);
+    const int z = r / xy, q = r - z * xy;
+    const int t0 = g.s_begin / (xy * g.L[2]);
+    return ((size_t)(t - t0) * (g.z_hi - g.z_lo) + (z - g.z_lo)) * xy + q;
+}
 
 // lexicographic 128-site chunk handled by block b
 __device__ __forceinline__ int swizzled_chunk(const Geom& g, int b) {
@@ -116,6 +143,7 @@ template <class T> __device__ __forceinline__ void load_link12(const typename Ve
 __device__ __forceinline__ int folded_sign(const Geom& g, int mu, int xmu) {
     if (g.bc[mu] > 0) return 1;
     if (mu == 3) return ((xmu + g.t_off + g.Lt_glob) % g.Lt_glob == g.Lt_glob - 1) ? -1 : 1;
+    if (mu == 2) return ((xmu + g.z_off + g.Lz_glob) % g.Lz_glob == g.Lz_glob - 1) ? -1 : 1;
     return (xmu == g.L[mu] - 1) ? -1 : 1;
 }
 template <class T, int NA = 0> __device__ __forceinline__ void load_spinor(const typename Vec2<T>::type* f, int s, cx<T> p[12]) {
@@ -412,7 +440,7 @@ template <class T> struct PushTo {
 // PF > 0 (variant 4): every thread first asks L2 for the lines the block PF positions further on in the grid will need
 // from DRAM first -- its forward links and its t+1 spinors -- so that those loads find their data in L2 (prefetches hold
 // no registers; PF = the number of co-resident blocks, i.e. the block that takes this block's place on the SM).
-template <class T, int DAG, int MODE, int PUSH = 0, int PFON = 0>
+template <class T, int DAG, int MODE, int PUSH = 0, int PFON = 0, int ZS = 0>
 __global__ void __launch_bounds__(128, 1) dslash_kernel(Geom g, const typename Vec2<T>::type* __restrict__ U,
                                                         const typename Vec2<T>::type* __restrict__ in,
                                                         typename Vec2<T>::type* __restrict__ out, T kappa, CgState* st,
@@ -442,7 +470,8 @@ __global__ void __launch_bounds__(128, 1) dslash_kernel(Geom g, const typename V
         }
     }
     double nrm = 0.0;
-    if (s < g.s_end) {
+    // ZS: a rank of a (Pt, Pz) grid -- the sites of its two ghost z planes are skipped like the sites past s_end
+    if (s < g.s_end && (!ZS || z_owned(g, z_of_site(g, s)))) {
         if (MODE == 2) {
             // r is only needed by the epilogue: pull its lines into L2 now, without holding registers, so that the
             // read-modify-write at the end does not expose a full DRAM latency
@@ -903,13 +932,26 @@ __global__ void __launch_bounds__(256, 1) dslash_tile_kernel(Geom g, const typen
     if (MODE != 0) block_partial(nrm, partials);
 }
 
+// Streaming reductions over a spinor field of a grid rank (two split directions) must leave the ghost z planes out of
+// the sum: element i of the range handed to the kernel (which starts at a time-slice boundary) belongs to the site
+// (i / 384) * 32 + i % 32 of that range.  xy = 0: no mask.
+struct ZMask {
+    int xy = 0, Lz = 1, z_lo = 0, z_hi = 1;
+};
+__device__ __forceinline__ bool zmask_owned(const ZMask& m, size_t i) {
+    if (m.xy == 0) return true;
+    const int s = (int)(i / (12 * W)) * W + (int)(i & 31);
+    const int z = (s / m.xy) % m.Lz;
+    return z >= m.z_lo && z < m.z_hi;
+}
+
 // ---------------------------------------------------------------------------- A3: CG BLAS-1 (fused)
 // r = b, p = b, x = 0, rr = bb = |b|^2
 template <class T>
 __global__ void __launch_bounds__(256) cg_init_kernel(size_t n, const typename Vec2<T>::type* __restrict__ b,
                                                       typename Vec2<T>::type* __restrict__ x, typename Vec2<T>::type* __restrict__ r,
                                                       typename Vec2<T>::type* __restrict__ p, CgState* st, double tol2, int max_iter,
-                                                      double* partials, unsigned* counter) {
+                                                      double* partials, unsigned* counter, ZMask zm = ZMask()) {
     double acc = 0.0;
     typename Vec2<T>::type zero;
     zero.x = 0;
@@ -919,7 +961,7 @@ __global__ void __launch_bounds__(256) cg_init_kernel(size_t n, const typename V
         x[i] = zero;
         r[i] = v;
         p[i] = v;
-        acc += (double)v.x * (double)v.x + (double)v.y * (double)v.y;
+        if (zmask_owned(zm, i)) acc += (double)v.x * (double)v.x + (double)v.y * (double)v.y;
     }
     block_reduce_finalize(acc, partials, counter, [=](double sum) {
         st->rr = sum;
@@ -980,9 +1022,10 @@ __global__ void __launch_bounds__(256) cg_update_p_ghost_kernel(size_t n, size_t
 template <class T>
 __global__ void __launch_bounds__(256) redot_kernel(size_t n, const typename Vec2<T>::type* __restrict__ a,
                                                     const typename Vec2<T>::type* __restrict__ b, double* result, double* partials,
-                                                    unsigned* counter) {
+                                                    unsigned* counter, ZMask zm = ZMask()) {
     double acc = 0.0;
     for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+        if (!zmask_owned(zm, i)) continue;
         typename Vec2<T>::type av = __ldg(a + i), bv = __ldg(b + i);
         acc += (double)av.x * (double)bv.x + (double)av.y * (double)bv.y;
     }
@@ -1062,6 +1105,7 @@ __global__ void __launch_bounds__(128, 1) fermion_force_kernel(Geom g, const typ
     const int s = g.s_begin + swizzled_chunk(g, blockIdx.x) * blockDim.x + threadIdx.x;
     if (s >= g.s_end) return;
     const Site c = site_coords(g, s);
+    if (!z_owned(g, c.x[2])) return;
     cx<T> Xs[12], Ys[12];
     load_spinor<T>(X, s, Xs);
     load_spinor<T>(Y, s, Ys);
@@ -1096,6 +1140,7 @@ __global__ void __launch_bounds__(128 * ROWS, ROWS == 1 ? 2 : 1)
     if (s >= g.s_end) return;
     const int mu = (threadIdx.x >> 5) & 3;
     const Site c = site_coords(g, s);
+    if (!z_owned(g, c.x[2])) return;
     const int smu = nbr_fwd(g, c, s, mu);
     cx<T> V[9];
     mat_zero(V);
@@ -1409,6 +1454,7 @@ __global__ void __launch_bounds__(128) stout_chain_kernel(Geom g, const typename
     if (s >= g.s_end) return;
     const int mu = threadIdx.x >> 5;
     const Site c = site_coords(g, s);
+    if (!z_owned(g, c.x[2])) return;
     const int smu = nbr_fwd(g, c, s, mu);
     cx<T> X[9], Ua[9], Ga[9];
     mat_zero(X);
@@ -1487,7 +1533,7 @@ __global__ void __launch_bounds__(128) plaquette_kernel(Geom g, const typename V
                                                         double* partials, unsigned* counter) {
     const int s = g.s_begin + blockIdx.x * blockDim.x + threadIdx.x;
     double acc = 0.0;
-    if (s < g.s_end) {
+    if (s < g.s_end && z_owned(g, z_of_site(g, s))) {
         const Site c = site_coords(g, s);
 #pragma unroll
         for (int mu = 0; mu < 4; mu++) {
@@ -1523,6 +1569,7 @@ __global__ void __launch_bounds__(256) kinetic_kernel(Geom g, const typename Vec
     const size_t nlinks = (size_t)4 * (g.s_end == g.V ? g.Vs : g.s_end);
     for (size_t i = (size_t)4 * g.s_begin + blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < nlinks; i += (size_t)gridDim.x * blockDim.x) {
         // i = (blk * 4 + mu) * 32 + lane
+        if (!z_owned(g, z_of_site(g, (int)(i >> 7) * W + (int)(i & 31)))) continue;  // a ghost z plane of a grid rank
         const typename Vec2<T>::type* b = P + (i >> 5) * (4 * W) + (i & 31);
         typename Vec2<T>::type d = __ldg(b);
         double d0 = d.x, d1 = d.y, d2 = -(d0 + d1);
@@ -1721,14 +1768,15 @@ __global__ void __launch_bounds__(256) up_axpy_kernel(size_t n, double2* __restr
 }
 // r = b - q, result = |r|^2 (fixed-order sum)
 __global__ void __launch_bounds__(256) residual_kernel(size_t n, const double2* __restrict__ b, const double2* __restrict__ q,
-                                                       double2* __restrict__ r, double* result, double* partials, unsigned* counter) {
+                                                       double2* __restrict__ r, double* result, double* partials, unsigned* counter,
+                                                       ZMask zm = ZMask()) {
     double acc = 0.0;
     for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
         double2 bv = __ldg(b + i), qv = __ldg(q + i);
         bv.x -= qv.x;
         bv.y -= qv.y;
         r[i] = bv;
-        acc += bv.x * bv.x + bv.y * bv.y;
+        if (zmask_owned(zm, i)) acc += bv.x * bv.x + bv.y * bv.y;
     }
     block_reduce_finalize(acc, partials, counter, [result](double sum) { *result = sum; });
 }
@@ -1780,10 +1828,10 @@ __global__ void __launch_bounds__(256) momentum_heatbath_kernel(Geom g, typename
         const int mu = (int)((i >> 5) & 3);
         const int s = (int)(i >> 7) * W + lane;
         double pi[8] = {0, 0, 0, 0, 0, 0, 0, 0};
-        if (s >= g.s_begin && s < g.s_end) {
+        if (s >= g.s_begin && s < g.s_end && z_owned(g, z_of_site(g, s))) {
 #pragma unroll
             for (int j = 0; j < 4; j++)
-                philox_gaussian_pair(seed, traj, 1u, (unsigned)(4 * (s + g.site_off) + mu), (unsigned)j, pi[2 * j], pi[2 * j + 1]);
+                philox_gaussian_pair(seed, traj, 1u, 4u * global_site(g, s) + (unsigned)mu, (unsigned)j, pi[2 * j], pi[2 * j + 1]);
         }
         // tau^a = i lambda^a / 2:  Im Pi00 = (pi3 + pi8/sqrt3)/2, Im Pi11 = (-pi3 + pi8/sqrt3)/2,
         // Pi01 = (pi2 + i pi1)/2, Pi02 = (pi5 + i pi4)/2, Pi12 = (pi7 + i pi6)/2      (pi1 = pi[0])
@@ -1811,7 +1859,8 @@ __global__ void __launch_bounds__(256) spinor_heatbath_kernel(Geom g, typename V
         const int k = (int)((i >> 5) % 12);
         const int s = (int)((i >> 5) / 12) * W + lane;
         double g0 = 0.0, g1 = 0.0;
-        if (s >= g.s_begin && s < g.s_end) philox_gaussian_pair(seed, traj, 2u, (unsigned)(s + g.site_off), (unsigned)k, g0, g1);
+        if (s >= g.s_begin && s < g.s_end && z_owned(g, z_of_site(g, s)))
+            philox_gaussian_pair(seed, traj, 2u, global_site(g, s), (unsigned)k, g0, g1);
         typename Vec2<T>::type v;
         v.x = (T)(0.70710678118654752440084436210485 * g0);
         v.y = (T)(0.70710678118654752440084436210485 * g1);
@@ -1846,6 +1895,7 @@ __device__ __forceinline__ int link_sign(const Geom& g, int s, int mu) {
     if (g.bc[mu] > 0) return 1;
     int x = (s / g.stride[mu]) % g.L[mu];
     if (mu == 3) return ((x + g.t_off + g.Lt_glob) % g.Lt_glob == g.Lt_glob - 1) ? -1 : 1;
+    if (mu == 2) return ((x + g.z_off + g.Lz_glob) % g.Lz_glob == g.Lz_glob - 1) ? -1 : 1;
     return (x == g.L[mu] - 1) ? -1 : 1;
 }
 
@@ -1861,14 +1911,14 @@ __global__ void __launch_bounds__(256) reorder_kernel(Geom g, const typename Vec
         const int k = (int)((i >> 5) % NCOMP);
         const int s = (int)((i >> 5) / NCOMP) * W + lane;
         T sg = 1;
-        const bool own = s >= g.s_begin && s < g.s_end;  // the canonical buffer holds the owned sites only
+        const bool own = s >= g.s_begin && s < g.s_end && z_owned(g, z_of_site(g, s));  // the canonical buffer holds the owned sites only
         if (LINKS && own) sg = (T)link_sign(g, s, k / 9);
         if (DIR == 0) {
             typename Vec2<T>::type v;
             v.x = 0;
             v.y = 0;
             if (own) {
-                v = __ldg(src + (size_t)(s - g.s_begin) * NCOMP + k);
+                v = __ldg(src + canonical_index(g, s) * NCOMP + k);
                 v.x *= sg;
                 v.y *= sg;
             }
@@ -1877,7 +1927,7 @@ __global__ void __launch_bounds__(256) reorder_kernel(Geom g, const typename Vec
             typename Vec2<T>::type v = __ldg(src + i);
             v.x *= sg;
             v.y *= sg;
-            dst[(size_t)(s - g.s_begin) * NCOMP + k] = v;
+            dst[canonical_index(g, s) * NCOMP + k] = v;
         }
     }
 }
@@ -1894,10 +1944,10 @@ __global__ void __launch_bounds__(256) momenta_reorder_kernel(Geom g, const type
         const int s = (int)(i >> 7) * W + lane;
         if (DIR == 0) {
             T c[8] = {0, 0, 0, 0, 0, 0, 0, 0};
-            if (s >= g.s_begin && s < g.s_end) {  // the canonical buffer holds the owned sites only
+            if (s >= g.s_begin && s < g.s_end && z_owned(g, z_of_site(g, s))) {  // the canonical buffer holds the owned sites only
                 cx<T> m[9];
 #pragma unroll
-                for (int k = 0; k < 9; k++) m[k] = ldc<T>(src + ((size_t)(s - g.s_begin) * 4 + mu) * 9 + k);
+                for (int k = 0; k < 9; k++) m[k] = ldc<T>(src + (canonical_index(g, s) * 4 + mu) * 9 + k);
                 ta_compact(m, (T)1, c);
             }
             typename Vec2<T>::type* b = mom_at(dst, s, mu);
@@ -1908,7 +1958,7 @@ __global__ void __launch_bounds__(256) momenta_reorder_kernel(Geom g, const type
                 v.y = c[2 * q + 1];
                 b[q * W] = v;
             }
-        } else if (s >= g.s_begin && s < g.s_end) {
+        } else if (s >= g.s_begin && s < g.s_end && z_owned(g, z_of_site(g, s))) {
             T c[8];
             const typename Vec2<T>::type* b = mom_at(src, s, mu);
 #pragma unroll
@@ -1920,7 +1970,7 @@ __global__ void __launch_bounds__(256) momenta_reorder_kernel(Geom g, const type
             cx<T> m[9];
             compact_expand(c, m);
 #pragma unroll
-            for (int k = 0; k < 9; k++) stc<T>(dst + ((size_t)(s - g.s_begin) * 4 + mu) * 9 + k, m[k]);
+            for (int k = 0; k < 9; k++) stc<T>(dst + (canonical_index(g, s) * 4 + mu) * 9 + k, m[k]);
         }
     }
 }

@@ -348,6 +348,19 @@ template <class T> struct Ops {
             return LGT_OK;
         }
 #undef DSLASH_PUSH_ARGS
+        if (c->g.z_hi - c->g.z_lo != c->g.L[2]) {  // a rank of a (Pt, Pz) grid: the kernel that skips the ghost z planes
+            if (mode == 0) {
+                if (dagger)
+                    LAUNCH(c, LGT_K_DSLASH, (dslash_kernel<T, 1, 0, 0, 0, 1>), grid, 128, DSLASH_ARGS);
+                else
+                    LAUNCH(c, LGT_K_DSLASH, (dslash_kernel<T, 0, 0, 0, 0, 1>), grid, 128, DSLASH_ARGS);
+            } else if (mode == 1) {
+                LAUNCH(c, LGT_K_DSLASH, (dslash_kernel<T, 0, 1, 0, 0, 1>), grid, 128, DSLASH_ARGS);
+            } else {
+                LAUNCH(c, LGT_K_DSLASH_R, (dslash_kernel<T, 1, 2, 0, 0, 1>), grid, 128, DSLASH_ARGS);
+            }
+            return LGT_OK;
+        }
         if (c->variant[LGT_K_DSLASH] == 1) {  // persistent, software-pipelined: one wave of blocks loops over the chunks
             const int pgrid = grid < 2 * c->num_sms ? grid : 2 * c->num_sms;
 #define DSLASH_PARGS c->g, (const T2*)U, (const T2*)in, (T2*)out, kappa, c->st, c->partials, (T2*)r, grid
@@ -1185,6 +1198,10 @@ int lgt_create(lgt_ctx** out, const int dims[4], double beta, double kappa, cons
     c->g.t_off = 0;
     c->g.Lt_glob = c->g.L[3];
     c->g.site_off = 0;
+    c->g.z_lo = 0;
+    c->g.z_hi = c->g.L[2];
+    c->g.z_off = 0;
+    c->g.Lz_glob = c->g.L[2];
     c->g.h_begin = 0;
     c->g.h_end = c->g.Vh;
     int sms = 148;

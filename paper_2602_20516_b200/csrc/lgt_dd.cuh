@@ -65,6 +65,12 @@ struct lgt_dd {
     int device = 0;
     cudaStream_t stream = nullptr;
     bool links_ghost_valid = false;
+    // (Pt, Pz) grid (lgt_dd_create_grid): Pz > 0; rank = pt * Pz + pz; every rank then also has two ghost z planes and
+    // V3 counts them (it is the size of a LOCAL time slice).  Time slabs: Pz = 0.
+    int Pt = 0, Pz = 0, Lz_loc = 0, LxLy = 0;
+    long long Vglob = 0;
+    void* d_stage = nullptr;  // device staging of the z faces for NCCL (2 outgoing, 2 incoming)
+    size_t d_stage_bytes = 0;
     void* comm = nullptr;  // ncclComm_t; null: host transport, or every rank is local
     // host transport (lgt_dd_set_host_transport): callbacks + pinned staging (2 outgoing, 2 incoming slices; sums)
     lgt_dd_sendrecv_fn host_sendrecv = nullptr;
@@ -154,10 +160,112 @@ int dd_host_stage(lgt_dd* d, size_t bytes) {
     return LGT_OK;
 }
 
+// ---- (Pt, Pz) grid: the halo of one split direction as two strided regions out, two in ("first T, then Z").
+// t: whole local time slices (one contiguous run each, z ghost planes included).  z: the xy planes z = 1 and z = Lz_loc of
+// EVERY local time slice, ghost slices included -- an xy plane is Lx*Ly/32 whole layout blocks, so a z face is Lt_loc + 2
+// contiguous runs at the pitch of a time slice and moves by 2-D copies, again without a packing kernel.  Doing t first
+// and z second fills the corners: the z neighbour's ghost time slices already hold the diagonal rank's planes, which is what
+// the staples U_nu(x + mu - nu) need.
+struct GridHalo {
+    int dn, up;            // peers: my first interior region goes to dn's upper ghost, my last to up's lower ghost
+    size_t send_off[2], recv_off[2];  // bytes from the field's base: sends (to dn, to up), receives (from up, from dn)
+    size_t width, pitch;   // bytes per run, distance between runs
+    int height;            // runs
+};
+GridHalo grid_halo(const lgt_dd* d, int rank, int dim /* 0: t, 1: z */, int per_site, size_t esize) {
+    GridHalo h;
+    const int pt = rank / d->Pz, pz = rank % d->Pz;
+    const size_t slice = (size_t)d->V3 * per_site * esize;
+    if (dim == 0) {
+        h.dn = ((pt + d->Pt - 1) % d->Pt) * d->Pz + pz;
+        h.up = ((pt + 1) % d->Pt) * d->Pz + pz;
+        h.width = slice;
+        h.pitch = slice;
+        h.height = 1;
+        h.send_off[0] = slice;
+        h.send_off[1] = (size_t)d->Lt_loc * slice;
+        h.recv_off[0] = (size_t)(d->Lt_loc + 1) * slice;
+        h.recv_off[1] = 0;
+    } else {
+        h.dn = pt * d->Pz + (pz + d->Pz - 1) % d->Pz;
+        h.up = pt * d->Pz + (pz + 1) % d->Pz;
+        h.width = (size_t)d->LxLy * per_site * esize;
+        h.pitch = slice;
+        h.height = d->Lt_loc + 2;
+        h.send_off[0] = h.width;
+        h.send_off[1] = (size_t)d->Lz_loc * h.width;
+        h.recv_off[0] = (size_t)(d->Lz_loc + 1) * h.width;
+        h.recv_off[1] = 0;
+    }
+    return h;
+}
+int dd_host_stage(lgt_dd* d, size_t bytes);
+int dd_exchange_grid(lgt_dd* d, void* const* base, int per_site, size_t esize) {
+    const int n = (int)d->rk.size();
+    for (int dim = 0; dim < 2; dim++) {
+        if (!d->comm && !d->host_sendrecv) {  // every rank in this process: device copies
+            for (int i = 0; i < n; i++) {
+                const GridHalo h = grid_halo(d, d->rank_of[i], dim, per_site, esize);
+                const int peers[2] = {h.dn, h.up};
+                for (int k = 0; k < 2; k++) {
+                    const int peer = dd_local_index(d, peers[k]);
+                    if (peer < 0) return dd_fail(d, LGT_ESTATE, "dd_exchange: a neighbour rank is not in this process");
+                    // my k-th send lands where the peer receives its k-th message (send 0, to dn, is dn's receive 0, from its up)
+                    DD_CU(cudaMemcpy2DAsync((char*)base[peer] + h.recv_off[k], h.pitch, (const char*)base[i] + h.send_off[k], h.pitch, h.width,
+                                            h.height, cudaMemcpyDeviceToDevice, d->stream));
+                }
+            }
+            continue;
+        }
+        const GridHalo h = grid_halo(d, d->rank_of[0], dim, per_site, esize);
+        const size_t bytes = h.width * h.height;
+        const int send_peer[2] = {h.dn, h.up}, recv_peer[2] = {h.up, h.dn};
+        char* mine = (char*)base[0];
+        if (d->comm) {
+            if (d->d_stage_bytes < 4 * bytes) {
+                DD_CU(cudaStreamSynchronize(d->stream));
+                if (d->d_stage) cudaFree(d->d_stage);
+                d->d_stage = nullptr;
+                d->d_stage_bytes = 0;
+                DD_CU(cudaMalloc(&d->d_stage, 4 * bytes));
+                d->d_stage_bytes = 4 * bytes;
+            }
+            char* st = (char*)d->d_stage;
+            for (int k = 0; k < 2; k++)
+                DD_CU(cudaMemcpy2DAsync(st + k * bytes, h.width, mine + h.send_off[k], h.pitch, h.width, h.height, cudaMemcpyDeviceToDevice, d->stream));
+            DD_NCCL(g_nccl.GroupStart());
+            for (int k = 0; k < 2; k++) DD_NCCL(g_nccl.Send(st + k * bytes, bytes, NCCL_CHAR, send_peer[k], d->comm, d->stream));
+            for (int k = 0; k < 2; k++) DD_NCCL(g_nccl.Recv(st + (2 + k) * bytes, bytes, NCCL_CHAR, recv_peer[k], d->comm, d->stream));
+            DD_NCCL(g_nccl.GroupEnd());
+            for (int k = 0; k < 2; k++)
+                DD_CU(cudaMemcpy2DAsync(mine + h.recv_off[k], h.pitch, st + (2 + k) * bytes, h.width, h.width, h.height, cudaMemcpyDeviceToDevice, d->stream));
+            continue;
+        }
+        int rc;
+        if ((rc = dd_host_stage(d, 4 * bytes)) != LGT_OK) return rc;
+        char* hs = d->h_stage;
+        for (int k = 0; k < 2; k++)
+            DD_CU(cudaMemcpy2DAsync(hs + k * bytes, h.width, mine + h.send_off[k], h.pitch, h.width, h.height, cudaMemcpyDeviceToHost, d->stream));
+        DD_CU(cudaStreamSynchronize(d->stream));
+        const void* const sb[2] = {hs, hs + bytes};
+        void* const rb[2] = {hs + 2 * bytes, hs + 3 * bytes};
+        if (d->host_sendrecv(d->host_user, sb, send_peer, rb, recv_peer, bytes) != 0)
+            return dd_fail(d, LGT_ECUDA, "dd_exchange: the host transport's send/receive callback failed");
+        for (int k = 0; k < 2; k++)
+            DD_CU(cudaMemcpy2DAsync(mine + h.recv_off[k], h.pitch, hs + (2 + k) * bytes, h.width, h.width, h.height, cudaMemcpyHostToDevice, d->stream));
+        DD_CU(cudaStreamSynchronize(d->stream));  // the staging buffer is reused by the z phase
+    }
+    return LGT_OK;
+}
+
 // Halo exchange of one native field per local rank: base[i] points to the field of local rank i, `per_site` = complex
 // (or pair) elements per site (12 spinor, 36 links, 16 compact momenta).
 int dd_exchange(lgt_dd* d, void* const* base, int per_site, size_t esize = 0) {
     if (!esize) esize = d->prec == LGT_F64 ? 16 : 8;
+    if (d->Pz > 0) {
+        int rcg = dd_need_transport(d);
+        return rcg != LGT_OK ? rcg : dd_exchange_grid(d, base, per_site, esize);
+    }
     const size_t slice = (size_t)d->V3 * per_site * esize;
     const int n = (int)d->rk.size();
     int rc;
@@ -260,6 +368,17 @@ template <class T> struct DdOps {
     typedef typename Vec2<T>::type T2;
     typedef Ops<T> O;
 
+    // the ghost z planes of a grid rank stay out of the streaming sums (none on time slabs)
+    static ZMask zmask(const lgt_ctx* c) {
+        ZMask m;
+        if (c->g.z_hi - c->g.z_lo != c->g.L[2]) {
+            m.xy = c->g.L[0] * c->g.L[1];
+            m.Lz = c->g.L[2];
+            m.z_lo = c->g.z_lo;
+            m.z_hi = c->g.z_hi;
+        }
+        return m;
+    }
     static size_t spinor_off(const lgt_ctx* c) { return (size_t)12 * c->g.s_begin; }
     static size_t spinor_n(const lgt_ctx* c) { return (size_t)12 * own_sites(c); }
 
@@ -435,7 +554,7 @@ template <class T> struct DdOps {
             const size_t off = spinor_off(c), cnt = spinor_n(c);
             const T2* b = (const T2*)fld(c, ib) + off;
             LAUNCH(c, LGT_K_CG_BLAS, (cg_init_kernel<T>), stream_blocks(c, cnt), 256, cnt, b, (T2*)fld(c, 0) + off, (T2*)fld(c, 1) + off,
-                   (T2*)fld(c, 2) + off, c->st, tol * tol, max_iter, c->partials, c->counter);
+                   (T2*)fld(c, 2) + off, c->st, tol * tol, max_iter, c->partials, c->counter, zmask(c));
             LAUNCH(c, LGT_K_CG_BLAS, cg_rr_to_tmp_kernel, 1, 1, c->st);
         }
         if ((rc = allreduce_tmp(d)) != LGT_OK) return rc;
@@ -576,7 +695,8 @@ template <class T> struct DdOps {
             } else if (ferm) {
                 const size_t off = spinor_off(c);
                 const T2 *a = (const T2*)(eta_norm ? c->ws[4] : c->phi) + off, *b = (const T2*)(eta_norm ? c->ws[4] : c->ws[0]) + off;
-                LAUNCH(c, LGT_K_OTHER, (redot_kernel<T>), stream_blocks(c, spinor_n(c)), 256, spinor_n(c), a, b, c->scal + 2, c->partials, c->counter);
+                LAUNCH(c, LGT_K_OTHER, (redot_kernel<T>), stream_blocks(c, spinor_n(c)), 256, spinor_n(c), a, b, c->scal + 2, c->partials, c->counter,
+                       zmask(c));
             } else {
                 DD_CU(cudaMemsetAsync(c->scal + 2, 0, sizeof(double), d->stream));
             }
@@ -586,7 +706,7 @@ template <class T> struct DdOps {
         lgt_ctx* c0 = d->rk[0];
         DD_CU(cudaMemcpyAsync(c0->h_scal, c0->scal, 3 * sizeof(double), cudaMemcpyDeviceToHost, d->stream));
         DD_CU(cudaStreamSynchronize(d->stream));
-        const double sites = (double)d->V3 * d->Lt_loc * d->nranks;
+        const double sites = d->Pz > 0 ? (double)d->Vglob : (double)d->V3 * d->Lt_loc * d->nranks;
         if (S_g) *S_g = c0->beta * (6.0 * sites - c0->h_scal[0]);
         if (K) *K = c0->h_scal[1];
         if (S_F) *S_F = ferm ? c0->h_scal[2] : 0.0;
@@ -891,7 +1011,8 @@ int dd_cg_mixed(lgt_dd* d, int ib, bool want_y, double tol, int max_iter, int* i
         DD_CU(cudaMemsetAsync(c->ws[0], 0, nfull * sizeof(double2), d->stream));
         DD_CU(cudaMemsetAsync(c->ws[3], 0, nfull * sizeof(double2), d->stream));
         DD_CU(cudaMemcpyAsync(c->ws[1], b, nfull * sizeof(double2), cudaMemcpyDeviceToDevice, d->stream));
-        LAUNCH(c, LGT_K_OTHER, (redot_kernel<double>), stream_blocks(c, cnt), 256, cnt, b + off, b + off, c->scal + 3, c->partials, c->counter);
+        LAUNCH(c, LGT_K_OTHER, (redot_kernel<double>), stream_blocks(c, cnt), 256, cnt, b + off, b + off, c->scal + 3, c->partials, c->counter,
+               D64::zmask(c));
         slot.push_back(c->scal + 3);
     }
     lgt_ctx* c0 = d->rk[0];
@@ -936,7 +1057,7 @@ int dd_cg_mixed(lgt_dd* d, int ib, bool want_y, double tol, int max_iter, int* i
             lgt_ctx* c = d->rk[i];
             const size_t off = D64::spinor_off(c), cnt = D64::spinor_n(c);
             LAUNCH(c, LGT_K_CG_BLAS, residual_kernel, stream_blocks(c, cnt), 256, cnt, (const double2*)D64::fld(c, ib) + off,
-                   (const double2*)c->ws[2] + off, (double2*)c->ws[1] + off, c->scal + 3, c->partials, c->counter);
+                   (const double2*)c->ws[2] + off, (double2*)c->ws[1] + off, c->scal + 3, c->partials, c->counter, D64::zmask(c));
         }
         if ((rc = read_sum(rr)) != LGT_OK) return rc;
     }
@@ -1055,6 +1176,7 @@ int lgt_dd_destroy(lgt_dd* d) {
             if (d->ipc_open[f][sd]) cudaIpcCloseMemHandle(d->ipc_peer[f][sd]);
     if (d->h_stage) cudaFreeHost(d->h_stage);
     if (d->h_sum) cudaFreeHost(d->h_sum);
+    if (d->d_stage) cudaFree(d->d_stage);
     for (lgt_ctx* c : d->rk) lgt_destroy(c);
     delete d;
     return LGT_OK;
@@ -1141,6 +1263,75 @@ int lgt_dd_create(lgt_dd** out, const int dims[4], int nranks, int nlocal, const
     return LGT_OK;
 }
 
+int lgt_dd_create_grid(lgt_dd** out, const int dims[4], const int grid[2], int nlocal, const int* local_ranks, double beta, double kappa,
+                       const int bc[4], int precision, int device, void* cuda_stream) {
+    lgt_dd* d = nullptr;
+    if (!out || !dims || !grid || !bc || !local_ranks) return dd_fail(nullptr, LGT_EINVAL, "lgt_dd_create_grid: null argument");
+    *out = nullptr;
+    const int Pt = grid[0], Pz = grid[1];
+    if (Pt < 1 || Pz < 1) return dd_fail(nullptr, LGT_EINVAL, "lgt_dd_create_grid: grid = {Pt, Pz} with both >= 1");
+    const int nranks = Pt * Pz;
+    if (nlocal < 1 || nlocal > nranks || nlocal > 8) return dd_fail(nullptr, LGT_EINVAL, "lgt_dd_create_grid: need 1 <= nlocal <= min(Pt * Pz, 8)");
+    if (nlocal != nranks && nlocal != 1) return dd_fail(nullptr, LGT_EINVAL, "lgt_dd_create_grid: either every rank is local or exactly one is");
+    for (int m = 0; m < 4; m++)
+        if (dims[m] < 1) return dd_fail(nullptr, LGT_EINVAL, "lgt_dd_create_grid: dims must be >= 1");
+    if (dims[3] % Pt != 0 || dims[2] % Pz != 0) return dd_fail(nullptr, LGT_EINVAL, "lgt_dd_create_grid: Lt must be a multiple of Pt and Lz of Pz");
+    const long long xy = (long long)dims[0] * dims[1];
+    if (xy % 32 != 0) return dd_fail(nullptr, LGT_EINVAL, "lgt_dd_create_grid: Lx*Ly must be a multiple of 32 (an xy plane is then whole layout blocks)");
+    for (int i = 0; i < nlocal; i++) {
+        if (local_ranks[i] < 0 || local_ranks[i] >= nranks) return dd_fail(nullptr, LGT_EINVAL, "lgt_dd_create_grid: bad local rank number");
+        for (int j = 0; j < i; j++)
+            if (local_ranks[j] == local_ranks[i]) return dd_fail(nullptr, LGT_EINVAL, "lgt_dd_create_grid: duplicate local rank number");
+    }
+    d = new lgt_dd();
+    d->nranks = nranks;
+    d->Pt = Pt;
+    d->Pz = Pz;
+    d->Lt_loc = dims[3] / Pt;
+    d->Lz_loc = dims[2] / Pz;
+    d->LxLy = (int)xy;
+    d->V3 = (int)(xy * (d->Lz_loc + 2));  // a LOCAL time slice, ghost z planes included
+    d->Vglob = xy * dims[2] * dims[3];
+    d->prec = precision;
+    d->device = device;
+    d->stream = (cudaStream_t)cuda_stream;
+    const int ldims[4] = {dims[0], dims[1], d->Lz_loc + 2, d->Lt_loc + 2};
+    for (int i = 0; i < nlocal; i++) {
+        lgt_ctx* c = nullptr;
+        int rc = lgt_create(&c, ldims, beta, kappa, bc, precision, device, cuda_stream);
+        if (rc != LGT_OK) {
+            g_dd_create_error = std::string("lgt_dd_create_grid: ") + lgt_last_error(nullptr);
+            lgt_dd_destroy(d);
+            return rc;
+        }
+        const int pt = local_ranks[i] / Pz, pz = local_ranks[i] % Pz;
+        c->g.s_begin = d->V3;
+        c->g.s_end = c->g.V - d->V3;
+        c->g.t_off = pt * d->Lt_loc - 1;
+        c->g.Lt_glob = dims[3];
+        c->g.z_lo = 1;
+        c->g.z_hi = d->Lz_loc + 1;
+        c->g.z_off = pz * d->Lz_loc - 1;
+        c->g.Lz_glob = dims[2];
+        c->g.site_off = 0;  // grid ranks number their elements through global_site()
+        c->g.h_begin = d->V3 / 2;
+        c->g.h_end = c->g.Vh - d->V3 / 2;
+        c->g.swz_Z = 0;
+        c->dd_links_valid = &d->links_ghost_valid;
+        d->rk.push_back(c);
+        d->rank_of.push_back(local_ranks[i]);
+        rc = precision == LGT_F64 ? Ops<double>::unit_links(c) : Ops<float>::unit_links(c);
+        if (rc != LGT_OK) {
+            g_dd_create_error = "lgt_dd_create_grid: " + c->err;
+            lgt_dd_destroy(d);
+            return rc;
+        }
+    }
+    d->links_ghost_valid = true;  // the unit field fills the ghost slices and planes too
+    *out = d;
+    return LGT_OK;
+}
+
 int lgt_dd_nccl_unique_id(void* id128) {
     if (!id128) return LGT_EINVAL;
     if (!g_nccl.load()) return dd_fail(nullptr, LGT_ECUDA, "lgt_dd_nccl_unique_id: libnccl.so.2 not found");
@@ -1166,6 +1357,7 @@ int lgt_dd_nccl_init(lgt_dd* d, const void* id128) {
 int lgt_dd_set_halo_mode(lgt_dd* d, int mode) {
     CHECK_DD(d);
     if (mode != LGT_DD_EXCHANGE && mode != LGT_DD_PUSH) return dd_fail(d, LGT_EINVAL, "lgt_dd_set_halo_mode: unknown mode");
+    if (mode == LGT_DD_PUSH && d->Pz > 0) return dd_fail(d, LGT_EINVAL, "lgt_dd_set_halo_mode: LGT_DD_PUSH is for time slabs; a (Pt, Pz) grid exchanges");
     if (mode == LGT_DD_PUSH && d->rk.size() != (size_t)d->nranks && d->nranks > 1)
         for (int f = 0; f < 2; f++)
             for (int s = 0; s < 2; s++)
@@ -1283,6 +1475,8 @@ int lgt_dd_md_trajectory(lgt_dd* d, int nsteps, double dt, double tol, int max_i
 int lgt_dd_set_fermion_action(lgt_dd* d, int action) {
     CHECK_DD(d);
     if (action != LGT_ACTION_FULL && action != LGT_ACTION_EO) return dd_fail(d, LGT_EINVAL, "lgt_dd_set_fermion_action: unknown action");
+    if (action == LGT_ACTION_EO && d->Pz > 0)
+        return dd_fail(d, LGT_EINVAL, "lgt_dd_set_fermion_action: the even/odd action runs on time slabs, not on a (Pt, Pz) grid");
     if (action == LGT_ACTION_EO) {
         const Geom& g = d->rk[0]->g;
         if (g.L[0] % 2 || g.L[1] % 2 || g.L[2] % 2 || d->Lt_loc % 2 || d->V3 % 64)

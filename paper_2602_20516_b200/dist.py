@@ -60,6 +60,28 @@ def slab_rows(dims, nranks, rank):
     return rank * per, (rank + 1) * per
 
 
+def grid_block(a, dims, grid, rank):
+    """Block of a canonical field a[V, ...] owned by `rank` = pt * Pz + pz of a (Pt, Pz) grid (lgt_dd_create_grid): time
+    slices [pt Lt/Pt, (pt+1) Lt/Pt), z planes [pz Lz/Pz, (pz+1) Lz/Pz), flattened in lexicographic order."""
+    Lx, Ly, Lz, Lt = [int(d) for d in dims]
+    Pt, Pz = int(grid[0]), int(grid[1])
+    if Pt < 1 or Pz < 1 or Lt % Pt or Lz % Pz:
+        raise ValueError("Lt must be a multiple of Pt and Lz of Pz")
+    if not 0 <= rank < Pt * Pz:
+        raise ValueError("bad rank")
+    pt, pz = divmod(int(rank), Pz)
+    lt, lz = Lt // Pt, Lz // Pz
+    b = a.reshape((Lt, Lz, Ly * Lx) + tuple(a.shape[1:]))[pt * lt:(pt + 1) * lt, pz * lz:(pz + 1) * lz]
+    return b.reshape((lt * lz * Ly * Lx,) + tuple(a.shape[1:]))
+
+
+def grid_neighbours(grid, rank):
+    """(t_down, t_up, z_down, z_up) ranks of `rank` on a periodic (Pt, Pz) grid -- the peers of the two exchange phases."""
+    Pt, Pz = int(grid[0]), int(grid[1])
+    pt, pz = divmod(int(rank), Pz)
+    return (((pt - 1) % Pt) * Pz + pz, ((pt + 1) % Pt) * Pz + pz, pt * Pz + (pz - 1) % Pz, pt * Pz + (pz + 1) % Pz)
+
+
 def broadcast_bytes(data, nbytes, src=0, device="cpu"):
     """Rank `src` passes `data` (bytes of length nbytes), everybody returns the same bytes.  Identity without a group."""
     import torch
@@ -132,19 +154,22 @@ def host_allreduce(buf, group=None):
 
 
 def decomposed_lattice(dims, beta, kappa, bc, precision=None, local_device=0, stream=None, halo="exchange", transport="nccl",
-                       host_group=None):
+                       host_group=None, grid=None):
     """This process's slab of ONE lattice shared by all ranks of the default process group: a DecomposedLattice with one
     local rank.  transport = "nccl": the library's own NCCL communicator, initialised from an id that rank 0 creates and
     broadcasts here.  transport = "host": halo slices and sums travel through host memory over `host_group` (a gloo
     group; the default group if None) -- for clusters without NCCL between the ranks and for running the inter-process
     path with several processes on ONE GPU, which NCCL refuses.
     halo = "push": the neighbours' CG buffers are mapped through CUDA IPC (handles all-gathered here) and the halo
-    slices travel inside the Dslash kernels (lgt.LGT_DD_PUSH)."""
+    slices travel inside the Dslash kernels (lgt.LGT_DD_PUSH).
+    grid = (Pt, Pz) with Pt * Pz = world size: two split directions (lgt_dd_create_grid), rank = pt * Pz + pz; exchange mode only."""
     from . import lgt
 
     rank, world, _ = env_rank_world()
+    if grid is not None and halo == "push":
+        raise ValueError("a (Pt, Pz) grid exchanges its halos; LGT_DD_PUSH is for time slabs")
     dd = lgt.DecomposedLattice(dims, world, [rank], beta, kappa, bc, lgt.LGT_F64 if precision is None else precision,
-                               local_device, stream)
+                               local_device, stream, grid=grid)
     on_cpu = transport == "host"
     if transport == "host":
         lgt.lgt_dd_set_host_transport(dd.d, lambda sb, sp, rb, rp: host_sendrecv(sb, sp, rb, rp, host_group),

@@ -67,6 +67,7 @@ SYMBOLS = {
     "lgt_eo_cg": (_i, [_vp, _vp, _vp, _d, _i, _ip, _dp]),
     "lgt_set_fermion_action": (_i, [_vp, _i]),
     "lgt_dd_create": (_i, [C.POINTER(_vp), _ip, _i, _i, _ip, _d, _d, _ip, _i, _i, _vp]),
+    "lgt_dd_create_grid": (_i, [C.POINTER(_vp), _ip, _ip, _i, _ip, _d, _d, _ip, _i, _i, _vp]),
     "lgt_dd_destroy": (_i, [_vp]),
     "lgt_dd_last_error": (C.c_char_p, [_vp]),
     "lgt_dd_nccl_unique_id": (_i, [_vp]),
@@ -433,6 +434,18 @@ def lgt_dd_create(dims, nranks, local_ranks, beta, kappa, bc, precision=LGT_F64,
     return h
 
 
+def lgt_dd_create_grid(dims, grid, local_ranks, beta, kappa, bc, precision=LGT_F64, device=0, stream=None):
+    """Two split directions: grid = (Pt, Pz), rank = pt * Pz + pz."""
+    h = _vp()
+    d4 = (C.c_int * 4)(*[int(x) for x in dims])
+    g2 = (C.c_int * 2)(*[int(x) for x in grid])
+    b4 = (C.c_int * 4)(*[int(x) for x in bc])
+    lr = (C.c_int * len(local_ranks))(*[int(r) for r in local_ranks])
+    rc = lib().lgt_dd_create_grid(C.byref(h), d4, g2, len(local_ranks), lr, beta, kappa, b4, precision, device, stream)
+    _dd_check(None, rc)
+    return h
+
+
 def lgt_dd_destroy(d):
     lib().lgt_dd_destroy(d)
     _host_transports.pop(getattr(d, "value", None), None)
@@ -690,7 +703,8 @@ class DecomposedLattice:
     """A group of time slabs (lgt_dd_*) with numpy in / numpy out helpers.  `local_ranks` = all ranks: the
     single-device verification mode; one rank: the production mode (call nccl_init with the broadcast id)."""
 
-    def __init__(self, dims, nranks, local_ranks, beta, kappa, bc, precision=LGT_F64, device=0, stream=None):
+    def __init__(self, dims, nranks, local_ranks, beta, kappa, bc, precision=LGT_F64, device=0, stream=None, grid=None):
+        """nranks time slabs, or with grid = (Pt, Pz) a two-direction decomposition (nranks is then Pt * Pz)."""
         import torch
 
         if not torch.cuda.is_available():
@@ -702,7 +716,13 @@ class DecomposedLattice:
         self.Vloc = self.V // self.nranks
         self.cdtype = torch.complex128 if precision == LGT_F64 else torch.complex64
         self.device = torch.device("cuda", device)
-        self.d = lgt_dd_create(dims, nranks, local_ranks, beta, kappa, bc, precision, device, stream)
+        self.grid = None if grid is None else (int(grid[0]), int(grid[1]))
+        if self.grid is None:
+            self.d = lgt_dd_create(dims, nranks, local_ranks, beta, kappa, bc, precision, device, stream)
+        else:
+            if self.grid[0] * self.grid[1] != self.nranks:
+                raise ValueError("nranks must be Pt * Pz")
+            self.d = lgt_dd_create_grid(dims, self.grid, local_ranks, beta, kappa, bc, precision, device, stream)
         self.ranks = [lgt_dd_rank(self.d, i) for i in range(len(self.local_ranks))]
 
     def close(self):
@@ -717,11 +737,18 @@ class DecomposedLattice:
             pass
 
     def slab(self, a, rank):
-        """Rows of a global canonical array [V, ...] that belong to `rank` (t is the slowest index)."""
-        return a[rank * self.Vloc:(rank + 1) * self.Vloc]
+        """Rows of a global canonical array [V, ...] that belong to `rank`: a run of time slices (t is the slowest index),
+        or on a grid the block [Lt/Pt][Lz/Pz][Ly][Lx] of rank = pt * Pz + pz, flattened in lexicographic order."""
+        if self.grid is None:
+            return a[rank * self.Vloc:(rank + 1) * self.Vloc]
+        from .dist import grid_block
+
+        return grid_block(a, self.dims, self.grid, rank)
 
     def _up(self, a, rank):
-        return self.torch.from_numpy(self.slab(a, rank)).to(self.cdtype).to(self.device).contiguous()
+        import numpy as np
+
+        return self.torch.from_numpy(np.ascontiguousarray(self.slab(a, rank))).to(self.cdtype).to(self.device).contiguous()
 
     def _scatter(self, a, setter):
         for i, r in enumerate(self.local_ranks):

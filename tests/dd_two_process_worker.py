@@ -104,6 +104,40 @@ def main():
         out[halo] = {"cg_iters": it, "md_cg_iters": traj[2], "eo_cg_iters": it_eo, "launches": lgt.lgt_launch_count(dd.ranks[0])}
         dd.close()
         dist.barrier()
+    # two split directions over the same transport: the z faces are strided (one run per local time slice) and are staged
+    # through pinned memory by 2-D copies; a direction that is not split makes the rank its own neighbour
+    gdims = (8, 4, 2 * world, 2 * world)
+    gU = synth.warm_links(gdims, 0.3, 611)
+    gP = synth.gaussian_momenta(gdims, 612)
+    gb = oracle.dslash(gdims, kappa, BC, gU, synth.gaussian_spinor(gdims, 613), dagger=True)
+    _, git_ref, _, gok = oracle.cg(gdims, kappa, BC, gU, gb, 1e-12, 5000)
+    assert gok
+    grids = [(1, world), (world, 1)] + ([(2, world // 2)] if world >= 4 else [])
+    out["grid"] = {}
+    for grid in grids:
+        ref = lgt.DecomposedLattice(gdims, world, list(range(world)), beta, kappa, BC, grid=grid)
+        ref.set_links(gU)
+        ref_ds = ref.dslash(gb)[rank]
+        ref_x, ref_it, _, _ = ref.cg(gb, 1e-12, 5000)
+        ref.set_momenta(gP)
+        ref.set_pseudofermion(gb)
+        ref_traj = lgt.lgt_dd_md_trajectory(ref.d, 2, 0.03, tol=1e-13, max_iter=5000)
+        ref_U, ref_P = ref.get_links()[rank], ref.get_momenta()[rank]
+        ref.close()
+        dd = dist.decomposed_lattice(gdims, beta, kappa, BC, lgt.LGT_F64, 0, None, transport="host", grid=grid)
+        dd.set_links(gU)
+        assert np.array_equal(dd.dslash(gb)[0], ref_ds)
+        assert np.abs(dd.dslash(gb)[0] - dd.slab(oracle.dslash(gdims, kappa, BC, gU, gb), rank)).max() < 1e-12
+        xs, it, rel, ok = dd.cg(gb, 1e-12, 5000)
+        assert ok and it == git_ref == ref_it and np.array_equal(xs[0], ref_x[rank])
+        dd.set_momenta(gP)
+        dd.set_pseudofermion(gb)
+        traj = lgt.lgt_dd_md_trajectory(dd.d, 2, 0.03, tol=1e-13, max_iter=5000)
+        assert traj == ref_traj
+        assert np.array_equal(dd.get_links()[0], ref_U) and np.array_equal(dd.get_momenta()[0], ref_P)
+        out["grid"]["%dx%d" % grid] = {"cg_iters": it, "md_cg_iters": traj[2]}
+        dd.close()
+        dist.barrier()
     print(json.dumps(out), flush=True)
     dist.shutdown()
 

@@ -175,3 +175,41 @@ def test_host_transport_single_rank_is_a_copy():
     buf = np.array([1.5, 2.5])
     dist.host_allreduce(buf)
     assert buf.tolist() == [1.5, 2.5]
+
+
+def test_grid_blocks_and_neighbours():
+    import pytest
+
+    """Host logic of the (Pt, Pz) decomposition: the ranks' blocks tile the lattice exactly once in lexicographic order, and
+    the neighbour table is the periodic grid's (a direction that is not split makes a rank its own neighbour)."""
+    import numpy as np
+
+    from paper_2602_20516_b200 import dist
+
+    dims = (4, 2, 6, 4)
+    V = 4 * 2 * 6 * 4
+    a = np.arange(V * 3).reshape(V, 3)
+    for grid in ((1, 1), (2, 3), (4, 2), (1, 6)):
+        n = grid[0] * grid[1]
+        seen = np.zeros(V, dtype=int)
+        for r in range(n):
+            b = dist.grid_block(a, dims, grid, r)
+            assert b.shape == (V // n, 3)
+            sites = b[:, 0] // 3
+            assert np.all(np.diff(sites) > 0)  # lexicographic inside the block
+            t, z = sites // (4 * 2 * 6), (sites // 8) % 6
+            pt, pz = divmod(r, grid[1])
+            assert np.all(t // (4 // grid[0]) == pt) and np.all(z // (6 // grid[1]) == pz)
+            seen[sites] += 1
+            dn_t, up_t, dn_z, up_z = dist.grid_neighbours(grid, r)
+            assert dist.grid_neighbours(grid, dn_t)[1] == r and dist.grid_neighbours(grid, up_t)[0] == r
+            assert dist.grid_neighbours(grid, dn_z)[3] == r and dist.grid_neighbours(grid, up_z)[2] == r
+            if grid[0] == 1:
+                assert dn_t == up_t == r
+            if grid[1] == 1:
+                assert dn_z == up_z == r
+        assert np.all(seen == 1)
+    with pytest.raises(ValueError):
+        dist.grid_block(a, dims, (3, 1), 0)
+    with pytest.raises(ValueError):
+        dist.grid_block(a, dims, (2, 2), 4)

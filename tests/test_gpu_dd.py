@@ -120,6 +120,29 @@ def test_dd_nccl_transport_one_rank(lgt):
     dd.close()
 
 
+def test_grid_nccl_transport_one_rank(lgt):
+    """The NCCL code path of the (Pt, Pz) grid with a single rank (1 x 1): the z faces are gathered into a device staging
+    buffer by 2-D copies, sent and received (to itself) through NCCL, and scattered into the ghost planes; kick with both
+    forces (the staples' corners go through the same two phases) against the oracle."""
+    dims, beta, kappa = (8, 4, 4, 4), 5.6, 0.12
+    U = synth.warm_links(dims, 0.3, 731)
+    P0 = synth.gaussian_momenta(dims, 732)
+    b = oracle.dslash(dims, kappa, BC, U, synth.gaussian_spinor(dims, 733), dagger=True)
+    dd = lgt.DecomposedLattice(dims, 1, [0], beta, kappa, BC, grid=(1, 1))
+    lgt.lgt_dd_nccl_init(dd.d, lgt.lgt_dd_nccl_unique_id())
+    dd.set_links(U)
+    assert np.abs(dd.dslash(b)[0] - oracle.dslash(dims, kappa, BC, U, b)).max() < 1e-12
+    x_ref, it_ref, _, _ = oracle.cg(dims, kappa, BC, U, b, 1e-12, 5000)
+    xs, it, rel, ok = dd.cg(b, 1e-12, 5000)
+    assert ok and it == it_ref and np.linalg.norm(xs[0] - x_ref) < 1e-10 * np.linalg.norm(x_ref)
+    dd.set_momenta(P0)
+    dd.set_pseudofermion(b)
+    lgt.lgt_dd_md_kick(dd.d, 0.05, 1e-13, 5000)
+    P1, _, _ = oracle.kick(dims, beta, kappa, BC, U, b, P0, 0.05, 1e-13, 5000)
+    assert link_rel_err(dd.get_momenta()[0], P1)[0] < TOL64
+    dd.close()
+
+
 def test_dd_argument_checks(lgt):
     with pytest.raises(lgt.LgtError):
         lgt.lgt_dd_create((4, 4, 2, 8), 3, [0, 1, 2], 5.5, 0.1, BC)  # Lt not divisible
@@ -505,3 +528,148 @@ def test_dd_between_processes_on_one_gpu(lgt, world):
     for o in outs:
         for halo in ("exchange", "push"):
             assert o[halo]["cg_iters"] == o["cg_iters_oracle"] and o[halo]["launches"] > 0
+        assert len(o["grid"]) >= 2  # (1, world) and (world, 1): the z faces over the host transport too
+
+
+# ---- two split directions (lgt_dd_create_grid, SURVEY 8(e) "first T, then Z") -------------------------------------
+def gather_grid(dims, grid, blocks):
+    """Global canonical array from the ranks' blocks [Lt/Pt][Lz/Pz][Ly][Lx] (rank = pt * Pz + pz)."""
+    Lx, Ly, Lz, Lt = dims
+    Pt, Pz = grid
+    lt, lz = Lt // Pt, Lz // Pz
+    tail = blocks[0].shape[1:]
+    out = np.empty((Lt, Lz, Ly * Lx) + tail, dtype=blocks[0].dtype)
+    for r, b in enumerate(blocks):
+        pt, pz = divmod(r, Pz)
+        out[pt * lt:(pt + 1) * lt, pz * lz:(pz + 1) * lz] = b.reshape((lt, lz, Ly * Lx) + tail)
+    return out.reshape((Lx * Ly * Lz * Lt,) + tail)
+
+
+GRIDS = [((8, 4, 4, 4), (1, 1)), ((8, 4, 4, 4), (1, 2)), ((8, 4, 4, 4), (2, 2)), ((8, 4, 8, 4), (2, 4)), ((8, 4, 4, 4), (4, 2)),
+         ((8, 8, 6, 6), (3, 2)), ((16, 2, 4, 2), (1, 4))]
+
+
+@pytest.mark.parametrize("dims,grid", GRIDS)
+def test_grid_dslash_is_bitwise_the_undivided_kernel(lgt, dims, grid):
+    """A (Pt, Pz) grid with every rank in this process: D and D^dag bitwise equal to the undivided handle (same kernel
+    arithmetic per site; ghost time slices and ghost z planes filled by the t-then-z exchange) and equal to the oracle,
+    with an antiperiodic direction in z as well (the boundary sign goes by the global z coordinate); set / get round trip."""
+    kappa = 0.12
+    n = grid[0] * grid[1]
+    U = synth.warm_links(dims, 0.3, 701)
+    psi = synth.gaussian_spinor(dims, 702)
+    for bc in (BC, (1, 1, -1, -1)):
+        dd = lgt.DecomposedLattice(dims, n, list(range(n)), 5.5, kappa, bc, grid=grid)
+        dd.set_links(U)
+        one = lgt.Lattice(dims, 5.5, kappa, bc)
+        one.set_links(U)
+        for dag in (False, True):
+            out = gather_grid(dims, grid, dd.dslash(psi, dagger=dag))
+            assert np.abs(out - oracle.dslash(dims, kappa, bc, U, psi, dagger=dag)).max() < 1e-12
+            assert np.array_equal(out, one.dslash(psi, dagger=dag))
+        assert np.array_equal(gather_grid(dims, grid, dd.get_links()), U)
+        dd.close()
+        one.close()
+
+
+@pytest.mark.parametrize("dims,grid", [((8, 4, 4, 4), (2, 2)), ((8, 4, 8, 4), (2, 4)), ((8, 4, 4, 4), (1, 2))])
+def test_grid_cg_and_md_trajectory(lgt, dims, grid):
+    """CG with the oracle's iteration count, the actions, kick, drift and a leapfrog trajectory with both forces on the grid
+    against the oracle on the undivided lattice (the staples reach into the corners that the t-then-z exchange fills)."""
+    beta, kappa = 5.6, 0.11
+    n = grid[0] * grid[1]
+    U0 = synth.warm_links(dims, 0.25, 711)
+    P0 = synth.gaussian_momenta(dims, 712)
+    phi = oracle.dslash(dims, kappa, BC, U0, synth.gaussian_spinor(dims, 713), dagger=True)
+    dd = lgt.DecomposedLattice(dims, n, list(range(n)), beta, kappa, BC, grid=grid)
+    dd.set_links(U0)
+    xs, it, rel, ok = dd.cg(phi, 1e-12, 5000)
+    x_ref, it_ref, _, ok_ref = oracle.cg(dims, kappa, BC, U0, phi, 1e-12, 5000)
+    assert ok and ok_ref and it == it_ref
+    x = gather_grid(dims, grid, xs)
+    assert np.linalg.norm(x - x_ref) < 1e-10 * np.linalg.norm(x_ref)
+    dd.set_momenta(P0)
+    dd.set_pseudofermion(phi)
+    S_g, S_F, K, _ = lgt.lgt_dd_action(dd.d, 1e-13, 5000)
+    H_ref, K_ref, Sg_ref, SF_ref = oracle.hamiltonian(dims, beta, kappa, BC, U0, phi, P0, 1e-13, 5000)
+    assert abs(S_g - Sg_ref) < 1e-11 * abs(Sg_ref) and abs(S_F - SF_ref) < 1e-10 * abs(SF_ref) and abs(K - K_ref) < 1e-12 * K_ref
+    H0, H1, its = lgt.lgt_dd_md_trajectory(dd.d, 3, 0.03, tol=1e-13, max_iter=5000)
+    U_ref, P_ref, its_ref, ok = oracle.trajectory(dims, beta, kappa, BC, U0, phi, P0, 3, 0.03, tol=1e-13, max_iter=5000)
+    assert ok and its == its_ref
+    assert np.abs(gather_grid(dims, grid, dd.get_links()) - U_ref).max() < 1e-12
+    assert link_rel_err(gather_grid(dims, grid, dd.get_momenta()), P_ref)[0] < TOL64
+    H1_ref = oracle.hamiltonian(dims, beta, kappa, BC, U_ref, phi, P_ref, 1e-13, 5000)[0]
+    assert abs((H1 - H0) - (H1_ref - H_ref)) < 1e-9 * abs(H_ref)
+    dd.set_links(U0)
+    dd.set_momenta(P0)
+    lgt.lgt_dd_md_kick(dd.d, 0.05, 1e-13, 5000)
+    P1, _, _ = oracle.kick(dims, beta, kappa, BC, U0, phi, P0, 0.05, 1e-13, 5000)
+    assert link_rel_err(gather_grid(dims, grid, dd.get_momenta()), P1)[0] < TOL64
+    lgt.lgt_dd_md_drift(dd.d, 0.05)
+    assert np.abs(gather_grid(dims, grid, dd.get_links()) - oracle.drift(dims, 0.05, P1, U0)).max() < 1e-13
+    # what a grid does not offer
+    for call in (lambda: lgt.lgt_dd_set_halo_mode(dd.d, lgt.LGT_DD_PUSH), lambda: lgt.lgt_dd_set_fermion_action(dd.d, lgt.LGT_ACTION_EO)):
+        with pytest.raises(lgt.LgtError) as e:
+            call()
+        assert e.value.code == lgt.LGT_EINVAL
+    dd.close()
+    for bad in ((3, 1), (1, 3), (0, 2)):  # Lt % Pt, Lz % Pz, Pt < 1
+        with pytest.raises(lgt.LgtError) as e:
+            lgt.lgt_dd_create_grid(dims, bad, [0], beta, kappa, BC)
+        assert e.value.code == lgt.LGT_EINVAL
+    with pytest.raises(lgt.LgtError):  # xy planes must be whole layout blocks
+        lgt.lgt_dd_create_grid((4, 4, 4, 4), (2, 2), [0], beta, kappa, BC)
+
+
+@pytest.mark.parametrize("grid", [(2, 2), (1, 4)])
+def test_grid_hmc_mixed_solver_and_stout(lgt, grid):
+    """On the (Pt, Pz) grid: the HMC trajectory (heat baths by GLOBAL element number, here formed from the coordinates) gives
+    the oracle's momenta, pseudofermion, dH and decision on the undivided lattice; the mixed-precision solver (fp32 copies incl.
+    ghost planes, masked fp64 residual sums) and one / two levels of stout smearing (every level's planes exchanged before the
+    next, G's before the chain kernel) give the oracle's kick."""
+    from oracle import hmc as ohmc
+    from oracle import stout as ost
+
+    dims, beta, kappa, seed = (8, 4, 4, 4), 5.5, 0.10, 97531
+    n = grid[0] * grid[1]
+    U = synth.warm_links(dims, 0.2, 721)
+    dd = lgt.DecomposedLattice(dims, n, list(range(n)), beta, kappa, BC, grid=grid)
+    dd.set_links(U)
+    for traj in range(2):
+        dH, acc, its, H0, ok = lgt.lgt_dd_hmc_trajectory(dd.d, 3, 0.03, seed, traj, tol=1e-13, max_iter=5000)
+        ref = ohmc.hmc_trajectory(dims, beta, kappa, BC, U, seed, traj, 3, 0.03, ohmc.LEAPFROG, tol=1e-13, max_iter=5000)
+        assert ok and abs(H0 - ref["H0"]) < 1e-12 * abs(ref["H0"]) and abs(dH - ref["dH"]) < 1e-9 * abs(ref["H0"])
+        if abs(ref["u"] - np.exp(-ref["dH"])) > 1e-6:
+            assert acc == ref["accepted"]
+            assert np.abs(gather_grid(dims, grid, dd.get_links()) - ref["U"]).max() < 1e-11
+        U = gather_grid(dims, grid, dd.get_links())
+    dd.close()
+
+    kappa, rho = 0.11, 0.3
+    U0 = synth.warm_links(dims, 0.25, 722)
+    P0 = synth.gaussian_momenta(dims, 723)
+    psi = synth.gaussian_spinor(dims, 724)
+    dd = lgt.DecomposedLattice(dims, n, list(range(n)), beta, kappa, BC, grid=grid)
+    dd.set_links(U0)
+    phi = oracle.dslash(dims, kappa, BC, U0, psi, dagger=True)
+    dd.set_momenta(P0)
+    dd.set_pseudofermion(phi)
+    lgt.lgt_dd_set_solver(dd.d, lgt.LGT_SOLVER_MIXED_CG, 1e-5)
+    lgt.lgt_dd_md_kick(dd.d, 0.05, 1e-12, 5000)
+    P1, _, _ = oracle.kick(dims, beta, kappa, BC, U0, phi, P0, 0.05, 1e-13, 5000)
+    assert link_rel_err(gather_grid(dims, grid, dd.get_momenta()), P1)[0] < 1e-10
+    lgt.lgt_dd_set_solver(dd.d, lgt.LGT_SOLVER_CG)
+    for levels in (1, 2):
+        Un = ost.smear_levels(dims, rho, levels, U0)[0][-1]
+        phi = oracle.dslash(dims, kappa, BC, Un, psi, dagger=True)
+        lgt.lgt_dd_set_smearing(dd.d, levels, rho)
+        dd.set_links(U0)
+        assert np.abs(gather_grid(dims, grid, dd.dslash(psi)) - oracle.dslash(dims, kappa, BC, Un, psi)).max() < 1e-12
+        dd.set_momenta(P0)
+        dd.set_pseudofermion(phi)
+        it = lgt.lgt_dd_md_kick(dd.d, 0.05, 1e-13, 5000)
+        Ff, it_ref, ok = ost.fermion_force(dims, kappa, BC, U0, phi, levels, rho, 1e-13, 5000)
+        assert ok and it == it_ref
+        P_ref = P0 - 0.05 * (oracle.gauge_force(dims, beta, U0) + Ff)
+        assert link_rel_err(gather_grid(dims, grid, dd.get_momenta()), P_ref)[0] < TOL64
+    dd.close()
