@@ -437,6 +437,28 @@ template <class T> struct PushTo {
     int da = 0, db = 0;
 };
 
+// L2 prefetch of what block `b` of the Dslash grid will read from DRAM first: its forward links and its t+1 spinors
+// (one lane per 128-byte line; the warp's link block is 36 x 32 complex, its spinor block 12 x 32, both contiguous).
+template <class T>
+__device__ __forceinline__ void dslash_prefetch_block(const Geom& g, const typename Vec2<T>::type* U, const typename Vec2<T>::type* in, int b) {
+    const int sp = g.s_begin + swizzled_chunk(g, b) * blockDim.x + threadIdx.x;
+    if (sp < g.s_end) {
+        const int lane = threadIdx.x & 31;
+        constexpr int CPL = 128 / (int)sizeof(typename Vec2<T>::type);  // complex numbers per line
+        const typename Vec2<T>::type* bu = link_at(U, sp - lane, 0);
+#pragma unroll
+        for (int j = 0; j < (36 * W / CPL + 31) / 32; j++)
+            if (lane + 32 * j < 36 * W / CPL) asm volatile("prefetch.global.L2 [%0];" ::"l"(bu + (lane + 32 * j) * CPL));
+        const int spt = sp - lane + g.stride[3];
+        if (spt < g.s_end) {
+            const typename Vec2<T>::type* bp = spinor_at(in, spt);
+#pragma unroll
+            for (int j = 0; j < (12 * W / CPL + 31) / 32; j++)
+                if (lane + 32 * j < 12 * W / CPL) asm volatile("prefetch.global.L2 [%0];" ::"l"(bp + (lane + 32 * j) * CPL));
+        }
+    }
+}
+
 // PF > 0 (variant 4): every thread first asks L2 for the lines the block PF positions further on in the grid will need
 // from DRAM first -- its forward links and its t+1 spinors -- so that those loads find their data in L2 (prefetches hold
 // no registers; PF = the number of co-resident blocks, i.e. the block that takes this block's place on the SM).
@@ -450,25 +472,7 @@ __global__ void __launch_bounds__(128, 1) dslash_kernel(Geom g, const typename V
     // fused scalar update, launches past convergence: the "x, p update due" flag is cleared here instead of by cg_scalars_kernel<1>
     if (MODE == 1 && fuse && done && blockIdx.x == 0 && threadIdx.x == 0) st->fresh = 0;
     const int s = g.s_begin + swizzled_chunk(g, blockIdx.x) * blockDim.x + threadIdx.x;
-    if (PFON == 1 && blockIdx.x + pf < gridDim.x && !(MODE != 0 && done)) {
-        const int sp = g.s_begin + swizzled_chunk(g, blockIdx.x + pf) * blockDim.x + threadIdx.x;
-        if (sp < g.s_end) {
-            // one lane per 128-byte line: the warp's link block is 36 x 32 complex, its spinor block 12 x 32, both contiguous
-            const int lane = threadIdx.x & 31;
-            constexpr int CPL = 128 / (int)sizeof(typename Vec2<T>::type);  // complex numbers per line
-            const typename Vec2<T>::type* bu = link_at(U, sp - lane, 0);
-#pragma unroll
-            for (int j = 0; j < (36 * W / CPL + 31) / 32; j++)
-                if (lane + 32 * j < 36 * W / CPL) asm volatile("prefetch.global.L2 [%0];" ::"l"(bu + (lane + 32 * j) * CPL));
-            const int spt = sp - lane + g.stride[3];
-            if (spt < g.s_end) {
-                const typename Vec2<T>::type* bp = spinor_at(in, spt);
-#pragma unroll
-                for (int j = 0; j < (12 * W / CPL + 31) / 32; j++)
-                    if (lane + 32 * j < 12 * W / CPL) asm volatile("prefetch.global.L2 [%0];" ::"l"(bp + (lane + 32 * j) * CPL));
-            }
-        }
-    }
+    if (PFON == 1 && blockIdx.x + pf < gridDim.x && !(MODE != 0 && done)) dslash_prefetch_block<T>(g, U, in, blockIdx.x + pf);
     double nrm = 0.0;
     // ZS: a rank of a (Pt, Pz) grid -- the sites of its two ghost z planes are skipped like the sites past s_end
     if (s < g.s_end && (!ZS || z_owned(g, z_of_site(g, s)))) {
@@ -519,6 +523,8 @@ __global__ void __launch_bounds__(128, 1) dslash_kernel(Geom g, const typename V
         hop_fwd<3, F, T, NA>(g, U, in, c, s, acc);
         hop_bwd<3, -F, T, NA>(g, U, in, c, s, acc);
         }
+        // variant 8: the prefetch of variant 4 issued at the END of the block, ~1 us before the block that takes its place starts
+        if (PFON == 5 && blockIdx.x + pf < gridDim.x) dslash_prefetch_block<T>(g, U, in, blockIdx.x + pf);
         const typename Vec2<T>::type* bi = spinor_at(in, s);
         if (MODE == 2) {
             const T alpha = (T)st->alpha;

@@ -422,6 +422,25 @@ template <class T> struct Ops {
             }
             return LGT_OK;
         }
+        // Variant 8: variant 4's prefetch issued at the end of the block instead of its start.  It is also what the DEFAULT
+        // (variant 0) means for the fp32 kernels on lattices of one wave of blocks up to 16384 chunks: bitwise the same
+        // results, 4 - 10 % per fp32 CG iteration (16^4 ... 32^4; the inner solve of the mixed-precision solver), nothing in fp64.
+        const bool late_pf = c->variant[LGT_K_DSLASH] == 8 ||
+                             (c->variant[LGT_K_DSLASH] == 0 && sizeof(T) == 4 && grid > 2 * c->num_sms && grid <= 16384 && !c->dd_links_valid);
+        if (late_pf) {
+            const int pf = 2 * c->num_sms;
+            if (mode == 0) {
+                if (dagger)
+                    LAUNCH(c, LGT_K_DSLASH, (dslash_kernel<T, 1, 0, 0, 5>), grid, 128, DSLASH_ARGS, pf);
+                else
+                    LAUNCH(c, LGT_K_DSLASH, (dslash_kernel<T, 0, 0, 0, 5>), grid, 128, DSLASH_ARGS, pf);
+            } else if (mode == 1) {
+                LAUNCH(c, LGT_K_DSLASH, (dslash_kernel<T, 0, 1, 0, 5>), grid, 128, DSLASH_ARGS, pf, fuse_counter(c));
+            } else {
+                LAUNCH(c, LGT_K_DSLASH_R, (dslash_kernel<T, 1, 2, 0, 5>), grid, 128, DSLASH_ARGS, pf, fuse_counter(c));
+            }
+            return LGT_OK;
+        }
         if (c->variant[LGT_K_DSLASH] == 7) {  // 12-real links: rows 0 and 1 read, row 2 rebuilt in registers
             if (mode == 0) {
                 if (dagger)
@@ -1334,7 +1353,7 @@ int lgt_set_kernel_variant(lgt_ctx* c, int kernel_class, int variant, int* in_ef
     CHECK_CTX(c);
     if (kernel_class < 0 || kernel_class >= LGT_K_COUNT) return fail(c, LGT_EINVAL, "lgt_set_kernel_variant: unknown kernel class");
     if (variant >= 0) {
-        const int nvar = (kernel_class == LGT_K_DSLASH) ? 8 : (kernel_class == LGT_K_GAUGE_FORCE) ? 3 : (kernel_class == LGT_K_CG_BLAS) ? 2 : 1;
+        const int nvar = (kernel_class == LGT_K_DSLASH) ? 9 : (kernel_class == LGT_K_GAUGE_FORCE) ? 3 : (kernel_class == LGT_K_CG_BLAS) ? 2 : 1;
         if (variant >= nvar) return fail(c, LGT_EINVAL, "lgt_set_kernel_variant: this kernel class has no such variant");
         if (c->variant[kernel_class] != variant) {
             // captured CG chunks hold the old kernels
