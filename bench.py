@@ -1068,7 +1068,7 @@ def main():
                     help="non-default: time the step with the mixed-precision solver (not the headline configuration)")
     ap.add_argument("--action", default="full", choices=["full", "eo"],
                     help="non-default: time the step with the even/odd preconditioned action (not the headline configuration)")
-    ap.add_argument("--halo", default="exchange", choices=["exchange", "push"],
+    ap.add_argument("--halo", default="exchange", choices=["exchange", "push", "overlap"],
                     help="decomposed lattice: separate exchange of the halo slices, or halos stored into the neighbours' ghost "
                          "slices by the Dslash kernels (CUDA IPC between processes)")
     ap.add_argument("--transport", default="nccl", choices=["nccl", "host"],

@@ -257,7 +257,11 @@ int lgt_dd_halo_plan(int nranks, int rank, int lt_local, int plan[8]);
  *     buffers are mapped with CUDA IPC: every rank exports 128 bytes (lgt_dd_ipc_export, HOST buffer), the caller
  *     all-gathers them, every rank imports the handles of ranks r-1 and r+1 (lgt_dd_ipc_import), then switches mode.
  *     Ranks that share a process need no import.  LGT_ESTATE if a neighbour's buffers are not reachable. */
-enum { LGT_DD_EXCHANGE = 0, LGT_DD_PUSH = 1 };
+/*   LGT_DD_OVERLAP: the exchange of LGT_DD_EXCHANGE, but issued on a second stream while every slab's bulk (the time slices
+ *     that touch no ghost slice) is computed; the two boundary slices are launched once the halo has landed (SURVEY.md 8(e):
+ *     "interior/boundary kernel split to overlap").  Inside the CG loop, for time slabs of at least three slices that are
+ *     whole 128-site chunks; elsewhere it behaves as LGT_DD_EXCHANGE.  Same iterates bit for bit. */
+enum { LGT_DD_EXCHANGE = 0, LGT_DD_PUSH = 1, LGT_DD_OVERLAP = 2 };
 int lgt_dd_set_halo_mode(lgt_dd* d, int mode);
 int lgt_dd_ipc_export(lgt_dd* d, void* handles128);
 int lgt_dd_ipc_import(lgt_dd* d, const void* lo_handles128, const void* hi_handles128);

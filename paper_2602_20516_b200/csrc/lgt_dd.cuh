@@ -82,6 +82,9 @@ struct lgt_dd {
     // LGT_DD_PUSH: halos of the CG fields t (ws[3]) and r (ws[1]) are stored into the neighbours' ghost slices by the
     // producing kernels.  Neighbours in other processes: their buffers mapped through CUDA IPC, [field r, t][lo, hi].
     int halo_mode = 0;
+    // LGT_DD_OVERLAP: the exchange runs on its own stream while the slab's bulk is computed (lazy)
+    cudaStream_t halo_stream = nullptr;
+    cudaEvent_t ev_ready = nullptr, ev_halo = nullptr;
     void* ipc_peer[2][2] = {{nullptr, nullptr}, {nullptr, nullptr}};
     bool ipc_open[2][2] = {{false, false}, {false, false}};
     std::string err;
@@ -225,6 +228,9 @@ int dd_exchange_grid(lgt_dd* d, void* const* base, int per_site, size_t esize) {
             if (d->d_stage_bytes < 4 * bytes) {
                 DD_CU(cudaStreamSynchronize(d->stream));
                 if (d->d_stage) cudaFree(d->d_stage);
+    if (d->halo_stream) cudaStreamDestroy(d->halo_stream);
+    if (d->ev_ready) cudaEventDestroy(d->ev_ready);
+    if (d->ev_halo) cudaEventDestroy(d->ev_halo);
                 d->d_stage = nullptr;
                 d->d_stage_bytes = 0;
                 DD_CU(cudaMalloc(&d->d_stage, 4 * bytes));
@@ -457,6 +463,61 @@ template <class T> struct DdOps {
                             [&](const PushTo<T>* push) { return O::dslash(c, fld(c, 7), in, out, dagger, mode, r, push); });
     }
 
+    // LGT_DD_OVERLAP (time slabs, CG loop): the stencil launch over field `k` split so that the halo exchange of `k` runs on
+    // the group's halo stream WHILE the bulk of every slab (the slices that touch no ghost slice) is computed; the two
+    // boundary slices follow once the halo has landed.  Block partials land where one launch over the slab would put them:
+    // the sums, hence the iterates, are bitwise those of LGT_DD_EXCHANGE.  `launch(c)` issues the kernel for the range
+    // currently set in c->g / c->partials.
+    template <class Launch> static int overlapped(lgt_dd* d, int k, Launch launch) {
+        int rc;
+        if (!d->halo_stream) {
+            DD_CU(cudaStreamCreateWithFlags(&d->halo_stream, cudaStreamNonBlocking));
+            DD_CU(cudaEventCreateWithFlags(&d->ev_ready, cudaEventDisableTiming));
+            DD_CU(cudaEventCreateWithFlags(&d->ev_halo, cudaEventDisableTiming));
+        }
+        const int slice = d->V3, n = (int)d->rk.size();
+        DD_CU(cudaEventRecord(d->ev_ready, d->stream));  // the field is complete
+        for (int i = 0; i < n; i++) {                    // bulk: local slices 2 .. Lt_loc - 1
+            lgt_ctx* c = d->rk[i];
+            const int b0 = c->g.s_begin, e0 = c->g.s_end;
+            double* const part0 = c->partials;
+            c->g.s_begin = b0 + slice;
+            c->g.s_end = e0 - slice;
+            c->partials = part0 + slice / 128;
+            rc = launch(c);
+            c->g.s_begin = b0;
+            c->g.s_end = e0;
+            c->partials = part0;
+            if (rc != LGT_OK) return dd_fail(d, rc, c->err.c_str());
+        }
+        DD_CU(cudaStreamWaitEvent(d->halo_stream, d->ev_ready, 0));
+        cudaStream_t const main_stream = d->stream;
+        d->stream = d->halo_stream;  // dd_exchange enqueues (and, for the host transport, waits) on d->stream
+        rc = exchange_spinor(d, k);
+        d->stream = main_stream;
+        if (rc != LGT_OK) return rc;
+        DD_CU(cudaEventRecord(d->ev_halo, d->halo_stream));
+        DD_CU(cudaStreamWaitEvent(d->stream, d->ev_halo, 0));
+        for (int i = 0; i < n; i++) {  // the two boundary slices
+            lgt_ctx* c = d->rk[i];
+            const int b0 = c->g.s_begin, e0 = c->g.s_end;
+            double* const part0 = c->partials;
+            c->g.s_end = b0 + slice;
+            rc = launch(c);
+            if (rc == LGT_OK) {
+                c->g.s_begin = e0 - slice;
+                c->g.s_end = e0;
+                c->partials = part0 + (e0 - slice - b0) / 128;
+                rc = launch(c);
+            }
+            c->g.s_begin = b0;
+            c->g.s_end = e0;
+            c->partials = part0;
+            if (rc != LGT_OK) return dd_fail(d, rc, c->err.c_str());
+        }
+        return LGT_OK;
+    }
+
     // Thin-link ghosts current, then the fermions' links c->Uf of every rank: the thin links, or the stout levels built
     // in lockstep with a halo exchange of each level's result (the next level's staples reach into the ghost slices).
     static int fermion_links(lgt_dd* d) {
@@ -562,6 +623,8 @@ template <class T> struct DdOps {
         // pushed halos need the neighbours' buffers of THIS precision: always there for local neighbours, mapped through
         // IPC only for the handle's own precision
         const bool push = d->halo_mode == LGT_DD_PUSH && d->V3 % 128 == 0 && (d->rk.size() == (size_t)d->nranks || !fp32_on_f64(d->rk[0]));
+        // LGT_DD_OVERLAP: time slabs of at least three slices whose slices are whole 128-site chunks; else plain exchange
+        const bool overlap = d->halo_mode == LGT_DD_OVERLAP && d->Pz == 0 && d->V3 % 128 == 0 && d->Lt_loc >= 3;
         std::vector<Neighbours<T>> push_t(n), push_r(n);
         if (push) {
             // r = p = b on the ghost slices too (one ordinary exchange of b); from here on p's ghosts follow by local
@@ -595,20 +658,25 @@ template <class T> struct DdOps {
             if (chunk > 8) chunk = 8;
             if (chunk <= 0) chunk = 1;
             for (int it = 0; it < chunk; it++) {
-                if (!push && (rc = exchange_spinor(d, 2)) != LGT_OK) return rc;  // p
+                if (overlap) {
+                    if ((rc = overlapped(d, 2, [&](lgt_ctx* c) { return O::dslash(c, fld(c, 7), fld(c, 2), fld(c, 3), 0, 1); })) != LGT_OK) return rc;
+                } else if (!push && (rc = exchange_spinor(d, 2)) != LGT_OK) return rc;  // p
                 for (int i = 0; i < n; i++) {
                     lgt_ctx* c = d->rk[i];
                     if (push) DD_RK(i, dslash_pushing(d, c, fld(c, 2), fld(c, 3), 0, 1, nullptr, push_t[i]));
-                    else DD_RK(i, O::dslash(c, fld(c, 7), fld(c, 2), fld(c, 3), 0, 1));  // t = D p, partials of |t|^2
+                    else if (!overlap) DD_RK(i, O::dslash(c, fld(c, 7), fld(c, 2), fld(c, 3), 0, 1));  // t = D p, partials of |t|^2
                     LAUNCH(c, LGT_K_CG_BLAS, cg_partial_sum_kernel, 1, 1024, site_blocks(c, 128), c->partials, c->st);
                 }
                 if ((rc = allreduce_tmp(d)) != LGT_OK) return rc;
                 for (int i = 0; i < n; i++) LAUNCH(d->rk[i], LGT_K_CG_BLAS, (cg_apply_kernel<1>), 1, 1, d->rk[i]->st);
-                if (!push && (rc = exchange_spinor(d, 3)) != LGT_OK) return rc;  // t
+                if (overlap) {
+                    if ((rc = overlapped(d, 3, [&](lgt_ctx* c) { return O::dslash(c, fld(c, 7), fld(c, 3), nullptr, 1, 2, fld(c, 1)); })) != LGT_OK)
+                        return rc;
+                } else if (!push && (rc = exchange_spinor(d, 3)) != LGT_OK) return rc;  // t
                 for (int i = 0; i < n; i++) {
                     lgt_ctx* c = d->rk[i];
                     if (push) DD_RK(i, dslash_pushing(d, c, fld(c, 3), nullptr, 1, 2, fld(c, 1), push_r[i]));
-                    else DD_RK(i, O::dslash(c, fld(c, 7), fld(c, 3), nullptr, 1, 2, fld(c, 1)));  // r -= alpha D^dag t, partials of |r|^2
+                    else if (!overlap) DD_RK(i, O::dslash(c, fld(c, 7), fld(c, 3), nullptr, 1, 2, fld(c, 1)));  // r -= alpha D^dag t, partials of |r|^2
                     LAUNCH(c, LGT_K_CG_BLAS, cg_partial_sum_kernel, 1, 1024, site_blocks(c, 128), c->partials, c->st);
                 }
                 if ((rc = allreduce_tmp(d)) != LGT_OK) return rc;
@@ -1356,7 +1424,7 @@ int lgt_dd_nccl_init(lgt_dd* d, const void* id128) {
 
 int lgt_dd_set_halo_mode(lgt_dd* d, int mode) {
     CHECK_DD(d);
-    if (mode != LGT_DD_EXCHANGE && mode != LGT_DD_PUSH) return dd_fail(d, LGT_EINVAL, "lgt_dd_set_halo_mode: unknown mode");
+    if (mode != LGT_DD_EXCHANGE && mode != LGT_DD_PUSH && mode != LGT_DD_OVERLAP) return dd_fail(d, LGT_EINVAL, "lgt_dd_set_halo_mode: unknown mode");
     if (mode == LGT_DD_PUSH && d->Pz > 0) return dd_fail(d, LGT_EINVAL, "lgt_dd_set_halo_mode: LGT_DD_PUSH is for time slabs; a (Pt, Pz) grid exchanges");
     if (mode == LGT_DD_PUSH && d->rk.size() != (size_t)d->nranks && d->nranks > 1)
         for (int f = 0; f < 2; f++)

@@ -183,6 +183,8 @@ def decomposed_lattice(dims, beta, kappa, bc, precision=None, local_device=0, st
         lgt.lgt_dd_ipc_import(dd.d, handles[(rank - 1) % world], handles[(rank + 1) % world])
     if halo == "push":
         lgt.lgt_dd_set_halo_mode(dd.d, lgt.LGT_DD_PUSH)
+    elif halo == "overlap":
+        lgt.lgt_dd_set_halo_mode(dd.d, lgt.LGT_DD_OVERLAP)
     return dd
 
 

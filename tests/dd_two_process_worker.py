@@ -104,6 +104,24 @@ def main():
         out[halo] = {"cg_iters": it, "md_cg_iters": traj[2], "eo_cg_iters": it_eo, "launches": lgt.lgt_launch_count(dd.ranks[0])}
         dd.close()
         dist.barrier()
+    # LGT_DD_OVERLAP between processes: slabs of four slices, the exchange (host transport, on the group's halo stream) under
+    # the bulk kernel, boundary slices after it; bitwise the plain exchange
+    odims = (8, 4, 4, 4 * world)
+    oU = synth.warm_links(odims, 0.3, 621)
+    ob = oracle.dslash(odims, kappa, BC, oU, synth.gaussian_spinor(odims, 622), dagger=True)
+    _, oit_ref, _, ook = oracle.cg(odims, kappa, BC, oU, ob, 1e-12, 5000)
+    ores = {}
+    for halo in ("exchange", "overlap"):
+        dd = dist.decomposed_lattice(odims, beta, kappa, BC, lgt.LGT_F64, 0, None, halo=halo, transport="host")
+        dd.set_links(oU)
+        xs, it, rel, ok = dd.cg(ob, 1e-12, 5000)
+        assert ook and ok and it == oit_ref
+        ores[halo] = xs[0]
+        dd.close()
+        dist.barrier()
+    assert np.array_equal(ores["exchange"], ores["overlap"])
+    out["overlap_cg_iters"] = oit_ref
+
     # two split directions over the same transport: the z faces are strided (one run per local time slice) and are staged
     # through pinned memory by 2-D copies; a direction that is not split makes the rank its own neighbour
     gdims = (8, 4, 2 * world, 2 * world)

@@ -216,7 +216,7 @@ def test_dd_pushed_halos_are_bitwise_the_exchanged_ones(lgt, nranks):
     b = oracle.dslash(dims, kappa, BC, U, synth.gaussian_spinor(dims, 563), dagger=True)
     x_ref, it_ref, _, ok = oracle.cg(dims, kappa, BC, U, b, 1e-12, 5000)
     res = {}
-    for mode in (lgt.LGT_DD_EXCHANGE, lgt.LGT_DD_PUSH):
+    for mode in (lgt.LGT_DD_EXCHANGE, lgt.LGT_DD_PUSH, lgt.LGT_DD_OVERLAP):
         dd = lgt.DecomposedLattice(dims, nranks, list(range(nranks)), beta, kappa, BC)
         lgt.lgt_dd_set_halo_mode(dd.d, mode)
         dd.set_links(U)
@@ -230,6 +230,11 @@ def test_dd_pushed_halos_are_bitwise_the_exchanged_ones(lgt, nranks):
     ex, pu = res[lgt.LGT_DD_EXCHANGE], res[lgt.LGT_DD_PUSH]
     assert np.array_equal(ex[0], pu[0]) and np.array_equal(ex[1], pu[1]) and np.array_equal(ex[2], pu[2])
     assert ex[3] == pu[3] and ex[4] == pu[4]
+    # LGT_DD_OVERLAP: the exchange on a second stream under the bulk of the slab, the boundary slices after it (slabs of
+    # three and more slices: 1 and 2 slabs here; thinner slabs fall back to the plain exchange) -- the same bits again
+    ov = res[lgt.LGT_DD_OVERLAP]
+    assert np.array_equal(ex[0], ov[0]) and np.array_equal(ex[1], ov[1]) and np.array_equal(ex[2], ov[2])
+    assert ex[3] == ov[3] and ex[4] == ov[4]
     assert np.linalg.norm(pu[0] - x_ref) < 1e-10 * np.linalg.norm(x_ref)
     U_ref, P_ref, its_ref, _ = oracle.trajectory(dims, beta, kappa, BC, U, b, P0, 2, 0.03, tol=1e-13, max_iter=5000)
     assert pu[4] == its_ref and np.abs(pu[1] - U_ref).max() < 1e-12 and link_rel_err(pu[2], P_ref)[0] < TOL64
