@@ -52,12 +52,12 @@ FLOPS = dict(dslash=1368, dslash_fused_r=1368 + 96, cg_update_xp=96, cg_iter=2 *
 # dram__bytes_read.sum + dram__bytes_write.sum per launch at 32^4 fp64 from the ncu --set full captures summarised in
 # profiles/ (the file named beside each figure); None = not captured for the current kernel.
 NCU_TRAFFIC_BYTES = {
-    "dslash": 1019771616,          # profiles/r01f_ncu_cg.md, dslash_kernel<double,0,1,0>: 1.0198 GB
-    "dslash_fused_r": 1224798400,  # profiles/r01f_ncu_cg.md, dslash_kernel<double,1,2,0>: 1.2248 GB
-    "cg_update_xp": 955738424,     # profiles/r01f_ncu_cg.md, cg_update_xp_kernel<double>: 0.9557 GB
-    "fermion_force": 1545000000,   # profiles/r01c_forces.md, fermion_force_kernel<double,1>: 1.289 + 0.256 GB
-    "gauge_force": None,
-    "link_update": None,
+    "dslash": 1022402560,          # profiles/r02b_bench_kernels.md, dslash_kernel<double,0,1>: 0.831 + 0.192 GB
+    "dslash_fused_r": 1226198936,  # profiles/r02b_bench_kernels.md, dslash_kernel<double,1,2>: 1.036 + 0.191 GB
+    "cg_update_xp": 954585528,     # profiles/r02b_bench_kernels.md, cg_update_xp_kernel<double>: 0.604 + 0.351 GB
+    "fermion_force": 1545540064,   # profiles/r02b_bench_kernels.md, fermion_force_kernel<double,1>: 1.290 + 0.256 GB
+    "gauge_force": 1237131631,     # profiles/r02b_bench_kernels.md, gauge_force_kernel<double,1,1>: 0.974 + 0.263 GB
+    "link_update": 1421068328,     # profiles/r02b_bench_kernels.md, link_update_kernel<double>: 0.872 + 0.549 GB
 }
 
 # even/odd action, per site of the FULL lattice: a half-lattice hop reads 8 links + 1 spinor and writes 1 spinor per
