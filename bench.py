@@ -82,7 +82,8 @@ VARIANT_NAMES = {
                "variant 0 + the L2 prefetch of variant 4 issued at the end of each block (the fp32 default)"],
     "gauge_force": ["one 32-site layout block x 4 directions per 128-thread block (default)",
                     "two layout blocks per 256-thread block",
-                    "four layout blocks per 512-thread block (128 registers)"],
+                    "four layout blocks per 512-thread block (128 registers)",
+                    "one thread per site: up staples plaquette by plaquette (3 products serve 2 links), 46 instead of 52 products per site"],
 }
 
 

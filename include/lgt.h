@@ -371,6 +371,8 @@ int lgt_set_block_swizzle(lgt_ctx* ctx, int z_planes, int* in_effect);
  *         that have drifted from unitarity by delta change the operator by O(delta).
  *   LGT_K_GAUGE_FORCE: 0 = one 32-site layout block x 4 directions per 128-thread block (default, fastest);
  *     1 / 2 = two / four layout blocks per 256- / 512-thread block (more sharing through L1; measured slower).  Same sums bit for bit.
+ *     3 = one thread per site: the down staples link by link, the up staples plaquette by plaquette (U_mu(s) U_nu(s+mu)
+ *         (U_nu(s) U_mu(s+nu))^dag serves the links (s, mu) and (s, nu)): 46 instead of 52 products per site; measured slower.
  *   LGT_K_CG_BLAS: 0 = the CG scalar updates (alpha; beta, count, stop test) as one-block kernels between the stencil
  *     kernels (default); 1 = fused into the stencil kernels: the block that finishes last forms the same fixed-order sum
  *     and applies the update (two launches fewer per iteration, bitwise the same iterates; measured slower: the fence

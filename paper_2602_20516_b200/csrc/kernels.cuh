@@ -1184,6 +1184,92 @@ __global__ void __launch_bounds__(128 * ROWS, ROWS == 1 ? 2 : 1)
     store_force<T, ACC>(P, s, mu, f, eps);
 }
 
+// Variant 3 of LGT_K_GAUGE_FORCE: one thread per SITE, all four links.  The up staples are taken plaquette by plaquette:
+// with t1 = U_mu(s) U_nu(s+mu), t2 = U_nu(s) U_mu(s+nu), the plaquette P = t1 t2^dag is U_mu(s) times the up staple of
+// (s, mu) in direction nu, and P^dag is U_nu(s) times the up staple of (s, nu) in direction mu, and P_su(3)[P^dag] =
+// -P_su(3)[P]: three products serve two links (18 per site instead of 24 + their share of the final U V).  The down
+// staples go link by link as in gauge_force_kernel (their sum multiplied by the link once).  46 products per site
+// instead of 52, and the site's links and forward neighbours are loaded once per site instead of once per link.
+// P_su(3) is linear, so the eight reals of each link's force are accumulated directly.
+template <class T> __device__ __forceinline__ void ta_accumulate(const cx<T> m[9], T sign, T acc[8]) {
+    T f[8];
+    ta_compact(m, sign, f);
+#pragma unroll
+    for (int q = 0; q < 8; q++) acc[q] += f[q];
+}
+template <class T, int ACC>
+__global__ void __launch_bounds__(128, 1) gauge_force_site_kernel(Geom g, const typename Vec2<T>::type* __restrict__ U,
+                                                                  typename Vec2<T>::type* __restrict__ P, T beta_over_6, T eps) {
+    // the 4 x 8 force components of the site accumulate in shared memory (one private column per thread): in registers
+    // they push the kernel over 255 and it spills 1.6 KB per thread
+    __shared__ T accs[32][128];
+    const int s = g.s_begin + swizzled_chunk(g, blockIdx.x) * blockDim.x + threadIdx.x;
+    if (s >= g.s_end) return;
+    const Site c = site_coords(g, s);
+    if (!z_owned(g, c.x[2])) return;
+    const int tid = threadIdx.x;
+    // down staples: V = sum_nu (U_mu(s-nu) U_nu(s+mu-nu))^dag U_nu(s-nu), then P_su(3)[U_mu(s) V].  The loops over links
+    // and planes are real loops (fully unrolled, the loads of all 46 products are hoisted and spill 2 KB per thread).
+#pragma unroll 1
+    for (int mu = 0; mu < 4; mu++) {
+        const int smu = nbr_fwd(g, c, s, mu);
+        Site cm = c;
+        cm.x[mu] = (c.x[mu] == g.L[mu] - 1) ? 0 : c.x[mu] + 1;
+        cx<T> V[9];
+        mat_zero(V);
+#pragma unroll
+        for (int k = 0; k < 3; k++) {
+            const int nu = k + (k >= mu ? 1 : 0);
+            cx<T> a[9], b[9], t[9], r[9];
+            const int sdn = nbr_bwd(g, c, s, nu);
+            const int smudn = nbr_bwd(g, cm, smu, nu);
+            load_link<T>(U, mu, sdn, a);
+            load_link<T>(U, nu, smudn, b);
+            mul_nn(a, b, t);
+            load_link<T>(U, nu, sdn, a);
+            mul_dn(t, a, r);
+#pragma unroll
+            for (int q = 0; q < 9; q++) V[q] = V[q] + r[q];
+        }
+        cx<T> u[9], M[9];
+        load_link<T>(U, mu, s, u);
+        mul_nn(u, V, M);
+        T f[8];
+        ta_compact(M, (T)1, f);
+#pragma unroll
+        for (int q = 0; q < 8; q++) accs[8 * mu + q][tid] = f[q];
+    }
+    // up staples, plaquette by plaquette: planes (0,1) (0,2) (0,3) (1,2) (1,3) (2,3)
+#pragma unroll 1
+    for (int pl_i = 0; pl_i < 6; pl_i++) {
+        const int mu = pl_i < 3 ? 0 : (pl_i < 5 ? 1 : 2);
+        const int nu = pl_i < 3 ? pl_i + 1 : (pl_i < 5 ? pl_i - 1 : 3);
+        const int smu = nbr_fwd(g, c, s, mu), snu = nbr_fwd(g, c, s, nu);
+        cx<T> a[9], b[9], t1[9], t2[9], pl[9];
+        load_link<T>(U, mu, s, a);
+        load_link<T>(U, nu, smu, b);
+        mul_nn(a, b, t1);
+        load_link<T>(U, nu, s, a);
+        load_link<T>(U, mu, snu, b);
+        mul_nn(a, b, t2);
+        mul_nd(t1, t2, pl);
+        T f[8];
+        ta_compact(pl, (T)1, f);
+#pragma unroll
+        for (int q = 0; q < 8; q++) {
+            accs[8 * mu + q][tid] += f[q];
+            accs[8 * nu + q][tid] -= f[q];
+        }
+    }
+#pragma unroll 1
+    for (int mu = 0; mu < 4; mu++) {
+        T f[8];
+#pragma unroll
+        for (int q = 0; q < 8; q++) f[q] = beta_over_6 * accs[8 * mu + q][tid];
+        store_force<T, ACC>(P, s, mu, f, eps);
+    }
+}
+
 // ---------------------------------------------------------------------------- A6: link update
 // U_mu(s) <- exp(eps Pi_mu(s)) U_mu(s) with exp(iQ), Q = -i eps Pi traceless Hermitian, by the Cayley-Hamilton
 // form of the paper's ref. [6]: exp(iQ) = f0 + f1 Q + f2 Q^2.

@@ -616,6 +616,12 @@ template <class T> struct Ops {
     static int gauge_force(lgt_ctx* c, void* P, int acc, double eps) {
         const int grid = site_blocks(c, 32);
         const int v = c->variant[LGT_K_GAUGE_FORCE];
+        if (v == 3) {  // one thread per site, up staples plaquette by plaquette
+            const int g1 = site_blocks(c, 128);
+            if (acc) LAUNCH(c, LGT_K_GAUGE_FORCE, (gauge_force_site_kernel<T, 1>), g1, 128, c->g, (const T2*)c->U, (T2*)P, (T)(c->beta / 6.0), (T)eps);
+            else LAUNCH(c, LGT_K_GAUGE_FORCE, (gauge_force_site_kernel<T, 0>), g1, 128, c->g, (const T2*)c->U, (T2*)P, (T)(c->beta / 6.0), (T)eps);
+            return LGT_OK;
+        }
         if (v == 1 || v == 2) {  // 2 / 4 layout blocks per thread block
             const int rows = 2 * v, g4 = site_blocks(c, 128) * (4 / rows);
 #define GF_ARGS c->g, (const T2*)c->U, (T2*)P, (T)(c->beta / 6.0), (T)eps
@@ -1353,7 +1359,7 @@ int lgt_set_kernel_variant(lgt_ctx* c, int kernel_class, int variant, int* in_ef
     CHECK_CTX(c);
     if (kernel_class < 0 || kernel_class >= LGT_K_COUNT) return fail(c, LGT_EINVAL, "lgt_set_kernel_variant: unknown kernel class");
     if (variant >= 0) {
-        const int nvar = (kernel_class == LGT_K_DSLASH) ? 9 : (kernel_class == LGT_K_GAUGE_FORCE) ? 3 : (kernel_class == LGT_K_CG_BLAS) ? 2 : 1;
+        const int nvar = (kernel_class == LGT_K_DSLASH) ? 9 : (kernel_class == LGT_K_GAUGE_FORCE) ? 4 : (kernel_class == LGT_K_CG_BLAS) ? 2 : 1;
         if (variant >= nvar) return fail(c, LGT_EINVAL, "lgt_set_kernel_variant: this kernel class has no such variant");
         if (c->variant[kernel_class] != variant) {
             // captured CG chunks hold the old kernels

@@ -121,6 +121,31 @@ def test_dslash_kernel_variants(lgt, dims):
     lat.close()
 
 
+@pytest.mark.parametrize("dims", [(8, 8, 8, 8), (4, 3, 5, 6), (16, 4, 6, 2)])
+def test_gauge_force_kernel_variants(lgt, dims):
+    """The implementation variants of the staple kernel (lgt_set_kernel_variant(LGT_K_GAUGE_FORCE)): 1 and 2 only regroup the
+    link threads into bigger blocks (the same sums bit for bit), 3 is one thread per site with the up staples taken plaquette
+    by plaquette (another summation order: per link 1e-13 of the oracle like the default)."""
+    U = synth.haar_links(dims, 47)
+    ref = oracle.gauge_force(dims, 5.7, U)
+    lat = lgt.Lattice(dims, 5.7, 0.0, BC)
+    lat.set_links(U)
+    base = lat.gauge_force()
+    assert link_rel_err(base, ref)[0] < 1e-13
+    for v in (1, 2, 3):
+        assert lgt.lgt_set_kernel_variant(lat.ctx, lgt.LGT_K_GAUGE_FORCE, v) == v
+        F = lat.gauge_force()
+        if v < 3:
+            assert np.array_equal(F, base)
+        assert link_rel_err(F, ref)[0] < 1e-13
+        lat.set_momenta(np.zeros_like(ref))
+        lgt.lgt_gauge_force_accumulate(lat.ctx, 0.5)  # the fused Pi -= eps F form of the same variant
+        assert link_rel_err(lat.get_momenta(), -0.5 * ref)[0] < 1e-13
+    with pytest.raises(lgt.LgtError):
+        lgt.lgt_set_kernel_variant(lat.ctx, lgt.LGT_K_GAUGE_FORCE, 4)
+    lat.close()
+
+
 @pytest.mark.parametrize("dims", [(8, 8, 8, 8), (6, 4, 10, 6), (4, 3, 5, 6)])
 def test_cg_fused_scalar_update_variant(lgt, dims):
     """Variant 1 of LGT_K_CG_BLAS: the CG scalar updates ride in the last block of the stencil kernels (ticket counter)
