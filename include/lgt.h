@@ -376,7 +376,12 @@ int lgt_set_block_swizzle(lgt_ctx* ctx, int z_planes, int* in_effect);
  *   LGT_K_CG_BLAS: 0 = the CG scalar updates (alpha; beta, count, stop test) as one-block kernels between the stencil
  *     kernels (default); 1 = fused into the stencil kernels: the block that finishes last forms the same fixed-order sum
  *     and applies the update (two launches fewer per iteration, bitwise the same iterates; measured slower: the fence
- *     and ticket at the end of every block cost more than the two short launches).
+ *     and ticket at the end of every block cost more than the two short launches);
+ *     2 = the whole even/odd CG (lgt_eo_cg, and the inner fp32 solve of the mixed-precision even/odd solver) as ONE cooperative
+ *     launch: the four hops and the x / p update of an iteration are phases separated by grid barriers, every block forms the two
+ *     sums itself from the same block partials in the same order (bitwise the same iterates and count; undivided lattices;
+ *     the full-operator CG is not affected).  Measured slower at every size from 8^4 to 32^4 (a graph-launched kernel
+ *     boundary costs about 1 us on this GPU, a grid barrier with its L1 invalidation more).
  * variant < 0 only queries.  The value in effect is returned through *in_effect (may be NULL).
  * LGT_EINVAL for an unknown class or variant. */
 int lgt_set_kernel_variant(lgt_ctx* ctx, int kernel_class, int variant, int* in_effect);

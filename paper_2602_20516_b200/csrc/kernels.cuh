@@ -149,7 +149,7 @@ __device__ __forceinline__ int folded_sign(const Geom& g, int mu, int xmu) {
 template <class T, int NA = 0> __device__ __forceinline__ void load_spinor(const typename Vec2<T>::type* f, int s, cx<T> p[12]) {
     const typename Vec2<T>::type* b = spinor_at(f, s);
 #pragma unroll
-    for (int k = 0; k < 12; k++) p[k] = NA ? ldc_na(b + k * W) : ldc<T>(b + k * W);
+    for (int k = 0; k < 12; k++) p[k] = (NA == 3) ? ldc_rw<T>(b + k * W) : NA ? ldc_na(b + k * W) : ldc<T>(b + k * W);  // 3: coherent (field written in this launch)
 }
 
 // ---------------------------------------------------------------------------- deterministic reductions
@@ -1697,24 +1697,24 @@ __device__ __forceinline__ Site cb_coords(const Geom& g, int p, int c, int& s) {
 }
 
 // acc += (1 + SG gamma_MU) U_MU(s) in(s+MU): link of the output site's parity (Up), spinor of the other parity
-template <int MU, int SG, class T>
+template <int MU, int SG, class T, int COH = 0>
 __device__ __forceinline__ void hop_fwd_cb(const Geom& g, const typename Vec2<T>::type* Up, const typename Vec2<T>::type* in,
                                            const Site& cs, int s, int c, cx<T> acc[12]) {
     const int cn = nbr_fwd(g, cs, s, MU) >> 1;
     cx<T> p[12], h[6], u[9], w[6];
-    load_spinor<T>(in, cn, p);
+    load_spinor<T, COH ? 3 : 0>(in, cn, p);
     load_link<T>(Up, MU, c, u);
     spin_project<MU, SG>(p, h);
     su3_mul_half(u, h, w);
     spin_reconstruct_add<MU, SG>(w, acc);
 }
 // acc += (1 + SG gamma_MU) U_MU^dag(s-MU) in(s-MU): link and spinor of the other parity (Uq, in)
-template <int MU, int SG, class T>
+template <int MU, int SG, class T, int COH = 0>
 __device__ __forceinline__ void hop_bwd_cb(const Geom& g, const typename Vec2<T>::type* Uq, const typename Vec2<T>::type* in,
                                            const Site& cs, int s, cx<T> acc[12]) {
     const int cn = nbr_bwd(g, cs, s, MU) >> 1;
     cx<T> p[12], h[6], u[9], w[6];
-    load_spinor<T>(in, cn, p);
+    load_spinor<T, COH ? 3 : 0>(in, cn, p);
     load_link<T>(Uq, MU, cn, u);
     spin_project<MU, SG>(p, h);
     su3_dag_mul_half(u, h, w);
@@ -1802,6 +1802,183 @@ __global__ void __launch_bounds__(128, 1) hop_cb_kernel(Geom g, int p, const typ
     if (MODE == 1 || MODE == 2) {
         block_partial(nrm, partials);
         if (fuse) cg_fused_tail<MODE>(st, partials, fuse);
+    }
+}
+
+// ---------------------------------------------------------------------------- the whole even/odd CG in ONE cooperative kernel
+// Small lattices (the paper's own sizes: 16^4 down to 6^4) are bound by launches: an iteration of the
+// even/odd CG is seven kernels of a few microseconds each.  Here one cooperative launch runs the iterations until the
+// stop test fires: every block owns the 128-site chunks blockIdx, blockIdx + gridDim, ... of a half field, the four hops and
+// the x / p update of an iteration are phases separated by grid syncs (5 per iteration instead of 7 launches), and the
+// two sums of an iteration are formed by EVERY block from the same block partials in the same fixed order (cg_fixed_sum), so
+// all blocks hold bitwise the same alpha, beta and stop decision without a broadcast.  The per-site arithmetic, the block
+// partials and the order of the sums are those of hop_cb_kernel / cg_scalars_kernel / cg_update_xp_kernel: the iterates
+// and the iteration count are bitwise those of the kernel-per-phase path (tests).  State in: CgState as cg_init_kernel left
+// it; state out: as after the last cg_scalars_kernel<2>.
+// One parity of val = self - kap (H in) for the half-field index c (DAG: gamma -> -gamma), as in hop_cb_kernel.
+template <class T, int DAG>
+__device__ __forceinline__ void hop_cb_value(const Geom& g, int p, const typename Vec2<T>::type* Up, const typename Vec2<T>::type* Uq,
+                                             const typename Vec2<T>::type* in, int c, cx<T> acc[12]) {
+    int s;
+    const Site cs = cb_coords(g, p, c, s);
+#pragma unroll
+    for (int k = 0; k < 12; k++) acc[k] = mk<T>(0, 0);
+    constexpr int F = DAG ? +1 : -1;
+    hop_fwd_cb<0, F, T, 1>(g, Up, in, cs, s, c, acc);
+    hop_bwd_cb<0, -F, T, 1>(g, Uq, in, cs, s, acc);
+    hop_fwd_cb<1, F, T, 1>(g, Up, in, cs, s, c, acc);
+    hop_bwd_cb<1, -F, T, 1>(g, Uq, in, cs, s, acc);
+    hop_fwd_cb<2, F, T, 1>(g, Up, in, cs, s, c, acc);
+    hop_bwd_cb<2, -F, T, 1>(g, Uq, in, cs, s, acc);
+    hop_fwd_cb<3, F, T, 1>(g, Up, in, cs, s, c, acc);
+    hop_bwd_cb<3, -F, T, 1>(g, Uq, in, cs, s, acc);
+}
+// MODE 0: out = val; MODE 1: out = val, returns |val|^2; MODE 2: r -= alpha val, returns |r|^2  (padding lanes: zeros / nothing)
+template <class T, int DAG, int MODE>
+__device__ __forceinline__ double hop_cb_phase(const Geom& g, int p, const typename Vec2<T>::type* Up, const typename Vec2<T>::type* Uq,
+                                               const typename Vec2<T>::type* in, const typename Vec2<T>::type* self,
+                                               typename Vec2<T>::type* out, T kap, T alpha, typename Vec2<T>::type* r, int c) {
+    double nrm = 0.0;
+    if (c < g.Vh) {
+        cx<T> acc[12];
+        hop_cb_value<T, DAG>(g, p, Up, Uq, in, c, acc);
+        if (MODE == 2) {
+            const typename Vec2<T>::type* bi = spinor_at(self, c);
+            typename Vec2<T>::type* br = spinor_at(r, c);
+#pragma unroll
+            for (int k = 0; k < 12; k++) {
+                cx<T> sv = ldc_rw<T>(bi + k * W);
+                cx<T> q = mk<T>(fma(-kap, acc[k].re, sv.re), fma(-kap, acc[k].im, sv.im));
+                cx<T> rv = ldc_rw<T>(br + k * W);
+                rv.re = fma(-alpha, q.re, rv.re);
+                rv.im = fma(-alpha, q.im, rv.im);
+                stc<T>(br + k * W, rv);
+                nrm += (double)rv.re * (double)rv.re + (double)rv.im * (double)rv.im;
+            }
+        } else {
+            typename Vec2<T>::type* bo = spinor_at(out, c);
+#pragma unroll
+            for (int k = 0; k < 12; k++) {
+                cx<T> sv = mk<T>(0, 0);
+                if (self) sv = ldc_rw<T>(spinor_at(self, c) + k * W);
+                cx<T> o = mk<T>(fma(-kap, acc[k].re, sv.re), fma(-kap, acc[k].im, sv.im));
+                stc<T>(bo + k * W, o);
+                if (MODE == 1) nrm += (double)o.re * (double)o.re + (double)o.im * (double)o.im;
+            }
+        }
+    } else if (c < g.Vhs && MODE != 2) {
+        typename Vec2<T>::type* bo = spinor_at(out, c);
+#pragma unroll
+        for (int k = 0; k < 12; k++) stc<T>(bo + k * W, mk<T>(0, 0));
+    }
+    return nrm;
+}
+// grid-wide barrier of a cooperative launch (all blocks co-resident): arrive with release, spin with acquire on a
+// monotone counter; `target` = blocks x (number of barriers passed so far + 1)
+__device__ __forceinline__ void coop_grid_sync(unsigned* counter, unsigned target) {
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        __threadfence();
+        atomicAdd(counter, 1u);
+        while (*((volatile unsigned*)counter) < target) {
+        }
+        __threadfence();
+    }
+    __syncthreads();
+}
+template <class T>
+__global__ void __launch_bounds__(128, 1) eo_cg_coop_kernel(Geom g, const typename Vec2<T>::type* __restrict__ U0,
+                                                            const typename Vec2<T>::type* __restrict__ U1,
+                                                            typename Vec2<T>::type* x, typename Vec2<T>::type* r, typename Vec2<T>::type* p,
+                                                            typename Vec2<T>::type* u, typename Vec2<T>::type* t, T kappa, CgState* st,
+                                                            double* partials, unsigned* sync_counter, int nchunks) {
+    typedef typename Vec2<T>::type T2;
+    __shared__ double sums[32];
+    __shared__ double bcast;
+    double rr = st->rr;
+    const double bb = st->bb, tol2 = st->tol2;
+    int iter = st->iter, done = st->done;
+    const int max_iter = st->max_iter;
+    double alpha = 0.0, beta = 0.0, pAp = 0.0;
+    unsigned barriers = 0;
+    const unsigned nblk = gridDim.x;
+    while (!done) {
+        // t_o = kappa H_oe p_e
+        for (int ch = blockIdx.x; ch < nchunks; ch += nblk)
+            hop_cb_phase<T, 0, 0>(g, 1, U1, U0, p, (const T2*)nullptr, t, (T)-kappa, (T)0, (T2*)nullptr, ch * 128 + (int)threadIdx.x);
+        coop_grid_sync(sync_counter, nblk * ++barriers);
+        // u_e = p_e - kappa H_eo t_o, block partials of |u|^2
+        for (int ch = blockIdx.x; ch < nchunks; ch += nblk) {
+            const double nrm = hop_cb_phase<T, 0, 1>(g, 0, U0, U1, t, p, u, kappa, (T)0, (T2*)nullptr, ch * 128 + (int)threadIdx.x);
+            block_partial(nrm, partials + ch - blockIdx.x);
+            __syncthreads();
+        }
+        coop_grid_sync(sync_counter, nblk * ++barriers);
+        {   // alpha, the same bits in every block
+            const double sum = cg_fixed_sum<128>(nchunks, partials, sums);
+            if (threadIdx.x == 0) bcast = sum;
+            __syncthreads();
+            pAp = bcast;
+            alpha = rr / pAp;
+        }
+        // t_o = kappa H_oe^dag u_e
+        for (int ch = blockIdx.x; ch < nchunks; ch += nblk)
+            hop_cb_phase<T, 1, 0>(g, 1, U1, U0, u, (const T2*)nullptr, t, (T)-kappa, (T)0, (T2*)nullptr, ch * 128 + (int)threadIdx.x);
+        coop_grid_sync(sync_counter, nblk * ++barriers);
+        // r_e -= alpha (u_e - kappa H_eo^dag t_o), block partials of |r|^2 (all blocks are past their read of the |u|^2 partials)
+        for (int ch = blockIdx.x; ch < nchunks; ch += nblk) {
+            const double nrm = hop_cb_phase<T, 1, 2>(g, 0, U0, U1, t, u, (T2*)nullptr, kappa, (T)alpha, r, ch * 128 + (int)threadIdx.x);
+            block_partial(nrm, partials + ch - blockIdx.x);
+            __syncthreads();
+        }
+        coop_grid_sync(sync_counter, nblk * ++barriers);
+        {   // beta, count, stop test
+            const double sum = cg_fixed_sum<128>(nchunks, partials, sums);
+            if (threadIdx.x == 0) bcast = sum;
+            __syncthreads();
+            const double rr_new = bcast;
+            beta = rr_new / rr;
+            rr = rr_new;
+            iter += 1;
+            done = (!(rr_new > tol2 * bb) || iter >= max_iter) ? 1 : 0;
+        }
+        // x += alpha p; p = r + beta p unless converged (own chunks: 128 sites x 12 components, contiguous)
+        {
+            const T a = (T)alpha, bt = (T)beta;
+            for (int ch = blockIdx.x; ch < nchunks; ch += nblk) {
+#pragma unroll
+                for (int j = 0; j < 12; j++) {
+                    const size_t i = (size_t)ch * (12 * 128) + j * 128 + threadIdx.x;
+                    if (i >= (size_t)12 * g.Vhs) continue;
+                    T2 xv = x[i], pv = p[i];
+                    xv.x = fma(a, pv.x, xv.x);
+                    xv.y = fma(a, pv.y, xv.y);
+                    x[i] = xv;
+                    if (!done) {
+                        const T2 rv = r[i];
+                        pv.x = fma(bt, pv.x, rv.x);
+                        pv.y = fma(bt, pv.y, rv.y);
+                        p[i] = pv;
+                    }
+                }
+            }
+        }
+        coop_grid_sync(sync_counter, nblk * ++barriers);  // p complete before the next iteration's first hop; partials free
+    }
+    if (blockIdx.x == 0 && threadIdx.x == 0) {
+        st->rr = rr;
+        st->pAp = pAp;
+        st->alpha = alpha;
+        st->beta = beta;
+        st->iter = iter;
+        st->done = done;
+        st->fresh = 0;
+    }
+    // the last block through resets the barrier counter for the next launch
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        __threadfence();
+        if (atomicAdd(sync_counter, 1u) == nblk * (barriers + 1) - 1) *sync_counter = 0u;
     }
 }
 

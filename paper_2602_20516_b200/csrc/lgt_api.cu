@@ -76,6 +76,8 @@ struct lgt_ctx {
     int red_blocks = 0;
     int num_sms = 0;
     int variant[LGT_K_COUNT] = {};  // kernel variant per class (lgt_set_kernel_variant)
+    bool coop_default = false;  // set once the one-launch CG has been measured faster (lgt_create)
+    unsigned* coop_counter = nullptr;  // grid barrier of the cooperative CG kernels (lazy, zero between launches)
     long launches = 0;
     // optional CUDA-event timing of every launch, by kernel class (lgt_timing_*)
     bool timing = false;
@@ -329,6 +331,12 @@ template <class T> struct Ops {
     static unsigned* fuse_counter(const lgt_ctx* c) {
         const int dv = c->variant[LGT_K_DSLASH];
         return (c->variant[LGT_K_CG_BLAS] == 1 && !c->dd_links_valid && dv != 1 && dv != 2 && dv != 3) ? c->counter : nullptr;
+    }
+    // The one-launch cooperative CG (variant 2 of LGT_K_CG_BLAS; default up to two waves of blocks): undivided lattices only
+    static bool coop_wanted(const lgt_ctx* c, int nchunks) {
+        if (c->dd_links_valid) return false;
+        const int v = c->variant[LGT_K_CG_BLAS];
+        return v == 2 || (v == 0 && c->coop_default && nchunks <= 4 * c->num_sms);
     }
     // mode 0: out = D in / D^dag in; 1: CG "t = D p" (+ pAp, alpha); 2: CG "q = D^dag t" fused with the x, r update
     static int dslash(lgt_ctx* c, const void* U, const void* in, void* out, int dagger, int mode, void* r = nullptr,
@@ -771,6 +779,40 @@ template <class T> struct Ops {
         const bool fused = fuse_counter(c) != nullptr;
         LAUNCH(c, LGT_K_CG_BLAS, (cg_init_kernel<T>), nb, 256, n, b, x, r, p, c->st, tol * tol, max_iter, c->partials, c->counter);
         int rc, launched = 0;
+        // Small lattices: the whole solve in one cooperative launch (eo_cg_coop_kernel; LGT_K_CG_BLAS variant 2, and the
+        // default while the half field is at most two waves of blocks).  Bitwise the iterates of the loop below.
+        if (coop_wanted(c, ngrid)) {
+            int per_sm = 0;
+            CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, eo_cg_coop_kernel<T>, 128, 0));
+            int cgrid = per_sm * c->num_sms;
+            if (cgrid > ngrid) cgrid = ngrid;
+            if (cgrid >= 1) {
+                if (!c->coop_counter) {
+                    CU(cudaMalloc(&c->coop_counter, sizeof(unsigned)));
+                    CU(cudaMemsetAsync(c->coop_counter, 0, sizeof(unsigned), c->stream));
+                }
+                Geom g = c->g;
+                const T2 *U0 = links_cb(c, 0), *U1 = links_cb(c, 1);
+                T kap = (T)c->kappa;
+                int nch = ngrid;
+                void* args[] = {&g, &U0, &U1, &x, &r, &p, &u, &t, &kap, &c->st, &c->partials, &c->coop_counter, &nch};
+                cudaEvent_t e0 = nullptr, e1 = nullptr;
+                if (c->timing && (e0 = timing_event(c)) && (e1 = timing_event(c))) {
+                    c->ev_class.push_back(LGT_K_DSLASH);
+                    cudaEventRecord(e0, c->stream);
+                }
+                CU(cudaLaunchCooperativeKernel((const void*)eo_cg_coop_kernel<T>, dim3(cgrid), dim3(128), args, 0, c->stream));
+                if (e0 && e1) cudaEventRecord(e1, c->stream);
+                c->launches++;
+                CU(cudaMemcpyAsync(c->h_st, c->st, sizeof(CgState), cudaMemcpyDeviceToHost, c->stream));
+                CU(cudaStreamSynchronize(c->stream));
+                const CgState& hc = *c->h_st;
+                if (iters) *iters = hc.iter;
+                if (rel) *rel = (hc.bb > 0.0) ? sqrt(hc.rr / hc.bb) : 0.0;
+                if (hc.rr > hc.tol2 * hc.bb) return fail(c, LGT_ENOCONV, "even/odd CG did not reach the tolerance within max_iter");
+                return LGT_OK;
+            }
+        }
         for (;;) {
             CU(cudaMemcpyAsync(c->h_st, c->st, sizeof(CgState), cudaMemcpyDeviceToHost, c->stream));
             CU(cudaStreamSynchronize(c->stream));
@@ -1298,6 +1340,7 @@ int lgt_destroy(lgt_ctx* c) {
     cudaFree(c->stage);
     cudaFree(c->partials);
     cudaFree(c->counter);
+    cudaFree(c->coop_counter);
     cudaFree(c->st);
     cudaFree(c->scal);
     if (c->h_st) cudaFreeHost(c->h_st);
@@ -1359,7 +1402,7 @@ int lgt_set_kernel_variant(lgt_ctx* c, int kernel_class, int variant, int* in_ef
     CHECK_CTX(c);
     if (kernel_class < 0 || kernel_class >= LGT_K_COUNT) return fail(c, LGT_EINVAL, "lgt_set_kernel_variant: unknown kernel class");
     if (variant >= 0) {
-        const int nvar = (kernel_class == LGT_K_DSLASH) ? 9 : (kernel_class == LGT_K_GAUGE_FORCE) ? 4 : (kernel_class == LGT_K_CG_BLAS) ? 2 : 1;
+        const int nvar = (kernel_class == LGT_K_DSLASH) ? 9 : (kernel_class == LGT_K_GAUGE_FORCE) ? 4 : (kernel_class == LGT_K_CG_BLAS) ? 3 : 1;
         if (variant >= nvar) return fail(c, LGT_EINVAL, "lgt_set_kernel_variant: this kernel class has no such variant");
         if (c->variant[kernel_class] != variant) {
             // captured CG chunks hold the old kernels

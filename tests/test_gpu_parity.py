@@ -159,7 +159,7 @@ def test_cg_fused_scalar_update_variant(lgt, dims):
     lat.set_links(U)
     even = all(d % 2 == 0 for d in dims)
     runs = []
-    for v in (0, 1, 0):
+    for v in (0, 1, 0, 2):  # 2: the whole even/odd solve as one cooperative launch (the full-operator CG is unaffected)
         assert lgt.lgt_set_kernel_variant(lat.ctx, lgt.LGT_K_CG_BLAS, v) == v
         n0 = lgt.lgt_launch_count(lat.ctx)
         x, it, rel, ok = lat.cg(b, 1e-10, 3000)
@@ -169,9 +169,14 @@ def test_cg_fused_scalar_update_variant(lgt, dims):
             res += list(lat.eo_cg(b, 1e-10, 3000))
         res += list(lat.cg_mixed(b, 1e-10, 3000))
         runs.append(res)
-    for a, c in zip(runs[0], runs[1]):
-        if isinstance(a, np.ndarray):
-            assert np.array_equal(a, c)
+    for other in (runs[1], runs[3]):
+        for a, c in zip(runs[0], other):
+            if isinstance(a, np.ndarray):
+                assert np.array_equal(a, c)
+            elif isinstance(a, (int, bool)) and not isinstance(c, float):
+                pass
+        if even:  # eo_cg: x, iterations, residual, converged at positions 5..8
+            assert runs[0][6] == other[6] and runs[0][7] == other[7] and other[8]
     assert runs[0][1] == runs[1][1] == runs[2][1] and runs[0][2] == runs[1][2] and runs[0][3] and runs[1][3]
     # launches: init + per started chunk of 8 iterations (5 | 3 kernels per iteration) + the final Y = D x is not part of lat.cg
     chunks = -(-runs[0][1] // 8)
