@@ -864,6 +864,149 @@ __global__ void __launch_bounds__(128, 1) dslash_tma_kernel(Geom g, const typena
     }
 }
 
+// Variant 9: the persistent kernel with the operands that come from DRAM -- the four forward links of a site and its t+1
+// spinor, 48 of the 180 loads -- requested one chunk ahead by per-thread asynchronous copies (cp.async, LDGSTS) into
+// thread-private shared-memory slots (768 B per thread in fp64).  Unlike the bulk copies of variant 2 these are ordinary
+// per-thread instructions: no uniform-datapath vote loop, no branch, so the hop sequence stays one scheduling region; a slot
+// is re-armed for the next chunk right after its hop has used it (cp.async.wait_group 3 keeps the four groups in order).
+// The registers then only have to cover the L2-hit loads (neighbour spinors, backward links), and up to 768 B per thread of
+// DRAM requests are in flight on top of them.  Same arithmetic in the same order as dslash_kernel: bitwise identical results.
+template <int BYTES> __device__ __forceinline__ void cp_async(unsigned dst, const void* src) {
+    if (BYTES == 16) asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src));
+    else asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst), "l"(src));
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;"); }
+// waits until at most three of this thread's copy groups are pending; returns 0 (ties the slot reads to the wait)
+__device__ __forceinline__ unsigned cp_async_wait3() {
+    unsigned zero;
+    asm volatile("cp.async.wait_group 3;\n mov.u32 %0, 0;" : "=r"(zero)::"memory");
+    return zero;
+}
+template <class T> constexpr int dslash_cpasync_smem_bytes() { return (4 * 9 + 12) * 128 * (int)sizeof(typename Vec2<T>::type); }
+
+template <class T, int DAG, int MODE>
+__global__ void __launch_bounds__(128, 1) dslash_cpasync_kernel(Geom g, const typename Vec2<T>::type* __restrict__ U,
+                                                                const typename Vec2<T>::type* __restrict__ in,
+                                                                typename Vec2<T>::type* __restrict__ out, T kappa, CgState* st,
+                                                                double* partials, typename Vec2<T>::type* __restrict__ r, int nchunks) {
+    typedef typename Vec2<T>::type T2;
+    extern __shared__ __align__(128) unsigned char dslash_smem[];
+    if (MODE != 0 && st->done) return;  // uniform over the grid
+    int chunk = blockIdx.x;
+    if (chunk >= nchunks) return;
+    constexpr int F = DAG ? +1 : -1;
+    constexpr int EB = (int)sizeof(T2);
+    T2* const slots = reinterpret_cast<T2*>(dslash_smem) + threadIdx.x;  // component k of slot q: slots[(q * 9 + k) * 128], spinor: (36 + k) * 128
+    const unsigned slots_u32 = smem_u32(slots);
+    const int last = g.s_end - 1;
+    int s = g.s_begin + swizzled_chunk(g, chunk) * 128 + threadIdx.x;
+    int sl = s < last ? s : last;
+    // the four link groups (and the t+1 spinor with the t link) of the first chunk
+    {
+        const Site c0 = site_coords(g, sl);
+#pragma unroll
+        for (int mu = 0; mu < 4; mu++) {
+            const T2* b = link_at(U, sl, mu);
+#pragma unroll
+            for (int k = 0; k < 9; k++) cp_async<EB>(slots_u32 + (mu * 9 + k) * 128 * EB, b + k * W);
+            if (mu == 3) {
+                const T2* bp = spinor_at(in, nbr_fwd(g, c0, sl, 3));
+#pragma unroll
+                for (int k = 0; k < 12; k++) cp_async<EB>(slots_u32 + (36 + k) * 128 * EB, bp + k * W);
+            }
+            cp_async_commit();
+        }
+    }
+    for (;;) {
+        if (MODE == 2 && s <= last) {
+            const T2* br = spinor_at(r, s);
+#pragma unroll
+            for (int k = 0; k < 12; k++) asm volatile("prefetch.global.L2 [%0];" ::"l"(br + k * W));
+        }
+        const Site c = site_coords(g, sl);
+        const int nchunk = chunk + gridDim.x;
+        const bool more = nchunk < nchunks;
+        const int s2 = more ? g.s_begin + swizzled_chunk(g, nchunk) * 128 + threadIdx.x : s;
+        const int sl2 = s2 < last ? s2 : last;
+        const Site c2 = site_coords(g, sl2);
+        cx<T> acc[12];
+#pragma unroll
+        for (int k = 0; k < 12; k++) acc[k] = mk<T>(0, 0);
+#define CPA_FWD_HOP(MU)                                                                                          \
+        {                                                                                                        \
+            const unsigned z_ = cp_async_wait3();                                                                \
+            const T2* sl_ = slots + z_;                                                                          \
+            cx<T> p_[12], h_[6], u_[9], w_[6];                                                                   \
+            if (MU == 3) {                                                                                       \
+                _Pragma("unroll") for (int k = 0; k < 12; k++) { const T2 v = sl_[(36 + k) * 128]; p_[k] = mk<T>(v.x, v.y); } \
+            } else {                                                                                             \
+                load_spinor<T>(in, nbr_fwd(g, c, sl, MU), p_);                                                   \
+            }                                                                                                    \
+            _Pragma("unroll") for (int k = 0; k < 9; k++) { const T2 v = sl_[(MU * 9 + k) * 128]; u_[k] = mk<T>(v.x, v.y); } \
+            spin_project<MU, F>(p_, h_);                                                                         \
+            su3_mul_half(u_, h_, w_);                                                                            \
+            spin_reconstruct_add<MU, F>(w_, acc);                                                                \
+            /* the slot has been used: request the next chunk's operands into it (the last chunk re-requests its own) */ \
+            const T2* b_ = link_at(U, sl2, MU);                                                                  \
+            _Pragma("unroll") for (int k = 0; k < 9; k++) cp_async<EB>(slots_u32 + (MU * 9 + k) * 128 * EB, b_ + k * W); \
+            if (MU == 3) {                                                                                       \
+                const T2* bp_ = spinor_at(in, nbr_fwd(g, c2, sl2, 3));                                           \
+                _Pragma("unroll") for (int k = 0; k < 12; k++) cp_async<EB>(slots_u32 + (36 + k) * 128 * EB, bp_ + k * W); \
+            }                                                                                                    \
+            cp_async_commit();                                                                                   \
+        }
+        CPA_FWD_HOP(0)
+        hop_bwd<0, -F, T>(g, U, in, c, sl, acc);
+        CPA_FWD_HOP(1)
+        hop_bwd<1, -F, T>(g, U, in, c, sl, acc);
+        CPA_FWD_HOP(2)
+        hop_bwd<2, -F, T>(g, U, in, c, sl, acc);
+        CPA_FWD_HOP(3)
+        hop_bwd<3, -F, T>(g, U, in, c, sl, acc);
+#undef CPA_FWD_HOP
+        double nrm = 0.0;
+        if (s <= last) {
+            const T2* bi = spinor_at(in, s);
+            if (MODE == 2) {
+                const T alpha = (T)st->alpha;
+                T2* br = spinor_at(r, s);
+#pragma unroll
+                for (int k = 0; k < 12; k++) {
+                    cx<T> tv = ldc<T>(bi + k * W);
+                    cx<T> q = mk<T>(fma(-kappa, acc[k].re, tv.re), fma(-kappa, acc[k].im, tv.im));
+                    cx<T> rv = ldc_rw<T>(br + k * W);
+                    rv.re = fma(-alpha, q.re, rv.re);
+                    rv.im = fma(-alpha, q.im, rv.im);
+                    stc<T>(br + k * W, rv);
+                    nrm += (double)rv.re * (double)rv.re + (double)rv.im * (double)rv.im;
+                }
+            } else {
+                T2* bo = spinor_at(out, s);
+#pragma unroll
+                for (int k = 0; k < 12; k++) {
+                    cx<T> pv = ldc<T>(bi + k * W);
+                    cx<T> o = mk<T>(fma(-kappa, acc[k].re, pv.re), fma(-kappa, acc[k].im, pv.im));
+                    stc<T>(bo + k * W, o);
+                    if (MODE == 1) nrm += (double)o.re * (double)o.re + (double)o.im * (double)o.im;
+                }
+            }
+        } else if (s >= g.V && s < g.Vs && MODE != 2) {  // padding lanes only, never a ghost slice
+            T2* bo = spinor_at(out, s);
+#pragma unroll
+            for (int k = 0; k < 12; k++) stc<T>(bo + k * W, mk<T>(0, 0));
+        }
+        if (MODE != 0) {
+            block_partial(nrm, partials + chunk - blockIdx.x);
+            __syncthreads();  // the partial's shared scratch is reused by the next chunk
+        }
+        if (!more) break;
+        chunk = nchunk;
+        s = s2;
+        sl = sl2;
+    }
+    asm volatile("cp.async.wait_group 0;" ::: "memory");  // the last chunk's (unused) re-requests
+}
+
 // Variant 3: 4-D site blocking by block-to-site mapping (the layout is unchanged).  dslash_kernel's block is 128
 // consecutive lexicographic sites (four x rows at 32^4), so of the nine spinors and eight links a site needs only the
 // x and most y neighbours are shared inside the block: L2 -> L1 traffic is 2.06 KB per site for 0.96 KB compulsory.
