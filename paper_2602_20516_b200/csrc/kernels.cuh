@@ -596,7 +596,10 @@ __global__ void __launch_bounds__(128, 1) dslash_persistent_kernel(Geom g, const
                                                                    const typename Vec2<T>::type* __restrict__ in,
                                                                    typename Vec2<T>::type* __restrict__ out, T kappa, CgState* st,
                                                                    double* partials, typename Vec2<T>::type* __restrict__ r,
-                                                                   int nchunks) {
+                                                                   int nchunks, unsigned* ticket = nullptr) {
+    // ticket != nullptr (variant 10): the chunks after a block's first are drawn from a global counter instead of taken at a
+    // fixed stride, so that a block on a slower SM simply draws fewer; the draw with the last number resets the counter.
+    __shared__ int next_chunk;
     if (MODE != 0 && st->done) return;  // uniform over the grid
     int chunk = blockIdx.x;
     if (chunk >= nchunks) return;
@@ -616,7 +619,16 @@ __global__ void __launch_bounds__(128, 1) dslash_persistent_kernel(Geom g, const
         }
         // where the next chunk is (the last chunk re-requests its own sites: L1 hits, results unused); computed here so
         // that no branch separates the loads below from the hops around them
-        const int nchunk = chunk + gridDim.x;
+        int nchunk = chunk + gridDim.x;
+        if (ticket) {
+            if (threadIdx.x == 0) {
+                const unsigned k = atomicAdd(ticket, 1u);
+                if (k == (unsigned)nchunks - 1u) *ticket = 0u;  // the last draw of the launch
+                next_chunk = (int)(gridDim.x + k);
+            }
+            __syncthreads();
+            nchunk = next_chunk;
+        }
         const bool more = nchunk < nchunks;
         const int s2 = more ? g.s_begin + swizzled_chunk(g, nchunk) * 128 + threadIdx.x : s;
         const int sl2 = s2 < last ? s2 : last;
@@ -670,6 +682,7 @@ __global__ void __launch_bounds__(128, 1) dslash_persistent_kernel(Geom g, const
             block_partial(nrm, partials + chunk - blockIdx.x);  // block_partial adds blockIdx.x
             __syncthreads();  // the partial's shared scratch is reused by the next chunk
         }
+        else if (ticket) __syncthreads();  // next_chunk is rewritten at the top of the next round
         if (!more) break;
         chunk = nchunk;
         s = s2;

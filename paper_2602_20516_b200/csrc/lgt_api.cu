@@ -330,7 +330,7 @@ template <class T> struct Ops {
     // tail, and the slabs of a decomposed lattice split their sums around an all-reduce.
     static unsigned* fuse_counter(const lgt_ctx* c) {
         const int dv = c->variant[LGT_K_DSLASH];
-        return (c->variant[LGT_K_CG_BLAS] == 1 && !c->dd_links_valid && dv != 1 && dv != 2 && dv != 3 && dv != 9) ? c->counter : nullptr;
+        return (c->variant[LGT_K_CG_BLAS] == 1 && !c->dd_links_valid && dv != 1 && dv != 2 && dv != 3 && dv != 9 && dv != 10) ? c->counter : nullptr;
     }
     // The one-launch cooperative CG (variant 2 of LGT_K_CG_BLAS; default up to two waves of blocks): undivided lattices only
     static bool coop_wanted(const lgt_ctx* c, int nchunks) {
@@ -367,6 +367,26 @@ template <class T> struct Ops {
             } else {
                 LAUNCH(c, LGT_K_DSLASH_R, (dslash_kernel<T, 1, 2, 0, 0, 1>), grid, 128, DSLASH_ARGS);
             }
+            return LGT_OK;
+        }
+        if (c->variant[LGT_K_DSLASH] == 10) {  // variant 1 with the chunks drawn from a counter instead of a fixed stride
+            const int pgrid = grid < 2 * c->num_sms ? grid : 2 * c->num_sms;
+            if (!c->coop_counter) {
+                CU(cudaMalloc(&c->coop_counter, sizeof(unsigned)));
+                CU(cudaMemsetAsync(c->coop_counter, 0, sizeof(unsigned), c->stream));
+            }
+#define DSLASH_DARGS c->g, (const T2*)U, (const T2*)in, (T2*)out, kappa, c->st, c->partials, (T2*)r, grid, c->coop_counter
+            if (mode == 0) {
+                if (dagger)
+                    LAUNCH(c, LGT_K_DSLASH, (dslash_persistent_kernel<T, 1, 0>), pgrid, 128, DSLASH_DARGS);
+                else
+                    LAUNCH(c, LGT_K_DSLASH, (dslash_persistent_kernel<T, 0, 0>), pgrid, 128, DSLASH_DARGS);
+            } else if (mode == 1) {
+                LAUNCH(c, LGT_K_DSLASH, (dslash_persistent_kernel<T, 0, 1>), pgrid, 128, DSLASH_DARGS);
+            } else {
+                LAUNCH(c, LGT_K_DSLASH_R, (dslash_persistent_kernel<T, 1, 2>), pgrid, 128, DSLASH_DARGS);
+            }
+#undef DSLASH_DARGS
             return LGT_OK;
         }
         if (c->variant[LGT_K_DSLASH] == 1) {  // persistent, software-pipelined: one wave of blocks loops over the chunks
@@ -1417,7 +1437,7 @@ int lgt_set_kernel_variant(lgt_ctx* c, int kernel_class, int variant, int* in_ef
     CHECK_CTX(c);
     if (kernel_class < 0 || kernel_class >= LGT_K_COUNT) return fail(c, LGT_EINVAL, "lgt_set_kernel_variant: unknown kernel class");
     if (variant >= 0) {
-        const int nvar = (kernel_class == LGT_K_DSLASH) ? 10 : (kernel_class == LGT_K_GAUGE_FORCE) ? 4 : (kernel_class == LGT_K_CG_BLAS) ? 3 : 1;
+        const int nvar = (kernel_class == LGT_K_DSLASH) ? 11 : (kernel_class == LGT_K_GAUGE_FORCE) ? 4 : (kernel_class == LGT_K_CG_BLAS) ? 3 : 1;
         if (variant >= nvar) return fail(c, LGT_EINVAL, "lgt_set_kernel_variant: this kernel class has no such variant");
         if (c->variant[kernel_class] != variant) {
             // captured CG chunks hold the old kernels
