@@ -646,11 +646,11 @@ def run_extras(args, lgt, synth, lat, cfg, hU, hP, hphi, reset_state, md_step, l
     lgt.lgt_set_fermion_action(ctx, lgt.LGT_ACTION_FULL)
     # the decomposed path (lgt_dd_*) on this one GPU: 1 and 4 time slabs in one process, halo exchange by device copies
     U_np, P_np, phi_np = hU.numpy(), hP.numpy(), hphi.numpy()
-    for nr, halo in ((1, "exchange"), (1, "push"), (4, "exchange")):
-        if dims[3] % nr or (dims[0] * dims[1] * dims[2]) % 32:
+    for nr, halo, grid in ((1, "exchange", None), (1, "push", None), (4, "exchange", None), (4, "overlap", None), (4, "exchange", (2, 2))):
+        if dims[3] % nr or (dims[0] * dims[1] * dims[2]) % 32 or (grid and (dims[3] % grid[0] or dims[2] % grid[1])):
             continue
-        dd = lgt.DecomposedLattice(dims, nr, list(range(nr)), beta, kappa, bc, lgt.LGT_F64, local, stream)
-        lgt.lgt_dd_set_halo_mode(dd.d, lgt.LGT_DD_PUSH if halo == "push" else lgt.LGT_DD_EXCHANGE)
+        dd = lgt.DecomposedLattice(dims, nr, list(range(nr)), beta, kappa, bc, lgt.LGT_F64, local, stream, grid=grid)
+        lgt.lgt_dd_set_halo_mode(dd.d, {"push": lgt.LGT_DD_PUSH, "overlap": lgt.LGT_DD_OVERLAP}.get(halo, lgt.LGT_DD_EXCHANGE))
 
         def dd_reset():
             dd.set_links(U_np)
@@ -670,10 +670,12 @@ def run_extras(args, lgt, synth, lat, cfg, hU, hP, hphi, reset_state, md_step, l
         dd_iters = [dd_step() for _ in range(2)]
         b.record()
         torch.cuda.synchronize()
-        extras["decomposed_%d_slabs_%s_one_gpu" % (nr, halo)] = {
+        shape = ("%dx%d_grid" % grid) if grid else "%d_slabs" % nr
+        extras["decomposed_%s_%s_one_gpu" % (shape, halo)] = {
             "ms_per_step": round(a.elapsed_time(b) / 2, 3), "cg_iters_per_step": dd_iters,
-            "note": "same MD step through lgt_dd_* with %d time slab(s) resident on this GPU, halo mode %s: the cost of the "
-                    "ghost slices, halo traffic and split reductions, not a multi-GPU number" % (nr, halo)}
+            "note": "same MD step through lgt_dd_* with %s resident on this GPU, halo mode %s: the cost of the "
+                    "ghost slices, halo traffic and split reductions, not a multi-GPU number" %
+                    (("a %d x %d (t, z) grid of ranks" % grid) if grid else "%d time slab(s)" % nr, halo)}
         dd.close()
         del dd
 

@@ -1465,11 +1465,11 @@ template <class T> __device__ __forceinline__ void exp_iQ(const cx<T> Q[9], cx<T
         xi0 = 1 - w2 * (T)(1.0 / 6.0) * (1 - w2 * (T)(1.0 / 20.0) * (1 - w2 * (T)(1.0 / 42.0)));
     else
         xi0 = sw / w;
-    T s2u, c2u, s1u, c1u;
-    sincos(2 * u, &s2u, &c2u);
+    T s1u, c1u;
     sincos(u, &s1u, &c1u);
-    cx<T> e2 = mk<T>(c2u, s2u);   // exp(2iu)
-    cx<T> em = mk<T>(c1u, -s1u);  // exp(-iu)
+    // exp(2iu) = (exp(iu))^2: one sincos less (the double-angle forms are exact to two roundings)
+    cx<T> e2 = mk<T>(fma(c1u, c1u, -s1u * s1u), 2 * s1u * c1u);  // exp(2iu)
+    cx<T> em = mk<T>(c1u, -s1u);                                 // exp(-iu)
     cx<T> h0 = (u2 - w2) * e2 + em * mk<T>(8 * u2 * cw, 2 * u * (3 * u2 + w2) * xi0);
     cx<T> h1 = (2 * u) * e2 - em * mk<T>(2 * u * cw, -(3 * u2 - w2) * xi0);
     cx<T> h2 = e2 - em * mk<T>(cw, 3 * u * xi0);
