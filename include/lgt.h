@@ -218,7 +218,8 @@ int lgt_dd_create(lgt_dd** out, const int dims[4], int nranks, int nlocal, const
  * field travels first in t (whole local slices) and then in z (the boundary xy planes of every local slice, ghost slices
  * included, which fills the corners the staples need), through the same three transports.  Slab arrays are the rank's
  * block [Lt/Pt][Lz/Pz][Ly][Lx] in lexicographic order.  Full operator with plain or mixed-precision CG, stout smearing,
- * all integrators and the HMC trajectory; LGT_DD_PUSH and the even/odd action are for time slabs only (LGT_EINVAL).
+ * the even/odd action (needs Lx*Ly % 64 == 0 and even Lz/Pz, Lt/Pt), all integrators and the HMC trajectory; LGT_DD_PUSH is for
+ * time slabs only (LGT_EINVAL).
  * grid = {nranks, 1} is a time-slab decomposition whose ranks are their own z neighbours. */
 int lgt_dd_create_grid(lgt_dd** out, const int dims[4], const int grid[2], int nlocal, const int* local_ranks, double beta,
                        double kappa, const int bc[4], int precision, int device, void* cuda_stream);

@@ -1885,7 +1885,7 @@ __device__ __forceinline__ void hop_bwd_cb(const Geom& g, const typename Vec2<T>
 // With kap = -kappa and no self this is the odd half "t_o = kappa H_oe p_e"; with kap = +kappa and self = p_e the
 // even half "p_e - kappa H_eo t_o" of the Schur complement M = 1 - kappa^2 H_eo H_oe.
 // PUSH (time slab, CG modes 1 and 2): as in dslash_kernel, for the half field the launch produces (u in MODE 1, r in MODE 2).
-template <class T, int DAG, int MODE, int PUSH = 0>
+template <class T, int DAG, int MODE, int PUSH = 0, int ZS = 0>
 __global__ void __launch_bounds__(128, 1) hop_cb_kernel(Geom g, int p, const typename Vec2<T>::type* __restrict__ Up,
                                                         const typename Vec2<T>::type* __restrict__ Uq,
                                                         const typename Vec2<T>::type* __restrict__ in,
@@ -1897,7 +1897,8 @@ __global__ void __launch_bounds__(128, 1) hop_cb_kernel(Geom g, int p, const typ
     if (MODE == 1 && fuse && done && blockIdx.x == 0 && threadIdx.x == 0) st->fresh = 0;  // as in dslash_kernel
     const int c = g.h_begin + blockIdx.x * blockDim.x + threadIdx.x;
     double nrm = 0.0;
-    if (c < g.h_end) {
+    // ZS: a rank of a (Pt, Pz) grid -- the half-field sites of its two ghost z planes are skipped (an xy plane holds L0 L1 / 2 of them)
+    if (c < g.h_end && (!ZS || z_owned(g, (c / ((g.L[0] * g.L[1]) >> 1)) % g.L[2]))) {
         if (MODE == 2) {
             const typename Vec2<T>::type* br = spinor_at(r, c);
 #pragma unroll

@@ -786,6 +786,20 @@ template <class T> struct Ops {
         }
 #undef HOP_PUSH_ARGS
 #define HOP_ARGS c->g, p, links_cb(c, p), links_cb(c, 1 - p), in, self, out, (T)kap, c->st, c->partials, r, PushTo<T>()
+        if (c->g.z_hi - c->g.z_lo != c->g.L[2]) {  // a rank of a (Pt, Pz) grid: the kernels that skip the ghost z planes
+            if (mode == 0) {
+                if (dagger) LAUNCH(c, LGT_K_DSLASH, (hop_cb_kernel<T, 1, 0, 0, 1>), grid, 128, HOP_ARGS);
+                else LAUNCH(c, LGT_K_DSLASH, (hop_cb_kernel<T, 0, 0, 0, 1>), grid, 128, HOP_ARGS);
+            } else if (mode == 3) {
+                if (dagger) LAUNCH(c, LGT_K_DSLASH, (hop_cb_kernel<T, 1, 3, 0, 1>), grid, 128, HOP_ARGS);
+                else LAUNCH(c, LGT_K_DSLASH, (hop_cb_kernel<T, 0, 3, 0, 1>), grid, 128, HOP_ARGS);
+            } else if (mode == 1) {
+                LAUNCH(c, LGT_K_DSLASH, (hop_cb_kernel<T, 0, 1, 0, 1>), grid, 128, HOP_ARGS);
+            } else {
+                LAUNCH(c, LGT_K_DSLASH_R, (hop_cb_kernel<T, 1, 2, 0, 1>), grid, 128, HOP_ARGS);
+            }
+            return LGT_OK;
+        }
         if (mode == 0) {
             if (dagger) LAUNCH(c, LGT_K_DSLASH, (hop_cb_kernel<T, 1, 0>), grid, 128, HOP_ARGS);
             else LAUNCH(c, LGT_K_DSLASH, (hop_cb_kernel<T, 0, 0>), grid, 128, HOP_ARGS);

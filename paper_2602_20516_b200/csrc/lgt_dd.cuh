@@ -758,7 +758,7 @@ template <class T> struct DdOps {
                 if (eta_norm) {  // |eta_e|^2; after a solve eo_solve() has left Re <phi_e, X_e> in the slot already
                     const size_t off = half_off(c), cnt = half_n(c);
                     LAUNCH(c, LGT_K_OTHER, (redot_kernel<T>), stream_blocks(c, cnt), 256, cnt, (const T2*)hB(c) + off, (const T2*)hB(c) + off,
-                           c->scal + 2, c->partials, c->counter);
+                           c->scal + 2, c->partials, c->counter, zmask_half(c));
                 }
             } else if (ferm) {
                 const size_t off = spinor_off(c);
@@ -786,7 +786,7 @@ template <class T> struct DdOps {
     // one by t_off, so the globally even sites are the local parity pe = t_off & 1; everything else is Ops<T>'s even/odd
     // code with (pe, 1 - pe) in place of (0, 1), the input half field's ghost slices exchanged before every hop and the
     // CG sums all-reduced.  Half fields have V3 / 2 sites per time slice, so their slices are contiguous runs too.
-    static int pe_of(const lgt_ctx* c) { return c->g.t_off & 1; }
+    static int pe_of(const lgt_ctx* c) { return (c->g.t_off + c->g.z_off) & 1; }  // z_off = 0 on time slabs
     static T2* E(lgt_ctx* c, int k) { return O::eo_field(c, k + pe_of(c)); }      // globally even member of the pair (k, k+1)
     static T2* Od(lgt_ctx* c, int k) { return O::eo_field(c, k + 1 - pe_of(c)); }  // globally odd member
     typedef T2* (*HalfSel)(lgt_ctx*);
@@ -800,6 +800,12 @@ template <class T> struct DdOps {
     static T2* hYe(lgt_ctx* c) { return E(c, 2); }
     static T2* hP(lgt_ctx* c) { return O::eo_field(c, 6); }
     static T2* hT(lgt_ctx* c) { return O::eo_field(c, 7); }
+    // the streaming sums over a half field of a grid rank: an xy plane holds L0 L1 / 2 half-field sites
+    static ZMask zmask_half(const lgt_ctx* c) {
+        ZMask m = zmask(c);
+        m.xy >>= 1;
+        return m;
+    }
     static size_t half_off(const lgt_ctx* c) { return (size_t)12 * c->g.h_begin; }
     static size_t half_n(const lgt_ctx* c) { return (size_t)12 * (c->g.h_end - c->g.h_begin); }
     // one hop on every rank, after the exchange of its input field
@@ -851,7 +857,7 @@ template <class T> struct DdOps {
             lgt_ctx* c = d->rk[i];
             const size_t off = half_off(c), cnt = half_n(c);
             LAUNCH(c, LGT_K_CG_BLAS, (cg_init_kernel<T>), stream_blocks(c, cnt), 256, cnt, (const T2*)B(c) + off, X(c) + off, R(c) + off,
-                   P(c) + off, c->st, tol * tol, max_iter, c->partials, c->counter);
+                   P(c) + off, c->st, tol * tol, max_iter, c->partials, c->counter, zmask_half(c));
             LAUNCH(c, LGT_K_CG_BLAS, cg_rr_to_tmp_kernel, 1, 1, c->st);
         }
         if ((rc = allreduce_tmp(d)) != LGT_OK) return rc;
@@ -947,7 +953,7 @@ template <class T> struct DdOps {
                 lgt_ctx* c = d->rk[i];
                 const size_t off = half_off(c), cnt = half_n(c);
                 LAUNCH(c, LGT_K_OTHER, (redot_kernel<T>), stream_blocks(c, cnt), 256, cnt, (const T2*)hB(c) + off, (const T2*)hXe(c) + off,
-                       c->scal + 2, c->partials, c->counter);
+                       c->scal + 2, c->partials, c->counter, zmask_half(c));
             }
         if (want_xy) {
             if ((rc = hop_all(d, false, hXe, nullptr, hXo, 0, 0, false)) != LGT_OK) return rc;  // X_o = kappa H_oe X_e
@@ -1161,7 +1167,7 @@ int dd_eo_cg_mixed(lgt_dd* d, double tol, int max_iter, int* iters) {
         DD_CU(cudaMemsetAsync(D64::hXe(c), 0, nh * sizeof(double2), d->stream));
         DD_CU(cudaMemcpyAsync(D64::hR(c), D64::hB(c), nh * sizeof(double2), cudaMemcpyDeviceToDevice, d->stream));
         LAUNCH(c, LGT_K_OTHER, (redot_kernel<double>), stream_blocks(c, cnt), 256, cnt, (const double2*)D64::hB(c) + off,
-               (const double2*)D64::hB(c) + off, c->scal + 3, c->partials, c->counter);
+               (const double2*)D64::hB(c) + off, c->scal + 3, c->partials, c->counter, D64::zmask_half(c));
         slot.push_back(c->scal + 3);
     }
     lgt_ctx* c0 = d->rk[0];
@@ -1210,7 +1216,7 @@ int dd_eo_cg_mixed(lgt_dd* d, double tol, int max_iter, int* iters) {
             lgt_ctx* c = d->rk[i];
             const size_t off = D64::half_off(c), cnt = D64::half_n(c);
             LAUNCH(c, LGT_K_CG_BLAS, residual_kernel, stream_blocks(c, cnt), 256, cnt, (const double2*)D64::hB(c) + off,
-                   (const double2*)D64::hP(c) + off, (double2*)D64::hR(c) + off, c->scal + 3, c->partials, c->counter);
+                   (const double2*)D64::hP(c) + off, (double2*)D64::hR(c) + off, c->scal + 3, c->partials, c->counter, D64::zmask_half(c));
         }
         if ((rc = read_sum(rr)) != LGT_OK) return rc;
     }
@@ -1543,13 +1549,14 @@ int lgt_dd_md_trajectory(lgt_dd* d, int nsteps, double dt, double tol, int max_i
 int lgt_dd_set_fermion_action(lgt_dd* d, int action) {
     CHECK_DD(d);
     if (action != LGT_ACTION_FULL && action != LGT_ACTION_EO) return dd_fail(d, LGT_EINVAL, "lgt_dd_set_fermion_action: unknown action");
-    if (action == LGT_ACTION_EO && d->Pz > 0)
-        return dd_fail(d, LGT_EINVAL, "lgt_dd_set_fermion_action: the even/odd action runs on time slabs, not on a (Pt, Pz) grid");
     if (action == LGT_ACTION_EO) {
         const Geom& g = d->rk[0]->g;
         if (g.L[0] % 2 || g.L[1] % 2 || g.L[2] % 2 || d->Lt_loc % 2 || d->V3 % 64)
             return dd_fail(d, LGT_EINVAL, "lgt_dd_set_fermion_action: the even/odd action needs even extents, an even number of time slices "
                                           "per slab and Lx*Ly*Lz a multiple of 64");
+        if (d->Pz > 0 && d->LxLy % 64)  // (Lz_loc + 2 even is the g.L[2] check above)
+            return dd_fail(d, LGT_EINVAL, "lgt_dd_set_fermion_action: on a (Pt, Pz) grid the even/odd action needs Lx*Ly a multiple of 64 "
+                                          "(the z faces of a half field are then whole layout blocks)");
     }
     for (lgt_ctx* c : d->rk) c->action = action;
     return LGT_OK;

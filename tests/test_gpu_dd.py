@@ -613,10 +613,12 @@ def test_grid_cg_and_md_trajectory(lgt, dims, grid):
     lgt.lgt_dd_md_drift(dd.d, 0.05)
     assert np.abs(gather_grid(dims, grid, dd.get_links()) - oracle.drift(dims, 0.05, P1, U0)).max() < 1e-13
     # what a grid does not offer
-    for call in (lambda: lgt.lgt_dd_set_halo_mode(dd.d, lgt.LGT_DD_PUSH), lambda: lgt.lgt_dd_set_fermion_action(dd.d, lgt.LGT_ACTION_EO)):
-        with pytest.raises(lgt.LgtError) as e:
-            call()
-        assert e.value.code == lgt.LGT_EINVAL
+    with pytest.raises(lgt.LgtError) as e:
+        lgt.lgt_dd_set_halo_mode(dd.d, lgt.LGT_DD_PUSH)
+    assert e.value.code == lgt.LGT_EINVAL
+    with pytest.raises(lgt.LgtError) as e:  # 32 sites per xy plane: a half field's z face would be half a layout block
+        lgt.lgt_dd_set_fermion_action(dd.d, lgt.LGT_ACTION_EO)
+    assert e.value.code == lgt.LGT_EINVAL
     dd.close()
     for bad in ((3, 1), (1, 3), (0, 2)):  # Lt % Pt, Lz % Pz, Pt < 1
         with pytest.raises(lgt.LgtError) as e:
@@ -677,4 +679,49 @@ def test_grid_hmc_mixed_solver_and_stout(lgt, grid):
         assert ok and it == it_ref
         P_ref = P0 - 0.05 * (oracle.gauge_force(dims, beta, U0) + Ff)
         assert link_rel_err(gather_grid(dims, grid, dd.get_momenta()), P_ref)[0] < TOL64
+    dd.close()
+
+
+@pytest.mark.parametrize("grid", [(2, 2), (1, 2), (2, 1)])
+def test_grid_even_odd_action(lgt, grid):
+    """The even/odd action on the (Pt, Pz) grid: a rank's local parity is the global one shifted by its time AND z offsets, the
+    half fields' z faces (Lx Ly / 2 sites per plane) travel like the full fields'.  Iteration count, kick and S_F against the
+    oracle's even/odd mode on the undivided lattice, the mixed-precision solver on top, and an HMC trajectory against the
+    single-handle even/odd trajectory with the same seed."""
+    from oracle import evenodd as oeo
+
+    dims, beta, kappa, tol = (8, 8, 4, 4), 5.6, 0.12, 1e-12
+    n = grid[0] * grid[1]
+    V = synth.volume(dims)
+    U0 = synth.warm_links(dims, 0.3, 741)
+    P0 = synth.gaussian_momenta(dims, 742)
+    phi = oeo.mhat(dims, kappa, BC, U0, oeo.keep(synth.gaussian_spinor(dims, 743), dims, 0), dagger=True)
+    F_ref, it_ref, _ = oeo.fermion_force(dims, kappa, BC, U0, phi, tol, 10 * V)
+    P_ref = P0 - 0.05 * (oracle.gauge_force(dims, beta, U0) + F_ref)
+    S_ref = oeo.action(dims, kappa, BC, U0, phi, tol, 10 * V)[0]
+    dd = lgt.DecomposedLattice(dims, n, list(range(n)), beta, kappa, BC, grid=grid)
+    lgt.lgt_dd_set_fermion_action(dd.d, lgt.LGT_ACTION_EO)
+    for solver, ptol in ((lgt.LGT_SOLVER_CG, TOL64), (lgt.LGT_SOLVER_MIXED_CG, 1e-10)):
+        lgt.lgt_dd_set_solver(dd.d, solver, 1e-5)
+        dd.set_links(U0)
+        dd.set_momenta(P0)
+        dd.set_pseudofermion(phi)
+        it = lgt.lgt_dd_md_kick(dd.d, 0.05, tol, 10 * V)
+        if solver == lgt.LGT_SOLVER_CG:
+            assert it == it_ref
+        assert link_rel_err(gather_grid(dims, grid, dd.get_momenta()), P_ref)[0] < ptol
+        _, S_F, _, _ = lgt.lgt_dd_action(dd.d, tol, 10 * V)
+        assert abs(S_F - S_ref) < 1e-10 * abs(S_ref)
+    lgt.lgt_dd_set_solver(dd.d, lgt.LGT_SOLVER_CG)
+    one = lgt.Lattice(dims, beta, kappa, BC)
+    lgt.lgt_set_fermion_action(one.ctx, lgt.LGT_ACTION_EO)
+    one.set_links(U0)
+    dd.set_links(U0)
+    for traj in range(2):
+        a = lgt.lgt_hmc_trajectory(one.ctx, 3, 0.03, 1357, traj, tol=1e-13, max_iter=5000)
+        b = lgt.lgt_dd_hmc_trajectory(dd.d, 3, 0.03, 1357, traj, tol=1e-13, max_iter=5000)
+        assert abs(a[3] - b[3]) < 1e-12 * abs(a[3]) and abs(a[0] - b[0]) < 1e-9 * abs(a[3])
+        assert a[1] == b[1] and a[2] == b[2]
+        assert np.abs(gather_grid(dims, grid, dd.get_links()) - one.get_links()).max() < 1e-11
+    one.close()
     dd.close()
