@@ -78,6 +78,17 @@ int lgt_set_momenta_host(lgt_ctx* ctx, const void* P);
 int lgt_get_momenta_host(lgt_ctx* ctx, void* P);
 int lgt_set_pseudofermion_host(lgt_ctx* ctx, const void* phi);
 
+/* Asynchronous forms (undivided lattices; LGT_ESTATE on a slab handle): the transfer and the layout conversion are enqueued --
+ * the copies on the handle's own copy stream -- and the call returns at once.  The library orders them against its kernels:
+ * a kernel that touches Pi waits for a pending upload of Pi (lgt_md_kick solves first, which does not need Pi, so the upload
+ * overlaps the solve), an upload starts after everything enqueued before it, a download converts on the handle's stream and
+ * copies behind it, so that the next step's uploads and kernels run under it.  HOST buffers (pinned, for any overlap to
+ * happen) must stay valid, and a downloaded buffer is complete, only after lgt_host_transfers_wait(ctx) has returned. */
+int lgt_set_momenta_host_async(lgt_ctx* ctx, const void* P);
+int lgt_get_links_host_async(lgt_ctx* ctx, void* U);
+int lgt_get_momenta_host_async(lgt_ctx* ctx, void* P);
+int lgt_host_transfers_wait(lgt_ctx* ctx);
+
 /* ---- A1: actions (configs[0]; PAPER.md:377 Eq. S3.1) ------------------------------------ */
 /* S_g = beta sum_x sum_{mu<nu} (1 - Re tr U_P/3);  S_F = Re phi^dag (D^dag D)^-1 phi (CG to `tol`,
  * 0 if kappa == 0 or no pseudofermion is set);  K = sum ||Pi||_F^2.  Any output pointer may be NULL.

@@ -66,6 +66,14 @@ struct lgt_ctx {
     int last_outer = 0;
     void* F = nullptr;      // compact force buffer for the canonical-output calls (lazy)
     void* stage = nullptr;  // canonical staging buffer for *_host calls and conversions (lazy)
+    // asynchronous host transfers (lgt_*_host_async): a copy stream, a staging buffer per transfer kind, and the events that
+    // order them against the handle's stream (lazy)
+    cudaStream_t copy_stream = nullptr;
+    cudaEvent_t ev_main = nullptr, ev_p_up = nullptr, ev_u_down = nullptr, ev_p_down = nullptr;
+    void* stage_p_in = nullptr;
+    void* stage_u_out = nullptr;
+    void* stage_p_out = nullptr;
+    bool p_pending = false, u_down_pending = false, p_down_pending = false;
     size_t stage_bytes = 0;
     double* partials = nullptr;
     unsigned* counter = nullptr;
@@ -209,6 +217,15 @@ int ensure_force_buf(lgt_ctx* c) {
     if (c->F) return LGT_OK;
     CU(cudaMalloc(&c->F, mom_bytes(c)));
     return LGT_OK;
+}
+
+// An asynchronous upload of the momenta (lgt_set_momenta_host_async) may still be in flight on the copy stream: whoever is
+// about to launch a kernel that touches c->P first makes the handle's stream wait for it.
+inline void p_ready(lgt_ctx* c) {
+    if (c->p_pending) {
+        cudaStreamWaitEvent(c->stream, c->ev_p_up, 0);
+        c->p_pending = false;
+    }
 }
 
 // every copy derived from the links (fp32, checkerboard, smeared, the slabs' ghost slices) is stale after a link change
@@ -691,6 +708,7 @@ template <class T> struct Ops {
     if (c->dd_links_valid) *c->dd_links_valid = false;
         c->ucb_valid = false;
     c->ucb32_valid = false;
+        p_ready(c);
         LAUNCH(c, LGT_K_LINK_UPDATE, (link_update_kernel<T>), grid, 128, c->g, (const T2*)c->U, (T2*)c->U, (const T2*)c->P, (T)eps);
         return LGT_OK;
     }
@@ -699,6 +717,7 @@ template <class T> struct Ops {
         return LGT_OK;
     }
     static int kinetic(lgt_ctx* c, double* dev_result) {
+        p_ready(c);
         LAUNCH(c, LGT_K_OTHER, (kinetic_kernel<T>), stream_blocks(c, (size_t)4 * c->g.Vs), 256, c->g, (const T2*)c->P, dev_result, c->partials, c->counter);
         return LGT_OK;
     }
@@ -709,6 +728,7 @@ template <class T> struct Ops {
     }
 
     static int momentum_heatbath(lgt_ctx* c, unsigned long long seed, unsigned traj) {
+        p_ready(c);
         LAUNCH(c, LGT_K_OTHER, (momentum_heatbath_kernel<T>), stream_blocks(c, (size_t)4 * c->g.Vs), 256, c->g, (T2*)c->P, seed, traj);
         return LGT_OK;
     }
@@ -1101,7 +1121,11 @@ double metropolis_uniform(unsigned long long seed, unsigned traj) {
 }
 
 // Pi -= eps F^g
-int kick_gauge(lgt_ctx* c, double eps) { return DISPATCH(c, gauge_force, c, c->P, 1, eps); }
+int kick_gauge(lgt_ctx* c, double eps) {
+    p_ready(c);
+    p_ready(c);
+    return DISPATCH(c, gauge_force, c, c->P, 1, eps);
+}
 // Pi -= eps F^f (solve, then the fused force kernel); nothing if there are no fermions
 int kick_fermion(lgt_ctx* c, double eps, double tol, int max_iter, int* cg_iters) {
     int rc, it = 0, conv = LGT_OK;
@@ -1109,16 +1133,27 @@ int kick_fermion(lgt_ctx* c, double eps, double tol, int max_iter, int* cg_iters
         rc = solve(c, true, tol, max_iter, &it, nullptr);
         if (rc == LGT_ENOCONV) conv = rc;
         else if (rc != LGT_OK) return rc;
+        p_ready(c);
         if ((rc = DISPATCH(c, fermion_force, c, c->ws[0], c->ws[3], c->P, 1, eps)) != LGT_OK) return rc;
     }
     if (cg_iters) *cg_iters = it;
     return conv;
 }
-// Pi -= eps (F^g + F^f)
+// Pi -= eps (F^g + F^f).  The solve comes first: it does not touch Pi, so a pending asynchronous upload of the momenta
+// (lgt_set_momenta_host_async) overlaps it; the two force kernels then update Pi in the same order as before
+// (gauge, then fermion), so the result is bitwise unchanged.
 int kick(lgt_ctx* c, double eps, double tol, int max_iter, int* cg_iters) {
-    int rc;
+    int rc, it = 0, conv = LGT_OK;
+    const bool ferm = fermions_on(c);
+    if (ferm) {
+        rc = solve(c, true, tol, max_iter, &it, nullptr);
+        if (rc == LGT_ENOCONV) conv = rc;
+        else if (rc != LGT_OK) return rc;
+    }
     if ((rc = kick_gauge(c, eps)) != LGT_OK) return rc;
-    return kick_fermion(c, eps, tol, max_iter, cg_iters);
+    if (ferm && (rc = DISPATCH(c, fermion_force, c, c->ws[0], c->ws[3], c->P, 1, eps)) != LGT_OK) return rc;
+    if (cg_iters) *cg_iters = it;
+    return conv;
 }
 
 // MD trajectory of nsteps steps of size dt, adjacent kicks merged (include/lgt.h "lgt_set_integrator").  S supplies the
@@ -1387,6 +1422,12 @@ int lgt_destroy(lgt_ctx* c) {
     cudaFree(c->eo32);
     for (int i = 0; i < 5; i++) cudaFree(c->ws32[i]);
     cudaFree(c->stage);
+    cudaFree(c->stage_p_in);
+    cudaFree(c->stage_u_out);
+    cudaFree(c->stage_p_out);
+    if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
+    for (cudaEvent_t e : {c->ev_main, c->ev_p_up, c->ev_u_down, c->ev_p_down})
+        if (e) cudaEventDestroy(e);
     cudaFree(c->partials);
     cudaFree(c->counter);
     cudaFree(c->coop_counter);
@@ -1485,11 +1526,13 @@ int lgt_get_links(lgt_ctx* c, void* U) {
 int lgt_set_momenta(lgt_ctx* c, const void* P) {
     CHECK_CTX(c);
     if (!P) return fail(c, LGT_EINVAL, "lgt_set_momenta: null pointer");
+    p_ready(c);
     return DISPATCH(c, momenta_to_native, c, P, c->P);
 }
 int lgt_get_momenta(lgt_ctx* c, void* P) {
     CHECK_CTX(c);
     if (!P) return fail(c, LGT_EINVAL, "lgt_get_momenta: null pointer");
+    p_ready(c);
     return DISPATCH(c, momenta_from_native, c, c->P, P);
 }
 int lgt_set_pseudofermion(lgt_ctx* c, const void* phi) {
@@ -1531,6 +1574,75 @@ HOST_GET(lgt_get_links_host, lgt_get_links, (size_t)36 * (c->g.s_end - c->g.s_be
 HOST_SET(lgt_set_momenta_host, lgt_set_momenta, (size_t)36 * (c->g.s_end - c->g.s_begin) * c->esize)
 HOST_GET(lgt_get_momenta_host, lgt_get_momenta, (size_t)36 * (c->g.s_end - c->g.s_begin) * c->esize)
 HOST_SET(lgt_set_pseudofermion_host, lgt_set_pseudofermion, (size_t)12 * (c->g.s_end - c->g.s_begin) * c->esize)
+
+// ---- asynchronous host transfers
+namespace {
+int ensure_async(lgt_ctx* c) {
+    if (c->dd_links_valid) return fail(c, LGT_ESTATE, "the asynchronous host transfers are for undivided lattices");
+    if (c->copy_stream) return LGT_OK;
+    CU(cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking));
+    CU(cudaEventCreateWithFlags(&c->ev_main, cudaEventDisableTiming));
+    CU(cudaEventCreateWithFlags(&c->ev_p_up, cudaEventDisableTiming));
+    CU(cudaEventCreateWithFlags(&c->ev_u_down, cudaEventDisableTiming));
+    CU(cudaEventCreateWithFlags(&c->ev_p_down, cudaEventDisableTiming));
+    return LGT_OK;
+}
+// device -> host of one field: conversion on the handle's stream into the field's own staging buffer (after the previous
+// download from that buffer has left it), then the copy on the copy stream
+int download_async(lgt_ctx* c, void** stage, bool* pending, cudaEvent_t done, int (*convert)(lgt_ctx*, void*), void* h, size_t bytes) {
+    int rc;
+    if ((rc = ensure_async(c)) != LGT_OK) return rc;
+    if (!*stage) CU(cudaMalloc(stage, bytes));
+    if (*pending) CU(cudaStreamWaitEvent(c->stream, done, 0));
+    if ((rc = convert(c, *stage)) != LGT_OK) return rc;
+    CU(cudaEventRecord(c->ev_main, c->stream));
+    CU(cudaStreamWaitEvent(c->copy_stream, c->ev_main, 0));
+    CU(cudaMemcpyAsync(h, *stage, bytes, cudaMemcpyDeviceToHost, c->copy_stream));
+    CU(cudaEventRecord(done, c->copy_stream));
+    *pending = true;
+    return LGT_OK;
+}
+}  // namespace
+
+int lgt_set_momenta_host_async(lgt_ctx* c, const void* h) {
+    CHECK_CTX(c);
+    if (!h) return fail(c, LGT_EINVAL, "lgt_set_momenta_host_async: null pointer");
+    int rc;
+    if ((rc = ensure_async(c)) != LGT_OK) return rc;
+    const size_t bytes = (size_t)36 * c->g.V * c->esize;
+    if (!c->stage_p_in) CU(cudaMalloc(&c->stage_p_in, bytes));
+    p_ready(c);  // an earlier pending upload: keep the order
+    // everything enqueued so far may still read or write Pi (and the staging buffer): the copy stream starts after it
+    CU(cudaEventRecord(c->ev_main, c->stream));
+    CU(cudaStreamWaitEvent(c->copy_stream, c->ev_main, 0));
+    CU(cudaMemcpyAsync(c->stage_p_in, h, bytes, cudaMemcpyHostToDevice, c->copy_stream));
+    cudaStream_t const main_stream = c->stream;
+    c->stream = c->copy_stream;  // the conversion kernel follows the copy on the copy stream
+    rc = DISPATCH(c, momenta_to_native, c, c->stage_p_in, c->P);
+    c->stream = main_stream;
+    if (rc != LGT_OK) return rc;
+    CU(cudaEventRecord(c->ev_p_up, c->copy_stream));
+    c->p_pending = true;
+    return LGT_OK;
+}
+int lgt_get_links_host_async(lgt_ctx* c, void* h) {
+    CHECK_CTX(c);
+    if (!h) return fail(c, LGT_EINVAL, "lgt_get_links_host_async: null pointer");
+    return download_async(c, &c->stage_u_out, &c->u_down_pending, c->ev_u_down, [](lgt_ctx* cc, void* st) { return lgt_get_links(cc, st); }, h,
+                          (size_t)36 * c->g.V * c->esize);
+}
+int lgt_get_momenta_host_async(lgt_ctx* c, void* h) {
+    CHECK_CTX(c);
+    if (!h) return fail(c, LGT_EINVAL, "lgt_get_momenta_host_async: null pointer");
+    return download_async(c, &c->stage_p_out, &c->p_down_pending, c->ev_p_down, [](lgt_ctx* cc, void* st) { return lgt_get_momenta(cc, st); }, h,
+                          (size_t)36 * c->g.V * c->esize);
+}
+int lgt_host_transfers_wait(lgt_ctx* c) {
+    CHECK_CTX(c);
+    if (c->copy_stream) CU(cudaStreamSynchronize(c->copy_stream));
+    c->u_down_pending = c->p_down_pending = false;
+    return LGT_OK;
+}
 
 // ---- actions
 int lgt_action(lgt_ctx* c, double tol, int max_iter, double* S_g, double* S_F, double* K, int* cg_iters) {
@@ -1700,6 +1812,7 @@ int lgt_fermion_force_native(lgt_ctx* c, const void* X, const void* Y, double ep
     CHECK_CTX(c);
     NOT_SLAB(c);
     if (!X || !Y) return fail(c, LGT_EINVAL, "lgt_fermion_force_native: null pointer");
+    p_ready(c);
     return DISPATCH(c, fermion_force, c, X, Y, c->P, 1, eps);
 }
 

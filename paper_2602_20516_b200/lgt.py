@@ -36,6 +36,10 @@ SYMBOLS = {
     "lgt_set_momenta_host": (_i, [_vp, _vp]),
     "lgt_get_momenta_host": (_i, [_vp, _vp]),
     "lgt_set_pseudofermion_host": (_i, [_vp, _vp]),
+    "lgt_set_momenta_host_async": (_i, [_vp, _vp]),
+    "lgt_get_links_host_async": (_i, [_vp, _vp]),
+    "lgt_get_momenta_host_async": (_i, [_vp, _vp]),
+    "lgt_host_transfers_wait": (_i, [_vp]),
     "lgt_action": (_i, [_vp, _d, _i, _dp, _dp, _dp, _ip]),
     "lgt_plaquette": (_i, [_vp, _dp]),
     "lgt_dslash": (_i, [_vp, _vp, _vp, _i]),
@@ -200,6 +204,22 @@ def lgt_get_momenta_host(ctx, P):
 
 def lgt_set_pseudofermion_host(ctx, phi):
     return _check(ctx, lib().lgt_set_pseudofermion_host(ctx, _ptr(phi)))
+
+
+def lgt_set_momenta_host_async(ctx, P):
+    return _check(ctx, lib().lgt_set_momenta_host_async(ctx, _ptr(P)))
+
+
+def lgt_get_links_host_async(ctx, U):
+    return _check(ctx, lib().lgt_get_links_host_async(ctx, _ptr(U)))
+
+
+def lgt_get_momenta_host_async(ctx, P):
+    return _check(ctx, lib().lgt_get_momenta_host_async(ctx, _ptr(P)))
+
+
+def lgt_host_transfers_wait(ctx):
+    return _check(ctx, lib().lgt_host_transfers_wait(ctx))
 
 
 def lgt_action(ctx, tol=1e-12, max_iter=100000):

@@ -121,6 +121,55 @@ def test_dslash_kernel_variants(lgt, dims):
     lat.close()
 
 
+def test_async_host_transfers_match_the_blocking_ones(lgt):
+    """lgt_set_momenta_host_async / lgt_get_*_host_async: the momenta upload runs on the copy stream under the solve (the
+    kick solves first and only then touches Pi), the downloads run under whatever follows.  Two MD steps driven through the
+    asynchronous calls give bitwise the links and momenta of the blocking calls, the downloaded buffers are complete after
+    lgt_host_transfers_wait, and a second upload / download issued before the first has drained keeps the order."""
+    import torch
+
+    dims, beta, kappa = (8, 8, 8, 8), 5.6, 0.12
+    V = synth.volume(dims)
+    U = synth.warm_links(dims, 0.3, 57)
+    P = synth.gaussian_momenta(dims, 58)
+    P2 = synth.gaussian_momenta(dims, 59)
+    phi = oracle.dslash(dims, kappa, BC, U, synth.gaussian_spinor(dims, 60), dagger=True)
+    hU, hP, hP2, hphi = [torch.from_numpy(a).pin_memory() for a in (U, P, P2, phi)]
+    out = {}
+    for mode in ("blocking", "async"):
+        lat = lgt.Lattice(dims, beta, kappa, BC)
+        hUo, hPo, hPo1 = [torch.zeros((V, 4, 3, 3), dtype=torch.complex128).pin_memory() for _ in range(3)]
+        lgt.lgt_set_links_host(lat.ctx, hU)
+        lgt.lgt_set_pseudofermion_host(lat.ctx, hphi)
+        if mode == "blocking":
+            lgt.lgt_set_momenta_host(lat.ctx, hP2)
+            lgt.lgt_set_momenta_host(lat.ctx, hP)
+        else:
+            lgt.lgt_set_momenta_host_async(lat.ctx, hP2)  # overwritten by the next upload, in order
+            lgt.lgt_set_momenta_host_async(lat.ctx, hP)
+        its = [lgt.lgt_md_kick(lat.ctx, 0.02, 1e-12, 5000)]
+        if mode == "blocking":
+            lgt.lgt_get_momenta_host(lat.ctx, hPo1)
+        else:
+            lgt.lgt_get_momenta_host_async(lat.ctx, hPo1)
+        lgt.lgt_md_drift(lat.ctx, 0.02)
+        its.append(lgt.lgt_md_kick(lat.ctx, 0.02, 1e-12, 5000))
+        if mode == "blocking":
+            lgt.lgt_get_links_host(lat.ctx, hUo)
+            lgt.lgt_get_momenta_host(lat.ctx, hPo)
+        else:
+            lgt.lgt_get_links_host_async(lat.ctx, hUo)
+            lgt.lgt_get_momenta_host_async(lat.ctx, hPo)
+            lgt.lgt_host_transfers_wait(lat.ctx)
+        out[mode] = (hUo.numpy().copy(), hPo.numpy().copy(), hPo1.numpy().copy(), its)
+        lat.close()
+    for a, b in zip(out["blocking"][:3], out["async"][:3]):
+        assert np.array_equal(a, b)
+    assert out["blocking"][3] == out["async"][3]
+    P1, _, _ = oracle.kick(dims, beta, kappa, BC, U, phi, P, 0.02, 1e-12, 5000)
+    assert link_rel_err(out["async"][2], P1)[0] < TOL64
+
+
 @pytest.mark.parametrize("dims", [(8, 8, 8, 8), (4, 3, 5, 6), (16, 4, 6, 2)])
 def test_gauge_force_kernel_variants(lgt, dims):
     """The implementation variants of the staple kernel (lgt_set_kernel_variant(LGT_K_GAUGE_FORCE)): 1 and 2 only regroup the
