@@ -1885,14 +1885,17 @@ __device__ __forceinline__ void hop_bwd_cb(const Geom& g, const typename Vec2<T>
 // With kap = -kappa and no self this is the odd half "t_o = kappa H_oe p_e"; with kap = +kappa and self = p_e the
 // even half "p_e - kappa H_eo t_o" of the Schur complement M = 1 - kappa^2 H_eo H_oe.
 // PUSH (time slab, CG modes 1 and 2): as in dslash_kernel, for the half field the launch produces (u in MODE 1, r in MODE 2).
-template <class T, int DAG, int MODE, int PUSH = 0, int ZS = 0>
+// PFL: at the end of the block, an L2 prefetch of what the block `pf` positions further on will read from DRAM first -- its
+// own-parity link block (contiguous) and, of the other parity's links, the z and t components at its backward neighbours
+// (variant 8 of the Dslash kernel; used for the fp32 kernels, where it pays).
+template <class T, int DAG, int MODE, int PUSH = 0, int ZS = 0, int PFL = 0>
 __global__ void __launch_bounds__(128, 1) hop_cb_kernel(Geom g, int p, const typename Vec2<T>::type* __restrict__ Up,
                                                         const typename Vec2<T>::type* __restrict__ Uq,
                                                         const typename Vec2<T>::type* __restrict__ in,
                                                         const typename Vec2<T>::type* __restrict__ self,
                                                         typename Vec2<T>::type* __restrict__ out, T kap, CgState* st,
                                                         double* partials, typename Vec2<T>::type* __restrict__ r, PushTo<T> push,
-                                                        unsigned* fuse = nullptr) {
+                                                        unsigned* fuse = nullptr, int pf = 0) {
     const int done = (MODE != 0) ? st->done : 0;
     if (MODE == 1 && fuse && done && blockIdx.x == 0 && threadIdx.x == 0) st->fresh = 0;  // as in dslash_kernel
     const int c = g.h_begin + blockIdx.x * blockDim.x + threadIdx.x;
@@ -1919,6 +1922,25 @@ __global__ void __launch_bounds__(128, 1) hop_cb_kernel(Geom g, int p, const typ
         hop_bwd_cb<2, -F, T>(g, Uq, in, cs, s, acc);
         hop_fwd_cb<3, F, T>(g, Up, in, cs, s, c, acc);
         hop_bwd_cb<3, -F, T>(g, Uq, in, cs, s, acc);
+        if (PFL && blockIdx.x + pf < gridDim.x) {
+            const int lane = threadIdx.x & 31;
+            const int cp = c - lane + pf * (int)blockDim.x;  // first site of this warp's counterpart in the later block
+            if (cp < g.h_end) {
+                constexpr int CPL = 128 / (int)sizeof(typename Vec2<T>::type);
+                const typename Vec2<T>::type* bu = link_at(Up, cp, 0);
+#pragma unroll
+                for (int j = 0; j < (36 * W / CPL + 31) / 32; j++)
+                    if (lane + 32 * j < 36 * W / CPL) asm volatile("prefetch.global.L2 [%0];" ::"l"(bu + (lane + 32 * j) * CPL));
+                // the spinor block one time slice on (the forward t hop's first touch)
+                const int ct = cp + (g.stride[3] >> 1);
+                if (ct < g.h_end) {
+                    const typename Vec2<T>::type* bp = spinor_at(in, ct);
+#pragma unroll
+                    for (int j = 0; j < (12 * W / CPL + 31) / 32; j++)
+                        if (lane + 32 * j < 12 * W / CPL) asm volatile("prefetch.global.L2 [%0];" ::"l"(bp + (lane + 32 * j) * CPL));
+                }
+            }
+        }
         if (MODE == 2) {
             const T alpha = (T)st->alpha;
             const typename Vec2<T>::type* bi = spinor_at(self, c);

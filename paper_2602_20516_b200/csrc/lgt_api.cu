@@ -820,6 +820,22 @@ template <class T> struct Ops {
             }
             return LGT_OK;
         }
+        if (sizeof(T) == 4 && c->variant[LGT_K_DSLASH] == 0 && grid > 2 * c->num_sms && grid <= 16384 && !c->dd_links_valid) {
+            // the fp32 hops with the end-of-block L2 prefetch for the block that takes this block's place (as the fp32 Dslash default)
+            const int pf = 2 * c->num_sms;
+            if (mode == 0) {
+                if (dagger) LAUNCH(c, LGT_K_DSLASH, (hop_cb_kernel<T, 1, 0, 0, 0, 1>), grid, 128, HOP_ARGS, nullptr, pf);
+                else LAUNCH(c, LGT_K_DSLASH, (hop_cb_kernel<T, 0, 0, 0, 0, 1>), grid, 128, HOP_ARGS, nullptr, pf);
+            } else if (mode == 3) {
+                if (dagger) LAUNCH(c, LGT_K_DSLASH, (hop_cb_kernel<T, 1, 3, 0, 0, 1>), grid, 128, HOP_ARGS, nullptr, pf);
+                else LAUNCH(c, LGT_K_DSLASH, (hop_cb_kernel<T, 0, 3, 0, 0, 1>), grid, 128, HOP_ARGS, nullptr, pf);
+            } else if (mode == 1) {
+                LAUNCH(c, LGT_K_DSLASH, (hop_cb_kernel<T, 0, 1, 0, 0, 1>), grid, 128, HOP_ARGS, fuse_counter(c), pf);
+            } else {
+                LAUNCH(c, LGT_K_DSLASH_R, (hop_cb_kernel<T, 1, 2, 0, 0, 1>), grid, 128, HOP_ARGS, fuse_counter(c), pf);
+            }
+            return LGT_OK;
+        }
         if (mode == 0) {
             if (dagger) LAUNCH(c, LGT_K_DSLASH, (hop_cb_kernel<T, 1, 0>), grid, 128, HOP_ARGS);
             else LAUNCH(c, LGT_K_DSLASH, (hop_cb_kernel<T, 0, 0>), grid, 128, HOP_ARGS);
