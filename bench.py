@@ -81,7 +81,8 @@ VARIANT_NAMES = {
                "12-real links: rows 0, 1 read, row 2 rebuilt in registers (768 B per site)",
                "variant 0 + the L2 prefetch of variant 4 issued at the end of each block (the fp32 default)",
                "persistent, DRAM-bound operands (forward links, t+1 spinor) by per-thread cp.async into shared memory one chunk ahead",
-               "variant 1 with the chunks drawn from a global counter instead of a fixed stride"],
+               "variant 1 with the chunks drawn from a global counter instead of a fixed stride",
+               "two chunks per block as straight-line code"],
     "gauge_force": ["one 32-site layout block x 4 directions per 128-thread block (default)",
                     "two layout blocks per 256-thread block",
                     "four layout blocks per 512-thread block (128 registers)",

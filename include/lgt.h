@@ -363,7 +363,7 @@ void* lgt_stream(const lgt_ctx* ctx);
 int lgt_set_block_swizzle(lgt_ctx* ctx, int z_planes, int* in_effect);
 /* Implementation variant of one kernel class (LGT_K_*); every variant computes the same operation and
  * the alternatives stay in the library so that each measurement in profiles/ can be repeated.
- *   LGT_K_DSLASH (covers LGT_K_DSLASH_R; D and D^dag bitwise the same in variants 0-5 and 8-10):
+ *   LGT_K_DSLASH (covers LGT_K_DSLASH_R; D and D^dag bitwise the same in variants 0-5 and 8-11):
  *     0 = one 128-site block per chunk (dslash_kernel; the default and, measured, the fastest in fp64; for the fp32 kernels
  *         on lattices of 297 ... 16384 chunks the default carries variant 8's prefetch, which gains 4-10 % per fp32 CG iteration);
  *     1 = persistent software-pipelined kernel: one wave of blocks loops over the chunks with the next chunk's first
@@ -381,6 +381,7 @@ int lgt_set_block_swizzle(lgt_ctx* ctx, int z_planes, int* in_effect);
  *     9 = persistent kernel with the DRAM-bound operands (the four forward links and the t+1 spinor of a site) requested one
  *         chunk ahead by per-thread cp.async into thread-private shared-memory slots (768 B per thread in fp64);
  *     10 = variant 1 with the chunks after a block's first drawn from a global counter (dynamic instead of strided assignment);
+ *     11 = two chunks per block as straight-line code (the first site's tail under the second site's first loads);
  *     7 = 12-real links: rows 0 and 1 of every link are read and row 2 = sign * conj(row0 x row1) is
  *         rebuilt in registers (768 instead of 960 compulsory bytes per site).  Exact for special unitary links; links
  *         that have drifted from unitarity by delta change the operator by O(delta).

@@ -1020,6 +1020,85 @@ __global__ void __launch_bounds__(128, 1) dslash_cpasync_kernel(Geom g, const ty
     asm volatile("cp.async.wait_group 0;" ::: "memory");  // the last chunk's (unused) re-requests
 }
 
+// Variant 11: two chunks per block, as straight-line code.  A block of dslash_kernel ends with a serial tail -- the own-site
+// loads, the (read-modify-)write, the block sum -- during which it has no loads in flight, and the next block starts with
+// empty registers.  Here every thread does the site of chunk 2b and then the site of chunk 2b + 1 in ONE basic block, so the
+// compiler's rolling window of loads runs on from the first site's last hops into the second site's first hops and the
+// first site's tail is covered.  Unlike the persistent kernels there is no loop-carried state and the hardware still hands
+// out blocks dynamically.  One block partial per chunk at the chunk's index: bitwise the sums of variant 0.
+template <class T, int DAG, int MODE>
+__device__ __forceinline__ double dslash_site_body(const Geom& g, const typename Vec2<T>::type* __restrict__ U,
+                                                   const typename Vec2<T>::type* __restrict__ in, typename Vec2<T>::type* __restrict__ out,
+                                                   T kappa, const CgState* st, typename Vec2<T>::type* __restrict__ r, int s) {
+    double nrm = 0.0;
+    if (s < g.s_end) {
+        if (MODE == 2) {
+            const typename Vec2<T>::type* br = spinor_at(r, s);
+#pragma unroll
+            for (int k = 0; k < 12; k++) asm volatile("prefetch.global.L2 [%0];" ::"l"(br + k * W));
+        }
+        const Site c = site_coords(g, s);
+        cx<T> acc[12];
+#pragma unroll
+        for (int k = 0; k < 12; k++) acc[k] = mk<T>(0, 0);
+        constexpr int F = DAG ? +1 : -1;
+        hop_fwd<0, F, T>(g, U, in, c, s, acc);
+        hop_bwd<0, -F, T>(g, U, in, c, s, acc);
+        hop_fwd<1, F, T>(g, U, in, c, s, acc);
+        hop_bwd<1, -F, T>(g, U, in, c, s, acc);
+        hop_fwd<2, F, T>(g, U, in, c, s, acc);
+        hop_bwd<2, -F, T>(g, U, in, c, s, acc);
+        hop_fwd<3, F, T>(g, U, in, c, s, acc);
+        hop_bwd<3, -F, T>(g, U, in, c, s, acc);
+        const typename Vec2<T>::type* bi = spinor_at(in, s);
+        if (MODE == 2) {
+            const T alpha = (T)st->alpha;
+            typename Vec2<T>::type* br = spinor_at(r, s);
+#pragma unroll
+            for (int k = 0; k < 12; k++) {
+                cx<T> tv = ldc<T>(bi + k * W);
+                cx<T> q = mk<T>(fma(-kappa, acc[k].re, tv.re), fma(-kappa, acc[k].im, tv.im));
+                cx<T> rv = ldc_rw<T>(br + k * W);
+                rv.re = fma(-alpha, q.re, rv.re);
+                rv.im = fma(-alpha, q.im, rv.im);
+                stc<T>(br + k * W, rv);
+                nrm += (double)rv.re * (double)rv.re + (double)rv.im * (double)rv.im;
+            }
+        } else {
+            typename Vec2<T>::type* bo = spinor_at(out, s);
+#pragma unroll
+            for (int k = 0; k < 12; k++) {
+                cx<T> pv = ldc<T>(bi + k * W);
+                cx<T> o = mk<T>(fma(-kappa, acc[k].re, pv.re), fma(-kappa, acc[k].im, pv.im));
+                stc<T>(bo + k * W, o);
+                if (MODE == 1) nrm += (double)o.re * (double)o.re + (double)o.im * (double)o.im;
+            }
+        }
+    } else if (s >= g.V && s < g.Vs && MODE != 2) {  // padding lanes only, never a ghost slice
+        typename Vec2<T>::type* bo = spinor_at(out, s);
+#pragma unroll
+        for (int k = 0; k < 12; k++) stc<T>(bo + k * W, mk<T>(0, 0));
+    }
+    return nrm;
+}
+template <class T, int DAG, int MODE>
+__global__ void __launch_bounds__(128, 1) dslash_two_kernel(Geom g, const typename Vec2<T>::type* __restrict__ U,
+                                                            const typename Vec2<T>::type* __restrict__ in,
+                                                            typename Vec2<T>::type* __restrict__ out, T kappa, CgState* st,
+                                                            double* partials, typename Vec2<T>::type* __restrict__ r, int nchunks) {
+    if (MODE != 0 && st->done) return;  // uniform over the grid
+    const int ch0 = 2 * blockIdx.x, ch1 = ch0 + 1;
+    const int s0 = g.s_begin + swizzled_chunk(g, ch0) * 128 + threadIdx.x;
+    const int s1 = ch1 < nchunks ? g.s_begin + swizzled_chunk(g, ch1) * 128 + threadIdx.x : g.Vs;  // past everything: nothing to do
+    const double n0 = dslash_site_body<T, DAG, MODE>(g, U, in, out, kappa, st, r, s0);
+    const double n1 = dslash_site_body<T, DAG, MODE>(g, U, in, out, kappa, st, r, s1);
+    if (MODE != 0) {
+        block_partial(n0, partials + ch0 - blockIdx.x);
+        __syncthreads();
+        if (ch1 < nchunks) block_partial(n1, partials + ch1 - blockIdx.x);
+    }
+}
+
 // Variant 3: 4-D site blocking by block-to-site mapping (the layout is unchanged).  dslash_kernel's block is 128
 // consecutive lexicographic sites (four x rows at 32^4), so of the nine spinors and eight links a site needs only the
 // x and most y neighbours are shared inside the block: L2 -> L1 traffic is 2.06 KB per site for 0.96 KB compulsory.

@@ -347,7 +347,7 @@ template <class T> struct Ops {
     // tail, and the slabs of a decomposed lattice split their sums around an all-reduce.
     static unsigned* fuse_counter(const lgt_ctx* c) {
         const int dv = c->variant[LGT_K_DSLASH];
-        return (c->variant[LGT_K_CG_BLAS] == 1 && !c->dd_links_valid && dv != 1 && dv != 2 && dv != 3 && dv != 9 && dv != 10) ? c->counter : nullptr;
+        return (c->variant[LGT_K_CG_BLAS] == 1 && !c->dd_links_valid && dv != 1 && dv != 2 && dv != 3 && dv != 9 && dv != 10 && dv != 11) ? c->counter : nullptr;
     }
     // The one-launch cooperative CG (variant 2 of LGT_K_CG_BLAS; default up to two waves of blocks): undivided lattices only
     static bool coop_wanted(const lgt_ctx* c, int nchunks) {
@@ -384,6 +384,22 @@ template <class T> struct Ops {
             } else {
                 LAUNCH(c, LGT_K_DSLASH_R, (dslash_kernel<T, 1, 2, 0, 0, 1>), grid, 128, DSLASH_ARGS);
             }
+            return LGT_OK;
+        }
+        if (c->variant[LGT_K_DSLASH] == 11) {  // two chunks per block as straight-line code
+            const int g2 = (grid + 1) / 2;
+#define DSLASH_2ARGS c->g, (const T2*)U, (const T2*)in, (T2*)out, kappa, c->st, c->partials, (T2*)r, grid
+            if (mode == 0) {
+                if (dagger)
+                    LAUNCH(c, LGT_K_DSLASH, (dslash_two_kernel<T, 1, 0>), g2, 128, DSLASH_2ARGS);
+                else
+                    LAUNCH(c, LGT_K_DSLASH, (dslash_two_kernel<T, 0, 0>), g2, 128, DSLASH_2ARGS);
+            } else if (mode == 1) {
+                LAUNCH(c, LGT_K_DSLASH, (dslash_two_kernel<T, 0, 1>), g2, 128, DSLASH_2ARGS);
+            } else {
+                LAUNCH(c, LGT_K_DSLASH_R, (dslash_two_kernel<T, 1, 2>), g2, 128, DSLASH_2ARGS);
+            }
+#undef DSLASH_2ARGS
             return LGT_OK;
         }
         if (c->variant[LGT_K_DSLASH] == 10) {  // variant 1 with the chunks drawn from a counter instead of a fixed stride
@@ -1508,7 +1524,7 @@ int lgt_set_kernel_variant(lgt_ctx* c, int kernel_class, int variant, int* in_ef
     CHECK_CTX(c);
     if (kernel_class < 0 || kernel_class >= LGT_K_COUNT) return fail(c, LGT_EINVAL, "lgt_set_kernel_variant: unknown kernel class");
     if (variant >= 0) {
-        const int nvar = (kernel_class == LGT_K_DSLASH) ? 11 : (kernel_class == LGT_K_GAUGE_FORCE) ? 4 : (kernel_class == LGT_K_CG_BLAS) ? 3 : 1;
+        const int nvar = (kernel_class == LGT_K_DSLASH) ? 12 : (kernel_class == LGT_K_GAUGE_FORCE) ? 4 : (kernel_class == LGT_K_CG_BLAS) ? 3 : 1;
         if (variant >= nvar) return fail(c, LGT_EINVAL, "lgt_set_kernel_variant: this kernel class has no such variant");
         if (c->variant[kernel_class] != variant) {
             // captured CG chunks hold the old kernels

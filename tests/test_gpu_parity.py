@@ -103,7 +103,7 @@ def test_dslash_kernel_variants(lgt, dims):
     x0, it0, _, ok0 = lat.cg(psi, 1e-10, 2000)
     _, it_ref, _, ok_ref = oracle.cg(dims, 0.12, BC, U, psi, 1e-10, 2000)
     assert ok0 and ok_ref and it0 == it_ref
-    for v in (1, 2, 3, 4, 5, 6, 7, 8, 9, 10):
+    for v in (1, 2, 3, 4, 5, 6, 7, 8, 9, 10, 11):
         assert lgt.lgt_set_kernel_variant(lat.ctx, lgt.LGT_K_DSLASH, v) == v
         for d in (False, True):
             if v in (6, 7):  # 6 sums the eight hops in another order, 7 rebuilds the third row of every link
@@ -114,7 +114,7 @@ def test_dslash_kernel_variants(lgt, dims):
         assert ok and it == it0, (v, it, it0)
         assert np.abs(x - x0).max() <= 1e-12 * np.abs(x0).max()  # variant 3 sums other block partials
     with pytest.raises(lgt.LgtError):
-        lgt.lgt_set_kernel_variant(lat.ctx, lgt.LGT_K_DSLASH, 11)
+        lgt.lgt_set_kernel_variant(lat.ctx, lgt.LGT_K_DSLASH, 12)
     with pytest.raises(lgt.LgtError):
         lgt.lgt_set_kernel_variant(lat.ctx, 99, 0)
     assert lgt.lgt_set_kernel_variant(lat.ctx, lgt.LGT_K_DSLASH, 0) == 0
