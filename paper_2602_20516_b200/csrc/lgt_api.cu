@@ -154,14 +154,12 @@ cudaEvent_t timing_event(lgt_ctx* c) {
         if (e_ != cudaSuccess) return fail((c), LGT_ECUDA, #kern, e_); \
     } while (0)
 
-// the same with dynamic shared memory (opt-in above 48 KB, once per kernel instantiation)
+// the same with dynamic shared memory (opt-in above 48 KB)
 #define LAUNCH_SMEM(c, kclass, kern, grid, block, smem, ...)        \
     do {                                                            \
-        static bool attr_set_ = false;                              \
-        if (!attr_set_) {                                           \
+        {   /* per device, so set on every launch (a host-side table lookup) */ \
             cudaError_t ea_ = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (smem)); \
             if (ea_ != cudaSuccess) return fail((c), LGT_ECUDA, "cudaFuncSetAttribute " #kern, ea_); \
-            attr_set_ = true;                                       \
         }                                                           \
         cudaEvent_t e0_ = nullptr, e1_ = nullptr;                   \
         if ((c)->timing) {                                          \
@@ -1434,6 +1432,7 @@ int lgt_destroy(lgt_ctx* c) {
     if (!c) return LGT_OK;
     DeviceGuard guard(c->device);
     cudaStreamSynchronize(c->stream);
+    if (c->copy_stream) cudaStreamSynchronize(c->copy_stream);  // pending asynchronous host transfers
     cudaFree(c->U);
     cudaFree(c->P);
     cudaFree(c->phi);
