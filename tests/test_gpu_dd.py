@@ -181,6 +181,14 @@ def test_dd_host_slab_roundtrip(lgt):
     dd.close()
 
 
+def lgt_dag(lgt, dims, c, U, psi):
+    one = lgt.Lattice(dims, c["beta"], c["kappa"], c["bc"])
+    one.set_links(U)
+    out = one.dslash(psi, dagger=True)
+    one.close()
+    return out
+
+
 def test_dd_full_size_dslash_four_slabs(lgt):
     """configs[3]'s 32^4 lattice in four slabs on this GPU: bitwise equal to the undivided Dslash, sampled sites against
     the oracle (incl. sites on slab boundaries and on the antiperiodic time boundary)."""
@@ -198,6 +206,12 @@ def test_dd_full_size_dslash_four_slabs(lgt):
     out = cat(dd.dslash(psi))
     dd.close()
     assert np.array_equal(out, ref)
+    # the same lattice on a 2 x 2 (t, z) grid of ranks
+    dg = lgt.DecomposedLattice(dims, 4, [0, 1, 2, 3], c["beta"], kappa, bc, grid=(2, 2))
+    dg.set_links(U)
+    assert np.array_equal(gather_grid(dims, (2, 2), dg.dslash(psi)), ref)
+    assert np.array_equal(gather_grid(dims, (2, 2), dg.dslash(psi, dagger=True)), lgt_dag(lgt, dims, c, U, psi))
+    dg.close()
     V3 = dims[0] * dims[1] * dims[2]
     sites = np.array([0, 5, V3 * 8 - 1, V3 * 8, V3 * 16 + 77, V3 * 24 - 3, V - V3 + 9, V - 1], dtype=np.int64)
     assert np.abs(out[sites] - oracle.dslash_sites(dims, kappa, bc, U, psi, sites)).max() < 1e-12
