@@ -462,8 +462,11 @@ __device__ __forceinline__ void dslash_prefetch_block(const Geom& g, const typen
 // PF > 0 (variant 4): every thread first asks L2 for the lines the block PF positions further on in the grid will need
 // from DRAM first -- its forward links and its t+1 spinors -- so that those loads find their data in L2 (prefetches hold
 // no registers; PF = the number of co-resident blocks, i.e. the block that takes this block's place on the SM).
-template <class T, int DAG, int MODE, int PUSH = 0, int PFON = 0, int ZS = 0>
-__global__ void __launch_bounds__(128, 1) dslash_kernel(Geom g, const typename Vec2<T>::type* __restrict__ U,
+// LB3: compiled for three blocks per SM (168 registers).  In fp64 that costs more in load batching than the extra warps give
+// (203 against 184 us); in fp32, where half the registers hold the same number of loads, it gains 5 % per CG iteration on
+// lattices of more than one wave of blocks (and loses 12 % on a single wave, where the default stays).
+template <class T, int DAG, int MODE, int PUSH = 0, int PFON = 0, int ZS = 0, int LB3 = 0>
+__global__ void __launch_bounds__(128, LB3 ? 3 : 1) dslash_kernel(Geom g, const typename Vec2<T>::type* __restrict__ U,
                                                         const typename Vec2<T>::type* __restrict__ in,
                                                         typename Vec2<T>::type* __restrict__ out, T kappa, CgState* st,
                                                         double* partials, typename Vec2<T>::type* __restrict__ r, PushTo<T> push,
@@ -1339,7 +1342,7 @@ __device__ __forceinline__ void fermion_force_link(const Geom& g, const typename
 // register budget is left to the compiler as in dslash_kernel: measured 258 us against 280 us for a one-link-per-
 // thread version on 32^4 fp64 (profiles/).
 template <class T, int ACC>
-__global__ void __launch_bounds__(128, 1) fermion_force_kernel(Geom g, const typename Vec2<T>::type* __restrict__ U,
+__global__ void __launch_bounds__(128, sizeof(T) == 4 ? 3 : 1) fermion_force_kernel(Geom g, const typename Vec2<T>::type* __restrict__ U,
                                                                const typename Vec2<T>::type* __restrict__ X,
                                                                const typename Vec2<T>::type* __restrict__ Y,
                                                                typename Vec2<T>::type* __restrict__ P, T kappa, T eps) {
@@ -1370,7 +1373,7 @@ __global__ void __launch_bounds__(128, 1) fermion_force_kernel(Geom g, const typ
 // constant (no indexed local Site array, 0 bytes of stack) was measured at 989 us against 606 us at 32^4 fp64 -- the
 // compiler then schedules each staple's loads behind the previous staple's arithmetic again.
 template <class T, int ACC, int ROWS = 1>
-__global__ void __launch_bounds__(128 * ROWS, ROWS == 1 ? 2 : 1)
+__global__ void __launch_bounds__(128 * ROWS, ROWS == 1 ? (sizeof(T) == 4 ? 4 : 2) : 1)
     gauge_force_kernel(Geom g, const typename Vec2<T>::type* __restrict__ U, typename Vec2<T>::type* __restrict__ P,
                        T beta_over_6, T eps) {
     // same slab-by-slab block order as the Dslash kernels on lattices whose time slice exceeds L2 (four 32-site blocks
@@ -1967,8 +1970,11 @@ __device__ __forceinline__ void hop_bwd_cb(const Geom& g, const typename Vec2<T>
 // PFL: at the end of the block, an L2 prefetch of what the block `pf` positions further on will read from DRAM first -- its
 // own-parity link block (contiguous) and, of the other parity's links, the z and t components at its backward neighbours
 // (variant 8 of the Dslash kernel; used for the fp32 kernels, where it pays).
+// PFL kernels are also compiled for three blocks per SM (168 registers): with fp32 operands the same number of loads needs
+// half the registers, and 12 warps per SM gain 10-13 % per fp32 even/odd CG iteration above one wave of blocks (on a
+// single wave the default build is 4 % faster and stays).
 template <class T, int DAG, int MODE, int PUSH = 0, int ZS = 0, int PFL = 0>
-__global__ void __launch_bounds__(128, 1) hop_cb_kernel(Geom g, int p, const typename Vec2<T>::type* __restrict__ Up,
+__global__ void __launch_bounds__(128, PFL ? 3 : 1) hop_cb_kernel(Geom g, int p, const typename Vec2<T>::type* __restrict__ Up,
                                                         const typename Vec2<T>::type* __restrict__ Uq,
                                                         const typename Vec2<T>::type* __restrict__ in,
                                                         const typename Vec2<T>::type* __restrict__ self,

@@ -500,7 +500,21 @@ template <class T> struct Ops {
         // (variant 0) means for the fp32 kernels on lattices of one wave of blocks up to 16384 chunks: bitwise the same
         // results, 4 - 10 % per fp32 CG iteration (16^4 ... 32^4; the inner solve of the mixed-precision solver), nothing in fp64.
         const bool late_pf = c->variant[LGT_K_DSLASH] == 8 ||
-                             (c->variant[LGT_K_DSLASH] == 0 && sizeof(T) == 4 && grid > 2 * c->num_sms && grid <= 16384 && !c->dd_links_valid);
+                             (c->variant[LGT_K_DSLASH] == 0 && sizeof(T) == 4 && grid > 2 * c->num_sms && !c->dd_links_valid);
+        if constexpr (sizeof(T) == 4) if (late_pf && c->variant[LGT_K_DSLASH] == 0) {  // the fp32 default: also compiled for three blocks per SM
+            const int pf = 3 * c->num_sms;
+            if (mode == 0) {
+                if (dagger)
+                    LAUNCH(c, LGT_K_DSLASH, (dslash_kernel<T, 1, 0, 0, 5, 0, 1>), grid, 128, DSLASH_ARGS, pf);
+                else
+                    LAUNCH(c, LGT_K_DSLASH, (dslash_kernel<T, 0, 0, 0, 5, 0, 1>), grid, 128, DSLASH_ARGS, pf);
+            } else if (mode == 1) {
+                LAUNCH(c, LGT_K_DSLASH, (dslash_kernel<T, 0, 1, 0, 5, 0, 1>), grid, 128, DSLASH_ARGS, pf, fuse_counter(c));
+            } else {
+                LAUNCH(c, LGT_K_DSLASH_R, (dslash_kernel<T, 1, 2, 0, 5, 0, 1>), grid, 128, DSLASH_ARGS, pf, fuse_counter(c));
+            }
+            return LGT_OK;
+        }
         if (late_pf) {
             const int pf = 2 * c->num_sms;
             if (mode == 0) {
@@ -834,7 +848,7 @@ template <class T> struct Ops {
             }
             return LGT_OK;
         }
-        if (sizeof(T) == 4 && c->variant[LGT_K_DSLASH] == 0 && grid > 2 * c->num_sms && grid <= 16384 && !c->dd_links_valid) {
+        if (sizeof(T) == 4 && c->variant[LGT_K_DSLASH] == 0 && grid > 2 * c->num_sms && !c->dd_links_valid) {
             // the fp32 hops with the end-of-block L2 prefetch for the block that takes this block's place (as the fp32 Dslash default)
             const int pf = 2 * c->num_sms;
             if (mode == 0) {
