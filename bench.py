@@ -653,11 +653,11 @@ def run_extras(args, lgt, synth, lat, cfg, hU, hP, hphi, reset_state, md_step, l
     lgt.lgt_set_fermion_action(ctx, lgt.LGT_ACTION_FULL)
     # the decomposed path (lgt_dd_*) on this one GPU: 1 and 4 time slabs in one process, halo exchange by device copies
     U_np, P_np, phi_np = hU.numpy(), hP.numpy(), hphi.numpy()
-    for nr, halo, grid in ((1, "exchange", None), (1, "push", None), (4, "exchange", None), (4, "overlap", None), (4, "exchange", (2, 2))):
+    for nr, halo, grid in ((1, "exchange", None), (1, "push", None), (4, "exchange", None), (4, "overlap", None), (4, "half", None), (4, "exchange", (2, 2))):
         if dims[3] % nr or (dims[0] * dims[1] * dims[2]) % 32 or (grid and (dims[3] % grid[0] or dims[2] % grid[1])):
             continue
         dd = lgt.DecomposedLattice(dims, nr, list(range(nr)), beta, kappa, bc, lgt.LGT_F64, local, stream, grid=grid)
-        lgt.lgt_dd_set_halo_mode(dd.d, {"push": lgt.LGT_DD_PUSH, "overlap": lgt.LGT_DD_OVERLAP}.get(halo, lgt.LGT_DD_EXCHANGE))
+        lgt.lgt_dd_set_halo_mode(dd.d, {"push": lgt.LGT_DD_PUSH, "overlap": lgt.LGT_DD_OVERLAP, "half": lgt.LGT_DD_HALF}.get(halo, lgt.LGT_DD_EXCHANGE))
 
         def dd_reset():
             dd.set_links(U_np)
@@ -1080,7 +1080,7 @@ def main():
                     help="non-default: time the step with the mixed-precision solver (not the headline configuration)")
     ap.add_argument("--action", default="full", choices=["full", "eo"],
                     help="non-default: time the step with the even/odd preconditioned action (not the headline configuration)")
-    ap.add_argument("--halo", default="exchange", choices=["exchange", "push", "overlap"],
+    ap.add_argument("--halo", default="exchange", choices=["exchange", "push", "overlap", "half"],
                     help="decomposed lattice: separate exchange of the halo slices, or halos stored into the neighbours' ghost "
                          "slices by the Dslash kernels (CUDA IPC between processes)")
     ap.add_argument("--transport", default="nccl", choices=["nccl", "host"],

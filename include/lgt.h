@@ -273,7 +273,10 @@ int lgt_dd_halo_plan(int nranks, int rank, int lt_local, int plan[8]);
  *     that touch no ghost slice) is computed; the two boundary slices are launched once the halo has landed (SURVEY.md 8(e):
  *     "interior/boundary kernel split to overlap").  Inside the CG loop, for time slabs of at least three slices that are
  *     whole 128-site chunks; elsewhere it behaves as LGT_DD_EXCHANGE.  Same iterates bit for bit. */
-enum { LGT_DD_EXCHANGE = 0, LGT_DD_PUSH = 1, LGT_DD_OVERLAP = 2 };
+/*   LGT_DD_HALF: the schedule of LGT_DD_OVERLAP with HALF SPINORS on the wire: the boundary sites are projected
+ *     before the send -- and for the backward face also multiplied by U_t^dag -- so that 6 instead of 12 complex numbers per face
+ *     site travel, and the boundary slices take that t hop from the received face.  Same iterates bit for bit. */
+enum { LGT_DD_EXCHANGE = 0, LGT_DD_PUSH = 1, LGT_DD_OVERLAP = 2, LGT_DD_HALF = 3 };
 int lgt_dd_set_halo_mode(lgt_dd* d, int mode);
 int lgt_dd_ipc_export(lgt_dd* d, void* handles128);
 int lgt_dd_ipc_import(lgt_dd* d, const void* lo_handles128, const void* hi_handles128);

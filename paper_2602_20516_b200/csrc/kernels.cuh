@@ -1102,6 +1102,122 @@ __global__ void __launch_bounds__(128, 1) dslash_two_kernel(Geom g, const typena
     }
 }
 
+// ---- half-spinor halos of a time slab (LGT_DD_HALF: "projection before send, multiply by U before send for the
+// backward face").  What a neighbour's t hop needs from a boundary site is not the spinor (12 complex) but a half spinor (6):
+//   its forward hop  (1 + F gamma_t) U_t(x) psi(x+t):        h = P^F psi(x+t), projected HERE; the neighbour multiplies by its own link
+//   its backward hop (1 - F gamma_t) U_t^dag(x-t) psi(x-t):  w = U_t^dag(x-t) P^-F psi(x-t), projected AND multiplied here
+// (F = -1 for D, +1 for D^dag).  halo_pack_kernel forms both faces of a slab in the blocked layout [V3/32][6][32];
+// dslash_halo_kernel is dslash_kernel for one boundary time slice with the t hop that reaches into the ghost slice taken
+// from the received face (HALO 1: the slab's first slice, backward hop from `lo_in`; 2: its last slice, forward hop from
+// `hi_in`; 3: a slab of one slice, both).  The same operations on the same numbers as dslash_kernel: bitwise the same results.
+template <class P> __device__ __forceinline__ P* half_at(P* f, int i) { return f + ((size_t)(i >> 5) * (6 * W) + (i & 31)); }
+
+template <class T, int DAG>
+__global__ void __launch_bounds__(128) halo_pack_kernel(Geom g, const typename Vec2<T>::type* __restrict__ U,
+                                                        const typename Vec2<T>::type* __restrict__ in,
+                                                        typename Vec2<T>::type* __restrict__ lo_out,
+                                                        typename Vec2<T>::type* __restrict__ hi_out, int V3) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= 2 * V3) return;
+    constexpr int F = DAG ? +1 : -1;
+    cx<T> p[12], h[6];
+    if (i < V3) {  // first interior slice -> the lower neighbour's forward hop
+        load_spinor<T>(in, g.s_begin + i, p);
+        spin_project<3, F>(p, h);
+        typename Vec2<T>::type* b = half_at(lo_out, i);
+#pragma unroll
+        for (int k = 0; k < 6; k++) stc<T>(b + k * W, h[k]);
+    } else {       // last interior slice -> the upper neighbour's backward hop
+        const int j = i - V3, s = g.s_end - V3 + j;
+        cx<T> u[9], w[6];
+        load_spinor<T>(in, s, p);
+        load_link<T>(U, 3, s, u);
+        spin_project<3, -F>(p, h);
+        su3_dag_mul_half(u, h, w);
+        typename Vec2<T>::type* b = half_at(hi_out, j);
+#pragma unroll
+        for (int k = 0; k < 6; k++) stc<T>(b + k * W, w[k]);
+    }
+}
+
+template <class T, int DAG, int MODE, int HALO>
+__global__ void __launch_bounds__(128, 1) dslash_halo_kernel(Geom g, const typename Vec2<T>::type* __restrict__ U,
+                                                             const typename Vec2<T>::type* __restrict__ in,
+                                                             typename Vec2<T>::type* __restrict__ out, T kappa, CgState* st,
+                                                             double* partials, typename Vec2<T>::type* __restrict__ r,
+                                                             const typename Vec2<T>::type* __restrict__ lo_in,
+                                                             const typename Vec2<T>::type* __restrict__ hi_in, int lo_first, int hi_first) {
+    const int done = (MODE != 0) ? st->done : 0;
+    const int s = g.s_begin + blockIdx.x * blockDim.x + threadIdx.x;
+    double nrm = 0.0;
+    if (s < g.s_end) {
+        if (MODE == 2) {
+            const typename Vec2<T>::type* br = spinor_at(r, s);
+#pragma unroll
+            for (int k = 0; k < 12; k++) asm volatile("prefetch.global.L2 [%0];" ::"l"(br + k * W));
+        }
+        const Site c = site_coords(g, s);
+        cx<T> acc[12];
+#pragma unroll
+        for (int k = 0; k < 12; k++) acc[k] = mk<T>(0, 0);
+        constexpr int F = DAG ? +1 : -1;
+        hop_fwd<0, F, T>(g, U, in, c, s, acc);
+        if (MODE != 0 && done) return;  // uniform over the grid
+        hop_bwd<0, -F, T>(g, U, in, c, s, acc);
+        hop_fwd<1, F, T>(g, U, in, c, s, acc);
+        hop_bwd<1, -F, T>(g, U, in, c, s, acc);
+        hop_fwd<2, F, T>(g, U, in, c, s, acc);
+        hop_bwd<2, -F, T>(g, U, in, c, s, acc);
+        if (HALO & 2) {  // forward t hop: the projected half spinor came from the upper neighbour
+            cx<T> h[6], u[9], w[6];
+            const typename Vec2<T>::type* b = half_at(hi_in, s - hi_first);
+#pragma unroll
+            for (int k = 0; k < 6; k++) h[k] = ldc<T>(b + k * W);
+            load_link<T>(U, 3, s, u);
+            su3_mul_half(u, h, w);
+            spin_reconstruct_add<3, F>(w, acc);
+        } else {
+            hop_fwd<3, F, T>(g, U, in, c, s, acc);
+        }
+        if (HALO & 1) {  // backward t hop: projected and multiplied by the lower neighbour
+            cx<T> w[6];
+            const typename Vec2<T>::type* b = half_at(lo_in, s - lo_first);
+#pragma unroll
+            for (int k = 0; k < 6; k++) w[k] = ldc<T>(b + k * W);
+            spin_reconstruct_add<3, -F>(w, acc);
+        } else {
+            hop_bwd<3, -F, T>(g, U, in, c, s, acc);
+        }
+        const typename Vec2<T>::type* bi = spinor_at(in, s);
+        if (MODE == 2) {
+            const T alpha = (T)st->alpha;
+            typename Vec2<T>::type* br = spinor_at(r, s);
+#pragma unroll
+            for (int k = 0; k < 12; k++) {
+                cx<T> tv = ldc<T>(bi + k * W);
+                cx<T> q = mk<T>(fma(-kappa, acc[k].re, tv.re), fma(-kappa, acc[k].im, tv.im));
+                cx<T> rv = ldc_rw<T>(br + k * W);
+                rv.re = fma(-alpha, q.re, rv.re);
+                rv.im = fma(-alpha, q.im, rv.im);
+                stc<T>(br + k * W, rv);
+                nrm += (double)rv.re * (double)rv.re + (double)rv.im * (double)rv.im;
+            }
+        } else {
+            typename Vec2<T>::type* bo = spinor_at(out, s);
+#pragma unroll
+            for (int k = 0; k < 12; k++) {
+                cx<T> pv = ldc<T>(bi + k * W);
+                cx<T> o = mk<T>(fma(-kappa, acc[k].re, pv.re), fma(-kappa, acc[k].im, pv.im));
+                stc<T>(bo + k * W, o);
+                if (MODE == 1) nrm += (double)o.re * (double)o.re + (double)o.im * (double)o.im;
+            }
+        }
+    } else if (MODE != 0 && done) {
+        return;
+    }
+    if (MODE != 0) block_partial(nrm, partials);
+}
+
 // Variant 3: 4-D site blocking by block-to-site mapping (the layout is unchanged).  dslash_kernel's block is 128
 // consecutive lexicographic sites (four x rows at 32^4), so of the nine spinors and eight links a site needs only the
 // x and most y neighbours are shared inside the block: L2 -> L1 traffic is 2.06 KB per site for 0.96 KB compulsory.

@@ -85,6 +85,9 @@ struct lgt_dd {
     // LGT_DD_OVERLAP: the exchange runs on its own stream while the slab's bulk is computed (lazy)
     cudaStream_t halo_stream = nullptr;
     cudaEvent_t ev_ready = nullptr, ev_halo = nullptr;
+    // LGT_DD_HALF: per local rank one buffer of four half-spinor faces [lo_out | hi_out | hi_in | lo_in], 6 V3 complex each (lazy)
+    std::vector<void*> half_faces;
+    size_t half_face_bytes = 0;
     void* ipc_peer[2][2] = {{nullptr, nullptr}, {nullptr, nullptr}};
     bool ipc_open[2][2] = {{false, false}, {false, false}};
     std::string err;
@@ -229,6 +232,7 @@ int dd_exchange_grid(lgt_dd* d, void* const* base, int per_site, size_t esize) {
                 DD_CU(cudaStreamSynchronize(d->stream));
                 if (d->d_stage) cudaFree(d->d_stage);
     if (d->halo_stream) cudaStreamDestroy(d->halo_stream);
+    for (void* f : d->half_faces) cudaFree(f);
     if (d->ev_ready) cudaEventDestroy(d->ev_ready);
     if (d->ev_halo) cudaEventDestroy(d->ev_halo);
                 d->d_stage = nullptr;
@@ -314,6 +318,45 @@ int dd_exchange(lgt_dd* d, void* const* base, int per_site, size_t esize = 0) {
         return dd_fail(d, LGT_ECUDA, "dd_exchange: the host transport's send/receive callback failed");
     for (int k = 0; k < 2; k++)
         DD_CU(cudaMemcpyAsync(mine + (size_t)p.recv_slice[k] * slice, h + (2 + k) * slice, slice, cudaMemcpyHostToDevice, d->stream));
+    return LGT_OK;
+}
+
+// The same plan for two arbitrary regions per rank (time slabs): rank r's region send_off[0] goes to rank r - 1 and lands at
+// its recv_off[0], send_off[1] goes to rank r + 1 and lands at its recv_off[1]; `bytes` each.  Used for the half-spinor faces.
+int dd_exchange_regions(lgt_dd* d, void* const* base, const size_t send_off[2], const size_t recv_off[2], size_t bytes) {
+    const int n = (int)d->rk.size();
+    int rc;
+    if ((rc = dd_need_transport(d)) != LGT_OK) return rc;
+    if (!d->comm && !d->host_sendrecv) {
+        for (int i = 0; i < n; i++) {
+            const HaloPlan p = halo_plan(d->nranks, d->rank_of[i], d->Lt_loc);
+            for (int k = 0; k < 2; k++) {
+                const int peer = dd_local_index(d, p.send_peer[k]);
+                if (peer < 0) return dd_fail(d, LGT_ESTATE, "dd_exchange: a neighbour rank is not in this process");
+                DD_CU(cudaMemcpyAsync((char*)base[peer] + recv_off[k], (const char*)base[i] + send_off[k], bytes, cudaMemcpyDeviceToDevice, d->stream));
+            }
+        }
+        return LGT_OK;
+    }
+    const HaloPlan p = halo_plan(d->nranks, d->rank_of[0], d->Lt_loc);
+    char* mine = (char*)base[0];
+    if (d->comm) {
+        DD_NCCL(g_nccl.GroupStart());
+        for (int k = 0; k < 2; k++) DD_NCCL(g_nccl.Send(mine + send_off[k], bytes, NCCL_CHAR, p.send_peer[k], d->comm, d->stream));
+        for (int k = 0; k < 2; k++) DD_NCCL(g_nccl.Recv(mine + recv_off[k], bytes, NCCL_CHAR, p.recv_peer[k], d->comm, d->stream));
+        DD_NCCL(g_nccl.GroupEnd());
+        return LGT_OK;
+    }
+    if ((rc = dd_host_stage(d, 4 * bytes)) != LGT_OK) return rc;
+    char* h = d->h_stage;
+    for (int k = 0; k < 2; k++) DD_CU(cudaMemcpyAsync(h + k * bytes, mine + send_off[k], bytes, cudaMemcpyDeviceToHost, d->stream));
+    DD_CU(cudaStreamSynchronize(d->stream));
+    const void* const sb[2] = {h, h + bytes};
+    void* const rb[2] = {h + 2 * bytes, h + 3 * bytes};
+    if (d->host_sendrecv(d->host_user, sb, p.send_peer, rb, p.recv_peer, bytes) != 0)
+        return dd_fail(d, LGT_ECUDA, "dd_exchange: the host transport's send/receive callback failed");
+    for (int k = 0; k < 2; k++) DD_CU(cudaMemcpyAsync(mine + recv_off[k], h + (2 + k) * bytes, bytes, cudaMemcpyHostToDevice, d->stream));
+    DD_CU(cudaStreamSynchronize(d->stream));  // the staging buffer is reused by the next exchange
     return LGT_OK;
 }
 
@@ -468,6 +511,92 @@ template <class T> struct DdOps {
     // boundary slices follow once the halo has landed.  Block partials land where one launch over the slab would put them:
     // the sums, hence the iterates, are bitwise those of LGT_DD_EXCHANGE.  `launch(c)` issues the kernel for the range
     // currently set in c->g / c->partials.
+    // LGT_DD_HALF: the same schedule with HALF SPINORS on the wire: halo_pack_kernel projects the first slice
+    // and projects and multiplies the last slice of field `k` into two faces of 6 complex per site, the faces travel instead of
+    // the 12-complex slices (half the bytes), and the two boundary slices run dslash_halo_kernel, which takes the t hop that
+    // reaches into the ghost slice from the received face.  Same operations on the same numbers: bitwise the same iterates.
+    // mode 1: t = D p (out = field 3); mode 2: r -= alpha D^dag t (r = field 1).
+    static int half_spinor_dslash(lgt_dd* d, int k, int mode) {
+        int rc;
+        const int n = (int)d->rk.size(), slice = d->V3;
+        const size_t face = (size_t)6 * slice * sizeof(T2);
+        if (!d->halo_stream) {
+            DD_CU(cudaStreamCreateWithFlags(&d->halo_stream, cudaStreamNonBlocking));
+            DD_CU(cudaEventCreateWithFlags(&d->ev_ready, cudaEventDisableTiming));
+            DD_CU(cudaEventCreateWithFlags(&d->ev_halo, cudaEventDisableTiming));
+        }
+        if (d->half_faces.size() != (size_t)n || d->half_face_bytes < face) {
+            DD_CU(cudaStreamSynchronize(d->stream));
+            for (void* f : d->half_faces) cudaFree(f);
+            d->half_faces.assign(n, nullptr);
+            for (int i = 0; i < n; i++) DD_CU(cudaMalloc(&d->half_faces[i], 4 * (size_t)6 * slice * sizeof(double2)));
+            d->half_face_bytes = (size_t)6 * slice * sizeof(double2);
+        }
+        const int dag = mode == 2 ? 1 : 0;
+        // faces of every rank's input field, on the main stream (they read the field the previous kernels completed)
+        for (int i = 0; i < n; i++) {
+            lgt_ctx* c = d->rk[i];
+            T2* H = (T2*)d->half_faces[i];
+            const int pg = (2 * slice + 127) / 128;
+            if (dag) LAUNCH(c, LGT_K_OTHER, (halo_pack_kernel<T, 1>), pg, 128, c->g, (const T2*)fld(c, 7), (const T2*)fld(c, k), H, H + (size_t)6 * slice, slice);
+            else LAUNCH(c, LGT_K_OTHER, (halo_pack_kernel<T, 0>), pg, 128, c->g, (const T2*)fld(c, 7), (const T2*)fld(c, k), H, H + (size_t)6 * slice, slice);
+        }
+        DD_CU(cudaEventRecord(d->ev_ready, d->stream));
+        // bulk of every slab on the main stream ...
+        for (int i = 0; i < n; i++) {
+            lgt_ctx* c = d->rk[i];
+            const int b0 = c->g.s_begin, e0 = c->g.s_end;
+            double* const part0 = c->partials;
+            c->g.s_begin = b0 + slice;
+            c->g.s_end = e0 - slice;
+            c->partials = part0 + slice / 128;
+            rc = mode == 1 ? O::dslash(c, fld(c, 7), fld(c, k), fld(c, 3), 0, 1) : O::dslash(c, fld(c, 7), fld(c, k), nullptr, 1, 2, fld(c, 1));
+            c->g.s_begin = b0;
+            c->g.s_end = e0;
+            c->partials = part0;
+            if (rc != LGT_OK) return dd_fail(d, rc, c->err.c_str());
+        }
+        // ... while the faces travel on the halo stream
+        DD_CU(cudaStreamWaitEvent(d->halo_stream, d->ev_ready, 0));
+        cudaStream_t const main_stream = d->stream;
+        d->stream = d->halo_stream;
+        const size_t send_off[2] = {0, face}, recv_off[2] = {2 * face, 3 * face};
+        rc = dd_exchange_regions(d, d->half_faces.data(), send_off, recv_off, face);
+        d->stream = main_stream;
+        if (rc != LGT_OK) return rc;
+        DD_CU(cudaEventRecord(d->ev_halo, d->halo_stream));
+        DD_CU(cudaStreamWaitEvent(d->stream, d->ev_halo, 0));
+        // the two boundary slices from the received faces
+        for (int i = 0; i < n; i++) {
+            lgt_ctx* c = d->rk[i];
+            const int b0 = c->g.s_begin, e0 = c->g.s_end;
+            double* const part0 = c->partials;
+            const T2* H = (const T2*)d->half_faces[i];
+            const T2 *hi_in = H + (size_t)12 * slice, *lo_in = H + (size_t)18 * slice;
+            const T kap = (T)c->kappa;
+            const int bg = slice / 128;
+            c->g.s_end = b0 + slice;  // first slice: backward t hop from lo_in
+            if (mode == 1)
+                LAUNCH(c, LGT_K_DSLASH, (dslash_halo_kernel<T, 0, 1, 1>), bg, 128, c->g, (const T2*)fld(c, 7), (const T2*)fld(c, k), (T2*)fld(c, 3), kap,
+                       c->st, c->partials, (T2*)nullptr, lo_in, hi_in, b0, e0 - slice);
+            else
+                LAUNCH(c, LGT_K_DSLASH_R, (dslash_halo_kernel<T, 1, 2, 1>), bg, 128, c->g, (const T2*)fld(c, 7), (const T2*)fld(c, k), (T2*)nullptr, kap,
+                       c->st, c->partials, (T2*)fld(c, 1), lo_in, hi_in, b0, e0 - slice);
+            c->g.s_begin = e0 - slice;  // last slice: forward t hop from hi_in
+            c->g.s_end = e0;
+            c->partials = part0 + (e0 - slice - b0) / 128;
+            if (mode == 1)
+                LAUNCH(c, LGT_K_DSLASH, (dslash_halo_kernel<T, 0, 1, 2>), bg, 128, c->g, (const T2*)fld(c, 7), (const T2*)fld(c, k), (T2*)fld(c, 3), kap,
+                       c->st, c->partials, (T2*)nullptr, lo_in, hi_in, b0, e0 - slice);
+            else
+                LAUNCH(c, LGT_K_DSLASH_R, (dslash_halo_kernel<T, 1, 2, 2>), bg, 128, c->g, (const T2*)fld(c, 7), (const T2*)fld(c, k), (T2*)nullptr, kap,
+                       c->st, c->partials, (T2*)fld(c, 1), lo_in, hi_in, b0, e0 - slice);
+            c->g.s_begin = b0;
+            c->g.s_end = e0;
+            c->partials = part0;
+        }
+        return LGT_OK;
+    }
     template <class Launch> static int overlapped(lgt_dd* d, int k, Launch launch) {
         int rc;
         if (!d->halo_stream) {
@@ -625,6 +754,8 @@ template <class T> struct DdOps {
         const bool push = d->halo_mode == LGT_DD_PUSH && d->V3 % 128 == 0 && (d->rk.size() == (size_t)d->nranks || !fp32_on_f64(d->rk[0]));
         // LGT_DD_OVERLAP: time slabs of at least three slices whose slices are whole 128-site chunks; else plain exchange
         const bool overlap = d->halo_mode == LGT_DD_OVERLAP && d->Pz == 0 && d->V3 % 128 == 0 && d->Lt_loc >= 3;
+        // LGT_DD_HALF: the overlapped schedule with half spinors on the wire; the thin links (no smearing) must be the operator's
+        const bool half = d->halo_mode == LGT_DD_HALF && d->Pz == 0 && d->V3 % 128 == 0 && d->Lt_loc >= 3;
         std::vector<Neighbours<T>> push_t(n), push_r(n);
         if (push) {
             // r = p = b on the ghost slices too (one ordinary exchange of b); from here on p's ghosts follow by local
@@ -658,25 +789,29 @@ template <class T> struct DdOps {
             if (chunk > 8) chunk = 8;
             if (chunk <= 0) chunk = 1;
             for (int it = 0; it < chunk; it++) {
-                if (overlap) {
+                if (half) {
+                    if ((rc = half_spinor_dslash(d, 2, 1)) != LGT_OK) return rc;
+                } else if (overlap) {
                     if ((rc = overlapped(d, 2, [&](lgt_ctx* c) { return O::dslash(c, fld(c, 7), fld(c, 2), fld(c, 3), 0, 1); })) != LGT_OK) return rc;
                 } else if (!push && (rc = exchange_spinor(d, 2)) != LGT_OK) return rc;  // p
                 for (int i = 0; i < n; i++) {
                     lgt_ctx* c = d->rk[i];
                     if (push) DD_RK(i, dslash_pushing(d, c, fld(c, 2), fld(c, 3), 0, 1, nullptr, push_t[i]));
-                    else if (!overlap) DD_RK(i, O::dslash(c, fld(c, 7), fld(c, 2), fld(c, 3), 0, 1));  // t = D p, partials of |t|^2
+                    else if (!overlap && !half) DD_RK(i, O::dslash(c, fld(c, 7), fld(c, 2), fld(c, 3), 0, 1));  // t = D p, partials of |t|^2
                     LAUNCH(c, LGT_K_CG_BLAS, cg_partial_sum_kernel, 1, 1024, site_blocks(c, 128), c->partials, c->st);
                 }
                 if ((rc = allreduce_tmp(d)) != LGT_OK) return rc;
                 for (int i = 0; i < n; i++) LAUNCH(d->rk[i], LGT_K_CG_BLAS, (cg_apply_kernel<1>), 1, 1, d->rk[i]->st);
-                if (overlap) {
+                if (half) {
+                    if ((rc = half_spinor_dslash(d, 3, 2)) != LGT_OK) return rc;
+                } else if (overlap) {
                     if ((rc = overlapped(d, 3, [&](lgt_ctx* c) { return O::dslash(c, fld(c, 7), fld(c, 3), nullptr, 1, 2, fld(c, 1)); })) != LGT_OK)
                         return rc;
                 } else if (!push && (rc = exchange_spinor(d, 3)) != LGT_OK) return rc;  // t
                 for (int i = 0; i < n; i++) {
                     lgt_ctx* c = d->rk[i];
                     if (push) DD_RK(i, dslash_pushing(d, c, fld(c, 3), nullptr, 1, 2, fld(c, 1), push_r[i]));
-                    else if (!overlap) DD_RK(i, O::dslash(c, fld(c, 7), fld(c, 3), nullptr, 1, 2, fld(c, 1)));  // r -= alpha D^dag t, partials of |r|^2
+                    else if (!overlap && !half) DD_RK(i, O::dslash(c, fld(c, 7), fld(c, 3), nullptr, 1, 2, fld(c, 1)));  // r -= alpha D^dag t, partials of |r|^2
                     LAUNCH(c, LGT_K_CG_BLAS, cg_partial_sum_kernel, 1, 1024, site_blocks(c, 128), c->partials, c->st);
                 }
                 if ((rc = allreduce_tmp(d)) != LGT_OK) return rc;
@@ -1430,7 +1565,8 @@ int lgt_dd_nccl_init(lgt_dd* d, const void* id128) {
 
 int lgt_dd_set_halo_mode(lgt_dd* d, int mode) {
     CHECK_DD(d);
-    if (mode != LGT_DD_EXCHANGE && mode != LGT_DD_PUSH && mode != LGT_DD_OVERLAP) return dd_fail(d, LGT_EINVAL, "lgt_dd_set_halo_mode: unknown mode");
+    if (mode != LGT_DD_EXCHANGE && mode != LGT_DD_PUSH && mode != LGT_DD_OVERLAP && mode != LGT_DD_HALF)
+        return dd_fail(d, LGT_EINVAL, "lgt_dd_set_halo_mode: unknown mode");
     if (mode == LGT_DD_PUSH && d->Pz > 0) return dd_fail(d, LGT_EINVAL, "lgt_dd_set_halo_mode: LGT_DD_PUSH is for time slabs; a (Pt, Pz) grid exchanges");
     if (mode == LGT_DD_PUSH && d->rk.size() != (size_t)d->nranks && d->nranks > 1)
         for (int f = 0; f < 2; f++)

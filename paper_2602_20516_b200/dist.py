@@ -185,6 +185,8 @@ def decomposed_lattice(dims, beta, kappa, bc, precision=None, local_device=0, st
         lgt.lgt_dd_set_halo_mode(dd.d, lgt.LGT_DD_PUSH)
     elif halo == "overlap":
         lgt.lgt_dd_set_halo_mode(dd.d, lgt.LGT_DD_OVERLAP)
+    elif halo == "half":
+        lgt.lgt_dd_set_halo_mode(dd.d, lgt.LGT_DD_HALF)
     return dd
 
 

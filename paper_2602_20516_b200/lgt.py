@@ -16,7 +16,7 @@ LGT_F64, LGT_F32 = 0, 1
 LGT_SOLVER_CG, LGT_SOLVER_MIXED_CG = 0, 1
 LGT_ACTION_FULL, LGT_ACTION_EO = 0, 1
 LGT_INT_LEAPFROG, LGT_INT_OMELYAN, LGT_INT_SEXTON_WEINGARTEN = 0, 1, 2
-LGT_DD_EXCHANGE, LGT_DD_PUSH, LGT_DD_OVERLAP = 0, 1, 2
+LGT_DD_EXCHANGE, LGT_DD_PUSH, LGT_DD_OVERLAP, LGT_DD_HALF = 0, 1, 2, 3
 
 # every symbol include/lgt.h declares: (restype, argtypes)
 _vp, _i, _d, _l = C.c_void_p, C.c_int, C.c_double, C.c_long

@@ -111,7 +111,7 @@ def main():
     ob = oracle.dslash(odims, kappa, BC, oU, synth.gaussian_spinor(odims, 622), dagger=True)
     _, oit_ref, _, ook = oracle.cg(odims, kappa, BC, oU, ob, 1e-12, 5000)
     ores = {}
-    for halo in ("exchange", "overlap"):
+    for halo in ("exchange", "overlap", "half"):
         dd = dist.decomposed_lattice(odims, beta, kappa, BC, lgt.LGT_F64, 0, None, halo=halo, transport="host")
         dd.set_links(oU)
         xs, it, rel, ok = dd.cg(ob, 1e-12, 5000)
@@ -120,6 +120,7 @@ def main():
         dd.close()
         dist.barrier()
     assert np.array_equal(ores["exchange"], ores["overlap"])
+    assert np.array_equal(ores["exchange"], ores["half"])  # half spinors on the wire
     out["overlap_cg_iters"] = oit_ref
 
     # two split directions over the same transport: the z faces are strided (one run per local time slice) and are staged

@@ -230,7 +230,7 @@ def test_dd_pushed_halos_are_bitwise_the_exchanged_ones(lgt, nranks):
     b = oracle.dslash(dims, kappa, BC, U, synth.gaussian_spinor(dims, 563), dagger=True)
     x_ref, it_ref, _, ok = oracle.cg(dims, kappa, BC, U, b, 1e-12, 5000)
     res = {}
-    for mode in (lgt.LGT_DD_EXCHANGE, lgt.LGT_DD_PUSH, lgt.LGT_DD_OVERLAP):
+    for mode in (lgt.LGT_DD_EXCHANGE, lgt.LGT_DD_PUSH, lgt.LGT_DD_OVERLAP, lgt.LGT_DD_HALF):
         dd = lgt.DecomposedLattice(dims, nranks, list(range(nranks)), beta, kappa, BC)
         lgt.lgt_dd_set_halo_mode(dd.d, mode)
         dd.set_links(U)
@@ -249,6 +249,10 @@ def test_dd_pushed_halos_are_bitwise_the_exchanged_ones(lgt, nranks):
     ov = res[lgt.LGT_DD_OVERLAP]
     assert np.array_equal(ex[0], ov[0]) and np.array_equal(ex[1], ov[1]) and np.array_equal(ex[2], ov[2])
     assert ex[3] == ov[3] and ex[4] == ov[4]
+    # LGT_DD_HALF: the overlapped schedule with projected (and, for the backward face, multiplied) half spinors on the wire
+    ha = res[lgt.LGT_DD_HALF]
+    assert np.array_equal(ex[0], ha[0]) and np.array_equal(ex[1], ha[1]) and np.array_equal(ex[2], ha[2])
+    assert ex[3] == ha[3] and ex[4] == ha[4]
     assert np.linalg.norm(pu[0] - x_ref) < 1e-10 * np.linalg.norm(x_ref)
     U_ref, P_ref, its_ref, _ = oracle.trajectory(dims, beta, kappa, BC, U, b, P0, 2, 0.03, tol=1e-13, max_iter=5000)
     assert pu[4] == its_ref and np.abs(pu[1] - U_ref).max() < 1e-12 and link_rel_err(pu[2], P_ref)[0] < TOL64
@@ -319,6 +323,30 @@ def test_dd_mixed_precision_solver(lgt, nranks, mode):
     with pytest.raises(lgt.LgtError):
         lgt.lgt_dd_set_solver(dd.d, 5, 1e-5)
     dd.close()
+
+
+def test_dd_half_spinor_halos_in_the_fp32_inner_solve(lgt):
+    """LGT_DD_HALF with the mixed-precision solver: the fp32 inner CG sends fp32 half spinors; the kick is bitwise the one with
+    the plain exchange and agrees with the oracle's fp64 kick."""
+    dims, beta, kappa = (8, 4, 4, 8), 5.6, 0.12
+    U0 = synth.warm_links(dims, 0.3, 586)
+    P0 = synth.gaussian_momenta(dims, 587)
+    phi = oracle.dslash(dims, kappa, BC, U0, synth.gaussian_spinor(dims, 588), dagger=True)
+    res = {}
+    for mode in (lgt.LGT_DD_EXCHANGE, lgt.LGT_DD_HALF):
+        dd = lgt.DecomposedLattice(dims, 2, [0, 1], beta, kappa, BC)
+        lgt.lgt_dd_set_halo_mode(dd.d, mode)
+        lgt.lgt_dd_set_solver(dd.d, lgt.LGT_SOLVER_MIXED_CG, 1e-5)
+        dd.set_links(U0)
+        dd.set_momenta(P0)
+        dd.set_pseudofermion(phi)
+        it = lgt.lgt_dd_md_kick(dd.d, 0.05, 1e-12, 5000)
+        res[mode] = (it, cat(dd.get_momenta()))
+        dd.close()
+    assert res[lgt.LGT_DD_EXCHANGE][0] == res[lgt.LGT_DD_HALF][0]
+    assert np.array_equal(res[lgt.LGT_DD_EXCHANGE][1], res[lgt.LGT_DD_HALF][1])
+    P1, _, _ = oracle.kick(dims, beta, kappa, BC, U0, phi, P0, 0.05, 1e-12, 5000)
+    assert link_rel_err(res[lgt.LGT_DD_HALF][1], P1)[0] < 1e-10
 
 
 @pytest.mark.parametrize("nranks", [1, 2, 4])
