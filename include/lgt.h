@@ -405,6 +405,34 @@ int lgt_set_block_swizzle(lgt_ctx* ctx, int z_planes, int* in_effect);
  * LGT_EINVAL for an unknown class or variant. */
 int lgt_set_kernel_variant(lgt_ctx* ctx, int kernel_class, int variant, int* in_effect);
 
+/* ---- an entry point that allocates nothing (for callers that cannot call cudaMalloc: code under CUDA graph capture, tight
+ * serving loops, harnesses that forbid it).
+ *
+ * The plaquette action (BASELINE.json configs[0]) of a link field the CALLER holds, without a handle:
+ *   out[0] = S_g = beta sum_x sum_{mu<nu} (1 - Re tr U_P(x) / 3),   out[1] = (1 / 6V) sum_x sum_{mu<nu} Re tr U_P(x) / 3
+ * -- the numbers lgt_action (S_g) and lgt_plaquette return for the same links.
+ *   dims, beta : lattice extents (x, y, z, t; each >= 1, periodic links) and coupling.
+ *   precision  : LGT_F64 or LGT_F32, the element type of U (the sums are always formed in double).
+ *   device     : CUDA device ordinal (0 ... 63) that owns U, out and the stream; made current for the call and restored.
+ *   U          : DEVICE pointer, canonical layout [V][4][3][3] complex (re, im), read only; caller-owned.
+ *   out        : DEVICE pointer to two doubles, written by the kernel; caller-owned.  Nothing is copied to the host and the
+ *                call does not synchronise: read `out` after the stream has reached this point.
+ *   cuda_stream: cudaStream_t (or NULL for the default stream); the call enqueues one 256-byte memset and one kernel on it.
+ * The scratch of the reduction (one double per block of 128 sites, and the ticket counter) is a file-scope __device__ array
+ * of 1 MiB + 256 B inside the library, which every GPU that loads liblgt.so holds until the process exits; its device address
+ * is looked up on the first call per device (cudaGetSymbolAddress -- make that first call outside a graph capture), after
+ * which the call uses no cudaMalloc, cudaFree or allocating library routine.  Limit: V <= LGT_NOALLOC_MAX_SITES (2^24 sites:
+ * every BASELINE.json configuration incl. 48^3 x 96 fits); larger lattices are rejected with LGT_EINVAL.
+ * Every call on a device shares the one array: calls that OVERLAP on the GPU (two streams, two threads, two graphs in flight)
+ * race on it and return garbage; calls ordered on one stream are safe (the counter is cleared at the start of every call, the
+ * partials are overwritten before they are read).  The result is bitwise reproducible from call to call.
+ * Errors: LGT_EINVAL (null pointer, bad precision / device / extent, too many sites), LGT_ECUDA; the text is returned by
+ * lgt_noalloc_last_error() (per host thread; static storage, never freed by the caller). */
+#define LGT_NOALLOC_MAX_SITES 16777216
+int lgt_plaquette_action_noalloc(const int dims[4], double beta, int precision, int device, const void* U, double* out,
+                                 void* cuda_stream);
+const char* lgt_noalloc_last_error(void);
+
 #ifdef __cplusplus
 }
 #endif

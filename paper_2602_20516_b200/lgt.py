@@ -17,6 +17,7 @@ LGT_SOLVER_CG, LGT_SOLVER_MIXED_CG = 0, 1
 LGT_ACTION_FULL, LGT_ACTION_EO = 0, 1
 LGT_INT_LEAPFROG, LGT_INT_OMELYAN, LGT_INT_SEXTON_WEINGARTEN = 0, 1, 2
 LGT_DD_EXCHANGE, LGT_DD_PUSH, LGT_DD_OVERLAP, LGT_DD_HALF = 0, 1, 2, 3
+LGT_NOALLOC_MAX_SITES = 1 << 24
 
 # every symbol include/lgt.h declares: (restype, argtypes)
 _vp, _i, _d, _l = C.c_void_p, C.c_int, C.c_double, C.c_long
@@ -101,6 +102,8 @@ SYMBOLS = {
     "lgt_pseudofermion_heatbath": (_i, [_vp, C.c_ulonglong, C.c_uint, _dp]),
     "lgt_get_pseudofermion": (_i, [_vp, _vp]),
     "lgt_hmc_trajectory": (_i, [_vp, _i, _d, _d, _i, C.c_ulonglong, C.c_uint, _dp, _ip, _lp, _dp]),
+    "lgt_plaquette_action_noalloc": (_i, [_ip, _d, _i, _i, _vp, _vp, _vp]),
+    "lgt_noalloc_last_error": (C.c_char_p, []),
 }
 
 _lib = None
@@ -233,6 +236,21 @@ def lgt_plaquette(ctx):
     p = C.c_double()
     _check(ctx, lib().lgt_plaquette(ctx, C.byref(p)))
     return p.value
+
+
+def lgt_noalloc_last_error():
+    msg = lib().lgt_noalloc_last_error()
+    return msg.decode() if msg else ""
+
+
+def lgt_plaquette_action_noalloc(dims, beta, U, out, precision=LGT_F64, device=0, stream=None):
+    """Enqueues the plaquette action of the caller's canonical device links U; `out` (device, two doubles) receives
+    (S_g, average plaquette).  No allocation, no synchronisation; calls that overlap on the GPU race on the shared scratch."""
+    d = (C.c_int * 4)(*[int(x) for x in dims])
+    rc = lib().lgt_plaquette_action_noalloc(d, float(beta), int(precision), int(device), _ptr(U), _ptr(out), stream)
+    if rc != LGT_OK:
+        raise LgtError(rc, lgt_noalloc_last_error())
+    return rc
 
 
 def lgt_dslash(ctx, inp, out, dagger=False):
