@@ -400,7 +400,13 @@ int lgt_set_block_swizzle(lgt_ctx* ctx, int z_planes, int* in_effect);
  *     launch: the four hops and the x / p update of an iteration are phases separated by grid barriers, every block forms the two
  *     sums itself from the same block partials in the same order (bitwise the same iterates and count; undivided lattices;
  *     the full-operator CG is not affected).  Measured slower at every size from 8^4 to 32^4 (a graph-launched kernel
- *     boundary costs about 1 us on this GPU, a grid barrier with its L1 invalidation more).
+ *     boundary costs about 1 us on this GPU, a grid barrier with its L1 invalidation more);
+ *     3 = even/odd CG with the scalar updates FOLDED into the kernels that follow them, without fence or ticket: block 0 of the
+ *     third hop forms pAp and alpha, every block of the x / p update forms |r|^2, beta and the stop decision from the same block
+ *     partials in the same fixed order and block 0 writes the next iteration's state into the other of two state records (five
+ *     launches per iteration instead of seven; bitwise the same iterates and count; undivided lattices of at most 2048 blocks
+ *     per half field, otherwise variant 0 runs).  Measured: 8^4 26.2 -> 24.9 us per iteration, but 16^4 fp32 29.9 -> 32.6 and
+ *     24^4 fp32 122.8 -> 126.4: the sum at the head of every block of the update costs more than two 2 us launches in a graph.
  * variant < 0 only queries.  The value in effect is returned through *in_effect (may be NULL).
  * LGT_EINVAL for an unknown class or variant. */
 int lgt_set_kernel_variant(lgt_ctx* ctx, int kernel_class, int variant, int* in_effect);

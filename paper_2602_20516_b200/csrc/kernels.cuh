@@ -1362,6 +1362,53 @@ __global__ void __launch_bounds__(256) cg_update_xp_kernel(size_t n, typename Ve
     }
 }
 
+// cg_update_xp_kernel with the "beta duty" of the folded scalar updates (LGT_K_CG_BLAS variant 3): EVERY block forms
+// |r|^2 from the `nparts` block partials of the kernel before it (cg_fixed_sum: the bits of cg_scalars_kernel<2> whatever
+// the thread count), hence beta and the stop decision, and block 0 writes the state of the NEXT iteration into a second
+// CgState -- `cur` is read-only during the launch, so no block can see a half-updated state; the host alternates the two
+// from iteration to iteration.  A launch past convergence copies the state on unchanged.
+template <class T>
+__global__ void __launch_bounds__(256) cg_update_xp_fold_kernel(size_t n, typename Vec2<T>::type* __restrict__ x,
+                                                                typename Vec2<T>::type* __restrict__ p,
+                                                                const typename Vec2<T>::type* __restrict__ r, const CgState* cur,
+                                                                CgState* next, const double* __restrict__ partials, int nparts) {
+    __shared__ double fold_sums[32];
+    __shared__ double fold_rr;
+    if (cur->done) {
+        if (blockIdx.x == 0 && threadIdx.x == 0) *next = *cur;
+        return;
+    }
+    const double sum = cg_fixed_sum<256>(nparts, partials, fold_sums);
+    if (threadIdx.x == 0) fold_rr = sum;
+    __syncthreads();
+    const double rr_new = fold_rr;
+    const double beta_d = rr_new / cur->rr;
+    const int iter = cur->iter + 1;
+    const bool done = !(rr_new > cur->tol2 * cur->bb) || iter >= cur->max_iter;
+    const T alpha = (T)cur->alpha, beta = (T)beta_d;
+    if (blockIdx.x == 0 && threadIdx.x == 0) {
+        CgState s = *cur;
+        s.beta = beta_d;
+        s.rr = rr_new;
+        s.iter = iter;
+        s.fresh = 1;
+        s.done = done ? 1 : 0;
+        *next = s;
+    }
+    for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+        typename Vec2<T>::type xv = x[i], pv = p[i];
+        xv.x = fma(alpha, pv.x, xv.x);
+        xv.y = fma(alpha, pv.y, xv.y);
+        x[i] = xv;
+        if (!done) {
+            typename Vec2<T>::type rv = __ldg(r + i);
+            pv.x = fma(beta, pv.x, rv.x);
+            pv.y = fma(beta, pv.y, rv.y);
+            p[i] = pv;
+        }
+    }
+}
+
 // Decomposed lattice with pushed halos: the ghost slices of p follow the owner's update p = r + beta p from the ghost
 // copy of r (bitwise the owner's arithmetic), so p never travels.  n complex numbers from each of the two ghost slices.
 template <class T>
@@ -2096,7 +2143,7 @@ __global__ void __launch_bounds__(128, PFL ? 3 : 1) hop_cb_kernel(Geom g, int p,
                                                         const typename Vec2<T>::type* __restrict__ self,
                                                         typename Vec2<T>::type* __restrict__ out, T kap, CgState* st,
                                                         double* partials, typename Vec2<T>::type* __restrict__ r, PushTo<T> push,
-                                                        unsigned* fuse = nullptr, int pf = 0) {
+                                                        unsigned* fuse = nullptr, int pf = 0, int nparts = 0) {
     const int done = (MODE != 0) ? st->done : 0;
     if (MODE == 1 && fuse && done && blockIdx.x == 0 && threadIdx.x == 0) st->fresh = 0;  // as in dslash_kernel
     const int c = g.h_begin + blockIdx.x * blockDim.x + threadIdx.x;
@@ -2182,6 +2229,18 @@ __global__ void __launch_bounds__(128, PFL ? 3 : 1) hop_cb_kernel(Geom g, int p,
     if (MODE == 1 || MODE == 2) {
         block_partial(nrm, partials);
         if (fuse) cg_fused_tail<MODE>(st, partials, fuse);
+    }
+    // MODE 4 = MODE 3 with the "alpha duty" of the folded scalar updates (LGT_K_CG_BLAS variant 3): this launch is the hop
+    // between "u = M p, block partials of |u|^2" and "r -= alpha M^dag u" and reduces nothing itself, so its block 0 forms
+    // pAp from the `nparts` partials of the kernel before it -- cg_fixed_sum: the bits of cg_scalars_kernel<1> -- and alpha
+    // for the kernel after it.  No fence, no ticket: the kernel boundaries order everything.
+    if (MODE == 4 && blockIdx.x == 0) {
+        __shared__ double duty_sums[32];
+        const double sum = cg_fixed_sum<128>(nparts, partials, duty_sums);
+        if (threadIdx.x == 0) {
+            st->pAp = sum;
+            st->alpha = st->rr / sum;
+        }
     }
 }
 

@@ -78,6 +78,8 @@ struct lgt_ctx {
     double* partials = nullptr;
     unsigned* counter = nullptr;
     CgState* st = nullptr;
+    bool fold_default = false;
+    CgState* st2 = nullptr;  // the second state of the folded scalar updates (LGT_K_CG_BLAS variant 3): iterations alternate
     double* scal = nullptr;  // device result slots
     CgState* h_st = nullptr;  // pinned
     double* h_scal = nullptr;  // pinned
@@ -352,6 +354,14 @@ template <class T> struct Ops {
         if (c->dd_links_valid) return false;
         const int v = c->variant[LGT_K_CG_BLAS];
         return v == 2 || (v == 0 && c->coop_default && nchunks <= 4 * c->num_sms);
+    }
+    // Folded scalar updates of the even/odd CG (LGT_K_CG_BLAS variant 3): undivided lattices whose half field is at most
+    // FOLD_MAX_CHUNKS blocks -- every block of the x, p update sums that many partials itself.
+    static constexpr int FOLD_MAX_CHUNKS = 2048;
+    static bool fold_wanted(const lgt_ctx* c, int nchunks) {
+        if (c->dd_links_valid || c->g.z_hi - c->g.z_lo != c->g.L[2] || nchunks > FOLD_MAX_CHUNKS) return false;
+        const int v = c->variant[LGT_K_CG_BLAS];
+        return v == 3 || (v == 0 && c->fold_default);
     }
     // mode 0: out = D in / D^dag in; 1: CG "t = D p" (+ pAp, alpha); 2: CG "q = D^dag t" fused with the x, r update
     static int dslash(lgt_ctx* c, const void* U, const void* in, void* out, int dagger, int mode, void* r = nullptr,
@@ -857,6 +867,8 @@ template <class T> struct Ops {
             } else if (mode == 3) {
                 if (dagger) LAUNCH(c, LGT_K_DSLASH, (hop_cb_kernel<T, 1, 3, 0, 0, 1>), grid, 128, HOP_ARGS, nullptr, pf);
                 else LAUNCH(c, LGT_K_DSLASH, (hop_cb_kernel<T, 0, 3, 0, 0, 1>), grid, 128, HOP_ARGS, nullptr, pf);
+            } else if (mode == 4) {  // mode 3 + the alpha duty of the folded scalar updates (D^dag half only)
+                LAUNCH(c, LGT_K_DSLASH, (hop_cb_kernel<T, 1, 4, 0, 0, 1>), grid, 128, HOP_ARGS, nullptr, pf, grid);
             } else if (mode == 1) {
                 LAUNCH(c, LGT_K_DSLASH, (hop_cb_kernel<T, 0, 1, 0, 0, 1>), grid, 128, HOP_ARGS, fuse_counter(c), pf);
             } else {
@@ -870,6 +882,8 @@ template <class T> struct Ops {
         } else if (mode == 3) {
             if (dagger) LAUNCH(c, LGT_K_DSLASH, (hop_cb_kernel<T, 1, 3>), grid, 128, HOP_ARGS);
             else LAUNCH(c, LGT_K_DSLASH, (hop_cb_kernel<T, 0, 3>), grid, 128, HOP_ARGS);
+        } else if (mode == 4) {
+            LAUNCH(c, LGT_K_DSLASH, (hop_cb_kernel<T, 1, 4>), grid, 128, HOP_ARGS, nullptr, 0, grid);
         } else if (mode == 1) {
             LAUNCH(c, LGT_K_DSLASH, (hop_cb_kernel<T, 0, 1>), grid, 128, HOP_ARGS, fuse_counter(c));
         } else {
@@ -925,6 +939,51 @@ template <class T> struct Ops {
                 if (hc.rr > hc.tol2 * hc.bb) return fail(c, LGT_ENOCONV, "even/odd CG did not reach the tolerance within max_iter");
                 return LGT_OK;
             }
+        }
+        // Small lattices, the scalar updates FOLDED into the kernels that follow them (LGT_K_CG_BLAS variant 3): five launches
+        // per iteration instead of seven, no fence or ticket.  pAp and alpha: block 0 of the third hop (hop mode 4); |r|^2,
+        // beta, count and stop test: every block of the x, p update, from the same partials in the same fixed order, block 0
+        // writing the next iteration's state into the other of two CgState (cg_update_xp_fold_kernel).  Bitwise the iterates
+        // of the loop below.
+        if (fold_wanted(c, ngrid)) {
+            CgState* const S[2] = {c->st, c->st2};
+            int par = 0;
+            for (;;) {
+                CU(cudaMemcpyAsync(c->h_st, S[par], sizeof(CgState), cudaMemcpyDeviceToHost, c->stream));
+                CU(cudaStreamSynchronize(c->stream));
+                if (c->h_st->done) break;
+                int chunk = max_iter - launched;
+                if (chunk > 8) chunk = 8;
+                if (chunk <= 0) chunk = 1;
+                const int par0 = par;
+                auto body = [&]() -> int {
+                    int r2 = LGT_OK, q = par0;
+                    for (int i = 0; i < chunk && r2 == LGT_OK; i++, q ^= 1) {
+                        c->st = S[q];
+                        if ((r2 = hop(c, 1, p, nullptr, t, 0, 3, -c->kappa)) != LGT_OK) break;   // t_o = kappa H_oe p
+                        if ((r2 = hop(c, 0, t, p, u, 0, 1, c->kappa)) != LGT_OK) break;          // u = M p, partials of |u|^2
+                        if ((r2 = hop(c, 1, u, nullptr, t, 1, 4, -c->kappa)) != LGT_OK) break;   // t_o = kappa H^dag_oe u; pAp, alpha
+                        if ((r2 = hop(c, 0, t, u, nullptr, 1, 2, c->kappa, r)) != LGT_OK) break; // r -= alpha M^dag u, partials of |r|^2
+                        r2 = [&]() -> int {
+                            LAUNCH(c, LGT_K_CG_UPDATE, (cg_update_xp_fold_kernel<T>), nb, 256, n, x, p, (const T2*)r, (const CgState*)S[q], S[q ^ 1],
+                                   (const double*)c->partials, ngrid);
+                            return LGT_OK;
+                        }();
+                    }
+                    c->st = S[0];
+                    return r2;
+                };
+                const void* const key[7] = {links_cb(c, 0), x, r, p, u, t, (const void*)(sizeof(T) + 128)};
+                if ((rc = (chunk == 8 && par == 0 ? chunk_graph(c, 1, key, body) : body())) != LGT_OK) return rc;
+                launched += chunk;
+                par ^= (chunk & 1);
+            }
+            if (par) CU(cudaMemcpyAsync(S[0], S[1], sizeof(CgState), cudaMemcpyDeviceToDevice, c->stream));
+            const CgState& h = *c->h_st;
+            if (iters) *iters = h.iter;
+            if (rel) *rel = (h.bb > 0.0) ? sqrt(h.rr / h.bb) : 0.0;
+            if (h.rr > h.tol2 * h.bb) return fail(c, LGT_ENOCONV, "even/odd CG did not reach the tolerance within max_iter");
+            return LGT_OK;
         }
         for (;;) {
             CU(cudaMemcpyAsync(c->h_st, c->st, sizeof(CgState), cudaMemcpyDeviceToHost, c->stream));
@@ -1417,6 +1476,7 @@ int lgt_create(lgt_ctx** out, const int dims[4], double beta, double kappa, cons
     alloc((void**)&c->partials, npart * sizeof(double));
     alloc((void**)&c->counter, sizeof(unsigned));
     alloc((void**)&c->st, sizeof(CgState));
+    alloc((void**)&c->st2, sizeof(CgState));
     alloc((void**)&c->scal, 8 * sizeof(double));
     if (rc == LGT_OK && (cudaMallocHost((void**)&c->h_st, sizeof(CgState)) != cudaSuccess ||
                          cudaMallocHost((void**)&c->h_scal, 8 * sizeof(double)) != cudaSuccess))
@@ -1477,6 +1537,7 @@ int lgt_destroy(lgt_ctx* c) {
     cudaFree(c->counter);
     cudaFree(c->coop_counter);
     cudaFree(c->st);
+    cudaFree(c->st2);
     cudaFree(c->scal);
     if (c->h_st) cudaFreeHost(c->h_st);
     if (c->h_scal) cudaFreeHost(c->h_scal);
@@ -1537,7 +1598,7 @@ int lgt_set_kernel_variant(lgt_ctx* c, int kernel_class, int variant, int* in_ef
     CHECK_CTX(c);
     if (kernel_class < 0 || kernel_class >= LGT_K_COUNT) return fail(c, LGT_EINVAL, "lgt_set_kernel_variant: unknown kernel class");
     if (variant >= 0) {
-        const int nvar = (kernel_class == LGT_K_DSLASH) ? 12 : (kernel_class == LGT_K_GAUGE_FORCE) ? 4 : (kernel_class == LGT_K_CG_BLAS) ? 3 : 1;
+        const int nvar = (kernel_class == LGT_K_DSLASH) ? 12 : (kernel_class == LGT_K_GAUGE_FORCE) ? 4 : (kernel_class == LGT_K_CG_BLAS) ? 4 : 1;
         if (variant >= nvar) return fail(c, LGT_EINVAL, "lgt_set_kernel_variant: this kernel class has no such variant");
         if (c->variant[kernel_class] != variant) {
             // captured CG chunks hold the old kernels

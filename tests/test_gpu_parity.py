@@ -208,7 +208,9 @@ def test_cg_fused_scalar_update_variant(lgt, dims):
     lat.set_links(U)
     even = all(d % 2 == 0 for d in dims)
     runs = []
-    for v in (0, 1, 0, 2):  # 2: the whole even/odd solve as one cooperative launch (the full-operator CG is unaffected)
+    # 2: the whole even/odd solve as one cooperative launch; 3: the scalar updates folded into the kernels that follow them
+    # (both: even/odd CG only, the full-operator CG is unaffected)
+    for v in (0, 1, 0, 2, 3):
         assert lgt.lgt_set_kernel_variant(lat.ctx, lgt.LGT_K_CG_BLAS, v) == v
         n0 = lgt.lgt_launch_count(lat.ctx)
         x, it, rel, ok = lat.cg(b, 1e-10, 3000)
@@ -218,7 +220,7 @@ def test_cg_fused_scalar_update_variant(lgt, dims):
             res += list(lat.eo_cg(b, 1e-10, 3000))
         res += list(lat.cg_mixed(b, 1e-10, 3000))
         runs.append(res)
-    for other in (runs[1], runs[3]):
+    for other in (runs[1], runs[3], runs[4]):
         for a, c in zip(runs[0], other):
             if isinstance(a, np.ndarray):
                 assert np.array_equal(a, c)
