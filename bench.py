@@ -82,7 +82,8 @@ VARIANT_NAMES = {
                "variant 0 + the L2 prefetch of variant 4 issued at the end of each block (the fp32 default)",
                "persistent, DRAM-bound operands (forward links, t+1 spinor) by per-thread cp.async into shared memory one chunk ahead",
                "variant 1 with the chunks drawn from a global counter instead of a fixed stride",
-               "two chunks per block as straight-line code"],
+               "two chunks per block as straight-line code",
+               "12-real links in the fp32 default's build (3 blocks per SM, late prefetch of rows 0, 1); fp64 runs variant 7"],
     "gauge_force": ["one 32-site layout block x 4 directions per 128-thread block (default)",
                     "two layout blocks per 256-thread block",
                     "four layout blocks per 512-thread block (128 registers)",

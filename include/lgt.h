@@ -388,6 +388,10 @@ int lgt_set_block_swizzle(lgt_ctx* ctx, int z_planes, int* in_effect);
  *     7 = 12-real links: rows 0 and 1 of every link are read and row 2 = sign * conj(row0 x row1) is
  *         rebuilt in registers (768 instead of 960 compulsory bytes per site).  Exact for special unitary links; links
  *         that have drifted from unitarity by delta change the operator by O(delta).
+ *     12 = variant 7 in the fp32 default's build (fp32 handles and the fp32 inner solve; fp64 runs variant 7): compiled for
+ *         three blocks per SM, with the end-of-block L2 prefetch restricted to rows 0 and 1.  384 instead of 480 compulsory
+ *         bytes per site, and still slower than the default (32^4: 94-97 against 91 us, CG iteration 303-321 against 274-278 us):
+ *         the fp32 kernel is not bound by bytes either.
  *   LGT_K_GAUGE_FORCE: 0 = one 32-site layout block x 4 directions per 128-thread block (default, fastest);
  *     1 / 2 = two / four layout blocks per 256- / 512-thread block (more sharing through L1; measured slower).  Same sums bit for bit.
  *     3 = one thread per site: the down staples link by link, the up staples plaquette by plaquette (U_mu(s) U_nu(s+mu)

@@ -439,13 +439,22 @@ template <class T> struct PushTo {
 
 // L2 prefetch of what block `b` of the Dslash grid will read from DRAM first: its forward links and its t+1 spinors
 // (one lane per 128-byte line; the warp's link block is 36 x 32 complex, its spinor block 12 x 32, both contiguous).
-template <class T>
+// TWELVE: only rows 0 and 1 of every link (the 12-real kernels never touch row 2).
+template <class T, bool TWELVE = false>
 __device__ __forceinline__ void dslash_prefetch_block(const Geom& g, const typename Vec2<T>::type* U, const typename Vec2<T>::type* in, int b) {
     const int sp = g.s_begin + swizzled_chunk(g, b) * blockDim.x + threadIdx.x;
     if (sp < g.s_end) {
         const int lane = threadIdx.x & 31;
         constexpr int CPL = 128 / (int)sizeof(typename Vec2<T>::type);  // complex numbers per line
         const typename Vec2<T>::type* bu = link_at(U, sp - lane, 0);
+        if (TWELVE) {
+            constexpr int LPD = 9 * W / CPL, NL = 6 * W / CPL;  // lines per direction, and those of rows 0 and 1
+#pragma unroll
+            for (int j = 0; j < (4 * NL + 31) / 32; j++) {
+                const int idx = lane + 32 * j;
+                if (idx < 4 * NL) asm volatile("prefetch.global.L2 [%0];" ::"l"(bu + ((idx / NL) * LPD + idx % NL) * CPL));
+            }
+        } else
 #pragma unroll
         for (int j = 0; j < (36 * W / CPL + 31) / 32; j++)
             if (lane + 32 * j < 36 * W / CPL) asm volatile("prefetch.global.L2 [%0];" ::"l"(bu + (lane + 32 * j) * CPL));
@@ -504,8 +513,8 @@ __global__ void __launch_bounds__(128, LB3 ? 3 : 1) dslash_kernel(Geom g, const 
             hop_bwd<1, -F, T>(g, U, in, c, s, acc);
             hop_bwd<2, -F, T>(g, U, in, c, s, acc);
             hop_bwd<3, -F, T>(g, U, in, c, s, acc);
-        } else if (PFON == 4) {
-            // variant 7: 12-real links, third row rebuilt in registers
+        } else if (PFON == 4 || PFON == 6) {
+            // variant 7: 12-real links, third row rebuilt in registers (PFON 6, variant 12: with the late prefetch of variant 8)
             hop_fwd<0, F, T, 2>(g, U, in, c, s, acc);
             if (MODE != 0 && done) return;  // uniform over the grid
             hop_bwd<0, -F, T, 2>(g, U, in, c, s, acc);
@@ -528,6 +537,7 @@ __global__ void __launch_bounds__(128, LB3 ? 3 : 1) dslash_kernel(Geom g, const 
         }
         // variant 8: the prefetch of variant 4 issued at the END of the block, ~1 us before the block that takes its place starts
         if (PFON == 5 && blockIdx.x + pf < gridDim.x) dslash_prefetch_block<T>(g, U, in, blockIdx.x + pf);
+        if (PFON == 6 && blockIdx.x + pf < gridDim.x) dslash_prefetch_block<T, true>(g, U, in, blockIdx.x + pf);
         const typename Vec2<T>::type* bi = spinor_at(in, s);
         if (MODE == 2) {
             const T alpha = (T)st->alpha;

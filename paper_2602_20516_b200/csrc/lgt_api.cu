@@ -539,7 +539,23 @@ template <class T> struct Ops {
             }
             return LGT_OK;
         }
-        if (c->variant[LGT_K_DSLASH] == 7) {  // 12-real links: rows 0 and 1 read, row 2 rebuilt in registers
+        // Variant 12 (fp32 only; fp64 runs variant 7): 12-real links in the fp32 default's build -- three blocks per SM and the
+        // end-of-block prefetch, of rows 0 and 1 only
+        if constexpr (sizeof(T) == 4) if (c->variant[LGT_K_DSLASH] == 12) {
+            const int pf = 3 * c->num_sms;
+            if (mode == 0) {
+                if (dagger)
+                    LAUNCH(c, LGT_K_DSLASH, (dslash_kernel<T, 1, 0, 0, 6, 0, 1>), grid, 128, DSLASH_ARGS, pf);
+                else
+                    LAUNCH(c, LGT_K_DSLASH, (dslash_kernel<T, 0, 0, 0, 6, 0, 1>), grid, 128, DSLASH_ARGS, pf);
+            } else if (mode == 1) {
+                LAUNCH(c, LGT_K_DSLASH, (dslash_kernel<T, 0, 1, 0, 6, 0, 1>), grid, 128, DSLASH_ARGS, pf, fuse_counter(c));
+            } else {
+                LAUNCH(c, LGT_K_DSLASH_R, (dslash_kernel<T, 1, 2, 0, 6, 0, 1>), grid, 128, DSLASH_ARGS, pf, fuse_counter(c));
+            }
+            return LGT_OK;
+        }
+        if (c->variant[LGT_K_DSLASH] == 7 || c->variant[LGT_K_DSLASH] == 12) {  // 12-real links: rows 0 and 1 read, row 2 rebuilt in registers
             if (mode == 0) {
                 if (dagger)
                     LAUNCH(c, LGT_K_DSLASH, (dslash_kernel<T, 1, 0, 0, 4>), grid, 128, DSLASH_ARGS, 0);
@@ -1598,7 +1614,7 @@ int lgt_set_kernel_variant(lgt_ctx* c, int kernel_class, int variant, int* in_ef
     CHECK_CTX(c);
     if (kernel_class < 0 || kernel_class >= LGT_K_COUNT) return fail(c, LGT_EINVAL, "lgt_set_kernel_variant: unknown kernel class");
     if (variant >= 0) {
-        const int nvar = (kernel_class == LGT_K_DSLASH) ? 12 : (kernel_class == LGT_K_GAUGE_FORCE) ? 4 : (kernel_class == LGT_K_CG_BLAS) ? 4 : 1;
+        const int nvar = (kernel_class == LGT_K_DSLASH) ? 13 : (kernel_class == LGT_K_GAUGE_FORCE) ? 4 : (kernel_class == LGT_K_CG_BLAS) ? 4 : 1;
         if (variant >= nvar) return fail(c, LGT_EINVAL, "lgt_set_kernel_variant: this kernel class has no such variant");
         if (c->variant[kernel_class] != variant) {
             // captured CG chunks hold the old kernels

@@ -103,10 +103,10 @@ def test_dslash_kernel_variants(lgt, dims):
     x0, it0, _, ok0 = lat.cg(psi, 1e-10, 2000)
     _, it_ref, _, ok_ref = oracle.cg(dims, 0.12, BC, U, psi, 1e-10, 2000)
     assert ok0 and ok_ref and it0 == it_ref
-    for v in (1, 2, 3, 4, 5, 6, 7, 8, 9, 10, 11):
+    for v in (1, 2, 3, 4, 5, 6, 7, 8, 9, 10, 11, 12):
         assert lgt.lgt_set_kernel_variant(lat.ctx, lgt.LGT_K_DSLASH, v) == v
         for d in (False, True):
-            if v in (6, 7):  # 6 sums the eight hops in another order, 7 rebuilds the third row of every link
+            if v in (6, 7, 12):  # 6 sums the eight hops in another order, 7 (and 12 = 7 in fp64) rebuilds the third row of every link
                 assert site_rel_err(lat.dslash(psi, dagger=d), base[d]) < 1e-13
             else:
                 assert np.array_equal(lat.dslash(psi, dagger=d), base[d]), (v, d)
@@ -114,10 +114,33 @@ def test_dslash_kernel_variants(lgt, dims):
         assert ok and it == it0, (v, it, it0)
         assert np.abs(x - x0).max() <= 1e-12 * np.abs(x0).max()  # variant 3 sums other block partials
     with pytest.raises(lgt.LgtError):
-        lgt.lgt_set_kernel_variant(lat.ctx, lgt.LGT_K_DSLASH, 12)
+        lgt.lgt_set_kernel_variant(lat.ctx, lgt.LGT_K_DSLASH, 13)
     with pytest.raises(lgt.LgtError):
         lgt.lgt_set_kernel_variant(lat.ctx, 99, 0)
     assert lgt.lgt_set_kernel_variant(lat.ctx, lgt.LGT_K_DSLASH, 0) == 0
+    lat.close()
+
+
+@pytest.mark.parametrize("dims", [(8, 8, 8, 8), (32, 4, 6, 3), (16, 16, 16, 24)])
+def test_dslash_fp32_twelve_real_links_variant(lgt, dims):
+    """Variant 12 of the Dslash kernels (fp32 handles): rows 0 and 1 of every link read, row 2 rebuilt in registers with the
+    folded fermion boundary sign, in the fp32 default's build (three blocks per SM, end-of-block prefetch of the two rows; the
+    last shape is more than two waves of blocks, where the default prefetches too).  D, D^dag against the oracle within
+    the fp32 tolerance and against variant 0 to fp32 rounding; CG with variant 0's count."""
+    U = round32(synth.warm_links(dims, 0.3, 47))
+    psi = round32(synth.gaussian_spinor(dims, 48))
+    lat = lgt.Lattice(dims, 5.6, 0.12, BC, precision=lgt.LGT_F32)
+    lat.set_links(U)
+    base = [lat.dslash(psi, dagger=d).astype(np.complex128) for d in (False, True)]
+    _, it0, _, ok0 = lat.cg(psi, 1e-5, 2000)
+    assert lgt.lgt_set_kernel_variant(lat.ctx, lgt.LGT_K_DSLASH, 12) == 12
+    for d in (False, True):
+        out = lat.dslash(psi, dagger=d).astype(np.complex128)
+        assert site_rel_err(out, base[d]) < 2e-6
+        if synth.volume(dims) <= 4096:
+            assert site_rel_err(out, oracle.dslash(dims, 0.12, BC, U, psi, dagger=d)) < TOL32
+    _, it, _, ok = lat.cg(psi, 1e-5, 2000)
+    assert ok0 and ok and abs(it - it0) <= 1
     lat.close()
 
 
