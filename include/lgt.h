@@ -391,7 +391,11 @@ int lgt_set_block_swizzle(lgt_ctx* ctx, int z_planes, int* in_effect);
  *     12 = variant 7 in the fp32 default's build (fp32 handles and the fp32 inner solve; fp64 runs variant 7): compiled for
  *         three blocks per SM, with the end-of-block L2 prefetch restricted to rows 0 and 1.  384 instead of 480 compulsory
  *         bytes per site, and still slower than the default (32^4: 94-97 against 91 us, CG iteration 303-321 against 274-278 us):
- *         the fp32 kernel is not bound by bytes either.
+ *         the fp32 kernel is not bound by bytes either.  The fp32 even/odd hop kernels ARE (0.95 of the copy bandwidth), and for
+ *         them variant 12 selects the same 12-real links (hop_cb_kernel PFL 2: 32^4 hop 67 -> 59 us).  In the fp32 INNER solve
+ *         of the mixed-precision even/odd solver on lattices of more than two waves of blocks that is the DEFAULT -- the fp64
+ *         defect correction keeps the exact operator, so links that are not special unitary cost iterations, never accuracy
+ *         (even/odd mixed-precision MD step at 32^4 27.9 -> 25.4 ms, same iteration count).
  *   LGT_K_GAUGE_FORCE: 0 = one 32-site layout block x 4 directions per 128-thread block (default, fastest);
  *     1 / 2 = two / four layout blocks per 256- / 512-thread block (more sharing through L1; measured slower).  Same sums bit for bit.
  *     3 = one thread per site: the down staples link by link, the up staples plaquette by plaquette (U_mu(s) U_nu(s+mu)

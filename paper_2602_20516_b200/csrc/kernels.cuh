@@ -2108,25 +2108,27 @@ __device__ __forceinline__ Site cb_coords(const Geom& g, int p, int c, int& s) {
 }
 
 // acc += (1 + SG gamma_MU) U_MU(s) in(s+MU): link of the output site's parity (Up), spinor of the other parity
-template <int MU, int SG, class T, int COH = 0>
+template <int MU, int SG, class T, int COH = 0, int TW = 0>
 __device__ __forceinline__ void hop_fwd_cb(const Geom& g, const typename Vec2<T>::type* Up, const typename Vec2<T>::type* in,
                                            const Site& cs, int s, int c, cx<T> acc[12]) {
     const int cn = nbr_fwd(g, cs, s, MU) >> 1;
     cx<T> p[12], h[6], u[9], w[6];
     load_spinor<T, COH ? 3 : 0>(in, cn, p);
-    load_link<T>(Up, MU, c, u);
+    if (TW) load_link12<T>(Up, MU, c, (T)folded_sign(g, MU, cs.x[MU]), u);  // rows 0 and 1 read, row 2 rebuilt
+    else load_link<T>(Up, MU, c, u);
     spin_project<MU, SG>(p, h);
     su3_mul_half(u, h, w);
     spin_reconstruct_add<MU, SG>(w, acc);
 }
 // acc += (1 + SG gamma_MU) U_MU^dag(s-MU) in(s-MU): link and spinor of the other parity (Uq, in)
-template <int MU, int SG, class T, int COH = 0>
+template <int MU, int SG, class T, int COH = 0, int TW = 0>
 __device__ __forceinline__ void hop_bwd_cb(const Geom& g, const typename Vec2<T>::type* Uq, const typename Vec2<T>::type* in,
                                            const Site& cs, int s, cx<T> acc[12]) {
     const int cn = nbr_bwd(g, cs, s, MU) >> 1;
     cx<T> p[12], h[6], u[9], w[6];
     load_spinor<T, COH ? 3 : 0>(in, cn, p);
-    load_link<T>(Uq, MU, cn, u);
+    if (TW) load_link12<T>(Uq, MU, cn, (T)folded_sign(g, MU, cs.x[MU] == 0 ? g.L[MU] - 1 : cs.x[MU] - 1), u);
+    else load_link<T>(Uq, MU, cn, u);
     spin_project<MU, SG>(p, h);
     su3_dag_mul_half(u, h, w);
     spin_reconstruct_add<MU, SG>(w, acc);
@@ -2171,21 +2173,30 @@ __global__ void __launch_bounds__(128, PFL ? 3 : 1) hop_cb_kernel(Geom g, int p,
 #pragma unroll
         for (int k = 0; k < 12; k++) acc[k] = mk<T>(0, 0);
         constexpr int F = DAG ? +1 : -1;
-        hop_fwd_cb<0, F, T>(g, Up, in, cs, s, c, acc);
+        constexpr int TW = (PFL == 2) ? 1 : 0;  // PFL 2 (variant 12 of LGT_K_DSLASH): 12-real links, 384 instead of 576 link bytes per site
+        hop_fwd_cb<0, F, T, 0, TW>(g, Up, in, cs, s, c, acc);
         if (MODE != 0 && done) return;  // uniform over the grid
-        hop_bwd_cb<0, -F, T>(g, Uq, in, cs, s, acc);
-        hop_fwd_cb<1, F, T>(g, Up, in, cs, s, c, acc);
-        hop_bwd_cb<1, -F, T>(g, Uq, in, cs, s, acc);
-        hop_fwd_cb<2, F, T>(g, Up, in, cs, s, c, acc);
-        hop_bwd_cb<2, -F, T>(g, Uq, in, cs, s, acc);
-        hop_fwd_cb<3, F, T>(g, Up, in, cs, s, c, acc);
-        hop_bwd_cb<3, -F, T>(g, Uq, in, cs, s, acc);
+        hop_bwd_cb<0, -F, T, 0, TW>(g, Uq, in, cs, s, acc);
+        hop_fwd_cb<1, F, T, 0, TW>(g, Up, in, cs, s, c, acc);
+        hop_bwd_cb<1, -F, T, 0, TW>(g, Uq, in, cs, s, acc);
+        hop_fwd_cb<2, F, T, 0, TW>(g, Up, in, cs, s, c, acc);
+        hop_bwd_cb<2, -F, T, 0, TW>(g, Uq, in, cs, s, acc);
+        hop_fwd_cb<3, F, T, 0, TW>(g, Up, in, cs, s, c, acc);
+        hop_bwd_cb<3, -F, T, 0, TW>(g, Uq, in, cs, s, acc);
         if (PFL && blockIdx.x + pf < gridDim.x) {
             const int lane = threadIdx.x & 31;
             const int cp = c - lane + pf * (int)blockDim.x;  // first site of this warp's counterpart in the later block
             if (cp < g.h_end) {
                 constexpr int CPL = 128 / (int)sizeof(typename Vec2<T>::type);
                 const typename Vec2<T>::type* bu = link_at(Up, cp, 0);
+                if (TW) {
+                    constexpr int LPD = 9 * W / CPL, NL = 6 * W / CPL;  // lines per direction, and those of rows 0 and 1
+#pragma unroll
+                    for (int j = 0; j < (4 * NL + 31) / 32; j++) {
+                        const int idx = lane + 32 * j;
+                        if (idx < 4 * NL) asm volatile("prefetch.global.L2 [%0];" ::"l"(bu + ((idx / NL) * LPD + idx % NL) * CPL));
+                    }
+                } else
 #pragma unroll
                 for (int j = 0; j < (36 * W / CPL + 31) / 32; j++)
                     if (lane + 32 * j < 36 * W / CPL) asm volatile("prefetch.global.L2 [%0];" ::"l"(bu + (lane + 32 * j) * CPL));

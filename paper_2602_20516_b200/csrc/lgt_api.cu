@@ -8,6 +8,7 @@
 #include <cstring>
 #include <new>
 #include <string>
+#include <type_traits>
 #include <vector>
 
 #include "../../include/lgt.h"
@@ -874,23 +875,36 @@ template <class T> struct Ops {
             }
             return LGT_OK;
         }
-        if (sizeof(T) == 4 && c->variant[LGT_K_DSLASH] == 0 && grid > 2 * c->num_sms && !c->dd_links_valid) {
-            // the fp32 hops with the end-of-block L2 prefetch for the block that takes this block's place (as the fp32 Dslash default)
+        if (sizeof(T) == 4 && (c->variant[LGT_K_DSLASH] == 0 || c->variant[LGT_K_DSLASH] == 12) && grid > 2 * c->num_sms && !c->dd_links_valid) {
+            // the fp32 hops with the end-of-block L2 prefetch for the block that takes this block's place (as the fp32 Dslash default);
+            // PFL 2: the same build with 12-real links -- rows 0 and 1 of every link read, row 2 rebuilt in registers.  These
+            // kernels ARE bound by bytes (0.95 of the copy bandwidth), so the 192 B per site less pay: 32^4 hop 67 -> 59 us, the
+            // even/odd mixed-precision MD step 27.9 -> 25.4 ms at the same iteration count.  It is the default where it cannot
+            // change an answer: in the fp32 INNER solve of the mixed-precision solver, whose result the fp64 defect correction
+            // checks against the exact operator (links that are not special unitary would cost iterations, not accuracy).  A
+            // plain fp32 handle keeps the exact 9-entry links unless variant 12 of LGT_K_DSLASH is selected.
+            const bool twelve = c->variant[LGT_K_DSLASH] == 12 || fp32_on_f64(c);
             const int pf = 2 * c->num_sms;
-            if (mode == 0) {
-                if (dagger) LAUNCH(c, LGT_K_DSLASH, (hop_cb_kernel<T, 1, 0, 0, 0, 1>), grid, 128, HOP_ARGS, nullptr, pf);
-                else LAUNCH(c, LGT_K_DSLASH, (hop_cb_kernel<T, 0, 0, 0, 0, 1>), grid, 128, HOP_ARGS, nullptr, pf);
-            } else if (mode == 3) {
-                if (dagger) LAUNCH(c, LGT_K_DSLASH, (hop_cb_kernel<T, 1, 3, 0, 0, 1>), grid, 128, HOP_ARGS, nullptr, pf);
-                else LAUNCH(c, LGT_K_DSLASH, (hop_cb_kernel<T, 0, 3, 0, 0, 1>), grid, 128, HOP_ARGS, nullptr, pf);
-            } else if (mode == 4) {  // mode 3 + the alpha duty of the folded scalar updates (D^dag half only)
-                LAUNCH(c, LGT_K_DSLASH, (hop_cb_kernel<T, 1, 4, 0, 0, 1>), grid, 128, HOP_ARGS, nullptr, pf, grid);
-            } else if (mode == 1) {
-                LAUNCH(c, LGT_K_DSLASH, (hop_cb_kernel<T, 0, 1, 0, 0, 1>), grid, 128, HOP_ARGS, fuse_counter(c), pf);
-            } else {
-                LAUNCH(c, LGT_K_DSLASH_R, (hop_cb_kernel<T, 1, 2, 0, 0, 1>), grid, 128, HOP_ARGS, fuse_counter(c), pf);
+            auto launch_pfl = [&](auto tag) -> int {
+                constexpr int PF = decltype(tag)::value;
+                if (mode == 0) {
+                    if (dagger) LAUNCH(c, LGT_K_DSLASH, (hop_cb_kernel<T, 1, 0, 0, 0, PF>), grid, 128, HOP_ARGS, nullptr, pf);
+                    else LAUNCH(c, LGT_K_DSLASH, (hop_cb_kernel<T, 0, 0, 0, 0, PF>), grid, 128, HOP_ARGS, nullptr, pf);
+                } else if (mode == 3) {
+                    if (dagger) LAUNCH(c, LGT_K_DSLASH, (hop_cb_kernel<T, 1, 3, 0, 0, PF>), grid, 128, HOP_ARGS, nullptr, pf);
+                    else LAUNCH(c, LGT_K_DSLASH, (hop_cb_kernel<T, 0, 3, 0, 0, PF>), grid, 128, HOP_ARGS, nullptr, pf);
+                } else if (mode == 4) {  // mode 3 + the alpha duty of the folded scalar updates (D^dag half only)
+                    LAUNCH(c, LGT_K_DSLASH, (hop_cb_kernel<T, 1, 4, 0, 0, PF>), grid, 128, HOP_ARGS, nullptr, pf, grid);
+                } else if (mode == 1) {
+                    LAUNCH(c, LGT_K_DSLASH, (hop_cb_kernel<T, 0, 1, 0, 0, PF>), grid, 128, HOP_ARGS, fuse_counter(c), pf);
+                } else {
+                    LAUNCH(c, LGT_K_DSLASH_R, (hop_cb_kernel<T, 1, 2, 0, 0, PF>), grid, 128, HOP_ARGS, fuse_counter(c), pf);
+                }
+                return LGT_OK;
+            };
+            if constexpr (sizeof(T) == 4) {
+                return twelve ? launch_pfl(std::integral_constant<int, 2>()) : launch_pfl(std::integral_constant<int, 1>());
             }
-            return LGT_OK;
         }
         if (mode == 0) {
             if (dagger) LAUNCH(c, LGT_K_DSLASH, (hop_cb_kernel<T, 1, 0>), grid, 128, HOP_ARGS);

@@ -498,6 +498,43 @@ def test_eo_mixed_precision_solver(lgt):
     lat.close()
 
 
+@pytest.mark.parametrize("bc", [BC, (-1, -1, -1, -1)])
+def test_eo_mixed_solver_inner_hops_on_twelve_real_links(lgt, bc):
+    """On lattices of more than two waves of blocks the fp32 INNER solve of the even/odd mixed-precision solver reads rows 0 and 1
+    of every link and rebuilds row 2 with the folded fermion boundary sign (hop_cb_kernel PFL 2; the fp64 defect correction
+    keeps the exact operator).  320 blocks per half field here: force against the oracle's fp64 even/odd solve, and the same
+    iteration count (+- 2) and force as with the exact-link inner hops (any other Dslash variant selects them).  A plain fp32
+    handle keeps the exact links unless variant 12 is selected; with it the solve agrees to fp32 rounding."""
+    dims, kappa, tol = (16, 16, 16, 20), 0.12, 1e-12
+    V = synth.volume(dims)
+    U = synth.warm_links(dims, 0.3, 147)
+    phi = oeo.mhat(dims, kappa, bc, U, oeo.keep(synth.gaussian_spinor(dims, 148), dims, 0), dagger=True)
+    F_ref, it_ref, _ = oeo.fermion_force(dims, kappa, bc, U, phi, tol, 10 * V)
+    lat = lgt.Lattice(dims, 5.5, kappa, bc)
+    lat.set_links(U)
+    lat.set_pseudofermion(phi)
+    lgt.lgt_set_fermion_action(lat.ctx, lgt.LGT_ACTION_EO)
+    lgt.lgt_set_solver(lat.ctx, lgt.LGT_SOLVER_MIXED_CG, 1e-5)
+    F, it = lat.fermion_force(None, None, tol=tol, max_iter=10 * V)
+    assert 0 < it < 2 * it_ref + 20
+    assert link_rel_err(F, F_ref)[0] < 1e-10
+    assert lgt.lgt_set_kernel_variant(lat.ctx, lgt.LGT_K_DSLASH, 8) == 8  # exact 9-entry links in the inner hops
+    F9, it9 = lat.fermion_force(None, None, tol=tol, max_iter=10 * V)
+    assert abs(it - it9) <= 2 and link_rel_err(F9, F_ref)[0] < 1e-10
+    lat.close()
+    # fp32 handle: variant 12 against the default's exact links
+    b = round32(synth.gaussian_spinor(dims, 149))
+    l32 = lgt.Lattice(dims, 5.5, kappa, bc, precision=lgt.LGT_F32)
+    l32.set_links(round32(U))
+    x0, it0, _, ok0 = l32.eo_cg(b, 1e-5, 3000)
+    assert lgt.lgt_set_kernel_variant(l32.ctx, lgt.LGT_K_DSLASH, 12) == 12
+    x12, it12, _, ok12 = l32.eo_cg(b, 1e-5, 3000)
+    assert ok0 and ok12 and abs(it0 - it12) <= 1
+    even = np.abs(x0).reshape(V, -1).max(axis=1) > 0
+    assert np.linalg.norm((x12 - x0)[even]) < 1e-4 * np.linalg.norm(x0[even])
+    l32.close()
+
+
 def test_eo_leapfrog_conserves_energy(lgt):
     """Leapfrog with the even/odd action on 8^4: |dH| ~ dt^2 and exact reversibility (pin P7 on this action)."""
     dims, beta, kappa = (8, 8, 8, 8), 5.6, 0.12
