@@ -654,11 +654,15 @@ def run_extras(args, lgt, synth, lat, cfg, hU, hP, hphi, reset_state, md_step, l
     lgt.lgt_set_fermion_action(ctx, lgt.LGT_ACTION_FULL)
     # the decomposed path (lgt_dd_*) on this one GPU: 1 and 4 time slabs in one process, halo exchange by device copies
     U_np, P_np, phi_np = hU.numpy(), hP.numpy(), hphi.numpy()
-    for nr, halo, grid in ((1, "exchange", None), (1, "push", None), (4, "exchange", None), (4, "overlap", None), (4, "half", None), (4, "exchange", (2, 2))):
+    for nr, halo, grid, fast in ((1, "exchange", None, False), (1, "push", None, False), (4, "exchange", None, False), (4, "overlap", None, False),
+                                 (4, "half", None, False), (4, "exchange", (2, 2), False), (4, "exchange", None, True)):
         if dims[3] % nr or (dims[0] * dims[1] * dims[2]) % 32 or (grid and (dims[3] % grid[0] or dims[2] % grid[1])):
             continue
         dd = lgt.DecomposedLattice(dims, nr, list(range(nr)), beta, kappa, bc, lgt.LGT_F64, local, stream, grid=grid)
         lgt.lgt_dd_set_halo_mode(dd.d, {"push": lgt.LGT_DD_PUSH, "overlap": lgt.LGT_DD_OVERLAP, "half": lgt.LGT_DD_HALF}.get(halo, lgt.LGT_DD_EXCHANGE))
+        if fast:  # the fastest configuration of the step, on slabs
+            lgt.lgt_dd_set_fermion_action(dd.d, lgt.LGT_ACTION_EO)
+            lgt.lgt_dd_set_solver(dd.d, lgt.LGT_SOLVER_MIXED_CG, 1e-5)
 
         def dd_reset():
             dd.set_links(U_np)
@@ -679,7 +683,7 @@ def run_extras(args, lgt, synth, lat, cfg, hU, hP, hphi, reset_state, md_step, l
         b.record()
         torch.cuda.synchronize()
         shape = ("%dx%d_grid" % grid) if grid else "%d_slabs" % nr
-        extras["decomposed_%s_%s_one_gpu" % (shape, halo)] = {
+        extras["decomposed_%s_%s%s_one_gpu" % (shape, halo, "_even_odd_mixed" if fast else "")] = {
             "ms_per_step": round(a.elapsed_time(b) / 2, 3), "cg_iters_per_step": dd_iters,
             "note": "same MD step through lgt_dd_* with %s resident on this GPU, halo mode %s: the cost of the "
                     "ghost slices, halo traffic and split reductions, not a multi-GPU number" %

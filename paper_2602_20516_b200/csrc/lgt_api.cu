@@ -511,7 +511,7 @@ template <class T> struct Ops {
         // (variant 0) means for the fp32 kernels on lattices of one wave of blocks up to 16384 chunks: bitwise the same
         // results, 4 - 10 % per fp32 CG iteration (16^4 ... 32^4; the inner solve of the mixed-precision solver), nothing in fp64.
         const bool late_pf = c->variant[LGT_K_DSLASH] == 8 ||
-                             (c->variant[LGT_K_DSLASH] == 0 && sizeof(T) == 4 && grid > 2 * c->num_sms && !c->dd_links_valid);
+                             (c->variant[LGT_K_DSLASH] == 0 && sizeof(T) == 4 && grid > 2 * c->num_sms);
         if constexpr (sizeof(T) == 4) if (late_pf && c->variant[LGT_K_DSLASH] == 0) {  // the fp32 default: also compiled for three blocks per SM
             const int pf = 3 * c->num_sms;
             if (mode == 0) {
@@ -875,7 +875,8 @@ template <class T> struct Ops {
             }
             return LGT_OK;
         }
-        if (sizeof(T) == 4 && (c->variant[LGT_K_DSLASH] == 0 || c->variant[LGT_K_DSLASH] == 12) && grid > 2 * c->num_sms && !c->dd_links_valid) {
+        // (time slabs of a decomposed lattice take it too: the prefetch never leaves [h_begin, h_end), the folded sign knows the slab's offset)
+        if (sizeof(T) == 4 && (c->variant[LGT_K_DSLASH] == 0 || c->variant[LGT_K_DSLASH] == 12) && grid > 2 * c->num_sms) {
             // the fp32 hops with the end-of-block L2 prefetch for the block that takes this block's place (as the fp32 Dslash default);
             // PFL 2: the same build with 12-real links -- rows 0 and 1 of every link read, row 2 rebuilt in registers.  These
             // kernels ARE bound by bytes (0.95 of the copy bandwidth), so the 192 B per site less pay: 32^4 hop 67 -> 59 us, the
