@@ -949,6 +949,63 @@ template <class T> struct DdOps {
     static int hop_all(lgt_dd* d, bool to_even, HalfSel in, HalfSel self, HalfSel out, int dagger, int mode, bool plus_kappa, HalfSel r = nullptr,
                        const std::vector<Neighbours<T>>* push = nullptr, bool input_current = false) {
         int rc;
+        // LGT_DD_OVERLAP (and LGT_DD_HALF, which has no half-field form): the exchange of the input half field on the halo
+        // stream under the bulk of the slab, the two boundary slices after it -- DdOps::overlapped for the half-field range.
+        // Block partials land where a single launch would put them: in fp64 bitwise the iterates of LGT_DD_EXCHANGE.
+        const int hslice = d->V3 / 2;
+        if (!input_current && !push && (d->halo_mode == LGT_DD_OVERLAP || d->halo_mode == LGT_DD_HALF) && d->Pz == 0 && hslice % 128 == 0 &&
+            d->Lt_loc >= 3) {
+            if (!d->halo_stream) {
+                DD_CU(cudaStreamCreateWithFlags(&d->halo_stream, cudaStreamNonBlocking));
+                DD_CU(cudaEventCreateWithFlags(&d->ev_ready, cudaEventDisableTiming));
+                DD_CU(cudaEventCreateWithFlags(&d->ev_halo, cudaEventDisableTiming));
+            }
+            auto launch = [&](lgt_ctx* c) {
+                const int p = to_even ? pe_of(c) : 1 - pe_of(c);
+                const double kap = plus_kappa ? c->kappa : -c->kappa;
+                return O::hop(c, p, in(c), self ? self(c) : nullptr, out ? out(c) : nullptr, dagger, mode, kap, r ? r(c) : nullptr);
+            };
+            DD_CU(cudaEventRecord(d->ev_ready, d->stream));  // the input field is complete
+            for (size_t i = 0; i < d->rk.size(); i++) {      // bulk: the slices that touch no ghost slice
+                lgt_ctx* c = d->rk[i];
+                const int b0 = c->g.h_begin, e0 = c->g.h_end;
+                double* const part0 = c->partials;
+                c->g.h_begin = b0 + hslice;
+                c->g.h_end = e0 - hslice;
+                c->partials = part0 + hslice / 128;
+                rc = launch(c);
+                c->g.h_begin = b0;
+                c->g.h_end = e0;
+                c->partials = part0;
+                if (rc != LGT_OK) return dd_fail(d, rc, c->err.c_str());
+            }
+            DD_CU(cudaStreamWaitEvent(d->halo_stream, d->ev_ready, 0));
+            cudaStream_t const main_stream = d->stream;
+            d->stream = d->halo_stream;
+            rc = exchange_half(d, in);
+            d->stream = main_stream;
+            if (rc != LGT_OK) return rc;
+            DD_CU(cudaEventRecord(d->ev_halo, d->halo_stream));
+            DD_CU(cudaStreamWaitEvent(d->stream, d->ev_halo, 0));
+            for (size_t i = 0; i < d->rk.size(); i++) {  // the two boundary slices
+                lgt_ctx* c = d->rk[i];
+                const int b0 = c->g.h_begin, e0 = c->g.h_end;
+                double* const part0 = c->partials;
+                c->g.h_end = b0 + hslice;
+                rc = launch(c);
+                if (rc == LGT_OK) {
+                    c->g.h_begin = e0 - hslice;
+                    c->g.h_end = e0;
+                    c->partials = part0 + (e0 - hslice - b0) / 128;
+                    rc = launch(c);
+                }
+                c->g.h_begin = b0;
+                c->g.h_end = e0;
+                c->partials = part0;
+                if (rc != LGT_OK) return dd_fail(d, rc, c->err.c_str());
+            }
+            return LGT_OK;
+        }
         if (!input_current && (rc = exchange_half(d, in)) != LGT_OK) return rc;
         for (size_t i = 0; i < d->rk.size(); i++) {
             lgt_ctx* c = d->rk[i];

@@ -121,6 +121,28 @@ def main():
         dist.barrier()
     assert np.array_equal(ores["exchange"], ores["overlap"])
     assert np.array_equal(ores["exchange"], ores["half"])  # half spinors on the wire
+    # the even/odd action between processes with the overlapped exchange of the half fields (time slices of 256 sites)
+    from oracle import evenodd as oeo2
+
+    edims = (8, 8, 4, 4 * world)
+    eV = synth.volume(edims)
+    eU = synth.warm_links(edims, 0.3, 631)
+    eP = synth.gaussian_momenta(edims, 632)
+    ephi = oeo2.mhat(edims, kappa, BC, eU, oeo2.keep(synth.gaussian_spinor(edims, 633), edims, 0), dagger=True)
+    _, eit_ref, _ = oeo2.fermion_force(edims, kappa, BC, eU, ephi, 1e-12, 10 * eV)
+    eres = {}
+    for halo in ("exchange", "overlap"):
+        dd = dist.decomposed_lattice(edims, beta, kappa, BC, lgt.LGT_F64, 0, None, halo=halo, transport="host")
+        lgt.lgt_dd_set_fermion_action(dd.d, lgt.LGT_ACTION_EO)
+        dd.set_links(eU)
+        dd.set_momenta(eP)
+        dd.set_pseudofermion(ephi)
+        assert lgt.lgt_dd_md_kick(dd.d, 0.05, 1e-12, 10 * eV) == eit_ref
+        eres[halo] = dd.get_momenta()[0]
+        dd.close()
+        dist.barrier()
+    assert np.array_equal(eres["exchange"], eres["overlap"])
+    out["eo_overlap_cg_iters"] = eit_ref
     out["overlap_cg_iters"] = oit_ref
 
     # two split directions over the same transport: the z faces are strided (one run per local time slice) and are staged

@@ -349,6 +349,42 @@ def test_dd_half_spinor_halos_in_the_fp32_inner_solve(lgt):
     assert link_rel_err(res[lgt.LGT_DD_HALF][1], P1)[0] < 1e-10
 
 
+@pytest.mark.parametrize("nranks", [1, 2])
+def test_dd_even_odd_overlapped_exchange(lgt, nranks):
+    """LGT_DD_OVERLAP (and LGT_DD_HALF, which falls back to it for half fields) with the even/odd action: every hop of the
+    CG on the Schur complement runs its bulk while the input half field's ghost slices travel on the halo stream, the two
+    boundary slices after.  Time slices of 256 sites (128 per parity) and slabs of 4 and 8 slices: momenta after a kick bitwise
+    those of LGT_DD_EXCHANGE, the oracle's iteration count; with the mixed-precision solver the same momenta to 1e-10."""
+    from oracle import evenodd as oeo
+
+    dims, beta, kappa, tol = (8, 8, 4, 8), 5.6, 0.12, 1e-12
+    V = synth.volume(dims)
+    U0 = synth.warm_links(dims, 0.3, 595)
+    P0 = synth.gaussian_momenta(dims, 596)
+    phi = oeo.mhat(dims, kappa, BC, U0, oeo.keep(synth.gaussian_spinor(dims, 597), dims, 0), dagger=True)
+    F_ref, it_ref, _ = oeo.fermion_force(dims, kappa, BC, U0, phi, tol, 10 * V)
+    P_ref = P0 - 0.05 * (oracle.gauge_force(dims, beta, U0) + F_ref)
+    res = {}
+    for mode in (lgt.LGT_DD_EXCHANGE, lgt.LGT_DD_OVERLAP, lgt.LGT_DD_HALF):
+        for mixed in (False, True):
+            dd = lgt.DecomposedLattice(dims, nranks, list(range(nranks)), beta, kappa, BC)
+            lgt.lgt_dd_set_halo_mode(dd.d, mode)
+            lgt.lgt_dd_set_fermion_action(dd.d, lgt.LGT_ACTION_EO)
+            if mixed:
+                lgt.lgt_dd_set_solver(dd.d, lgt.LGT_SOLVER_MIXED_CG, 1e-5)
+            dd.set_links(U0)
+            dd.set_momenta(P0)
+            dd.set_pseudofermion(phi)
+            it = lgt.lgt_dd_md_kick(dd.d, 0.05, tol, 10 * V)
+            res[mode, mixed] = (it, cat(dd.get_momenta()))
+            dd.close()
+    ex = res[lgt.LGT_DD_EXCHANGE, False]
+    assert ex[0] == it_ref and link_rel_err(ex[1], P_ref)[0] < TOL64
+    for mode in (lgt.LGT_DD_OVERLAP, lgt.LGT_DD_HALF):
+        assert res[mode, False][0] == it_ref and np.array_equal(res[mode, False][1], ex[1])
+        assert link_rel_err(res[mode, True][1], P_ref)[0] < 1e-10
+
+
 @pytest.mark.parametrize("nranks", [1, 2, 4])
 def test_dd_even_odd_action(lgt, nranks):
     """The even/odd action on slabs (local parity = global parity shifted by the slab's time offset): iteration count,
