@@ -80,6 +80,7 @@ struct lgt_ctx {
     unsigned* counter = nullptr;
     CgState* st = nullptr;
     bool fold_default = false;
+    bool inner_exact = false;  // the fp32 inner hops of the mixed even/odd solver stopped contracting on 12-real links: exact links until the links change
     CgState* st2 = nullptr;  // the second state of the folded scalar updates (LGT_K_CG_BLAS variant 3): iterations alternate
     double* scal = nullptr;  // device result slots
     CgState* h_st = nullptr;  // pinned
@@ -236,6 +237,7 @@ inline void invalidate_link_copies(lgt_ctx* c) {
     if (c->dd_links_valid) *c->dd_links_valid = false;
     c->ucb_valid = false;
     c->ucb32_valid = false;
+    c->inner_exact = false;
 }
 
 int eo_cg_mixed(lgt_ctx* c, void* b, void* x, void* r, void* q, void* u, void* t_o, double tol, int max_iter, int* iters);
@@ -330,6 +332,7 @@ template <class T> struct Ops {
     if (c->dd_links_valid) *c->dd_links_valid = false;
         c->ucb_valid = false;
     c->ucb32_valid = false;
+    c->inner_exact = false;
         LAUNCH(c, LGT_K_OTHER, (unit_links_kernel<T>), stream_blocks(c, (size_t)36 * c->g.Vs), 256, c->g, (T2*)c->U);
         return LGT_OK;
     }
@@ -763,6 +766,7 @@ template <class T> struct Ops {
     if (c->dd_links_valid) *c->dd_links_valid = false;
         c->ucb_valid = false;
     c->ucb32_valid = false;
+    c->inner_exact = false;
         p_ready(c);
         LAUNCH(c, LGT_K_LINK_UPDATE, (link_update_kernel<T>), grid, 128, c->g, (const T2*)c->U, (T2*)c->U, (const T2*)c->P, (T)eps);
         return LGT_OK;
@@ -821,6 +825,7 @@ template <class T> struct Ops {
             CU(cudaMalloc(&c->Ucb, (size_t)2 * 36 * c->g.Vhs * sizeof(T2)));
             c->ucb_valid = false;
     c->ucb32_valid = false;
+    c->inner_exact = false;
         }
         if (!c->eo) {
             CU(cudaMalloc(&c->eo, (size_t)8 * 12 * c->g.Vhs * sizeof(T2)));
@@ -884,7 +889,7 @@ template <class T> struct Ops {
             // change an answer: in the fp32 INNER solve of the mixed-precision solver, whose result the fp64 defect correction
             // checks against the exact operator (links that are not special unitary would cost iterations, not accuracy).  A
             // plain fp32 handle keeps the exact 9-entry links unless variant 12 of LGT_K_DSLASH is selected.
-            const bool twelve = c->variant[LGT_K_DSLASH] == 12 || fp32_on_f64(c);
+            const bool twelve = c->variant[LGT_K_DSLASH] == 12 || (fp32_on_f64(c) && !c->inner_exact);
             const int pf = 2 * c->num_sms;
             auto launch_pfl = [&](auto tag) -> int {
                 constexpr int PF = decltype(tag)::value;
@@ -1091,6 +1096,19 @@ int read_scalars(lgt_ctx* c, int n) {
 // Mixed-precision solve of (M^dag M) x_e = b_e on an fp64 handle: the defect correction of cg_mixed() with the even/odd
 // operator -- fp32 CG on the Schur complement (fp32 checkerboard links and half fields) inside, true fp64 residual
 // r = b - M^dag M x outside, stop on |r| <= tol |b|.  b, x, r, q, u: fp64 even half fields; t_o: an odd scratch field.
+//
+// Safety net of the 12-real inner hops (hop(): PFL 2): a correction cycle that was asked for a reduction of the residual by
+// eps and delivered less than a factor 100 -- and less than a tenth of what was asked -- means that the inner operator is not
+// the outer one to fp32 accuracy, i.e. the links are not special unitary.  The inner hops then read the exact 9-entry links
+// from here on (the flag holds until the links change; captured CG chunks are dropped, they hold the 12-real kernels).
+// rr_old, rr_new: |r|^2 before and after the cycle.  Returns true if it switched.
+bool mixed_inner_fallback(lgt_ctx* c, double rr_old, double rr_new, double eps) {
+    if (c->inner_exact || !(rr_new > 1e-4 * rr_old && rr_new > 100.0 * eps * eps * rr_old)) return false;
+    c->inner_exact = true;
+    for (lgt_ctx::ChunkGraph& g : c->graphs) cudaGraphExecDestroy(g.exec);
+    c->graphs.clear();
+    return true;
+}
 int eo_cg_mixed(lgt_ctx* c, void* b, void* x, void* r, void* q, void* u, void* t_o, double tol, int max_iter, int* iters) {
     typedef Ops<double> O64;
     typedef Ops<float> O32;
@@ -1100,6 +1118,7 @@ int eo_cg_mixed(lgt_ctx* c, void* b, void* x, void* r, void* q, void* u, void* t
         CU(cudaMalloc(&c->eo32, (size_t)6 * n * sizeof(float2)));
         CU(cudaMemsetAsync(c->eo32, 0, (size_t)6 * n * sizeof(float2), c->stream));
         c->ucb32_valid = false;
+        c->inner_exact = false;
     }
     const int nb = stream_blocks(c, n);
     if (!c->ucb32_valid) {
@@ -1137,6 +1156,7 @@ int eo_cg_mixed(lgt_ctx* c, void* b, void* x, void* r, void* q, void* u, void* t
         LAUNCH(c, LGT_K_CG_BLAS, residual_kernel, nb, 256, n, (const double2*)b, (const double2*)q, (double2*)r, c->scal + 3, c->partials, c->counter);
         CU(cudaMemcpyAsync(c->h_scal + 3, c->scal + 3, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
         CU(cudaStreamSynchronize(c->stream));
+        mixed_inner_fallback(c, rr, c->h_scal[3], eps);
         rr = c->h_scal[3];
     }
     c->last_outer = outer;
@@ -1663,6 +1683,7 @@ int lgt_set_links(lgt_ctx* c, const void* U) {
     if (c->dd_links_valid) *c->dd_links_valid = false;
     c->ucb_valid = false;
     c->ucb32_valid = false;
+    c->inner_exact = false;
     return DISPATCH(c, to_native, c, U, c->U, 36);
 }
 int lgt_get_links(lgt_ctx* c, void* U) {
@@ -2076,6 +2097,7 @@ int lgt_hmc_trajectory(lgt_ctx* c, int nsteps, double dt, double tol, int max_it
     if (c->dd_links_valid) *c->dd_links_valid = false;
         c->ucb_valid = false;
     c->ucb32_valid = false;
+    c->inner_exact = false;
     }
     CU(cudaStreamSynchronize(c->stream));
     if (dH) *dH = d;
@@ -2159,6 +2181,7 @@ int lgt_set_smearing(lgt_ctx* c, int n_levels, double rho) {
     c->u32_valid = false;
     c->ucb_valid = false;
     c->ucb32_valid = false;
+    c->inner_exact = false;
     return LGT_OK;
 }
 int lgt_get_smeared_links(lgt_ctx* c, void* U) {

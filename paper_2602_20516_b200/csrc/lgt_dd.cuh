@@ -1410,7 +1410,9 @@ int dd_eo_cg_mixed(lgt_dd* d, double tol, int max_iter, int* iters) {
             LAUNCH(c, LGT_K_CG_BLAS, residual_kernel, stream_blocks(c, cnt), 256, cnt, (const double2*)D64::hB(c) + off,
                    (const double2*)D64::hP(c) + off, (double2*)D64::hR(c) + off, c->scal + 3, c->partials, c->counter, D64::zmask_half(c));
         }
+        const double rr_old = rr;
         if ((rc = read_sum(rr)) != LGT_OK) return rc;
+        for (int i = 0; i < n; i++) mixed_inner_fallback(d->rk[i], rr_old, rr, eps);  // the same decision on every rank: rr is the global sum
     }
     if (iters) *iters = total;
     if (conv != LGT_OK) return dd_fail(d, LGT_ENOCONV, "mixed-precision even/odd CG did not reach the tolerance");

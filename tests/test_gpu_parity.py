@@ -535,6 +535,28 @@ def test_eo_mixed_solver_inner_hops_on_twelve_real_links(lgt, bc):
     l32.close()
 
 
+def test_eo_mixed_solver_survives_links_off_the_group(lgt):
+    """Links that are not special unitary (here 1.03 U): the 12-real inner hops rebuild a third row that is off by 3 %, the first
+    correction cycle does not contract, and the solver falls back to the exact fp32 links (mixed_inner_fallback).  The force is
+    the oracle's for these links to 1e-10; the price is iterations, never accuracy."""
+    dims, kappa, tol = (16, 16, 16, 20), 0.11, 1e-12
+    V = synth.volume(dims)
+    U = 1.03 * synth.warm_links(dims, 0.3, 157)
+    phi = oeo.mhat(dims, kappa, BC, U, oeo.keep(synth.gaussian_spinor(dims, 158), dims, 0), dagger=True)
+    F_ref, it_ref, _ = oeo.fermion_force(dims, kappa, BC, U, phi, tol, 10 * V)
+    lat = lgt.Lattice(dims, 5.5, kappa, BC)
+    lat.set_links(U)
+    lat.set_pseudofermion(phi)
+    lgt.lgt_set_fermion_action(lat.ctx, lgt.LGT_ACTION_EO)
+    lgt.lgt_set_solver(lat.ctx, lgt.LGT_SOLVER_MIXED_CG, 1e-5)
+    F, it = lat.fermion_force(None, None, tol=tol, max_iter=10 * V)
+    assert link_rel_err(F, F_ref)[0] < 1e-10
+    assert it_ref <= it < 4 * it_ref + 40  # one wasted inner solve at most, then the usual count
+    F2, it2 = lat.fermion_force(None, None, tol=tol, max_iter=10 * V)  # the fallback holds while the links stay
+    assert link_rel_err(F2, F_ref)[0] < 1e-10 and it2 < it  # (78, then 48 fp32 iterations when this was written)
+    lat.close()
+
+
 def test_eo_leapfrog_conserves_energy(lgt):
     """Leapfrog with the even/odd action on 8^4: |dH| ~ dt^2 and exact reversibility (pin P7 on this action)."""
     dims, beta, kappa = (8, 8, 8, 8), 5.6, 0.12
