@@ -276,8 +276,9 @@ int lgt_dd_halo_plan(int nranks, int rank, int lt_local, int plan[8]);
 /*   LGT_DD_HALF: the schedule of LGT_DD_OVERLAP with HALF SPINORS on the wire: the boundary sites are projected
  *     before the send -- and for the backward face also multiplied by U_t^dag -- so that 6 instead of 12 complex numbers per face
  *     site travel, and the boundary slices take that t hop from the received face.  Same iterates bit for bit.
- *   With the even/odd action LGT_DD_OVERLAP and LGT_DD_HALF both overlap the exchange of the input half field of every hop with
- *     the bulk of the slab (whole half spinors on the wire; V3/2 % 128 == 0, slabs of three or more slices, else the plain exchange). */
+ *   With the even/odd action LGT_DD_OVERLAP and LGT_DD_HALF overlap the halo of every hop's input half field with the bulk of
+ *     the slab in the same way (ghost slices, respectively projected / multiplied faces of V3/2 half spinors, on the wire;
+ *     V3/2 % 128 == 0, slabs of three or more slices, else the plain exchange). */
 enum { LGT_DD_EXCHANGE = 0, LGT_DD_PUSH = 1, LGT_DD_OVERLAP = 2, LGT_DD_HALF = 3 };
 int lgt_dd_set_halo_mode(lgt_dd* d, int mode);
 int lgt_dd_ipc_export(lgt_dd* d, void* handles128);

@@ -2265,6 +2265,117 @@ __global__ void __launch_bounds__(128, PFL ? 3 : 1) hop_cb_kernel(Geom g, int p,
     }
 }
 
+// ---- half-spinor halos of a time slab for the even/odd hops (LGT_DD_HALF with LGT_ACTION_EO).  As halo_pack_kernel /
+// dslash_halo_kernel above, on half fields: the input field has the parity 1 - p of the hop's output, its links are Uq; the
+// faces hold V3/2 sites in the order of the checkerboard index within a time slice, which is the same function of (x, y, z)
+// for both parities, so an output site and its t neighbour share the face index.
+template <class T, int DAG>
+__global__ void __launch_bounds__(128) halo_pack_cb_kernel(Geom g, const typename Vec2<T>::type* __restrict__ Uq,
+                                                           const typename Vec2<T>::type* __restrict__ in,
+                                                           typename Vec2<T>::type* __restrict__ lo_out,
+                                                           typename Vec2<T>::type* __restrict__ hi_out, int Vh3) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= 2 * Vh3) return;
+    constexpr int F = DAG ? +1 : -1;
+    cx<T> p[12], h[6];
+    if (i < Vh3) {  // first interior slice -> the lower neighbour's forward t hop (which multiplies by its own link)
+        load_spinor<T>(in, g.h_begin + i, p);
+        spin_project<3, F>(p, h);
+        typename Vec2<T>::type* b = half_at(lo_out, i);
+#pragma unroll
+        for (int k = 0; k < 6; k++) stc<T>(b + k * W, h[k]);
+    } else {        // last interior slice -> the upper neighbour's backward t hop, link applied here
+        const int j = i - Vh3, c = g.h_end - Vh3 + j;
+        cx<T> u[9], w[6];
+        load_spinor<T>(in, c, p);
+        load_link<T>(Uq, 3, c, u);
+        spin_project<3, -F>(p, h);
+        su3_dag_mul_half(u, h, w);
+        typename Vec2<T>::type* b = half_at(hi_out, j);
+#pragma unroll
+        for (int k = 0; k < 6; k++) stc<T>(b + k * W, w[k]);
+    }
+}
+
+// hop_cb_kernel (modes 0 - 3, no push) for ONE boundary time slice [g.h_begin, g.h_end) of a slab: HALO 1 = the slab's first
+// slice, backward t hop from the received face `lo_in`; HALO 2 = its last slice, forward t hop from `hi_in` times the own link.
+template <class T, int DAG, int MODE, int HALO>
+__global__ void __launch_bounds__(128, 1) hop_cb_halo_kernel(Geom g, int p, const typename Vec2<T>::type* __restrict__ Up,
+                                                             const typename Vec2<T>::type* __restrict__ Uq,
+                                                             const typename Vec2<T>::type* __restrict__ in,
+                                                             const typename Vec2<T>::type* __restrict__ self,
+                                                             typename Vec2<T>::type* __restrict__ out, T kap, CgState* st,
+                                                             double* partials, typename Vec2<T>::type* __restrict__ r,
+                                                             const typename Vec2<T>::type* __restrict__ lo_in,
+                                                             const typename Vec2<T>::type* __restrict__ hi_in) {
+    const int done = (MODE != 0) ? st->done : 0;
+    const int c = g.h_begin + blockIdx.x * blockDim.x + threadIdx.x;
+    double nrm = 0.0;
+    if (c < g.h_end) {
+        int s;
+        const Site cs = cb_coords(g, p, c, s);
+        cx<T> acc[12];
+#pragma unroll
+        for (int k = 0; k < 12; k++) acc[k] = mk<T>(0, 0);
+        constexpr int F = DAG ? +1 : -1;
+        hop_fwd_cb<0, F, T>(g, Up, in, cs, s, c, acc);
+        if (MODE != 0 && done) return;  // uniform over the grid
+        hop_bwd_cb<0, -F, T>(g, Uq, in, cs, s, acc);
+        hop_fwd_cb<1, F, T>(g, Up, in, cs, s, c, acc);
+        hop_bwd_cb<1, -F, T>(g, Uq, in, cs, s, acc);
+        hop_fwd_cb<2, F, T>(g, Up, in, cs, s, c, acc);
+        hop_bwd_cb<2, -F, T>(g, Uq, in, cs, s, acc);
+        if (HALO & 2) {
+            cx<T> h[6], u[9], w[6];
+            const typename Vec2<T>::type* b = half_at(hi_in, c - g.h_begin);
+#pragma unroll
+            for (int k = 0; k < 6; k++) h[k] = ldc<T>(b + k * W);
+            load_link<T>(Up, 3, c, u);
+            su3_mul_half(u, h, w);
+            spin_reconstruct_add<3, F>(w, acc);
+        } else {
+            hop_fwd_cb<3, F, T>(g, Up, in, cs, s, c, acc);
+        }
+        if (HALO & 1) {
+            cx<T> w[6];
+            const typename Vec2<T>::type* b = half_at(lo_in, c - g.h_begin);
+#pragma unroll
+            for (int k = 0; k < 6; k++) w[k] = ldc<T>(b + k * W);
+            spin_reconstruct_add<3, -F>(w, acc);
+        } else {
+            hop_bwd_cb<3, -F, T>(g, Uq, in, cs, s, acc);
+        }
+        if (MODE == 2) {
+            const T alpha = (T)st->alpha;
+            const typename Vec2<T>::type* bi = spinor_at(self, c);
+            typename Vec2<T>::type* br = spinor_at(r, c);
+#pragma unroll
+            for (int k = 0; k < 12; k++) {
+                cx<T> sv = ldc<T>(bi + k * W);
+                cx<T> q = mk<T>(fma(-kap, acc[k].re, sv.re), fma(-kap, acc[k].im, sv.im));
+                cx<T> rv = ldc_rw<T>(br + k * W);
+                rv.re = fma(-alpha, q.re, rv.re);
+                rv.im = fma(-alpha, q.im, rv.im);
+                stc<T>(br + k * W, rv);
+                nrm += (double)rv.re * (double)rv.re + (double)rv.im * (double)rv.im;
+            }
+        } else {
+            typename Vec2<T>::type* bo = spinor_at(out, c);
+#pragma unroll
+            for (int k = 0; k < 12; k++) {
+                cx<T> sv = mk<T>(0, 0);
+                if (self) sv = ldc<T>(spinor_at(self, c) + k * W);
+                cx<T> o = mk<T>(fma(-kap, acc[k].re, sv.re), fma(-kap, acc[k].im, sv.im));
+                stc<T>(bo + k * W, o);
+                if (MODE == 1) nrm += (double)o.re * (double)o.re + (double)o.im * (double)o.im;
+            }
+        }
+    } else if (MODE != 0 && done) {
+        return;
+    }
+    if (MODE == 1 || MODE == 2) block_partial(nrm, partials);
+}
+
 // ---------------------------------------------------------------------------- the whole even/odd CG in ONE cooperative kernel
 // Small lattices (the paper's own sizes: 16^4 down to 6^4) are bound by launches: an iteration of the
 // even/odd CG is seven kernels of a few microseconds each.  Here one cooperative launch runs the iterations until the

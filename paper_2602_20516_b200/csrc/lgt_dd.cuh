@@ -516,10 +516,11 @@ template <class T> struct DdOps {
     // the 12-complex slices (half the bytes), and the two boundary slices run dslash_halo_kernel, which takes the t hop that
     // reaches into the ghost slice from the received face.  Same operations on the same numbers: bitwise the same iterates.
     // mode 1: t = D p (out = field 3); mode 2: r -= alpha D^dag t (r = field 1).
-    static int half_spinor_dslash(lgt_dd* d, int k, int mode) {
-        int rc;
-        const int n = (int)d->rk.size(), slice = d->V3;
-        const size_t face = (size_t)6 * slice * sizeof(T2);
+    // the halo stream with its events, and per local rank four faces of 6 V3 complex doubles (enough for either precision and
+    // for the half fields of the even/odd hops)
+    static int ensure_half_faces(lgt_dd* d) {
+        const int n = (int)d->rk.size();
+        const size_t face = (size_t)6 * d->V3 * sizeof(double2);
         if (!d->halo_stream) {
             DD_CU(cudaStreamCreateWithFlags(&d->halo_stream, cudaStreamNonBlocking));
             DD_CU(cudaEventCreateWithFlags(&d->ev_ready, cudaEventDisableTiming));
@@ -529,9 +530,16 @@ template <class T> struct DdOps {
             DD_CU(cudaStreamSynchronize(d->stream));
             for (void* f : d->half_faces) cudaFree(f);
             d->half_faces.assign(n, nullptr);
-            for (int i = 0; i < n; i++) DD_CU(cudaMalloc(&d->half_faces[i], 4 * (size_t)6 * slice * sizeof(double2)));
-            d->half_face_bytes = (size_t)6 * slice * sizeof(double2);
+            for (int i = 0; i < n; i++) DD_CU(cudaMalloc(&d->half_faces[i], 4 * face));
+            d->half_face_bytes = face;
         }
+        return LGT_OK;
+    }
+    static int half_spinor_dslash(lgt_dd* d, int k, int mode) {
+        int rc;
+        const int n = (int)d->rk.size(), slice = d->V3;
+        const size_t face = (size_t)6 * slice * sizeof(T2);
+        if ((rc = ensure_half_faces(d)) != LGT_OK) return rc;
         const int dag = mode == 2 ? 1 : 0;
         // faces of every rank's input field, on the main stream (they read the field the previous kernels completed)
         for (int i = 0; i < n; i++) {
@@ -953,6 +961,93 @@ template <class T> struct DdOps {
         // stream under the bulk of the slab, the two boundary slices after it -- DdOps::overlapped for the half-field range.
         // Block partials land where a single launch would put them: in fp64 bitwise the iterates of LGT_DD_EXCHANGE.
         const int hslice = d->V3 / 2;
+        // LGT_DD_HALF: the same schedule with half spinors on the wire (halo_pack_cb_kernel / hop_cb_halo_kernel; modes 0 - 3)
+        if (!input_current && !push && d->halo_mode == LGT_DD_HALF && d->Pz == 0 && hslice % 128 == 0 && d->Lt_loc >= 3) {
+            if ((rc = ensure_half_faces(d)) != LGT_OK) return rc;
+            const size_t face = (size_t)6 * hslice * sizeof(T2);
+            const int n = (int)d->rk.size();
+            for (int i = 0; i < n; i++) {  // faces of the input field, on the main stream
+                lgt_ctx* c = d->rk[i];
+                const int p = to_even ? pe_of(c) : 1 - pe_of(c);
+                T2* H = (T2*)d->half_faces[i];
+                const int pg = (2 * hslice + 127) / 128;
+                if (dagger) LAUNCH(c, LGT_K_OTHER, (halo_pack_cb_kernel<T, 1>), pg, 128, c->g, O::links_cb(c, 1 - p), (const T2*)in(c), H, H + (size_t)6 * hslice, hslice);
+                else LAUNCH(c, LGT_K_OTHER, (halo_pack_cb_kernel<T, 0>), pg, 128, c->g, O::links_cb(c, 1 - p), (const T2*)in(c), H, H + (size_t)6 * hslice, hslice);
+            }
+            DD_CU(cudaEventRecord(d->ev_ready, d->stream));
+            for (int i = 0; i < n; i++) {  // bulk
+                lgt_ctx* c = d->rk[i];
+                const int p = to_even ? pe_of(c) : 1 - pe_of(c);
+                const double kap = plus_kappa ? c->kappa : -c->kappa;
+                const int b0 = c->g.h_begin, e0 = c->g.h_end;
+                double* const part0 = c->partials;
+                c->g.h_begin = b0 + hslice;
+                c->g.h_end = e0 - hslice;
+                c->partials = part0 + hslice / 128;
+                rc = O::hop(c, p, in(c), self ? self(c) : nullptr, out ? out(c) : nullptr, dagger, mode, kap, r ? r(c) : nullptr);
+                c->g.h_begin = b0;
+                c->g.h_end = e0;
+                c->partials = part0;
+                if (rc != LGT_OK) return dd_fail(d, rc, c->err.c_str());
+            }
+            DD_CU(cudaStreamWaitEvent(d->halo_stream, d->ev_ready, 0));
+            cudaStream_t const main_stream = d->stream;
+            d->stream = d->halo_stream;
+            const size_t send_off[2] = {0, face}, recv_off[2] = {2 * face, 3 * face};
+            rc = dd_exchange_regions(d, d->half_faces.data(), send_off, recv_off, face);
+            d->stream = main_stream;
+            if (rc != LGT_OK) return rc;
+            DD_CU(cudaEventRecord(d->ev_halo, d->halo_stream));
+            DD_CU(cudaStreamWaitEvent(d->stream, d->ev_halo, 0));
+            for (int i = 0; i < n; i++) {  // the two boundary slices from the received faces
+                lgt_ctx* c = d->rk[i];
+                const int p = to_even ? pe_of(c) : 1 - pe_of(c);
+                const T kap = (T)(plus_kappa ? c->kappa : -c->kappa);
+                const int b0 = c->g.h_begin, e0 = c->g.h_end;
+                double* const part0 = c->partials;
+                const T2* H = (const T2*)d->half_faces[i];
+                const T2 *hi_in = H + (size_t)12 * hslice, *lo_in = H + (size_t)18 * hslice;
+                const int bg = hslice / 128;
+                const T2 *Up = O::links_cb(c, p), *Uq = O::links_cb(c, 1 - p);
+                const T2* sf = self ? (const T2*)self(c) : nullptr;
+                T2* of = out ? out(c) : nullptr;
+                T2* rf = r ? r(c) : nullptr;
+                rc = LGT_OK;
+                for (int side = 0; side < 2 && rc == LGT_OK; side++) {
+                    if (side == 0) {
+                        c->g.h_begin = b0;
+                        c->g.h_end = b0 + hslice;
+                        c->partials = part0;
+                    } else {
+                        c->g.h_begin = e0 - hslice;
+                        c->g.h_end = e0;
+                        c->partials = part0 + (e0 - hslice - b0) / 128;
+                    }
+                    rc = [&]() -> int {
+#define HALO_ARGS c->g, p, Up, Uq, (const T2*)in(c), sf, of, kap, c->st, c->partials, rf, lo_in, hi_in
+#define HALO_LAUNCH(DAG, MODE, KC)                                                                                   \
+    do {                                                                                                             \
+        if (side == 0) LAUNCH(c, KC, (hop_cb_halo_kernel<T, DAG, MODE, 1>), bg, 128, HALO_ARGS);                     \
+        else LAUNCH(c, KC, (hop_cb_halo_kernel<T, DAG, MODE, 2>), bg, 128, HALO_ARGS);                               \
+    } while (0)
+                        if (mode == 0 && !dagger) HALO_LAUNCH(0, 0, LGT_K_DSLASH);
+                        else if (mode == 0) HALO_LAUNCH(1, 0, LGT_K_DSLASH);
+                        else if (mode == 3 && !dagger) HALO_LAUNCH(0, 3, LGT_K_DSLASH);
+                        else if (mode == 3) HALO_LAUNCH(1, 3, LGT_K_DSLASH);
+                        else if (mode == 1) HALO_LAUNCH(0, 1, LGT_K_DSLASH);
+                        else HALO_LAUNCH(1, 2, LGT_K_DSLASH_R);
+#undef HALO_LAUNCH
+#undef HALO_ARGS
+                        return LGT_OK;
+                    }();
+                }
+                c->g.h_begin = b0;
+                c->g.h_end = e0;
+                c->partials = part0;
+                if (rc != LGT_OK) return dd_fail(d, rc, c->err.c_str());
+            }
+            return LGT_OK;
+        }
         if (!input_current && !push && (d->halo_mode == LGT_DD_OVERLAP || d->halo_mode == LGT_DD_HALF) && d->Pz == 0 && hslice % 128 == 0 &&
             d->Lt_loc >= 3) {
             if (!d->halo_stream) {

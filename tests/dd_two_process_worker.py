@@ -131,7 +131,7 @@ def main():
     ephi = oeo2.mhat(edims, kappa, BC, eU, oeo2.keep(synth.gaussian_spinor(edims, 633), edims, 0), dagger=True)
     _, eit_ref, _ = oeo2.fermion_force(edims, kappa, BC, eU, ephi, 1e-12, 10 * eV)
     eres = {}
-    for halo in ("exchange", "overlap"):
+    for halo in ("exchange", "overlap", "half"):
         dd = dist.decomposed_lattice(edims, beta, kappa, BC, lgt.LGT_F64, 0, None, halo=halo, transport="host")
         lgt.lgt_dd_set_fermion_action(dd.d, lgt.LGT_ACTION_EO)
         dd.set_links(eU)
@@ -142,6 +142,7 @@ def main():
         dd.close()
         dist.barrier()
     assert np.array_equal(eres["exchange"], eres["overlap"])
+    assert np.array_equal(eres["exchange"], eres["half"])  # half-spinor faces of the half fields
     out["eo_overlap_cg_iters"] = eit_ref
     out["overlap_cg_iters"] = oit_ref
 
