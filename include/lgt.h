@@ -398,7 +398,9 @@ int lgt_set_block_swizzle(lgt_ctx* ctx, int z_planes, int* in_effect);
  *         them variant 12 selects the same 12-real links (hop_cb_kernel PFL 2: 32^4 hop 67 -> 59 us).  In the fp32 INNER solve
  *         of the mixed-precision even/odd solver on lattices of more than two waves of blocks that is the DEFAULT -- the fp64
  *         defect correction keeps the exact operator, so links that are not special unitary cost iterations, never accuracy
- *         (even/odd mixed-precision MD step at 32^4 27.9 -> 25.4 ms, same iteration count).
+ *         (even/odd mixed-precision MD step at 32^4 27.9 -> 25.4 ms, same iteration count).  On an fp64 handle variant 12 also
+ *         puts the fp64 even/odd hops on 12-real links (plain build; 32^4 even/odd CG 645-660 -> 601-626 us per iteration, same
+ *         count, solutions equal to 6e-16) -- opt-in only: exact for special unitary links.
  *   LGT_K_GAUGE_FORCE: 0 = one 32-site layout block x 4 directions per 128-thread block (default, fastest);
  *     1 / 2 = two / four layout blocks per 256- / 512-thread block (more sharing through L1; measured slower).  Same sums bit for bit.
  *     3 = one thread per site: the down staples link by link, the up staples plaquette by plaquette (U_mu(s) U_nu(s+mu)

@@ -2149,7 +2149,7 @@ __device__ __forceinline__ void hop_bwd_cb(const Geom& g, const typename Vec2<T>
 // half the registers, and 12 warps per SM gain 10-13 % per fp32 even/odd CG iteration above one wave of blocks (on a
 // single wave the default build is 4 % faster and stays).
 template <class T, int DAG, int MODE, int PUSH = 0, int ZS = 0, int PFL = 0>
-__global__ void __launch_bounds__(128, PFL ? 3 : 1) hop_cb_kernel(Geom g, int p, const typename Vec2<T>::type* __restrict__ Up,
+__global__ void __launch_bounds__(128, (PFL == 1 || PFL == 2) ? 3 : 1) hop_cb_kernel(Geom g, int p, const typename Vec2<T>::type* __restrict__ Up,
                                                         const typename Vec2<T>::type* __restrict__ Uq,
                                                         const typename Vec2<T>::type* __restrict__ in,
                                                         const typename Vec2<T>::type* __restrict__ self,
@@ -2173,7 +2173,9 @@ __global__ void __launch_bounds__(128, PFL ? 3 : 1) hop_cb_kernel(Geom g, int p,
 #pragma unroll
         for (int k = 0; k < 12; k++) acc[k] = mk<T>(0, 0);
         constexpr int F = DAG ? +1 : -1;
-        constexpr int TW = (PFL == 2) ? 1 : 0;  // PFL 2 (variant 12 of LGT_K_DSLASH): 12-real links, 384 instead of 576 link bytes per site
+        // PFL 2 (variant 12 of LGT_K_DSLASH): 12-real links, 384 instead of 576 link bytes per site (fp32); PFL 4: 12-real links in
+        // the plain build -- one block per SM, no prefetch -- for the fp64 hops (768 instead of 1152 link bytes per site)
+        constexpr int TW = (PFL == 2 || PFL == 4) ? 1 : 0;
         hop_fwd_cb<0, F, T, 0, TW>(g, Up, in, cs, s, c, acc);
         if (MODE != 0 && done) return;  // uniform over the grid
         hop_bwd_cb<0, -F, T, 0, TW>(g, Uq, in, cs, s, acc);
@@ -2183,7 +2185,7 @@ __global__ void __launch_bounds__(128, PFL ? 3 : 1) hop_cb_kernel(Geom g, int p,
         hop_bwd_cb<2, -F, T, 0, TW>(g, Uq, in, cs, s, acc);
         hop_fwd_cb<3, F, T, 0, TW>(g, Up, in, cs, s, c, acc);
         hop_bwd_cb<3, -F, T, 0, TW>(g, Uq, in, cs, s, acc);
-        if (PFL && blockIdx.x + pf < gridDim.x) {
+        if ((PFL == 1 || PFL == 2) && blockIdx.x + pf < gridDim.x) {
             const int lane = threadIdx.x & 31;
             const int cp = c - lane + pf * (int)blockDim.x;  // first site of this warp's counterpart in the later block
             if (cp < g.h_end) {

@@ -912,6 +912,22 @@ template <class T> struct Ops {
                 return twelve ? launch_pfl(std::integral_constant<int, 2>()) : launch_pfl(std::integral_constant<int, 1>());
             }
         }
+        if constexpr (sizeof(T) == 8) if (c->variant[LGT_K_DSLASH] == 12) {  // fp64 hops on 12-real links (opt-in: exact for special unitary links only)
+            if (mode == 0) {
+                if (dagger) LAUNCH(c, LGT_K_DSLASH, (hop_cb_kernel<T, 1, 0, 0, 0, 4>), grid, 128, HOP_ARGS);
+                else LAUNCH(c, LGT_K_DSLASH, (hop_cb_kernel<T, 0, 0, 0, 0, 4>), grid, 128, HOP_ARGS);
+            } else if (mode == 3) {
+                if (dagger) LAUNCH(c, LGT_K_DSLASH, (hop_cb_kernel<T, 1, 3, 0, 0, 4>), grid, 128, HOP_ARGS);
+                else LAUNCH(c, LGT_K_DSLASH, (hop_cb_kernel<T, 0, 3, 0, 0, 4>), grid, 128, HOP_ARGS);
+            } else if (mode == 4) {
+                LAUNCH(c, LGT_K_DSLASH, (hop_cb_kernel<T, 1, 4, 0, 0, 4>), grid, 128, HOP_ARGS, nullptr, 0, grid);
+            } else if (mode == 1) {
+                LAUNCH(c, LGT_K_DSLASH, (hop_cb_kernel<T, 0, 1, 0, 0, 4>), grid, 128, HOP_ARGS, fuse_counter(c));
+            } else {
+                LAUNCH(c, LGT_K_DSLASH_R, (hop_cb_kernel<T, 1, 2, 0, 0, 4>), grid, 128, HOP_ARGS, fuse_counter(c));
+            }
+            return LGT_OK;
+        }
         if (mode == 0) {
             if (dagger) LAUNCH(c, LGT_K_DSLASH, (hop_cb_kernel<T, 1, 0>), grid, 128, HOP_ARGS);
             else LAUNCH(c, LGT_K_DSLASH, (hop_cb_kernel<T, 0, 0>), grid, 128, HOP_ARGS);

@@ -521,6 +521,14 @@ def test_eo_mixed_solver_inner_hops_on_twelve_real_links(lgt, bc):
     assert lgt.lgt_set_kernel_variant(lat.ctx, lgt.LGT_K_DSLASH, 8) == 8  # exact 9-entry links in the inner hops
     F9, it9 = lat.fermion_force(None, None, tol=tol, max_iter=10 * V)
     assert abs(it - it9) <= 2 and link_rel_err(F9, F_ref)[0] < 1e-10
+    # the fp64 hops themselves on 12-real links (variant 12, opt-in): same solve to rounding, same count
+    lgt.lgt_set_solver(lat.ctx, lgt.LGT_SOLVER_CG)
+    b64 = synth.gaussian_spinor(dims, 150)
+    assert lgt.lgt_set_kernel_variant(lat.ctx, lgt.LGT_K_DSLASH, 0) == 0
+    x0, it0, _, ok0 = lat.eo_cg(b64, tol, 10 * V)
+    assert lgt.lgt_set_kernel_variant(lat.ctx, lgt.LGT_K_DSLASH, 12) == 12
+    x12, it12, _, ok12 = lat.eo_cg(b64, tol, 10 * V)
+    assert ok0 and ok12 and it0 == it12 and np.abs(x12 - x0).max() < 1e-12 * np.abs(x0).max()
     lat.close()
     # fp32 handle: variant 12 against the default's exact links
     b = round32(synth.gaussian_spinor(dims, 149))
