@@ -1020,13 +1020,18 @@ def run_kernel_variants(args):
     dims, kappa, bc = cfg["dims"], cfg["kappa"], cfg["bc"]
     V = synth.volume(dims)
     U, _, eta = make_inputs(cfg)
-    lat = lgt.Lattice(dims, cfg["beta"], kappa, bc, lgt.LGT_F64, 0, torch.cuda.current_stream().cuda_stream)
+    f32 = args.variant_precision == "f32"
+    if f32 and args.variant_class != "dslash":
+        raise SystemExit("--variant-precision f32 is for --variant-class dslash")
+    lat = lgt.Lattice(dims, cfg["beta"], kappa, bc, lgt.LGT_F32 if f32 else lgt.LGT_F64, 0, torch.cuda.current_stream().cuda_stream)
     ctx = lat.ctx
-    lgt.lgt_set_links_host(ctx, torch.from_numpy(U).pin_memory())
+    lgt.lgt_set_links_host(ctx, torch.from_numpy(U.astype("complex64") if f32 else U).pin_memory())
     nat = [lat.native_spinor() for _ in range(4)]
     lgt.lgt_spinor_to_native(ctx, lat.to_device(eta), nat[0])
     del U, eta
-    out = {"lattice": "x".join(map(str, dims)), "dtype": "f64", "kernel_class": args.variant_class, "variants": {}}
+    esize = 4 if f32 else 8
+    cg_tol = 1e-5 if f32 else cfg.get("cg_tol", 1e-12)
+    out = {"lattice": "x".join(map(str, dims)), "dtype": "f32" if f32 else "f64", "kernel_class": args.variant_class, "variants": {}}
     kclass = lgt.KERNEL_CLASSES.index(args.variant_class)
     ref = {}
     names = VARIANT_NAMES[args.variant_class]
@@ -1039,7 +1044,7 @@ def run_kernel_variants(args):
                 t = time_calls(lambda: lgt.lgt_dslash_native(ctx, nat[0], nat[1], dag), n=args.variant_launches,
                                warm=min(5, args.variant_launches))
                 key = "dslash_dagger" if dag else "dslash"
-                res[key] = {"us": round(t * 1e6, 1), "GB/s": round(REALS["dslash"] * 8 * V / t / 1e9, 1)}
+                res[key] = {"us": round(t * 1e6, 1), "GB/s": round(REALS["dslash"] * esize * V / t / 1e9, 1)}
                 got = nat[1].clone()
                 res[key]["bitwise_variant0"] = bool(torch.equal(got, ref.setdefault(key, got)))
             if args.variant_no_cg:  # ncu captures: the isolated launches only
@@ -1049,7 +1054,7 @@ def run_kernel_variants(args):
             for _ in range(2):
                 torch.cuda.synchronize()
                 t0 = time.perf_counter()
-                it, rel, ok = lgt.lgt_cg_native(ctx, nat[2], nat[3], None, cfg.get("cg_tol", 1e-12), 10 * V)
+                it, rel, ok = lgt.lgt_cg_native(ctx, nat[2], nat[3], None, cg_tol, 10 * V)
                 torch.cuda.synchronize()
                 dt = time.perf_counter() - t0
             got = nat[3].clone()
@@ -1111,6 +1116,8 @@ def main():
     ap.add_argument("--variant-class", default="dslash", choices=sorted(VARIANT_NAMES))
     ap.add_argument("--only-variants", default="", help="comma-separated variant numbers (default: all)")
     ap.add_argument("--variant-launches", type=int, default=20)
+    ap.add_argument("--variant-precision", default="f64", choices=["f64", "f32"],
+                    help="--kernel-variants --variant-class dslash: precision of the handle (f32: CG to 1e-5)")
     ap.add_argument("--variant-no-cg", action="store_true", help="--kernel-variants: isolated launches only (for ncu captures)")
     ap.add_argument("--peaks", action="store_true", help="print the measured fp64 / fp32 FMA and copy peaks and exit")
     args = ap.parse_args()
