@@ -115,6 +115,8 @@ int lgt_cg(lgt_ctx* ctx, const void* b, void* x, double tol, int max_iter, int* 
  * tolerance: defect correction x <- x + e where e ~ (D^dag D)^-1 r comes from a CG run entirely in fp32 on the
  * residual scaled to unit norm, to relative residual max(inner_tol, tol |b| / (4 |r|)); then r = b - D^dag D x in
  * fp64.  Stops when the TRUE residual satisfies |r| <= tol |b| (so rel_resid is a true, not a recurrence, residual).
+ * From the second cycle on the inner CG keeps the previous cycle's last search direction (p = r + beta p_k, a reliable update
+ * instead of a restart) as long as the previous cycle delivered the reduction it was asked for.
  * inner_iters = fp32 CG iterations in total (capped by max_iter), outer_cycles = corrections; any may be NULL.
  * LGT_ENOCONV if the cap (or 40 cycles) was hit; x then holds the last iterate. */
 int lgt_cg_mixed(lgt_ctx* ctx, const void* b, void* x, double tol, int max_iter, double inner_tol,

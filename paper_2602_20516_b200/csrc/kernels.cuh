@@ -1316,12 +1316,14 @@ __device__ __forceinline__ bool zmask_owned(const ZMask& m, size_t i) {
 }
 
 // ---------------------------------------------------------------------------- A3: CG BLAS-1 (fused)
-// r = b, p = b, x = 0, rr = bb = |b|^2
+// r = b, p = b, x = 0, rr = bb = |b|^2.
+// pcoef != 0 (the mixed-precision solvers' later correction cycles): p = b + pcoef * p instead -- the search direction of the
+// previous cycle is kept across the replacement of the residual by the true one ("reliable update") instead of restarting CG.
 template <class T>
 __global__ void __launch_bounds__(256) cg_init_kernel(size_t n, const typename Vec2<T>::type* __restrict__ b,
                                                       typename Vec2<T>::type* __restrict__ x, typename Vec2<T>::type* __restrict__ r,
                                                       typename Vec2<T>::type* __restrict__ p, CgState* st, double tol2, int max_iter,
-                                                      double* partials, unsigned* counter, ZMask zm = ZMask()) {
+                                                      double* partials, unsigned* counter, ZMask zm = ZMask(), T pcoef = 0) {
     double acc = 0.0;
     typename Vec2<T>::type zero;
     zero.x = 0;
@@ -1330,7 +1332,14 @@ __global__ void __launch_bounds__(256) cg_init_kernel(size_t n, const typename V
         typename Vec2<T>::type v = __ldg(b + i);
         x[i] = zero;
         r[i] = v;
-        p[i] = v;
+        if (pcoef != 0) {
+            typename Vec2<T>::type pv = p[i];
+            pv.x = fma(pcoef, pv.x, v.x);
+            pv.y = fma(pcoef, pv.y, v.y);
+            p[i] = pv;
+        } else {
+            p[i] = v;
+        }
         if (zmask_owned(zm, i)) acc += (double)v.x * (double)v.x + (double)v.y * (double)v.y;
     }
     block_reduce_finalize(acc, partials, counter, [=](double sum) {

@@ -617,13 +617,13 @@ template <class T> struct Ops {
     // x += alpha p, p = r + beta p.
     // U: native links of precision T; wr, wp, wt: three native spinor workspaces of precision T.
     static int cg(lgt_ctx* c, const void* U, void* wr, void* wp, void* wt, const void* b, void* x, void* y, double tol,
-                  int max_iter, int* iters, double* rel) {
+                  int max_iter, int* iters, double* rel, double pcoef = 0.0) {
         T2 *r = (T2*)wr, *p = (T2*)wp, *t = (T2*)wt;
         const size_t n = (size_t)12 * c->g.Vs;
         const int nb = stream_blocks(c, n);
         const int ngrid = dslash_partials(c);  // blocks (= partials) of the stencil kernels
         const bool fused = fuse_counter(c) != nullptr;
-        LAUNCH(c, LGT_K_CG_BLAS, (cg_init_kernel<T>), nb, 256, n, (const T2*)b, (T2*)x, r, p, c->st, tol * tol, max_iter, c->partials, c->counter);
+        LAUNCH(c, LGT_K_CG_BLAS, (cg_init_kernel<T>), nb, 256, n, (const T2*)b, (T2*)x, r, p, c->st, tol * tol, max_iter, c->partials, c->counter, ZMask(), (T)pcoef);
         int rc;
         int launched = 0;
         for (;;) {
@@ -951,12 +951,14 @@ template <class T> struct Ops {
         return hop(c, 0, scratch_o, in_e, out_e, dagger, 0, c->kappa);
     }
     // CG on M^dag M x_e = b_e, x0 = 0, same recurrence and stop rule as cg(); u_e, t_o are scratch half fields.
-    static int eo_cg(lgt_ctx* c, const T2* b, T2* x, T2* r, T2* p, T2* u, T2* t, double tol, int max_iter, int* iters, double* rel) {
+    // pcoef != 0: p = b + pcoef p instead of p = b at the start (the previous solve's search direction is kept; eo_cg_mixed)
+    static int eo_cg(lgt_ctx* c, const T2* b, T2* x, T2* r, T2* p, T2* u, T2* t, double tol, int max_iter, int* iters, double* rel,
+                     double pcoef = 0.0) {
         const size_t n = (size_t)12 * c->g.Vhs;
         const int nb = stream_blocks(c, n);
         const int ngrid = (own_half_sites(c) + 127) / 128;
         const bool fused = fuse_counter(c) != nullptr;
-        LAUNCH(c, LGT_K_CG_BLAS, (cg_init_kernel<T>), nb, 256, n, b, x, r, p, c->st, tol * tol, max_iter, c->partials, c->counter);
+        LAUNCH(c, LGT_K_CG_BLAS, (cg_init_kernel<T>), nb, 256, n, b, x, r, p, c->st, tol * tol, max_iter, c->partials, c->counter, ZMask(), (T)pcoef);
         int rc, launched = 0;
         // Small lattices: the whole solve in one cooperative launch (eo_cg_coop_kernel; LGT_K_CG_BLAS variant 2, and the
         // default while the half field is at most two waves of blocks).  Bitwise the iterates of the loop below.
@@ -1144,7 +1146,9 @@ int eo_cg_mixed(lgt_ctx* c, void* b, void* x, void* r, void* q, void* u, void* t
     }
     float2 *b32 = O32::eo_field(c, 0), *e32 = O32::eo_field(c, 1), *r32 = O32::eo_field(c, 2), *p32 = O32::eo_field(c, 3),
            *u32 = O32::eo_field(c, 4), *t32 = O32::eo_field(c, 5);
-    int rc, total = 0, outer = 0, conv = LGT_OK;
+    int rc, total = 0, outer = 0, conv = LGT_OK, prev_it = 0;
+    double prev_scale = 1.0;
+    bool prev_good = false;
     CU(cudaMemsetAsync(x, 0, n * sizeof(double2), c->stream));
     CU(cudaMemcpyAsync(r, b, n * sizeof(double2), cudaMemcpyDeviceToDevice, c->stream));
     if ((rc = O64::redot(c, b, b, c->scal + 3, n)) != LGT_OK) return rc;
@@ -1161,9 +1165,20 @@ int eo_cg_mixed(lgt_ctx* c, void* b, void* x, void* r, void* q, void* u, void* t
         LAUNCH(c, LGT_K_CG_BLAS, down_convert_kernel, nb, 256, n, (const double2*)r, b32, scale);
         double eps = 0.25 * tol * sqrt(bb / rr);
         if (eps < c->inner_tol) eps = c->inner_tol;
+        // Reliable update instead of a restart: the last search direction p_k of the previous cycle (the x, p update leaves p alone
+        // in the iteration that converges) continues, p = r_true + beta p_k with beta = |r_true|^2 / |r_k|^2, |r_k|^2 = rr / beta_k
+        // of the previous cycle's last state; in the units of this cycle (residual scaled to norm 1, p_k rescaled by scale /
+        // prev_scale) that is p = r + pcoef p with pcoef = beta_k / (rr_k+1 * (scale / prev_scale)).
+        // Only while the true residual is the iterated one to fp32 accuracy (the previous cycle delivered within a factor 10 of
+        // what it was asked for): otherwise p_k is not orthogonal to the new residual and CG's step length formula does not hold.
+        double pcoef = 0.0;
+        if (outer > 0 && prev_it > 0 && prev_good && c->h_st->rr > 0.0 && c->h_st->beta > 0.0)
+            pcoef = c->h_st->beta / (c->h_st->rr * (scale / prev_scale));
         int it = 0;
-        rc = O32::eo_cg(c, b32, e32, r32, p32, u32, t32, eps, max_iter - total, &it, nullptr);
+        rc = O32::eo_cg(c, b32, e32, r32, p32, u32, t32, eps, max_iter - total, &it, nullptr, pcoef);
         if (rc != LGT_OK && rc != LGT_ENOCONV) return rc;
+        prev_scale = scale;
+        prev_it = it;
         total += it;
         outer++;
         LAUNCH(c, LGT_K_CG_BLAS, up_axpy_kernel, nb, 256, n, (double2*)x, (const float2*)e32, 1.0 / scale);
@@ -1173,6 +1188,7 @@ int eo_cg_mixed(lgt_ctx* c, void* b, void* x, void* r, void* q, void* u, void* t
         CU(cudaMemcpyAsync(c->h_scal + 3, c->scal + 3, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
         CU(cudaStreamSynchronize(c->stream));
         mixed_inner_fallback(c, rr, c->h_scal[3], eps);
+        prev_good = c->h_scal[3] <= 100.0 * eps * eps * rr;
         rr = c->h_scal[3];
     }
     c->last_outer = outer;
@@ -1222,7 +1238,9 @@ int cg_mixed(lgt_ctx* c, const void* b, void* x, void* y, double tol, int max_it
     double2 *r = (double2*)c->ws[1], *q = (double2*)c->ws[2];
     double2* t = (double2*)(y ? y : c->ws[3]);
     float2 *b32 = (float2*)c->ws32[0], *e32 = (float2*)c->ws32[1];
-    int rc, total = 0, outer = 0, conv = LGT_OK;
+    int rc, total = 0, outer = 0, conv = LGT_OK, prev_it = 0;
+    double prev_scale = 1.0;
+    bool prev_good = false;
     CU(cudaMemsetAsync(x, 0, n * sizeof(double2), c->stream));
     CU(cudaMemsetAsync(t, 0, n * sizeof(double2), c->stream));
     CU(cudaMemcpyAsync(r, b, n * sizeof(double2), cudaMemcpyDeviceToDevice, c->stream));
@@ -1241,9 +1259,15 @@ int cg_mixed(lgt_ctx* c, const void* b, void* x, void* y, double tol, int max_it
         // the inner solve need not go below what the outer tolerance still asks for
         double eps = 0.25 * tol * sqrt(bb / rr);
         if (eps < c->inner_tol) eps = c->inner_tol;
+        // reliable update instead of a restart, as in eo_cg_mixed: p = r + pcoef p_k while the true residual is the iterated one
+        double pcoef = 0.0;
+        if (outer > 0 && prev_it > 0 && prev_good && c->h_st->rr > 0.0 && c->h_st->beta > 0.0)
+            pcoef = c->h_st->beta / (c->h_st->rr * (scale / prev_scale));
         int it = 0;
-        rc = O32::cg(c, c->U32, c->ws32[2], c->ws32[3], c->ws32[4], b32, e32, nullptr, eps, max_iter - total, &it, nullptr);
+        rc = O32::cg(c, c->U32, c->ws32[2], c->ws32[3], c->ws32[4], b32, e32, nullptr, eps, max_iter - total, &it, nullptr, pcoef);
         if (rc != LGT_OK && rc != LGT_ENOCONV) return rc;
+        prev_scale = scale;
+        prev_it = it;
         total += it;
         outer++;
         LAUNCH(c, LGT_K_CG_BLAS, up_axpy_kernel, nb, 256, n, (double2*)x, (const float2*)e32, 1.0 / scale);
@@ -1252,6 +1276,7 @@ int cg_mixed(lgt_ctx* c, const void* b, void* x, void* y, double tol, int max_it
         LAUNCH(c, LGT_K_CG_BLAS, residual_kernel, nb, 256, n, (const double2*)b, (const double2*)q, r, c->scal + 3, c->partials, c->counter);
         CU(cudaMemcpyAsync(c->h_scal + 3, c->scal + 3, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
         CU(cudaStreamSynchronize(c->stream));
+        prev_good = c->h_scal[3] <= 100.0 * eps * eps * rr;
         rr = c->h_scal[3];
     }
     c->last_outer = outer;

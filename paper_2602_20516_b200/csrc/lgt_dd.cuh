@@ -743,8 +743,11 @@ template <class T> struct DdOps {
 
     // CG on D^dag D, b = ws[ib] (or phi for ib == 6), x = ws[0], workspaces r, p, t = ws[1..3]; leaves Y = D x in ws[3]
     // if want_y.  Same recurrence, stop rule and fused kernels as Ops::cg; every sum is all-reduced over the ranks.
-    static int cg(lgt_dd* d, int ib, bool want_y, double tol, int max_iter, int* iters, double* rel) {
+    // pcoef != 0: p = b + pcoef p at the start (the mixed driver's reliable update, as Ops::cg; with pushed halos the ghost
+    // slices of p are set from b, so the solve restarts there)
+    static int cg(lgt_dd* d, int ib, bool want_y, double tol, int max_iter, int* iters, double* rel, double pcoef = 0.0) {
         int rc;
+        if (d->halo_mode == LGT_DD_PUSH) pcoef = 0.0;
         if (!fp32_on_f64(d->rk[0]) && (rc = fermion_links(d)) != LGT_OK) return rc;  // (the mixed driver has done it in fp64)
         const int n = (int)d->rk.size();
         for (int i = 0; i < n; i++) {
@@ -752,7 +755,7 @@ template <class T> struct DdOps {
             const size_t off = spinor_off(c), cnt = spinor_n(c);
             const T2* b = (const T2*)fld(c, ib) + off;
             LAUNCH(c, LGT_K_CG_BLAS, (cg_init_kernel<T>), stream_blocks(c, cnt), 256, cnt, b, (T2*)fld(c, 0) + off, (T2*)fld(c, 1) + off,
-                   (T2*)fld(c, 2) + off, c->st, tol * tol, max_iter, c->partials, c->counter, zmask(c));
+                   (T2*)fld(c, 2) + off, c->st, tol * tol, max_iter, c->partials, c->counter, zmask(c), (T)pcoef);
             LAUNCH(c, LGT_K_CG_BLAS, cg_rr_to_tmp_kernel, 1, 1, c->st);
         }
         if ((rc = allreduce_tmp(d)) != LGT_OK) return rc;
@@ -1137,14 +1140,15 @@ template <class T> struct DdOps {
     // of Ops::eo_cg, input ghost slices exchanged before every hop, sums all-reduced.  B, X, R, P, U: even half fields,
     // Tt: an odd scratch field.  Returns the final recurrence state through *state.
     static int eo_cg_loop(lgt_dd* d, HalfSel B, HalfSel X, HalfSel R, HalfSel P, HalfSel Uu, HalfSel Tt, double tol, int max_iter,
-                          CgState* state) {
+                          CgState* state, double pcoef = 0.0) {
         int rc;
+        if (d->halo_mode == LGT_DD_PUSH) pcoef = 0.0;  // as in cg()
         const int n = (int)d->rk.size();
         for (int i = 0; i < n; i++) {
             lgt_ctx* c = d->rk[i];
             const size_t off = half_off(c), cnt = half_n(c);
             LAUNCH(c, LGT_K_CG_BLAS, (cg_init_kernel<T>), stream_blocks(c, cnt), 256, cnt, (const T2*)B(c) + off, X(c) + off, R(c) + off,
-                   P(c) + off, c->st, tol * tol, max_iter, c->partials, c->counter, zmask_half(c));
+                   P(c) + off, c->st, tol * tol, max_iter, c->partials, c->counter, zmask_half(c), (T)pcoef);
             LAUNCH(c, LGT_K_CG_BLAS, cg_rr_to_tmp_kernel, 1, 1, c->st);
         }
         if ((rc = allreduce_tmp(d)) != LGT_OK) return rc;
@@ -1388,7 +1392,9 @@ int dd_cg_mixed(lgt_dd* d, int ib, bool want_y, double tol, int max_iter, int* i
     double bb = 0.0;
     if ((rc = read_sum(bb)) != LGT_OK) return rc;
     double rr = bb;
-    int total = 0, outer = 0, conv = LGT_OK;
+    int total = 0, outer = 0, conv = LGT_OK, prev_it = 0;
+    double prev_scale = 1.0;
+    bool prev_good = false;
     while (bb > 0.0 && rr > tol * tol * bb) {
         if (total >= max_iter || outer >= 40) {
             conv = LGT_ENOCONV;
@@ -1402,9 +1408,14 @@ int dd_cg_mixed(lgt_dd* d, int ib, bool want_y, double tol, int max_iter, int* i
         }
         double eps = 0.25 * tol * sqrt(bb / rr);
         if (eps < c0->inner_tol) eps = c0->inner_tol;
+        double pcoef = 0.0;  // reliable update instead of a restart, as in cg_mixed()
+        if (outer > 0 && prev_it > 0 && prev_good && c0->h_st->rr > 0.0 && c0->h_st->beta > 0.0)
+            pcoef = c0->h_st->beta / (c0->h_st->rr * (scale / prev_scale));
         int it = 0;
-        rc = D32::cg(d, 5, false, eps, max_iter - total, &it, nullptr);
+        rc = D32::cg(d, 5, false, eps, max_iter - total, &it, nullptr, pcoef);
         if (rc != LGT_OK && rc != LGT_ENOCONV) return rc;
+        prev_scale = scale;
+        prev_it = it;
         total += it;
         outer++;
         for (int i = 0; i < n; i++) {
@@ -1420,7 +1431,9 @@ int dd_cg_mixed(lgt_dd* d, int ib, bool want_y, double tol, int max_iter, int* i
             LAUNCH(c, LGT_K_CG_BLAS, residual_kernel, stream_blocks(c, cnt), 256, cnt, (const double2*)D64::fld(c, ib) + off,
                    (const double2*)c->ws[2] + off, (double2*)c->ws[1] + off, c->scal + 3, c->partials, c->counter, D64::zmask(c));
         }
+        const double rr_before = rr;
         if ((rc = read_sum(rr)) != LGT_OK) return rc;
+        prev_good = rr <= 100.0 * eps * eps * rr_before;
     }
     (void)want_y;  // Y = D x is what the last residual evaluation left in ws[3]
     if (iters) *iters = total;
@@ -1469,7 +1482,9 @@ int dd_eo_cg_mixed(lgt_dd* d, double tol, int max_iter, int* iters) {
     double bb = 0.0;
     if ((rc = read_sum(bb)) != LGT_OK) return rc;
     double rr = bb;
-    int total = 0, outer = 0, conv = LGT_OK;
+    int total = 0, outer = 0, conv = LGT_OK, prev_it = 0;
+    double prev_scale = 1.0;
+    bool prev_good = false;
     while (bb > 0.0 && rr > tol * tol * bb) {
         if (total >= max_iter || outer >= 40) {
             conv = LGT_ENOCONV;
@@ -1483,10 +1498,15 @@ int dd_eo_cg_mixed(lgt_dd* d, double tol, int max_iter, int* iters) {
         }
         double eps = 0.25 * tol * sqrt(bb / rr);
         if (eps < c0->inner_tol) eps = c0->inner_tol;
+        double pcoef = 0.0;  // reliable update instead of a restart, as in eo_cg_mixed()
+        if (outer > 0 && prev_it > 0 && prev_good && c0->h_st->rr > 0.0 && c0->h_st->beta > 0.0)
+            pcoef = c0->h_st->beta / (c0->h_st->rr * (scale / prev_scale));
         CgState st32;
         rc = D32::eo_cg_loop(d, D32::template F<0>, D32::template F<1>, D32::template F<2>, D32::template F<3>, D32::template F<4>,
-                             D32::template F<5>, eps, max_iter - total, &st32);
+                             D32::template F<5>, eps, max_iter - total, &st32, pcoef);
         if (rc != LGT_OK) return rc;
+        prev_scale = scale;
+        prev_it = st32.iter;
         total += st32.iter;
         outer++;
         for (int i = 0; i < n; i++) {
@@ -1508,6 +1528,7 @@ int dd_eo_cg_mixed(lgt_dd* d, double tol, int max_iter, int* iters) {
         const double rr_old = rr;
         if ((rc = read_sum(rr)) != LGT_OK) return rc;
         for (int i = 0; i < n; i++) mixed_inner_fallback(d->rk[i], rr_old, rr, eps);  // the same decision on every rank: rr is the global sum
+        prev_good = rr <= 100.0 * eps * eps * rr_old;
     }
     if (iters) *iters = total;
     if (conv != LGT_OK) return dd_fail(d, LGT_ENOCONV, "mixed-precision even/odd CG did not reach the tolerance");
