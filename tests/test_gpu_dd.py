@@ -349,6 +349,41 @@ def test_dd_half_spinor_halos_in_the_fp32_inner_solve(lgt):
     assert link_rel_err(res[lgt.LGT_DD_HALF][1], P1)[0] < 1e-10
 
 
+def test_dd_mixed_even_odd_inner_hops_on_twelve_real_links(lgt):
+    """Slabs large enough (320 blocks per half field and rank) for the fp32 inner hops of the mixed-precision even/odd solver to
+    take the three-blocks-per-SM build on 12-real links: the folded boundary sign must come out right with the slab's time
+    offset (antiperiodic t: the last slice of the LAST slab only).  Kick against the oracle's on the undivided lattice, fp32
+    iteration count that of the undivided handle (+- 2)."""
+    from oracle import evenodd as oeo
+
+    dims, beta, kappa, tol = (16, 16, 16, 40), 5.6, 0.12, 1e-12
+    V = synth.volume(dims)
+    U0 = synth.warm_links(dims, 0.3, 641)
+    P0 = synth.gaussian_momenta(dims, 642)
+    phi = oeo.mhat(dims, kappa, BC, U0, oeo.keep(synth.gaussian_spinor(dims, 643), dims, 0), dagger=True)
+    F_ref, it_ref, _ = oeo.fermion_force(dims, kappa, BC, U0, phi, tol, 10 * V)
+    P_ref = P0 - 0.05 * (oracle.gauge_force(dims, beta, U0) + F_ref)
+    one = lgt.Lattice(dims, beta, kappa, BC)
+    lgt.lgt_set_fermion_action(one.ctx, lgt.LGT_ACTION_EO)
+    lgt.lgt_set_solver(one.ctx, lgt.LGT_SOLVER_MIXED_CG, 1e-5)
+    one.set_links(U0)
+    one.set_momenta(P0)
+    one.set_pseudofermion(phi)
+    it_one = lgt.lgt_md_kick(one.ctx, 0.05, tol, 10 * V)
+    assert link_rel_err(one.get_momenta(), P_ref)[0] < 1e-10
+    one.close()
+    dd = lgt.DecomposedLattice(dims, 2, [0, 1], beta, kappa, BC)
+    lgt.lgt_dd_set_fermion_action(dd.d, lgt.LGT_ACTION_EO)
+    lgt.lgt_dd_set_solver(dd.d, lgt.LGT_SOLVER_MIXED_CG, 1e-5)
+    dd.set_links(U0)
+    dd.set_momenta(P0)
+    dd.set_pseudofermion(phi)
+    it = lgt.lgt_dd_md_kick(dd.d, 0.05, tol, 10 * V)
+    assert abs(it - it_one) <= 2 and it < 2 * it_ref + 20
+    assert link_rel_err(cat(dd.get_momenta()), P_ref)[0] < 1e-10
+    dd.close()
+
+
 @pytest.mark.parametrize("nranks", [1, 2])
 def test_dd_even_odd_overlapped_exchange(lgt, nranks):
     """LGT_DD_OVERLAP (and LGT_DD_HALF, which falls back to it for half fields) with the even/odd action: every hop of the

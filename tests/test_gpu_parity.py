@@ -521,6 +521,13 @@ def test_eo_mixed_solver_inner_hops_on_twelve_real_links(lgt, bc):
     assert lgt.lgt_set_kernel_variant(lat.ctx, lgt.LGT_K_DSLASH, 8) == 8  # exact 9-entry links in the inner hops
     F9, it9 = lat.fermion_force(None, None, tol=tol, max_iter=10 * V)
     assert abs(it - it9) <= 2 and link_rel_err(F9, F_ref)[0] < 1e-10
+    # the same on one level of stout links (special unitary as well, boundary sign folded the same way)
+    lgt.lgt_set_smearing(lat.ctx, 1, 0.3)
+    Fs9, its9 = lat.fermion_force(None, None, tol=tol, max_iter=10 * V)
+    assert lgt.lgt_set_kernel_variant(lat.ctx, lgt.LGT_K_DSLASH, 0) == 0
+    Fs12, its12 = lat.fermion_force(None, None, tol=tol, max_iter=10 * V)
+    assert abs(its9 - its12) <= 2 and link_rel_err(Fs12, Fs9)[0] < 1e-10
+    lgt.lgt_set_smearing(lat.ctx, 0, 0.0)
     # the fp64 hops themselves on 12-real links (variant 12, opt-in): same solve to rounding, same count
     lgt.lgt_set_solver(lat.ctx, lgt.LGT_SOLVER_CG)
     b64 = synth.gaussian_spinor(dims, 150)
